@@ -1,0 +1,98 @@
+"""Oracle O1-O3: all-experts-resident routed MoE forward, fp64, plain PyTorch CPU ops.
+
+TEST INFRASTRUCTURE (see oracle/__init__.py).  The method is exact -- paging changes where weights
+live, not what is computed -- so the oracle for the numerical result is the
+plain definition with every expert resident.  The paper never defines the router or the FFN (they
+are the engine's); BASELINE.json's configs do: top-k routing with renormalised
+softmax over the top-k, SwiGLU experts (readings G7, G8).
+
+Canonical expert blob (one expert, model dtype), row-major out x in:
+    [ gate (d_ff x d) | up (d_ff x d) | down (d x d_ff) ]
+"""
+from __future__ import annotations
+
+import torch
+
+F64 = torch.float64
+
+
+def router_logits(x: torch.Tensor, w_r: torch.Tensor, bias: torch.Tensor | None) -> torch.Tensor:
+    """O1: z[t, e] = bias[e] + sum_j W_r[e, j] * x[t, j], in fp64 from the stored values.
+
+    x [T, d], w_r [E, d] (model dtype; widened exactly), bias [E] fp32 or None -> z [T, E] fp64."""
+    z = x.to(F64) @ w_r.to(F64).T
+    if bias is not None:
+        z = z + bias.to(F64)[None, :]
+    return z
+
+
+def topk_softmax(z: torch.Tensor, k: int) -> tuple[torch.Tensor, torch.Tensor]:
+    """O1: ids = the k indices with largest z ordered by (z descending, id ascending);
+    w_i = exp(z_ids[i] - z_ids[0]) / sum_{j<k} exp(z_ids[j] - z_ids[0])
+    (softmax over the k selected logits == full softmax renormalised over the top-k).
+
+    Full sort of all E logits (stable, so equal logits keep ascending id).  z [T, E] fp64."""
+    order = torch.sort(z, dim=-1, descending=True, stable=True).indices
+    ids = order[:, :k].contiguous()
+    zs = torch.gather(z, 1, ids)
+    ex = torch.exp(zs - zs[:, :1])
+    w = ex / ex.sum(dim=1, keepdim=True)
+    return ids, w
+
+
+def split_expert_blob(blob: torch.Tensor, d: int, d_ff: int):
+    """Views (G [d_ff, d], U [d_ff, d], D [d, d_ff]) of one canonical expert blob."""
+    n = d * d_ff
+    return blob[:n].view(d_ff, d), blob[n:2 * n].view(d_ff, d), blob[2 * n:3 * n].view(d, d_ff)
+
+
+def silu(v: torch.Tensor) -> torch.Tensor:
+    """silu(v) = v / (1 + e^{-v})."""
+    return v / (1.0 + torch.exp(-v))
+
+
+def expert_ffn(x: torch.Tensor, g: torch.Tensor, u: torch.Tensor, dn: torch.Tensor) -> torch.Tensor:
+    """O2: y_e(x) = D (silu(G x) * (U x)), fp64, no intermediate rounding.  x [n, d] -> [n, d]."""
+    x = x.to(F64)
+    a = silu(x @ g.to(F64).T) * (x @ u.to(F64).T)
+    return a @ dn.to(F64).T
+
+
+def moe_layer(x: torch.Tensor, experts: torch.Tensor, w_r: torch.Tensor, bias: torch.Tensor | None,
+              k: int, d_ff: int, ids: torch.Tensor | None = None, w: torch.Tensor | None = None):
+    """O1 + O2 for one layer: out[t] = sum_{i<k} w[t,i] * y_{ids[t,i]}(x[t]), summed in rank order, fp64.
+
+    experts [E, 3*d*d_ff] canonical blobs.  If `ids`/`w` are given the routing is forced (used when a
+    near-tie makes two id sets equally correct, G7/G22).  No shared expert, no FFN bias, no
+    normalisation, no capacity factor.  Returns (out [T, d] fp64, ids [T, k] int64, w [T, k] fp64, z)."""
+    T, d = x.shape
+    z = router_logits(x, w_r, bias)
+    if ids is None:
+        ids, w = topk_softmax(z, k)
+    elif w is None:
+        zs = torch.gather(z, 1, ids)
+        ex = torch.exp(zs - zs.max(dim=1, keepdim=True).values)
+        w = ex / ex.sum(dim=1, keepdim=True)
+    out = torch.zeros((T, d), dtype=F64)
+    for i in range(k):                       # rank order
+        for e in torch.unique(ids[:, i]).tolist():
+            rows = (ids[:, i] == e).nonzero().flatten()
+            g, u, dn = split_expert_blob(experts[e], d, d_ff)
+            out[rows] += w[rows, i:i + 1] * expert_ffn(x[rows], g, u, dn)
+    return out, ids, w, z
+
+
+def stack_forward(h: torch.Tensor, experts: list, routers: list, k: int, d_ff: int, model_dtype):
+    """O3 (harness-level semantics): x_0 = h; y_l = MoE_l(x_l); x_{l+1} = x_l + y_l.
+
+    The residual add is done in fp32 on the model-dtype values and stored in the model dtype, and the
+    layer output y_l is stored in the model dtype, exactly as the GPU harness stores them; the MoE
+    itself is fp64.  Returns (x_L, [per-layer dict(x, out, ids, w)])."""
+    x = h.to(model_dtype)
+    per_layer = []
+    for (blob, (w_r, bias)) in zip(experts, routers):
+        out, ids, w, z = moe_layer(x, blob, w_r, bias, k, d_ff)
+        y = out.to(model_dtype)
+        per_layer.append(dict(x=x, out=out, ids=ids, w=w, z=z))
+        x = (x.to(torch.float32) + y.to(torch.float32)).to(model_dtype)
+    return x, per_layer

@@ -1,0 +1,154 @@
+"""Oracle O4: CPU simulation of the expert pager, Algorithm 1 `WISPLAYER.STEP(R)`.
+
+TEST INFRASTRUCTURE (see oracle/__init__.py).  Pure Python integers, one layer per object.
+Follows the algorithm line by line in the paper's notation (pi, pi^-1, tau, c); the readings the
+paper leaves open are those of SURVEY.md §8(c) / DESIGN.md:
+  G1  line 2 (lost in extraction):  M <- R \\ dom(pi)
+  G2  victims "in increasing tau": ties -> lower slot index
+  G3  ASSIGN: M in ascending expert id  <->  U in key order
+  G4  empty slot: occupant is None (not in R), tau = 0  -> taken first
+  G5  |R| > C: R sorted ascending is cut into consecutive waves of at most C ids; Alg. 1 per wave
+  G6  LFU (not in the paper): key (f[occupant], tau, slot); f counts steps in which e was in R,
+      survives eviction, never decays; an empty slot has f = -1
+  G13 resize: keep the most-recently-used C~ residents, compact to slots < C~ (device move, byte-equal
+      to the paper's re-page from host)
+  G20 a reference = one (layer, step, distinct expert); hit iff resident when its wave begins
+  G24 one tick per wave shared by all of R_w
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+HIT, MISS, RESIZE_DROP, RESIZE_MOVE = 0, 1, 2, 3
+LRU, LFU = 0, 1
+
+
+@dataclass
+class Event:
+    step: int
+    wave: int
+    expert: int
+    slot: int
+    evicted: int      # -1 none
+    kind: int
+
+    def key(self):
+        return (self.step, self.wave, self.expert, self.slot, self.evicted, self.kind)
+
+
+@dataclass
+class PagerLayer:
+    C: int
+    E: int
+    policy: int = LRU
+    pi: dict = field(default_factory=dict)        # expert -> slot
+    pi_inv: list = field(default_factory=list)    # slot -> expert or None
+    tau: list = field(default_factory=list)       # per-slot LRU tick
+    f: list = field(default_factory=list)         # per-expert LFU count
+    c: int = 0                                    # clock
+    steps: int = 0
+    hits: int = 0
+    misses: int = 0
+    evictions: int = 0
+    references: int = 0
+
+    def __post_init__(self):
+        self.pi_inv = [None] * self.C
+        self.tau = [0] * self.C
+        self.f = [0] * self.E
+
+    # -- Algorithm 1 -------------------------------------------------------------------------
+    def _victim_key(self, s: int):
+        if self.policy == LRU:
+            return (self.tau[s], s)
+        occ = self.pi_inv[s]
+        return (-1 if occ is None else self.f[occ], self.tau[s], s)
+
+    def step(self, routed) -> list[Event]:
+        """One forward of this layer.  `routed` = expert ids routed by all tokens (any order, repeats
+        allowed); R is their set.  Returns the trace events in emission order."""
+        R = sorted(set(int(e) for e in routed))
+        if not R:
+            return []                                   # n_tokens = 0: no-op, no tick (G23)
+        events: list[Event] = []
+        step_no = self.steps
+        for wv, lo in enumerate(range(0, len(R), self.C)):
+            Rw = R[lo:lo + self.C]
+            in_wave = set(Rw)
+            # 2: M <- R \ dom(pi)   (faults)
+            M = [e for e in Rw if e not in self.pi]
+            hit_set = [e for e in Rw if e in self.pi]
+            # 3: U <- {s : pi^-1(s) not in R} in increasing tau   (victims; ties -> lower slot)
+            U = sorted((s for s in range(self.C) if self.pi_inv[s] not in in_wave), key=self._victim_key)
+            # 4-8: assign each e in M a victim slot; copy; update maps
+            assign = {}
+            for i, e in enumerate(M):
+                s = U[i]
+                old = self.pi_inv[s]
+                if old is not None:
+                    del self.pi[old]
+                    self.evictions += 1
+                self.pi[e] = s
+                self.pi_inv[s] = e
+                assign[e] = (s, -1 if old is None else old)
+            # 9: c <- c+1; tau[pi(e)] <- c for e in R ; LFU count
+            self.c += 1
+            for e in Rw:
+                self.tau[self.pi[e]] = self.c
+                self.f[e] += 1
+            self.hits += len(hit_set)
+            self.misses += len(M)
+            self.references += len(Rw)
+            for e in Rw:                                 # ascending expert id within the wave
+                if e in assign:
+                    events.append(Event(step_no, wv, e, assign[e][0], assign[e][1], MISS))
+                else:
+                    events.append(Event(step_no, wv, e, self.pi[e], -1, HIT))
+        self.steps += 1
+        return events
+
+    # -- resize (a7) ---------------------------------------------------------------------------
+    def resize(self, C_new: int) -> list[Event]:
+        events: list[Event] = []
+        step_no = self.steps
+        if C_new < self.C:
+            occ = [s for s in range(self.C) if self.pi_inv[s] is not None]
+            if self.policy == LRU:
+                occ.sort(key=lambda s: (-self.tau[s], s))
+            else:
+                occ.sort(key=lambda s: (-self.f[self.pi_inv[s]], -self.tau[s], s))
+            keep, drop = occ[:C_new], occ[C_new:]
+            for s in sorted(drop):
+                e = self.pi_inv[s]
+                del self.pi[e]
+                self.pi_inv[s] = None
+                self.tau[s] = 0
+                events.append(Event(step_no, 0, e, s, -1, RESIZE_DROP))
+            for s in sorted(x for x in keep if x >= C_new):
+                dst = next(t for t in range(C_new) if self.pi_inv[t] is None)
+                e = self.pi_inv[s]
+                self.pi_inv[dst], self.tau[dst] = e, self.tau[s]
+                self.pi_inv[s], self.tau[s] = None, 0
+                self.pi[e] = dst
+                events.append(Event(step_no, 0, e, dst, s, RESIZE_MOVE))   # `evicted` carries the source slot
+            self.pi_inv = self.pi_inv[:C_new]
+            self.tau = self.tau[:C_new]
+        elif C_new > self.C:
+            self.pi_inv += [None] * (C_new - self.C)
+            self.tau += [0] * (C_new - self.C)
+        self.C = C_new
+        return events
+
+    def slots(self) -> list:
+        return list(self.pi_inv)
+
+    def check_invariants(self):
+        """P9: pi and pi^-1 mutually inverse; distinct slots."""
+        for e, s in self.pi.items():
+            assert self.pi_inv[s] == e
+        for s, e in enumerate(self.pi_inv):
+            if e is not None:
+                assert self.pi[e] == s
+            else:
+                assert self.tau[s] == 0
+        assert len(set(self.pi.values())) == len(self.pi)

@@ -1,0 +1,209 @@
+"""Seeded synthetic inputs for the WiSP hot path (BASELINE.json configs).
+
+This module is shared by the oracle (`oracle/`), the tests and `bench.py`.  It holds NONE of the
+method's arithmetic (no router, no FFN, no paging policy): only the shapes of the five
+BASELINE.json configs and a counter-based random generator that fills weight / router / hidden
+buffers.  Both the CPU oracle and the CUDA library *read the buffers produced here*; neither side
+re-derives them, so the generator may run on either the CPU or the GPU (the bits of a given run
+are whatever this module wrote into the host buffers of that run).
+
+Recipe:
+  * expert and router weights ~ N(0, 0.02^2), rounded to the model dtype (bf16: RNE of the fp32 draw);
+  * router bias[perm[r-1]] = -0.5 * alpha * ln(r), r = 1..E, one seeded permutation per layer
+    (alpha = 1.1; 0.8 for the Mixtral-shaped config)  -> Zipf-skewed popularity;
+  * decode hidden states: AR(1) h_t = 0.9 h_{t-1} + 0.1 xi_t, xi ~ N(0,1), stationary start
+    h_{-1} ~ N(0, 0.01/0.19), kept in fp32 and cast when fed; batch streams are independent;
+  * prefill hidden states: i.i.d. N(0,1).
+Base seed 21868; tensor-kind ids: 1 experts, 2 router W, 3 permutation, 4 hidden stream, 5 prompt
+lengths, 6 prefill tokens.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, replace
+
+import torch
+
+BASE_SEED = 21868
+KIND_EXPERTS, KIND_ROUTER, KIND_PERM, KIND_HIDDEN, KIND_PROMPT_LEN, KIND_PREFILL = 1, 2, 3, 4, 5, 6
+
+_M1 = 0xBF58476D1CE4E5B9
+_M2 = 0x94D049BB133111EB
+_GOLD = 0x9E3779B97F4A7C15
+
+
+def _s64(v: int) -> int:
+    """Python int -> the signed 64-bit value with the same bits (torch int64 arithmetic wraps)."""
+    v &= (1 << 64) - 1
+    return v - (1 << 64) if v >= (1 << 63) else v
+
+
+def _lsr(z: torch.Tensor, s: int) -> torch.Tensor:
+    return (z >> s) & ((1 << (64 - s)) - 1)
+
+
+def _mix64(z: torch.Tensor) -> torch.Tensor:
+    """SplitMix64 finaliser on an int64 tensor (wrapping arithmetic)."""
+    z = (z ^ _lsr(z, 30)) * _s64(_M1)
+    z = (z ^ _lsr(z, 27)) * _s64(_M2)
+    return z ^ _lsr(z, 31)
+
+
+def _mix64_int(v: int) -> int:
+    m = (1 << 64) - 1
+    v &= m
+    v = ((v ^ (v >> 30)) * _M1) & m
+    v = ((v ^ (v >> 27)) * _M2) & m
+    return v ^ (v >> 31)
+
+
+def stream_key(seed: int, kind: int, *idx: int) -> int:
+    """Fold (seed, tensor-kind, indices...) into one 64-bit stream key."""
+    h = _mix64_int(seed * _GOLD + kind)
+    for i in idx:
+        h = _mix64_int(h ^ ((i + 1) * _GOLD))
+    return h
+
+
+def _hash_counter(key: int, n: int, device, offset: int = 0) -> torch.Tensor:
+    ctr = torch.arange(offset, offset + n, dtype=torch.int64, device=device)
+    return _mix64(ctr * _s64(_GOLD) + _s64(key))
+
+
+def normal(key: int, n: int, device="cpu", offset: int = 0) -> torch.Tensor:
+    """n standard normals (fp32) from the counter stream `key`, elements offset..offset+n-1.
+
+    One Box-Muller draw per 64-bit hash: u1 from the high 32 bits, u2 from the low 32 bits."""
+    h = _hash_counter(key, n, device, offset)
+    hi = _lsr(h, 32).to(torch.float32)
+    lo = (h & 0xFFFFFFFF).to(torch.float32)
+    u1 = (hi + 0.5) * (1.0 / 4294967296.0)
+    u2 = (lo + 0.5) * (1.0 / 4294967296.0)
+    u1 = u1.clamp_(min=1e-10, max=1.0 - 2.0 ** -24)
+    r = torch.sqrt(-2.0 * torch.log(u1))
+    return r * torch.cos((2.0 * math.pi) * u2)
+
+
+def uniform_int(key: int, n: int, lo: int, hi: int) -> list[int]:
+    """n integers uniform over lo..hi inclusive (host side, pure Python)."""
+    span = hi - lo + 1
+    return [lo + _mix64_int(key + (i + 1) * _GOLD) % span for i in range(n)]
+
+
+def permutation(key: int, n: int) -> list[int]:
+    """Seeded permutation of range(n): argsort of per-index hashes (ties impossible in practice)."""
+    return sorted(range(n), key=lambda i: (_mix64_int(key + (i + 1) * _GOLD), i))
+
+
+@dataclass(frozen=True)
+class MoEShape:
+    """Layer shapes (uniform across layers) plus the config's workload constants."""
+    name: str
+    n_layers: int
+    n_experts: int
+    top_k: int
+    d_model: int
+    d_ff: int
+    dtype: str            # "f32" | "bf16"
+    zipf_alpha: float
+    seed: int = BASE_SEED
+
+    @property
+    def torch_dtype(self):
+        return torch.float32 if self.dtype == "f32" else torch.bfloat16
+
+    @property
+    def elem_bytes(self) -> int:
+        return 4 if self.dtype == "f32" else 2
+
+    @property
+    def expert_elems(self) -> int:
+        return 3 * self.d_model * self.d_ff
+
+    @property
+    def expert_bytes(self) -> int:          # M_e
+        return self.expert_elems * self.elem_bytes
+
+    @property
+    def slot_unit_bytes(self) -> int:       # a = L * M_e
+        return self.n_layers * self.expert_bytes
+
+    def with_layers(self, n_layers: int) -> "MoEShape":
+        return replace(self, n_layers=n_layers)
+
+
+# BASELINE.json configs[0..3] (config 5 reuses QWEN3).
+TINY = MoEShape("tiny", 2, 16, 2, 256, 512, "f32", 1.1)
+QWEN3 = MoEShape("qwen3-30b-a3b-shaped", 48, 128, 8, 2048, 768, "bf16", 1.1)
+MIXTRAL = MoEShape("mixtral-8x7b-shaped", 32, 8, 2, 4096, 14336, "bf16", 0.8)
+SHAPES = {s.name: s for s in (TINY, QWEN3, MIXTRAL)}
+
+
+def slots_for_budget(shape: MoEShape, expert_bytes: int) -> int:
+    """C = floor(B_exp / a) clipped to [0, E]."""
+    return max(0, min(shape.n_experts, expert_bytes // shape.slot_unit_bytes))
+
+
+def gen_layer_experts(shape: MoEShape, layer: int, device="cpu", out: torch.Tensor | None = None,
+                      chunk_experts: int = 16) -> torch.Tensor:
+    """Expert blobs of one layer, canonical layout [E, gate(d_ff x d) | up(d_ff x d) | down(d x d_ff)],
+    row-major out x in, in the model dtype.  `out` may be a preallocated (pinned) host tensor."""
+    E, n = shape.n_experts, shape.expert_elems
+    if out is None:
+        out = torch.empty((E, n), dtype=shape.torch_dtype)
+    for e0 in range(0, E, chunk_experts):
+        e1 = min(E, e0 + chunk_experts)
+        for e in range(e0, e1):
+            key = stream_key(shape.seed, KIND_EXPERTS, layer, e)
+            v = normal(key, n, device).mul_(0.02).to(shape.torch_dtype)
+            out[e].copy_(v)
+    return out
+
+
+def gen_router(shape: MoEShape, layer: int) -> tuple[torch.Tensor, torch.Tensor]:
+    """(W_r [E, d] in the model dtype, bias [E] fp32) for one layer (host tensors)."""
+    E, d = shape.n_experts, shape.d_model
+    w = normal(stream_key(shape.seed, KIND_ROUTER, layer), E * d).mul_(0.02).to(shape.torch_dtype).view(E, d)
+    perm = permutation(stream_key(shape.seed, KIND_PERM, layer), E)
+    bias = torch.empty(E, dtype=torch.float32)
+    for r in range(1, E + 1):
+        bias[perm[r - 1]] = -0.5 * shape.zipf_alpha * math.log(r)
+    return w, bias
+
+
+def gen_decode_hidden(shape: MoEShape, n_steps: int, batch: int = 1, stream_base: int = 0,
+                      rho: float = 0.9, noise: float = 0.1) -> torch.Tensor:
+    """AR(1) decode hidden states [n_steps, batch, d] in fp32 (cast by the caller when fed).
+
+    h_t = rho*h_{t-1} + noise*xi_t with a stationary start; stream b uses key (.., stream_base+b)."""
+    d = shape.d_model
+    out = torch.empty((n_steps, batch, d), dtype=torch.float32)
+    var0 = noise * noise / (1.0 - rho * rho)
+    for b in range(batch):
+        key = stream_key(shape.seed, KIND_HIDDEN, stream_base + b)
+        xi = normal(key, (n_steps + 1) * d).view(n_steps + 1, d)
+        h = xi[0] * math.sqrt(var0)
+        for t in range(n_steps):
+            h = rho * h + noise * xi[t + 1]
+            out[t, b] = h
+    return out
+
+
+def gen_prefill_hidden(shape: MoEShape, n_tokens: int, request: int = 0) -> torch.Tensor:
+    """Prefill hidden states [n_tokens, d] i.i.d. N(0,1), fp32."""
+    key = stream_key(shape.seed, KIND_PREFILL, request)
+    return normal(key, n_tokens * shape.d_model).view(n_tokens, shape.d_model)
+
+
+def gen_prompt_lengths(shape: MoEShape, n_requests: int, lo: int = 1024, hi: int = 16384) -> list[int]:
+    return uniform_int(stream_key(shape.seed, KIND_PROMPT_LEN), n_requests, lo, hi)
+
+
+def gen_model(shape: MoEShape, device="cpu", pin: bool = False):
+    """All layers: list of expert blobs [E, 3*d*d_ff], list of (W_r, bias).  Host tensors."""
+    experts, routers = [], []
+    for l in range(shape.n_layers):
+        buf = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=pin)
+        experts.append(gen_layer_experts(shape, l, device, out=buf))
+        routers.append(gen_router(shape, l))
+    return experts, routers

@@ -1,0 +1,152 @@
+"""Pins for oracle O4 (Algorithm 1): SURVEY.md §8(c) P3, P4, P7, P9."""
+import random
+
+import pytest
+
+from golden_util import num, read_golden
+from oracle import mvwsa
+from oracle.paging import HIT, LFU, LRU, MISS, RESIZE_DROP, RESIZE_MOVE, PagerLayer
+
+TR = read_golden("hand_paging_trace.txt")
+STEPS = [{1, 4}, {1, 2}, {3, 5}, {1, 2}, {2, 3}, {0, 4}]
+
+
+def _parse_step(txt):
+    misses, slots, tau = (p.strip() for p in txt.split("|"))
+    m = []
+    for tok in misses.split():
+        e, rest = tok.split(">")
+        s, ev = rest.split("/")
+        m.append((int(e), int(s), -1 if ev == "-" else int(ev)))
+    sl = [None if t == "-" else int(t) for t in slots.split()]
+    ta = [int(t) for t in tau.split()] if tau else None
+    return m, sl, ta
+
+
+@pytest.mark.parametrize("name,policy", [("lru", LRU), ("lfu", LFU)])
+def test_p4_hand_trace(name, policy):
+    sec = TR[name]
+    p = PagerLayer(C=3, E=6, policy=policy)
+    for i, R in enumerate(STEPS):
+        ev = p.step(R)
+        m, sl, ta = _parse_step(sec[f"step{i}"])
+        assert [(e.expert, e.slot, e.evicted) for e in ev if e.kind == MISS] == m
+        assert p.slots() == sl
+        if ta is not None:
+            assert p.tau == ta
+        assert [e.expert for e in ev] == sorted(R)
+        p.check_invariants()
+    assert p.hits == num(sec["hits"]) and p.misses == num(sec["misses"])
+    if "evictions" in sec:
+        assert p.evictions == num(sec["evictions"])
+
+
+def test_p4_overflow_waves():
+    sec = TR["overflow"]
+    p = PagerLayer(C=2, E=6, policy=LRU)
+    ev = p.step([0, 1, 2, 3, 5])
+    m, sl, ta = _parse_step(sec["step0"])
+    assert [(e.expert, e.slot, e.evicted) for e in ev if e.kind == MISS] == m
+    assert [e.wave for e in ev] == [0, 0, 1, 1, 2]
+    assert p.slots() == sl and p.tau == ta
+    ev = p.step([3, 5])
+    _, sl, ta = _parse_step(sec["step1"])
+    assert sum(e.kind == HIT for e in ev) == num(sec["step1_hits"]) and p.slots() == sl and p.tau == ta
+
+
+def test_p3_fig4_printed_fault_counts():
+    g = {k: num(v) for k, v in read_golden("fig4_fault_counts.txt").items()}
+    for cap in (8, 4, 2):
+        faults = hits = 0
+        for _ in range(g["n_layers"]):
+            p = PagerLayer(C=cap, E=g["n_experts"], policy=LRU)
+            for _ in range(g["n_steps"]):
+                p.step(range(g["n_experts"]))
+            faults += p.misses
+            hits += p.hits
+        assert (faults, hits) == (g[f"cap{cap}_faults"], g[f"cap{cap}_hits"])
+
+
+def test_p7_mattson_hand_case():
+    sec = TR["mattson"]
+    stream = sec["stream"].split()
+    want = [mvwsa.INF if t == "inf" else int(t) for t in sec["distances"].split()]
+    assert mvwsa.stack_distances(stream) == want
+    mc = mvwsa.miss_curve_from_hist(mvwsa.histogram(want, 4), 4)
+    assert [mc[c] for c in (1, 2, 3, 4)] == [num(sec[f"m{c}"]) for c in (1, 2, 3, 4)]
+
+
+def test_p7_k1_is_textbook_lru_and_matches_stack_distances():
+    rng = random.Random(11)
+    for trial in range(20):
+        E = rng.randint(2, 12)
+        stream = [rng.randrange(E) for _ in range(200)]
+        dist = mvwsa.stack_distances(stream)
+        for C in range(1, E + 1):
+            # Algorithm 1 at k = 1
+            p = PagerLayer(C=C, E=E, policy=LRU)
+            for e in stream:
+                p.step([e])
+            # textbook LRU written independently: ordered list, most recent last
+            cache, miss = [], 0
+            for e in stream:
+                if e in cache:
+                    cache.remove(e)
+                else:
+                    miss += 1
+                    if len(cache) == C:
+                        cache.pop(0)
+                cache.append(e)
+            assert p.misses == miss == sum(d > C for d in dist)
+
+
+@pytest.mark.parametrize("policy", [LRU, LFU])
+def test_p9_invariants_random_streams(policy):
+    rng = random.Random(5)
+    for trial in range(30):
+        E = rng.randint(2, 40)
+        C = rng.randint(1, E)
+        k = rng.randint(1, min(E, 9))
+        p = PagerLayer(C=C, E=E, policy=policy)
+        total_refs, distinct = 0, set()
+        for t in range(60):
+            R = set(rng.sample(range(E), k))
+            resident_before = set(p.pi)
+            ev = p.step(R)
+            total_refs += len(R)
+            distinct |= R
+            assert [e.expert for e in ev] == sorted(R)
+            # every expert of the LAST wave is resident at its FFN time; slots distinct within a wave
+            for wv in set(e.wave for e in ev):
+                sl = [e.slot for e in ev if e.wave == wv]
+                assert len(set(sl)) == len(sl) and len(sl) <= C
+                evicted = {e.evicted for e in ev if e.wave == wv and e.evicted >= 0}
+                assert not evicted & {e.expert for e in ev if e.wave == wv}
+            if len(R) <= C:
+                assert all((e.kind == HIT) == (e.expert in resident_before) for e in ev)
+                assert R <= set(p.pi)
+            p.check_invariants()
+        assert p.hits + p.misses == total_refs == p.references
+        if C >= E:
+            assert p.misses == len(distinct) and p.evictions == 0
+
+
+def test_resize_shrink_grow_cycle():
+    p = PagerLayer(C=4, E=8, policy=LRU)
+    for R in ([0, 1], [2, 3], [0, 2]):
+        p.step(R)
+    # slots [0,1,2,3], tau [3,1,3,2]; shrink to 2 keeps the two most recent: slots 0 (e0) and 2 (e2)
+    ev = p.resize(2)
+    assert [(e.kind, e.expert, e.slot) for e in ev] == [(RESIZE_DROP, 1, 1), (RESIZE_DROP, 3, 3), (RESIZE_MOVE, 2, 1)]
+    assert p.slots() == [0, 2] and p.tau == [3, 3] and p.C == 2
+    p.check_invariants()
+    ev = p.resize(5)
+    assert ev == [] and p.slots() == [0, 2, None, None, None] and p.tau == [3, 3, 0, 0, 0]
+    ev = p.step([0, 5])
+    assert [(e.expert, e.slot, e.kind) for e in ev] == [(0, 0, HIT), (5, 2, MISS)]
+    p.check_invariants()
+
+
+def test_empty_step_is_noop():
+    p = PagerLayer(C=2, E=4)
+    assert p.step([]) == [] and p.c == 0 and p.steps == 0
