@@ -1,0 +1,223 @@
+/* wisp.h -- C ABI of libwisp: the routed-MoE hot path of WiSP ("Working-Set Paging",
+ * arxiv/paper_2606_21868) on one B200 (sm_100a).
+ *
+ * What the library computes (citations are PAPER.md line numbers; readings Gn are listed in DESIGN.md):
+ *   A routed MoE layer forward whose expert weights live in a fixed-budget, slot-indexed VRAM expert
+ *   pool while the full expert set stays in pinned host memory (Fig. 1).  Per
+ *   layer call: (a1) router GEMV + softmax + top-k; (a2) slot-table residency lookup = Algorithm 1
+ *   `WISPLAYER.STEP(R)` with LRU (paper) or LFU (G6) eviction, overflow waves when
+ *   |R| > C (G5); (a3) demand fetch of every missing expert from the pinned host master
+ *   into its victim slot (Alg. 1 line 6); (a4) SwiGLU expert FFN over slot-indirected weights with a
+ *   rank-ordered weighted combine.  The residency requirement is PAPER.md:97: "every expert e in R
+ *   must be resident when that layer executes".  Routed experts and KV blocks share ONE pageable
+ *   budget B = B_exp + B_kv (Eq. 1); wisp_set_split moves the boundary.
+ *
+ * Conventions
+ *   - Every call returns a wisp_status (0 = OK, negative = error); on error the context is unchanged.
+ *     wisp_last_error() gives a human-readable message for the last failing call on that context.
+ *   - "host" / "device" on a pointer says where the memory lives.  The library never takes or returns
+ *     framework (torch) types.  `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *   - One context is used from one thread at a time.  No CPU fallback exists: without a CUDA device
+ *     wisp_create fails with WISP_ECUDA.
+ *   - Canonical expert blob (one expert, M_e = 3*d_model*d_ff*sizeof(dtype) bytes),
+ *     row-major out x in:  [ gate (d_ff x d_model) | up (d_ff x d_model) | down (d_model x d_ff) ].
+ *     Slot bytes == master bytes (the exactness invariant).
+ *   - Arena: one device allocation of `budget_bytes`.  Expert slot s of layer l lives at byte offset
+ *     (s*L + l)*M_e  (slot-major, so growing C by one appends a = L*M_e bytes); the KV
+ *     pool is the top kappa*b bytes and is modelled as block reservations (BASELINE.json config 5).
+ */
+#ifndef WISP_H_
+#define WISP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wisp_ctx wisp_ctx; /* opaque; owned by the library */
+
+typedef enum {
+  WISP_OK = 0,
+  WISP_EINVAL = -1,   /* bad argument */
+  WISP_ENOMEM = -2,   /* host or device allocation failed */
+  WISP_ECUDA = -3,    /* CUDA runtime error, or no CUDA device */
+  WISP_ESTATE = -4,   /* call not legal in this state (e.g. forward before registration) */
+  WISP_EBUDGET = -5   /* split does not fit the budget / floor / reservations */
+} wisp_status;
+
+typedef enum { WISP_F32 = 0, WISP_BF16 = 1 } wisp_dtype;
+typedef enum { WISP_LRU = 0, WISP_LFU = 1 } wisp_policy;
+/* Miss path (a3): MEMCPY = cudaMemcpyAsync per miss on a dedicated copy stream fenced with events (the
+ * host reads the miss list: one host sync per layer call); ZEROCOPY = a device-initiated copy kernel that
+ * reads the mapped pinned master (no host round trip; the whole call is stream-ordered). */
+typedef enum { WISP_FETCH_MEMCPY = 0, WISP_FETCH_ZEROCOPY = 1 } wisp_fetch;
+
+typedef struct {
+  int32_t n_layers;   /* L */
+  int32_t n_experts;  /* N (E), 1..1024 */
+  int32_t top_k;      /* k, 1..min(E,32) */
+  int32_t d_model;    /* multiple of 256 */
+  int32_t d_ff;       /* multiple of 256 */
+  int32_t max_tokens; /* largest n_tokens passed to wisp_moe_forward (sizes staging buffers) */
+  int32_t dtype;      /* wisp_dtype: dtype of weights, hidden and out */
+  int32_t policy;     /* wisp_policy */
+  int32_t fetch;      /* wisp_fetch */
+  int32_t reserved0;
+  uint64_t kv_block_bytes;  /* b: bytes per KV block summed over layers; 0 = no KV accounting */
+  uint64_t kv_floor_blocks; /* kappa_min of Eq. 4; wisp_set_split refuses to go below it */
+  uint64_t trace_capacity;  /* trace ring capacity in events; 0 = library default (1<<20) */
+} wisp_config;
+
+typedef struct {
+  uint64_t steps;         /* forwards of this layer with n_tokens > 0 */
+  uint64_t references;    /* sum over steps of |R| (distinct experts, G20) */
+  uint64_t hits, misses;  /* hits + misses == references */
+  uint64_t evictions;
+  uint64_t bytes_fetched; /* misses * M_e */
+} wisp_layer_stats;
+
+typedef struct {
+  wisp_layer_stats total;        /* summed over layers */
+  int32_t n_layers;
+  int32_t slots_per_layer;       /* C */
+  uint64_t budget_bytes;         /* B */
+  uint64_t expert_bytes;         /* C * a */
+  uint64_t kv_bytes;             /* kappa * b */
+  uint64_t kv_blocks;            /* kappa */
+  uint64_t kv_blocks_reserved;   /* currently reserved */
+  uint64_t kv_blocks_peak;       /* peak reserved since the previous wisp_stats call (p of Eq. 6) */
+  uint64_t resize_count;         /* successful wisp_set_split calls that changed C or kappa */
+  uint64_t failed_resize_count;  /* refused wisp_set_split calls (state kept) */
+  uint64_t trace_dropped;        /* events lost because the ring was full */
+  uint64_t fetch_ns;             /* event-timed busy time of the miss path (only while fetch timing is on) */
+} wisp_stats_t;
+
+/* kind: 0 hit, 1 miss, 2 resize-drop, 3 resize-move (for a move `evicted` carries the source slot).
+ * Events of one wave are emitted in ascending expert id; waves in order; layers/steps in call order. */
+typedef struct {
+  uint64_t step;   /* per-layer step counter (0-based) */
+  uint32_t layer;
+  uint32_t wave;
+  int32_t expert;
+  int32_t slot;
+  int32_t evicted; /* -1 none */
+  uint32_t kind;
+} wisp_trace_event;
+
+/* Inputs of the MV-WSA proposal (PAPER.md:126-169 and App. B).  mode 0 = live law, Eq. 6-8
+ * (PAPER.md:353-363): kappa~ = max(kappa_min, ceil((1+h)p)); C~ = clip(floor((B-kappa~ b)/a), C_min, C_max);
+ * kappa~ <- floor((B - C~ a)/b); moves smaller than `dead_zone` experts are suppressed.
+ * mode 1 = configurator, Eq. 2-5: argmin over C of c_exp*m_exp(C) + c_kv*m_kv(kappa(C))
+ * subject to the admission floor, with m_exp taken from the library's decayed reuse-distance histograms
+ * and m_kv given by the caller as a table. */
+typedef struct {
+  int32_t mode;
+  int32_t c_min, c_max;      /* clip range for C; c_max <= 0 means "knee of the measured miss curve" (G11) */
+  int32_t dead_zone;         /* Delta, experts */
+  double headroom;           /* h */
+  uint64_t kv_peak_blocks;   /* p; UINT64_MAX = use the peak recorded by wisp_kv_reserve */
+  double c_exp;              /* cost of one expert miss  (M_e * t_byte), seconds */
+  double c_kv;               /* cost of one KV miss unit (beta * b_tok), seconds */
+  const double* m_kv;        /* host, m_kv[kappa] for kappa = 0..m_kv_len-1 (last value extends); may be NULL */
+  uint64_t m_kv_len;
+} wisp_mvwsa_in;
+
+/* ---- mandated entry points (BASELINE.json north_star) ------------------------------------------- */
+
+/* Create a context with a pageable budget of `budget_bytes` (B).  Allocates the arena and all
+ * per-layer state.  Initial split: kv = kv_floor_blocks*b, experts = the rest (C = min(E, floor(./a))).
+ * Errors: EINVAL (shape), EBUDGET (fewer than 1 slot per layer fits), ENOMEM, ECUDA.  *out receives the
+ * context; destroy with wisp_destroy. */
+int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out);
+int wisp_destroy(wisp_ctx* ctx);
+
+/* Register one layer's full expert set: the "CPU master W^cpu" of Algorithm 1.
+ *   experts     host, E canonical blobs, E*M_e bytes, in cfg.dtype.
+ *   router_w    host, [E, d_model] row-major in cfg.dtype.
+ *   router_bias host, [E] fp32, or NULL (zeros).
+ * The library COPIES all three (experts into its own pinned, device-mapped host memory; router into
+ * device memory, which is a fixed cost outside B); the caller may free its buffers on return.
+ * Re-registering a layer is an error (ESTATE).  The pool starts empty (cold). */
+int wisp_register_host_experts(wisp_ctx* ctx, int32_t layer, const void* experts, const void* router_w,
+                               const float* router_bias);
+
+/* One forward of one MoE layer = one "step" of that layer's clock (Alg. 1).
+ *   hidden  device, [n_tokens, d_model] row-major, cfg.dtype, 16-byte aligned.
+ *   out     device, [n_tokens, d_model], cfg.dtype; out[t] = sum_i w[t,i] * FFN_{ids[t,i]}(hidden[t]).
+ * Work is enqueued on `cuda_stream`; `out` is valid once the caller synchronises that stream.  With
+ * WISP_FETCH_MEMCPY the call blocks the host until the layer's routing is known.  n_tokens == 0 is a
+ * no-op (no tick).  Errors: EINVAL (layer, n_tokens > max_tokens), ESTATE (layer not registered). */
+int wisp_moe_forward(wisp_ctx* ctx, int32_t layer, const void* hidden, int32_t n_tokens, void* out,
+                     void* cuda_stream);
+
+/* Move the expert<->KV boundary: C = min(E, floor(expert_bytes / a)),
+ * kappa = floor(kv_bytes / b).  Legal only between forwards (the "drained barrier"); synchronises the
+ * device.  Shrink keeps the C~ best residents by the policy key and compacts them into slots < C~
+ * (device-to-device moves, byte-equal to the paper's re-page); grow adds empty slots.  Transactional:
+ * EBUDGET (and failed_resize_count++) when expert_bytes + kv_bytes > B, C~ < 1, kappa~ < kv_floor_blocks
+ * or kappa~ < blocks currently reserved; the previous split then stays in force. */
+int wisp_set_split(wisp_ctx* ctx, uint64_t expert_bytes, uint64_t kv_bytes);
+
+/* Totals and the current split.  Synchronises the device.  Resets kv_blocks_peak to the current level. */
+int wisp_stats(wisp_ctx* ctx, wisp_stats_t* out);
+
+/* ---- whole-token helpers (same kernels; O3 semantics of DESIGN.md) ------------------------------- */
+
+/* x_0 = hidden; for l = 0..L-1: y_l = MoE_l(x_l); x_{l+1} = x_l + y_l (add in fp32 on the model-dtype
+ * values, stored in cfg.dtype); hidden_out = x_L.  Each layer ticks once.  With WISP_FETCH_ZEROCOPY the
+ * chain is replayed from a CUDA graph cached per n_tokens.  hidden/hidden_out: device [n_tokens, d_model]. */
+int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void* hidden_out,
+                       void* cuda_stream);
+/* out = x + y elementwise with the rounding stated above (device pointers, n_elems elements of cfg.dtype). */
+int wisp_residual_add(wisp_ctx* ctx, const void* x, const void* y, void* out, int64_t n_elems,
+                      void* cuda_stream);
+
+/* ---- parity / test surface ------------------------------------------------------------------------ */
+
+int wisp_layer_stats_read(wisp_ctx* ctx, int32_t layer, wisp_layer_stats* out);
+/* Trace ring: when on, every reference / resize action appends one wisp_trace_event. */
+int wisp_trace_enable(wisp_ctx* ctx, int32_t on);
+/* Drain up to `cap` events into host `buf` (oldest first); *n_out = number written.  Synchronises. */
+int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t* n_out);
+/* Routing of the most recent forward of `layer`: host ids [n_tokens, k] (rank order) and w [n_tokens, k].
+ * *n_tokens_out (may be NULL) receives that forward's n_tokens.  Either array may be NULL.  Synchronises. */
+int wisp_last_topk(wisp_ctx* ctx, int32_t layer, int32_t* ids, float* w, int32_t* n_tokens_out);
+/* Router logits of the most recent forward overall: host z [n_tokens, E] fp32.  Synchronises. */
+int wisp_last_logits(wisp_ctx* ctx, float* z, int32_t n_tokens);
+/* Drive the pager with a given routed-id list (host, n_ids ids, repeats allowed): runs the residency
+ * lookup and the demand fetch of one step of `layer`, no router and no FFN.  Synchronises. */
+int wisp_debug_step_routing(wisp_ctx* ctx, int32_t layer, const int32_t* ids, int32_t n_ids);
+/* Residency state of `layer`: host pi_inv [C] (expert per slot, -1 empty), tau [C], freq [E], *clock.
+ * Any pointer may be NULL.  Synchronises. */
+int wisp_debug_residency(wisp_ctx* ctx, int32_t layer, int32_t* pi_inv, uint64_t* tau, uint64_t* freq,
+                         uint64_t* clock);
+/* Exactness invariant check: compares every occupied slot of `layer` byte for byte with
+ * the host master of the expert it claims to hold; *mismatched_slots = number of slots that differ. */
+int wisp_debug_verify_pool(wisp_ctx* ctx, int32_t layer, int32_t* mismatched_slots);
+/* Time the miss path with CUDA events (adds a little host work per forward); totals in wisp_stats.fetch_ns. */
+int wisp_fetch_timing_enable(wisp_ctx* ctx, int32_t on);
+
+/* ---- KV reservations and MV-WSA (CPU side) ----------------------------- */
+
+/* Reserve (delta > 0) or release (delta < 0) KV blocks; EBUDGET if it would exceed kappa or go below 0. */
+int wisp_kv_reserve(wisp_ctx* ctx, int64_t delta_blocks);
+/* Propose a split (does not apply it): see wisp_mvwsa_in.  Outputs are byte counts that wisp_set_split
+ * accepts: expert_bytes = C~*a, kv_bytes = kappa~*b.  *moved (may be NULL) = 0 when the dead zone held. */
+int wisp_mvwsa_propose(wisp_ctx* ctx, const wisp_mvwsa_in* in, uint64_t* expert_bytes, uint64_t* kv_bytes,
+                       int32_t* moved);
+/* Expert miss curve from the library's reuse-distance histograms: host m_exp[0..n-1],
+ * m_exp[C] = (decayed) number of references with stack distance > C, summed over layers.  `decay` in
+ * (0,1] multiplies all bins AFTER the read ("decayed"); 1.0 = leave unchanged.
+ * Histograms are fed from the routing of every forward while tracking is on (wisp_mvwsa_track). */
+int wisp_mvwsa_miss_curve(wisp_ctx* ctx, double* m_exp, int32_t n, double decay);
+int wisp_mvwsa_track(wisp_ctx* ctx, int32_t on);
+
+const char* wisp_last_error(wisp_ctx* ctx);
+/* Library build info, e.g. "libwisp sm_100a ..." (static string). */
+const char* wisp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WISP_H_ */

@@ -1,0 +1,375 @@
+// residency.cuh -- (a2) slot-table residency lookup = Algorithm 1 WISPLAYER.STEP(R)
+// run ON THE DEVICE (the paper runs it in Python on the host and names that the overhead to remove,
+// PAPER.md:444), plus the resize of a7.  Integer work only; one CTA per layer call.
+//
+// Readings: G1 M = R \ dom(pi); G2 ties -> lower slot; G3 M ascending id <-> U in key order;
+// G4 empty slots (tau = 0) first; G5 waves of <= C ascending ids; G6 LFU key (f, tau, slot), empty f = -1;
+// G24 one tick per wave.
+#pragma once
+#include "common.cuh"
+
+namespace wisp {
+
+constexpr int kPlanThreads = 1024;
+
+struct PlanArgs {
+  const int* ids;   // [n_pairs] routed expert ids (t*k + rank order)
+  int n_pairs;
+  int E, C, policy, layer;
+  LayerState st;
+  PlanPtrs plan;
+  HostPlan* host_plan;            // nullable (MEMCPY path)
+  wisp_trace_event* trace;        // ring
+  u64* trace_ctr;                 // [0] count, [1] dropped
+  u64 trace_cap;
+  int trace_on;
+  int track;                      // MV-WSA reuse-distance tracking
+  int build_pairs;                // build pair_list here (small n_pairs) or leave it to group_pairs_kernel
+};
+
+// exclusive scan over the block (blockDim.x == kPlanThreads); ws = 33 ints of scratch
+__device__ __forceinline__ int block_excl_scan(int v, int* ws, int& total) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int n = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += n;
+  }
+  if (lane == 31) ws[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    int s = ws[lane], si = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int n = __shfl_up_sync(0xffffffffu, si, o);
+      if (lane >= o) si += n;
+    }
+    ws[lane] = si - s;
+    if (lane == 31) ws[32] = si;
+  }
+  __syncthreads();
+  total = ws[32];
+  int r = inc - v + ws[wid];
+  __syncthreads();
+  return r;
+}
+
+// victim order: LRU (tau, slot); LFU (f+1 or 0 for empty, tau, slot)   -- ascending
+__device__ __forceinline__ bool key_less(u64 fa, u64 ta, int sa, u64 fb, u64 tb, int sb) {
+  if (fa != fb) return fa < fb;
+  if (ta != tb) return ta < tb;
+  return sa < sb;
+}
+
+__global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a) {
+  __shared__ unsigned bitmap[kMaxExperts / 32];
+  __shared__ int s_cnt[kMaxExperts];
+  __shared__ int s_R[kMaxExperts];        // sorted distinct routed ids
+  __shared__ int s_pi[kMaxExperts];
+  __shared__ int s_pinv[kMaxExperts];
+  __shared__ u64 s_tau[kMaxExperts];
+  __shared__ u64 s_kf[kMaxExperts];       // LFU component of the victim key per slot
+  __shared__ unsigned char s_inw[kMaxExperts];
+  __shared__ unsigned char s_elig[kMaxExperts];
+  __shared__ int s_victim[kMaxExperts];
+  __shared__ int s_ws[33];
+  __shared__ int s_nR;
+  __shared__ u64 s_clock;
+  __shared__ int s_evict;
+
+  const int tid = threadIdx.x;
+  const int E = a.E, C = a.C;
+  if (tid < kMaxExperts / 32) bitmap[tid] = 0u;
+  if (tid < E) { s_cnt[tid] = 0; s_pi[tid] = a.st.pi[tid]; }
+  if (tid < C) { s_pinv[tid] = a.st.pi_inv[tid]; s_tau[tid] = a.st.tau[tid]; }
+  if (tid == 0) { s_clock = a.st.scal[0]; s_evict = 0; }
+  __syncthreads();
+
+  // ---- R = set of routed ids; per-expert pair counts ----
+  for (int p = tid; p < a.n_pairs; p += kPlanThreads) {
+    int e = a.ids[p];
+    atomicOr(&bitmap[e >> 5], 1u << (e & 31));
+    atomicAdd(&s_cnt[e], 1);
+  }
+  __syncthreads();
+  int total = 0;
+  {
+    const int present = (tid < E) ? ((bitmap[tid >> 5] >> (tid & 31)) & 1) : 0;
+    int pos = block_excl_scan(present, s_ws, total);
+    if (present) s_R[pos] = tid;
+    if (tid == 0) s_nR = total;
+  }
+  const int nR = total;
+  {
+    int tot2;
+    int off = block_excl_scan(tid < E ? s_cnt[tid] : 0, s_ws, tot2);
+    if (tid < E) { a.plan.exp_offset[tid] = off; a.plan.exp_count[tid] = s_cnt[tid]; }
+    if (tid == 0) a.plan.exp_offset[E] = tot2;
+    if (a.build_pairs && tid < a.n_pairs) {
+      // stable grouping for small n_pairs: rank among lower-indexed pairs of the same expert
+      const int e = a.ids[tid];
+      int r = 0;
+      for (int q = 0; q < tid; ++q) r += (a.ids[q] == e);
+      // offset of expert e (recompute from the scan of thread e: read back from global after sync below)
+      s_victim[tid] = r;   // borrow as scratch (n_pairs <= kMaxExperts in this mode)
+    }
+  }
+  __syncthreads();
+  if (a.build_pairs && tid < a.n_pairs) {
+    const int e = a.ids[tid];
+    // exp_offset[e] was written by thread e of this block; visible after __syncthreads + same-CTA global write
+    a.plan.pair_list[a.plan.exp_offset[e] + s_victim[tid]] = tid;
+  }
+  __syncthreads();
+
+  // ---- MV-WSA reuse-distance tracking: stack distance of every reference ----
+  if (a.track && nR > 0) {
+    __shared__ u64 s_last[kMaxExperts];
+    if (tid < E) s_last[tid] = a.st.last_pos[tid];
+    __syncthreads();
+    const u64 base = a.st.scal[6];   // linear position counter of this layer
+    if (tid < nR) {
+      const int e = s_R[tid];
+      const u64 mine = s_last[e];
+      int bin;
+      if (mine == 0) {
+        bin = E + 1;                 // first reference: infinite distance
+      } else {
+        int dist = 1 + tid;          // e itself + the tid lower ids of this step (referenced just before)
+        for (int o = 0; o < E; ++o) {
+          if (o == e) continue;
+          const bool in_step_before = ((bitmap[o >> 5] >> (o & 31)) & 1) && o < e;
+          if (!in_step_before && s_last[o] > mine) ++dist;
+        }
+        bin = dist > E ? E + 1 : dist;
+      }
+      atomicAdd(&a.st.hist[bin], 1ull);
+    }
+    __syncthreads();
+    if (tid < nR) a.st.last_pos[s_R[tid]] = base + 1 + tid;
+    if (tid == 0) a.st.scal[6] = base + nR;
+    __syncthreads();
+  }
+
+  // ---- Algorithm 1 per wave ----
+  const int n_waves = (nR + C - 1) / C;
+  const u64 step_no = a.st.scal[1];
+  bool trace_ok = false;
+  u64 trace_base = 0;
+  if (a.trace_on) {
+    trace_base = a.trace_ctr[0];
+    trace_ok = trace_base + (u64)nR <= a.trace_cap;
+  }
+  int hits_total = 0, miss_total = 0;
+  for (int wv = 0; wv < n_waves; ++wv) {
+    const int lo = wv * C;
+    const int nw = min(C, nR - lo);
+    if (tid < E) s_inw[tid] = 0;
+    __syncthreads();
+    int e = -1, is_miss = 0;
+    if (tid < nw) { e = s_R[lo + tid]; s_inw[e] = 1; is_miss = s_pi[e] < 0; }
+    __syncthreads();
+    int n_miss;
+    const int mi = block_excl_scan(is_miss, s_ws, n_miss);       // line 2: M = R \ dom(pi), ascending id
+    // line 3: U = {s : pi^-1(s) not in R} in increasing key
+    if (tid < C) {
+      const int occ = s_pinv[tid];
+      s_elig[tid] = (occ < 0) || !s_inw[occ];
+      s_kf[tid] = (a.policy == WISP_LFU) ? (occ < 0 ? 0ull : a.st.freq[occ] + 1ull) : 0ull;
+    }
+    __syncthreads();
+    if (tid < C && s_elig[tid] && n_miss > 0) {
+      const u64 kf = s_kf[tid], kt = s_tau[tid];
+      int rank = 0;
+      for (int o = 0; o < C; ++o)
+        if (s_elig[o] && key_less(s_kf[o], s_tau[o], o, kf, kt, tid)) ++rank;
+      if (rank < n_miss) s_victim[rank] = tid;
+    }
+    __syncthreads();
+    // lines 4-8: assign, (copy happens in the fetch step), update the maps
+    int slot = -1, old = -1;
+    if (tid < nw) {
+      if (is_miss) {
+        slot = s_victim[mi];
+        old = s_pinv[slot];
+        if (old >= 0) { s_pi[old] = -1; atomicAdd(&s_evict, 1); }
+        s_pi[e] = slot;
+        s_pinv[slot] = e;
+      } else {
+        slot = s_pi[e];
+      }
+    }
+    if (tid == 0) s_clock += 1;                                   // line 9: c <- c + 1
+    __syncthreads();
+    if (tid < nw) {
+      s_tau[slot] = s_clock;                                      // tau[pi(e)] <- c
+      a.st.freq[e] += 1ull;
+      const int idx = lo + tid;
+      a.plan.entry_expert[idx] = e;
+      a.plan.entry_slot[idx] = slot;
+      a.plan.entry_miss[idx] = is_miss;
+      if (a.host_plan) {
+        a.host_plan->entry_expert[idx] = e;
+        a.host_plan->entry_slot[idx] = slot;
+        a.host_plan->entry_miss[idx] = is_miss;
+      }
+      if (trace_ok) {
+        wisp_trace_event ev;
+        ev.step = step_no; ev.layer = (uint32_t)a.layer; ev.wave = (uint32_t)wv;
+        ev.expert = e; ev.slot = slot; ev.evicted = old; ev.kind = is_miss ? 1u : 0u;
+        a.trace[trace_base + idx] = ev;
+      }
+    }
+    hits_total += nw - n_miss;
+    miss_total += n_miss;
+    __syncthreads();
+  }
+
+  // ---- write back ----
+  if (tid < E) a.st.pi[tid] = s_pi[tid];
+  if (tid < C) { a.st.pi_inv[tid] = s_pinv[tid]; a.st.tau[tid] = s_tau[tid]; }
+  if (tid == 0) {
+    a.plan.hdr[0] = n_waves; a.plan.hdr[1] = nR; a.plan.hdr[2] = miss_total; a.plan.hdr[3] = a.n_pairs;
+    if (a.host_plan) {
+      a.host_plan->n_ref = nR; a.host_plan->n_miss = miss_total; a.host_plan->n_pairs = a.n_pairs;
+      __threadfence_system();
+      a.host_plan->n_waves = n_waves;
+    }
+    a.st.scal[0] = s_clock;
+    if (nR > 0) a.st.scal[1] = step_no + 1;
+    a.st.scal[2] += (u64)hits_total;
+    a.st.scal[3] += (u64)miss_total;
+    a.st.scal[4] += (u64)s_evict;
+    a.st.scal[5] += (u64)nR;
+    if (a.trace_on) {
+      if (trace_ok) a.trace_ctr[0] = trace_base + (u64)nR;
+      else a.trace_ctr[1] += (u64)nR;
+    }
+  }
+}
+
+// Stable grouping of (token, rank) pairs by expert for large n_pairs: one CTA per expert.
+__global__ void __launch_bounds__(256) group_pairs_kernel(const int* __restrict__ ids, int n_pairs, PlanPtrs plan) {
+  __shared__ int s_ws[9];
+  const int e = blockIdx.x;
+  if (plan.exp_count[e] == 0) return;
+  int pos = plan.exp_offset[e];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int base = 0; base < n_pairs; base += 256) {
+    const int p = base + threadIdx.x;
+    const bool m = p < n_pairs && ids[p] == e;
+    const unsigned bal = __ballot_sync(0xffffffffu, m);
+    if (lane == 0) s_ws[wid] = __popc(bal);
+    __syncthreads();
+    int before = 0, tot = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { const int c = s_ws[i]; if (i < wid) before += c; tot += c; }
+    if (m) plan.pair_list[pos + before + __popc(bal & ((1u << lane) - 1u))] = p;
+    pos += tot;
+    __syncthreads();
+  }
+}
+
+// ---- resize (a7, G13) -------------------------------------------------------
+// One CTA, one layer.  Shrink: keep the C_new best residents (LRU: tau desc, slot asc; LFU: f desc, tau
+// desc, slot asc), drop the rest, move survivors living in slots >= C_new to the lowest free slots.
+// moves[2*i] = src slot, moves[2*i+1] = dst slot; *n_moves = count.  Grow: new slots empty, tau = 0.
+struct ResizeArgs {
+  int E, C_old, C_new, policy, layer;
+  LayerState st;
+  int* moves;
+  int* n_moves;
+  wisp_trace_event* trace;
+  u64* trace_ctr;
+  u64 trace_cap;
+  int trace_on;
+};
+
+__global__ void __launch_bounds__(kPlanThreads) residency_resize_kernel(ResizeArgs a) {
+  __shared__ int s_pinv[kMaxExperts];
+  __shared__ u64 s_tau[kMaxExperts];
+  __shared__ u64 s_f[kMaxExperts];
+  __shared__ unsigned char s_keep[kMaxExperts];
+  __shared__ int s_ws[33];
+  const int tid = threadIdx.x;
+  const int Co = a.C_old, Cn = a.C_new;
+  if (Cn >= Co) {
+    if (tid >= Co && tid < Cn) { a.st.pi_inv[tid] = -1; a.st.tau[tid] = 0; }
+    if (tid == 0) *a.n_moves = 0;
+    return;
+  }
+  if (tid < Co) {
+    s_pinv[tid] = a.st.pi_inv[tid];
+    s_tau[tid] = a.st.tau[tid];
+    s_f[tid] = (a.policy == WISP_LFU && s_pinv[tid] >= 0) ? a.st.freq[s_pinv[tid]] : 0ull;
+  }
+  __syncthreads();
+  int occ = -1, keep = 0;
+  if (tid < Co) {
+    occ = s_pinv[tid];
+    if (occ >= 0) {
+      int rank = 0;   // number of occupied slots that come before this one in the keep order
+      for (int o = 0; o < Co; ++o) {
+        if (o == tid || s_pinv[o] < 0) continue;
+        bool before;
+        if (s_f[o] != s_f[tid]) before = s_f[o] > s_f[tid];
+        else if (s_tau[o] != s_tau[tid]) before = s_tau[o] > s_tau[tid];
+        else before = o < tid;
+        rank += before;
+      }
+      keep = rank < Cn;
+    }
+    s_keep[tid] = (unsigned char)keep;
+  }
+  __syncthreads();
+  const int is_drop = (tid < Co && occ >= 0 && !keep);
+  const int is_move = (tid < Co && keep && tid >= Cn);
+  const int is_free = (tid < Cn && !(occ >= 0 && keep));
+  int n_drop, n_move, n_free;
+  const int di = block_excl_scan(is_drop, s_ws, n_drop);
+  const int mi = block_excl_scan(is_move, s_ws, n_move);
+  const int fi = block_excl_scan(is_free, s_ws, n_free);
+  __shared__ int s_free[kMaxExperts];
+  if (is_free) s_free[fi] = tid;
+  __syncthreads();
+  bool trace_ok = false;
+  u64 tb = 0;
+  if (a.trace_on) { tb = a.trace_ctr[0]; trace_ok = tb + (u64)(n_drop + n_move) <= a.trace_cap; }
+  const u64 step_no = a.st.scal[1];
+  if (is_drop) {
+    a.st.pi[occ] = -1;
+    a.st.pi_inv[tid] = -1;
+    a.st.tau[tid] = 0;
+    if (trace_ok) {
+      wisp_trace_event ev;
+      ev.step = step_no; ev.layer = (uint32_t)a.layer; ev.wave = 0; ev.expert = occ; ev.slot = tid; ev.evicted = -1; ev.kind = 2u;
+      a.trace[tb + di] = ev;
+    }
+  }
+  __syncthreads();
+  if (is_move) {
+    const int dst = s_free[mi];
+    a.st.pi[occ] = dst;
+    a.st.pi_inv[dst] = occ;
+    a.st.tau[dst] = s_tau[tid];
+    a.st.pi_inv[tid] = -1;
+    a.st.tau[tid] = 0;
+    a.moves[2 * mi] = tid;
+    a.moves[2 * mi + 1] = dst;
+    if (trace_ok) {
+      wisp_trace_event ev;
+      ev.step = step_no; ev.layer = (uint32_t)a.layer; ev.wave = 0; ev.expert = occ; ev.slot = dst; ev.evicted = tid; ev.kind = 3u;
+      a.trace[tb + n_drop + mi] = ev;
+    }
+  }
+  if (tid == 0) {
+    *a.n_moves = n_move;
+    if (a.trace_on) {
+      if (trace_ok) a.trace_ctr[0] = tb + (u64)(n_drop + n_move);
+      else a.trace_ctr[1] += (u64)(n_drop + n_move);
+    }
+  }
+}
+
+}  // namespace wisp

@@ -1,0 +1,797 @@
+// wisp.cu -- context, C ABI (include/wisp.h) and launch orchestration of libwisp (sm_100a).
+// Host code only enqueues work; every step of the hot path (router, residency, fetch, FFN, combine)
+// runs in the kernels of router.cuh / residency.cuh / fetch.cuh / ffn_decode.cuh / ffn_prefill.cuh.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+#include "fetch.cuh"
+#include "ffn_decode.cuh"
+#include "ffn_prefill.cuh"
+#include "mvwsa.h"
+#include "residency.cuh"
+#include "router.cuh"
+
+using namespace wisp;
+
+struct wisp_ctx {
+  wisp_config cfg{};
+  u64 budget = 0;
+  size_t elem = 0, Me = 0, a_bytes = 0, blob_elems = 0;
+  int C = 0;
+  u64 kappa = 0, kv_reserved = 0, kv_peak = 0;
+  u64 resize_count = 0, failed_resize = 0;
+  int num_sms = 0;
+
+  char* arena = nullptr;
+  std::vector<void*> master;       // pinned, mapped; one allocation per layer
+  std::vector<char> registered;
+  char* router_w = nullptr;        // device [L][E][d]
+  float* router_bias = nullptr;    // device [L][E]
+
+  // per-layer residency state (device), each [L][...]
+  int *pi = nullptr, *pi_inv = nullptr;
+  u64 *tau = nullptr, *freq = nullptr, *scal = nullptr, *last_pos = nullptr, *hist = nullptr;
+
+  // per-forward scratch (device)
+  float* logits = nullptr;         // [maxT][E]
+  int* ids = nullptr;              // [L][maxT*k]
+  float* topw = nullptr;           // [L][maxT*k]
+  std::vector<int> last_T;
+  int last_layer = -1;
+  int* plan_mem = nullptr;
+  PlanPtrs plan{};
+  HostPlan* host_plan = nullptr;   // mapped pinned
+  float* act_f32 = nullptr;        // [kDecodeMaxTokens*k][d_ff]
+  char* act_T = nullptr;           // [maxT*k][d_ff] model dtype (prefill)
+  float* ystage = nullptr;         // [maxT*k][d]
+  char* xbuf[2] = {nullptr, nullptr};
+  char* ybuf = nullptr;
+  int* dbg_ids = nullptr;
+  size_t dbg_ids_cap = 0;
+  int* moves = nullptr;            // [2*E] + n_moves
+  int* bad_slots = nullptr;        // [E]
+
+  wisp_trace_event* trace = nullptr;
+  u64* trace_ctr = nullptr;        // device [2]
+  u64 trace_cap = 0;
+  int trace_on = 0;
+  int track = 0;
+  std::vector<double> host_hist;
+
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_plan = nullptr, ev_compute = nullptr, ev_copy = nullptr;
+  int fetch_timing = 0;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> timing_pool;
+  size_t timing_used = 0;
+  double fetch_ms = 0.0;
+
+  std::map<int, cudaGraphExec_t> graphs;
+  int grid_gate_up = 0, grid_down = 0, grid_fetch = 0;
+  std::string err;
+};
+
+namespace {
+
+const char* kVersion = "libwisp 0.1 (sm_100a; router/residency/fetch/ffn kernels; build " __DATE__ ")";
+
+int fail(wisp_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+
+#define CK(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess)                                                                         \
+      return fail(ctx, e_ == cudaErrorMemoryAllocation ? WISP_ENOMEM : WISP_ECUDA,                 \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                             \
+  } while (0)
+
+LayerState layer_state(wisp_ctx* c, int l) {
+  const size_t E = c->cfg.n_experts;
+  LayerState s;
+  s.pi = c->pi + l * E;
+  s.pi_inv = c->pi_inv + l * E;
+  s.tau = c->tau + l * E;
+  s.freq = c->freq + l * E;
+  s.scal = c->scal + l * 8;
+  s.last_pos = c->last_pos + l * E;
+  s.hist = c->hist + l * (E + 2);
+  return s;
+}
+
+void drop_graphs(wisp_ctx* c) {
+  for (auto& g : c->graphs) cudaGraphExecDestroy(g.second);
+  c->graphs.clear();
+}
+
+void harvest_timing(wisp_ctx* c, bool all) {
+  size_t keep = 0;
+  for (size_t i = 0; i < c->timing_used; ++i) {
+    auto& p = c->timing_pool[i];
+    if (all) cudaEventSynchronize(p.second);
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) c->fetch_ms += ms;
+    else std::swap(c->timing_pool[keep++], p);
+  }
+  c->timing_used = keep;
+}
+
+bool timing_pair(wisp_ctx* c, cudaEvent_t* a, cudaEvent_t* b) {
+  if (c->timing_used == c->timing_pool.size()) {
+    harvest_timing(c, false);
+    if (c->timing_used == c->timing_pool.size()) {
+      if (c->timing_pool.size() >= 4096) harvest_timing(c, true);
+      else {
+        cudaEvent_t x, y;
+        if (cudaEventCreate(&x) != cudaSuccess || cudaEventCreate(&y) != cudaSuccess) return false;
+        c->timing_pool.push_back({x, y});
+      }
+    }
+  }
+  *a = c->timing_pool[c->timing_used].first;
+  *b = c->timing_pool[c->timing_used].second;
+  ++c->timing_used;
+  return true;
+}
+
+template <typename T>
+int launch_router(wisp_ctx* ctx, int layer, const void* x, int T_, cudaStream_t st) {
+  const auto& cfg = ctx->cfg;
+  const int E = cfg.n_experts, d = cfg.d_model, k = cfg.top_k;
+  const T* wr = reinterpret_cast<const T*>(ctx->router_w) + (size_t)layer * E * d;
+  dim3 g((E + 7) / 8, (T_ + kRouterTokTile - 1) / kRouterTokTile);
+  router_logits_kernel<T><<<g, 256, 0, st>>>(reinterpret_cast<const T*>(x), wr, ctx->router_bias + (size_t)layer * E,
+                                             ctx->logits, T_, E, d);
+  const size_t off = (size_t)layer * cfg.max_tokens * k;
+  topk_softmax_kernel<<<(T_ + 3) / 4, 128, 4 * E * sizeof(float), st>>>(ctx->logits, ctx->ids + off, ctx->topw + off, T_,
+                                                                        E, k);
+  CK(cudaGetLastError());
+  return WISP_OK;
+}
+
+int launch_plan(wisp_ctx* ctx, int layer, const int* ids, int n_pairs, bool want_host, cudaStream_t st) {
+  PlanArgs a;
+  a.ids = ids;
+  a.n_pairs = n_pairs;
+  a.E = ctx->cfg.n_experts;
+  a.C = ctx->C;
+  a.policy = ctx->cfg.policy;
+  a.layer = layer;
+  a.st = layer_state(ctx, layer);
+  a.plan = ctx->plan;
+  a.host_plan = want_host ? ctx->host_plan : nullptr;
+  a.trace = ctx->trace;
+  a.trace_ctr = ctx->trace_ctr;
+  a.trace_cap = ctx->trace_cap;
+  a.trace_on = ctx->trace_on;
+  a.track = ctx->track;
+  a.build_pairs = n_pairs <= 256;
+  residency_plan_kernel<<<1, kPlanThreads, 0, st>>>(a);
+  if (!a.build_pairs) group_pairs_kernel<<<a.E, 256, 0, st>>>(ids, n_pairs, ctx->plan);
+  CK(cudaGetLastError());
+  return WISP_OK;
+}
+
+// Miss path for one wave.  ZEROCOPY: one kernel on the compute stream.  MEMCPY: host-read miss list ->
+// cudaMemcpyAsync on the copy stream, fenced both ways with events.
+int fetch_wave(wisp_ctx* ctx, int layer, int wave, bool host_known, cudaStream_t st) {
+  const auto& cfg = ctx->cfg;
+  const size_t blob_vec = ctx->Me / 16;
+  cudaEvent_t t0 = nullptr, t1 = nullptr;
+  if (!host_known) {
+    if (ctx->fetch_timing && timing_pair(ctx, &t0, &t1)) CK(cudaEventRecord(t0, st));
+    fetch_zerocopy_kernel<<<ctx->grid_fetch, kFetchThreads, 0, st>>>(
+        ctx->plan, wave, ctx->C, reinterpret_cast<const uint4*>(ctx->master[layer]),
+        reinterpret_cast<uint4*>(ctx->arena), blob_vec, cfg.n_layers, layer);
+    CK(cudaGetLastError());
+    if (t1) CK(cudaEventRecord(t1, st));
+    return WISP_OK;
+  }
+  const HostPlan* hp = ctx->host_plan;
+  const int lo = wave * ctx->C, hi = std::min(hp->n_ref, lo + ctx->C);
+  bool any = false;
+  for (int i = lo; i < hi; ++i) any |= hp->entry_miss[i] != 0;
+  if (!any) return WISP_OK;
+  CK(cudaEventRecord(ctx->ev_compute, st));
+  CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_compute, 0));
+  if (ctx->fetch_timing && timing_pair(ctx, &t0, &t1)) CK(cudaEventRecord(t0, ctx->copy_stream));
+  for (int i = lo; i < hi; ++i) {
+    if (!hp->entry_miss[i]) continue;
+    const char* src = static_cast<const char*>(ctx->master[layer]) + (size_t)hp->entry_expert[i] * ctx->Me;
+    char* dst = ctx->arena + ((size_t)hp->entry_slot[i] * cfg.n_layers + layer) * ctx->Me;
+    CK(cudaMemcpyAsync(dst, src, ctx->Me, cudaMemcpyHostToDevice, ctx->copy_stream));
+  }
+  if (t1) CK(cudaEventRecord(t1, ctx->copy_stream));
+  CK(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
+  CK(cudaStreamWaitEvent(st, ctx->ev_copy, 0));
+  return WISP_OK;
+}
+
+template <typename T>
+int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, cudaStream_t st) {
+  const auto& cfg = ctx->cfg;
+  const int d = cfg.d_model, dff = cfg.d_ff, k = cfg.top_k, L = cfg.n_layers;
+  const T* pool = reinterpret_cast<const T*>(ctx->arena);
+  if (T_ <= kDecodeMaxTokens) {
+    decode_gate_up_kernel<T><<<ctx->grid_gate_up, kFfnThreads, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L,
+                                                                        layer, reinterpret_cast<const T*>(x),
+                                                                        ctx->act_f32, d, dff, k);
+    decode_down_kernel<T><<<ctx->grid_down, kFfnThreads, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
+                                                                  ctx->act_f32, ctx->ystage, d, dff);
+  } else {
+    const int ptiles = (T_ + kPfTile - 1) / kPfTile;   // an expert can receive at most T pairs
+    dim3 g0(dff / kPfTile, ptiles, ctx->C), g1(d / kPfTile, ptiles, ctx->C);
+    prefill_ffn_kernel<T, 0><<<g0, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
+                                                 reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
+                                                 ctx->ystage, d, dff, k);
+    prefill_ffn_kernel<T, 1><<<g1, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
+                                                 reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
+                                                 ctx->ystage, d, dff, k);
+  }
+  CK(cudaGetLastError());
+  return WISP_OK;
+}
+
+// One MoE layer: router -> residency -> per wave (fetch, FFN) -> combine.  x_next != nullptr also writes
+// the residual successor (stack helper).
+template <typename T>
+int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
+  const auto& cfg = ctx->cfg;
+  const int k = cfg.top_k, E = cfg.n_experts;
+  const int n_pairs = T_ * k;
+  int rc = launch_router<T>(ctx, layer, x, T_, st);
+  if (rc) return rc;
+  const size_t off = (size_t)layer * cfg.max_tokens * k;
+  const bool memcpy_path = cfg.fetch == WISP_FETCH_MEMCPY;
+  rc = launch_plan(ctx, layer, ctx->ids + off, n_pairs, memcpy_path, st);
+  if (rc) return rc;
+  int n_waves;
+  if (memcpy_path) {
+    CK(cudaEventRecord(ctx->ev_plan, st));
+    CK(cudaEventSynchronize(ctx->ev_plan));      // the host must see the miss list
+    n_waves = ctx->host_plan->n_waves;
+  } else {
+    n_waves = (std::min(E, n_pairs) + ctx->C - 1) / ctx->C;   // worst case; empty waves exit at once
+  }
+  for (int w = 0; w < n_waves; ++w) {
+    rc = fetch_wave(ctx, layer, w, memcpy_path, st);
+    if (rc) return rc;
+    rc = launch_ffn_wave<T>(ctx, layer, w, x, T_, st);
+    if (rc) return rc;
+  }
+  const size_t n = (size_t)T_ * cfg.d_model;
+  combine_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(ctx->ystage, ctx->topw + off, reinterpret_cast<T*>(out),
+                                                                 x_next ? reinterpret_cast<const T*>(x) : nullptr,
+                                                                 reinterpret_cast<T*>(x_next), T_, cfg.d_model, k);
+  CK(cudaGetLastError());
+  ctx->last_T[layer] = T_;
+  ctx->last_layer = layer;
+  return WISP_OK;
+}
+
+int forward_layer_any(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
+  return ctx->cfg.dtype == WISP_F32 ? forward_layer<float>(ctx, layer, x, T_, out, x_next, st)
+                                    : forward_layer<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st);
+}
+
+int check_forward_args(wisp_ctx* ctx, int layer_lo, int layer_hi, const void* hidden, int n_tokens, void* out) {
+  if (!ctx) return WISP_EINVAL;
+  if (n_tokens < 0 || n_tokens > ctx->cfg.max_tokens) return fail(ctx, WISP_EINVAL, "n_tokens out of range");
+  if (n_tokens > 0 && (!hidden || !out)) return fail(ctx, WISP_EINVAL, "null hidden/out");
+  for (int l = layer_lo; l < layer_hi; ++l) {
+    if (l < 0 || l >= ctx->cfg.n_layers) return fail(ctx, WISP_EINVAL, "layer out of range");
+    if (!ctx->registered[l]) return fail(ctx, WISP_ESTATE, "layer not registered");
+  }
+  return WISP_OK;
+}
+
+template <typename F>
+int occupancy_grid(wisp_ctx* ctx, F kernel, int threads, int cap_per_sm) {
+  int nb = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, threads, 0) != cudaSuccess || nb < 1) nb = 1;
+  return ctx->num_sms * std::min(nb, cap_per_sm);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* wisp_version(void) { return kVersion; }
+
+const char* wisp_last_error(wisp_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
+  if (!cfg || !out) return WISP_EINVAL;
+  *out = nullptr;
+  if (cfg->n_layers < 1 || cfg->n_experts < 1 || cfg->n_experts > kMaxExperts || cfg->top_k < 1 ||
+      cfg->top_k > kMaxTopK || cfg->top_k > cfg->n_experts || cfg->d_model < 256 || cfg->d_model % 256 ||
+      cfg->d_ff < 256 || cfg->d_ff % 256 || cfg->max_tokens < 1 ||
+      (cfg->dtype != WISP_F32 && cfg->dtype != WISP_BF16) || (cfg->policy != WISP_LRU && cfg->policy != WISP_LFU) ||
+      (cfg->fetch != WISP_FETCH_MEMCPY && cfg->fetch != WISP_FETCH_ZEROCOPY))
+    return WISP_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return WISP_ECUDA;   // no CPU fallback
+  wisp_ctx* ctx = new wisp_ctx();
+  ctx->cfg = *cfg;
+  ctx->budget = budget_bytes;
+  ctx->elem = cfg->dtype == WISP_F32 ? 4 : 2;
+  ctx->blob_elems = 3 * (size_t)cfg->d_model * cfg->d_ff;
+  ctx->Me = ctx->blob_elems * ctx->elem;
+  ctx->a_bytes = ctx->Me * cfg->n_layers;
+  const u64 b = cfg->kv_block_bytes;
+  const u64 kv0 = b ? cfg->kv_floor_blocks * b : 0;
+  if (kv0 > budget_bytes || (budget_bytes - kv0) / ctx->a_bytes < 1) {
+    delete ctx;
+    return WISP_EBUDGET;
+  }
+  ctx->C = (int)std::min<u64>(cfg->n_experts, (budget_bytes - kv0) / ctx->a_bytes);
+  ctx->kappa = b ? (budget_bytes - (u64)ctx->C * ctx->a_bytes) / b : 0;
+  const int L = cfg->n_layers, E = cfg->n_experts, k = cfg->top_k, d = cfg->d_model, dff = cfg->d_ff;
+  const size_t maxT = cfg->max_tokens;
+  ctx->master.assign(L, nullptr);
+  ctx->registered.assign(L, 0);
+  ctx->last_T.assign(L, 0);
+  ctx->host_hist.assign(E + 2, 0.0);
+  ctx->trace_cap = cfg->trace_capacity ? cfg->trace_capacity : (1ull << 20);
+  cudaDeviceProp prop;
+  int dev = 0;
+  auto bail = [&](int code, const char* what, cudaError_t e) {
+    std::fprintf(stderr, "wisp_create: %s: %s\n", what, cudaGetErrorString(e));
+    wisp_destroy(ctx);
+    return code;
+  };
+#define CKC(call)                                                                                            \
+  do {                                                                                                       \
+    cudaError_t e_ = (call);                                                                                 \
+    if (e_ != cudaSuccess) return bail(e_ == cudaErrorMemoryAllocation ? WISP_ENOMEM : WISP_ECUDA, #call, e_); \
+  } while (0)
+  CKC(cudaGetDevice(&dev));
+  CKC(cudaGetDeviceProperties(&prop, dev));
+  ctx->num_sms = prop.multiProcessorCount;
+  CKC(cudaMalloc(&ctx->arena, budget_bytes));
+  CKC(cudaMalloc(&ctx->router_w, (size_t)L * E * d * ctx->elem));
+  CKC(cudaMalloc(&ctx->router_bias, (size_t)L * E * sizeof(float)));
+  CKC(cudaMalloc(&ctx->pi, (size_t)L * E * sizeof(int)));
+  CKC(cudaMalloc(&ctx->pi_inv, (size_t)L * E * sizeof(int)));
+  CKC(cudaMalloc(&ctx->tau, (size_t)L * E * sizeof(u64)));
+  CKC(cudaMalloc(&ctx->freq, (size_t)L * E * sizeof(u64)));
+  CKC(cudaMalloc(&ctx->scal, (size_t)L * 8 * sizeof(u64)));
+  CKC(cudaMalloc(&ctx->last_pos, (size_t)L * E * sizeof(u64)));
+  CKC(cudaMalloc(&ctx->hist, (size_t)L * (E + 2) * sizeof(u64)));
+  CKC(cudaMemset(ctx->pi, 0xff, (size_t)L * E * sizeof(int)));
+  CKC(cudaMemset(ctx->pi_inv, 0xff, (size_t)L * E * sizeof(int)));
+  CKC(cudaMemset(ctx->tau, 0, (size_t)L * E * sizeof(u64)));
+  CKC(cudaMemset(ctx->freq, 0, (size_t)L * E * sizeof(u64)));
+  CKC(cudaMemset(ctx->scal, 0, (size_t)L * 8 * sizeof(u64)));
+  CKC(cudaMemset(ctx->last_pos, 0, (size_t)L * E * sizeof(u64)));
+  CKC(cudaMemset(ctx->hist, 0, (size_t)L * (E + 2) * sizeof(u64)));
+  CKC(cudaMalloc(&ctx->logits, maxT * E * sizeof(float)));
+  CKC(cudaMalloc(&ctx->ids, (size_t)L * maxT * k * sizeof(int)));
+  CKC(cudaMalloc(&ctx->topw, (size_t)L * maxT * k * sizeof(float)));
+  {
+    const size_t n_int = 4 + 3 * (size_t)E + E + (E + 1) + maxT * k;
+    CKC(cudaMalloc(&ctx->plan_mem, n_int * sizeof(int)));
+    CKC(cudaMemset(ctx->plan_mem, 0, n_int * sizeof(int)));
+    int* p = ctx->plan_mem;
+    ctx->plan.hdr = p; p += 4;
+    ctx->plan.entry_expert = p; p += E;
+    ctx->plan.entry_slot = p; p += E;
+    ctx->plan.entry_miss = p; p += E;
+    ctx->plan.exp_count = p; p += E;
+    ctx->plan.exp_offset = p; p += E + 1;
+    ctx->plan.pair_list = p;
+  }
+  CKC(cudaHostAlloc(&ctx->host_plan, sizeof(HostPlan), cudaHostAllocMapped));
+  std::memset(ctx->host_plan, 0, sizeof(HostPlan));
+  CKC(cudaMalloc(&ctx->act_f32, (size_t)kDecodeMaxTokens * k * dff * sizeof(float)));
+  CKC(cudaMalloc(&ctx->act_T, maxT * k * dff * ctx->elem));
+  CKC(cudaMalloc(&ctx->ystage, maxT * k * d * sizeof(float)));
+  CKC(cudaMalloc(&ctx->xbuf[0], maxT * d * ctx->elem));
+  CKC(cudaMalloc(&ctx->xbuf[1], maxT * d * ctx->elem));
+  CKC(cudaMalloc(&ctx->ybuf, maxT * d * ctx->elem));
+  CKC(cudaMalloc(&ctx->moves, (2 * (size_t)E + 1) * sizeof(int)));
+  CKC(cudaMalloc(&ctx->bad_slots, (size_t)E * sizeof(int)));
+  CKC(cudaMalloc(&ctx->trace, ctx->trace_cap * sizeof(wisp_trace_event)));
+  CKC(cudaMalloc(&ctx->trace_ctr, 2 * sizeof(u64)));
+  CKC(cudaMemset(ctx->trace_ctr, 0, 2 * sizeof(u64)));
+  CKC(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+  CKC(cudaEventCreateWithFlags(&ctx->ev_plan, cudaEventDisableTiming));
+  CKC(cudaEventCreateWithFlags(&ctx->ev_compute, cudaEventDisableTiming));
+  CKC(cudaEventCreateWithFlags(&ctx->ev_copy, cudaEventDisableTiming));
+#undef CKC
+  if (cfg->dtype == WISP_F32) {
+    ctx->grid_gate_up = occupancy_grid(ctx, decode_gate_up_kernel<float>, kFfnThreads, 8);
+    ctx->grid_down = occupancy_grid(ctx, decode_down_kernel<float>, kFfnThreads, 8);
+  } else {
+    ctx->grid_gate_up = occupancy_grid(ctx, decode_gate_up_kernel<__nv_bfloat16>, kFfnThreads, 8);
+    ctx->grid_down = occupancy_grid(ctx, decode_down_kernel<__nv_bfloat16>, kFfnThreads, 8);
+  }
+  ctx->grid_fetch = ctx->num_sms * 2;
+  *out = ctx;
+  return WISP_OK;
+}
+
+int wisp_destroy(wisp_ctx* ctx) {
+  if (!ctx) return WISP_EINVAL;
+  cudaDeviceSynchronize();
+  drop_graphs(ctx);
+  for (void* m : ctx->master)
+    if (m) cudaFreeHost(m);
+  void* dev_ptrs[] = {ctx->arena,    ctx->router_w, ctx->router_bias, ctx->pi,      ctx->pi_inv,  ctx->tau,
+                      ctx->freq,     ctx->scal,     ctx->last_pos,    ctx->hist,    ctx->logits,  ctx->ids,
+                      ctx->topw,     ctx->plan_mem, ctx->act_f32,     ctx->act_T,   ctx->ystage,  ctx->xbuf[0],
+                      ctx->xbuf[1],  ctx->ybuf,     ctx->dbg_ids,     ctx->moves,   ctx->bad_slots, ctx->trace,
+                      ctx->trace_ctr};
+  for (void* p : dev_ptrs)
+    if (p) cudaFree(p);
+  if (ctx->host_plan) cudaFreeHost(ctx->host_plan);
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+  for (cudaEvent_t e : {ctx->ev_plan, ctx->ev_compute, ctx->ev_copy})
+    if (e) cudaEventDestroy(e);
+  for (auto& p : ctx->timing_pool) {
+    cudaEventDestroy(p.first);
+    cudaEventDestroy(p.second);
+  }
+  delete ctx;
+  return WISP_OK;
+}
+
+int wisp_register_host_experts(wisp_ctx* ctx, int32_t layer, const void* experts, const void* router_w,
+                               const float* router_bias) {
+  if (!ctx || !experts || !router_w) return fail(ctx, WISP_EINVAL, "null argument");
+  if (layer < 0 || layer >= ctx->cfg.n_layers) return fail(ctx, WISP_EINVAL, "layer out of range");
+  if (ctx->registered[layer]) return fail(ctx, WISP_ESTATE, "layer already registered");
+  const size_t E = ctx->cfg.n_experts, d = ctx->cfg.d_model;
+  void* m = nullptr;
+  CK(cudaHostAlloc(&m, E * ctx->Me, cudaHostAllocMapped | cudaHostAllocPortable));
+  std::memcpy(m, experts, E * ctx->Me);
+  ctx->master[layer] = m;
+  CK(cudaMemcpy(ctx->router_w + (size_t)layer * E * d * ctx->elem, router_w, E * d * ctx->elem, cudaMemcpyHostToDevice));
+  if (router_bias) CK(cudaMemcpy(ctx->router_bias + (size_t)layer * E, router_bias, E * sizeof(float), cudaMemcpyHostToDevice));
+  else CK(cudaMemset(ctx->router_bias + (size_t)layer * E, 0, E * sizeof(float)));
+  ctx->registered[layer] = 1;
+  return WISP_OK;
+}
+
+int wisp_moe_forward(wisp_ctx* ctx, int32_t layer, const void* hidden, int32_t n_tokens, void* out, void* cuda_stream) {
+  int rc = check_forward_args(ctx, layer, layer + 1, hidden, n_tokens, out);
+  if (rc) return rc;
+  if (n_tokens == 0) return WISP_OK;
+  return forward_layer_any(ctx, layer, hidden, n_tokens, out, nullptr, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void* hidden_out, void* cuda_stream) {
+  int rc = check_forward_args(ctx, 0, ctx ? ctx->cfg.n_layers : 0, hidden, n_tokens, hidden_out);
+  if (rc) return rc;
+  if (n_tokens == 0) return WISP_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int L = ctx->cfg.n_layers;
+  const size_t bytes = (size_t)n_tokens * ctx->cfg.d_model * ctx->elem;
+  CK(cudaMemcpyAsync(ctx->xbuf[0], hidden, bytes, cudaMemcpyDeviceToDevice, st));
+  auto chain = [&](cudaStream_t s) -> int {
+    for (int l = 0; l < L; ++l) {
+      int r = forward_layer_any(ctx, l, ctx->xbuf[l & 1], n_tokens, ctx->ybuf, ctx->xbuf[(l + 1) & 1], s);
+      if (r) return r;
+    }
+    return WISP_OK;
+  };
+  if (ctx->cfg.fetch == WISP_FETCH_ZEROCOPY && !ctx->fetch_timing && st != nullptr) {
+    auto it = ctx->graphs.find(n_tokens);
+    if (it == ctx->graphs.end()) {
+      cudaGraph_t g = nullptr;
+      CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+      rc = chain(st);
+      cudaError_t e = cudaStreamEndCapture(st, &g);
+      if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+      if (e != cudaSuccess) return fail(ctx, WISP_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+      cudaGraphExec_t ge = nullptr;
+      e = cudaGraphInstantiate(&ge, g, 0);
+      cudaGraphDestroy(g);
+      if (e != cudaSuccess) return fail(ctx, WISP_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
+      it = ctx->graphs.emplace(n_tokens, ge).first;
+    }
+    CK(cudaGraphLaunch(it->second, st));
+    for (int l = 0; l < L; ++l) ctx->last_T[l] = n_tokens;
+    ctx->last_layer = L - 1;
+  } else {
+    rc = chain(st);
+    if (rc) return rc;
+  }
+  CK(cudaMemcpyAsync(hidden_out, ctx->xbuf[L & 1], bytes, cudaMemcpyDeviceToDevice, st));
+  return WISP_OK;
+}
+
+int wisp_residual_add(wisp_ctx* ctx, const void* x, const void* y, void* out, int64_t n_elems, void* cuda_stream) {
+  if (!ctx || !x || !y || !out || n_elems < 0) return fail(ctx, WISP_EINVAL, "bad argument");
+  if (n_elems == 0) return WISP_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const unsigned g = (unsigned)((n_elems + 255) / 256);
+  if (ctx->cfg.dtype == WISP_F32)
+    residual_add_kernel<float><<<g, 256, 0, st>>>((const float*)x, (const float*)y, (float*)out, (size_t)n_elems);
+  else
+    residual_add_kernel<__nv_bfloat16><<<g, 256, 0, st>>>((const __nv_bfloat16*)x, (const __nv_bfloat16*)y,
+                                                          (__nv_bfloat16*)out, (size_t)n_elems);
+  CK(cudaGetLastError());
+  return WISP_OK;
+}
+
+int wisp_set_split(wisp_ctx* ctx, uint64_t expert_bytes, uint64_t kv_bytes) {
+  if (!ctx) return WISP_EINVAL;
+  const u64 b = ctx->cfg.kv_block_bytes;
+  const u64 Cn64 = std::min<u64>(ctx->cfg.n_experts, expert_bytes / ctx->a_bytes);
+  const u64 kap = b ? kv_bytes / b : 0;
+  const bool over = expert_bytes > ctx->budget || kv_bytes > ctx->budget - expert_bytes;
+  if (over || Cn64 < 1 || kap < ctx->cfg.kv_floor_blocks || kap < ctx->kv_reserved ||
+      Cn64 * ctx->a_bytes + kap * b > ctx->budget) {
+    ++ctx->failed_resize;   // "If a resize fails, the engine keeps the previous valid split."
+    return fail(ctx, WISP_EBUDGET, "split refused: over budget, below the KV floor/reservations, or C < 1");
+  }
+  const int Cn = (int)Cn64;
+  CK(cudaDeviceSynchronize());   // drained barrier
+  const bool changed = Cn != ctx->C || kap != ctx->kappa;
+  if (Cn != ctx->C) {
+    // Free-before-grow: the arena is fixed, so "freeing" the shrinking side is the validation
+    // above (the two regions never overlap); a shrink compacts survivors before C changes.
+    for (int l = 0; l < ctx->cfg.n_layers; ++l) {
+      ResizeArgs a;
+      a.E = ctx->cfg.n_experts; a.C_old = ctx->C; a.C_new = Cn; a.policy = ctx->cfg.policy; a.layer = l;
+      a.st = layer_state(ctx, l);
+      a.moves = ctx->moves; a.n_moves = ctx->moves + 2 * ctx->cfg.n_experts;
+      a.trace = ctx->trace; a.trace_ctr = ctx->trace_ctr; a.trace_cap = ctx->trace_cap; a.trace_on = ctx->trace_on;
+      residency_resize_kernel<<<1, kPlanThreads>>>(a);
+      if (Cn < ctx->C) {
+        dim3 g(64, Cn);   // at most Cn moves
+        move_slots_kernel<<<g, 256>>>(ctx->moves, a.n_moves, reinterpret_cast<uint4*>(ctx->arena), ctx->Me / 16,
+                                      ctx->cfg.n_layers, l);
+      }
+    }
+    CK(cudaGetLastError());
+    CK(cudaDeviceSynchronize());
+    ctx->C = Cn;
+    drop_graphs(ctx);
+  }
+  ctx->kappa = kap;
+  if (changed) ++ctx->resize_count;
+  return WISP_OK;
+}
+
+int wisp_layer_stats_read(wisp_ctx* ctx, int32_t layer, wisp_layer_stats* out) {
+  if (!ctx || !out || layer < 0 || layer >= ctx->cfg.n_layers) return fail(ctx, WISP_EINVAL, "bad argument");
+  u64 s[8];
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(s, ctx->scal + (size_t)layer * 8, sizeof(s), cudaMemcpyDeviceToHost));
+  out->steps = s[1]; out->hits = s[2]; out->misses = s[3]; out->evictions = s[4]; out->references = s[5];
+  out->bytes_fetched = s[3] * ctx->Me;
+  return WISP_OK;
+}
+
+int wisp_stats(wisp_ctx* ctx, wisp_stats_t* out) {
+  if (!ctx || !out) return fail(ctx, WISP_EINVAL, "bad argument");
+  std::memset(out, 0, sizeof(*out));
+  const int L = ctx->cfg.n_layers;
+  std::vector<u64> s((size_t)L * 8);
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(s.data(), ctx->scal, s.size() * sizeof(u64), cudaMemcpyDeviceToHost));
+  for (int l = 0; l < L; ++l) {
+    out->total.steps += s[l * 8 + 1]; out->total.hits += s[l * 8 + 2]; out->total.misses += s[l * 8 + 3];
+    out->total.evictions += s[l * 8 + 4]; out->total.references += s[l * 8 + 5];
+  }
+  out->total.bytes_fetched = out->total.misses * ctx->Me;
+  u64 tc[2];
+  CK(cudaMemcpy(tc, ctx->trace_ctr, sizeof(tc), cudaMemcpyDeviceToHost));
+  harvest_timing(ctx, true);
+  out->n_layers = L;
+  out->slots_per_layer = ctx->C;
+  out->budget_bytes = ctx->budget;
+  out->expert_bytes = (u64)ctx->C * ctx->a_bytes;
+  out->kv_bytes = ctx->kappa * ctx->cfg.kv_block_bytes;
+  out->kv_blocks = ctx->kappa;
+  out->kv_blocks_reserved = ctx->kv_reserved;
+  out->kv_blocks_peak = ctx->kv_peak;
+  out->resize_count = ctx->resize_count;
+  out->failed_resize_count = ctx->failed_resize;
+  out->trace_dropped = tc[1];
+  out->fetch_ns = (u64)(ctx->fetch_ms * 1e6);
+  ctx->kv_peak = ctx->kv_reserved;
+  return WISP_OK;
+}
+
+int wisp_trace_enable(wisp_ctx* ctx, int32_t on) {
+  if (!ctx) return WISP_EINVAL;
+  CK(cudaDeviceSynchronize());
+  ctx->trace_on = on ? 1 : 0;
+  drop_graphs(ctx);   // the flag is a kernel argument baked into captured graphs
+  return WISP_OK;
+}
+
+int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t* n_out) {
+  if (!ctx || !n_out || (cap && !buf)) return fail(ctx, WISP_EINVAL, "bad argument");
+  CK(cudaDeviceSynchronize());
+  u64 tc[2];
+  CK(cudaMemcpy(tc, ctx->trace_ctr, sizeof(tc), cudaMemcpyDeviceToHost));
+  const u64 n = std::min<u64>(cap, tc[0]);
+  if (n) CK(cudaMemcpy(buf, ctx->trace, n * sizeof(wisp_trace_event), cudaMemcpyDeviceToHost));
+  const u64 rest = tc[0] - n;
+  if (rest) {   // keep the undrained tail at the front
+    std::vector<wisp_trace_event> tmp(rest);
+    CK(cudaMemcpy(tmp.data(), ctx->trace + n, rest * sizeof(wisp_trace_event), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(ctx->trace, tmp.data(), rest * sizeof(wisp_trace_event), cudaMemcpyHostToDevice));
+  }
+  tc[0] = rest;
+  CK(cudaMemcpy(ctx->trace_ctr, tc, sizeof(u64), cudaMemcpyHostToDevice));
+  *n_out = n;
+  return WISP_OK;
+}
+
+int wisp_last_topk(wisp_ctx* ctx, int32_t layer, int32_t* ids, float* w, int32_t* n_tokens_out) {
+  if (!ctx || layer < 0 || layer >= ctx->cfg.n_layers) return fail(ctx, WISP_EINVAL, "bad argument");
+  CK(cudaDeviceSynchronize());
+  const int T_ = ctx->last_T[layer];
+  const size_t off = (size_t)layer * ctx->cfg.max_tokens * ctx->cfg.top_k, n = (size_t)T_ * ctx->cfg.top_k;
+  if (ids && n) CK(cudaMemcpy(ids, ctx->ids + off, n * sizeof(int), cudaMemcpyDeviceToHost));
+  if (w && n) CK(cudaMemcpy(w, ctx->topw + off, n * sizeof(float), cudaMemcpyDeviceToHost));
+  if (n_tokens_out) *n_tokens_out = T_;
+  return WISP_OK;
+}
+
+int wisp_last_logits(wisp_ctx* ctx, float* z, int32_t n_tokens) {
+  if (!ctx || !z || n_tokens < 0 || n_tokens > ctx->cfg.max_tokens) return fail(ctx, WISP_EINVAL, "bad argument");
+  CK(cudaDeviceSynchronize());
+  if (n_tokens) CK(cudaMemcpy(z, ctx->logits, (size_t)n_tokens * ctx->cfg.n_experts * sizeof(float), cudaMemcpyDeviceToHost));
+  return WISP_OK;
+}
+
+int wisp_debug_step_routing(wisp_ctx* ctx, int32_t layer, const int32_t* ids, int32_t n_ids) {
+  if (!ctx || layer < 0 || layer >= ctx->cfg.n_layers || n_ids < 0 || (n_ids && !ids)) return fail(ctx, WISP_EINVAL, "bad argument");
+  if (!ctx->registered[layer]) return fail(ctx, WISP_ESTATE, "layer not registered");
+  if (n_ids == 0) return WISP_OK;
+  for (int i = 0; i < n_ids; ++i)
+    if (ids[i] < 0 || ids[i] >= ctx->cfg.n_experts) return fail(ctx, WISP_EINVAL, "expert id out of range");
+  if ((size_t)n_ids > ctx->dbg_ids_cap) {
+    if (ctx->dbg_ids) cudaFree(ctx->dbg_ids);
+    ctx->dbg_ids = nullptr;
+    ctx->dbg_ids_cap = 0;
+    CK(cudaMalloc(&ctx->dbg_ids, (size_t)n_ids * sizeof(int)));
+    ctx->dbg_ids_cap = n_ids;
+  }
+  CK(cudaMemcpy(ctx->dbg_ids, ids, (size_t)n_ids * sizeof(int), cudaMemcpyHostToDevice));
+  // pair lists are not needed (no FFN): run the plan with build_pairs off by passing the ids directly
+  PlanArgs a;
+  a.ids = ctx->dbg_ids; a.n_pairs = n_ids; a.E = ctx->cfg.n_experts; a.C = ctx->C; a.policy = ctx->cfg.policy; a.layer = layer;
+  a.st = layer_state(ctx, layer); a.plan = ctx->plan; a.host_plan = ctx->host_plan;
+  a.trace = ctx->trace; a.trace_ctr = ctx->trace_ctr; a.trace_cap = ctx->trace_cap; a.trace_on = ctx->trace_on;
+  a.track = ctx->track; a.build_pairs = 0;
+  residency_plan_kernel<<<1, kPlanThreads>>>(a);
+  CK(cudaGetLastError());
+  CK(cudaDeviceSynchronize());
+  const bool memcpy_path = ctx->cfg.fetch == WISP_FETCH_MEMCPY;
+  for (int w = 0; w < ctx->host_plan->n_waves; ++w) {
+    int rc = fetch_wave(ctx, layer, w, memcpy_path, nullptr);
+    if (rc) return rc;
+    CK(cudaDeviceSynchronize());   // wave w+1 may overwrite slots of wave w: keep them serial
+  }
+  return WISP_OK;
+}
+
+int wisp_debug_residency(wisp_ctx* ctx, int32_t layer, int32_t* pi_inv, uint64_t* tau, uint64_t* freq, uint64_t* clock) {
+  if (!ctx || layer < 0 || layer >= ctx->cfg.n_layers) return fail(ctx, WISP_EINVAL, "bad argument");
+  CK(cudaDeviceSynchronize());
+  LayerState s = layer_state(ctx, layer);
+  if (pi_inv) CK(cudaMemcpy(pi_inv, s.pi_inv, (size_t)ctx->C * sizeof(int), cudaMemcpyDeviceToHost));
+  if (tau) CK(cudaMemcpy(tau, s.tau, (size_t)ctx->C * sizeof(u64), cudaMemcpyDeviceToHost));
+  if (freq) CK(cudaMemcpy(freq, s.freq, (size_t)ctx->cfg.n_experts * sizeof(u64), cudaMemcpyDeviceToHost));
+  if (clock) CK(cudaMemcpy(clock, s.scal, sizeof(u64), cudaMemcpyDeviceToHost));
+  return WISP_OK;
+}
+
+int wisp_debug_verify_pool(wisp_ctx* ctx, int32_t layer, int32_t* mismatched_slots) {
+  if (!ctx || !mismatched_slots || layer < 0 || layer >= ctx->cfg.n_layers) return fail(ctx, WISP_EINVAL, "bad argument");
+  if (!ctx->registered[layer]) return fail(ctx, WISP_ESTATE, "layer not registered");
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemset(ctx->bad_slots, 0, (size_t)ctx->cfg.n_experts * sizeof(int)));
+  dim3 g(32, ctx->C);
+  verify_pool_kernel<<<g, 256>>>(layer_state(ctx, layer).pi_inv, reinterpret_cast<const uint4*>(ctx->master[layer]),
+                                 reinterpret_cast<const uint4*>(ctx->arena), ctx->Me / 16, ctx->cfg.n_layers, layer,
+                                 ctx->bad_slots);
+  CK(cudaGetLastError());
+  std::vector<int> bad(ctx->C);
+  CK(cudaMemcpy(bad.data(), ctx->bad_slots, (size_t)ctx->C * sizeof(int), cudaMemcpyDeviceToHost));
+  int n = 0;
+  for (int v : bad) n += v != 0;
+  *mismatched_slots = n;
+  return WISP_OK;
+}
+
+int wisp_fetch_timing_enable(wisp_ctx* ctx, int32_t on) {
+  if (!ctx) return WISP_EINVAL;
+  ctx->fetch_timing = on ? 1 : 0;
+  return WISP_OK;
+}
+
+int wisp_kv_reserve(wisp_ctx* ctx, int64_t delta_blocks) {
+  if (!ctx) return WISP_EINVAL;
+  if (delta_blocks >= 0) {
+    if (ctx->kv_reserved + (u64)delta_blocks > ctx->kappa) return fail(ctx, WISP_EBUDGET, "KV pool exhausted");
+    ctx->kv_reserved += (u64)delta_blocks;
+  } else {
+    if ((u64)(-delta_blocks) > ctx->kv_reserved) return fail(ctx, WISP_EBUDGET, "releasing more KV blocks than reserved");
+    ctx->kv_reserved -= (u64)(-delta_blocks);
+  }
+  ctx->kv_peak = std::max(ctx->kv_peak, ctx->kv_reserved);
+  return WISP_OK;
+}
+
+int wisp_mvwsa_track(wisp_ctx* ctx, int32_t on) {
+  if (!ctx) return WISP_EINVAL;
+  CK(cudaDeviceSynchronize());
+  ctx->track = on ? 1 : 0;
+  drop_graphs(ctx);
+  return WISP_OK;
+}
+
+static int pull_hist(wisp_ctx* ctx) {
+  const int L = ctx->cfg.n_layers, E = ctx->cfg.n_experts;
+  std::vector<u64> h((size_t)L * (E + 2));
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(h.data(), ctx->hist, h.size() * sizeof(u64), cudaMemcpyDeviceToHost));
+  CK(cudaMemset(ctx->hist, 0, h.size() * sizeof(u64)));
+  for (int l = 0; l < L; ++l)
+    for (int i = 0; i < E + 2; ++i) ctx->host_hist[i] += (double)h[(size_t)l * (E + 2) + i];
+  return WISP_OK;
+}
+
+int wisp_mvwsa_miss_curve(wisp_ctx* ctx, double* m_exp, int32_t n, double decay) {
+  if (!ctx || !m_exp || n < 1 || !(decay > 0.0 && decay <= 1.0)) return fail(ctx, WISP_EINVAL, "bad argument");
+  int rc = pull_hist(ctx);
+  if (rc) return rc;
+  const int E = ctx->cfg.n_experts;
+  std::vector<double> m = mvwsa::miss_curve(ctx->host_hist, E);
+  for (int i = 0; i < n; ++i) m_exp[i] = m[std::min(i, E)];
+  if (decay != 1.0)
+    for (double& v : ctx->host_hist) v *= decay;
+  return WISP_OK;
+}
+
+int wisp_mvwsa_propose(wisp_ctx* ctx, const wisp_mvwsa_in* in, uint64_t* expert_bytes, uint64_t* kv_bytes, int32_t* moved) {
+  if (!ctx || !in || !expert_bytes || !kv_bytes) return fail(ctx, WISP_EINVAL, "bad argument");
+  const u64 b = ctx->cfg.kv_block_bytes;
+  if (!b) return fail(ctx, WISP_ESTATE, "no KV accounting (kv_block_bytes == 0)");
+  const int E = ctx->cfg.n_experts;
+  int64_t c_min = std::max(1, in->c_min), c_max = in->c_max;
+  std::vector<double> m;
+  if (c_max <= 0 || in->mode == 1) {
+    int rc = pull_hist(ctx);
+    if (rc) return rc;
+    m = mvwsa::miss_curve(ctx->host_hist, E);
+  }
+  if (c_max <= 0) c_max = std::max<int64_t>(c_min, mvwsa::knee(m, E));
+  c_max = std::min<int64_t>(c_max, E);
+  int64_t Cn, kap;
+  bool mv;
+  if (in->mode == 0) {
+    const double p = in->kv_peak_blocks == UINT64_MAX ? (double)ctx->kv_peak : (double)in->kv_peak_blocks;
+    mvwsa::Split s = mvwsa::live_law(ctx->budget, ctx->a_bytes, b, ctx->cfg.kv_floor_blocks, p, in->headroom, c_min,
+                                     c_max, ctx->C, std::max(1, in->dead_zone));
+    Cn = s.C; kap = s.kappa; mv = s.moved;
+  } else if (in->mode == 1) {
+    Cn = mvwsa::configurator(ctx->budget, ctx->a_bytes, b, ctx->cfg.kv_floor_blocks, in->c_exp, in->c_kv, m, in->m_kv,
+                             in->m_kv_len, c_min, c_max);
+    if (Cn < 0) return fail(ctx, WISP_EBUDGET, "no feasible split above the admission floor");
+    kap = (int64_t)((ctx->budget - (u64)Cn * ctx->a_bytes) / b);
+    mv = Cn != ctx->C;
+  } else {
+    return fail(ctx, WISP_EINVAL, "unknown mode");
+  }
+  *expert_bytes = (u64)Cn * ctx->a_bytes;
+  *kv_bytes = (u64)kap * b;
+  if (moved) *moved = mv ? 1 : 0;
+  return WISP_OK;
+}
+
+}  // extern "C"
