@@ -1,0 +1,436 @@
+#!/usr/bin/env python
+"""bench.py -- WiSP hot path on B200: decode tokens/s at a fixed expert-pool budget (BASELINE.json metric).
+
+A "step" = one decode token batch through the WHOLE hot path of every layer: router GEMV + top-k,
+slot-table residency lookup (Algorithm 1), demand fetch of misses from pinned host memory, slot-indirected
+SwiGLU FFN, weighted combine, residual chain.  Default workload = BASELINE.json configs[1]: Qwen3-30B-A3B-shaped
+stack (48 layers, 128 experts, top-8, d=2048, d_ff=768, bf16), batch 1, expert pool 8 GiB of 54 GiB, LRU.
+
+  python bench.py --gpus N --steps K --warmup W            # our arm (CUDA library through the C ABI)
+  python bench.py --impl reference --steps K --warmup W     # the CPU oracle, as it stands, on host cores
+
+Prints ONE JSON line.  Multi-GPU: replicas only: each rank
+runs an independent replica; value = tokens all ranks processed / max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+import synth_inputs as si  # noqa: E402
+
+GIB = 1 << 30
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=128)
+    ap.add_argument("--warmup", type=int, default=16)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="qwen3", choices=["qwen3", "mixtral", "tiny"])
+    ap.add_argument("--layers", type=int, default=0, help="override the layer count (0 = the config's)")
+    ap.add_argument("--budget-gib", type=float, default=0.0, help="expert-pool budget (0 = the config's)")
+    ap.add_argument("--batch", type=int, default=1)
+    ap.add_argument("--policy", default="lru", choices=["lru", "lfu"])
+    ap.add_argument("--fetch", default="zerocopy", choices=["zerocopy", "memcpy"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-miss-path", action="store_true")
+    ap.add_argument("--per-layer-api", action="store_true", help="drive wisp_moe_forward per layer instead of wisp_stack_forward")
+    return ap.parse_args()
+
+
+def workload(args):
+    shape = {"qwen3": si.QWEN3, "mixtral": si.MIXTRAL, "tiny": si.TINY}[args.workload]
+    budget = {"qwen3": 8 * GIB, "mixtral": 24 * GIB, "tiny": 6 * si.TINY.slot_unit_bytes}[args.workload]
+    if args.budget_gib > 0:
+        budget = int(args.budget_gib * GIB)
+    if args.layers > 0:
+        # keep the per-layer slot count of the full config: scale the budget with the layer count
+        budget = budget // shape.n_layers * args.layers
+        shape = shape.with_layers(args.layers)
+    return shape, budget
+
+
+def mem_available_bytes():
+    with open("/proc/meminfo") as fh:
+        for line in fh:
+            if line.startswith("MemAvailable"):
+                return int(line.split()[1]) * 1024
+    return 0
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._pump, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(kernel):
+    """dram read+write bytes per launch of `kernel` from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return json.load(fh).get(kernel)
+    return None
+
+
+# ---------------------------------------------------------------------------------------------------------
+def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=None, gen_device="cuda"):
+    import paper_2606_21868_b200 as wp
+    ctx = wp.Wisp(budget, n_layers=shape.n_layers, n_experts=shape.n_experts, top_k=shape.top_k, d_model=shape.d_model,
+                  d_ff=shape.d_ff, max_tokens=max_tokens, dtype=wp.WISP_F32 if shape.dtype == "f32" else wp.WISP_BF16,
+                  policy=wp.WISP_LFU if args.policy == "lfu" else wp.WISP_LRU,
+                  fetch=(wp.WISP_FETCH_MEMCPY if (fetch or args.fetch) == "memcpy" else wp.WISP_FETCH_ZEROCOPY))
+    staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
+    for l in (register_layers if register_layers is not None else range(shape.n_layers)):
+        si.gen_layer_experts(shape, l, gen_device, out=staging)
+        w_r, bias = si.gen_router(shape, l)
+        ctx.register_host_experts(l, staging, w_r, bias)
+    return ctx, staging
+
+
+def run_steps(ctx, shape, x_dev, y_dev, stream, per_layer_api, scratch):
+    """Enqueue one decode step per row of x_dev ([n, B, d]); outputs into y_dev."""
+    for t in range(x_dev.shape[0]):
+        if not per_layer_api:
+            ctx.stack_forward(x_dev[t], y_dev[t], stream.cuda_stream)
+        else:
+            a, b, o = scratch
+            a.copy_(x_dev[t])
+            for l in range(shape.n_layers):
+                ctx.moe_forward(l, a, o, stream.cuda_stream)
+                ctx.residual_add(a, o, b, stream.cuda_stream)
+                a, b = b, a
+            y_dev[t].copy_(a)
+
+
+def miss_path_microbench(shape, args):
+    """m2: demand fetch only.  One-layer context, C slots; every step references C experts that are not resident, so
+    each wave is C misses of M_e bytes.  GB/s per fetch path vs the box's pinned->device cudaMemcpyAsync peak."""
+    out = {}
+    n = 1 << 30
+    h = torch.empty(n, dtype=torch.uint8, pin_memory=True)
+    d = torch.empty(n, dtype=torch.uint8, device="cuda")
+    best = 0.0
+    for _ in range(10):
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s.record(); d.copy_(h, non_blocking=True); e.record(); torch.cuda.synchronize()
+        best = max(best, n / (s.elapsed_time(e) * 1e-3) / 1e9)
+    del h, d
+    out["link_peak_gbs"] = round(best, 2)
+    out["link_peak_how"] = "pinned->device cudaMemcpyAsync, 1 GiB, best of 10"
+    one = shape.with_layers(1)
+    C = min(16, shape.n_experts // 2) if shape.expert_bytes < (64 << 20) else 2
+    for path in ("zerocopy", "memcpy"):
+        ctx, staging = build_context(one, C * one.slot_unit_bytes, args, 1, fetch=path)
+        ctx.timing_enable(1)
+        E = shape.n_experts
+        groups = [[(g * C + j) % E for j in range(C)] for g in range(max(2, E // C))]
+        for g in groups[:2]:
+            ctx.debug_step_routing(0, g)            # warm-up (first touches)
+        ctx.timing_read(reset=True)
+        m0 = ctx.stats().total.misses
+        reps = 0
+        for _ in range(3):
+            for g in groups[2:] + groups[:2]:
+                ctx.debug_step_routing(0, g)
+                reps += 1
+        ms, _n = ctx.timing_read()["fetch"]
+        nbytes = (ctx.stats().total.misses - m0) * shape.expert_bytes
+        out[path + "_gbs"] = round(nbytes / (ms * 1e-3) / 1e9, 2) if ms > 0 else None
+        out[path + "_bytes"] = nbytes
+        ctx.close()
+        del staging
+    best_path = max(("zerocopy", "memcpy"), key=lambda p: out[p + "_gbs"] or 0)
+    out["kept"] = best_path
+    out["frac_of_link_peak"] = round((out[best_path + "_gbs"] or 0) / best, 4)
+    return out
+
+
+def cpu_oracle_sample(shape, layers, hidden_row, threads=None):
+    """The oracle as it stands (oracle/moe_forward.py) on `layers` layers of one decode token batch.  Returns
+    (seconds, layers_done)."""
+    from oracle import moe_forward as mf
+    x = hidden_row.to(shape.torch_dtype)
+    gen_dev = "cuda" if torch.cuda.is_available() else "cpu"
+    t_total = 0.0
+    for l in layers:
+        blob = si.gen_layer_experts(shape, l, gen_dev)
+        w_r, bias = si.gen_router(shape, l)
+        t0 = time.perf_counter()
+        out, ids, w, z = mf.moe_layer(x, blob, w_r, bias, shape.top_k, shape.d_ff)
+        y = out.to(shape.torch_dtype)
+        x = (x.float() + y.float()).to(shape.torch_dtype)
+        t_total += time.perf_counter() - t0
+        del blob
+    return t_total, len(list(layers))
+
+
+def main_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    shape, budget = workload(args)
+    hidden = si.gen_decode_hidden(shape, args.warmup + args.steps, args.batch)
+    gen_dev = "cuda" if torch.cuda.is_available() else "cpu"
+    from oracle import moe_forward as mf
+    # bounded sample: every step runs the first `nl` layers of the stack on one token batch
+    blobs, routers = [], []
+    probe_layers = 1
+    blobs.append(si.gen_layer_experts(shape, 0, gen_dev)); routers.append(si.gen_router(shape, 0))
+    x = hidden[0].to(shape.torch_dtype)
+    t0 = time.perf_counter()
+    mf.moe_layer(x, blobs[0], routers[0][0], routers[0][1], shape.top_k, shape.d_ff)
+    t_layer = time.perf_counter() - t0
+    nl = int(max(1, min(shape.n_layers, 150.0 / max(1e-6, (args.steps + args.warmup) * t_layer))))
+    nl = min(nl, 4 if shape.expert_bytes * shape.n_experts > (256 << 20) else shape.n_layers)
+    for l in range(probe_layers, nl):
+        blobs.append(si.gen_layer_experts(shape, l, gen_dev)); routers.append(si.gen_router(shape, l))
+
+    def step(t):
+        x = hidden[t].to(shape.torch_dtype)
+        for l in range(nl):
+            out, *_ = mf.moe_layer(x, blobs[l], routers[l][0], routers[l][1], shape.top_k, shape.d_ff)
+            x = (x.float() + out.to(shape.torch_dtype).float()).to(shape.torch_dtype)
+
+    for t in range(args.warmup):
+        step(t)
+    t0 = time.perf_counter()
+    for t in range(args.warmup, args.warmup + args.steps):
+        step(t)
+    dt = time.perf_counter() - t0
+    tokens = args.steps * args.batch * nl / shape.n_layers      # a token = all L layers; the sample covers nl of them
+    val = tokens / dt
+    sample = f"{nl} of {shape.n_layers} layers per step, batch {args.batch} (tokens/s scaled by {nl}/{shape.n_layers})"
+    line = {"impl": "reference", "metric": "decode_tokens_per_s", "value": val, "unit": "tokens/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{shape.name} decode batch {args.batch}, all experts resident (oracle has no pool)",
+                       "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "tokens/s", "cores": torch.get_num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main_ours(args):
+    import paper_2606_21868_b200 as wp
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    shape, budget = workload(args)
+    full_layers = shape.n_layers
+    # host-RAM guard: masters are pinned host memory (L*E*M_e per replica)
+    need = shape.n_layers * shape.n_experts * shape.expert_bytes
+    avail = mem_available_bytes() * 0.75 / max(1, world)
+    reduced = False
+    if need > avail:
+        nl = max(1, int(avail // (shape.n_experts * shape.expert_bytes)))
+        budget = budget // shape.n_layers * nl
+        shape = shape.with_layers(nl)
+        reduced = True
+    B = args.batch
+    t_setup = time.time()
+    ctx, staging = build_context(shape, budget, args, max(B, 1))
+    del staging
+    t_setup = time.time() - t_setup
+    C = ctx.stats().slots_per_layer
+    n_all = args.warmup + args.steps
+    hidden = si.gen_decode_hidden(shape, n_all, B).to(shape.torch_dtype)          # [n, B, d]
+    x_dev = hidden.cuda()
+    y_dev = torch.empty_like(x_dev)
+    stream = torch.cuda.Stream()
+    scratch = tuple(torch.empty((B, shape.d_model), dtype=shape.torch_dtype, device="cuda") for _ in range(3))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    with torch.cuda.stream(stream):
+        run_steps(ctx, shape, x_dev[:args.warmup], y_dev[:args.warmup], stream, args.per_layer_api, scratch)
+        stream.synchronize()
+        st0 = ctx.stats()
+        sampler = ClockSampler(local)
+        barrier(); torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        run_steps(ctx, shape, x_dev[args.warmup:], y_dev[args.warmup:], stream, args.per_layer_api, scratch)
+        e1.record(stream)
+        torch.cuda.synchronize(); barrier()
+        clocks = sampler.stop()
+        ms = e0.elapsed_time(e1)
+        st1 = ctx.stats()
+        if dist is not None:
+            tms = torch.tensor([ms], device="cuda")
+            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+            ms = float(tms.item())
+        value = args.steps * B * world / (ms * 1e-3)
+
+        # ---- e2e: host buffers, H2D + D2H inside the timed region, through the public call ----
+        h_in = hidden[args.warmup:].contiguous().pin_memory()
+        h_out = torch.empty_like(h_in).pin_memory()
+        xin = torch.empty((B, shape.d_model), dtype=shape.torch_dtype, device="cuda")
+        xout = torch.empty_like(xin)
+        barrier(); torch.cuda.synchronize()
+        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e2.record(stream)
+        for t in range(args.steps):
+            xin.copy_(h_in[t], non_blocking=True)
+            run_steps(ctx, shape, xin[None], xout[None], stream, args.per_layer_api, scratch)
+            h_out[t].copy_(xout, non_blocking=True)
+            stream.synchronize()                       # the caller consumes each token's result before the next step
+        e3.record(stream)
+        torch.cuda.synchronize(); barrier()
+        ms_e2e = e2.elapsed_time(e3)
+        if dist is not None:
+            tms = torch.tensor([ms_e2e], device="cuda")
+            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+            ms_e2e = float(tms.item())
+        io_bytes = B * shape.d_model * shape.elem_bytes
+        same = torch.equal(h_out.view(torch.uint8), y_dev[args.warmup:].cpu().view(torch.uint8))
+
+        # ---- per-kernel durations over the same steps (CUDA events on the launching stream; no graph) ----
+        n_prof = min(args.steps, 32)
+        ctx.timing_enable(2)
+        ctx.timing_read(reset=True)
+        run_steps(ctx, shape, x_dev[args.warmup:args.warmup + n_prof], y_dev[args.warmup:args.warmup + n_prof], stream,
+                  args.per_layer_api, scratch)
+        stream.synchronize()
+        kt = ctx.timing_read()
+        ctx.timing_enable(0)
+
+    hbm_peak, peak_how = measured_peaks()
+    refs = st1.total.references - st0.total.references
+    misses = st1.total.misses - st0.total.misses
+    # algorithmic bytes of one gate_up launch = experts of the wave x (gate + up) bytes
+    avg_R = refs / max(1, args.steps * shape.n_layers)
+    gu_bytes = avg_R * 2 * shape.d_model * shape.d_ff * shape.elem_bytes
+    dn_bytes = avg_R * shape.d_model * shape.d_ff * shape.elem_bytes
+    kern = {}
+    for name, (tot_ms, n) in kt.items():
+        if n:
+            kern[name] = {"avg_us": round(tot_ms / n * 1e3, 3), "launches": int(n)}
+    step_us = sum(v["avg_us"] * v["launches"] for v in kern.values()) / max(1, n_prof)
+    for name in kern:
+        kern[name]["share_of_kernel_time"] = round(kern[name]["avg_us"] * kern[name]["launches"] / max(1e-9, step_us * n_prof), 4)
+    roof = None
+    if "gate_up" in kern:
+        ach = gu_bytes / (kern["gate_up"]["avg_us"] * 1e-6) / 1e9
+        roof = {"bound": "hbm", "kernel": "decode_gate_up_kernel", "achieved": round(ach, 1), "peak": hbm_peak, "unit": "GB/s",
+                "frac": round(ach / hbm_peak, 4), "traffic": ncu_traffic("decode_gate_up_kernel"),
+                "bytes_per_launch": int(gu_bytes), "avg_launch_us": kern["gate_up"]["avg_us"], "peak_source": peak_how,
+                "frac_of_nominal_8TBs": round(ach / 8000.0, 4)}
+        if "down" in kern:
+            ach_d = dn_bytes / (kern["down"]["avg_us"] * 1e-6) / 1e9
+            roof["down_kernel"] = {"achieved": round(ach_d, 1), "frac": round(ach_d / hbm_peak, 4), "bytes_per_launch": int(dn_bytes),
+                                   "avg_launch_us": kern["down"]["avg_us"]}
+        ffn_us = kern["gate_up"]["avg_us"] + kern.get("down", {"avg_us": 0})["avg_us"]
+        roof["ffn_gbs"] = round((gu_bytes + dn_bytes) / (ffn_us * 1e-6) / 1e9, 1)
+
+    line = {"metric": "decode_tokens_per_s", "value": value, "unit": "tokens/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16" if shape.dtype == "bf16" else "f32", "data": "synthetic",
+            "config": {"workload": f"{shape.name} decode, batch {B}, {shape.n_layers} layers, E={shape.n_experts}, top-{shape.top_k}, "
+                                   f"d={shape.d_model}, d_ff={shape.d_ff}, expert pool {budget / GIB:.3f} GiB -> C={C} slots/layer, "
+                                   f"{args.policy.upper()}, fetch={args.fetch}",
+                       "api": "wisp_moe_forward per layer" if args.per_layer_api else "wisp_stack_forward (CUDA graph per token)",
+                       "l2": f"weights streamed per step {avg_R * shape.n_layers * shape.expert_bytes / GIB:.2f} GiB >> 126 MB L2 (no flush needed)",
+                       "layers_reduced_for_host_ram": reduced, "full_config_layers": full_layers, "parallelism": "replicas" if world > 1 else "single"},
+            "clocks": clocks,
+            "e2e": {"value": args.steps * B * world / (ms_e2e * 1e-3), "unit": "tokens/s", "h2d_bytes_per_step": io_bytes,
+                    "d2h_bytes_per_step": io_bytes, "outputs_equal_device_run": bool(same)},
+            "gpu_launches": int(st1.kernel_launches - st0.kernel_launches),
+            "roofline": roof,
+            "paging": {"hit_rate": round(1 - misses / max(1, refs), 5), "misses": int(misses), "references": int(refs),
+                       "miss_bytes_per_step": misses * shape.expert_bytes / args.steps,
+                       "hbm_bound_tokens_per_s": round(hbm_peak * 1e9 / max(1.0, avg_R * shape.n_layers * shape.expert_bytes), 1)},
+            "kernels": kern, "setup_s": round(t_setup, 1)}
+    if rank == 0 and world == 1 and not args.no_miss_path:
+        try:
+            line["miss_path"] = miss_path_microbench(shape, args)
+        except Exception as ex:                        # the microbenchmark must never take the headline down
+            line["miss_path"] = {"error": repr(ex)[:200]}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nl = min(shape.n_layers, 4 if shape.expert_bytes * shape.n_experts > (256 << 20) else shape.n_layers)
+        reps = 2 if nl < shape.n_layers else 8
+        tot, done = 0.0, 0
+        for r in range(reps):
+            t, n = cpu_oracle_sample(shape, range(nl), hidden[args.warmup + r].float())
+            tot += t; done += n
+        line["cpu_baseline"] = {"value": (done / shape.n_layers) * B / tot, "unit": "tokens/s", "cores": torch.get_num_threads(),
+                                "kind": "oracle", "sample": f"{reps} decode tokens x first {nl} of {shape.n_layers} layers, "
+                                f"tokens/s scaled by layers done / {shape.n_layers} ({tot:.1f} s of CPU work)"}
+    ctx.close()
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        main_reference(a)
+    else:
+        main_ours(a)

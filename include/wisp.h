@@ -90,8 +90,13 @@ typedef struct {
   uint64_t resize_count;         /* successful wisp_set_split calls that changed C or kappa */
   uint64_t failed_resize_count;  /* refused wisp_set_split calls (state kept) */
   uint64_t trace_dropped;        /* events lost because the ring was full */
-  uint64_t fetch_ns;             /* event-timed busy time of the miss path (only while fetch timing is on) */
+  uint64_t fetch_ns;             /* event-timed busy time of the miss path (only while wisp_timing_enable >= 1) */
+  uint64_t kernel_launches;      /* library kernels launched so far (graph replays count their kernel nodes) */
 } wisp_stats_t;
+
+/* Kernel classes of wisp_timing_read. */
+enum { WISP_K_ROUTER = 0, WISP_K_TOPK = 1, WISP_K_RESIDENCY = 2, WISP_K_FETCH = 3, WISP_K_GATE_UP = 4, WISP_K_DOWN = 5,
+       WISP_K_COMBINE = 6, WISP_K_PREFILL_GATE_UP = 7, WISP_K_PREFILL_DOWN = 8, WISP_K_OTHER = 9, WISP_N_KERNEL_CLASSES = 10 };
 
 /* kind: 0 hit, 1 miss, 2 resize-drop, 3 resize-move (for a move `evicted` carries the source slot).
  * Events of one wave are emitted in ascending expert id; waves in order; layers/steps in call order. */
@@ -195,8 +200,13 @@ int wisp_debug_residency(wisp_ctx* ctx, int32_t layer, int32_t* pi_inv, uint64_t
 /* Exactness invariant check: compares every occupied slot of `layer` byte for byte with
  * the host master of the expert it claims to hold; *mismatched_slots = number of slots that differ. */
 int wisp_debug_verify_pool(wisp_ctx* ctx, int32_t layer, int32_t* mismatched_slots);
-/* Time the miss path with CUDA events (adds a little host work per forward); totals in wisp_stats.fetch_ns. */
-int wisp_fetch_timing_enable(wisp_ctx* ctx, int32_t on);
+/* CUDA-event timing of the library's own launches, on the stream each is launched on.  level 0 = off,
+ * 1 = the miss path only (WISP_K_FETCH; also summed into wisp_stats.fetch_ns), 2 = every kernel class.  While
+ * level > 0 wisp_stack_forward does not replay CUDA graphs.  wisp_timing_read: host ms[WISP_N_KERNEL_CLASSES]
+ * (summed event-to-event milliseconds) and launches[WISP_N_KERNEL_CLASSES] (timed spans); reset != 0 zeroes
+ * the totals after the read.  Synchronises. */
+int wisp_timing_enable(wisp_ctx* ctx, int32_t level);
+int wisp_timing_read(wisp_ctx* ctx, double* ms, uint64_t* launches, int32_t reset);
 
 /* ---- KV reservations and MV-WSA (CPU side) ----------------------------- */
 

@@ -7,5 +7,5 @@ fails with WISP_ECUDA without a CUDA device.
 """
 from .binding import (  # noqa: F401
     WISP_BF16, WISP_F32, WISP_FETCH_MEMCPY, WISP_FETCH_ZEROCOPY, WISP_LFU, WISP_LRU, WispConfig, WispError,
-    WispLayerStats, WispMvwsaIn, WispStats, WispTraceEvent, Wisp, lib, lib_path, STATUS_NAMES,
+    WispLayerStats, WispMvwsaIn, WispStats, WispTraceEvent, Wisp, lib, lib_path, STATUS_NAMES, KERNEL_CLASSES,
 )

@@ -11,6 +11,9 @@ _LIB = None
 WISP_F32, WISP_BF16 = 0, 1
 WISP_LRU, WISP_LFU = 0, 1
 WISP_FETCH_MEMCPY, WISP_FETCH_ZEROCOPY = 0, 1
+KERNEL_CLASSES = ("router", "topk", "residency", "fetch", "gate_up", "down", "combine", "prefill_gate_up",
+                  "prefill_down", "other")
+N_KERNEL_CLASSES = len(KERNEL_CLASSES)
 STATUS_NAMES = {0: "WISP_OK", -1: "WISP_EINVAL", -2: "WISP_ENOMEM", -3: "WISP_ECUDA", -4: "WISP_ESTATE", -5: "WISP_EBUDGET"}
 
 
@@ -28,7 +31,8 @@ class WispLayerStats(C.Structure):
 class WispStats(C.Structure):
     _fields_ = [("total", WispLayerStats), ("n_layers", C.c_int32), ("slots_per_layer", C.c_int32)] + [
         (n, C.c_uint64) for n in ("budget_bytes", "expert_bytes", "kv_bytes", "kv_blocks", "kv_blocks_reserved",
-                                  "kv_blocks_peak", "resize_count", "failed_resize_count", "trace_dropped", "fetch_ns")]
+                                  "kv_blocks_peak", "resize_count", "failed_resize_count", "trace_dropped", "fetch_ns",
+                                  "kernel_launches")]
 
 
 class WispTraceEvent(C.Structure):
@@ -69,7 +73,8 @@ _SIGS = {
     "wisp_debug_step_routing": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_int32]),
     "wisp_debug_residency": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "wisp_debug_verify_pool": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_int32)]),
-    "wisp_fetch_timing_enable": (C.c_int, [C.c_void_p, C.c_int32]),
+    "wisp_timing_enable": (C.c_int, [C.c_void_p, C.c_int32]),
+    "wisp_timing_read": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_uint64), C.c_int32]),
     "wisp_kv_reserve": (C.c_int, [C.c_void_p, C.c_int64]),
     "wisp_mvwsa_propose": (C.c_int, [C.c_void_p, C.POINTER(WispMvwsaIn), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
                                      C.POINTER(C.c_int32)]),
@@ -203,8 +208,14 @@ class Wisp:
         self._ck(self.L.wisp_debug_verify_pool(self.ctx, layer, C.byref(n)), "wisp_debug_verify_pool")
         return n.value
 
-    def fetch_timing_enable(self, on=True):
-        self._ck(self.L.wisp_fetch_timing_enable(self.ctx, int(on)), "wisp_fetch_timing_enable")
+    def timing_enable(self, level=2):
+        self._ck(self.L.wisp_timing_enable(self.ctx, int(level)), "wisp_timing_enable")
+
+    def timing_read(self, reset=True):
+        ms = (C.c_double * N_KERNEL_CLASSES)()
+        n = (C.c_uint64 * N_KERNEL_CLASSES)()
+        self._ck(self.L.wisp_timing_read(self.ctx, ms, n, int(reset)), "wisp_timing_read")
+        return {name: (ms[i], n[i]) for i, name in enumerate(KERNEL_CLASSES)}
 
     def kv_reserve(self, delta_blocks):
         self._ck(self.L.wisp_kv_reserve(self.ctx, delta_blocks), "wisp_kv_reserve")

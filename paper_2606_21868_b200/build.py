@@ -15,7 +15,7 @@ SOURCES = ["wisp.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-shared", "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr",
-    "-cudart", "static",
+    "-cudart", "static", "-Xcompiler", "-pthread",
 ]
 
 

@@ -6,6 +6,7 @@
 #include <cstring>
 #include <map>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "common.cuh"
@@ -65,10 +66,14 @@ struct wisp_ctx {
 
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t ev_plan = nullptr, ev_compute = nullptr, ev_copy = nullptr;
-  int fetch_timing = 0;
-  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> timing_pool;
+  int timing_level = 0;            // 0 off, 1 miss path only, 2 every kernel class
+  struct TimedSpan { cudaEvent_t a, b; int cls; };
+  std::vector<TimedSpan> timing_pool;
   size_t timing_used = 0;
-  double fetch_ms = 0.0;
+  double class_ms[WISP_N_KERNEL_CLASSES] = {};
+  u64 class_n[WISP_N_KERNEL_CLASSES] = {};
+  u64 launches = 0;
+  std::map<int, u64> graph_nodes;
 
   std::map<int, cudaGraphExec_t> graphs;
   int grid_gate_up = 0, grid_down = 0, grid_fetch = 0;
@@ -114,31 +119,40 @@ void harvest_timing(wisp_ctx* c, bool all) {
   size_t keep = 0;
   for (size_t i = 0; i < c->timing_used; ++i) {
     auto& p = c->timing_pool[i];
-    if (all) cudaEventSynchronize(p.second);
+    if (all) cudaEventSynchronize(p.b);
     float ms = 0.f;
-    if (cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) c->fetch_ms += ms;
+    if (cudaEventElapsedTime(&ms, p.a, p.b) == cudaSuccess) { c->class_ms[p.cls] += ms; c->class_n[p.cls] += 1; }
     else std::swap(c->timing_pool[keep++], p);
   }
   c->timing_used = keep;
 }
 
-bool timing_pair(wisp_ctx* c, cudaEvent_t* a, cudaEvent_t* b) {
-  if (c->timing_used == c->timing_pool.size()) {
-    harvest_timing(c, false);
+// RAII span around one launch: counts it, and when timing is on brackets it with CUDA events on `st`.
+struct Span {
+  wisp_ctx* c;
+  cudaStream_t st;
+  cudaEvent_t b = nullptr;
+  Span(wisp_ctx* c_, int cls, cudaStream_t st_, bool is_kernel = true) : c(c_), st(st_) {
+    if (is_kernel) ++c->launches;
+    if (c->timing_level == 0 || (c->timing_level == 1 && cls != WISP_K_FETCH)) return;
     if (c->timing_used == c->timing_pool.size()) {
-      if (c->timing_pool.size() >= 4096) harvest_timing(c, true);
-      else {
-        cudaEvent_t x, y;
-        if (cudaEventCreate(&x) != cudaSuccess || cudaEventCreate(&y) != cudaSuccess) return false;
-        c->timing_pool.push_back({x, y});
+      harvest_timing(c, false);
+      if (c->timing_used == c->timing_pool.size()) {
+        if (c->timing_pool.size() >= 8192) harvest_timing(c, true);
+        else {
+          cudaEvent_t x, y;
+          if (cudaEventCreate(&x) != cudaSuccess || cudaEventCreate(&y) != cudaSuccess) return;
+          c->timing_pool.push_back({x, y, 0});
+        }
       }
     }
+    auto& p = c->timing_pool[c->timing_used++];
+    p.cls = cls;
+    cudaEventRecord(p.a, st);
+    b = p.b;
   }
-  *a = c->timing_pool[c->timing_used].first;
-  *b = c->timing_pool[c->timing_used].second;
-  ++c->timing_used;
-  return true;
-}
+  ~Span() { if (b) cudaEventRecord(b, st); }
+};
 
 template <typename T>
 int launch_router(wisp_ctx* ctx, int layer, const void* x, int T_, cudaStream_t st) {
@@ -146,11 +160,17 @@ int launch_router(wisp_ctx* ctx, int layer, const void* x, int T_, cudaStream_t 
   const int E = cfg.n_experts, d = cfg.d_model, k = cfg.top_k;
   const T* wr = reinterpret_cast<const T*>(ctx->router_w) + (size_t)layer * E * d;
   dim3 g((E + 7) / 8, (T_ + kRouterTokTile - 1) / kRouterTokTile);
-  router_logits_kernel<T><<<g, 256, 0, st>>>(reinterpret_cast<const T*>(x), wr, ctx->router_bias + (size_t)layer * E,
-                                             ctx->logits, T_, E, d);
+  {
+    Span sp(ctx, WISP_K_ROUTER, st);
+    router_logits_kernel<T><<<g, 256, 0, st>>>(reinterpret_cast<const T*>(x), wr, ctx->router_bias + (size_t)layer * E,
+                                               ctx->logits, T_, E, d);
+  }
   const size_t off = (size_t)layer * cfg.max_tokens * k;
-  topk_softmax_kernel<<<(T_ + 3) / 4, 128, 4 * E * sizeof(float), st>>>(ctx->logits, ctx->ids + off, ctx->topw + off, T_,
-                                                                        E, k);
+  {
+    Span sp(ctx, WISP_K_TOPK, st);
+    topk_softmax_kernel<<<(T_ + 3) / 4, 128, 4 * E * sizeof(float), st>>>(ctx->logits, ctx->ids + off, ctx->topw + off,
+                                                                          T_, E, k);
+  }
   CK(cudaGetLastError());
   return WISP_OK;
 }
@@ -172,8 +192,14 @@ int launch_plan(wisp_ctx* ctx, int layer, const int* ids, int n_pairs, bool want
   a.trace_on = ctx->trace_on;
   a.track = ctx->track;
   a.build_pairs = n_pairs <= 256;
-  residency_plan_kernel<<<1, kPlanThreads, 0, st>>>(a);
-  if (!a.build_pairs) group_pairs_kernel<<<a.E, 256, 0, st>>>(ids, n_pairs, ctx->plan);
+  {
+    Span sp(ctx, WISP_K_RESIDENCY, st);
+    residency_plan_kernel<<<1, kPlanThreads, 0, st>>>(a);
+  }
+  if (!a.build_pairs) {
+    Span sp(ctx, WISP_K_RESIDENCY, st);
+    group_pairs_kernel<<<a.E, 256, 0, st>>>(ids, n_pairs, ctx->plan);
+  }
   CK(cudaGetLastError());
   return WISP_OK;
 }
@@ -183,14 +209,14 @@ int launch_plan(wisp_ctx* ctx, int layer, const int* ids, int n_pairs, bool want
 int fetch_wave(wisp_ctx* ctx, int layer, int wave, bool host_known, cudaStream_t st) {
   const auto& cfg = ctx->cfg;
   const size_t blob_vec = ctx->Me / 16;
-  cudaEvent_t t0 = nullptr, t1 = nullptr;
   if (!host_known) {
-    if (ctx->fetch_timing && timing_pair(ctx, &t0, &t1)) CK(cudaEventRecord(t0, st));
-    fetch_zerocopy_kernel<<<ctx->grid_fetch, kFetchThreads, 0, st>>>(
-        ctx->plan, wave, ctx->C, reinterpret_cast<const uint4*>(ctx->master[layer]),
-        reinterpret_cast<uint4*>(ctx->arena), blob_vec, cfg.n_layers, layer);
+    {
+      Span sp(ctx, WISP_K_FETCH, st);
+      fetch_zerocopy_kernel<<<ctx->grid_fetch, kFetchThreads, 0, st>>>(
+          ctx->plan, wave, ctx->C, reinterpret_cast<const uint4*>(ctx->master[layer]),
+          reinterpret_cast<uint4*>(ctx->arena), blob_vec, cfg.n_layers, layer);
+    }
     CK(cudaGetLastError());
-    if (t1) CK(cudaEventRecord(t1, st));
     return WISP_OK;
   }
   const HostPlan* hp = ctx->host_plan;
@@ -200,14 +226,15 @@ int fetch_wave(wisp_ctx* ctx, int layer, int wave, bool host_known, cudaStream_t
   if (!any) return WISP_OK;
   CK(cudaEventRecord(ctx->ev_compute, st));
   CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_compute, 0));
-  if (ctx->fetch_timing && timing_pair(ctx, &t0, &t1)) CK(cudaEventRecord(t0, ctx->copy_stream));
-  for (int i = lo; i < hi; ++i) {
-    if (!hp->entry_miss[i]) continue;
-    const char* src = static_cast<const char*>(ctx->master[layer]) + (size_t)hp->entry_expert[i] * ctx->Me;
-    char* dst = ctx->arena + ((size_t)hp->entry_slot[i] * cfg.n_layers + layer) * ctx->Me;
-    CK(cudaMemcpyAsync(dst, src, ctx->Me, cudaMemcpyHostToDevice, ctx->copy_stream));
+  {
+    Span sp(ctx, WISP_K_FETCH, ctx->copy_stream, /*is_kernel=*/false);
+    for (int i = lo; i < hi; ++i) {
+      if (!hp->entry_miss[i]) continue;
+      const char* src = static_cast<const char*>(ctx->master[layer]) + (size_t)hp->entry_expert[i] * ctx->Me;
+      char* dst = ctx->arena + ((size_t)hp->entry_slot[i] * cfg.n_layers + layer) * ctx->Me;
+      CK(cudaMemcpyAsync(dst, src, ctx->Me, cudaMemcpyHostToDevice, ctx->copy_stream));
+    }
   }
-  if (t1) CK(cudaEventRecord(t1, ctx->copy_stream));
   CK(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
   CK(cudaStreamWaitEvent(st, ctx->ev_copy, 0));
   return WISP_OK;
@@ -219,20 +246,32 @@ int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, c
   const int d = cfg.d_model, dff = cfg.d_ff, k = cfg.top_k, L = cfg.n_layers;
   const T* pool = reinterpret_cast<const T*>(ctx->arena);
   if (T_ <= kDecodeMaxTokens) {
-    decode_gate_up_kernel<T><<<ctx->grid_gate_up, kFfnThreads, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L,
-                                                                        layer, reinterpret_cast<const T*>(x),
-                                                                        ctx->act_f32, d, dff, k);
-    decode_down_kernel<T><<<ctx->grid_down, kFfnThreads, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
-                                                                  ctx->act_f32, ctx->ystage, d, dff);
+    {
+      Span sp(ctx, WISP_K_GATE_UP, st);
+      decode_gate_up_kernel<T><<<ctx->grid_gate_up, kFfnThreads, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L,
+                                                                          layer, reinterpret_cast<const T*>(x),
+                                                                          ctx->act_f32, d, dff, k);
+    }
+    {
+      Span sp(ctx, WISP_K_DOWN, st);
+      decode_down_kernel<T><<<ctx->grid_down, kFfnThreads, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L,
+                                                                    layer, ctx->act_f32, ctx->ystage, d, dff);
+    }
   } else {
     const int ptiles = (T_ + kPfTile - 1) / kPfTile;   // an expert can receive at most T pairs
     dim3 g0(dff / kPfTile, ptiles, ctx->C), g1(d / kPfTile, ptiles, ctx->C);
-    prefill_ffn_kernel<T, 0><<<g0, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
-                                                 reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
-                                                 ctx->ystage, d, dff, k);
-    prefill_ffn_kernel<T, 1><<<g1, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
-                                                 reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
-                                                 ctx->ystage, d, dff, k);
+    {
+      Span sp(ctx, WISP_K_PREFILL_GATE_UP, st);
+      prefill_ffn_kernel<T, 0><<<g0, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
+                                                   reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
+                                                   ctx->ystage, d, dff, k);
+    }
+    {
+      Span sp(ctx, WISP_K_PREFILL_DOWN, st);
+      prefill_ffn_kernel<T, 1><<<g1, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
+                                                   reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
+                                                   ctx->ystage, d, dff, k);
+    }
   }
   CK(cudaGetLastError());
   return WISP_OK;
@@ -266,9 +305,12 @@ int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, vo
     if (rc) return rc;
   }
   const size_t n = (size_t)T_ * cfg.d_model;
-  combine_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(ctx->ystage, ctx->topw + off, reinterpret_cast<T*>(out),
-                                                                 x_next ? reinterpret_cast<const T*>(x) : nullptr,
-                                                                 reinterpret_cast<T*>(x_next), T_, cfg.d_model, k);
+  {
+    Span sp(ctx, WISP_K_COMBINE, st);
+    combine_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(ctx->ystage, ctx->topw + off, reinterpret_cast<T*>(out),
+                                                                   x_next ? reinterpret_cast<const T*>(x) : nullptr,
+                                                                   reinterpret_cast<T*>(x_next), T_, cfg.d_model, k);
+  }
   CK(cudaGetLastError());
   ctx->last_T[layer] = T_;
   ctx->last_layer = layer;
@@ -435,8 +477,8 @@ int wisp_destroy(wisp_ctx* ctx) {
   for (cudaEvent_t e : {ctx->ev_plan, ctx->ev_compute, ctx->ev_copy})
     if (e) cudaEventDestroy(e);
   for (auto& p : ctx->timing_pool) {
-    cudaEventDestroy(p.first);
-    cudaEventDestroy(p.second);
+    cudaEventDestroy(p.a);
+    cudaEventDestroy(p.b);
   }
   delete ctx;
   return WISP_OK;
@@ -450,7 +492,16 @@ int wisp_register_host_experts(wisp_ctx* ctx, int32_t layer, const void* experts
   const size_t E = ctx->cfg.n_experts, d = ctx->cfg.d_model;
   void* m = nullptr;
   CK(cudaHostAlloc(&m, E * ctx->Me, cudaHostAllocMapped | cudaHostAllocPortable));
-  std::memcpy(m, experts, E * ctx->Me);
+  {  // parallel host copy: 1 GiB-class blobs per layer, one memcpy thread is far below DRAM bandwidth
+    const size_t total = E * ctx->Me, nthr = 8, part = (total / nthr + 4095) & ~(size_t)4095;
+    std::vector<std::thread> th;
+    for (size_t i = 0; i < nthr; ++i) {
+      const size_t lo = i * part, hi = std::min(total, lo + part);
+      if (lo >= hi) break;
+      th.emplace_back([=] { std::memcpy(static_cast<char*>(m) + lo, static_cast<const char*>(experts) + lo, hi - lo); });
+    }
+    for (auto& t : th) t.join();
+  }
   ctx->master[layer] = m;
   CK(cudaMemcpy(ctx->router_w + (size_t)layer * E * d * ctx->elem, router_w, E * d * ctx->elem, cudaMemcpyHostToDevice));
   if (router_bias) CK(cudaMemcpy(ctx->router_bias + (size_t)layer * E, router_bias, E * sizeof(float), cudaMemcpyHostToDevice));
@@ -481,12 +532,15 @@ int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void
     }
     return WISP_OK;
   };
-  if (ctx->cfg.fetch == WISP_FETCH_ZEROCOPY && !ctx->fetch_timing && st != nullptr) {
+  if (ctx->cfg.fetch == WISP_FETCH_ZEROCOPY && ctx->timing_level == 0 && st != nullptr) {
     auto it = ctx->graphs.find(n_tokens);
     if (it == ctx->graphs.end()) {
       cudaGraph_t g = nullptr;
+      const u64 l0 = ctx->launches;
       CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
       rc = chain(st);
+      ctx->graph_nodes[n_tokens] = ctx->launches - l0;
+      ctx->launches = l0;
       cudaError_t e = cudaStreamEndCapture(st, &g);
       if (rc) { if (g) cudaGraphDestroy(g); return rc; }
       if (e != cudaSuccess) return fail(ctx, WISP_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
@@ -497,6 +551,7 @@ int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void
       it = ctx->graphs.emplace(n_tokens, ge).first;
     }
     CK(cudaGraphLaunch(it->second, st));
+    ctx->launches += ctx->graph_nodes[n_tokens];
     for (int l = 0; l < L; ++l) ctx->last_T[l] = n_tokens;
     ctx->last_layer = L - 1;
   } else {
@@ -512,6 +567,7 @@ int wisp_residual_add(wisp_ctx* ctx, const void* x, const void* y, void* out, in
   if (n_elems == 0) return WISP_OK;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const unsigned g = (unsigned)((n_elems + 255) / 256);
+  Span sp(ctx, WISP_K_OTHER, st);
   if (ctx->cfg.dtype == WISP_F32)
     residual_add_kernel<float><<<g, 256, 0, st>>>((const float*)x, (const float*)y, (float*)out, (size_t)n_elems);
   else
@@ -597,7 +653,8 @@ int wisp_stats(wisp_ctx* ctx, wisp_stats_t* out) {
   out->resize_count = ctx->resize_count;
   out->failed_resize_count = ctx->failed_resize;
   out->trace_dropped = tc[1];
-  out->fetch_ns = (u64)(ctx->fetch_ms * 1e6);
+  out->fetch_ns = (u64)(ctx->class_ms[WISP_K_FETCH] * 1e6);
+  out->kernel_launches = ctx->launches;
   ctx->kv_peak = ctx->kv_reserved;
   return WISP_OK;
 }
@@ -708,9 +765,19 @@ int wisp_debug_verify_pool(wisp_ctx* ctx, int32_t layer, int32_t* mismatched_slo
   return WISP_OK;
 }
 
-int wisp_fetch_timing_enable(wisp_ctx* ctx, int32_t on) {
-  if (!ctx) return WISP_EINVAL;
-  ctx->fetch_timing = on ? 1 : 0;
+int wisp_timing_enable(wisp_ctx* ctx, int32_t level) {
+  if (!ctx || level < 0 || level > 2) return fail(ctx, WISP_EINVAL, "bad argument");
+  ctx->timing_level = level;
+  return WISP_OK;
+}
+
+int wisp_timing_read(wisp_ctx* ctx, double* ms, uint64_t* launches, int32_t reset) {
+  if (!ctx || !ms || !launches) return fail(ctx, WISP_EINVAL, "bad argument");
+  CK(cudaDeviceSynchronize());
+  harvest_timing(ctx, true);
+  for (int i = 0; i < WISP_N_KERNEL_CLASSES; ++i) { ms[i] = ctx->class_ms[i]; launches[i] = ctx->class_n[i]; }
+  if (reset)
+    for (int i = 0; i < WISP_N_KERNEL_CLASSES; ++i) { ctx->class_ms[i] = 0.0; ctx->class_n[i] = 0; }
   return WISP_OK;
 }
 

@@ -144,19 +144,33 @@ def slots_for_budget(shape: MoEShape, expert_bytes: int) -> int:
     return max(0, min(shape.n_experts, expert_bytes // shape.slot_unit_bytes))
 
 
+def normal_multi(keys: list[int], n: int, device="cpu") -> torch.Tensor:
+    """[len(keys), n] standard normals: row r is exactly normal(keys[r], n) (same counter streams)."""
+    ctr = torch.arange(0, n, dtype=torch.int64, device=device) * _s64(_GOLD)
+    kt = torch.tensor([_s64(k) for k in keys], dtype=torch.int64, device=device)
+    h = _mix64(ctr[None, :] + kt[:, None])
+    hi = _lsr(h, 32).to(torch.float32)
+    lo = (h & 0xFFFFFFFF).to(torch.float32)
+    del h
+    u1 = ((hi + 0.5) * (1.0 / 4294967296.0)).clamp_(min=1e-10, max=1.0 - 2.0 ** -24)
+    u2 = (lo + 0.5) * (1.0 / 4294967296.0)
+    return torch.sqrt(-2.0 * torch.log(u1)) * torch.cos((2.0 * math.pi) * u2)
+
+
 def gen_layer_experts(shape: MoEShape, layer: int, device="cpu", out: torch.Tensor | None = None,
-                      chunk_experts: int = 16) -> torch.Tensor:
+                      chunk_experts: int | None = None) -> torch.Tensor:
     """Expert blobs of one layer, canonical layout [E, gate(d_ff x d) | up(d_ff x d) | down(d x d_ff)],
     row-major out x in, in the model dtype.  `out` may be a preallocated (pinned) host tensor."""
     E, n = shape.n_experts, shape.expert_elems
     if out is None:
         out = torch.empty((E, n), dtype=shape.torch_dtype)
+    if chunk_experts is None:
+        chunk_experts = max(1, min(E, (1 << 27) // n)) if str(device) != "cpu" else 1
     for e0 in range(0, E, chunk_experts):
         e1 = min(E, e0 + chunk_experts)
-        for e in range(e0, e1):
-            key = stream_key(shape.seed, KIND_EXPERTS, layer, e)
-            v = normal(key, n, device).mul_(0.02).to(shape.torch_dtype)
-            out[e].copy_(v)
+        keys = [stream_key(shape.seed, KIND_EXPERTS, layer, e) for e in range(e0, e1)]
+        v = normal_multi(keys, n, device).mul_(0.02).to(shape.torch_dtype)
+        out[e0:e1].copy_(v)
     return out
 
 
