@@ -50,8 +50,11 @@ typedef enum { WISP_F32 = 0, WISP_BF16 = 1 } wisp_dtype;
 typedef enum { WISP_LRU = 0, WISP_LFU = 1 } wisp_policy;
 /* Miss path (a3): MEMCPY = cudaMemcpyAsync per miss on a dedicated copy stream fenced with events (the
  * host reads the miss list: one host sync per layer call); ZEROCOPY = a device-initiated copy kernel that
- * reads the mapped pinned master (no host round trip; the whole call is stream-ordered). */
-typedef enum { WISP_FETCH_MEMCPY = 0, WISP_FETCH_ZEROCOPY = 1 } wisp_fetch;
+ * reads the mapped pinned master (no host round trip; the whole call is stream-ordered); FUSED = no separate
+ * copy step in decode: the FFN kernels' TMA producer reads a missing expert's tiles straight from the mapped
+ * pinned master, computes on them and writes them into the victim slot (same bytes, same summation order as
+ * a hit, so outputs stay byte-identical).  Prefill calls (n_tokens > 8) under FUSED use the ZEROCOPY kernel. */
+typedef enum { WISP_FETCH_MEMCPY = 0, WISP_FETCH_ZEROCOPY = 1, WISP_FETCH_FUSED = 2 } wisp_fetch;
 
 typedef struct {
   int32_t n_layers;   /* L */
@@ -63,7 +66,7 @@ typedef struct {
   int32_t dtype;      /* wisp_dtype: dtype of weights, hidden and out */
   int32_t policy;     /* wisp_policy */
   int32_t fetch;      /* wisp_fetch */
-  int32_t reserved0;
+  int32_t ring_stages; /* shared-memory ring depth of the decode FFN kernels, 2..8; 0 = library default */
   uint64_t kv_block_bytes;  /* b: bytes per KV block summed over layers; 0 = no KV accounting */
   uint64_t kv_floor_blocks; /* kappa_min of Eq. 4; wisp_set_split refuses to go below it */
   uint64_t trace_capacity;  /* trace ring capacity in events; 0 = library default (1<<20) */

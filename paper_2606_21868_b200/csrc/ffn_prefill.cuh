@@ -5,7 +5,7 @@
 //   ystage[pair, j] = <D[j], act[pair]>                   fp32
 #pragma once
 #include "common.cuh"
-#include "ffn_decode.cuh"
+#include "ffn_stream.cuh"
 
 namespace wisp {
 

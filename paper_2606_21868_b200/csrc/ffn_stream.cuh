@@ -1,0 +1,378 @@
+// ffn_stream.cuh -- (a4) decode expert SwiGLU FFN over slot-indirected weights as HBM-streaming GEMV
+// kernels for sm_100a (1 flop/byte: plain ALUs, no tensor cores), with the fused variant of the miss
+// path (a3).  The FFN itself is the engine's in the paper ("unmodified fused-MoE kernel",
+// PAPER.md:108-110); BASELINE.json fixes SwiGLU (G8, G21):
+//   MODE 0 (gate_up): g = W_gate[s] x_t, u = W_up[s] x_t, act = silu(g) * u     (act kept in fp32)
+//   MODE 1 (down)   : y = W_down[s] act                                        (y staged in fp32)
+// One persistent CTA per SM.  A producer warp streams the wave's weight tiles through a shared-memory
+// ring with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx); 8 consumer warps hold a
+// thread-stationary K-slice of the operand (x or act) in registers, FMA against the tile and reduce.
+//
+// Work decomposition:
+//   segment  = seg_chunks 16-byte chunks of one weight row (seg_chunks = P <= 256 threads, one chunk each)
+//   stage    = RB rows x n_mats matrices x one segment  (<= 32 KiB)      -> one ring slot
+//   unit     = (wave entry, row block of RB rows), all NSEG segments      -> one reduction + epilogue
+//   CTA c takes the contiguous unit range [c*U/grid, (c+1)*U/grid).
+// Canonical summation order of every (row, pair) dot product (parity (b)): thread p
+// accumulates elements of chunk p of segment 0, 1, ... in ascending order with fmaf into one fp32
+// accumulator; the P/32 warps' lanes are combined by an xor butterfly (16, 8, 4, 2, 1); the warp sums are
+// added in ascending warp order.  Nothing in it depends on the slot, the wave, the CTA, the number of
+// tokens in the call or whether the tile came from HBM or from the host master.
+//
+// Fused miss path (WISP_FETCH_FUSED): for an entry that the residency step marked as a miss, the producer
+// reads the tile from the mapped pinned host master (Alg. 1 line 6) instead of the slot,
+// and consumer warp 0 writes the landed tile from shared memory into the victim slot with a bulk store.
+// The FFN consumes the same bytes in the same order as on a hit, so outputs are byte-identical.
+#pragma once
+#include "common.cuh"
+
+namespace wisp {
+
+constexpr int kStreamConsumers = 256;                       // 8 consumer warps
+constexpr int kStreamThreads = kStreamConsumers + 32;       // + 1 producer warp
+constexpr int kStreamMaxStages = 8;
+constexpr int kStreamVals = 8;                              // weight rows per thread per stage (4 gate + 4 up | 8 down)
+
+__device__ __forceinline__ float silu_f(float v) { return v / (1.0f + expf(-v)); }
+
+// ---- PTX wrappers: mbarrier, TMA bulk copies, programmatic dependent launch ---------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+// global -> shared bulk copy, completion signalled on `bar` (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t policy) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
+}
+// shared -> global bulk copy (bulk async-group)
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// ---- geometry (computed on the host once per context) ---------------------------------------------------
+struct StreamGeom {
+  int K;                 // reduction length in elements (d_model for gate/up, d_ff for down)
+  int rows;              // rows per matrix (d_ff | d_model)
+  int n_mats;            // 2 (gate, up) | 1 (down)
+  unsigned long long mat_off[2];   // byte offset of each matrix inside the expert blob
+  int row_bytes;         // K * sizeof(T)
+  int P;                 // threads per row group = chunks per segment
+  int G;                 // row groups per CTA (G * P <= 256)
+  int RB;                // rows per matrix per stage = (kStreamVals / n_mats) * G
+  int NSEG;              // segments per row
+  int seg_bytes;         // P * 16
+  int stage_bytes;       // n_mats * RB * seg_bytes
+  int upe;               // units per entry = rows / RB
+  int n_active;          // G * P consumer threads that do work
+  int n_stages;          // ring depth
+};
+
+struct StreamArgs {
+  PlanPtrs plan;
+  int wave, C;
+  const char* pool;      // arena base; slot s of layer l at ((size_t)s * L + l) * blob_bytes
+  const char* master;    // mapped pinned host master of this layer (E blobs) or nullptr (no fused fill)
+  unsigned long long blob_bytes;
+  int L, layer;
+  const void* operand;   // MODE 0: x [T, d] model dtype; MODE 1: act [T*k, d_ff] fp32
+  float* result;         // MODE 0: act [T*k, d_ff] fp32; MODE 1: ystage [T*k, d] fp32
+  int k;                 // top_k (pair index = t*k + rank)
+  int out_ld;            // leading dimension of result (d_ff | d)
+  int pdl;               // launched with programmatic stream serialization
+};
+
+// Transposed butterfly: reduces NV per-lane values over the 32 lanes with NV-1 (+ log) shuffles.  The sum
+// of value i ends up in v[j] of lane L with (L*NV)/32 + j == i (j < max(1, NV/32)); for every value the
+// addition tree is the xor butterfly 16, 8, 4, 2, 1 (fp add commutes, so all lanes agree bit for bit).
+template <int NV>
+__device__ __forceinline__ void warp_multi_reduce(float (&v)[NV], int lane) {
+  int n = NV;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const bool up = (lane & o) != 0;
+    if (n > 1) {
+      const int h = n >> 1;
+#pragma unroll
+      for (int i = 0; i < NV / 2; ++i) {
+        if (i < h) {
+          const float keep = up ? v[i + h] : v[i];
+          const float send = up ? v[i] : v[i + h];
+          v[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+        }
+      }
+      n = h;
+    } else {
+      v[0] += __shfl_xor_sync(0xffffffffu, v[0], o);
+    }
+  }
+}
+
+template <typename T> struct ChunkW;   // a 16-byte weight chunk widened to fp32
+template <> struct ChunkW<float> {
+  static constexpr int N = 4;
+  __device__ __forceinline__ static void widen(const uint4& r, float (&v)[4]) {
+    v[0] = __uint_as_float(r.x); v[1] = __uint_as_float(r.y); v[2] = __uint_as_float(r.z); v[3] = __uint_as_float(r.w);
+  }
+};
+template <> struct ChunkW<__nv_bfloat16> {
+  static constexpr int N = 8;
+  __device__ __forceinline__ static void widen(const uint4& r, float (&v)[8]) { widen_bf16x8(r, v); }
+};
+
+// MODE 0 = gate/up + SwiGLU, MODE 1 = down.  NP = max pairs per expert handled (>= n_tokens of the call).
+template <typename T, int MODE, int NP>
+__global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const StreamArgs a, const StreamGeom gm) {
+  constexpr int EPC = ChunkW<T>::N;                         // elements per 16-byte chunk
+  constexpr int NVAL = kStreamVals * NP;                    // values reduced per thread per unit
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ __align__(8) unsigned long long s_full[kStreamMaxStages], s_empty[kStreamMaxStages];
+  __shared__ float s_red[2][kStreamConsumers / 32][NVAL];
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int NS = gm.n_stages;
+  const int n_act_warps = gm.n_active >> 5;
+  if (tid == 0) {
+    for (int s = 0; s < NS; ++s) {
+      mbar_init(smem_u32(&s_full[s]), 1);
+      mbar_init(smem_u32(&s_empty[s]), n_act_warps);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (a.pdl) {
+    // Everything this kernel reads was written by preceding kernels.  The down producer is exempt: the plan
+    // dates from before the gate/up kernel's own wait and down weights are never written by that kernel, so it
+    // starts streaming while the gate/up kernel (the immediate predecessor) drains.
+    if (MODE == 0 || warp != kStreamConsumers / 32) pdl_wait();
+    pdl_launch_dependents();          // the next kernel may start its prologue as SMs drain
+  }
+  if (a.wave >= a.plan.hdr[0]) return;
+  const int lo = a.wave * a.C, nw = min(a.plan.hdr[1], lo + a.C) - lo;
+  const long long U = (long long)nw * gm.upe;
+  const int u_lo = (int)(U * blockIdx.x / gridDim.x), u_hi = (int)(U * (blockIdx.x + 1) / gridDim.x);
+  if (u_lo >= u_hi) return;
+  const uint32_t stage0 = smem_u32(smem_raw);
+
+  if (warp == kStreamConsumers / 32) {
+    // ===================== producer warp: TMA bulk loads into the ring =====================
+    const uint64_t pol = l2_evict_first_policy();
+    const int n_copies = gm.NSEG == 1 ? gm.n_mats : gm.n_mats * gm.RB;
+    int s = 0;
+    uint32_t ph = 0;
+    for (int u = u_lo; u < u_hi; ++u) {
+      const int i = lo + u / gm.upe, rb = u % gm.upe;
+      const bool from_host = a.master != nullptr && a.plan.entry_miss[i] != 0;
+      const char* blob = from_host ? a.master + (size_t)a.plan.entry_expert[i] * a.blob_bytes
+                                   : a.pool + ((size_t)a.plan.entry_slot[i] * a.L + a.layer) * a.blob_bytes;
+      for (int seg = 0; seg < gm.NSEG; ++seg) {
+        mbar_wait(smem_u32(&s_empty[s]), ph ^ 1u);
+        const uint32_t bar = smem_u32(&s_full[s]);
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)gm.stage_bytes);
+        __syncwarp();
+        for (int c = lane; c < n_copies; c += 32) {
+          const char* src;
+          uint32_t dst, bytes;
+          if (gm.NSEG == 1) {        // the RB rows of one matrix are contiguous: one copy per matrix
+            bytes = (uint32_t)gm.RB * gm.row_bytes;
+            src = blob + gm.mat_off[c] + (size_t)rb * gm.RB * gm.row_bytes;
+            dst = stage0 + s * gm.stage_bytes + c * bytes;
+          } else {                   // one copy per (matrix, row): a seg_bytes slice of the row
+            const int m = c / gm.RB, r = c % gm.RB;
+            bytes = (uint32_t)gm.seg_bytes;
+            src = blob + gm.mat_off[m] + ((size_t)rb * gm.RB + r) * gm.row_bytes + (size_t)seg * gm.seg_bytes;
+            dst = stage0 + s * gm.stage_bytes + c * bytes;
+          }
+          bulk_g2s(dst, src, bytes, bar, pol);
+        }
+        if (++s == NS) { s = 0; ph ^= 1u; }
+      }
+    }
+    return;
+  }
+
+  // ===================== consumer warps =====================
+  if (tid >= gm.n_active) return;
+  const int g = tid / gm.P, p = tid % gm.P;
+  constexpr int RPT = kStreamVals / (MODE == 0 ? 2 : 1);     // rows per thread per matrix
+  const int warps_per_group = gm.P >> 5;
+  int s = 0;
+  uint32_t ph = 0;
+  int par = 0;
+  int cur_entry = -1, cnt = 0;
+  const int* pl = nullptr;
+  float xr[NP][EPC];
+  for (int u = u_lo; u < u_hi; ++u) {
+    const int i = lo + u / gm.upe, rb = u % gm.upe;
+    const bool new_entry = i != cur_entry;
+    if (new_entry) {
+      cur_entry = i;
+      const int e = a.plan.entry_expert[i];
+      cnt = min(a.plan.exp_count[e], NP);
+      pl = a.plan.pair_list + a.plan.exp_offset[e];
+    }
+    const bool fill = a.master != nullptr && a.plan.entry_miss[i] != 0;
+    float acc[kStreamVals][NP];
+#pragma unroll
+    for (int v = 0; v < kStreamVals; ++v)
+#pragma unroll
+      for (int q = 0; q < NP; ++q) acc[v][q] = 0.f;
+    for (int seg = 0; seg < gm.NSEG; ++seg) {
+      if (new_entry || gm.NSEG > 1) {    // (re)load the thread-stationary operand slice
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          if (q < cnt) {
+            const int pr = pl[q];
+            const size_t col = (size_t)seg * gm.P * EPC + (size_t)p * EPC;
+            if (MODE == 0) {
+              const T* xp = reinterpret_cast<const T*>(a.operand) + (size_t)(pr / a.k) * gm.K + col;
+              ChunkW<T>::widen(*reinterpret_cast<const uint4*>(xp), xr[q]);
+            } else {
+              const float* ap = reinterpret_cast<const float*>(a.operand) + (size_t)pr * gm.K + col;
+#pragma unroll
+              for (int j = 0; j < EPC; j += 4) {
+                const float4 f = *reinterpret_cast<const float4*>(ap + j);
+                xr[q][j] = f.x; xr[q][j + 1] = f.y; xr[q][j + 2] = f.z; xr[q][j + 3] = f.w;
+              }
+            }
+          }
+        }
+      }
+      mbar_wait(smem_u32(&s_full[s]), ph);
+      const uint32_t sbase = stage0 + s * gm.stage_bytes;
+      if (fill && warp == 0) {           // fused miss path: landed tile -> victim slot (same bytes)
+        char* slot = const_cast<char*>(a.pool) + ((size_t)a.plan.entry_slot[i] * a.L + a.layer) * a.blob_bytes;
+        const int n_copies = gm.NSEG == 1 ? gm.n_mats : gm.n_mats * gm.RB;
+        for (int c = lane; c < n_copies; c += 32) {
+          if (gm.NSEG == 1) {
+            const uint32_t bytes = (uint32_t)gm.RB * gm.row_bytes;
+            bulk_s2g(slot + gm.mat_off[c] + (size_t)rb * gm.RB * gm.row_bytes, sbase + c * bytes, bytes);
+          } else {
+            const int m = c / gm.RB, r = c % gm.RB;
+            bulk_s2g(slot + gm.mat_off[m] + ((size_t)rb * gm.RB + r) * gm.row_bytes + (size_t)seg * gm.seg_bytes,
+                     sbase + c * gm.seg_bytes, (uint32_t)gm.seg_bytes);
+          }
+        }
+        bulk_commit();
+      }
+      // this thread's 8 weight chunks of the stage: matrix m, row g*RPT + i, chunk p
+      uint4 wq[kStreamVals];
+#pragma unroll
+      for (int v = 0; v < kStreamVals; ++v) {
+        const int m = MODE == 0 ? v / RPT : 0, r = g * RPT + (MODE == 0 ? v % RPT : v);
+        const uint32_t addr = sbase + (uint32_t)((m * gm.RB + r) * gm.seg_bytes + p * 16);
+        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(wq[v].x), "=r"(wq[v].y), "=r"(wq[v].z), "=r"(wq[v].w) : "r"(addr));
+      }
+      if (fill && warp == 0) bulk_wait_read0();   // the bulk store has finished reading the stage
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&s_empty[s]));   // stage free: the data lives in registers now
+      if (++s == NS) { s = 0; ph ^= 1u; }
+#pragma unroll
+      for (int v = 0; v < kStreamVals; ++v) {
+        float wv[EPC];
+        ChunkW<T>::widen(wq[v], wv);
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          if (q < cnt) {
+#pragma unroll
+            for (int j = 0; j < EPC; ++j) acc[v][q] = fmaf(wv[j], xr[q][j], acc[v][q]);
+          }
+        }
+      }
+    }
+    // ---- reduce over the group's P threads: lanes (butterfly), then warps (ascending) ----
+    float red[NVAL];
+#pragma unroll
+    for (int v = 0; v < kStreamVals; ++v)
+#pragma unroll
+      for (int q = 0; q < NP; ++q) red[v * NP + q] = acc[v][q];
+    warp_multi_reduce<NVAL>(red, lane);
+    constexpr int PER_LANE = NVAL >= 32 ? NVAL / 32 : 1;
+#pragma unroll
+    for (int j = 0; j < PER_LANE; ++j) s_red[par][warp][(lane * NVAL) / 32 + j] = red[j];
+    asm volatile("bar.sync 1, %0;" ::"r"(gm.n_active) : "memory");
+    for (int o = tid; o < gm.RB * cnt; o += gm.n_active) {
+      const int r = o / cnt, q = o % cnt;                  // row inside the block, pair
+      const int rg = r / RPT, ri = r % RPT;
+      const int w0 = (rg * gm.P) >> 5;
+      const int pr = pl[q];
+      const size_t row = (size_t)rb * gm.RB + r;
+      if (MODE == 0) {
+        float gs = 0.f, us = 0.f;
+        for (int w = 0; w < warps_per_group; ++w) {
+          gs += s_red[par][w0 + w][ri * NP + q];
+          us += s_red[par][w0 + w][(RPT + ri) * NP + q];
+        }
+        a.result[(size_t)pr * a.out_ld + row] = silu_f(gs) * us;
+      } else {
+        float ys = 0.f;
+        for (int w = 0; w < warps_per_group; ++w) ys += s_red[par][w0 + w][ri * NP + q];
+        a.result[(size_t)pr * a.out_ld + row] = ys;
+      }
+    }
+    par ^= 1;
+  }
+  if (a.master != nullptr && warp == 0) bulk_wait0();   // slot writes complete before the kernel ends
+}
+
+// out[t, j] = sum_i w[t,i] * ystage[t*k+i, j] in rank order (fp32), stored in the model dtype; the optional
+// residual successor x_next = x + out uses the rounding of DESIGN.md O3.  One function so that the fused
+// (router prologue) and the standalone combine produce the same bits.
+template <typename T>
+__device__ __forceinline__ void combine_elem(const float* __restrict__ ystage, const float* __restrict__ w, int t, int j, int d, int k,
+                                             T x_in, T& out, T& x_next) {
+  float acc = 0.f;
+  for (int i = 0; i < k; ++i) acc = fmaf(w[(size_t)t * k + i], ystage[((size_t)t * k + i) * d + j], acc);
+  out = from_f32<T>(acc);
+  x_next = from_f32<T>(to_f32<T>(x_in) + to_f32<T>(out));
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ ystage, const float* __restrict__ w,
+                                                      T* __restrict__ out, const T* __restrict__ x_res,
+                                                      T* __restrict__ x_next, int n_tokens, int d, int k, int pdl) {
+  if (pdl) { pdl_wait(); pdl_launch_dependents(); }
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)n_tokens * d) return;
+  const int t = (int)(idx / d), j = (int)(idx % d);
+  T o, xn;
+  combine_elem<T>(ystage, w, t, j, d, k, x_res ? x_res[idx] : from_f32<T>(0.f), o, xn);
+  out[idx] = o;
+  if (x_res) x_next[idx] = xn;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) residual_add_kernel(const T* __restrict__ x, const T* __restrict__ y,
+                                                           T* __restrict__ out, size_t n) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < n) out[idx] = from_f32<T>(to_f32<T>(x[idx]) + to_f32<T>(y[idx]));
+}
+
+}  // namespace wisp

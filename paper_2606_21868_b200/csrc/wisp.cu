@@ -11,8 +11,8 @@
 
 #include "common.cuh"
 #include "fetch.cuh"
-#include "ffn_decode.cuh"
 #include "ffn_prefill.cuh"
+#include "ffn_stream.cuh"
 #include "mvwsa.h"
 #include "residency.cuh"
 #include "router.cuh"
@@ -76,8 +76,12 @@ struct wisp_ctx {
   std::map<int, u64> graph_nodes;
 
   std::map<int, cudaGraphExec_t> graphs;
-  int grid_gate_up = 0, grid_down = 0, grid_fetch = 0;
+  int grid_fetch = 0;
+  StreamGeom geom_gu{}, geom_dn{};   // decode FFN stream geometry (gate/up, down)
   std::string err;
+  // programmatic dependent launch between the kernels of a layer (not with host-driven copies or event timing)
+  int use_pdl() const { return cfg.fetch != WISP_FETCH_MEMCPY && timing_level == 0 && pdl_enabled; }
+  int pdl_enabled = 1;
 };
 
 namespace {
@@ -240,23 +244,87 @@ int fetch_wave(wisp_ctx* ctx, int layer, int wave, bool host_known, cudaStream_t
   return WISP_OK;
 }
 
+constexpr size_t kStreamSmemMax = 216u << 10;   // dynamic shared memory ceiling of the ring (227 KiB per CTA minus static)
+
+// ---- decode FFN (ffn_stream.cuh) -------------------------------------------------------------------------
+StreamGeom make_geom(int K, int rows, int n_mats, size_t elem, size_t off0, size_t off1, int want_stages) {
+  StreamGeom g{};
+  g.K = K; g.rows = rows; g.n_mats = n_mats;
+  g.mat_off[0] = off0; g.mat_off[1] = off1;
+  g.row_bytes = (int)(K * elem);
+  const int n_chunks = g.row_bytes / 16;            // multiple of 32 (K is a multiple of 256)
+  int q = 8;                                        // segment = 32*q chunks, the largest divisor of the row that fits 256 threads
+  while ((n_chunks / 32) % q) --q;
+  g.P = 32 * q;
+  g.NSEG = n_chunks / g.P;
+  g.G = kStreamConsumers / g.P;
+  g.RB = (kStreamVals / n_mats) * g.G;
+  g.seg_bytes = g.P * 16;
+  g.stage_bytes = n_mats * g.RB * g.seg_bytes;
+  g.upe = rows / g.RB;
+  g.n_active = g.G * g.P;
+  int ns = want_stages > 0 ? want_stages : kStreamMaxStages;
+  ns = std::min(ns, (int)(kStreamSmemMax / g.stage_bytes));
+  g.n_stages = std::max(2, std::min(ns, kStreamMaxStages));
+  return g;
+}
+
+template <typename T, int MODE, int NP>
+int launch_stream(wisp_ctx* ctx, const StreamArgs& a, const StreamGeom& g, cudaStream_t st) {
+  auto kern = ffn_stream_kernel<T, MODE, NP>;
+  const size_t smem = (size_t)g.n_stages * g.stage_bytes;
+  static bool attr_done = false;                    // per instantiation
+  if (!attr_done) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStreamSmemMax));
+    attr_done = true;
+  }
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(ctx->num_sms);
+  cfg.blockDim = dim3(kStreamThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = a.pdl ? 1 : 0;
+  CK(cudaLaunchKernelEx(&cfg, kern, a, g));
+  return WISP_OK;
+}
+
+template <typename T, int MODE>
+int launch_stream_np(wisp_ctx* ctx, const StreamArgs& a, const StreamGeom& g, int T_, cudaStream_t st) {
+  if (T_ <= 1) return launch_stream<T, MODE, 1>(ctx, a, g, st);
+  if (T_ <= 2) return launch_stream<T, MODE, 2>(ctx, a, g, st);
+  if (T_ <= 4) return launch_stream<T, MODE, 4>(ctx, a, g, st);
+  return launch_stream<T, MODE, 8>(ctx, a, g, st);
+}
+
 template <typename T>
 int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, cudaStream_t st) {
   const auto& cfg = ctx->cfg;
   const int d = cfg.d_model, dff = cfg.d_ff, k = cfg.top_k, L = cfg.n_layers;
   const T* pool = reinterpret_cast<const T*>(ctx->arena);
   if (T_ <= kDecodeMaxTokens) {
+    StreamArgs a{};
+    a.plan = ctx->plan; a.wave = wave; a.C = ctx->C;
+    a.pool = ctx->arena;
+    a.master = cfg.fetch == WISP_FETCH_FUSED ? static_cast<const char*>(ctx->master[layer]) : nullptr;
+    a.blob_bytes = ctx->Me; a.L = L; a.layer = layer; a.k = k;
+    a.pdl = ctx->use_pdl();
+    int rc;
     {
       Span sp(ctx, WISP_K_GATE_UP, st);
-      decode_gate_up_kernel<T><<<ctx->grid_gate_up, kFfnThreads, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L,
-                                                                          layer, reinterpret_cast<const T*>(x),
-                                                                          ctx->act_f32, d, dff, k);
+      a.operand = x; a.result = ctx->act_f32; a.out_ld = dff;
+      rc = launch_stream_np<T, 0>(ctx, a, ctx->geom_gu, T_, st);
     }
+    if (rc) return rc;
     {
       Span sp(ctx, WISP_K_DOWN, st);
-      decode_down_kernel<T><<<ctx->grid_down, kFfnThreads, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L,
-                                                                    layer, ctx->act_f32, ctx->ystage, d, dff);
+      a.operand = ctx->act_f32; a.result = ctx->ystage; a.out_ld = d;
+      rc = launch_stream_np<T, 1>(ctx, a, ctx->geom_dn, T_, st);
     }
+    if (rc) return rc;
   } else {
     const int ptiles = (T_ + kPfTile - 1) / kPfTile;   // an expert can receive at most T pairs
     dim3 g0(dff / kPfTile, ptiles, ctx->C), g1(d / kPfTile, ptiles, ctx->C);
@@ -298,9 +366,12 @@ int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, vo
   } else {
     n_waves = (std::min(E, n_pairs) + ctx->C - 1) / ctx->C;   // worst case; empty waves exit at once
   }
+  const bool fused_fill = cfg.fetch == WISP_FETCH_FUSED && T_ <= kDecodeMaxTokens;   // the FFN kernels fetch their own misses
   for (int w = 0; w < n_waves; ++w) {
-    rc = fetch_wave(ctx, layer, w, memcpy_path, st);
-    if (rc) return rc;
+    if (!fused_fill) {
+      rc = fetch_wave(ctx, layer, w, memcpy_path, st);
+      if (rc) return rc;
+    }
     rc = launch_ffn_wave<T>(ctx, layer, w, x, T_, st);
     if (rc) return rc;
   }
@@ -309,7 +380,7 @@ int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, vo
     Span sp(ctx, WISP_K_COMBINE, st);
     combine_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(ctx->ystage, ctx->topw + off, reinterpret_cast<T*>(out),
                                                                    x_next ? reinterpret_cast<const T*>(x) : nullptr,
-                                                                   reinterpret_cast<T*>(x_next), T_, cfg.d_model, k);
+                                                                   reinterpret_cast<T*>(x_next), T_, cfg.d_model, k, 0);
   }
   CK(cudaGetLastError());
   ctx->last_T[layer] = T_;
@@ -355,7 +426,8 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
       cfg->top_k > kMaxTopK || cfg->top_k > cfg->n_experts || cfg->d_model < 256 || cfg->d_model % 256 ||
       cfg->d_ff < 256 || cfg->d_ff % 256 || cfg->max_tokens < 1 ||
       (cfg->dtype != WISP_F32 && cfg->dtype != WISP_BF16) || (cfg->policy != WISP_LRU && cfg->policy != WISP_LFU) ||
-      (cfg->fetch != WISP_FETCH_MEMCPY && cfg->fetch != WISP_FETCH_ZEROCOPY))
+      (cfg->fetch != WISP_FETCH_MEMCPY && cfg->fetch != WISP_FETCH_ZEROCOPY && cfg->fetch != WISP_FETCH_FUSED) ||
+      cfg->ring_stages < 0 || cfg->ring_stages > kStreamMaxStages)
     return WISP_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return WISP_ECUDA;   // no CPU fallback
@@ -447,12 +519,10 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   CKC(cudaEventCreateWithFlags(&ctx->ev_compute, cudaEventDisableTiming));
   CKC(cudaEventCreateWithFlags(&ctx->ev_copy, cudaEventDisableTiming));
 #undef CKC
-  if (cfg->dtype == WISP_F32) {
-    ctx->grid_gate_up = occupancy_grid(ctx, decode_gate_up_kernel<float>, kFfnThreads, 8);
-    ctx->grid_down = occupancy_grid(ctx, decode_down_kernel<float>, kFfnThreads, 8);
-  } else {
-    ctx->grid_gate_up = occupancy_grid(ctx, decode_gate_up_kernel<__nv_bfloat16>, kFfnThreads, 8);
-    ctx->grid_down = occupancy_grid(ctx, decode_down_kernel<__nv_bfloat16>, kFfnThreads, 8);
+  {
+    const size_t gu = (size_t)d * dff * ctx->elem;
+    ctx->geom_gu = make_geom(d, dff, 2, ctx->elem, 0, gu, cfg->ring_stages);
+    ctx->geom_dn = make_geom(dff, d, 1, ctx->elem, 2 * gu, 0, cfg->ring_stages);
   }
   ctx->grid_fetch = ctx->num_sms * 2;
   *out = ctx;
@@ -532,7 +602,7 @@ int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void
     }
     return WISP_OK;
   };
-  if (ctx->cfg.fetch == WISP_FETCH_ZEROCOPY && ctx->timing_level == 0 && st != nullptr) {
+  if (ctx->cfg.fetch != WISP_FETCH_MEMCPY && ctx->timing_level == 0 && st != nullptr) {
     auto it = ctx->graphs.find(n_tokens);
     if (it == ctx->graphs.end()) {
       cudaGraph_t g = nullptr;

@@ -27,7 +27,7 @@ def streams(E, C, k):
 
 @pytest.mark.parametrize("C", [1, 2, 6, 15, 16])
 @pytest.mark.parametrize("policy", [0, 1])
-@pytest.mark.parametrize("fetch", [0, 1])
+@pytest.mark.parametrize("fetch", [0, 1, 2])
 def test_adversarial_routing_trace_and_state(C, policy, fetch):
     E = SH.n_experts
     for name, steps in streams(E, C, 3):

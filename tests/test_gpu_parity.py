@@ -48,7 +48,7 @@ def test_config1_tiny_decode_all_four_parities():
     shape = si.TINY
     hidden = si.gen_decode_hidden(shape, 128, 1)
     ref = None
-    for slots, policy, fetch in ((16, 0, 1), (6, 0, 1), (6, 0, 0), (6, 1, 1), (2, 0, 1)):
+    for slots, policy, fetch in ((16, 0, 1), (6, 0, 1), (6, 0, 0), (6, 0, 2), (6, 1, 1), (2, 0, 1), (2, 0, 2), (1, 1, 2)):
         ctx = make_ctx(shape, slots, policy=policy, fetch=fetch)
         res = run_chain(ctx, shape, hidden)
         routed = [[rec["ids"].flatten().tolist() for rec in per] for per in res]
@@ -93,12 +93,14 @@ def test_batch_decode_overflow_waves(T):
     shape = si.TINY
     hidden = si.gen_decode_hidden(shape, 12, T)
     ref = None
-    for slots in (16, 5, 1):
-        ctx = make_ctx(shape, slots, max_tokens=T)
+    for slots, fetch in ((16, 1), (5, 1), (5, 2), (1, 1), (1, 2), (3, 0)):
+        ctx = make_ctx(shape, slots, max_tokens=T, fetch=fetch)
         res = run_chain(ctx, shape, hidden)
         routed = [[rec["ids"].flatten().tolist() for rec in per] for per in res]
         want, _ = sim_trace(shape, slots, 0, routed)
         assert ctx.trace_read() == want
+        for l in range(shape.n_layers):
+            assert ctx.debug_verify_pool(l) == 0
         if ref is None:
             ref = res
             check_vs_oracle(shape, res, TOL["f32"])
@@ -111,7 +113,7 @@ def test_batch_decode_overflow_waves(T):
 def test_prefill_grouped_path(shape, T):
     hidden = si.gen_prefill_hidden(shape, T).view(1, T, shape.d_model)
     ref = None
-    for slots, fetch in ((shape.n_experts, 1), (5, 1), (5, 0), (3, 1)):
+    for slots, fetch in ((shape.n_experts, 1), (5, 1), (5, 0), (3, 1), (3, 2)):
         ctx = make_ctx(shape, slots, fetch=fetch, max_tokens=T)
         res = run_chain(ctx, shape, hidden)
         routed = [[rec["ids"].flatten().tolist() for rec in per] for per in res]
@@ -129,12 +131,14 @@ def test_bf16_decode_medium_shape():
     shape = MED
     hidden = si.gen_decode_hidden(shape, 24, 2)
     ref = None
-    for slots, policy in ((32, 0), (9, 0), (9, 1), (3, 0)):
-        ctx = make_ctx(shape, slots, policy=policy)
+    for slots, policy, fetch in ((32, 0, 1), (9, 0, 1), (9, 1, 2), (3, 0, 2), (3, 0, 0)):
+        ctx = make_ctx(shape, slots, policy=policy, fetch=fetch)
         res = run_chain(ctx, shape, hidden)
         routed = [[rec["ids"].flatten().tolist() for rec in per] for per in res]
         want, _ = sim_trace(shape, slots, policy, routed)
         assert ctx.trace_read() == want
+        for l in range(shape.n_layers):
+            assert ctx.debug_verify_pool(l) == 0
         if ref is None:
             ref = res
             worst = check_vs_oracle(shape, res, TOL["bf16"])
