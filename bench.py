@@ -43,7 +43,8 @@ def parse():
     ap.add_argument("--budget-gib", type=float, default=0.0, help="expert-pool budget (0 = the config's)")
     ap.add_argument("--batch", type=int, default=1)
     ap.add_argument("--policy", default="lru", choices=["lru", "lfu"])
-    ap.add_argument("--fetch", default="zerocopy", choices=["zerocopy", "memcpy"])
+    ap.add_argument("--fetch", default="fused", choices=["fused", "zerocopy", "memcpy"],
+                    help="miss path: fused = persistent decode kernel whose TMA producer reads misses from the mapped master")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-miss-path", action="store_true")
     ap.add_argument("--per-layer-api", action="store_true", help="drive wisp_moe_forward per layer instead of wisp_stack_forward")
@@ -134,7 +135,7 @@ def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=N
     ctx = wp.Wisp(budget, n_layers=shape.n_layers, n_experts=shape.n_experts, top_k=shape.top_k, d_model=shape.d_model,
                   d_ff=shape.d_ff, max_tokens=max_tokens, dtype=wp.WISP_F32 if shape.dtype == "f32" else wp.WISP_BF16,
                   policy=wp.WISP_LFU if args.policy == "lfu" else wp.WISP_LRU,
-                  fetch=(wp.WISP_FETCH_MEMCPY if (fetch or args.fetch) == "memcpy" else wp.WISP_FETCH_ZEROCOPY))
+                  fetch={"memcpy": wp.WISP_FETCH_MEMCPY, "zerocopy": wp.WISP_FETCH_ZEROCOPY, "fused": wp.WISP_FETCH_FUSED}[fetch or args.fetch])
     staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
     for l in (register_layers if register_layers is not None else range(shape.n_layers)):
         si.gen_layer_experts(shape, l, gen_device, out=staging)

@@ -147,85 +147,80 @@ template <> struct ChunkW<__nv_bfloat16> {
   __device__ __forceinline__ static void widen(const uint4& r, float (&v)[8]) { widen_bf16x8(r, v); }
 };
 
-// MODE 0 = gate/up + SwiGLU, MODE 1 = down.  NP = max pairs per expert handled (>= n_tokens of the call).
+// ---- the shared-memory ring ------------------------------------------------------------------------------
+struct Ring {
+  uint32_t stage0;         // shared address of stage 0
+  uint32_t full0, empty0;  // shared addresses of the full / empty mbarrier arrays (8 bytes per stage)
+  int NS;                  // stages in use
+  int stride;              // bytes between stages (>= the stage_bytes of every geometry that uses the ring)
+};
+struct RingPos { int s; uint32_t ph; };
+__device__ __forceinline__ void ring_advance(const Ring& r, RingPos& p) { if (++p.s == r.NS) { p.s = 0; p.ph ^= 1u; } }
+// full barriers: 1 arrival (the producer's expect_tx); empty barriers: one arrival per consumer warp
+__device__ __forceinline__ void ring_init(const Ring& r) {
+  for (int s = 0; s < r.NS; ++s) {
+    mbar_init(r.full0 + 8u * s, 1);
+    mbar_init(r.empty0 + 8u * s, kStreamConsumers / 32);
+  }
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+// Units [u_lo, u_hi) of the wave whose first plan entry is `lo`: the producer warp issues the TMA bulk loads.
+__device__ __forceinline__ void stream_produce(const StreamArgs& a, const StreamGeom& gm, const Ring& ring, RingPos& rp,
+                                               int lo, int u_lo, int u_hi, int lane, uint64_t pol) {
+  const int n_copies = gm.NSEG == 1 ? gm.n_mats : gm.n_mats * gm.RB;
+  for (int u = u_lo; u < u_hi; ++u) {
+    const int i = lo + u / gm.upe, rb = u % gm.upe;
+    const bool from_host = a.master != nullptr && a.plan.entry_miss[i] != 0;
+    const char* blob = from_host ? a.master + (size_t)a.plan.entry_expert[i] * a.blob_bytes
+                                 : a.pool + ((size_t)a.plan.entry_slot[i] * a.L + a.layer) * a.blob_bytes;
+    for (int seg = 0; seg < gm.NSEG; ++seg) {
+      mbar_wait(ring.empty0 + 8u * rp.s, rp.ph ^ 1u);
+      const uint32_t bar = ring.full0 + 8u * rp.s;
+      if (lane == 0) mbar_expect_tx(bar, (uint32_t)gm.stage_bytes);
+      __syncwarp();
+      const uint32_t sbase = ring.stage0 + (uint32_t)rp.s * ring.stride;
+      for (int c = lane; c < n_copies; c += 32) {
+        const char* src;
+        uint32_t bytes;
+        if (gm.NSEG == 1) {        // the RB rows of one matrix are contiguous: one copy per matrix
+          bytes = (uint32_t)gm.RB * gm.row_bytes;
+          src = blob + gm.mat_off[c] + (size_t)rb * gm.RB * gm.row_bytes;
+        } else {                   // one copy per (matrix, row): a seg_bytes slice of the row
+          const int m = c / gm.RB, r = c % gm.RB;
+          bytes = (uint32_t)gm.seg_bytes;
+          src = blob + gm.mat_off[m] + ((size_t)rb * gm.RB + r) * gm.row_bytes + (size_t)seg * gm.seg_bytes;
+        }
+        bulk_g2s(sbase + c * bytes, src, bytes, bar, pol);
+      }
+      ring_advance(ring, rp);
+    }
+  }
+}
+
+// The 8 consumer warps (tid 0..255) take the same units from the ring.  MODE 0 = gate/up + SwiGLU, MODE 1 = down.
+// NP = max pairs per expert handled (>= n_tokens of the call).  s_red: [2][8][kStreamVals*NP] floats of shared
+// memory; `par` alternates between its halves.  `red_bar` = id of a named barrier free for the n_active threads.
 template <typename T, int MODE, int NP>
-__global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const StreamArgs a, const StreamGeom gm) {
+__device__ __forceinline__ void stream_consume(const StreamArgs& a, const StreamGeom& gm, const Ring& ring, RingPos& rp,
+                                               int lo, int u_lo, int u_hi, float* s_red, int& par, int red_bar) {
   constexpr int EPC = ChunkW<T>::N;                         // elements per 16-byte chunk
   constexpr int NVAL = kStreamVals * NP;                    // values reduced per thread per unit
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  __shared__ __align__(8) unsigned long long s_full[kStreamMaxStages], s_empty[kStreamMaxStages];
-  __shared__ float s_red[2][kStreamConsumers / 32][NVAL];
-
+  constexpr int RPT = kStreamVals / (MODE == 0 ? 2 : 1);    // rows per thread per matrix
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int NS = gm.n_stages;
-  const int n_act_warps = gm.n_active >> 5;
-  if (tid == 0) {
-    for (int s = 0; s < NS; ++s) {
-      mbar_init(smem_u32(&s_full[s]), 1);
-      mbar_init(smem_u32(&s_empty[s]), n_act_warps);
+  if (tid >= gm.n_active) {
+    // a warp without work in this geometry still takes part in the ring protocol (the empty barriers count 8 warps)
+    const int n_st = (u_hi - u_lo) * gm.NSEG;
+    for (int j = 0; j < n_st; ++j) {
+      mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
+      if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);
+      ring_advance(ring, rp);
     }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  if (a.pdl) {
-    // Everything this kernel reads was written by preceding kernels.  The down producer is exempt: the plan
-    // dates from before the gate/up kernel's own wait and down weights are never written by that kernel, so it
-    // starts streaming while the gate/up kernel (the immediate predecessor) drains.
-    if (MODE == 0 || warp != kStreamConsumers / 32) pdl_wait();
-    pdl_launch_dependents();          // the next kernel may start its prologue as SMs drain
-  }
-  if (a.wave >= a.plan.hdr[0]) return;
-  const int lo = a.wave * a.C, nw = min(a.plan.hdr[1], lo + a.C) - lo;
-  const long long U = (long long)nw * gm.upe;
-  const int u_lo = (int)(U * blockIdx.x / gridDim.x), u_hi = (int)(U * (blockIdx.x + 1) / gridDim.x);
-  if (u_lo >= u_hi) return;
-  const uint32_t stage0 = smem_u32(smem_raw);
-
-  if (warp == kStreamConsumers / 32) {
-    // ===================== producer warp: TMA bulk loads into the ring =====================
-    const uint64_t pol = l2_evict_first_policy();
-    const int n_copies = gm.NSEG == 1 ? gm.n_mats : gm.n_mats * gm.RB;
-    int s = 0;
-    uint32_t ph = 0;
-    for (int u = u_lo; u < u_hi; ++u) {
-      const int i = lo + u / gm.upe, rb = u % gm.upe;
-      const bool from_host = a.master != nullptr && a.plan.entry_miss[i] != 0;
-      const char* blob = from_host ? a.master + (size_t)a.plan.entry_expert[i] * a.blob_bytes
-                                   : a.pool + ((size_t)a.plan.entry_slot[i] * a.L + a.layer) * a.blob_bytes;
-      for (int seg = 0; seg < gm.NSEG; ++seg) {
-        mbar_wait(smem_u32(&s_empty[s]), ph ^ 1u);
-        const uint32_t bar = smem_u32(&s_full[s]);
-        if (lane == 0) mbar_expect_tx(bar, (uint32_t)gm.stage_bytes);
-        __syncwarp();
-        for (int c = lane; c < n_copies; c += 32) {
-          const char* src;
-          uint32_t dst, bytes;
-          if (gm.NSEG == 1) {        // the RB rows of one matrix are contiguous: one copy per matrix
-            bytes = (uint32_t)gm.RB * gm.row_bytes;
-            src = blob + gm.mat_off[c] + (size_t)rb * gm.RB * gm.row_bytes;
-            dst = stage0 + s * gm.stage_bytes + c * bytes;
-          } else {                   // one copy per (matrix, row): a seg_bytes slice of the row
-            const int m = c / gm.RB, r = c % gm.RB;
-            bytes = (uint32_t)gm.seg_bytes;
-            src = blob + gm.mat_off[m] + ((size_t)rb * gm.RB + r) * gm.row_bytes + (size_t)seg * gm.seg_bytes;
-            dst = stage0 + s * gm.stage_bytes + c * bytes;
-          }
-          bulk_g2s(dst, src, bytes, bar, pol);
-        }
-        if (++s == NS) { s = 0; ph ^= 1u; }
-      }
-    }
+    par ^= (u_hi - u_lo) & 1;       // stay in step with the active warps' s_red half
     return;
   }
-
-  // ===================== consumer warps =====================
-  if (tid >= gm.n_active) return;
   const int g = tid / gm.P, p = tid % gm.P;
-  constexpr int RPT = kStreamVals / (MODE == 0 ? 2 : 1);     // rows per thread per matrix
   const int warps_per_group = gm.P >> 5;
-  int s = 0;
-  uint32_t ph = 0;
-  int par = 0;
   int cur_entry = -1, cnt = 0;
   const int* pl = nullptr;
   float xr[NP][EPC];
@@ -265,8 +260,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const Str
           }
         }
       }
-      mbar_wait(smem_u32(&s_full[s]), ph);
-      const uint32_t sbase = stage0 + s * gm.stage_bytes;
+      mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
+      const uint32_t sbase = ring.stage0 + (uint32_t)rp.s * ring.stride;
       if (fill && warp == 0) {           // fused miss path: landed tile -> victim slot (same bytes)
         char* slot = const_cast<char*>(a.pool) + ((size_t)a.plan.entry_slot[i] * a.L + a.layer) * a.blob_bytes;
         const int n_copies = gm.NSEG == 1 ? gm.n_mats : gm.n_mats * gm.RB;
@@ -292,8 +287,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const Str
       }
       if (fill && warp == 0) bulk_wait_read0();   // the bulk store has finished reading the stage
       __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&s_empty[s]));   // stage free: the data lives in registers now
-      if (++s == NS) { s = 0; ph ^= 1u; }
+      if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);   // stage free: the data lives in registers now
+      ring_advance(ring, rp);
 #pragma unroll
       for (int v = 0; v < kStreamVals; ++v) {
         float wv[EPC];
@@ -315,9 +310,10 @@ __global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const Str
       for (int q = 0; q < NP; ++q) red[v * NP + q] = acc[v][q];
     warp_multi_reduce<NVAL>(red, lane);
     constexpr int PER_LANE = NVAL >= 32 ? NVAL / 32 : 1;
+    float* sr = s_red + (size_t)par * (kStreamConsumers / 32) * NVAL;
 #pragma unroll
-    for (int j = 0; j < PER_LANE; ++j) s_red[par][warp][(lane * NVAL) / 32 + j] = red[j];
-    asm volatile("bar.sync 1, %0;" ::"r"(gm.n_active) : "memory");
+    for (int j = 0; j < PER_LANE; ++j) sr[warp * NVAL + (lane * NVAL) / 32 + j] = red[j];
+    asm volatile("bar.sync %0, %1;" ::"r"(red_bar), "r"(gm.n_active) : "memory");
     for (int o = tid; o < gm.RB * cnt; o += gm.n_active) {
       const int r = o / cnt, q = o % cnt;                  // row inside the block, pair
       const int rg = r / RPT, ri = r % RPT;
@@ -327,26 +323,59 @@ __global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const Str
       if (MODE == 0) {
         float gs = 0.f, us = 0.f;
         for (int w = 0; w < warps_per_group; ++w) {
-          gs += s_red[par][w0 + w][ri * NP + q];
-          us += s_red[par][w0 + w][(RPT + ri) * NP + q];
+          gs += sr[(w0 + w) * NVAL + ri * NP + q];
+          us += sr[(w0 + w) * NVAL + (RPT + ri) * NP + q];
         }
         a.result[(size_t)pr * a.out_ld + row] = silu_f(gs) * us;
       } else {
         float ys = 0.f;
-        for (int w = 0; w < warps_per_group; ++w) ys += s_red[par][w0 + w][ri * NP + q];
+        for (int w = 0; w < warps_per_group; ++w) ys += sr[(w0 + w) * NVAL + ri * NP + q];
         a.result[(size_t)pr * a.out_ld + row] = ys;
       }
     }
     par ^= 1;
   }
-  if (a.master != nullptr && warp == 0) bulk_wait0();   // slot writes complete before the kernel ends
+  if (a.master != nullptr && warp == 0) bulk_wait0();   // this warp's slot writes are complete
+}
+
+// One wave of one FFN half as its own launch (multi-kernel path: MEMCPY / ZEROCOPY contexts, timing level 2).
+template <typename T, int MODE, int NP>
+__global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const StreamArgs a, const StreamGeom gm) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ __align__(8) unsigned long long s_full[kStreamMaxStages], s_empty[kStreamMaxStages];
+  __shared__ float s_red[2 * (kStreamConsumers / 32) * kStreamVals * NP];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  Ring ring;
+  ring.stage0 = smem_u32(smem_raw); ring.full0 = smem_u32(s_full); ring.empty0 = smem_u32(s_empty);
+  ring.NS = gm.n_stages; ring.stride = gm.stage_bytes;
+  if (tid == 0) ring_init(ring);
+  __syncthreads();
+  if (a.pdl) {
+    // Everything this kernel reads was written by preceding kernels.  The down producer is exempt: the plan
+    // dates from before the gate/up kernel's own wait and down weights are never written by that kernel, so it
+    // starts streaming while the gate/up kernel (the immediate predecessor) drains.
+    if (MODE == 0 || warp != kStreamConsumers / 32) pdl_wait();
+    pdl_launch_dependents();          // the next kernel may start its prologue as SMs drain
+  }
+  if (a.wave >= a.plan.hdr[0]) return;
+  const int lo = a.wave * a.C, nw = min(a.plan.hdr[1], lo + a.C) - lo;
+  const long long U = (long long)nw * gm.upe;
+  const int u_lo = (int)(U * blockIdx.x / gridDim.x), u_hi = (int)(U * (blockIdx.x + 1) / gridDim.x);
+  if (u_lo >= u_hi) return;
+  RingPos rp{0, 0u};
+  if (warp == kStreamConsumers / 32) {
+    stream_produce(a, gm, ring, rp, lo, u_lo, u_hi, lane, l2_evict_first_policy());
+  } else {
+    int par = 0;
+    stream_consume<T, MODE, NP>(a, gm, ring, rp, lo, u_lo, u_hi, s_red, par, 1);
+  }
 }
 
 // out[t, j] = sum_i w[t,i] * ystage[t*k+i, j] in rank order (fp32), stored in the model dtype; the optional
 // residual successor x_next = x + out uses the rounding of DESIGN.md O3.  One function so that the fused
 // (router prologue) and the standalone combine produce the same bits.
 template <typename T>
-__device__ __forceinline__ void combine_elem(const float* __restrict__ ystage, const float* __restrict__ w, int t, int j, int d, int k,
+__device__ __forceinline__ void combine_elem(const float* ystage, const float* w, int t, int j, int d, int k,
                                              T x_in, T& out, T& x_next) {
   float acc = 0.f;
   for (int i = 0; i < k; ++i) acc = fmaf(w[(size_t)t * k + i], ystage[((size_t)t * k + i) * d + j], acc);

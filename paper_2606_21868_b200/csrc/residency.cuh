@@ -27,8 +27,33 @@ struct PlanArgs {
   int build_pairs;                // build pair_list here (small n_pairs) or leave it to group_pairs_kernel
 };
 
-// exclusive scan over the block (blockDim.x == kPlanThreads); ws = 33 ints of scratch
-__device__ __forceinline__ int block_excl_scan(int v, int* ws, int& total) {
+// ---- Algorithm 1 as a device function, usable by a standalone CTA (NT = 1024 threads) and by every CTA of the
+// persistent decode kernel (NT = 256 consumer threads, all CTAs compute the same plan, one of them is the writer).
+// NT = participating threads (threadIdx.x < NT) = capacity in experts (E <= NT); `bar` = named barrier id for them.
+template <int NT>
+struct PlanShared {
+  unsigned bitmap[NT / 32];
+  int cnt[NT];
+  int R[NT];              // sorted distinct routed ids
+  int pi[NT];
+  int pinv[NT];
+  u64 tau[NT];
+  u64 freq[NT];
+  u64 kf[NT];             // LFU component of the victim key per slot (also scratch of the MV-WSA tracking pass)
+  unsigned char inw[NT], elig[NT];
+  int victim[NT];
+  int ws[NT / 32 + 1];
+  u64 clock;
+  int evict;
+};
+
+template <int NT>
+__device__ __forceinline__ void plan_sync(int bar) { asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(NT) : "memory"); }
+
+// exclusive scan over the NT participating threads; ws = NT/32 + 1 ints of scratch
+template <int NT>
+__device__ __forceinline__ int block_excl_scan(int v, int* ws, int& total, int bar) {
+  constexpr int NW = NT / 32;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int inc = v;
 #pragma unroll
@@ -37,21 +62,21 @@ __device__ __forceinline__ int block_excl_scan(int v, int* ws, int& total) {
     if (lane >= o) inc += n;
   }
   if (lane == 31) ws[wid] = inc;
-  __syncthreads();
+  plan_sync<NT>(bar);
   if (wid == 0) {
-    int s = ws[lane], si = s;
+    int s = lane < NW ? ws[lane] : 0, si = s;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       int n = __shfl_up_sync(0xffffffffu, si, o);
       if (lane >= o) si += n;
     }
-    ws[lane] = si - s;
-    if (lane == 31) ws[32] = si;
+    if (lane < NW) ws[lane] = si - s;
+    if (lane == 31) ws[NW] = si;
   }
-  __syncthreads();
-  total = ws[32];
+  plan_sync<NT>(bar);
+  total = ws[NW];
   int r = inc - v + ws[wid];
-  __syncthreads();
+  plan_sync<NT>(bar);
   return r;
 }
 
@@ -62,75 +87,68 @@ __device__ __forceinline__ bool key_less(u64 fa, u64 ta, int sa, u64 fb, u64 tb,
   return sa < sb;
 }
 
-__global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a) {
-  __shared__ unsigned bitmap[kMaxExperts / 32];
-  __shared__ int s_cnt[kMaxExperts];
-  __shared__ int s_R[kMaxExperts];        // sorted distinct routed ids
-  __shared__ int s_pi[kMaxExperts];
-  __shared__ int s_pinv[kMaxExperts];
-  __shared__ u64 s_tau[kMaxExperts];
-  __shared__ u64 s_kf[kMaxExperts];       // LFU component of the victim key per slot
-  __shared__ unsigned char s_inw[kMaxExperts];
-  __shared__ unsigned char s_elig[kMaxExperts];
-  __shared__ int s_victim[kMaxExperts];
-  __shared__ int s_ws[33];
-  __shared__ int s_nR;
-  __shared__ u64 s_clock;
-  __shared__ int s_evict;
+// pi, pi^-1, tau, f, clock of this layer -> shared memory.  The caller synchronises before plan_compute.
+template <int NT>
+__device__ __forceinline__ void plan_load(PlanShared<NT>& sh, const LayerState& st, int E, int C) {
+  const int tid = threadIdx.x;
+  if (tid < E) { sh.pi[tid] = st.pi[tid]; sh.freq[tid] = st.freq[tid]; }
+  if (tid < C) { sh.pinv[tid] = st.pi_inv[tid]; sh.tau[tid] = st.tau[tid]; }
+  if (tid == 0) sh.clock = st.scal[0];
+}
 
+// One WISPLAYER.STEP(R) (all waves) on the state in `sh`; the plan goes to a.plan (global or shared pointers).
+// writer: this CTA also writes the state back, counts, traces and feeds the MV-WSA histograms.
+template <int NT>
+__device__ __forceinline__ void plan_compute(const PlanArgs& a, PlanShared<NT>& sh, bool writer, int bar) {
   const int tid = threadIdx.x;
   const int E = a.E, C = a.C;
-  if (tid < kMaxExperts / 32) bitmap[tid] = 0u;
-  if (tid < E) { s_cnt[tid] = 0; s_pi[tid] = a.st.pi[tid]; }
-  if (tid < C) { s_pinv[tid] = a.st.pi_inv[tid]; s_tau[tid] = a.st.tau[tid]; }
-  if (tid == 0) { s_clock = a.st.scal[0]; s_evict = 0; }
-  __syncthreads();
+  if (tid < NT / 32) sh.bitmap[tid] = 0u;
+  if (tid < E) sh.cnt[tid] = 0;
+  if (tid == 0) sh.evict = 0;
+  plan_sync<NT>(bar);
 
   // ---- R = set of routed ids; per-expert pair counts ----
-  for (int p = tid; p < a.n_pairs; p += kPlanThreads) {
+  for (int p = tid; p < a.n_pairs; p += NT) {
     int e = a.ids[p];
-    atomicOr(&bitmap[e >> 5], 1u << (e & 31));
-    atomicAdd(&s_cnt[e], 1);
+    atomicOr(&sh.bitmap[e >> 5], 1u << (e & 31));
+    atomicAdd(&sh.cnt[e], 1);
   }
-  __syncthreads();
+  plan_sync<NT>(bar);
   int total = 0;
   {
-    const int present = (tid < E) ? ((bitmap[tid >> 5] >> (tid & 31)) & 1) : 0;
-    int pos = block_excl_scan(present, s_ws, total);
-    if (present) s_R[pos] = tid;
-    if (tid == 0) s_nR = total;
+    const int present = (tid < E) ? ((sh.bitmap[tid >> 5] >> (tid & 31)) & 1) : 0;
+    int pos = block_excl_scan<NT>(present, sh.ws, total, bar);
+    if (present) sh.R[pos] = tid;
   }
   const int nR = total;
   {
     int tot2;
-    int off = block_excl_scan(tid < E ? s_cnt[tid] : 0, s_ws, tot2);
-    if (tid < E) { a.plan.exp_offset[tid] = off; a.plan.exp_count[tid] = s_cnt[tid]; }
+    int off = block_excl_scan<NT>(tid < E ? sh.cnt[tid] : 0, sh.ws, tot2, bar);
+    if (tid < E) { a.plan.exp_offset[tid] = off; a.plan.exp_count[tid] = sh.cnt[tid]; }
     if (tid == 0) a.plan.exp_offset[E] = tot2;
     if (a.build_pairs && tid < a.n_pairs) {
       // stable grouping for small n_pairs: rank among lower-indexed pairs of the same expert
       const int e = a.ids[tid];
       int r = 0;
       for (int q = 0; q < tid; ++q) r += (a.ids[q] == e);
-      // offset of expert e (recompute from the scan of thread e: read back from global after sync below)
-      s_victim[tid] = r;   // borrow as scratch (n_pairs <= kMaxExperts in this mode)
+      sh.victim[tid] = r;   // borrowed as scratch (n_pairs <= NT in this mode)
     }
   }
-  __syncthreads();
+  plan_sync<NT>(bar);
   if (a.build_pairs && tid < a.n_pairs) {
     const int e = a.ids[tid];
-    // exp_offset[e] was written by thread e of this block; visible after __syncthreads + same-CTA global write
-    a.plan.pair_list[a.plan.exp_offset[e] + s_victim[tid]] = tid;
+    a.plan.pair_list[a.plan.exp_offset[e] + sh.victim[tid]] = tid;   // exp_offset written by thread e above
   }
-  __syncthreads();
+  plan_sync<NT>(bar);
 
   // ---- MV-WSA reuse-distance tracking: stack distance of every reference ----
-  if (a.track && nR > 0) {
-    __shared__ u64 s_last[kMaxExperts];
+  if (writer && a.track && nR > 0) {
+    u64* s_last = sh.kf;
     if (tid < E) s_last[tid] = a.st.last_pos[tid];
-    __syncthreads();
+    plan_sync<NT>(bar);
     const u64 base = a.st.scal[6];   // linear position counter of this layer
     if (tid < nR) {
-      const int e = s_R[tid];
+      const int e = sh.R[tid];
       const u64 mine = s_last[e];
       int bin;
       if (mine == 0) {
@@ -139,25 +157,25 @@ __global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a
         int dist = 1 + tid;          // e itself + the tid lower ids of this step (referenced just before)
         for (int o = 0; o < E; ++o) {
           if (o == e) continue;
-          const bool in_step_before = ((bitmap[o >> 5] >> (o & 31)) & 1) && o < e;
+          const bool in_step_before = ((sh.bitmap[o >> 5] >> (o & 31)) & 1) && o < e;
           if (!in_step_before && s_last[o] > mine) ++dist;
         }
         bin = dist > E ? E + 1 : dist;
       }
       atomicAdd(&a.st.hist[bin], 1ull);
     }
-    __syncthreads();
-    if (tid < nR) a.st.last_pos[s_R[tid]] = base + 1 + tid;
+    plan_sync<NT>(bar);
+    if (tid < nR) a.st.last_pos[sh.R[tid]] = base + 1 + tid;
     if (tid == 0) a.st.scal[6] = base + nR;
-    __syncthreads();
+    plan_sync<NT>(bar);
   }
 
   // ---- Algorithm 1 per wave ----
   const int n_waves = (nR + C - 1) / C;
-  const u64 step_no = a.st.scal[1];
+  const u64 step_no = writer ? a.st.scal[1] : 0ull;
   bool trace_ok = false;
   u64 trace_base = 0;
-  if (a.trace_on) {
+  if (writer && a.trace_on) {
     trace_base = a.trace_ctr[0];
     trace_ok = trace_base + (u64)nR <= a.trace_cap;
   }
@@ -165,51 +183,51 @@ __global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a
   for (int wv = 0; wv < n_waves; ++wv) {
     const int lo = wv * C;
     const int nw = min(C, nR - lo);
-    if (tid < E) s_inw[tid] = 0;
-    __syncthreads();
+    if (tid < E) sh.inw[tid] = 0;
+    plan_sync<NT>(bar);
     int e = -1, is_miss = 0;
-    if (tid < nw) { e = s_R[lo + tid]; s_inw[e] = 1; is_miss = s_pi[e] < 0; }
-    __syncthreads();
+    if (tid < nw) { e = sh.R[lo + tid]; sh.inw[e] = 1; is_miss = sh.pi[e] < 0; }
+    plan_sync<NT>(bar);
     int n_miss;
-    const int mi = block_excl_scan(is_miss, s_ws, n_miss);       // line 2: M = R \ dom(pi), ascending id
+    const int mi = block_excl_scan<NT>(is_miss, sh.ws, n_miss, bar);       // line 2: M = R \ dom(pi), ascending id
     // line 3: U = {s : pi^-1(s) not in R} in increasing key
     if (tid < C) {
-      const int occ = s_pinv[tid];
-      s_elig[tid] = (occ < 0) || !s_inw[occ];
-      s_kf[tid] = (a.policy == WISP_LFU) ? (occ < 0 ? 0ull : a.st.freq[occ] + 1ull) : 0ull;
+      const int occ = sh.pinv[tid];
+      sh.elig[tid] = (occ < 0) || !sh.inw[occ];
+      sh.kf[tid] = (a.policy == WISP_LFU) ? (occ < 0 ? 0ull : sh.freq[occ] + 1ull) : 0ull;
     }
-    __syncthreads();
-    if (tid < C && s_elig[tid] && n_miss > 0) {
-      const u64 kf = s_kf[tid], kt = s_tau[tid];
+    plan_sync<NT>(bar);
+    if (tid < C && sh.elig[tid] && n_miss > 0) {
+      const u64 kf = sh.kf[tid], kt = sh.tau[tid];
       int rank = 0;
       for (int o = 0; o < C; ++o)
-        if (s_elig[o] && key_less(s_kf[o], s_tau[o], o, kf, kt, tid)) ++rank;
-      if (rank < n_miss) s_victim[rank] = tid;
+        if (sh.elig[o] && key_less(sh.kf[o], sh.tau[o], o, kf, kt, tid)) ++rank;
+      if (rank < n_miss) sh.victim[rank] = tid;
     }
-    __syncthreads();
-    // lines 4-8: assign, (copy happens in the fetch step), update the maps
+    plan_sync<NT>(bar);
+    // lines 4-8: assign, (the copy happens in the fetch step), update the maps
     int slot = -1, old = -1;
     if (tid < nw) {
       if (is_miss) {
-        slot = s_victim[mi];
-        old = s_pinv[slot];
-        if (old >= 0) { s_pi[old] = -1; atomicAdd(&s_evict, 1); }
-        s_pi[e] = slot;
-        s_pinv[slot] = e;
+        slot = sh.victim[mi];
+        old = sh.pinv[slot];
+        if (old >= 0) { sh.pi[old] = -1; atomicAdd(&sh.evict, 1); }
+        sh.pi[e] = slot;
+        sh.pinv[slot] = e;
       } else {
-        slot = s_pi[e];
+        slot = sh.pi[e];
       }
     }
-    if (tid == 0) s_clock += 1;                                   // line 9: c <- c + 1
-    __syncthreads();
+    if (tid == 0) sh.clock += 1;                                   // line 9: c <- c + 1
+    plan_sync<NT>(bar);
     if (tid < nw) {
-      s_tau[slot] = s_clock;                                      // tau[pi(e)] <- c
-      a.st.freq[e] += 1ull;
+      sh.tau[slot] = sh.clock;                                     // tau[pi(e)] <- c
+      sh.freq[e] += 1ull;
       const int idx = lo + tid;
       a.plan.entry_expert[idx] = e;
       a.plan.entry_slot[idx] = slot;
       a.plan.entry_miss[idx] = is_miss;
-      if (a.host_plan) {
+      if (writer && a.host_plan) {
         a.host_plan->entry_expert[idx] = e;
         a.host_plan->entry_slot[idx] = slot;
         a.host_plan->entry_miss[idx] = is_miss;
@@ -223,30 +241,40 @@ __global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a
     }
     hits_total += nw - n_miss;
     miss_total += n_miss;
-    __syncthreads();
+    plan_sync<NT>(bar);
   }
+  if (tid == 0) { a.plan.hdr[0] = n_waves; a.plan.hdr[1] = nR; a.plan.hdr[2] = miss_total; a.plan.hdr[3] = a.n_pairs; }
 
   // ---- write back ----
-  if (tid < E) a.st.pi[tid] = s_pi[tid];
-  if (tid < C) { a.st.pi_inv[tid] = s_pinv[tid]; a.st.tau[tid] = s_tau[tid]; }
-  if (tid == 0) {
-    a.plan.hdr[0] = n_waves; a.plan.hdr[1] = nR; a.plan.hdr[2] = miss_total; a.plan.hdr[3] = a.n_pairs;
-    if (a.host_plan) {
-      a.host_plan->n_ref = nR; a.host_plan->n_miss = miss_total; a.host_plan->n_pairs = a.n_pairs;
-      __threadfence_system();
-      a.host_plan->n_waves = n_waves;
-    }
-    a.st.scal[0] = s_clock;
-    if (nR > 0) a.st.scal[1] = step_no + 1;
-    a.st.scal[2] += (u64)hits_total;
-    a.st.scal[3] += (u64)miss_total;
-    a.st.scal[4] += (u64)s_evict;
-    a.st.scal[5] += (u64)nR;
-    if (a.trace_on) {
-      if (trace_ok) a.trace_ctr[0] = trace_base + (u64)nR;
-      else a.trace_ctr[1] += (u64)nR;
+  if (writer) {
+    if (tid < E) { a.st.pi[tid] = sh.pi[tid]; a.st.freq[tid] = sh.freq[tid]; }
+    if (tid < C) { a.st.pi_inv[tid] = sh.pinv[tid]; a.st.tau[tid] = sh.tau[tid]; }
+    if (tid == 0) {
+      if (a.host_plan) {
+        a.host_plan->n_ref = nR; a.host_plan->n_miss = miss_total; a.host_plan->n_pairs = a.n_pairs;
+        __threadfence_system();
+        a.host_plan->n_waves = n_waves;
+      }
+      a.st.scal[0] = sh.clock;
+      if (nR > 0) a.st.scal[1] = step_no + 1;
+      a.st.scal[2] += (u64)hits_total;
+      a.st.scal[3] += (u64)miss_total;
+      a.st.scal[4] += (u64)sh.evict;
+      a.st.scal[5] += (u64)nR;
+      if (a.trace_on) {
+        if (trace_ok) a.trace_ctr[0] = trace_base + (u64)nR;
+        else a.trace_ctr[1] += (u64)nR;
+      }
     }
   }
+  plan_sync<NT>(bar);
+}
+
+__global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a) {
+  __shared__ PlanShared<kPlanThreads> sh;
+  plan_load<kPlanThreads>(sh, a.st, a.E, a.C);
+  __syncthreads();
+  plan_compute<kPlanThreads>(a, sh, /*writer=*/true, /*bar=*/0);
 }
 
 // Stable grouping of (token, rank) pairs by expert for large n_pairs: one CTA per expert.
@@ -327,9 +355,9 @@ __global__ void __launch_bounds__(kPlanThreads) residency_resize_kernel(ResizeAr
   const int is_move = (tid < Co && keep && tid >= Cn);
   const int is_free = (tid < Cn && !(occ >= 0 && keep));
   int n_drop, n_move, n_free;
-  const int di = block_excl_scan(is_drop, s_ws, n_drop);
-  const int mi = block_excl_scan(is_move, s_ws, n_move);
-  const int fi = block_excl_scan(is_free, s_ws, n_free);
+  const int di = block_excl_scan<kPlanThreads>(is_drop, s_ws, n_drop, 0);
+  const int mi = block_excl_scan<kPlanThreads>(is_move, s_ws, n_move, 0);
+  const int fi = block_excl_scan<kPlanThreads>(is_free, s_ws, n_free, 0);
   __shared__ int s_free[kMaxExperts];
   if (is_free) s_free[fi] = tid;
   __syncthreads();

@@ -9,19 +9,14 @@ namespace wisp {
 
 constexpr int kRouterTokTile = 4;
 
-// grid (ceil(E/8), ceil(T/4)), block 256: warp = one expert row against up to 4 tokens.
+// One warp: logits of expert row `wrow` against tokens t0 .. t0+nt-1 (nt <= 4) of x.  Canonical order (common.cuh):
+// lane l takes the 16-byte chunks l, l+32, ... in ascending order into one fp32 accumulator per token, then the
+// xor butterfly; lane 0 writes z[t][e] = sum + bias.  Used by the standalone kernel and the persistent decode kernel.
 template <typename T>
-__global__ void __launch_bounds__(256) router_logits_kernel(const T* __restrict__ x, const T* __restrict__ w_r,
-                                                            const float* __restrict__ bias, float* __restrict__ z,
-                                                            int n_tokens, int E, int d) {
+__device__ __forceinline__ void router_row_warp(const T* x, const T* wrow, float bias_e, float* z, int e, int t0, int nt,
+                                                int E, int d, int lane) {
   constexpr int N = Chunk<T>::N;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int e = blockIdx.x * 8 + warp;
-  const int t0 = blockIdx.y * kRouterTokTile;
-  if (e >= E) return;
-  const int nt = min(kRouterTokTile, n_tokens - t0);
   float acc[kRouterTokTile] = {0.f, 0.f, 0.f, 0.f};
-  const T* wrow = w_r + (size_t)e * d;
   for (int c = lane * N; c < d; c += 32 * N) {
     float wv[N];
     Chunk<T>::load(wrow + c, wv);
@@ -35,24 +30,28 @@ __global__ void __launch_bounds__(256) router_logits_kernel(const T* __restrict_
       }
     }
   }
-  const float b = bias ? bias[e] : 0.f;
 #pragma unroll
   for (int tt = 0; tt < kRouterTokTile; ++tt) {
     float s = warp_sum(acc[tt]);
-    if (tt < nt && lane == 0) z[(size_t)(t0 + tt) * E + e] = s + b;
+    if (tt < nt && lane == 0) z[(size_t)(t0 + tt) * E + e] = s + bias_e;
   }
 }
 
-// One warp per token; block 128 = 4 tokens.  smem: 4 * E floats.
-__global__ void __launch_bounds__(128) topk_softmax_kernel(const float* __restrict__ z, int* __restrict__ ids,
-                                                           float* __restrict__ w, int n_tokens, int E, int k) {
-  extern __shared__ float sz[];
+// grid (ceil(E/8), ceil(T/4)), block 256: warp = one expert row against up to 4 tokens.
+template <typename T>
+__global__ void __launch_bounds__(256) router_logits_kernel(const T* __restrict__ x, const T* __restrict__ w_r,
+                                                            const float* __restrict__ bias, float* __restrict__ z,
+                                                            int n_tokens, int E, int d) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int t = blockIdx.x * 4 + warp;
-  if (t >= n_tokens) return;
-  float* row = sz + warp * E;
-  for (int e = lane; e < E; e += 32) row[e] = z[(size_t)t * E + e];
-  __syncwarp();
+  const int e = blockIdx.x * 8 + warp;
+  const int t0 = blockIdx.y * kRouterTokTile;
+  if (e >= E) return;
+  router_row_warp<T>(x, w_r + (size_t)e * d, bias ? bias[e] : 0.f, z, e, t0, min(kRouterTokTile, n_tokens - t0), E, d, lane);
+}
+
+// One warp, one token: `row` = that token's E logits in shared memory (destroyed).  ids (z desc, id asc) and the
+// softmax over the selected k (G7) go to ids_out[0..k) / w_out[0..k) (any address space).
+__device__ __forceinline__ void topk_softmax_warp(float* row, int E, int k, int lane, int* ids_out, float* w_out) {
   float my_z = 0.f;  // lane i keeps the i-th selected logit
   int my_id = 0;
   for (int i = 0; i < k; ++i) {
@@ -77,9 +76,22 @@ __global__ void __launch_bounds__(128) topk_softmax_kernel(const float* __restri
   float den = 0.f;
   for (int i = 0; i < k; ++i) den += __shfl_sync(0xffffffffu, ex, i);   // fixed order
   if (lane < k) {
-    ids[(size_t)t * k + lane] = my_id;
-    w[(size_t)t * k + lane] = ex / den;
+    ids_out[lane] = my_id;
+    w_out[lane] = ex / den;
   }
+}
+
+// One warp per token; block 128 = 4 tokens.  smem: 4 * E floats.
+__global__ void __launch_bounds__(128) topk_softmax_kernel(const float* __restrict__ z, int* __restrict__ ids,
+                                                           float* __restrict__ w, int n_tokens, int E, int k) {
+  extern __shared__ float sz[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int t = blockIdx.x * 4 + warp;
+  if (t >= n_tokens) return;
+  float* row = sz + warp * E;
+  for (int e = lane; e < E; e += 32) row[e] = z[(size_t)t * E + e];
+  __syncwarp();
+  topk_softmax_warp(row, E, k, lane, ids + (size_t)t * k, w + (size_t)t * k);
 }
 
 }  // namespace wisp

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "common.cuh"
+#include "decode_persistent.cuh"
 #include "fetch.cuh"
 #include "ffn_prefill.cuh"
 #include "ffn_stream.cuh"
@@ -78,6 +79,16 @@ struct wisp_ctx {
   std::map<int, cudaGraphExec_t> graphs;
   int grid_fetch = 0;
   StreamGeom geom_gu{}, geom_dn{};   // decode FFN stream geometry (gate/up, down)
+  // persistent decode kernel (decode_persistent.cuh)
+  const char** d_masters = nullptr;  // device [L]: mapped master pointers
+  unsigned* gbar = nullptr;          // grid barrier counter
+  int* dev_err = nullptr;            // device error flag (grid barrier timeout)
+  u64* phase_ns = nullptr;           // device [kPersistPhases]
+  int persist_enabled = 1;
+  u64 persist_layers_timed = 0;
+  bool use_persistent(int T_) const {
+    return persist_enabled && cfg.fetch == WISP_FETCH_FUSED && T_ <= kDecodeMaxTokens && cfg.n_experts <= kPersistMaxExperts;
+  }
   std::string err;
   // programmatic dependent launch between the kernels of a layer (not with host-driven copies or event timing)
   int use_pdl() const { return cfg.fetch != WISP_FETCH_MEMCPY && timing_level == 0 && pdl_enabled; }
@@ -345,6 +356,64 @@ int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, c
   return WISP_OK;
 }
 
+// ---- persistent decode kernel: layers [lo, hi) of one token batch in one cooperative launch ----------------------
+template <typename T, int NP>
+int launch_persistent_np(wisp_ctx* ctx, PersistArgs& pa, cudaStream_t st) {
+  auto kern = decode_persistent_kernel<T, NP>;
+  static int n_stages = 0, stride = 0;
+  static size_t smem = 0;
+  if (!n_stages) {                                  // per instantiation (geometry is per context shape: recomputed below if it changes)
+    cudaFuncAttributes fa;
+    CK(cudaFuncGetAttributes(&fa, kern));
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((227u << 10) - fa.sharedSizeBytes)));
+    smem = (227u << 10) - fa.sharedSizeBytes;
+  }
+  stride = std::max(ctx->geom_gu.stage_bytes, ctx->geom_dn.stage_bytes);
+  n_stages = (int)std::min<size_t>(kStreamMaxStages, smem / stride);
+  if (ctx->cfg.ring_stages > 0) n_stages = std::min(n_stages, (int)ctx->cfg.ring_stages);
+  if (n_stages < 2) return fail(ctx, WISP_EINVAL, "persistent decode kernel: ring does not fit shared memory");
+  CK(cudaMemsetAsync(ctx->gbar, 0, sizeof(unsigned), st));
+  StreamGeom ggu = ctx->geom_gu, gdn = ctx->geom_dn;
+  void* args[] = {&pa, &ggu, &gdn, &n_stages, &stride};
+  CK(cudaLaunchCooperativeKernel((const void*)kern, dim3(ctx->num_sms), dim3(kStreamThreads), args, (size_t)n_stages * stride, st));
+  ++ctx->launches;
+  return WISP_OK;
+}
+
+template <typename T>
+int launch_persistent(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out, bool residual, cudaStream_t st) {
+  const auto& cfg = ctx->cfg;
+  PersistArgs pa{};
+  pa.L = cfg.n_layers; pa.E = cfg.n_experts; pa.k = cfg.top_k; pa.d = cfg.d_model; pa.dff = cfg.d_ff; pa.T = T_; pa.C = ctx->C;
+  pa.policy = cfg.policy; pa.layer_lo = lo; pa.layer_hi = hi; pa.residual = residual ? 1 : 0; pa.fused = 1;
+  pa.pool = ctx->arena; pa.masters = reinterpret_cast<const char* const*>(ctx->d_masters); pa.blob_bytes = ctx->Me;
+  pa.router_w = ctx->router_w; pa.router_bias = ctx->router_bias;
+  pa.pi = ctx->pi; pa.pi_inv = ctx->pi_inv; pa.tau = ctx->tau; pa.freq = ctx->freq; pa.scal = ctx->scal;
+  pa.last_pos = ctx->last_pos; pa.hist = ctx->hist;
+  pa.logits = ctx->logits; pa.ids = ctx->ids; pa.topw = ctx->topw; pa.max_tokens = cfg.max_tokens;
+  pa.act = ctx->act_f32; pa.ystage = ctx->ystage;
+  pa.x_in = x; pa.xbuf[0] = ctx->xbuf[0]; pa.xbuf[1] = ctx->xbuf[1]; pa.out = out;
+  pa.gbar = ctx->gbar; pa.err = ctx->dev_err;
+  pa.trace = ctx->trace; pa.trace_ctr = ctx->trace_ctr; pa.trace_cap = ctx->trace_cap; pa.trace_on = ctx->trace_on;
+  pa.track = ctx->track;
+  pa.phase_ns = ctx->timing_level >= 2 ? ctx->phase_ns : nullptr;
+  int rc;
+  if (T_ <= 1) rc = launch_persistent_np<T, 1>(ctx, pa, st);
+  else if (T_ <= 2) rc = launch_persistent_np<T, 2>(ctx, pa, st);
+  else if (T_ <= 4) rc = launch_persistent_np<T, 4>(ctx, pa, st);
+  else rc = launch_persistent_np<T, 8>(ctx, pa, st);
+  if (rc) return rc;
+  for (int l = lo; l < hi; ++l) ctx->last_T[l] = T_;
+  ctx->last_layer = hi - 1;
+  if (ctx->timing_level >= 2) ctx->persist_layers_timed += (u64)(hi - lo);
+  return WISP_OK;
+}
+
+int launch_persistent_any(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out, bool residual, cudaStream_t st) {
+  return ctx->cfg.dtype == WISP_F32 ? launch_persistent<float>(ctx, lo, hi, x, T_, out, residual, st)
+                                    : launch_persistent<__nv_bfloat16>(ctx, lo, hi, x, T_, out, residual, st);
+}
+
 // One MoE layer: router -> residency -> per wave (fetch, FFN) -> combine.  x_next != nullptr also writes
 // the residual successor (stack helper).
 template <typename T>
@@ -514,6 +583,13 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   CKC(cudaMalloc(&ctx->trace, ctx->trace_cap * sizeof(wisp_trace_event)));
   CKC(cudaMalloc(&ctx->trace_ctr, 2 * sizeof(u64)));
   CKC(cudaMemset(ctx->trace_ctr, 0, 2 * sizeof(u64)));
+  CKC(cudaMalloc(&ctx->d_masters, (size_t)L * sizeof(char*)));
+  CKC(cudaMemset(ctx->d_masters, 0, (size_t)L * sizeof(char*)));
+  CKC(cudaMalloc(&ctx->gbar, sizeof(unsigned)));
+  CKC(cudaMalloc(&ctx->dev_err, sizeof(int)));
+  CKC(cudaMemset(ctx->dev_err, 0, sizeof(int)));
+  CKC(cudaMalloc(&ctx->phase_ns, kPersistPhases * sizeof(u64)));
+  CKC(cudaMemset(ctx->phase_ns, 0, kPersistPhases * sizeof(u64)));
   CKC(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
   CKC(cudaEventCreateWithFlags(&ctx->ev_plan, cudaEventDisableTiming));
   CKC(cudaEventCreateWithFlags(&ctx->ev_compute, cudaEventDisableTiming));
@@ -539,7 +615,7 @@ int wisp_destroy(wisp_ctx* ctx) {
                       ctx->freq,     ctx->scal,     ctx->last_pos,    ctx->hist,    ctx->logits,  ctx->ids,
                       ctx->topw,     ctx->plan_mem, ctx->act_f32,     ctx->act_T,   ctx->ystage,  ctx->xbuf[0],
                       ctx->xbuf[1],  ctx->ybuf,     ctx->dbg_ids,     ctx->moves,   ctx->bad_slots, ctx->trace,
-                      ctx->trace_ctr};
+                      ctx->trace_ctr, ctx->d_masters, ctx->gbar, ctx->dev_err, ctx->phase_ns};
   for (void* p : dev_ptrs)
     if (p) cudaFree(p);
   if (ctx->host_plan) cudaFreeHost(ctx->host_plan);
@@ -573,6 +649,7 @@ int wisp_register_host_experts(wisp_ctx* ctx, int32_t layer, const void* experts
     for (auto& t : th) t.join();
   }
   ctx->master[layer] = m;
+  CK(cudaMemcpy(ctx->d_masters + layer, &m, sizeof(char*), cudaMemcpyHostToDevice));
   CK(cudaMemcpy(ctx->router_w + (size_t)layer * E * d * ctx->elem, router_w, E * d * ctx->elem, cudaMemcpyHostToDevice));
   if (router_bias) CK(cudaMemcpy(ctx->router_bias + (size_t)layer * E, router_bias, E * sizeof(float), cudaMemcpyHostToDevice));
   else CK(cudaMemset(ctx->router_bias + (size_t)layer * E, 0, E * sizeof(float)));
@@ -584,6 +661,8 @@ int wisp_moe_forward(wisp_ctx* ctx, int32_t layer, const void* hidden, int32_t n
   int rc = check_forward_args(ctx, layer, layer + 1, hidden, n_tokens, out);
   if (rc) return rc;
   if (n_tokens == 0) return WISP_OK;
+  if (ctx->use_persistent(n_tokens))
+    return launch_persistent_any(ctx, layer, layer + 1, hidden, n_tokens, out, false, static_cast<cudaStream_t>(cuda_stream));
   return forward_layer_any(ctx, layer, hidden, n_tokens, out, nullptr, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -593,6 +672,7 @@ int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void
   if (n_tokens == 0) return WISP_OK;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const int L = ctx->cfg.n_layers;
+  if (ctx->use_persistent(n_tokens)) return launch_persistent_any(ctx, 0, L, hidden, n_tokens, hidden_out, true, st);
   const size_t bytes = (size_t)n_tokens * ctx->cfg.d_model * ctx->elem;
   CK(cudaMemcpyAsync(ctx->xbuf[0], hidden, bytes, cudaMemcpyDeviceToDevice, st));
   auto chain = [&](cudaStream_t s) -> int {
@@ -703,6 +783,11 @@ int wisp_stats(wisp_ctx* ctx, wisp_stats_t* out) {
   const int L = ctx->cfg.n_layers;
   std::vector<u64> s((size_t)L * 8);
   CK(cudaDeviceSynchronize());
+  {
+    int derr = 0;
+    CK(cudaMemcpy(&derr, ctx->dev_err, sizeof(int), cudaMemcpyDeviceToHost));
+    if (derr) return fail(ctx, WISP_ECUDA, "persistent decode kernel: grid barrier timed out");
+  }
   CK(cudaMemcpy(s.data(), ctx->scal, s.size() * sizeof(u64), cudaMemcpyDeviceToHost));
   for (int l = 0; l < L; ++l) {
     out->total.steps += s[l * 8 + 1]; out->total.hits += s[l * 8 + 2]; out->total.misses += s[l * 8 + 3];
@@ -845,6 +930,14 @@ int wisp_timing_read(wisp_ctx* ctx, double* ms, uint64_t* launches, int32_t rese
   if (!ctx || !ms || !launches) return fail(ctx, WISP_EINVAL, "bad argument");
   CK(cudaDeviceSynchronize());
   harvest_timing(ctx, true);
+  if (ctx->persist_layers_timed) {   // phases of the persistent decode kernel, stamped with %globaltimer by CTA 0
+    u64 ns[kPersistPhases];
+    CK(cudaMemcpy(ns, ctx->phase_ns, sizeof(ns), cudaMemcpyDeviceToHost));
+    CK(cudaMemset(ctx->phase_ns, 0, sizeof(ns)));
+    const int cls[kPersistPhases] = {WISP_K_ROUTER, WISP_K_RESIDENCY, WISP_K_GATE_UP, WISP_K_DOWN, WISP_K_COMBINE};
+    for (int i = 0; i < kPersistPhases; ++i) { ctx->class_ms[cls[i]] += (double)ns[i] * 1e-6; ctx->class_n[cls[i]] += ctx->persist_layers_timed; }
+    ctx->persist_layers_timed = 0;
+  }
   for (int i = 0; i < WISP_N_KERNEL_CLASSES; ++i) { ms[i] = ctx->class_ms[i]; launches[i] = ctx->class_n[i]; }
   if (reset)
     for (int i = 0; i < WISP_N_KERNEL_CLASSES; ++i) { ctx->class_ms[i] = 0.0; ctx->class_n[i] = 0; }
