@@ -50,6 +50,18 @@ template <> struct Chunk<__nv_bfloat16> {
   }
 };
 
+template <typename T> struct ChunkW;   // a 16-byte weight chunk widened to fp32
+template <> struct ChunkW<float> {
+  static constexpr int N = 4;
+  __device__ __forceinline__ static void widen(const uint4& r, float (&v)[4]) {
+    v[0] = __uint_as_float(r.x); v[1] = __uint_as_float(r.y); v[2] = __uint_as_float(r.z); v[3] = __uint_as_float(r.w);
+  }
+};
+template <> struct ChunkW<__nv_bfloat16> {
+  static constexpr int N = 8;
+  __device__ __forceinline__ static void widen(const uint4& r, float (&v)[8]) { widen_bf16x8(r, v); }
+};
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

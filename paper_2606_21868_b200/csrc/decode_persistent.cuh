@@ -16,7 +16,7 @@
 //   phase X  combine (+ residual)     distributed over all CTAs, rank order (combine_elem)        -> barrier E
 //
 // Every arithmetic step calls the same device function as the multi-kernel path (router_row_warp,
-// topk_softmax_warp, plan_compute, stream_consume, combine_elem), so both paths give the same bits (parity (b)).
+// topk_softmax_block, plan_compute, stream_consume, combine_elem), so both paths give the same bits (parity (b)).
 #pragma once
 #include "common.cuh"
 #include "ffn_stream.cuh"
@@ -66,6 +66,18 @@ struct PersistPlan {            // the per-layer plan in shared memory (same fie
   int pair_list[kDecodeMaxTokens * kMaxTopK];
 };
 
+__device__ __forceinline__ LayerState layer_state_of(const PersistArgs& a, int l) {
+  LayerState st;
+  const size_t E = a.E;
+  st.pi = a.pi + l * E; st.pi_inv = a.pi_inv + l * E; st.tau = a.tau + l * E; st.freq = a.freq + l * E;
+  st.scal = a.scal + (size_t)l * 8; st.last_pos = a.last_pos + l * E; st.hist = a.hist + l * (E + 2);
+  return st;
+}
+
+__device__ __forceinline__ void l2_prefetch(const void* p, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 __device__ __forceinline__ u64 globaltimer_ns() {
   u64 t;
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
@@ -94,10 +106,11 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
                                                                               const StreamGeom gdn, int n_stages, int stage_stride) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(8) unsigned long long s_full[kStreamMaxStages], s_empty[kStreamMaxStages], s_plan_ready;
-  __shared__ float s_red[2 * (kStreamConsumers / 32) * kStreamVals * NP];
+  __shared__ float s_red[2 * (kStreamConsumers / 32) * StreamBatch<NP>::NVAL];
   __shared__ PlanShared<kPersistMaxExperts> sh;
   __shared__ PersistPlan pl;
-  __shared__ float s_z[NP][kPersistMaxExperts];
+  __shared__ float s_z[NP * kPersistMaxExperts];   // logits, rows packed E apart
+  __shared__ float s_selz[NP * kMaxTopK];
   __shared__ int s_ids[NP * kMaxTopK];
   __shared__ float s_w[NP * kMaxTopK];
 
@@ -150,17 +163,14 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
   };
   unsigned gen = 0;
   int par = 0;
+  plan_load<kPersistMaxExperts>(sh, layer_state_of(a, a.layer_lo), E, C);
   for (int l = a.layer_lo; l < a.layer_hi; ++l) {
     const int rel = l - a.layer_lo;
     const T* x_l = reinterpret_cast<const T*>(rel == 0 ? a.x_in : a.xbuf[(rel - 1) & 1]);
     T* x_next = reinterpret_cast<T*>(l == a.layer_hi - 1 ? a.out : a.xbuf[rel & 1]);
-    LayerState st;
-    st.pi = a.pi + (size_t)l * E; st.pi_inv = a.pi_inv + (size_t)l * E; st.tau = a.tau + (size_t)l * E;
-    st.freq = a.freq + (size_t)l * E; st.scal = a.scal + (size_t)l * 8; st.last_pos = a.last_pos + (size_t)l * E;
-    st.hist = a.hist + (size_t)l * (E + 2);
+    const LayerState st = layer_state_of(a, l);
 
-    // ---- phase R: residency state -> smem (stable: only this layer's plan phase writes it); router logits ----
-    plan_load<kPersistMaxExperts>(sh, st, E, C);
+    // ---- phase R: router logits (this layer's residency state is already in `sh`, its router rows in L2) ----
     {
       const T* wr = reinterpret_cast<const T*>(a.router_w) + (size_t)l * E * d;
       const float* bias = a.router_bias + (size_t)l * E;
@@ -172,12 +182,9 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
     stamp(0);
 
     // ---- phase P: top-k + softmax per token (one warp each), then Algorithm 1, redundantly in every CTA ----
-    for (int t = warp; t < T_; t += kStreamConsumers / 32) {
-      for (int e = lane; e < E; e += 32) s_z[t][e] = a.logits[(size_t)t * E + e];
-      __syncwarp();
-      topk_softmax_warp(s_z[t], E, k, lane, s_ids + t * k, s_w + t * k);
-    }
+    for (int i = tid; i < T_ * E; i += kStreamConsumers) s_z[i] = a.logits[i];
     asm volatile("bar.sync 1, 256;" ::: "memory");
+    topk_softmax_block(s_z, T_, E, k, s_ids, s_w, s_selz, kStreamConsumers, 1);
     if (writer && tid < T_ * k) {
       const size_t off = (size_t)l * a.max_tokens * k;
       a.ids[off + tid] = s_ids[tid];
@@ -192,6 +199,14 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
       plan_compute<kPersistMaxExperts>(pa, sh, writer, 1);
     }
     if (tid == 0) mbar_arrive(smem_u32(&s_plan_ready));                      // the producer may start streaming
+    if (l + 1 < a.layer_hi) {
+      // While the ring fills: the next layer's residency state -> smem (stable until that layer's own plan phase)
+      // and its router rows -> L2, so the serial router -> top-k -> plan chain of layer l+1 starts from warm data.
+      plan_load<kPersistMaxExperts>(sh, layer_state_of(a, l + 1), E, C);
+      const char* wr = a.router_w + (size_t)(l + 1) * E * d * sizeof(T);
+      for (int e = warp * gridDim.x + blockIdx.x; e < E; e += (kStreamConsumers / 32) * gridDim.x)
+        if (lane == 0) l2_prefetch(wr + (size_t)e * d * sizeof(T), (uint32_t)(d * sizeof(T)));
+    }
     stamp(1);
 
     // ---- phases G, D per wave ----

@@ -135,18 +135,6 @@ __device__ __forceinline__ void warp_multi_reduce(float (&v)[NV], int lane) {
   }
 }
 
-template <typename T> struct ChunkW;   // a 16-byte weight chunk widened to fp32
-template <> struct ChunkW<float> {
-  static constexpr int N = 4;
-  __device__ __forceinline__ static void widen(const uint4& r, float (&v)[4]) {
-    v[0] = __uint_as_float(r.x); v[1] = __uint_as_float(r.y); v[2] = __uint_as_float(r.z); v[3] = __uint_as_float(r.w);
-  }
-};
-template <> struct ChunkW<__nv_bfloat16> {
-  static constexpr int N = 8;
-  __device__ __forceinline__ static void widen(const uint4& r, float (&v)[8]) { widen_bf16x8(r, v); }
-};
-
 // ---- the shared-memory ring ------------------------------------------------------------------------------
 struct Ring {
   uint32_t stage0;         // shared address of stage 0
@@ -198,15 +186,43 @@ __device__ __forceinline__ void stream_produce(const StreamArgs& a, const Stream
   }
 }
 
-// The 8 consumer warps (tid 0..255) take the same units from the ring.  MODE 0 = gate/up + SwiGLU, MODE 1 = down.
-// NP = max pairs per expert handled (>= n_tokens of the call).  s_red: [2][8][kStreamVals*NP] floats of shared
-// memory; `par` alternates between its halves.  `red_bar` = id of a named barrier free for the n_active threads.
+// Accumulators per consumer thread between two reductions: 32 (64 for NP = 8) = row blocks per batch x 8 rows x NP.
+template <int NP> struct StreamBatch {
+  static constexpr int SPU = NP <= 4 ? 4 / NP : 1;          // row blocks (ring stages per segment) per batch
+  static constexpr int NVAL = SPU * kStreamVals * NP;       // values reduced per thread per batch
+};
+
+// acc[v][q] += <weight chunk v, operand chunk of pair q> for q < CNT, elements in ascending order (canonical order).
+template <typename T, int NP, int CNT>
+__device__ __forceinline__ void stream_fma(const uint4 (&wq)[kStreamVals], const float (&xr)[NP][ChunkW<T>::N],
+                                           float (&acc)[kStreamVals][NP]) {
+  constexpr int EPC = ChunkW<T>::N;
+#pragma unroll
+  for (int v = 0; v < kStreamVals; ++v) {
+    float wv[EPC];
+    ChunkW<T>::widen(wq[v], wv);
+#pragma unroll
+    for (int q = 0; q < CNT; ++q)
+#pragma unroll
+      for (int j = 0; j < EPC; ++j) acc[v][q] = fmaf(wv[j], xr[q][j], acc[v][q]);
+  }
+}
+
+// The 8 consumer warps (tid 0..255) take the same row blocks from the ring.  MODE 0 = gate/up + SwiGLU, MODE 1 = down.
+// NP = max pairs per expert handled (>= n_tokens of the call).  Thread p of a row group keeps chunk p of the operand
+// in registers and one fp32 accumulator per (row, pair); up to SPU consecutive row blocks of an entry are accumulated
+// before ONE cross-thread reduction (lanes: transposed xor butterfly; warps: ascending, through s_red) and one
+// epilogue, so the block-wide barrier and the SiLU/store tail are paid once per batch, not once per ring stage.
+// Batching changes which dot products are reduced together, never the summation order inside one of them.
+// s_red: [2][8][NVAL] floats of shared memory; `par` alternates between its halves; `red_bar` = a named barrier id
+// free for the n_active threads.
 template <typename T, int MODE, int NP>
 __device__ __forceinline__ void stream_consume(const StreamArgs& a, const StreamGeom& gm, const Ring& ring, RingPos& rp,
                                                int lo, int u_lo, int u_hi, float* s_red, int& par, int red_bar) {
   constexpr int EPC = ChunkW<T>::N;                         // elements per 16-byte chunk
-  constexpr int NVAL = kStreamVals * NP;                    // values reduced per thread per unit
-  constexpr int RPT = kStreamVals / (MODE == 0 ? 2 : 1);    // rows per thread per matrix
+  constexpr int SPU = StreamBatch<NP>::SPU;
+  constexpr int NVAL = StreamBatch<NP>::NVAL;
+  constexpr int RPT = kStreamVals / (MODE == 0 ? 2 : 1);    // rows per thread per matrix per row block
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid >= gm.n_active) {
     // a warp without work in this geometry still takes part in the ring protocol (the empty barriers count 8 warps)
@@ -216,7 +232,11 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
       if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);
       ring_advance(ring, rp);
     }
-    par ^= (u_hi - u_lo) & 1;       // stay in step with the active warps' s_red half
+    for (int u = u_lo; u < u_hi;) {   // stay in step with the active warps' s_red half: one flip per batch
+      const int rb = u % gm.upe;
+      u += min(SPU, min(u_hi - u, gm.upe - rb));
+      par ^= 1;
+    }
     return;
   }
   const int g = tid / gm.P, p = tid % gm.P;
@@ -224,9 +244,10 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
   int cur_entry = -1, cnt = 0;
   const int* pl = nullptr;
   float xr[NP][EPC];
-  for (int u = u_lo; u < u_hi; ++u) {
-    const int i = lo + u / gm.upe, rb = u % gm.upe;
-    const bool new_entry = i != cur_entry;
+  for (int u = u_lo; u < u_hi;) {
+    const int i = lo + u / gm.upe, rb0 = u % gm.upe;
+    const int nb = min(SPU, min(u_hi - u, gm.upe - rb0));   // row blocks of this batch (all of entry i)
+    bool new_entry = i != cur_entry;
     if (new_entry) {
       cur_entry = i;
       const int e = a.plan.entry_expert[i];
@@ -234,106 +255,128 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
       pl = a.plan.pair_list + a.plan.exp_offset[e];
     }
     const bool fill = a.master != nullptr && a.plan.entry_miss[i] != 0;
-    float acc[kStreamVals][NP];
+    float acc[SPU][kStreamVals][NP];
 #pragma unroll
-    for (int v = 0; v < kStreamVals; ++v)
+    for (int b = 0; b < SPU; ++b)
 #pragma unroll
-      for (int q = 0; q < NP; ++q) acc[v][q] = 0.f;
-    for (int seg = 0; seg < gm.NSEG; ++seg) {
-      if (new_entry || gm.NSEG > 1) {    // (re)load the thread-stationary operand slice
+      for (int v = 0; v < kStreamVals; ++v)
 #pragma unroll
-        for (int q = 0; q < NP; ++q) {
-          if (q < cnt) {
-            const int pr = pl[q];
-            const size_t col = (size_t)seg * gm.P * EPC + (size_t)p * EPC;
-            if (MODE == 0) {
-              const T* xp = reinterpret_cast<const T*>(a.operand) + (size_t)(pr / a.k) * gm.K + col;
-              ChunkW<T>::widen(*reinterpret_cast<const uint4*>(xp), xr[q]);
-            } else {
-              const float* ap = reinterpret_cast<const float*>(a.operand) + (size_t)pr * gm.K + col;
+        for (int q = 0; q < NP; ++q) acc[b][v][q] = 0.f;
 #pragma unroll
-              for (int j = 0; j < EPC; j += 4) {
-                const float4 f = *reinterpret_cast<const float4*>(ap + j);
-                xr[q][j] = f.x; xr[q][j + 1] = f.y; xr[q][j + 2] = f.z; xr[q][j + 3] = f.w;
+    for (int b = 0; b < SPU; ++b) {
+      if (b < nb) {
+        const int rb = rb0 + b;
+        for (int seg = 0; seg < gm.NSEG; ++seg) {
+          if (new_entry || gm.NSEG > 1) {    // (re)load the thread-stationary operand slice
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+              if (q < cnt) {
+                const int pr = pl[q];
+                const size_t col = (size_t)seg * gm.P * EPC + (size_t)p * EPC;
+                if (MODE == 0) {
+                  const T* xp = reinterpret_cast<const T*>(a.operand) + (size_t)(pr / a.k) * gm.K + col;
+                  ChunkW<T>::widen(*reinterpret_cast<const uint4*>(xp), xr[q]);
+                } else {
+                  const float* ap = reinterpret_cast<const float*>(a.operand) + (size_t)pr * gm.K + col;
+#pragma unroll
+                  for (int j = 0; j < EPC; j += 4) {
+                    const float4 f = *reinterpret_cast<const float4*>(ap + j);
+                    xr[q][j] = f.x; xr[q][j + 1] = f.y; xr[q][j + 2] = f.z; xr[q][j + 3] = f.w;
+                  }
+                }
               }
             }
+            new_entry = false;
           }
-        }
-      }
-      mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
-      const uint32_t sbase = ring.stage0 + (uint32_t)rp.s * ring.stride;
-      if (fill && warp == 0) {           // fused miss path: landed tile -> victim slot (same bytes)
-        char* slot = const_cast<char*>(a.pool) + ((size_t)a.plan.entry_slot[i] * a.L + a.layer) * a.blob_bytes;
-        const int n_copies = gm.NSEG == 1 ? gm.n_mats : gm.n_mats * gm.RB;
-        for (int c = lane; c < n_copies; c += 32) {
-          if (gm.NSEG == 1) {
-            const uint32_t bytes = (uint32_t)gm.RB * gm.row_bytes;
-            bulk_s2g(slot + gm.mat_off[c] + (size_t)rb * gm.RB * gm.row_bytes, sbase + c * bytes, bytes);
-          } else {
-            const int m = c / gm.RB, r = c % gm.RB;
-            bulk_s2g(slot + gm.mat_off[m] + ((size_t)rb * gm.RB + r) * gm.row_bytes + (size_t)seg * gm.seg_bytes,
-                     sbase + c * gm.seg_bytes, (uint32_t)gm.seg_bytes);
+          mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
+#ifdef WISP_PROBE_SKIP_MATH   // profiling probe only (never built into the product): the ring's pure streaming rate
+          __syncwarp();
+          if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);
+          ring_advance(ring, rp);
+          continue;
+#endif
+          const uint32_t sbase = ring.stage0 + (uint32_t)rp.s * ring.stride;
+          if (fill && warp == 0) {           // fused miss path: landed tile -> victim slot (same bytes)
+            char* slot = const_cast<char*>(a.pool) + ((size_t)a.plan.entry_slot[i] * a.L + a.layer) * a.blob_bytes;
+            const int n_copies = gm.NSEG == 1 ? gm.n_mats : gm.n_mats * gm.RB;
+            for (int c = lane; c < n_copies; c += 32) {
+              if (gm.NSEG == 1) {
+                const uint32_t bytes = (uint32_t)gm.RB * gm.row_bytes;
+                bulk_s2g(slot + gm.mat_off[c] + (size_t)rb * gm.RB * gm.row_bytes, sbase + c * bytes, bytes);
+              } else {
+                const int m = c / gm.RB, r = c % gm.RB;
+                bulk_s2g(slot + gm.mat_off[m] + ((size_t)rb * gm.RB + r) * gm.row_bytes + (size_t)seg * gm.seg_bytes,
+                         sbase + c * gm.seg_bytes, (uint32_t)gm.seg_bytes);
+              }
+            }
+            bulk_commit();
           }
-        }
-        bulk_commit();
-      }
-      // this thread's 8 weight chunks of the stage: matrix m, row g*RPT + i, chunk p
-      uint4 wq[kStreamVals];
+          // this thread's 8 weight chunks of the stage: matrix m, row g*RPT + i, chunk p
+          uint4 wq[kStreamVals];
 #pragma unroll
-      for (int v = 0; v < kStreamVals; ++v) {
-        const int m = MODE == 0 ? v / RPT : 0, r = g * RPT + (MODE == 0 ? v % RPT : v);
-        const uint32_t addr = sbase + (uint32_t)((m * gm.RB + r) * gm.seg_bytes + p * 16);
-        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(wq[v].x), "=r"(wq[v].y), "=r"(wq[v].z), "=r"(wq[v].w) : "r"(addr));
-      }
-      if (fill && warp == 0) bulk_wait_read0();   // the bulk store has finished reading the stage
-      __syncwarp();
-      if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);   // stage free: the data lives in registers now
-      ring_advance(ring, rp);
+          for (int v = 0; v < kStreamVals; ++v) {
+            const int m = MODE == 0 ? v / RPT : 0, r = g * RPT + (MODE == 0 ? v % RPT : v);
+            const uint32_t addr = sbase + (uint32_t)((m * gm.RB + r) * gm.seg_bytes + p * 16);
+            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(wq[v].x), "=r"(wq[v].y), "=r"(wq[v].z), "=r"(wq[v].w) : "r"(addr));
+          }
+          if (fill && warp == 0) bulk_wait_read0();   // the bulk store has finished reading the stage
+          __syncwarp();
+          if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);   // stage free: the data lives in registers now
+          ring_advance(ring, rp);
+          if (NP == 1 || cnt == 1) stream_fma<T, NP, 1>(wq, xr, acc[b]);
+          else if (NP == 2 || cnt == 2) stream_fma<T, NP, (NP >= 2 ? 2 : 1)>(wq, xr, acc[b]);
+          else if (cnt == 3) stream_fma<T, NP, (NP >= 3 ? 3 : 1)>(wq, xr, acc[b]);
+          else if (NP == 4 || cnt == 4) stream_fma<T, NP, (NP >= 4 ? 4 : 1)>(wq, xr, acc[b]);
+          else {                                         // NP == 8, cnt in 5..8: unused pairs hold stale operands,
+#pragma unroll                                           // their sums are never read
+            for (int q = 0; q < NP; ++q) if (q >= cnt)
 #pragma unroll
-      for (int v = 0; v < kStreamVals; ++v) {
-        float wv[EPC];
-        ChunkW<T>::widen(wq[v], wv);
-#pragma unroll
-        for (int q = 0; q < NP; ++q) {
-          if (q < cnt) {
-#pragma unroll
-            for (int j = 0; j < EPC; ++j) acc[v][q] = fmaf(wv[j], xr[q][j], acc[v][q]);
+              for (int j = 0; j < EPC; ++j) xr[q][j] = 0.f;
+            stream_fma<T, NP, NP>(wq, xr, acc[b]);
           }
         }
       }
     }
+#ifndef WISP_PROBE_SKIP_MATH
     // ---- reduce over the group's P threads: lanes (butterfly), then warps (ascending) ----
     float red[NVAL];
 #pragma unroll
-    for (int v = 0; v < kStreamVals; ++v)
+    for (int b = 0; b < SPU; ++b)
 #pragma unroll
-      for (int q = 0; q < NP; ++q) red[v * NP + q] = acc[v][q];
+      for (int v = 0; v < kStreamVals; ++v)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) red[(b * kStreamVals + v) * NP + q] = acc[b][v][q];
     warp_multi_reduce<NVAL>(red, lane);
     constexpr int PER_LANE = NVAL >= 32 ? NVAL / 32 : 1;
     float* sr = s_red + (size_t)par * (kStreamConsumers / 32) * NVAL;
 #pragma unroll
     for (int j = 0; j < PER_LANE; ++j) sr[warp * NVAL + (lane * NVAL) / 32 + j] = red[j];
     asm volatile("bar.sync %0, %1;" ::"r"(red_bar), "r"(gm.n_active) : "memory");
-    for (int o = tid; o < gm.RB * cnt; o += gm.n_active) {
-      const int r = o / cnt, q = o % cnt;                  // row inside the block, pair
+    const int n_out = nb * gm.RB * cnt;                    // (row block, row inside the block, pair)
+    for (int o = tid; o < n_out; o += gm.n_active) {
+      const int q = o % cnt, rr = o / cnt;
+      const int b = rr / gm.RB, r = rr % gm.RB;
       const int rg = r / RPT, ri = r % RPT;
       const int w0 = (rg * gm.P) >> 5;
       const int pr = pl[q];
-      const size_t row = (size_t)rb * gm.RB + r;
+      const size_t row = (size_t)(rb0 + b) * gm.RB + r;
+      const float* base = sr + (size_t)w0 * NVAL + (b * kStreamVals) * NP + q;
       if (MODE == 0) {
         float gs = 0.f, us = 0.f;
         for (int w = 0; w < warps_per_group; ++w) {
-          gs += sr[(w0 + w) * NVAL + ri * NP + q];
-          us += sr[(w0 + w) * NVAL + (RPT + ri) * NP + q];
+          gs += base[w * NVAL + ri * NP];
+          us += base[w * NVAL + (RPT + ri) * NP];
         }
         a.result[(size_t)pr * a.out_ld + row] = silu_f(gs) * us;
       } else {
         float ys = 0.f;
-        for (int w = 0; w < warps_per_group; ++w) ys += sr[(w0 + w) * NVAL + ri * NP + q];
+        for (int w = 0; w < warps_per_group; ++w) ys += base[w * NVAL + ri * NP];
         a.result[(size_t)pr * a.out_ld + row] = ys;
       }
     }
+#endif
     par ^= 1;
+    u += nb;
   }
   if (a.master != nullptr && warp == 0) bulk_wait0();   // this warp's slot writes are complete
 }
@@ -343,7 +386,7 @@ template <typename T, int MODE, int NP>
 __global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const StreamArgs a, const StreamGeom gm) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(8) unsigned long long s_full[kStreamMaxStages], s_empty[kStreamMaxStages];
-  __shared__ float s_red[2 * (kStreamConsumers / 32) * kStreamVals * NP];
+  __shared__ float s_red[2 * (kStreamConsumers / 32) * StreamBatch<NP>::NVAL];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   Ring ring;
   ring.stage0 = smem_u32(smem_raw); ring.full0 = smem_u32(s_full); ring.empty0 = smem_u32(s_empty);

@@ -43,6 +43,7 @@ struct PlanShared {
   unsigned char inw[NT], elig[NT];
   int victim[NT];
   int ws[NT / 32 + 1];
+  u64 scal[8];            // the layer's scalars as loaded (clock, step, hits, misses, evictions, references, position)
   u64 clock;
   int evict;
 };
@@ -93,6 +94,7 @@ __device__ __forceinline__ void plan_load(PlanShared<NT>& sh, const LayerState& 
   const int tid = threadIdx.x;
   if (tid < E) { sh.pi[tid] = st.pi[tid]; sh.freq[tid] = st.freq[tid]; }
   if (tid < C) { sh.pinv[tid] = st.pi_inv[tid]; sh.tau[tid] = st.tau[tid]; }
+  if (tid < 8) sh.scal[tid] = st.scal[tid];
   if (tid == 0) sh.clock = st.scal[0];
 }
 
@@ -146,7 +148,7 @@ __device__ __forceinline__ void plan_compute(const PlanArgs& a, PlanShared<NT>& 
     u64* s_last = sh.kf;
     if (tid < E) s_last[tid] = a.st.last_pos[tid];
     plan_sync<NT>(bar);
-    const u64 base = a.st.scal[6];   // linear position counter of this layer
+    const u64 base = sh.scal[6];     // linear position counter of this layer
     if (tid < nR) {
       const int e = sh.R[tid];
       const u64 mine = s_last[e];
@@ -172,7 +174,7 @@ __device__ __forceinline__ void plan_compute(const PlanArgs& a, PlanShared<NT>& 
 
   // ---- Algorithm 1 per wave ----
   const int n_waves = (nR + C - 1) / C;
-  const u64 step_no = writer ? a.st.scal[1] : 0ull;
+  const u64 step_no = sh.scal[1];
   bool trace_ok = false;
   u64 trace_base = 0;
   if (writer && a.trace_on) {
@@ -255,12 +257,12 @@ __device__ __forceinline__ void plan_compute(const PlanArgs& a, PlanShared<NT>& 
         __threadfence_system();
         a.host_plan->n_waves = n_waves;
       }
-      a.st.scal[0] = sh.clock;
+      a.st.scal[0] = sh.clock;                    // stores only: the old values were loaded by plan_load
       if (nR > 0) a.st.scal[1] = step_no + 1;
-      a.st.scal[2] += (u64)hits_total;
-      a.st.scal[3] += (u64)miss_total;
-      a.st.scal[4] += (u64)sh.evict;
-      a.st.scal[5] += (u64)nR;
+      a.st.scal[2] = sh.scal[2] + (u64)hits_total;
+      a.st.scal[3] = sh.scal[3] + (u64)miss_total;
+      a.st.scal[4] = sh.scal[4] + (u64)sh.evict;
+      a.st.scal[5] = sh.scal[5] + (u64)nR;
       if (a.trace_on) {
         if (trace_ok) a.trace_ctr[0] = trace_base + (u64)nR;
         else a.trace_ctr[1] += (u64)nR;

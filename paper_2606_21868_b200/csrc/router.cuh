@@ -16,17 +16,30 @@ template <typename T>
 __device__ __forceinline__ void router_row_warp(const T* x, const T* wrow, float bias_e, float* z, int e, int t0, int nt,
                                                 int E, int d, int lane) {
   constexpr int N = Chunk<T>::N;
+  constexpr int UN = 8;                       // weight chunks in flight per lane (loads hoisted; the FMA order is unchanged)
   float acc[kRouterTokTile] = {0.f, 0.f, 0.f, 0.f};
-  for (int c = lane * N; c < d; c += 32 * N) {
-    float wv[N];
-    Chunk<T>::load(wrow + c, wv);
+  for (int c0 = lane * N; c0 < d; c0 += UN * 32 * N) {
+    uint4 raw[UN];
 #pragma unroll
-    for (int tt = 0; tt < kRouterTokTile; ++tt) {
-      if (tt < nt) {
-        float xv[N];
-        Chunk<T>::load(x + (size_t)(t0 + tt) * d + c, xv);
+    for (int u = 0; u < UN; ++u) {
+      const int c = c0 + u * 32 * N;
+      if (c < d) raw[u] = *reinterpret_cast<const uint4*>(wrow + c);
+    }
 #pragma unroll
-        for (int j = 0; j < N; ++j) acc[tt] = fmaf(wv[j], xv[j], acc[tt]);
+    for (int u = 0; u < UN; ++u) {
+      const int c = c0 + u * 32 * N;
+      if (c < d) {
+        float wv[N];
+        ChunkW<T>::widen(raw[u], wv);
+#pragma unroll
+        for (int tt = 0; tt < kRouterTokTile; ++tt) {
+          if (tt < nt) {
+            float xv[N];
+            Chunk<T>::load(x + (size_t)(t0 + tt) * d + c, xv);
+#pragma unroll
+            for (int j = 0; j < N; ++j) acc[tt] = fmaf(wv[j], xv[j], acc[tt]);
+          }
+        }
       }
     }
   }
@@ -49,49 +62,44 @@ __global__ void __launch_bounds__(256) router_logits_kernel(const T* __restrict_
   router_row_warp<T>(x, w_r + (size_t)e * d, bias ? bias[e] : 0.f, z, e, t0, min(kRouterTokTile, n_tokens - t0), E, d, lane);
 }
 
-// One warp, one token: `row` = that token's E logits in shared memory (destroyed).  ids (z desc, id asc) and the
-// softmax over the selected k (G7) go to ids_out[0..k) / w_out[0..k) (any address space).
-__device__ __forceinline__ void topk_softmax_warp(float* row, int E, int k, int lane, int* ids_out, float* w_out) {
-  float my_z = 0.f;  // lane i keeps the i-th selected logit
-  int my_id = 0;
-  for (int i = 0; i < k; ++i) {
-    float bz = -INFINITY;
-    int be = 0x7fffffff;
-    for (int e = lane; e < E; e += 32) {     // ascending e within a lane: first max wins -> lower id
-      float v = row[e];
-      if (v > bz) { bz = v; be = e; }
+// Top-k + softmax of n_tokens rows of logits held in shared memory (z [n_tokens][E], read only), by `nthr` threads
+// (threadIdx.x < nthr) that synchronise through named barrier `bar`.  Selection by rank counting, which IS the
+// definition (G7): rank(e) = #{j : z_j > z_e or (z_j == z_e and j < e)}; the experts of rank < k are the top-k in
+// (z desc, id asc) order.  w_i = exp(z_i - z_0) / sum_j exp(z_j - z_0), the sum taken in rank order j = 0..k-1.
+// ids_out / w_out: [n_tokens][k] (any address space); selz: [n_tokens][k] floats of shared scratch.
+__device__ __forceinline__ void topk_softmax_block(const float* z, int n_tokens, int E, int k, int* ids_out, float* w_out,
+                                                   float* selz, int nthr, int bar) {
+  const int tid = threadIdx.x;
+  for (int idx = tid; idx < n_tokens * E; idx += nthr) {
+    const int t = idx / E, e = idx % E;
+    const float* row = z + (size_t)t * E;
+    const float ze = row[e];
+    int rank = 0;
+    for (int j = 0; j < E; ++j) {          // all lanes read the same address: shared-memory broadcast
+      const float zj = row[j];
+      rank += (zj > ze) || (zj == ze && j < e);
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      float oz = __shfl_xor_sync(0xffffffffu, bz, o);
-      int oe = __shfl_xor_sync(0xffffffffu, be, o);
-      if (oz > bz || (oz == bz && oe < be)) { bz = oz; be = oe; }
-    }
-    if (lane == i) { my_z = bz; my_id = be; }
-    if (lane == 0) row[be] = -INFINITY;
-    __syncwarp();
+    if (rank < k) { ids_out[t * k + rank] = e; selz[t * k + rank] = ze; }
   }
-  const float z0 = __shfl_sync(0xffffffffu, my_z, 0);
-  const float ex = (lane < k) ? expf(my_z - z0) : 0.f;
-  float den = 0.f;
-  for (int i = 0; i < k; ++i) den += __shfl_sync(0xffffffffu, ex, i);   // fixed order
-  if (lane < k) {
-    ids_out[lane] = my_id;
-    w_out[lane] = ex / den;
+  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthr) : "memory");
+  for (int idx = tid; idx < n_tokens * k; idx += nthr) {
+    const int t = idx / k;
+    const float z0 = selz[t * k];
+    float den = 0.f;
+    for (int j = 0; j < k; ++j) den += expf(selz[t * k + j] - z0);   // fixed order
+    w_out[idx] = expf(selz[idx] - z0) / den;
   }
+  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthr) : "memory");
 }
 
-// One warp per token; block 128 = 4 tokens.  smem: 4 * E floats.
+// 4 tokens per block of 128 threads.  smem: 4 * E floats (logits) + 4 * k floats.
 __global__ void __launch_bounds__(128) topk_softmax_kernel(const float* __restrict__ z, int* __restrict__ ids,
                                                            float* __restrict__ w, int n_tokens, int E, int k) {
   extern __shared__ float sz[];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int t = blockIdx.x * 4 + warp;
-  if (t >= n_tokens) return;
-  float* row = sz + warp * E;
-  for (int e = lane; e < E; e += 32) row[e] = z[(size_t)t * E + e];
-  __syncwarp();
-  topk_softmax_warp(row, E, k, lane, ids + (size_t)t * k, w + (size_t)t * k);
+  const int t0 = blockIdx.x * 4, nt = min(4, n_tokens - t0);
+  for (int i = threadIdx.x; i < nt * E; i += 128) sz[i] = z[(size_t)t0 * E + i];
+  __syncthreads();
+  topk_softmax_block(sz, nt, E, k, ids + (size_t)t0 * k, w + (size_t)t0 * k, sz + 4 * E, 128, 0);
 }
 
 }  // namespace wisp

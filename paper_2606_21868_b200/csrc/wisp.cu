@@ -183,7 +183,7 @@ int launch_router(wisp_ctx* ctx, int layer, const void* x, int T_, cudaStream_t 
   const size_t off = (size_t)layer * cfg.max_tokens * k;
   {
     Span sp(ctx, WISP_K_TOPK, st);
-    topk_softmax_kernel<<<(T_ + 3) / 4, 128, 4 * E * sizeof(float), st>>>(ctx->logits, ctx->ids + off, ctx->topw + off,
+    topk_softmax_kernel<<<(T_ + 3) / 4, 128, 4 * (E + k) * sizeof(float), st>>>(ctx->logits, ctx->ids + off, ctx->topw + off,
                                                                           T_, E, k);
   }
   CK(cudaGetLastError());
