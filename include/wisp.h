@@ -99,7 +99,9 @@ typedef struct {
 
 /* Kernel classes of wisp_timing_read. */
 enum { WISP_K_ROUTER = 0, WISP_K_TOPK = 1, WISP_K_RESIDENCY = 2, WISP_K_FETCH = 3, WISP_K_GATE_UP = 4, WISP_K_DOWN = 5,
-       WISP_K_COMBINE = 6, WISP_K_PREFILL_GATE_UP = 7, WISP_K_PREFILL_DOWN = 8, WISP_K_OTHER = 9, WISP_N_KERNEL_CLASSES = 10 };
+       WISP_K_COMBINE = 6, WISP_K_PREFILL_GATE_UP = 7, WISP_K_PREFILL_DOWN = 8, WISP_K_OTHER = 9,
+       WISP_K_GATE_UP_MISS = 10, WISP_K_DOWN_MISS = 11,   /* decode FFN phases of layer calls that had >= 1 miss (fused path) */
+       WISP_N_KERNEL_CLASSES = 12 };
 
 /* kind: 0 hit, 1 miss, 2 resize-drop, 3 resize-move (for a move `evicted` carries the source slot).
  * Events of one wave are emitted in ascending expert id; waves in order; layers/steps in call order. */

@@ -12,7 +12,7 @@ WISP_F32, WISP_BF16 = 0, 1
 WISP_LRU, WISP_LFU = 0, 1
 WISP_FETCH_MEMCPY, WISP_FETCH_ZEROCOPY, WISP_FETCH_FUSED = 0, 1, 2
 KERNEL_CLASSES = ("router", "topk", "residency", "fetch", "gate_up", "down", "combine", "prefill_gate_up",
-                  "prefill_down", "other")
+                  "prefill_down", "other", "gate_up_miss", "down_miss")
 N_KERNEL_CLASSES = len(KERNEL_CLASSES)
 STATUS_NAMES = {0: "WISP_OK", -1: "WISP_EINVAL", -2: "WISP_ENOMEM", -3: "WISP_ECUDA", -4: "WISP_ESTATE", -5: "WISP_EBUDGET"}
 

@@ -75,9 +75,22 @@ __device__ __forceinline__ void topk_softmax_block(const float* z, int n_tokens,
     const float* row = z + (size_t)t * E;
     const float ze = row[e];
     int rank = 0;
-    for (int j = 0; j < E; ++j) {          // all lanes read the same address: shared-memory broadcast
-      const float zj = row[j];
-      rank += (zj > ze) || (zj == ze && j < e);
+    if ((E & 3) == 0 && (((size_t)row) & 15) == 0) {       // all lanes read the same address: shared-memory broadcast
+      const float4* row4 = reinterpret_cast<const float4*>(row);
+#pragma unroll 4
+      for (int j4 = 0; j4 < E / 4; ++j4) {
+        const float4 v = row4[j4];
+        const int j = j4 * 4;
+        rank += (v.x > ze) || (v.x == ze && j < e);
+        rank += (v.y > ze) || (v.y == ze && j + 1 < e);
+        rank += (v.z > ze) || (v.z == ze && j + 2 < e);
+        rank += (v.w > ze) || (v.w == ze && j + 3 < e);
+      }
+    } else {
+      for (int j = 0; j < E; ++j) {
+        const float zj = row[j];
+        rank += (zj > ze) || (zj == ze && j < e);
+      }
     }
     if (rank < k) { ids_out[t * k + rank] = e; selz[t * k + rank] = ze; }
   }

@@ -369,13 +369,19 @@ int launch_persistent_np(wisp_ctx* ctx, PersistArgs& pa, cudaStream_t st) {
     smem = (227u << 10) - fa.sharedSizeBytes;
   }
   stride = std::max(ctx->geom_gu.stage_bytes, ctx->geom_dn.stage_bytes);
-  n_stages = (int)std::min<size_t>(kStreamMaxStages, smem / stride);
+  int xs_bytes = (int)(((size_t)pa.T * pa.d * ctx->elem + 1023) & ~(size_t)1023);   // hidden state copy per CTA
+  const int rows_per_cta = (pa.E + ctx->num_sms - 1) / ctx->num_sms;               // router rows staged per CTA
+  int rw_bytes = (int)(((size_t)rows_per_cta * pa.d * ctx->elem + 1023) & ~(size_t)1023);
+  xs_bytes += 0;
+  if ((size_t)xs_bytes + rw_bytes + 2 * (size_t)stride > smem) return fail(ctx, WISP_EINVAL, "persistent decode kernel: shared memory too small");
+  n_stages = (int)std::min<size_t>(kStreamMaxStages, (smem - xs_bytes - rw_bytes) / stride);
   if (ctx->cfg.ring_stages > 0) n_stages = std::min(n_stages, (int)ctx->cfg.ring_stages);
   if (n_stages < 2) return fail(ctx, WISP_EINVAL, "persistent decode kernel: ring does not fit shared memory");
   CK(cudaMemsetAsync(ctx->gbar, 0, sizeof(unsigned), st));
   StreamGeom ggu = ctx->geom_gu, gdn = ctx->geom_dn;
-  void* args[] = {&pa, &ggu, &gdn, &n_stages, &stride};
-  CK(cudaLaunchCooperativeKernel((const void*)kern, dim3(ctx->num_sms), dim3(kStreamThreads), args, (size_t)n_stages * stride, st));
+  void* args[] = {&pa, &ggu, &gdn, &n_stages, &stride, &xs_bytes, &rw_bytes};
+  CK(cudaLaunchCooperativeKernel((const void*)kern, dim3(ctx->num_sms), dim3(kStreamThreads), args,
+                                 (size_t)xs_bytes + rw_bytes + (size_t)n_stages * stride, st));
   ++ctx->launches;
   return WISP_OK;
 }
@@ -486,6 +492,13 @@ extern "C" {
 
 const char* wisp_version(void) { return kVersion; }
 
+#ifdef WISP_PROBE_TIMELINE
+int wisp_debug_probe_read(wisp_ctx* ctx, unsigned long long* out, int n) {   // profiling probe builds only
+  cudaDeviceSynchronize();
+  return cudaMemcpy(out, ctx->phase_ns + 16, (size_t)n * sizeof(u64), cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -3;
+}
+#endif
+
 const char* wisp_last_error(wisp_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
 int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
@@ -588,8 +601,8 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   CKC(cudaMalloc(&ctx->gbar, sizeof(unsigned)));
   CKC(cudaMalloc(&ctx->dev_err, sizeof(int)));
   CKC(cudaMemset(ctx->dev_err, 0, sizeof(int)));
-  CKC(cudaMalloc(&ctx->phase_ns, kPersistPhases * sizeof(u64)));
-  CKC(cudaMemset(ctx->phase_ns, 0, kPersistPhases * sizeof(u64)));
+  CKC(cudaMalloc(&ctx->phase_ns, (16 + 8 * 256) * sizeof(u64)));   // phases, 2 counters, (probe builds) per-CTA times
+  CKC(cudaMemset(ctx->phase_ns, 0, (16 + 8 * 256) * sizeof(u64)));
   CKC(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
   CKC(cudaEventCreateWithFlags(&ctx->ev_plan, cudaEventDisableTiming));
   CKC(cudaEventCreateWithFlags(&ctx->ev_compute, cudaEventDisableTiming));
@@ -934,8 +947,20 @@ int wisp_timing_read(wisp_ctx* ctx, double* ms, uint64_t* launches, int32_t rese
     u64 ns[kPersistPhases];
     CK(cudaMemcpy(ns, ctx->phase_ns, sizeof(ns), cudaMemcpyDeviceToHost));
     CK(cudaMemset(ctx->phase_ns, 0, sizeof(ns)));
-    const int cls[kPersistPhases] = {WISP_K_ROUTER, WISP_K_RESIDENCY, WISP_K_GATE_UP, WISP_K_DOWN, WISP_K_COMBINE};
-    for (int i = 0; i < kPersistPhases; ++i) { ctx->class_ms[cls[i]] += (double)ns[i] * 1e-6; ctx->class_n[cls[i]] += ctx->persist_layers_timed; }
+    const int cls[kPersistPhases] = {WISP_K_ROUTER, WISP_K_TOPK, WISP_K_RESIDENCY, WISP_K_OTHER, WISP_K_GATE_UP, WISP_K_DOWN,
+                                     WISP_K_COMBINE, WISP_K_GATE_UP_MISS, WISP_K_DOWN_MISS};
+    u64 cnt[2];                       // [0] layer calls without a miss, [1] with
+    CK(cudaMemcpy(cnt, ctx->phase_ns + kPersistPhases, sizeof(cnt), cudaMemcpyDeviceToHost));
+    CK(cudaMemset(ctx->phase_ns + kPersistPhases, 0, sizeof(cnt)));
+    for (int i = 0; i < kPersistPhases; ++i) {
+      ctx->class_ms[cls[i]] += (double)ns[i] * 1e-6;
+#ifdef WISP_PROBE_TIMELINE
+      ctx->class_n[cls[i]] += cnt[0];
+      continue;
+#endif
+      ctx->class_n[cls[i]] += cls[i] == WISP_K_GATE_UP || cls[i] == WISP_K_DOWN ? cnt[0]
+                              : cls[i] == WISP_K_GATE_UP_MISS || cls[i] == WISP_K_DOWN_MISS ? cnt[1] : cnt[0] + cnt[1];
+    }
     ctx->persist_layers_timed = 0;
   }
   for (int i = 0; i < WISP_N_KERNEL_CLASSES; ++i) { ms[i] = ctx->class_ms[i]; launches[i] = ctx->class_n[i]; }
