@@ -1,0 +1,208 @@
+// ffn_prefill_mma.cuh -- (a4, prefill) grouped expert FFN over slot-indexed experts on the 5th-generation tensor
+// cores (tcgen05.mma, accumulators in TMEM, operands staged by TMA with the 128-byte swizzle).  bf16 only; the fp32
+// model dtype keeps the plain tiled kernel of ffn_prefill.cuh.  The paper runs the engine's unmodified fused-MoE
+// kernel here; this is the part of the path that really is a dense contraction.
+//
+// Per wave entry (expert e resident in slot s, n_e routed (token, rank) pairs, sorted positions pos0..pos0+n_e-1):
+//   GEMM 1 (MODE 0):  Hg = G_s Xe^T, Hu = U_s Xe^T     [128 weight rows x NT tokens] per CTA, K = d_model
+//                     act[pos, r] = silu(Hg[r, pos]) * Hu[r, pos]   (bf16, sorted-pair order, G21)
+//   GEMM 2 (MODE 1):  Y = D_s act_e^T                   [128 rows x NT tokens], K = d_ff  -> ystage[pair, r] fp32
+// "Swap AB": the weight rows are the MMA M dimension (always 128 full rows), the ragged token count is N.
+// Operands are K-major; A tiles come straight from the slot through a 3-D tensor map over the arena
+// (K, row, blob index = slot*L + layer), B tiles from the gathered token rows xg / the act buffer.
+// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer, warps 2..5 = epilogue.
+// Determinism (parity (b)): a column (token) of the accumulator depends only on that token's row and the weight
+// tile, the K order is fixed, and nothing depends on the slot, the wave or the other tokens of the tile.
+#pragma once
+#include <cuda.h>
+
+#include "common.cuh"
+#include "ffn_stream.cuh"
+
+namespace wisp {
+
+constexpr int kMmaThreads = 192;
+constexpr int kMmaM = 128;        // weight rows per CTA tile (UMMA_M)
+constexpr int kMmaNT = 128;       // tokens per CTA tile (UMMA_N <= 128)
+constexpr int kMmaBK = 64;        // K elements per stage = one 128-byte swizzle atom of bf16
+constexpr int kMmaTileBytes = kMmaM * kMmaBK * 2;   // 16 KiB: [128 rows][128 B]
+
+struct MmaArgs {
+  PlanPtrs plan;
+  int wave, C, L, layer;
+  int d, dff, k;
+  __nv_bfloat16* act;     // [n_pairs][dff] bf16, SORTED pair order (position = exp_offset[e] + j)
+  float* ystage;          // [n_pairs][d] fp32, indexed by pair id (t*k + rank)
+};
+
+// ---- PTX wrappers -----------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(tm), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+               ::"r"(dst), "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t cols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(cols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// D[tmem] (+)= A[smem desc] * B[smem desc]^T, bf16 inputs, fp32 accumulate, issued by one thread
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
+      ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
+}
+// mbarrier arrive once every tcgen05.mma issued so far by this thread has completed
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// 16 consecutive fp32 columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
+  uint32_t r[16];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                 "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+               : "r"(taddr) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// Shared-memory matrix descriptor of a K-major tile [rows][64 bf16] written by TMA with the 128-byte swizzle:
+// 8-row groups are 1024 B apart (SBO), descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+  uint64_t desc = 0;
+  desc |= (uint64_t)((smem_addr >> 4) & 0x3fffu);            // start address, 16-byte units
+  desc |= (uint64_t)1 << 16;                                 // leading byte offset (unused for swizzled K-major)
+  desc |= (uint64_t)(1024u >> 4) << 32;                      // stride byte offset
+  desc |= (uint64_t)1 << 46;                                 // version
+  desc |= (uint64_t)2 << 61;                                 // SWIZZLE_128B
+  return desc;
+}
+// Instruction descriptor: D fp32, A and B bf16, both K-major, M x N tile.
+__device__ __forceinline__ uint32_t umma_idesc_bf16(int M, int N) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+// grid: x = 128-row tiles of the weight matrix, y = token tiles of kMmaNT, z = wave entry (<= C).
+// tm_w: 3-D map over the arena (K, weight row, blob); tm_x: 2-D map over the B rows (K, sorted pair position).
+template <int MODE>
+__global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __grid_constant__ CUtensorMap tm_w,
+                                                                     const __grid_constant__ CUtensorMap tm_x,
+                                                                     const MmaArgs a, const int n_stages) {
+  extern __shared__ __align__(1024) unsigned char smem_mma[];
+  __shared__ __align__(8) unsigned long long s_full[8], s_empty[8], s_tfull;
+  __shared__ uint32_t s_tmem;
+  constexpr int NA = MODE == 0 ? 2 : 1;                       // weight tiles per stage (gate + up | down)
+  constexpr uint32_t kStage = (NA + 1) * kMmaTileBytes;
+  constexpr uint32_t kCols = MODE == 0 ? 256 : 128;           // TMEM columns: one fp32 accumulator of <= 128 tokens per matrix
+
+  if (a.wave >= a.plan.hdr[0]) return;
+  const int lo = a.wave * a.C, nw = min(a.plan.hdr[1], lo + a.C) - lo;
+  if ((int)blockIdx.z >= nw) return;
+  const int i = lo + blockIdx.z;
+  const int e = a.plan.entry_expert[i];
+  const int cnt = a.plan.exp_count[e];
+  const int p0 = blockIdx.y * kMmaNT;
+  if (p0 >= cnt) return;
+  const int pos0 = a.plan.exp_offset[e] + p0;
+  const int nt = min(kMmaNT, cnt - p0);
+  const int N = max(16, (nt + 15) & ~15);
+  const int r0 = blockIdx.x * kMmaM;
+  const int blob = a.plan.entry_slot[i] * a.L + a.layer;
+  const int K = MODE == 0 ? a.d : a.dff;
+  const int nkb = K / kMmaBK;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t smem0 = (smem_u32(smem_mma) + 1023u) & ~1023u;   // swizzle-128B tiles need 1024-byte alignment
+  if (tid == 0) {
+    for (int s = 0; s < n_stages; ++s) { mbar_init(smem_u32(&s_full[s]), 1); mbar_init(smem_u32(&s_empty[s]), 1); }
+    mbar_init(smem_u32(&s_tfull), 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) tmem_alloc(smem_u32(&s_tmem), kCols);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = s_tmem;
+
+  if (warp == 0) {
+    if (lane == 0) {      // ===== TMA producer =====
+      int s = 0; uint32_t ph = 0;
+      for (int kb = 0; kb < nkb; ++kb) {
+        mbar_wait(smem_u32(&s_empty[s]), ph ^ 1u);
+        const uint32_t bar = smem_u32(&s_full[s]);
+        mbar_expect_tx(bar, kStage);
+        const uint32_t base = smem0 + s * kStage;
+        tma_load_3d(base, &tm_w, kb * kMmaBK, r0, blob, bar);
+        if (MODE == 0) tma_load_3d(base + kMmaTileBytes, &tm_w, kb * kMmaBK, a.dff + r0, blob, bar);
+        tma_load_2d(base + NA * kMmaTileBytes, &tm_x, kb * kMmaBK, pos0, bar);
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {      // ===== MMA issuer =====
+      const uint32_t idesc = umma_idesc_bf16(kMmaM, N);
+      int s = 0; uint32_t ph = 0;
+      for (int kb = 0; kb < nkb; ++kb) {
+        mbar_wait(smem_u32(&s_full[s]), ph);
+        tc_fence_after();
+        const uint32_t base = smem0 + s * kStage;
+        const uint64_t da0 = umma_desc_sw128(base), da1 = umma_desc_sw128(base + kMmaTileBytes);
+        const uint64_t db = umma_desc_sw128(base + NA * kMmaTileBytes);
+#pragma unroll
+        for (int k4 = 0; k4 < kMmaBK / 16; ++k4) {            // UMMA_K = 16 bf16 = 32 bytes = 2 sixteen-byte units
+          const uint32_t acc = (kb | k4) != 0;
+          umma_bf16(tmem, da0 + 2 * k4, db + 2 * k4, idesc, acc);
+          if (MODE == 0) umma_bf16(tmem + 128, da1 + 2 * k4, db + 2 * k4, idesc, acc);
+        }
+        umma_commit(smem_u32(&s_empty[s]));                   // frees the stage once these MMAs have read it
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
+      }
+      umma_commit(smem_u32(&s_tfull));                        // accumulators complete
+    }
+  } else {                // ===== epilogue warps: TMEM lane quarter = warp % 4 =====
+    mbar_wait(smem_u32(&s_tfull), 0u);
+    tc_fence_after();
+    const int q = warp & 3;
+    const int row = r0 + 32 * q + lane;                       // weight row = d_ff index (MODE 0) | d index (MODE 1)
+    const uint32_t tlane = tmem + ((uint32_t)(32 * q) << 16);
+    const int* pl = a.plan.pair_list + a.plan.exp_offset[e] + p0;
+    for (int c0 = 0; c0 < N; c0 += 16) {
+      float g[16], u[16];
+      tmem_ld16(tlane + c0, g);
+      if (MODE == 0) tmem_ld16(tlane + 128 + c0, u);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const int col = c0 + j;
+        if (col < nt) {
+          if (MODE == 0) a.act[(size_t)(pos0 + col) * a.dff + row] = __float2bfloat16_rn(silu_f(g[j]) * u[j]);
+          else a.ystage[(size_t)pl[col] * a.d + row] = g[j];
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem, kCols);
+}
+
+// xg[pos][:] = x[pair_list[pos] / k][:] for every routed pair (sorted by expert): the B operand of GEMM 1.
+__global__ void __launch_bounds__(256) gather_tokens_kernel(const int* __restrict__ pair_list, int n_pairs, int k, int d_vec,
+                                                            const uint4* __restrict__ x, uint4* __restrict__ xg) {
+  for (int pos = blockIdx.x; pos < n_pairs; pos += gridDim.x) {
+    const uint4* src = x + (size_t)(pair_list[pos] / k) * d_vec;
+    uint4* dst = xg + (size_t)pos * d_vec;
+    for (int c = threadIdx.x; c < d_vec; c += blockDim.x) dst[c] = src[c];
+  }
+}
+
+}  // namespace wisp

@@ -13,6 +13,7 @@
 #include "decode_persistent.cuh"
 #include "fetch.cuh"
 #include "ffn_prefill.cuh"
+#include "ffn_prefill_mma.cuh"
 #include "ffn_stream.cuh"
 #include "mvwsa.h"
 #include "residency.cuh"
@@ -85,6 +86,10 @@ struct wisp_ctx {
   int* dev_err = nullptr;            // device error flag (grid barrier timeout)
   u64* phase_ns = nullptr;           // device [kPersistPhases]
   int persist_enabled = 1;
+  // tcgen05 prefill path (ffn_prefill_mma.cuh): TMA tensor maps over the arena / the B-operand buffers
+  bool mma_ok = false;
+  CUtensorMap tm_gu{}, tm_dn{}, tm_xg{}, tm_act{};
+  char* xg = nullptr;                // [maxT*k][d] gathered token rows (bf16)
   u64 persist_layers_timed = 0;
   bool use_persistent(int T_) const {
     return persist_enabled && cfg.fetch == WISP_FETCH_FUSED && T_ <= kDecodeMaxTokens && cfg.n_experts <= kPersistMaxExperts;
@@ -336,6 +341,22 @@ int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, c
       rc = launch_stream_np<T, 1>(ctx, a, ctx->geom_dn, T_, st);
     }
     if (rc) return rc;
+  } else if (ctx->mma_ok) {
+    // tcgen05 grouped GEMM (bf16): xg was gathered once per forward (forward_layer); 4 / 6 ring stages of 48 / 32 KiB
+    MmaArgs m{};
+    m.plan = ctx->plan; m.wave = wave; m.C = ctx->C; m.L = L; m.layer = layer; m.d = d; m.dff = dff; m.k = k;
+    m.act = reinterpret_cast<__nv_bfloat16*>(ctx->act_T); m.ystage = ctx->ystage;
+    const int ttiles = (T_ + kMmaNT - 1) / kMmaNT;
+    {
+      Span sp(ctx, WISP_K_PREFILL_GATE_UP, st);
+      const int ns = 4;
+      prefill_mma_kernel<0><<<dim3(dff / kMmaM, ttiles, ctx->C), kMmaThreads, ns * 3 * kMmaTileBytes + 1024, st>>>(ctx->tm_gu, ctx->tm_xg, m, ns);
+    }
+    {
+      Span sp(ctx, WISP_K_PREFILL_DOWN, st);
+      const int ns = 6;
+      prefill_mma_kernel<1><<<dim3(d / kMmaM, ttiles, ctx->C), kMmaThreads, ns * 2 * kMmaTileBytes + 1024, st>>>(ctx->tm_dn, ctx->tm_act, m, ns);
+    }
   } else {
     const int ptiles = (T_ + kPfTile - 1) / kPfTile;   // an expert can receive at most T pairs
     dim3 g0(dff / kPfTile, ptiles, ctx->C), g1(d / kPfTile, ptiles, ctx->C);
@@ -354,6 +375,55 @@ int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, c
   }
   CK(cudaGetLastError());
   return WISP_OK;
+}
+
+// ---- tcgen05 prefill path: tensor maps -----------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+bool make_tmap(EncodeTiledFn fn, CUtensorMap* tm, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides_bytes,
+               const cuuint32_t* box) {
+  cuuint32_t estr[3] = {1, 1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, base, dims, strides_bytes, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// K-major bf16 operands in boxes of [64 K-elements][128 rows]: weights through a 3-D view of the arena
+// (K, weight row, blob = slot*L + layer), tokens / activations through 2-D views of xg and act.
+bool setup_mma_path(wisp_ctx* ctx) {
+  const auto& cfg = ctx->cfg;
+  if (cfg.dtype != WISP_BF16 || cfg.max_tokens <= kDecodeMaxTokens) return false;
+  void* sym = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess || !sym) return false;
+  EncodeTiledFn fn = reinterpret_cast<EncodeTiledFn>(sym);
+  const cuuint64_t d = cfg.d_model, dff = cfg.d_ff, n_blobs = ctx->budget / ctx->Me, rows = (cuuint64_t)cfg.max_tokens * cfg.top_k;
+  if (n_blobs < 1) return false;
+  const cuuint32_t box3[3] = {kMmaBK, kMmaM, 1}, box2[2] = {kMmaBK, kMmaNT};
+  {
+    const cuuint64_t dims[3] = {d, 2 * dff, n_blobs}, str[2] = {d * 2, ctx->Me};
+    if (!make_tmap(fn, &ctx->tm_gu, ctx->arena, 3, dims, str, box3)) return false;
+  }
+  {
+    const cuuint64_t dims[3] = {dff, d, n_blobs}, str[2] = {dff * 2, ctx->Me};
+    if (!make_tmap(fn, &ctx->tm_dn, ctx->arena + 2 * d * dff * 2, 3, dims, str, box3)) return false;
+  }
+  if (cudaMalloc(&ctx->xg, rows * d * 2) != cudaSuccess) return false;
+  {
+    const cuuint64_t dims[2] = {d, rows}, str[1] = {d * 2};
+    if (!make_tmap(fn, &ctx->tm_xg, ctx->xg, 2, dims, str, box2)) return false;
+  }
+  {
+    const cuuint64_t dims[2] = {dff, rows}, str[1] = {dff * 2};
+    if (!make_tmap(fn, &ctx->tm_act, ctx->act_T, 2, dims, str, box2)) return false;
+  }
+  for (int mode = 0; mode < 2; ++mode) {
+    const void* k = mode == 0 ? (const void*)prefill_mma_kernel<0> : (const void*)prefill_mma_kernel<1>;
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) return false;
+  }
+  return true;
 }
 
 // ---- persistent decode kernel: layers [lo, hi) of one token batch in one cooperative launch ----------------------
@@ -440,6 +510,11 @@ int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, vo
     n_waves = ctx->host_plan->n_waves;
   } else {
     n_waves = (std::min(E, n_pairs) + ctx->C - 1) / ctx->C;   // worst case; empty waves exit at once
+  }
+  if (T_ > kDecodeMaxTokens && ctx->mma_ok) {      // B operand of GEMM 1: token rows in sorted-pair order
+    Span sp(ctx, WISP_K_OTHER, st);
+    gather_tokens_kernel<<<std::min(n_pairs, 4 * ctx->num_sms), 256, 0, st>>>(ctx->plan.pair_list, n_pairs, k, cfg.d_model * 2 / 16,
+                                                                             reinterpret_cast<const uint4*>(x), reinterpret_cast<uint4*>(ctx->xg));
   }
   const bool fused_fill = cfg.fetch == WISP_FETCH_FUSED && T_ <= kDecodeMaxTokens;   // the FFN kernels fetch their own misses
   for (int w = 0; w < n_waves; ++w) {
@@ -614,6 +689,12 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
     ctx->geom_dn = make_geom(dff, d, 1, ctx->elem, 2 * gu, 0, cfg->ring_stages);
   }
   ctx->grid_fetch = ctx->num_sms * 2;
+  ctx->mma_ok = setup_mma_path(ctx);
+  if (cfg->dtype == WISP_BF16 && cfg->max_tokens > kDecodeMaxTokens && !ctx->mma_ok) {
+    std::fprintf(stderr, "wisp_create: tcgen05 prefill path unavailable (tensor map setup failed)\n");
+    wisp_destroy(ctx);
+    return WISP_ECUDA;
+  }
   *out = ctx;
   return WISP_OK;
 }
@@ -628,7 +709,7 @@ int wisp_destroy(wisp_ctx* ctx) {
                       ctx->freq,     ctx->scal,     ctx->last_pos,    ctx->hist,    ctx->logits,  ctx->ids,
                       ctx->topw,     ctx->plan_mem, ctx->act_f32,     ctx->act_T,   ctx->ystage,  ctx->xbuf[0],
                       ctx->xbuf[1],  ctx->ybuf,     ctx->dbg_ids,     ctx->moves,   ctx->bad_slots, ctx->trace,
-                      ctx->trace_ctr, ctx->d_masters, ctx->gbar, ctx->dev_err, ctx->phase_ns};
+                      ctx->trace_ctr, ctx->d_masters, ctx->gbar, ctx->dev_err, ctx->phase_ns, ctx->xg};
   for (void* p : dev_ptrs)
     if (p) cudaFree(p);
   if (ctx->host_plan) cudaFreeHost(ctx->host_plan);
