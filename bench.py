@@ -47,6 +47,7 @@ def parse():
                     help="miss path: fused = persistent decode kernel whose TMA producer reads misses from the mapped master")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-miss-path", action="store_true")
+    ap.add_argument("--no-prefill", action="store_true")
     ap.add_argument("--per-layer-api", action="store_true", help="drive wisp_moe_forward per layer instead of wisp_stack_forward")
     return ap.parse_args()
 
@@ -228,6 +229,51 @@ def miss_path_microbench(shape, args):
     out["frac_of_link_peak"] = round((out[best_path + "_gbs"] or 0) / best, 4)
     if out.get("fused_gbs"):
         out["fused_frac_of_link_peak"] = round(out["fused_gbs"] / best, 4)
+    return out
+
+
+def prefill_bench(shape, args, n_layers=8, T=2048):
+    """m4: prefill of T i.i.d. N(0,1) tokens (BASELINE.json config 3) through n_layers layers, all experts resident, so
+    the grouped GEMM (tcgen05) is what is timed; plus one cold pass that also pays the demand fetch of every expert."""
+    sh = shape.with_layers(n_layers)
+    ctx, staging = build_context(sh, shape.n_experts * sh.slot_unit_bytes, args, T, fetch="zerocopy")
+    del staging
+    x = si.gen_prefill_hidden(sh, T).to(sh.torch_dtype).cuda()
+    y = torch.empty_like(x)
+    stream = torch.cuda.Stream()
+    out = {"tokens": T, "layers": n_layers, "pool": "all-resident"}
+    with torch.cuda.stream(stream):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ev[0].record(stream); ctx.stack_forward(x, y, stream.cuda_stream); ev[1].record(stream); stream.synchronize()
+        cold_ms = ev[0].elapsed_time(ev[1])
+        st0 = ctx.stats()
+        ctx.stack_forward(x, y, stream.cuda_stream); stream.synchronize()          # warm-up
+        reps = 5
+        ev[0].record(stream)
+        for _ in range(reps):
+            ctx.stack_forward(x, y, stream.cuda_stream)
+        ev[1].record(stream); stream.synchronize()
+        ms = ev[0].elapsed_time(ev[1]) / reps
+        ctx.timing_enable(2); ctx.timing_read(reset=True)
+        ctx.stack_forward(x, y, stream.cuda_stream); stream.synchronize()
+        kt = ctx.timing_read(); ctx.timing_enable(0)
+    flops = T * sh.top_k * 6.0 * sh.d_model * sh.d_ff * n_layers
+    out["ms_per_pass"] = round(ms, 3)
+    out["tokens_per_s_scaled_to_full_stack"] = round(T / (ms * 1e-3) * n_layers / shape.n_layers, 1)
+    out["tflops"] = round(flops / (ms * 1e-3) / 1e12, 1)
+    gemm_ms = sum(kt[k][0] for k in ("prefill_gate_up", "prefill_down"))
+    out["gemm_kernels_tflops"] = round(flops / (gemm_ms * 1e-3) / 1e12, 1) if gemm_ms > 0 else None
+    out["kernels_ms"] = {k: round(v[0], 3) for k, v in kt.items() if v[1]}
+    miss_bytes = st0.total.misses * sh.expert_bytes
+    out["cold_pass"] = {"ms": round(cold_ms, 2), "miss_gib": round(miss_bytes / GIB, 2), "host_link_gbs": round(miss_bytes / (cold_ms * 1e-3) / 1e9, 1)}
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            pk = json.load(fh)
+        out["tensor_peak_tflops"] = pk.get("bf16_tflops_sustained")
+        if out["gemm_kernels_tflops"] and out["tensor_peak_tflops"]:
+            out["gemm_frac_of_tensor_peak"] = round(out["gemm_kernels_tflops"] / out["tensor_peak_tflops"], 4)
+    ctx.close()
     return out
 
 
@@ -466,6 +512,11 @@ def main_ours(args):
                 roof["frac_of_step_lower_bound"] = round(roof["step_lower_bound_us"] / roof["avg_launch_us"], 4)
         except Exception as ex:                        # the microbenchmark must never take the headline down
             line["miss_path"] = {"error": repr(ex)[:200]}
+    if rank == 0 and world == 1 and not args.no_prefill and shape.dtype == "bf16":
+        try:
+            line["prefill"] = prefill_bench(shape, args)
+        except Exception as ex:
+            line["prefill"] = {"error": repr(ex)[:300]}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         nl = min(shape.n_layers, 4 if shape.expert_bytes * shape.n_experts > (256 << 20) else shape.n_layers)
         reps = 2 if nl < shape.n_layers else 8

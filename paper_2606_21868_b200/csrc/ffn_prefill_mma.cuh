@@ -92,40 +92,49 @@ __device__ __forceinline__ uint32_t umma_idesc_bf16(int M, int N) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
-// grid: x = 128-row tiles of the weight matrix, y = token tiles of kMmaNT, z = wave entry (<= C).
+// Work list of one wave: one item per (wave entry, tile of kMmaNT routed pairs).  work[2*w] = plan entry index,
+// work[2*w+1] = first pair of the tile inside the expert's sorted range; *n_work = item count.  One warp.
+__global__ void __launch_bounds__(32) build_work_kernel(PlanPtrs plan, int wave, int C, int* __restrict__ work, int* __restrict__ n_work) {
+  if (threadIdx.x != 0) return;
+  int n = 0;
+  if (wave < plan.hdr[0]) {
+    const int lo = wave * C, hi = min(plan.hdr[1], lo + C);
+    for (int i = lo; i < hi; ++i) {
+      const int cnt = plan.exp_count[plan.entry_expert[i]];
+      for (int p0 = 0; p0 < cnt; p0 += kMmaNT) { work[2 * n] = i; work[2 * n + 1] = p0; ++n; }
+    }
+  }
+  *n_work = n;
+}
+
+// Persistent: one CTA per SM walks the tiles t = blockIdx.x, blockIdx.x + gridDim.x, ...; tile t = (work item t / RT,
+// 128-row tile t % RT) with RT = weight rows / 128.  Two TMEM accumulator stages: the epilogue of tile j drains
+// stage j & 1 while the MMA warp already fills the other stage with tile j + 1.
 // tm_w: 3-D map over the arena (K, weight row, blob); tm_x: 2-D map over the B rows (K, sorted pair position).
 template <int MODE>
 __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __grid_constant__ CUtensorMap tm_w,
                                                                      const __grid_constant__ CUtensorMap tm_x,
-                                                                     const MmaArgs a, const int n_stages) {
+                                                                     const MmaArgs a, const int* __restrict__ work,
+                                                                     const int* __restrict__ n_work_p, const int n_stages) {
   extern __shared__ __align__(1024) unsigned char smem_mma[];
-  __shared__ __align__(8) unsigned long long s_full[8], s_empty[8], s_tfull;
+  __shared__ __align__(8) unsigned long long s_full[8], s_empty[8], s_tfull[2], s_tempty[2];
   __shared__ uint32_t s_tmem;
   constexpr int NA = MODE == 0 ? 2 : 1;                       // weight tiles per stage (gate + up | down)
   constexpr uint32_t kStage = (NA + 1) * kMmaTileBytes;
-  constexpr uint32_t kCols = MODE == 0 ? 256 : 128;           // TMEM columns: one fp32 accumulator of <= 128 tokens per matrix
+  constexpr uint32_t kAccCols = MODE == 0 ? 256 : 128;        // TMEM columns of one accumulator stage
+  constexpr uint32_t kCols = 2 * kAccCols;
 
-  if (a.wave >= a.plan.hdr[0]) return;
-  const int lo = a.wave * a.C, nw = min(a.plan.hdr[1], lo + a.C) - lo;
-  if ((int)blockIdx.z >= nw) return;
-  const int i = lo + blockIdx.z;
-  const int e = a.plan.entry_expert[i];
-  const int cnt = a.plan.exp_count[e];
-  const int p0 = blockIdx.y * kMmaNT;
-  if (p0 >= cnt) return;
-  const int pos0 = a.plan.exp_offset[e] + p0;
-  const int nt = min(kMmaNT, cnt - p0);
-  const int N = max(16, (nt + 15) & ~15);
-  const int r0 = blockIdx.x * kMmaM;
-  const int blob = a.plan.entry_slot[i] * a.L + a.layer;
   const int K = MODE == 0 ? a.d : a.dff;
   const int nkb = K / kMmaBK;
+  const int RT = (MODE == 0 ? a.dff : a.d) / kMmaM;
+  const int n_tiles = *n_work_p * RT;
+  if ((int)blockIdx.x >= n_tiles) return;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t smem0 = (smem_u32(smem_mma) + 1023u) & ~1023u;   // swizzle-128B tiles need 1024-byte alignment
   if (tid == 0) {
     for (int s = 0; s < n_stages; ++s) { mbar_init(smem_u32(&s_full[s]), 1); mbar_init(smem_u32(&s_empty[s]), 1); }
-    mbar_init(smem_u32(&s_tfull), 1);
+    for (int s = 0; s < 2; ++s) { mbar_init(smem_u32(&s_tfull[s]), 1); mbar_init(smem_u32(&s_tempty[s]), 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) tmem_alloc(smem_u32(&s_tmem), kCols);
@@ -137,57 +146,86 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
   if (warp == 0) {
     if (lane == 0) {      // ===== TMA producer =====
       int s = 0; uint32_t ph = 0;
-      for (int kb = 0; kb < nkb; ++kb) {
-        mbar_wait(smem_u32(&s_empty[s]), ph ^ 1u);
-        const uint32_t bar = smem_u32(&s_full[s]);
-        mbar_expect_tx(bar, kStage);
-        const uint32_t base = smem0 + s * kStage;
-        tma_load_3d(base, &tm_w, kb * kMmaBK, r0, blob, bar);
-        if (MODE == 0) tma_load_3d(base + kMmaTileBytes, &tm_w, kb * kMmaBK, a.dff + r0, blob, bar);
-        tma_load_2d(base + NA * kMmaTileBytes, &tm_x, kb * kMmaBK, pos0, bar);
-        if (++s == n_stages) { s = 0; ph ^= 1u; }
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        const int w = t / RT, r0 = (t % RT) * kMmaM;
+        const int i = work[2 * w], p0 = work[2 * w + 1];
+        const int pos0 = a.plan.exp_offset[a.plan.entry_expert[i]] + p0;
+        const int blob = a.plan.entry_slot[i] * a.L + a.layer;
+        for (int kb = 0; kb < nkb; ++kb) {
+          mbar_wait(smem_u32(&s_empty[s]), ph ^ 1u);
+          const uint32_t bar = smem_u32(&s_full[s]);
+          mbar_expect_tx(bar, kStage);
+          const uint32_t base = smem0 + s * kStage;
+          tma_load_3d(base, &tm_w, kb * kMmaBK, r0, blob, bar);
+          if (MODE == 0) tma_load_3d(base + kMmaTileBytes, &tm_w, kb * kMmaBK, a.dff + r0, blob, bar);
+          tma_load_2d(base + NA * kMmaTileBytes, &tm_x, kb * kMmaBK, pos0, bar);
+          if (++s == n_stages) { s = 0; ph ^= 1u; }
+        }
       }
     }
   } else if (warp == 1) {
     if (lane == 0) {      // ===== MMA issuer =====
-      const uint32_t idesc = umma_idesc_bf16(kMmaM, N);
       int s = 0; uint32_t ph = 0;
-      for (int kb = 0; kb < nkb; ++kb) {
-        mbar_wait(smem_u32(&s_full[s]), ph);
+      int j = 0;
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++j) {
+        const int w = t / RT;
+        const int i = work[2 * w], p0 = work[2 * w + 1];
+        const int nt = min(kMmaNT, a.plan.exp_count[a.plan.entry_expert[i]] - p0);
+        const uint32_t idesc = umma_idesc_bf16(kMmaM, max(16, (nt + 15) & ~15));
+        const int as = j & 1;
+        mbar_wait(smem_u32(&s_tempty[as]), ((uint32_t)(j >> 1) & 1u) ^ 1u);   // the epilogue has drained this stage
         tc_fence_after();
-        const uint32_t base = smem0 + s * kStage;
-        const uint64_t da0 = umma_desc_sw128(base), da1 = umma_desc_sw128(base + kMmaTileBytes);
-        const uint64_t db = umma_desc_sw128(base + NA * kMmaTileBytes);
+        const uint32_t acc_base = tmem + as * kAccCols;
+        for (int kb = 0; kb < nkb; ++kb) {
+          mbar_wait(smem_u32(&s_full[s]), ph);
+          tc_fence_after();
+          const uint32_t base = smem0 + s * kStage;
+          const uint64_t da0 = umma_desc_sw128(base), da1 = umma_desc_sw128(base + kMmaTileBytes);
+          const uint64_t db = umma_desc_sw128(base + NA * kMmaTileBytes);
 #pragma unroll
-        for (int k4 = 0; k4 < kMmaBK / 16; ++k4) {            // UMMA_K = 16 bf16 = 32 bytes = 2 sixteen-byte units
-          const uint32_t acc = (kb | k4) != 0;
-          umma_bf16(tmem, da0 + 2 * k4, db + 2 * k4, idesc, acc);
-          if (MODE == 0) umma_bf16(tmem + 128, da1 + 2 * k4, db + 2 * k4, idesc, acc);
+          for (int k4 = 0; k4 < kMmaBK / 16; ++k4) {          // UMMA_K = 16 bf16 = 32 bytes = 2 sixteen-byte units
+            const uint32_t acc = (kb | k4) != 0;
+            umma_bf16(acc_base, da0 + 2 * k4, db + 2 * k4, idesc, acc);
+            if (MODE == 0) umma_bf16(acc_base + 128, da1 + 2 * k4, db + 2 * k4, idesc, acc);
+          }
+          umma_commit(smem_u32(&s_empty[s]));                 // frees the stage once these MMAs have read it
+          if (++s == n_stages) { s = 0; ph ^= 1u; }
         }
-        umma_commit(smem_u32(&s_empty[s]));                   // frees the stage once these MMAs have read it
-        if (++s == n_stages) { s = 0; ph ^= 1u; }
+        umma_commit(smem_u32(&s_tfull[as]));                  // accumulators of this tile complete
       }
-      umma_commit(smem_u32(&s_tfull));                        // accumulators complete
     }
   } else {                // ===== epilogue warps: TMEM lane quarter = warp % 4 =====
-    mbar_wait(smem_u32(&s_tfull), 0u);
-    tc_fence_after();
     const int q = warp & 3;
-    const int row = r0 + 32 * q + lane;                       // weight row = d_ff index (MODE 0) | d index (MODE 1)
-    const uint32_t tlane = tmem + ((uint32_t)(32 * q) << 16);
-    const int* pl = a.plan.pair_list + a.plan.exp_offset[e] + p0;
-    for (int c0 = 0; c0 < N; c0 += 16) {
-      float g[16], u[16];
-      tmem_ld16(tlane + c0, g);
-      if (MODE == 0) tmem_ld16(tlane + 128 + c0, u);
+    int j = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++j) {
+      const int w = t / RT, r0 = (t % RT) * kMmaM;
+      const int i = work[2 * w], p0 = work[2 * w + 1];
+      const int e = a.plan.entry_expert[i];
+      const int pos0 = a.plan.exp_offset[e] + p0;
+      const int nt = min(kMmaNT, a.plan.exp_count[e] - p0);
+      const int N = max(16, (nt + 15) & ~15);
+      const int as = j & 1;
+      mbar_wait(smem_u32(&s_tfull[as]), (uint32_t)(j >> 1) & 1u);
+      tc_fence_after();
+      const int row = r0 + 32 * q + lane;                     // weight row = d_ff index (MODE 0) | d index (MODE 1)
+      const uint32_t tlane = tmem + as * kAccCols + ((uint32_t)(32 * q) << 16);
+      const int* pl = a.plan.pair_list + pos0;
+      for (int c0 = 0; c0 < N; c0 += 16) {
+        float g[16], u[16];
+        tmem_ld16(tlane + c0, g);
+        if (MODE == 0) tmem_ld16(tlane + 128 + c0, u);
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const int col = c0 + j;
-        if (col < nt) {
-          if (MODE == 0) a.act[(size_t)(pos0 + col) * a.dff + row] = __float2bfloat16_rn(silu_f(g[j]) * u[j]);
-          else a.ystage[(size_t)pl[col] * a.d + row] = g[j];
+        for (int jj = 0; jj < 16; ++jj) {
+          const int col = c0 + jj;
+          if (col < nt) {
+            if (MODE == 0) a.act[(size_t)(pos0 + col) * a.dff + row] = __float2bfloat16_rn(silu_f(g[jj]) * u[jj]);
+            else a.ystage[(size_t)pl[col] * a.d + row] = g[jj];
+          }
         }
       }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&s_tempty[as]));    // this warp's quarter of the stage is drained
     }
   }
   tc_fence_before();

@@ -90,6 +90,7 @@ struct wisp_ctx {
   bool mma_ok = false;
   CUtensorMap tm_gu{}, tm_dn{}, tm_xg{}, tm_act{};
   char* xg = nullptr;                // [maxT*k][d] gathered token rows (bf16)
+  int* mma_work = nullptr;           // work list of the current wave: (entry, first pair) items + count
   u64 persist_layers_timed = 0;
   bool use_persistent(int T_) const {
     return persist_enabled && cfg.fetch == WISP_FETCH_FUSED && T_ <= kDecodeMaxTokens && cfg.n_experts <= kPersistMaxExperts;
@@ -346,16 +347,20 @@ int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, c
     MmaArgs m{};
     m.plan = ctx->plan; m.wave = wave; m.C = ctx->C; m.L = L; m.layer = layer; m.d = d; m.dff = dff; m.k = k;
     m.act = reinterpret_cast<__nv_bfloat16*>(ctx->act_T); m.ystage = ctx->ystage;
-    const int ttiles = (T_ + kMmaNT - 1) / kMmaNT;
+    {
+      Span sp(ctx, WISP_K_OTHER, st);
+      build_work_kernel<<<1, 32, 0, st>>>(ctx->plan, wave, ctx->C, ctx->mma_work, ctx->mma_work + 2 * (cfg.n_experts + cfg.max_tokens * k / kMmaNT + 1));
+    }
+    const int* n_work = ctx->mma_work + 2 * (cfg.n_experts + cfg.max_tokens * k / kMmaNT + 1);
     {
       Span sp(ctx, WISP_K_PREFILL_GATE_UP, st);
       const int ns = 4;
-      prefill_mma_kernel<0><<<dim3(dff / kMmaM, ttiles, ctx->C), kMmaThreads, ns * 3 * kMmaTileBytes + 1024, st>>>(ctx->tm_gu, ctx->tm_xg, m, ns);
+      prefill_mma_kernel<0><<<ctx->num_sms, kMmaThreads, ns * 3 * kMmaTileBytes + 1024, st>>>(ctx->tm_gu, ctx->tm_xg, m, ctx->mma_work, n_work, ns);
     }
     {
       Span sp(ctx, WISP_K_PREFILL_DOWN, st);
       const int ns = 6;
-      prefill_mma_kernel<1><<<dim3(d / kMmaM, ttiles, ctx->C), kMmaThreads, ns * 2 * kMmaTileBytes + 1024, st>>>(ctx->tm_dn, ctx->tm_act, m, ns);
+      prefill_mma_kernel<1><<<ctx->num_sms, kMmaThreads, ns * 2 * kMmaTileBytes + 1024, st>>>(ctx->tm_dn, ctx->tm_act, m, ctx->mma_work, n_work, ns);
     }
   } else {
     const int ptiles = (T_ + kPfTile - 1) / kPfTile;   // an expert can receive at most T pairs
@@ -411,6 +416,7 @@ bool setup_mma_path(wisp_ctx* ctx) {
     if (!make_tmap(fn, &ctx->tm_dn, ctx->arena + 2 * d * dff * 2, 3, dims, str, box3)) return false;
   }
   if (cudaMalloc(&ctx->xg, rows * d * 2) != cudaSuccess) return false;
+  if (cudaMalloc(&ctx->mma_work, (2 * (size_t)(cfg.n_experts + cfg.max_tokens * cfg.top_k / kMmaNT + 1) + 1) * sizeof(int)) != cudaSuccess) return false;
   {
     const cuuint64_t dims[2] = {d, rows}, str[1] = {d * 2};
     if (!make_tmap(fn, &ctx->tm_xg, ctx->xg, 2, dims, str, box2)) return false;
@@ -709,7 +715,7 @@ int wisp_destroy(wisp_ctx* ctx) {
                       ctx->freq,     ctx->scal,     ctx->last_pos,    ctx->hist,    ctx->logits,  ctx->ids,
                       ctx->topw,     ctx->plan_mem, ctx->act_f32,     ctx->act_T,   ctx->ystage,  ctx->xbuf[0],
                       ctx->xbuf[1],  ctx->ybuf,     ctx->dbg_ids,     ctx->moves,   ctx->bad_slots, ctx->trace,
-                      ctx->trace_ctr, ctx->d_masters, ctx->gbar, ctx->dev_err, ctx->phase_ns, ctx->xg};
+                      ctx->trace_ctr, ctx->d_masters, ctx->gbar, ctx->dev_err, ctx->phase_ns, ctx->xg, ctx->mma_work};
   for (void* p : dev_ptrs)
     if (p) cudaFree(p);
   if (ctx->host_plan) cudaFreeHost(ctx->host_plan);
