@@ -273,6 +273,13 @@ def prefill_bench(shape, args, n_layers=8, T=2048):
         out["tensor_peak_tflops"] = pk.get("bf16_tflops_sustained")
         if out["gemm_kernels_tflops"] and out["tensor_peak_tflops"]:
             out["gemm_frac_of_tensor_peak"] = round(out["gemm_kernels_tflops"] / out["tensor_peak_tflops"], 4)
+            # at T/E*k = 128 tokens per expert the grouped GEMM sits below the ridge: every expert's weights are read once
+            w_bytes = n_layers * sh.n_experts * sh.expert_bytes
+            t_hbm = w_bytes / (pk["hbm_gbs"] * 1e9)
+            t_mma = flops / (out["tensor_peak_tflops"] * 1e12)
+            out["gemm_bound"] = "hbm" if t_hbm > t_mma else "tensor"
+            out["gemm_lower_bound_ms"] = round(max(t_hbm, t_mma) * 1e3, 3)
+            out["gemm_frac_of_bound"] = round(max(t_hbm, t_mma) * 1e3 / gemm_ms, 4)
     ctx.close()
     return out
 
