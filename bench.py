@@ -38,7 +38,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=128)
     ap.add_argument("--warmup", type=int, default=16)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="qwen3", choices=["qwen3", "mixtral", "tiny"])
+    ap.add_argument("--workload", default="qwen3", choices=["qwen3", "mixtral", "tiny", "mvwsa"])
+    ap.add_argument("--mvwsa-decode", type=int, default=512, help="decode steps per request (config 5)")
+    ap.add_argument("--mvwsa-prompt-scale", type=float, default=1.0, help="scale the U{1k..16k} prompt lengths (config 5)")
     ap.add_argument("--layers", type=int, default=0, help="override the layer count (0 = the config's)")
     ap.add_argument("--budget-gib", type=float, default=0.0, help="expert-pool budget (0 = the config's)")
     ap.add_argument("--batch", type=int, default=1)
@@ -282,6 +284,175 @@ def prefill_bench(shape, args, n_layers=8, T=2048):
             out["gemm_frac_of_bound"] = round(max(t_hbm, t_mma) * 1e3 / gemm_ms, 4)
     ctx.close()
     return out
+
+
+class KvSched:
+    """Harness-level KV-reservation scheduler of BASELINE.json config 5 (G12/G14/G15): FCFS admission on
+    block reservations, a request holds ceil((P+g)/16) blocks, the most recently admitted request is preempted when a
+    block is needed and none is free (it re-prefills P+g tokens).  Reservations go through wisp_kv_reserve."""
+
+    def __init__(self, ctx, prompts, target):
+        self.ctx, self.target = ctx, target
+        self.waiting = [dict(rid=i, prompt=p, gen=0, blocks=0, t_first=None) for i, p in enumerate(prompts)]
+        self.running, self.done = [], []
+        self.preemptions = self.reprefill = 0
+
+    def kappa(self):
+        return self.ctx.stats().kv_blocks
+
+    def used(self):
+        return sum(r["blocks"] for r in self.running)
+
+    def admit(self):
+        out = []
+        while self.waiting:
+            r = self.waiting[0]
+            n = -(-(r["prompt"] + r["gen"]) // 16)
+            if self.used() + n > self.kappa():
+                break
+            self.waiting.pop(0)
+            self.ctx.kv_reserve(n)
+            r["blocks"] = n
+            self.running.append(r)
+            out.append(r)
+        return out
+
+    def grow_for_decode(self):
+        i = 0
+        while i < len(self.running):
+            r = self.running[i]
+            n = -(-(r["prompt"] + r["gen"] + 1) // 16)
+            evicted_self = False
+            while n > r["blocks"] and self.used() + (n - r["blocks"]) > self.kappa() and len(self.running) > 1:
+                v = self.running.pop()
+                self.ctx.kv_reserve(-v["blocks"])
+                v["blocks"] = 0
+                self.preemptions += 1
+                self.reprefill += v["prompt"] + v["gen"]
+                self.waiting.insert(0, v)
+                if v is r:
+                    evicted_self = True
+                    break
+            if evicted_self:
+                continue
+            if n > r["blocks"]:
+                self.ctx.kv_reserve(n - r["blocks"])
+                r["blocks"] = n
+            i += 1
+
+    def finish(self):
+        for r in [x for x in self.running if x["gen"] >= self.target]:
+            self.ctx.kv_reserve(-r["blocks"])
+            self.running.remove(r)
+            self.done.append(r)
+
+
+def mvwsa_arm(shape, args, arm, prompts, n_decode, ctx, streams):
+    """One arm of config 5 on an existing context: arm = "live" or a fixed expert fraction.  Returns the arm's report."""
+    B = 12 * GIB
+    a, b = shape.slot_unit_bytes, 2 * 16 * shape.n_layers * 4 * 128 * 2          # G14: 1.5 MiB per block at L = 48
+    floor_blocks = -(-(16384 + n_decode) // 16)
+    frac = 0.5 if arm == "live" else float(arm)
+    C0 = max(1, int(B * frac) // a)
+    ctx.set_split(a, (B - a) // b * b)                                # shrink to one slot first: every arm starts (almost) cold
+    ctx.set_split(C0 * a, (B - C0 * a) // b * b)
+    ctx.mvwsa_track(arm == "live")
+    sched = KvSched(ctx, prompts, n_decode)
+    stream = torch.cuda.Stream()
+    T = 2048
+    xin = torch.empty((T, shape.d_model), dtype=shape.torch_dtype, device="cuda")
+    xout = torch.empty_like(xin)
+    splits = [(0, C0, ctx.stats().kv_blocks)]
+    st0 = ctx.stats()
+    t_prefill = t_decode = 0.0
+    decode_iters = 0
+    t_start = time.perf_counter()
+    with torch.cuda.stream(stream):
+        while sched.waiting or sched.running:
+            for r in sched.admit():                                   # prefill (or re-prefill) in chunks of 2048 tokens
+                n_tok = r["prompt"] + r["gen"]
+                t0 = time.perf_counter()
+                for c0 in range(0, n_tok, T):
+                    n = min(T, n_tok - c0)
+                    ctx.stack_forward(streams["prefill"][r["rid"]][:n], xout[:n], stream.cuda_stream)
+                stream.synchronize()
+                t_prefill += time.perf_counter() - t0
+                if r["t_first"] is None:
+                    r["t_first"] = time.perf_counter() - t_start
+            if not sched.running:
+                if sched.waiting:
+                    raise RuntimeError("KV pool too small for the head request (admission floor violated)")
+                break
+            sched.grow_for_decode()
+            nb = len(sched.running)
+            t0 = time.perf_counter()
+            for i, r in enumerate(sched.running):
+                xin[i].copy_(streams["decode"][r["rid"]][r["gen"]], non_blocking=True)
+            ctx.stack_forward(xin[:nb], xout[:nb], stream.cuda_stream)
+            stream.synchronize()
+            t_decode += time.perf_counter() - t0
+            for r in sched.running:
+                r["gen"] += 1
+            sched.finish()
+            decode_iters += 1
+            if arm == "live" and decode_iters % 64 == 0:              # G16: Eq. 6-8 every 64 decode steps, between forwards
+                eb, kb, moved = ctx.mvwsa_propose(mode=0, c_min=shape.top_k, c_max=0, dead_zone=1, headroom=0.2)
+                ctx.mvwsa_miss_curve(shape.n_experts + 1, decay=0.5)
+                if moved:
+                    try:
+                        ctx.set_split(eb, kb)
+                        splits.append((decode_iters, eb // a, kb // b))
+                    except Exception:
+                        pass                                          # refused resize: the previous split stays (PAPER.md:169)
+                ctx.stats()                                           # resets the KV peak window
+    wall = time.perf_counter() - t_start
+    st1 = ctx.stats()
+    refs = st1.total.references - st0.total.references
+    miss = st1.total.misses - st0.total.misses
+    ttft = sorted(r["t_first"] for r in sched.done)
+    return {"arm": arm, "e2e_s": round(wall, 2), "ttft_median_s": round(ttft[len(ttft) // 2], 2), "prefill_s": round(t_prefill, 2),
+            "decode_s": round(t_decode, 2), "decode_tokens_per_s": round(len(prompts) * n_decode / max(t_decode, 1e-9), 1),
+            "preemptions": sched.preemptions, "reprefilled_tokens": sched.reprefill, "splits_step_C_kappa": splits,
+            "hit_rate": round(1 - miss / max(1, refs), 4), "miss_gib": round(miss * shape.expert_bytes / GIB, 1),
+            "kv_floor_blocks": floor_blocks}
+
+
+def main_mvwsa(args):
+    """BASELINE.json config 5: one 12 GiB budget shared by expert slots and KV reservations, 4 concurrent requests."""
+    shape = si.QWEN3 if args.layers <= 0 else si.QWEN3.with_layers(args.layers)
+    n_decode = args.mvwsa_decode
+    prompts = [max(64, int(p * args.mvwsa_prompt_scale)) for p in si.gen_prompt_lengths(shape, 4)]
+    B = 12 * GIB
+    b = 2 * 16 * shape.n_layers * 4 * 128 * 2
+    floor_blocks = -(-(int(16384 * args.mvwsa_prompt_scale) + n_decode) // 16)
+    import paper_2606_21868_b200 as wp
+    ctx = wp.Wisp(B, n_layers=shape.n_layers, n_experts=shape.n_experts, top_k=shape.top_k, d_model=shape.d_model, d_ff=shape.d_ff,
+                  max_tokens=2048, dtype=wp.WISP_BF16, policy=wp.WISP_LRU, fetch=wp.WISP_FETCH_FUSED, kv_block_bytes=b,
+                  kv_floor_blocks=floor_blocks)
+    staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
+    for l in range(shape.n_layers):
+        si.gen_layer_experts(shape, l, "cuda", out=staging)
+        w_r, bias = si.gen_router(shape, l)
+        ctx.register_host_experts(l, staging, w_r, bias)
+    del staging
+    streams = {"decode": [si.gen_decode_hidden(shape, n_decode, 1, stream_base=r)[:, 0].to(shape.torch_dtype).cuda() for r in range(4)],
+               # one 2048-token chunk of i.i.d. N(0,1) prompt states per request, reused for each of its chunks
+               "prefill": [si.gen_prefill_hidden(shape, 2048, request=r).to(shape.torch_dtype).cuda() for r in range(4)]}
+    arms = []
+    for arm in ("live", "0.25", "0.5", "0.75"):
+        try:
+            arms.append(mvwsa_arm(shape, args, arm, prompts, n_decode, ctx, streams))
+        except Exception as ex:
+            arms.append({"arm": arm, "error": repr(ex)[:300]})
+    ctx.close()
+    base = next((x for x in arms if x.get("arm") == "0.5" and "e2e_s" in x), None)
+    live = next((x for x in arms if x.get("arm") == "live" and "e2e_s" in x), None)
+    line = {"metric": "mvwsa_e2e_seconds", "value": live["e2e_s"] if live else None, "unit": "s", "n_gpus": 1, "higher_is_better": False,
+            "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": f"config 5: {shape.name}, {shape.n_layers} layers, B = 12 GiB shared by expert slots and KV reservations, "
+                                   f"4 requests, prompts {prompts}, {n_decode} decode steps each, KV floor {floor_blocks} blocks"},
+            "live_vs_fixed_50": round(base["e2e_s"] / live["e2e_s"], 3) if base and live else None, "arms": arms}
+    print(json.dumps(line))
 
 
 def cpu_oracle_sample(shape, layers, hidden_row, threads=None):
@@ -543,7 +714,9 @@ def main_ours(args):
 
 if __name__ == "__main__":
     a = parse()
-    if a.impl == "reference":
+    if a.workload == "mvwsa":
+        main_mvwsa(a)
+    elif a.impl == "reference":
         main_reference(a)
     else:
         main_ours(a)
