@@ -57,7 +57,6 @@ struct PersistArgs {
   u64 trace_cap;
   int trace_on, track;
   u64* phase_ns;                // nullable: [kPersistPhases] globaltimer ns summed by CTA 0
-  unsigned* cta_rate;           // [2][256] per-CTA streaming rate of the previous layer (units << 24 per ns), 0 = unknown
 };
 
 struct PersistPlan {            // the per-layer plan in shared memory (same fields as PlanPtrs)
@@ -115,12 +114,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
   __shared__ float s_selz[NP * kMaxTopK];
   __shared__ int s_ids[NP * kMaxTopK];
   __shared__ float s_w[NP * kMaxTopK];
-  // Share of the wave's units this CTA and its predecessors take, as a 20-bit fixed-point cumulative fraction.  The two
-  // dies of a B200 stream at different rates (about 0.85 vs 1.04 us per 32 KiB stage, measured per CTA), so an even
-  // split makes the faster die wait at every barrier; the split follows the rates measured in the previous layer.
-  // Which CTA computes a unit never changes its value (every dot product lives inside one row group).
-  __shared__ unsigned s_cum[kPersistMaxExperts + 1];
-  __shared__ unsigned s_rate[kPersistMaxExperts];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   Ring ring;
@@ -133,7 +126,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
   }
   __syncthreads();
   RingPos rp{0, 0u};
-  auto unit_lo = [&](long long U, unsigned c) { return (int)((U * (long long)s_cum[c]) >> 20); };
   const int E = a.E, k = a.k, d = a.d, dff = a.dff, T_ = a.T, C = a.C;
   PlanPtrs pp;
   pp.hdr = pl.hdr; pp.entry_expert = pl.entry_expert; pp.entry_slot = pl.entry_slot; pp.entry_miss = pl.entry_miss;
@@ -153,11 +145,11 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
         const int lo = w * C, nw = min(nR, lo + C) - lo;
         {
           const long long U = (long long)nw * ggu.upe;
-          stream_produce(sa, ggu, ring, rp, lo, unit_lo(U, blockIdx.x), unit_lo(U, blockIdx.x + 1), lane, pol);
+          stream_produce(sa, ggu, ring, rp, lo, (int)(U * blockIdx.x / gridDim.x), (int)(U * (blockIdx.x + 1) / gridDim.x), lane, pol);
         }
         {
           const long long U = (long long)nw * gdn.upe;
-          stream_produce(sa, gdn, ring, rp, lo, unit_lo(U, blockIdx.x), unit_lo(U, blockIdx.x + 1), lane, pol);
+          stream_produce(sa, gdn, ring, rp, lo, (int)(U * blockIdx.x / gridDim.x), (int)(U * (blockIdx.x + 1) / gridDim.x), lane, pol);
         }
       }
     }
@@ -234,37 +226,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
 #ifndef WISP_PROBE_TIMELINE
     stamp(1);
 #endif
-    {   // unit split of this layer from the rates published in the previous layer (first layer of a launch: even)
-      const int G = (int)gridDim.x;
-      if (tid < G) s_rate[tid] = l > a.layer_lo ? a.cta_rate[(l & 1) * kPersistMaxExperts + tid] : 0u;
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      if (tid < 32) {
-        unsigned lo_r = 0xffffffffu; u64 sum = 0;
-        for (int c = tid; c < G; c += 32) { lo_r = min(lo_r, s_rate[c]); sum += s_rate[c]; }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          lo_r = min(lo_r, __shfl_xor_sync(0xffffffffu, lo_r, o));
-          sum += __shfl_xor_sync(0xffffffffu, sum, o);
-        }
-        const bool even = lo_r == 0u;                                         // some CTA has no clean measurement
-        const u64 mean = sum / (u64)G;
-        u64 tot = 0;                                                          // clamp to [3/4, 4/3] of the mean, then prefix
-        for (int c = 0; c < G; ++c) tot += even ? 1u : (u64)min(max((u64)s_rate[c], mean * 3 / 4), mean * 4 / 3);
-        u64 run = 0;
-        for (int c0 = 0; c0 < G; c0 += 32) {
-          const int c = c0 + tid;
-          u64 w = 0;
-          if (c < G) w = even ? 1u : (u64)min(max((u64)s_rate[c], mean * 3 / 4), mean * 4 / 3);
-          u64 inc = w;
-#pragma unroll
-          for (int o = 1; o < 32; o <<= 1) { const u64 n = __shfl_up_sync(0xffffffffu, inc, o); if (tid >= o) inc += n; }
-          if (c < G) s_cum[c] = (unsigned)(((run + inc - w) << 20) / tot);
-          run += __shfl_sync(0xffffffffu, inc, 31);
-        }
-        if (tid == 0) s_cum[G] = 1u << 20;
-      }
-      // made visible to all consumers by plan_compute's barriers and to the producer by the plan_ready arrive below
-    }
     if (writer && tid < T_ * k) {
       const size_t off = (size_t)l * a.max_tokens * k;
       a.ids[off + tid] = s_ids[tid];
@@ -311,14 +272,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
         if (tid == 0 && a.phase_ns && l == a.layer_hi - 1) { cta_probe[1] = globaltimer_ns(); cta_probe[5] = (u64)((int)(U * (blockIdx.x + 1) / gridDim.x) - (int)(U * blockIdx.x / gridDim.x)); }
         stamp(1);
 #endif
-        const int gu_lo = unit_lo(U, blockIdx.x), gu_hi = unit_lo(U, blockIdx.x + 1);
-        const u64 tg0 = globaltimer_ns();
-        stream_consume<T, 0, NP>(sa, ggu, ring, rp, lo, gu_lo, gu_hi, s_red, par, 2);
-        if (tid == 0) {               // publish this CTA's rate for the next layer's split (other parity: no reader this layer)
-          const u64 dt = globaltimer_ns() - tg0;
-          const bool clean = n_waves == 1 && pl.hdr[2] == 0 && gu_hi > gu_lo && dt > 0;
-          a.cta_rate[((l + 1) & 1) * kPersistMaxExperts + blockIdx.x] = clean ? (unsigned)((((u64)(gu_hi - gu_lo)) << 24) / dt) : 0u;
-        }
+        stream_consume<T, 0, NP>(sa, ggu, ring, rp, lo, (int)(U * blockIdx.x / gridDim.x), (int)(U * (blockIdx.x + 1) / gridDim.x),
+                                 s_red, par, 2);
       }
 #ifdef WISP_PROBE_TIMELINE
       if (tid == 0 && a.phase_ns && l == a.layer_hi - 1) a.phase_ns[16 + blockIdx.x * 8 + 2] = globaltimer_ns();
@@ -335,7 +290,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
       {
         const long long U = (long long)nw * gdn.upe;
         sa.operand = a.act; sa.result = a.ystage; sa.out_ld = d;
-        stream_consume<T, 1, NP>(sa, gdn, ring, rp, lo, unit_lo(U, blockIdx.x), unit_lo(U, blockIdx.x + 1), s_red, par, 2);
+        stream_consume<T, 1, NP>(sa, gdn, ring, rp, lo, (int)(U * blockIdx.x / gridDim.x), (int)(U * (blockIdx.x + 1) / gridDim.x),
+                                 s_red, par, 2);
       }
 #ifdef WISP_PROBE_TIMELINE
       if (tid == 0 && a.phase_ns && l == a.layer_hi - 1) a.phase_ns[16 + blockIdx.x * 8 + 4] = globaltimer_ns();

@@ -85,7 +85,6 @@ struct wisp_ctx {
   unsigned* gbar = nullptr;          // grid barrier counter
   int* dev_err = nullptr;            // device error flag (grid barrier timeout)
   u64* phase_ns = nullptr;           // device [kPersistPhases]
-  unsigned* cta_rate = nullptr;      // device [2][256]: per-CTA streaming rates (adaptive unit split)
   int persist_enabled = 1;
   // tcgen05 prefill path (ffn_prefill_mma.cuh): TMA tensor maps over the arena / the B-operand buffers
   bool mma_ok = false;
@@ -480,7 +479,6 @@ int launch_persistent(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void
   pa.trace = ctx->trace; pa.trace_ctr = ctx->trace_ctr; pa.trace_cap = ctx->trace_cap; pa.trace_on = ctx->trace_on;
   pa.track = ctx->track;
   pa.phase_ns = ctx->timing_level >= 2 ? ctx->phase_ns : nullptr;
-  pa.cta_rate = ctx->cta_rate;
   int rc;
   if (T_ <= 1) rc = launch_persistent_np<T, 1>(ctx, pa, st);
   else if (T_ <= 2) rc = launch_persistent_np<T, 2>(ctx, pa, st);
@@ -682,8 +680,6 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   CKC(cudaMalloc(&ctx->d_masters, (size_t)L * sizeof(char*)));
   CKC(cudaMemset(ctx->d_masters, 0, (size_t)L * sizeof(char*)));
   CKC(cudaMalloc(&ctx->gbar, sizeof(unsigned)));
-  CKC(cudaMalloc(&ctx->cta_rate, 2 * kPersistMaxExperts * sizeof(unsigned)));
-  CKC(cudaMemset(ctx->cta_rate, 0, 2 * kPersistMaxExperts * sizeof(unsigned)));
   CKC(cudaMalloc(&ctx->dev_err, sizeof(int)));
   CKC(cudaMemset(ctx->dev_err, 0, sizeof(int)));
   CKC(cudaMalloc(&ctx->phase_ns, (16 + 8 * 256) * sizeof(u64)));   // phases, 2 counters, (probe builds) per-CTA times
@@ -719,7 +715,7 @@ int wisp_destroy(wisp_ctx* ctx) {
                       ctx->freq,     ctx->scal,     ctx->last_pos,    ctx->hist,    ctx->logits,  ctx->ids,
                       ctx->topw,     ctx->plan_mem, ctx->act_f32,     ctx->act_T,   ctx->ystage,  ctx->xbuf[0],
                       ctx->xbuf[1],  ctx->ybuf,     ctx->dbg_ids,     ctx->moves,   ctx->bad_slots, ctx->trace,
-                      ctx->trace_ctr, ctx->d_masters, ctx->gbar, ctx->dev_err, ctx->phase_ns, ctx->xg, ctx->mma_work, ctx->cta_rate};
+                      ctx->trace_ctr, ctx->d_masters, ctx->gbar, ctx->dev_err, ctx->phase_ns, ctx->xg, ctx->mma_work};
   for (void* p : dev_ptrs)
     if (p) cudaFree(p);
   if (ctx->host_plan) cudaFreeHost(ctx->host_plan);
