@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
                                                                               int xs_bytes, int rw_bytes) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(8) unsigned long long s_full[kStreamMaxStages], s_empty[kStreamMaxStages], s_plan_ready, s_rw_bar;
-  __shared__ float s_red[2 * (kStreamConsumers / 32) * StreamBatch<NP>::NVAL];
+  __shared__ float s_red[StreamRed<NP>::kFloats];
   __shared__ PlanShared<kPersistMaxExperts> sh;
   __shared__ PersistPlan pl;
   __shared__ float s_z[NP * kPersistMaxExperts];   // logits, rows packed E apart

@@ -190,90 +190,66 @@ __device__ __forceinline__ void stream_produce(const StreamArgs& a, const Stream
   }
 }
 
-// Accumulators per consumer thread between two reductions: 32 (64 for NP = 8) = row blocks per batch x 8 rows x NP.
-template <int NP> struct StreamBatch {
-  static constexpr int SPU = NP <= 4 ? 4 / NP : 1;          // row blocks (ring stages per segment) per batch
-  static constexpr int NVAL = SPU * kStreamVals * NP;       // values reduced per thread per batch
+// Accumulators per consumer thread between two reductions: 32 (64 for 8 pairs) = row blocks per batch x 8 rows x CNT,
+// CNT = routed pairs of the expert rounded up to 1, 2, 4 or 8.  The shared-memory scratch is sized for the kernel's NP.
+template <int CNT> struct StreamBatch {
+  static constexpr int SPU = CNT <= 4 ? 4 / CNT : 1;        // row blocks (ring stages per segment) per batch
+  static constexpr int NVAL = SPU * kStreamVals * CNT;      // values reduced per thread per batch
 };
+__device__ __forceinline__ int stream_cnt_class(int cnt) { return cnt <= 1 ? 1 : cnt <= 2 ? 2 : cnt <= 4 ? 4 : 8; }
 
-// acc[v][q] += <weight chunk v, operand chunk of pair q> for q < CNT, elements in ascending order (canonical order).
-template <typename T, int NP, int CNT>
-__device__ __forceinline__ void stream_fma(const uint4 (&wq)[kStreamVals], const float (&xr)[NP][ChunkW<T>::N],
-                                           float (&acc)[kStreamVals][NP]) {
-  constexpr int EPC = ChunkW<T>::N;
-#pragma unroll
-  for (int v = 0; v < kStreamVals; ++v) {
-    float wv[EPC];
-    ChunkW<T>::widen(wq[v], wv);
-#pragma unroll
-    for (int q = 0; q < CNT; ++q)
-#pragma unroll
-      for (int j = 0; j < EPC; ++j) acc[v][q] = fmaf(wv[j], xr[q][j], acc[v][q]);
-  }
-}
-
-// The 8 consumer warps (tid 0..255) take the same row blocks from the ring.  MODE 0 = gate/up + SwiGLU, MODE 1 = down.
-// NP = max pairs per expert handled (>= n_tokens of the call).  Thread p of a row group keeps chunk p of the operand
-// in registers and one fp32 accumulator per (row, pair); up to SPU consecutive row blocks of an entry are accumulated
-// before ONE cross-thread reduction (lanes: transposed xor butterfly; warps: ascending, through s_red) and one
-// epilogue, so the block-wide barrier and the SiLU/store tail are paid once per batch, not once per ring stage.
-// Batching changes which dot products are reduced together, never the summation order inside one of them.
-// s_red: [2][8][NVAL] floats of shared memory; `par` alternates between its halves; `red_bar` = a named barrier id
-// free for the n_active threads.
-template <typename T, int MODE, int NP>
-__device__ __forceinline__ void stream_consume(const StreamArgs& a, const StreamGeom& gm, const Ring& ring, RingPos& rp,
-                                               int lo, int u_lo, int u_hi, float* s_red, int& par, int red_bar) {
+// Row blocks [u, u_end) of ONE plan entry i (all inside this CTA's unit range), pairs pl[0..cnt), cnt <= CNT.
+// Thread p of a row group keeps chunk p of each pair's operand in registers and one fp32 accumulator per (row, pair);
+// up to SPU consecutive row blocks are accumulated before ONE cross-thread reduction (lanes: transposed xor butterfly;
+// warps: ascending, through s_red) and one epilogue, so the block-wide barrier and the SiLU/store tail are paid once
+// per batch, not once per ring stage.  Batching changes which dot products are reduced together, never the summation
+// order inside one of them; an unused pair slot (cnt < CNT) multiplies by a zero operand and is never stored.
+template <typename T, int MODE, int CNT>
+__device__ __forceinline__ void stream_consume_entry(const StreamArgs& a, const StreamGeom& gm, const Ring& ring, RingPos& rp,
+                                                     int i, int u, int u_end, int cnt, const int* pl, float* s_red, int& par,
+                                                     int red_bar) {
   constexpr int EPC = ChunkW<T>::N;                         // elements per 16-byte chunk
-  constexpr int SPU = StreamBatch<NP>::SPU;
-  constexpr int NVAL = StreamBatch<NP>::NVAL;
+  constexpr int SPU = StreamBatch<CNT>::SPU;
+  constexpr int NVAL = StreamBatch<CNT>::NVAL;
   constexpr int RPT = kStreamVals / (MODE == 0 ? 2 : 1);    // rows per thread per matrix per row block
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid >= gm.n_active) {
     // a warp without work in this geometry still takes part in the ring protocol (the empty barriers count 8 warps)
-    const int n_st = (u_hi - u_lo) * gm.NSEG;
-    for (int j = 0; j < n_st; ++j) {
-      mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
-      if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);
-      ring_advance(ring, rp);
-    }
-    for (int u = u_lo; u < u_hi;) {   // stay in step with the active warps' s_red half: one flip per batch
-      const int rb = u % gm.upe;
-      u += min(SPU, min(u_hi - u, gm.upe - rb));
-      par ^= 1;
+    while (u < u_end) {
+      const int nb = min(SPU, u_end - u);
+      for (int j = 0; j < nb * gm.NSEG; ++j) {
+        mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
+        if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);
+        ring_advance(ring, rp);
+      }
+      u += nb;
+      par ^= 1;                     // stay in step with the active warps' s_red half: one flip per batch
     }
     return;
   }
   const int g = tid / gm.P, p = tid % gm.P;
   const int warps_per_group = gm.P >> 5;
-  int cur_entry = -1, cnt = 0;
-  const int* pl = nullptr;
-  float xr[NP][EPC];
-  for (int u = u_lo; u < u_hi;) {
-    const int i = lo + u / gm.upe, rb0 = u % gm.upe;
-    const int nb = min(SPU, min(u_hi - u, gm.upe - rb0));   // row blocks of this batch (all of entry i)
-    bool new_entry = i != cur_entry;
-    if (new_entry) {
-      cur_entry = i;
-      const int e = a.plan.entry_expert[i];
-      cnt = min(a.plan.exp_count[e], NP);
-      pl = a.plan.pair_list + a.plan.exp_offset[e];
-    }
-    const bool fill = a.master != nullptr && a.plan.entry_miss[i] != 0;
-    float acc[SPU][kStreamVals][NP];
+  const bool fill = a.master != nullptr && a.plan.entry_miss[i] != 0;
+  float xr[CNT][EPC];
+  bool need_operand = true;
+  while (u < u_end) {
+    const int rb0 = u % gm.upe;
+    const int nb = min(SPU, u_end - u);                     // row blocks of this batch
+    float acc[SPU][kStreamVals][CNT];
 #pragma unroll
     for (int b = 0; b < SPU; ++b)
 #pragma unroll
       for (int v = 0; v < kStreamVals; ++v)
 #pragma unroll
-        for (int q = 0; q < NP; ++q) acc[b][v][q] = 0.f;
+        for (int q = 0; q < CNT; ++q) acc[b][v][q] = 0.f;
 #pragma unroll
     for (int b = 0; b < SPU; ++b) {
       if (b < nb) {
         const int rb = rb0 + b;
         for (int seg = 0; seg < gm.NSEG; ++seg) {
-          if (new_entry || gm.NSEG > 1) {    // (re)load the thread-stationary operand slice
+          if (need_operand || gm.NSEG > 1) {    // (re)load the thread-stationary operand slice
 #pragma unroll
-            for (int q = 0; q < NP; ++q) {
+            for (int q = 0; q < CNT; ++q) {
               if (q < cnt) {
                 const int pr = pl[q];
                 const size_t col = (size_t)seg * gm.P * EPC + (size_t)p * EPC;
@@ -288,9 +264,12 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
                     xr[q][j] = f.x; xr[q][j + 1] = f.y; xr[q][j + 2] = f.z; xr[q][j + 3] = f.w;
                   }
                 }
+              } else {
+#pragma unroll
+                for (int j = 0; j < EPC; ++j) xr[q][j] = 0.f;
               }
             }
-            new_entry = false;
+            need_operand = false;
           }
           mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
 #ifdef WISP_PROBE_SKIP_MATH   // profiling probe only (never built into the product): the ring's pure streaming rate
@@ -315,28 +294,49 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
             }
             bulk_commit();
           }
-          // this thread's 8 weight chunks of the stage: matrix m, row g*RPT + i, chunk p
-          uint4 wq[kStreamVals];
+          if constexpr (CNT <= 2) {
+            // this thread's 8 weight chunks of the stage: matrix m, row g*RPT + i, chunk p; the stage is released as
+            // soon as they are in registers
+            uint4 wq[kStreamVals];
 #pragma unroll
-          for (int v = 0; v < kStreamVals; ++v) {
-            const int m = MODE == 0 ? v / RPT : 0, r = g * RPT + (MODE == 0 ? v % RPT : v);
-            const uint32_t addr = sbase + (uint32_t)((m * gm.RB + r) * gm.seg_bytes + p * 16);
-            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(wq[v].x), "=r"(wq[v].y), "=r"(wq[v].z), "=r"(wq[v].w) : "r"(addr));
-          }
-          if (fill && warp == 0) bulk_wait_read0();   // the bulk store has finished reading the stage
-          __syncwarp();
-          if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);   // stage free: the data lives in registers now
-          ring_advance(ring, rp);
-          if (NP == 1 || cnt == 1) stream_fma<T, NP, 1>(wq, xr, acc[b]);
-          else if (NP == 2 || cnt == 2) stream_fma<T, NP, (NP >= 2 ? 2 : 1)>(wq, xr, acc[b]);
-          else if (cnt == 3) stream_fma<T, NP, (NP >= 3 ? 3 : 1)>(wq, xr, acc[b]);
-          else if (NP == 4 || cnt == 4) stream_fma<T, NP, (NP >= 4 ? 4 : 1)>(wq, xr, acc[b]);
-          else {                                         // NP == 8, cnt in 5..8: unused pairs hold stale operands,
-#pragma unroll                                           // their sums are never read
-            for (int q = 0; q < NP; ++q) if (q >= cnt)
+            for (int v = 0; v < kStreamVals; ++v) {
+              const int m = MODE == 0 ? v / RPT : 0, r = g * RPT + (MODE == 0 ? v % RPT : v);
+              const uint32_t addr = sbase + (uint32_t)((m * gm.RB + r) * gm.seg_bytes + p * 16);
+              asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(wq[v].x), "=r"(wq[v].y), "=r"(wq[v].z), "=r"(wq[v].w) : "r"(addr));
+            }
+            if (fill && warp == 0) bulk_wait_read0();   // the bulk store has finished reading the stage
+            __syncwarp();
+            if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);   // stage free: the data lives in registers now
+            ring_advance(ring, rp);
 #pragma unroll
-              for (int j = 0; j < EPC; ++j) xr[q][j] = 0.f;
-            stream_fma<T, NP, NP>(wq, xr, acc[b]);
+            for (int v = 0; v < kStreamVals; ++v) {
+              float wv[EPC];
+              ChunkW<T>::widen(wq[v], wv);
+#pragma unroll
+              for (int q = 0; q < CNT; ++q)
+#pragma unroll
+                for (int j = 0; j < EPC; ++j) acc[b][v][q] = fmaf(wv[j], xr[q][j], acc[b][v][q]);
+            }
+          } else {
+            // 4 or 8 pairs: operands and accumulators already fill the register file, so the weight chunks are taken
+            // from shared memory one at a time and the stage is released after the last one (same FMA order)
+#pragma unroll
+            for (int v = 0; v < kStreamVals; ++v) {
+              const int m = MODE == 0 ? v / RPT : 0, r = g * RPT + (MODE == 0 ? v % RPT : v);
+              const uint32_t addr = sbase + (uint32_t)((m * gm.RB + r) * gm.seg_bytes + p * 16);
+              uint4 w1;
+              asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w1.x), "=r"(w1.y), "=r"(w1.z), "=r"(w1.w) : "r"(addr));
+              float wv[EPC];
+              ChunkW<T>::widen(w1, wv);
+#pragma unroll
+              for (int q = 0; q < CNT; ++q)
+#pragma unroll
+                for (int j = 0; j < EPC; ++j) acc[b][v][q] = fmaf(wv[j], xr[q][j], acc[b][v][q]);
+            }
+            if (fill && warp == 0) bulk_wait_read0();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);
+            ring_advance(ring, rp);
           }
         }
       }
@@ -349,7 +349,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
 #pragma unroll
       for (int v = 0; v < kStreamVals; ++v)
 #pragma unroll
-        for (int q = 0; q < NP; ++q) red[(b * kStreamVals + v) * NP + q] = acc[b][v][q];
+        for (int q = 0; q < CNT; ++q) red[(b * kStreamVals + v) * CNT + q] = acc[b][v][q];
     warp_multi_reduce<NVAL>(red, lane);
     constexpr int PER_LANE = NVAL >= 32 ? NVAL / 32 : 1;
     float* sr = s_red + (size_t)par * (kStreamConsumers / 32) * NVAL;
@@ -364,17 +364,17 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
       const int w0 = (rg * gm.P) >> 5;
       const int pr = pl[q];
       const size_t row = (size_t)(rb0 + b) * gm.RB + r;
-      const float* base = sr + (size_t)w0 * NVAL + (b * kStreamVals) * NP + q;
+      const float* base = sr + (size_t)w0 * NVAL + (b * kStreamVals) * CNT + q;
       if (MODE == 0) {
         float gs = 0.f, us = 0.f;
         for (int w = 0; w < warps_per_group; ++w) {
-          gs += base[w * NVAL + ri * NP];
-          us += base[w * NVAL + (RPT + ri) * NP];
+          gs += base[w * NVAL + ri * CNT];
+          us += base[w * NVAL + (RPT + ri) * CNT];
         }
         a.result[(size_t)pr * a.out_ld + row] = silu_f(gs) * us;
       } else {
         float ys = 0.f;
-        for (int w = 0; w < warps_per_group; ++w) ys += base[w * NVAL + ri * NP];
+        for (int w = 0; w < warps_per_group; ++w) ys += base[w * NVAL + ri * CNT];
         a.result[(size_t)pr * a.out_ld + row] = ys;
       }
     }
@@ -382,15 +382,41 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
     par ^= 1;
     u += nb;
   }
-  if (a.master != nullptr && warp == 0) bulk_wait0();   // this warp's slot writes are complete
 }
+
+// The 8 consumer warps (tid 0..255) take units [u_lo, u_hi) of the wave whose first plan entry is `lo` from the ring, entry
+// by entry; each entry runs the routine instantiated for its pair count class (1, 2, 4, 8 <= NP), so an expert routed by
+// one token of a batch still batches 4 row blocks per reduction.  MODE 0 = gate/up + SwiGLU, MODE 1 = down.
+// s_red: [2][8][StreamBatch<NP>::NVAL-or-32] floats of shared memory; `par` alternates between its halves; `red_bar` = a
+// named barrier id free for the n_active threads.
+template <typename T, int MODE, int NP>
+__device__ __forceinline__ void stream_consume(const StreamArgs& a, const StreamGeom& gm, const Ring& ring, RingPos& rp,
+                                               int lo, int u_lo, int u_hi, float* s_red, int& par, int red_bar) {
+  for (int u = u_lo; u < u_hi;) {
+    const int i = lo + u / gm.upe;
+    const int u_end = min(u_hi, (u / gm.upe + 1) * gm.upe);            // this entry's row blocks inside the range
+    const int e = a.plan.entry_expert[i];
+    const int cnt = min(a.plan.exp_count[e], NP);
+    const int* pl = a.plan.pair_list + a.plan.exp_offset[e];
+    const int cls = stream_cnt_class(cnt);
+    if (NP == 1 || cls == 1) stream_consume_entry<T, MODE, 1>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
+    else if (NP == 2 || cls == 2) stream_consume_entry<T, MODE, (NP >= 2 ? 2 : 1)>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
+    else if (NP == 4 || cls == 4) stream_consume_entry<T, MODE, (NP >= 4 ? 4 : 1)>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
+    else stream_consume_entry<T, MODE, (NP >= 8 ? 8 : 1)>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
+    u = u_end;
+  }
+  if (a.master != nullptr && threadIdx.x < 32) bulk_wait0();   // warp 0's slot writes are complete
+}
+
+// shared-memory floats of s_red for a kernel instantiated for NP pairs: two halves x 8 warps x the largest batch
+template <int NP> struct StreamRed { static constexpr int kFloats = 2 * (kStreamConsumers / 32) * (NP >= 8 ? 64 : 32); };
 
 // One wave of one FFN half as its own launch (multi-kernel path: MEMCPY / ZEROCOPY contexts, timing level 2).
 template <typename T, int MODE, int NP>
 __global__ void __launch_bounds__(kStreamThreads, 1) ffn_stream_kernel(const StreamArgs a, const StreamGeom gm) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(8) unsigned long long s_full[kStreamMaxStages], s_empty[kStreamMaxStages];
-  __shared__ float s_red[2 * (kStreamConsumers / 32) * StreamBatch<NP>::NVAL];
+  __shared__ float s_red[StreamRed<NP>::kFloats];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   Ring ring;
   ring.stage0 = smem_u32(smem_raw); ring.full0 = smem_u32(s_full); ring.empty0 = smem_u32(s_empty);
