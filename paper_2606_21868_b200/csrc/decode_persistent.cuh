@@ -304,14 +304,19 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
 #endif
     }
 
-    // ---- phase X: ordered combine (+ residual): every CTA computes the whole x_{l+1} into its own xs ----
+    // ---- phase X: ordered combine (+ residual) ----
+    // One token: every CTA recomputes the whole x_{l+1} into its own xs (64 KiB of L2 reads, no grid barrier).  More
+    // tokens: that redundant read (T x 64 KiB per CTA from the same L2 lines) costs more than a barrier, so the work is
+    // split over the grid, x_{l+1} goes through global memory and one grid barrier, and every CTA reloads it into xs.
     {
       const int n = T_ * d;
       const bool last = l == a.layer_hi - 1;
-      T* outp = reinterpret_cast<T*>(a.out);
+      const bool split = T_ > 1;
+      T* xg = reinterpret_cast<T*>(last ? a.out : a.xbuf[(l - a.layer_lo) & 1]);
       // 4 consecutive elements per thread; the ystage loads of up to 8 ranks are issued together (one L2 round trip),
       // the sum itself is combine_elem's: fmaf in rank order from 0.f, per element.
-      for (int v4 = tid; v4 < n / 4; v4 += kStreamConsumers) {
+      for (int v4 = split ? (int)blockIdx.x * kStreamConsumers + tid : tid; v4 < n / 4;
+           v4 += split ? (int)gridDim.x * kStreamConsumers : kStreamConsumers) {
         const int idx = v4 * 4, t = idx / d, j = idx % d;
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
         for (int i0 = 0; i0 < k; i0 += 8) {
@@ -331,9 +336,18 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
         for (int c = 0; c < 4; ++c) {
           const T o = from_f32<T>(acc[c]);
           const T v = a.residual ? from_f32<T>(to_f32<T>(xs[idx + c]) + to_f32<T>(o)) : o;
-          xs[idx + c] = v;
-          if (last && v4 % (int)gridDim.x == (int)blockIdx.x) outp[idx + c] = v;
+          if (split) xg[idx + c] = v;
+          else {
+            xs[idx + c] = v;
+            if (last && v4 % (int)gridDim.x == (int)blockIdx.x) xg[idx + c] = v;
+          }
         }
+      }
+      if (split && !last) {
+        grid_barrier(a.gbar, gen, a.err);                                    // E: x_{l+1} complete in global memory
+        const uint4* src = reinterpret_cast<const uint4*>(xg);
+        uint4* dst = reinterpret_cast<uint4*>(xs);
+        for (int i = tid; i < n * (int)sizeof(T) / 16; i += kStreamConsumers) dst[i] = src[i];
       }
     }
     asm volatile("bar.sync 1, 256;" ::: "memory");                           // xs complete in this CTA
