@@ -66,6 +66,20 @@ def workload(args):
     return shape, budget
 
 
+def max_over_ranks(ms, dist, device):
+    """Replicas only: the job's step time is the slowest rank's device time."""
+    if dist is None:
+        return float(ms)
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_throughput(units_per_rank, world, ms):
+    """Whole-job units/s of `world` independent replicas that each processed units_per_rank in at most ms."""
+    return units_per_rank * world / (ms * 1e-3)
+
+
 def mem_available_bytes():
     with open("/proc/meminfo") as fh:
         for line in fh:
@@ -575,11 +589,8 @@ def main_ours(args):
         clocks = sampler.stop()
         ms = e0.elapsed_time(e1)
         st1 = ctx.stats()
-        if dist is not None:
-            tms = torch.tensor([ms], device="cuda")
-            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-            ms = float(tms.item())
-        value = args.steps * B * world / (ms * 1e-3)
+        ms = max_over_ranks(ms, dist, "cuda")
+        value = replica_throughput(args.steps * B, world, ms)
 
         # ---- e2e: host buffers, H2D + D2H inside the timed region, through the public call ----
         h_in = hidden[args.warmup:].contiguous().pin_memory()
@@ -597,10 +608,7 @@ def main_ours(args):
         e3.record(stream)
         torch.cuda.synchronize(); barrier()
         ms_e2e = e2.elapsed_time(e3)
-        if dist is not None:
-            tms = torch.tensor([ms_e2e], device="cuda")
-            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-            ms_e2e = float(tms.item())
+        ms_e2e = max_over_ranks(ms_e2e, dist, "cuda")
         io_bytes = B * shape.d_model * shape.elem_bytes
         same = torch.equal(h_out.view(torch.uint8), y_dev[args.warmup:].cpu().view(torch.uint8))
 
