@@ -142,7 +142,8 @@ def ncu_traffic(kernel):
     p = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(p):
         with open(p) as fh:
-            return json.load(fh).get(kernel)
+            v = json.load(fh).get(kernel)
+            return v.get("traffic") if isinstance(v, dict) else v
     return None
 
 
@@ -704,14 +705,23 @@ def main_ours(args):
         except Exception as ex:
             line["prefill"] = {"error": repr(ex)[:300]}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        # bounded sample: the first nl layers (weights generated once), as many decode tokens as fit in about 12 s of CPU time
+        from oracle import moe_forward as mf
         nl = min(shape.n_layers, 4 if shape.expert_bytes * shape.n_experts > (256 << 20) else shape.n_layers)
-        reps = 2 if nl < shape.n_layers else 8
-        tot, done = 0.0, 0
-        for r in range(reps):
-            t, n = cpu_oracle_sample(shape, range(nl), hidden[args.warmup + r].float())
-            tot += t; done += n
+        blobs = [si.gen_layer_experts(shape, l, "cuda") for l in range(nl)]
+        routers = [si.gen_router(shape, l) for l in range(nl)]
+        tot, done, toks = 0.0, 0, 0
+        while tot < 12.0 and toks < args.steps:
+            x = hidden[args.warmup + toks].to(shape.torch_dtype)
+            t0 = time.perf_counter()
+            for l in range(nl):
+                out, *_ = mf.moe_layer(x, blobs[l], routers[l][0], routers[l][1], shape.top_k, shape.d_ff)
+                x = (x.float() + out.to(shape.torch_dtype).float()).to(shape.torch_dtype)
+            tot += time.perf_counter() - t0
+            done += nl
+            toks += 1
         line["cpu_baseline"] = {"value": (done / shape.n_layers) * B / tot, "unit": "tokens/s", "cores": torch.get_num_threads(),
-                                "kind": "oracle", "sample": f"{reps} decode tokens x first {nl} of {shape.n_layers} layers, "
+                                "kind": "oracle", "sample": f"{toks} decode tokens x first {nl} of {shape.n_layers} layers, "
                                 f"tokens/s scaled by layers done / {shape.n_layers} ({tot:.1f} s of CPU work)"}
     ctx.close()
     if rank == 0:
