@@ -16,6 +16,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -50,6 +51,9 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-miss-path", action="store_true")
     ap.add_argument("--no-prefill", action="store_true")
+    ap.add_argument("--stress", action="store_true",
+                    help="extra, clearly labelled locality stress (never the headline): router bias x 0.25 and AR(1) coefficient 0.5 "
+                         "(same stationary variance) -> adjacent-step carry-over near the paper's 0.44-0.48 (PAPER.md:187)")
     ap.add_argument("--per-layer-api", action="store_true", help="drive wisp_moe_forward per layer instead of wisp_stack_forward")
     return ap.parse_args()
 
@@ -59,6 +63,9 @@ def workload(args):
     budget = {"qwen3": 8 * GIB, "mixtral": 24 * GIB, "tiny": 6 * si.TINY.slot_unit_bytes}[args.workload]
     if args.budget_gib > 0:
         budget = int(args.budget_gib * GIB)
+    if args.stress:
+        from dataclasses import replace
+        shape = replace(shape, zipf_alpha=shape.zipf_alpha * 0.25, name=shape.name + " [STRESS: bias x0.25, AR 0.5]")
     if args.layers > 0:
         # keep the per-layer slot count of the full config: scale the budget with the layer count
         budget = budget // shape.n_layers * args.layers
@@ -566,7 +573,10 @@ def main_ours(args):
     t_setup = time.time() - t_setup
     C = ctx.stats().slots_per_layer
     n_all = args.warmup + args.steps
-    hidden = si.gen_decode_hidden(shape, n_all, B).to(shape.torch_dtype)          # [n, B, d]
+    if args.stress:
+        hidden = si.gen_decode_hidden(shape, n_all, B, rho=0.5, noise=math.sqrt(0.01 / 0.19 * 0.75)).to(shape.torch_dtype)
+    else:
+        hidden = si.gen_decode_hidden(shape, n_all, B).to(shape.torch_dtype)          # [n, B, d]
     x_dev = hidden.cuda()
     y_dev = torch.empty_like(x_dev)
     stream = torch.cuda.Stream()
@@ -711,8 +721,8 @@ def main_ours(args):
         blobs = [si.gen_layer_experts(shape, l, "cuda") for l in range(nl)]
         routers = [si.gen_router(shape, l) for l in range(nl)]
         tot, done, toks = 0.0, 0, 0
-        while tot < 12.0 and toks < args.steps:
-            x = hidden[args.warmup + toks].to(shape.torch_dtype)
+        while tot < 12.0 and toks < 4096:
+            x = hidden[(args.warmup + toks) % n_all].to(shape.torch_dtype)
             t0 = time.perf_counter()
             for l in range(nl):
                 out, *_ = mf.moe_layer(x, blobs[l], routers[l][0], routers[l][1], shape.top_k, shape.d_ff)
