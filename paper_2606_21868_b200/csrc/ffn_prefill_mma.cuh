@@ -33,7 +33,30 @@ struct MmaArgs {
   int d, dff, k;
   __nv_bfloat16* act;     // [n_pairs][dff] bf16, SORTED pair order (position = exp_offset[e] + j)
   float* ystage;          // [n_pairs][d] fp32, indexed by pair id (t*k + rank)
+  // MODE 2 (router logits, a1 for prefill): z[t][e] = bias[e] + <W_r[e], x_t>, E a multiple of 128
+  float* z;               // [n_tokens][E] fp32
+  const float* bias;      // [E] of this layer
+  int n_tokens, E;
 };
+
+struct MmaTile { int pos0, nt, blob, r0; };
+// tile t -> (first B row, valid B rows, weight blob, first weight row)
+template <int MODE>
+__device__ __forceinline__ MmaTile mma_tile(const MmaArgs& a, const int* work, int t, int RT) {
+  MmaTile m;
+  const int w = t / RT;
+  m.r0 = (t % RT) * kMmaM;
+  if (MODE == 2) {
+    m.pos0 = w * kMmaNT; m.nt = min(kMmaNT, a.n_tokens - m.pos0); m.blob = a.layer;
+  } else {
+    const int i = work[2 * w], p0 = work[2 * w + 1];
+    const int e = a.plan.entry_expert[i];
+    m.pos0 = a.plan.exp_offset[e] + p0;
+    m.nt = min(kMmaNT, a.plan.exp_count[e] - p0);
+    m.blob = a.plan.entry_slot[i] * a.L + a.layer;
+  }
+  return m;
+}
 
 // ---- PTX wrappers -----------------------------------------------------------------------------------------------
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, uint32_t bar) {
@@ -95,16 +118,23 @@ __device__ __forceinline__ uint32_t umma_idesc_bf16(int M, int N) {
 // Work list of one wave: one item per (wave entry, tile of kMmaNT routed pairs).  work[2*w] = plan entry index,
 // work[2*w+1] = first pair of the tile inside the expert's sorted range; *n_work = item count.  One warp.
 __global__ void __launch_bounds__(32) build_work_kernel(PlanPtrs plan, int wave, int C, int* __restrict__ work, int* __restrict__ n_work) {
-  if (threadIdx.x != 0) return;
+  const int lane = threadIdx.x;
   int n = 0;
   if (wave < plan.hdr[0]) {
     const int lo = wave * C, hi = min(plan.hdr[1], lo + C);
-    for (int i = lo; i < hi; ++i) {
-      const int cnt = plan.exp_count[plan.entry_expert[i]];
-      for (int p0 = 0; p0 < cnt; p0 += kMmaNT) { work[2 * n] = i; work[2 * n + 1] = p0; ++n; }
+    for (int i0 = lo; i0 < hi; i0 += 32) {                    // 32 entries at a time: tile counts, warp prefix sum, scatter
+      const int i = i0 + lane;
+      const int cnt = i < hi ? plan.exp_count[plan.entry_expert[i]] : 0;
+      const int tiles = (cnt + kMmaNT - 1) / kMmaNT;
+      int inc = tiles;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+      int pos = n + inc - tiles;
+      for (int p0 = 0; p0 < cnt; p0 += kMmaNT, ++pos) { work[2 * pos] = i; work[2 * pos + 1] = p0; }
+      n += __shfl_sync(0xffffffffu, inc, 31);
     }
   }
-  *n_work = n;
+  if (lane == 0) *n_work = n;
 }
 
 // Persistent: one CTA per SM walks the tiles t = blockIdx.x, blockIdx.x + gridDim.x, ...; tile t = (work item t / RT,
@@ -124,10 +154,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
   constexpr uint32_t kAccCols = MODE == 0 ? 256 : 128;        // TMEM columns of one accumulator stage
   constexpr uint32_t kCols = 2 * kAccCols;
 
-  const int K = MODE == 0 ? a.d : a.dff;
+  const int K = MODE == 1 ? a.dff : a.d;
   const int nkb = K / kMmaBK;
-  const int RT = (MODE == 0 ? a.dff : a.d) / kMmaM;
-  const int n_tiles = *n_work_p * RT;
+  const int RT = (MODE == 0 ? a.dff : MODE == 1 ? a.d : a.E) / kMmaM;
+  const int n_tiles = (MODE == 2 ? (a.n_tokens + kMmaNT - 1) / kMmaNT : *n_work_p) * RT;
   if ((int)blockIdx.x >= n_tiles) return;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -147,10 +177,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
     if (lane == 0) {      // ===== TMA producer =====
       int s = 0; uint32_t ph = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        const int w = t / RT, r0 = (t % RT) * kMmaM;
-        const int i = work[2 * w], p0 = work[2 * w + 1];
-        const int pos0 = a.plan.exp_offset[a.plan.entry_expert[i]] + p0;
-        const int blob = a.plan.entry_slot[i] * a.L + a.layer;
+        const MmaTile mt = mma_tile<MODE>(a, work, t, RT);
+        const int r0 = mt.r0, pos0 = mt.pos0, blob = mt.blob;
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(smem_u32(&s_empty[s]), ph ^ 1u);
           const uint32_t bar = smem_u32(&s_full[s]);
@@ -168,9 +196,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
       int s = 0; uint32_t ph = 0;
       int j = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++j) {
-        const int w = t / RT;
-        const int i = work[2 * w], p0 = work[2 * w + 1];
-        const int nt = min(kMmaNT, a.plan.exp_count[a.plan.entry_expert[i]] - p0);
+        const int nt = mma_tile<MODE>(a, work, t, RT).nt;
         const uint32_t idesc = umma_idesc_bf16(kMmaM, max(16, (nt + 15) & ~15));
         const int as = j & 1;
         mbar_wait(smem_u32(&s_tempty[as]), ((uint32_t)(j >> 1) & 1u) ^ 1u);   // the epilogue has drained this stage
@@ -198,18 +224,16 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
     const int q = warp & 3;
     int j = 0;
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++j) {
-      const int w = t / RT, r0 = (t % RT) * kMmaM;
-      const int i = work[2 * w], p0 = work[2 * w + 1];
-      const int e = a.plan.entry_expert[i];
-      const int pos0 = a.plan.exp_offset[e] + p0;
-      const int nt = min(kMmaNT, a.plan.exp_count[e] - p0);
+      const MmaTile mt = mma_tile<MODE>(a, work, t, RT);
+      const int r0 = mt.r0, pos0 = mt.pos0, nt = mt.nt;
       const int N = max(16, (nt + 15) & ~15);
       const int as = j & 1;
       mbar_wait(smem_u32(&s_tfull[as]), (uint32_t)(j >> 1) & 1u);
       tc_fence_after();
       const int row = r0 + 32 * q + lane;                     // weight row = d_ff index (MODE 0) | d index (MODE 1)
       const uint32_t tlane = tmem + as * kAccCols + ((uint32_t)(32 * q) << 16);
-      const int* pl = a.plan.pair_list + pos0;
+      const int* pl = MODE == 2 ? nullptr : a.plan.pair_list + pos0;
+      const float bias_r = MODE == 2 ? a.bias[row] : 0.f;
       for (int c0 = 0; c0 < N; c0 += 16) {
         float g[16], u[16];
         tmem_ld16(tlane + c0, g);
@@ -219,7 +243,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
           const int col = c0 + jj;
           if (col < nt) {
             if (MODE == 0) a.act[(size_t)(pos0 + col) * a.dff + row] = __float2bfloat16_rn(silu_f(g[jj]) * u[jj]);
-            else a.ystage[(size_t)pl[col] * a.d + row] = g[jj];
+            else if (MODE == 1) a.ystage[(size_t)pl[col] * a.d + row] = g[jj];
+            else a.z[(size_t)(pos0 + col) * a.E + row] = g[jj] + bias_r;
           }
         }
       }

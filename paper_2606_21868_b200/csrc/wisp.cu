@@ -88,7 +88,8 @@ struct wisp_ctx {
   int persist_enabled = 1;
   // tcgen05 prefill path (ffn_prefill_mma.cuh): TMA tensor maps over the arena / the B-operand buffers
   bool mma_ok = false;
-  CUtensorMap tm_gu{}, tm_dn{}, tm_xg{}, tm_act{};
+  CUtensorMap tm_gu{}, tm_dn{}, tm_xg{}, tm_act{}, tm_rw{};
+  void* encode_fn = nullptr;         // cuTensorMapEncodeTiled (per-call map over the caller's hidden states)
   char* xg = nullptr;                // [maxT*k][d] gathered token rows (bf16)
   int* mma_work = nullptr;           // work list of the current wave: (entry, first pair) items + count
   u64 persist_layers_timed = 0;
@@ -175,13 +176,39 @@ struct Span {
   ~Span() { if (b) cudaEventRecord(b, st); }
 };
 
+// ---- TMA tensor maps (tcgen05 prefill path) ----
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+bool make_tmap(EncodeTiledFn fn, CUtensorMap* tm, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides_bytes,
+               const cuuint32_t* box) {
+  cuuint32_t estr[3] = {1, 1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, base, dims, strides_bytes, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <typename T>
 int launch_router(wisp_ctx* ctx, int layer, const void* x, int T_, cudaStream_t st) {
   const auto& cfg = ctx->cfg;
   const int E = cfg.n_experts, d = cfg.d_model, k = cfg.top_k;
   const T* wr = reinterpret_cast<const T*>(ctx->router_w) + (size_t)layer * E * d;
   dim3 g((E + 7) / 8, (T_ + kRouterTokTile - 1) / kRouterTokTile);
-  {
+  if (ctx->mma_ok && T_ > kDecodeMaxTokens && E % kMmaM == 0 && sizeof(T) == 2) {
+    // prefill: the router is a [T x d] x [d x E] GEMM -> same tcgen05 kernel (MODE 2), B operand = the caller's rows
+    CUtensorMap tm_x;
+    const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)T_}, str[1] = {(cuuint64_t)d * 2};
+    const cuuint32_t box2[2] = {kMmaBK, kMmaNT};
+    if (!make_tmap(reinterpret_cast<EncodeTiledFn>(ctx->encode_fn), &tm_x, const_cast<void*>(x), 2, dims, str, box2))
+      return fail(ctx, WISP_ECUDA, "tensor map over the hidden states failed (16-byte aligned rows required)");
+    MmaArgs m{};
+    m.L = cfg.n_layers; m.layer = layer; m.d = d; m.dff = cfg.d_ff; m.k = k;
+    m.z = ctx->logits; m.bias = ctx->router_bias + (size_t)layer * E; m.n_tokens = T_; m.E = E;
+    Span sp(ctx, WISP_K_ROUTER, st);
+    const int ns = 6;
+    prefill_mma_kernel<2><<<ctx->num_sms, kMmaThreads, ns * 2 * kMmaTileBytes + 1024, st>>>(ctx->tm_rw, tm_x, m, nullptr, nullptr, ns);
+  } else {
     Span sp(ctx, WISP_K_ROUTER, st);
     router_logits_kernel<T><<<g, 256, 0, st>>>(reinterpret_cast<const T*>(x), wr, ctx->router_bias + (size_t)layer * E,
                                                ctx->logits, T_, E, d);
@@ -383,18 +410,6 @@ int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, c
 }
 
 // ---- tcgen05 prefill path: tensor maps -----------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-bool make_tmap(EncodeTiledFn fn, CUtensorMap* tm, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides_bytes,
-               const cuuint32_t* box) {
-  cuuint32_t estr[3] = {1, 1, 1};
-  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, base, dims, strides_bytes, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 // K-major bf16 operands in boxes of [64 K-elements][128 rows]: weights through a 3-D view of the arena
 // (K, weight row, blob = slot*L + layer), tokens / activations through 2-D views of xg and act.
 bool setup_mma_path(wisp_ctx* ctx) {
@@ -404,6 +419,7 @@ bool setup_mma_path(wisp_ctx* ctx) {
   cudaDriverEntryPointQueryResult qres;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess || !sym) return false;
   EncodeTiledFn fn = reinterpret_cast<EncodeTiledFn>(sym);
+  ctx->encode_fn = sym;
   const cuuint64_t d = cfg.d_model, dff = cfg.d_ff, n_blobs = ctx->budget / ctx->Me, rows = (cuuint64_t)cfg.max_tokens * cfg.top_k;
   if (n_blobs < 1) return false;
   const cuuint32_t box3[3] = {kMmaBK, kMmaM, 1}, box2[2] = {kMmaBK, kMmaNT};
@@ -425,8 +441,12 @@ bool setup_mma_path(wisp_ctx* ctx) {
     const cuuint64_t dims[2] = {dff, rows}, str[1] = {dff * 2};
     if (!make_tmap(fn, &ctx->tm_act, ctx->act_T, 2, dims, str, box2)) return false;
   }
-  for (int mode = 0; mode < 2; ++mode) {
-    const void* k = mode == 0 ? (const void*)prefill_mma_kernel<0> : (const void*)prefill_mma_kernel<1>;
+  if (cfg.n_experts % kMmaM == 0) {   // router weights [L][E][d] as (K, expert row, layer)
+    const cuuint64_t dims[3] = {d, (cuuint64_t)cfg.n_experts, (cuuint64_t)cfg.n_layers}, str[2] = {d * 2, (cuuint64_t)cfg.n_experts * d * 2};
+    if (!make_tmap(fn, &ctx->tm_rw, ctx->router_w, 3, dims, str, box3)) return false;
+  }
+  for (int mode = 0; mode < 3; ++mode) {
+    const void* k = mode == 0 ? (const void*)prefill_mma_kernel<0> : mode == 1 ? (const void*)prefill_mma_kernel<1> : (const void*)prefill_mma_kernel<2>;
     if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) return false;
   }
   return true;
