@@ -279,14 +279,16 @@ __global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a
   plan_compute<kPlanThreads>(a, sh, /*writer=*/true, /*bar=*/0);
 }
 
-// Stable grouping of (token, rank) pairs by expert for large n_pairs: one CTA per expert.
-__global__ void __launch_bounds__(256) group_pairs_kernel(const int* __restrict__ ids, int n_pairs, PlanPtrs plan) {
-  __shared__ int s_ws[9];
+// Stable grouping of (token, rank) pairs by expert for large n_pairs: one CTA of kGroupThreads per expert.
+constexpr int kGroupThreads = 1024;
+__global__ void __launch_bounds__(kGroupThreads) group_pairs_kernel(const int* __restrict__ ids, int n_pairs, PlanPtrs plan) {
+  constexpr int NW = kGroupThreads / 32;
+  __shared__ int s_ws[NW];
   const int e = blockIdx.x;
   if (plan.exp_count[e] == 0) return;
   int pos = plan.exp_offset[e];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (int base = 0; base < n_pairs; base += 256) {
+  for (int base = 0; base < n_pairs; base += kGroupThreads) {
     const int p = base + threadIdx.x;
     const bool m = p < n_pairs && ids[p] == e;
     const unsigned bal = __ballot_sync(0xffffffffu, m);
@@ -294,7 +296,7 @@ __global__ void __launch_bounds__(256) group_pairs_kernel(const int* __restrict_
     __syncthreads();
     int before = 0, tot = 0;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) { const int c = s_ws[i]; if (i < wid) before += c; tot += c; }
+    for (int i = 0; i < NW; ++i) { const int c = s_ws[i]; if (i < wid) before += c; tot += c; }
     if (m) plan.pair_list[pos + before + __popc(bal & ((1u << lane) - 1u))] = p;
     pos += tot;
     __syncthreads();

@@ -246,7 +246,7 @@ int launch_plan(wisp_ctx* ctx, int layer, const int* ids, int n_pairs, bool want
   }
   if (!a.build_pairs) {
     Span sp(ctx, WISP_K_RESIDENCY, st);
-    group_pairs_kernel<<<a.E, 256, 0, st>>>(ids, n_pairs, ctx->plan);
+    group_pairs_kernel<<<a.E, kGroupThreads, 0, st>>>(ids, n_pairs, ctx->plan);
   }
   CK(cudaGetLastError());
   return WISP_OK;
