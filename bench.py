@@ -51,6 +51,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-miss-path", action="store_true")
     ap.add_argument("--no-prefill", action="store_true")
+    ap.add_argument("--ring-stages", type=int, default=0, help="shared-memory ring depth of the decode FFN (0 = library default)")
     ap.add_argument("--stress", action="store_true",
                     help="extra, clearly labelled locality stress (never the headline): router bias x 0.25 and AR(1) coefficient 0.5 "
                          "(same stationary variance) -> adjacent-step carry-over near the paper's 0.44-0.48 (PAPER.md:187)")
@@ -160,7 +161,8 @@ def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=N
     ctx = wp.Wisp(budget, n_layers=shape.n_layers, n_experts=shape.n_experts, top_k=shape.top_k, d_model=shape.d_model,
                   d_ff=shape.d_ff, max_tokens=max_tokens, dtype=wp.WISP_F32 if shape.dtype == "f32" else wp.WISP_BF16,
                   policy=wp.WISP_LFU if args.policy == "lfu" else wp.WISP_LRU,
-                  fetch={"memcpy": wp.WISP_FETCH_MEMCPY, "zerocopy": wp.WISP_FETCH_ZEROCOPY, "fused": wp.WISP_FETCH_FUSED}[fetch or args.fetch])
+                  fetch={"memcpy": wp.WISP_FETCH_MEMCPY, "zerocopy": wp.WISP_FETCH_ZEROCOPY, "fused": wp.WISP_FETCH_FUSED}[fetch or args.fetch],
+                  ring_stages=getattr(args, "ring_stages", 0))
     staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
     for l in (register_layers if register_layers is not None else range(shape.n_layers)):
         si.gen_layer_experts(shape, l, gen_device, out=staging)

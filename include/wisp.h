@@ -66,7 +66,7 @@ typedef struct {
   int32_t dtype;      /* wisp_dtype: dtype of weights, hidden and out */
   int32_t policy;     /* wisp_policy */
   int32_t fetch;      /* wisp_fetch */
-  int32_t ring_stages; /* shared-memory ring depth of the decode FFN kernels, 2..8; 0 = library default */
+  int32_t ring_stages; /* shared-memory ring depth of the decode FFN kernels, 2..8; 0 = library default (3 in the persistent kernel) */
   uint64_t kv_block_bytes;  /* b: bytes per KV block summed over layers; 0 = no KV accounting */
   uint64_t kv_floor_blocks; /* kappa_min of Eq. 4; wisp_set_split refuses to go below it */
   uint64_t trace_capacity;  /* trace ring capacity in events; 0 = library default (1<<20) */

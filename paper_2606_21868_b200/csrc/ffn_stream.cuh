@@ -183,7 +183,11 @@ __device__ __forceinline__ void stream_produce(const StreamArgs& a, const Stream
           bytes = (uint32_t)gm.seg_bytes;
           src = blob + gm.mat_off[m] + ((size_t)rb * gm.RB + r) * gm.row_bytes + (size_t)seg * gm.seg_bytes;
         }
+#ifdef WISP_PROBE_NO_L2_HINT   // profiling probe only
+        bulk_g2s_nohint(sbase + c * bytes, src, bytes, bar);
+#else
         bulk_g2s(sbase + c * bytes, src, bytes, bar, pol);
+#endif
       }
       ring_advance(ring, rp);
     }

@@ -471,7 +471,10 @@ int launch_persistent_np(wisp_ctx* ctx, PersistArgs& pa, cudaStream_t st) {
   xs_bytes += 0;
   if ((size_t)xs_bytes + rw_bytes + 2 * (size_t)stride > smem) return fail(ctx, WISP_EINVAL, "persistent decode kernel: shared memory too small");
   n_stages = (int)std::min<size_t>(kStreamMaxStages, (smem - xs_bytes - rw_bytes) / stride);
-  if (ctx->cfg.ring_stages > 0) n_stages = std::min(n_stages, (int)ctx->cfg.ring_stages);
+  // Measured on B200 (Qwen3 shape, all-resident, 12 layers): 2 / 3 / 4 / 5 / 6 stages -> 0.581 / 0.577 / 0.578 / 0.593 / 0.597 ms
+  // per token at batch 1 and 1.09 vs 1.24 ms (3 vs 6) at batch 4; no difference at the Mixtral shape.  A deeper ring lets
+  // the producer run further into the down tiles while gate/up is still streaming, which costs more than it hides.
+  n_stages = std::min(n_stages, ctx->cfg.ring_stages > 0 ? (int)ctx->cfg.ring_stages : 3);
   if (n_stages < 2) return fail(ctx, WISP_EINVAL, "persistent decode kernel: ring does not fit shared memory");
   CK(cudaMemsetAsync(ctx->gbar, 0, sizeof(unsigned), st));
   StreamGeom ggu = ctx->geom_gu, gdn = ctx->geom_dn;
