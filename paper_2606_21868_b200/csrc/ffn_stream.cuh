@@ -31,7 +31,11 @@ namespace wisp {
 constexpr int kStreamConsumers = 256;                       // 8 consumer warps
 constexpr int kStreamThreads = kStreamConsumers + 32;       // + 1 producer warp
 constexpr int kStreamMaxStages = 8;
-constexpr int kStreamVals = 8;                              // weight rows per thread per stage (4 gate + 4 up | 8 down)
+// Weight rows per consumer thread per ring stage: 16 (8 gate + 8 up | 16 down; 64 KiB stages) when at most 2 tokens are in
+// flight, 8 (32 KiB stages) otherwise.  Measured on B200 at the Qwen3 shape: 64 KiB stages x 2 beat 32 KiB x 3 by 5 % at batch 1
+// (larger TMA copies), but at batch 4 their 64 accumulators per thread spill.  The geometry (StreamGeom.RB) follows the same rule.
+template <int NP> struct StreamVals { static constexpr int V = NP <= 2 ? 16 : 8; };
+__host__ __device__ constexpr int stream_vals_for_tokens(int n_tokens) { return n_tokens <= 2 ? 16 : 8; }
 
 __device__ __forceinline__ float silu_f(float v) { return v / (1.0f + expf(-v)); }
 
@@ -90,7 +94,7 @@ struct StreamGeom {
   int row_bytes;         // K * sizeof(T)
   int P;                 // threads per row group = chunks per segment
   int G;                 // row groups per CTA (G * P <= 256)
-  int RB;                // rows per matrix per stage = (kStreamVals / n_mats) * G
+  int RB;                // rows per matrix per stage = (vals / n_mats) * G
   int NSEG;              // segments per row
   int seg_bytes;         // P * 16
   int stage_bytes;       // n_mats * RB * seg_bytes
@@ -196,9 +200,9 @@ __device__ __forceinline__ void stream_produce(const StreamArgs& a, const Stream
 
 // Accumulators per consumer thread between two reductions: 32 (64 for 8 pairs) = row blocks per batch x 8 rows x CNT,
 // CNT = routed pairs of the expert rounded up to 1, 2, 4 or 8.  The shared-memory scratch is sized for the kernel's NP.
-template <int CNT> struct StreamBatch {
-  static constexpr int SPU = CNT <= 4 ? 4 / CNT : 1;        // row blocks (ring stages per segment) per batch
-  static constexpr int NVAL = SPU * kStreamVals * CNT;      // values reduced per thread per batch
+template <int CNT, int V> struct StreamBatch {
+  static constexpr int SPU = (32 / V) / CNT > 0 ? (32 / V) / CNT : 1;   // row blocks (ring stages per segment) per batch
+  static constexpr int NVAL = SPU * V * CNT;                // values reduced per thread per batch
 };
 __device__ __forceinline__ int stream_cnt_class(int cnt) { return cnt <= 1 ? 1 : cnt <= 2 ? 2 : cnt <= 4 ? 4 : 8; }
 
@@ -208,13 +212,14 @@ __device__ __forceinline__ int stream_cnt_class(int cnt) { return cnt <= 1 ? 1 :
 // warps: ascending, through s_red) and one epilogue, so the block-wide barrier and the SiLU/store tail are paid once
 // per batch, not once per ring stage.  Batching changes which dot products are reduced together, never the summation
 // order inside one of them; an unused pair slot (cnt < CNT) multiplies by a zero operand and is never stored.
-template <typename T, int MODE, int CNT>
+template <typename T, int MODE, int CNT, int V>
 __device__ __forceinline__ void stream_consume_entry(const StreamArgs& a, const StreamGeom& gm, const Ring& ring, RingPos& rp,
                                                      int i, int u, int u_end, int cnt, const int* pl, float* s_red, int& par,
                                                      int red_bar) {
   constexpr int EPC = ChunkW<T>::N;                         // elements per 16-byte chunk
-  constexpr int SPU = StreamBatch<CNT>::SPU;
-  constexpr int NVAL = StreamBatch<CNT>::NVAL;
+  constexpr int kStreamVals = V;
+  constexpr int SPU = StreamBatch<CNT, V>::SPU;
+  constexpr int NVAL = StreamBatch<CNT, V>::NVAL;
   constexpr int RPT = kStreamVals / (MODE == 0 ? 2 : 1);    // rows per thread per matrix per row block
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid >= gm.n_active) {
@@ -403,10 +408,10 @@ __device__ __forceinline__ void stream_consume(const StreamArgs& a, const Stream
     const int cnt = min(a.plan.exp_count[e], NP);
     const int* pl = a.plan.pair_list + a.plan.exp_offset[e];
     const int cls = stream_cnt_class(cnt);
-    if (NP == 1 || cls == 1) stream_consume_entry<T, MODE, 1>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
-    else if (NP == 2 || cls == 2) stream_consume_entry<T, MODE, (NP >= 2 ? 2 : 1)>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
-    else if (NP == 4 || cls == 4) stream_consume_entry<T, MODE, (NP >= 4 ? 4 : 1)>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
-    else stream_consume_entry<T, MODE, (NP >= 8 ? 8 : 1)>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
+    if (NP == 1 || cls == 1) stream_consume_entry<T, MODE, 1, StreamVals<NP>::V>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
+    else if (NP == 2 || cls == 2) stream_consume_entry<T, MODE, (NP >= 2 ? 2 : 1), StreamVals<NP>::V>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
+    else if (NP == 4 || cls == 4) stream_consume_entry<T, MODE, (NP >= 4 ? 4 : 1), StreamVals<NP>::V>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
+    else stream_consume_entry<T, MODE, (NP >= 8 ? 8 : 1), StreamVals<NP>::V>(a, gm, ring, rp, i, u, u_end, cnt, pl, s_red, par, red_bar);
     u = u_end;
   }
   if (a.master != nullptr && threadIdx.x < 32) bulk_wait0();   // warp 0's slot writes are complete

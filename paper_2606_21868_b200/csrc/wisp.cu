@@ -79,7 +79,7 @@ struct wisp_ctx {
 
   std::map<int, cudaGraphExec_t> graphs;
   int grid_fetch = 0;
-  StreamGeom geom_gu{}, geom_dn{};   // decode FFN stream geometry (gate/up, down)
+  StreamGeom geom_gu[2]{}, geom_dn[2]{};   // decode FFN stream geometry (gate/up, down); [0]: <= 2 tokens (16 rows per thread per stage), [1]: more (8)
   // persistent decode kernel (decode_persistent.cuh)
   const char** d_masters = nullptr;  // device [L]: mapped master pointers
   unsigned* gbar = nullptr;          // grid barrier counter
@@ -291,7 +291,7 @@ int fetch_wave(wisp_ctx* ctx, int layer, int wave, bool host_known, cudaStream_t
 constexpr size_t kStreamSmemMax = 216u << 10;   // dynamic shared memory ceiling of the ring (227 KiB per CTA minus static)
 
 // ---- decode FFN (ffn_stream.cuh) -------------------------------------------------------------------------
-StreamGeom make_geom(int K, int rows, int n_mats, size_t elem, size_t off0, size_t off1, int want_stages) {
+StreamGeom make_geom(int K, int rows, int n_mats, size_t elem, size_t off0, size_t off1, int want_stages, int vals) {
   StreamGeom g{};
   g.K = K; g.rows = rows; g.n_mats = n_mats;
   g.mat_off[0] = off0; g.mat_off[1] = off1;
@@ -302,7 +302,7 @@ StreamGeom make_geom(int K, int rows, int n_mats, size_t elem, size_t off0, size
   g.P = 32 * q;
   g.NSEG = n_chunks / g.P;
   g.G = kStreamConsumers / g.P;
-  g.RB = (kStreamVals / n_mats) * g.G;
+  g.RB = (vals / n_mats) * g.G;
   g.seg_bytes = g.P * 16;
   g.stage_bytes = n_mats * g.RB * g.seg_bytes;
   g.upe = rows / g.RB;
@@ -360,13 +360,13 @@ int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, c
     {
       Span sp(ctx, WISP_K_GATE_UP, st);
       a.operand = x; a.result = ctx->act_f32; a.out_ld = dff;
-      rc = launch_stream_np<T, 0>(ctx, a, ctx->geom_gu, T_, st);
+      rc = launch_stream_np<T, 0>(ctx, a, ctx->geom_gu[T_ <= 2 ? 0 : 1], T_, st);
     }
     if (rc) return rc;
     {
       Span sp(ctx, WISP_K_DOWN, st);
       a.operand = ctx->act_f32; a.result = ctx->ystage; a.out_ld = d;
-      rc = launch_stream_np<T, 1>(ctx, a, ctx->geom_dn, T_, st);
+      rc = launch_stream_np<T, 1>(ctx, a, ctx->geom_dn[T_ <= 2 ? 0 : 1], T_, st);
     }
     if (rc) return rc;
   } else if (ctx->mma_ok) {
@@ -464,7 +464,8 @@ int launch_persistent_np(wisp_ctx* ctx, PersistArgs& pa, cudaStream_t st) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((227u << 10) - fa.sharedSizeBytes)));
     smem = (227u << 10) - fa.sharedSizeBytes;
   }
-  stride = std::max(ctx->geom_gu.stage_bytes, ctx->geom_dn.stage_bytes);
+  const int gi = pa.T <= 2 ? 0 : 1;
+  stride = std::max(ctx->geom_gu[gi].stage_bytes, ctx->geom_dn[gi].stage_bytes);
   int xs_bytes = (int)(((size_t)pa.T * pa.d * ctx->elem + 1023) & ~(size_t)1023);   // hidden state copy per CTA
   const int rows_per_cta = (pa.E + ctx->num_sms - 1) / ctx->num_sms;               // router rows staged per CTA
   int rw_bytes = (int)(((size_t)rows_per_cta * pa.d * ctx->elem + 1023) & ~(size_t)1023);
@@ -474,10 +475,10 @@ int launch_persistent_np(wisp_ctx* ctx, PersistArgs& pa, cudaStream_t st) {
   // Measured on B200 (Qwen3 shape, all-resident, 12 layers): 2 / 3 / 4 / 5 / 6 stages -> 0.581 / 0.577 / 0.578 / 0.593 / 0.597 ms
   // per token at batch 1 and 1.09 vs 1.24 ms (3 vs 6) at batch 4; no difference at the Mixtral shape.  A deeper ring lets
   // the producer run further into the down tiles while gate/up is still streaming, which costs more than it hides.
-  n_stages = std::min(n_stages, ctx->cfg.ring_stages > 0 ? (int)ctx->cfg.ring_stages : 3);
+  n_stages = std::min(n_stages, ctx->cfg.ring_stages > 0 ? (int)ctx->cfg.ring_stages : (gi == 0 ? 2 : 3));
   if (n_stages < 2) return fail(ctx, WISP_EINVAL, "persistent decode kernel: ring does not fit shared memory");
   CK(cudaMemsetAsync(ctx->gbar, 0, sizeof(unsigned), st));
-  StreamGeom ggu = ctx->geom_gu, gdn = ctx->geom_dn;
+  StreamGeom ggu = ctx->geom_gu[gi], gdn = ctx->geom_dn[gi];
   void* args[] = {&pa, &ggu, &gdn, &n_stages, &stride, &xs_bytes, &rw_bytes};
   CK(cudaLaunchCooperativeKernel((const void*)kern, dim3(ctx->num_sms), dim3(kStreamThreads), args,
                                  (size_t)xs_bytes + rw_bytes + (size_t)n_stages * stride, st));
@@ -714,8 +715,11 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
 #undef CKC
   {
     const size_t gu = (size_t)d * dff * ctx->elem;
-    ctx->geom_gu = make_geom(d, dff, 2, ctx->elem, 0, gu, cfg->ring_stages);
-    ctx->geom_dn = make_geom(dff, d, 1, ctx->elem, 2 * gu, 0, cfg->ring_stages);
+    for (int gi = 0; gi < 2; ++gi) {
+      const int vals = stream_vals_for_tokens(gi == 0 ? 1 : kDecodeMaxTokens);
+      ctx->geom_gu[gi] = make_geom(d, dff, 2, ctx->elem, 0, gu, cfg->ring_stages, vals);
+      ctx->geom_dn[gi] = make_geom(dff, d, 1, ctx->elem, 2 * gu, 0, cfg->ring_stages, vals);
+    }
   }
   ctx->grid_fetch = ctx->num_sms * 2;
   ctx->mma_ok = setup_mma_path(ctx);
