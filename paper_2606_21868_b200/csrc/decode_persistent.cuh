@@ -13,7 +13,8 @@
 //   phase D  down                     written into its victim slot on the way (Alg. 1 line 6).  The
 //                                     producer warp runs ahead: down tiles land in the ring while the CTA waits at
 //                                     barrier C for the other CTAs' act rows                      -> barriers C, D
-//   phase X  combine (+ residual)     every CTA recomputes x_{l+1} into its own shared memory (combine_elem): no barrier
+//   phase X  combine (+ residual)     split over the grid (combine_elem's sum), x_{l+1} via global memory -> barrier E,
+//                                     then every CTA reloads x_{l+1} into its shared memory
 //
 // Every arithmetic step calls the same device function as the multi-kernel path (router_row_warp,
 // topk_softmax_block, plan_compute, stream_consume, combine_elem), so both paths give the same bits (parity (b)).
@@ -304,19 +305,17 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
 #endif
     }
 
-    // ---- phase X: ordered combine (+ residual) ----
-    // One token: every CTA recomputes the whole x_{l+1} into its own xs (64 KiB of L2 reads, no grid barrier).  More
-    // tokens: that redundant read (T x 64 KiB per CTA from the same L2 lines) costs more than a barrier, so the work is
-    // split over the grid, x_{l+1} goes through global memory and one grid barrier, and every CTA reloads it into xs.
+    // ---- phase X: ordered combine (+ residual), split over the grid ----
+    // x_{l+1} goes through global memory and one grid barrier, then every CTA reloads it into its xs.  (Recomputing the whole
+    // x_{l+1} in every CTA saves the barrier but makes 148 CTAs read the same T x 64 KiB of ystage from L2: measured slower, 490 vs
+    // 500 tokens/s at one token, 674 vs 764 at four.)
     {
       const int n = T_ * d;
       const bool last = l == a.layer_hi - 1;
-      const bool split = T_ > 1;
       T* xg = reinterpret_cast<T*>(last ? a.out : a.xbuf[(l - a.layer_lo) & 1]);
       // 4 consecutive elements per thread; the ystage loads of up to 8 ranks are issued together (one L2 round trip),
       // the sum itself is combine_elem's: fmaf in rank order from 0.f, per element.
-      for (int v4 = split ? (int)blockIdx.x * kStreamConsumers + tid : tid; v4 < n / 4;
-           v4 += split ? (int)gridDim.x * kStreamConsumers : kStreamConsumers) {
+      for (int v4 = (int)blockIdx.x * kStreamConsumers + tid; v4 < n / 4; v4 += (int)gridDim.x * kStreamConsumers) {
         const int idx = v4 * 4, t = idx / d, j = idx % d;
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
         for (int i0 = 0; i0 < k; i0 += 8) {
@@ -335,15 +334,10 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           const T o = from_f32<T>(acc[c]);
-          const T v = a.residual ? from_f32<T>(to_f32<T>(xs[idx + c]) + to_f32<T>(o)) : o;
-          if (split) xg[idx + c] = v;
-          else {
-            xs[idx + c] = v;
-            if (last && v4 % (int)gridDim.x == (int)blockIdx.x) xg[idx + c] = v;
-          }
+          xg[idx + c] = a.residual ? from_f32<T>(to_f32<T>(xs[idx + c]) + to_f32<T>(o)) : o;
         }
       }
-      if (split && !last) {
+      if (!last) {
         grid_barrier(a.gbar, gen, a.err);                                    // E: x_{l+1} complete in global memory
         const uint4* src = reinterpret_cast<const uint4*>(xg);
         uint4* dst = reinterpret_cast<uint4*>(xs);
