@@ -14,6 +14,10 @@ paper leaves open are those of SURVEY.md §8(c) / DESIGN.md:
       to the paper's re-page from host)
   G20 a reference = one (layer, step, distinct expert); hit iff resident when its wave begins
   G24 one tick per wave shared by all of R_w
+  G25 wave order (PAPER.md:112 calls overflow handling an implementation detail):
+      ASCENDING = G5; HITS_FIRST = only when |R| > C, R is listed as (members resident when the step
+      begins, ascending id) followed by (the faults, ascending id) before it is cut into waves, so a
+      resident member is never evicted by an earlier wave of the same step.  |R| <= C: identical to G5.
 """
 from __future__ import annotations
 
@@ -21,6 +25,7 @@ from dataclasses import dataclass, field
 
 HIT, MISS, RESIZE_DROP, RESIZE_MOVE = 0, 1, 2, 3
 LRU, LFU = 0, 1
+ASCENDING, HITS_FIRST = 0, 1
 
 
 @dataclass
@@ -41,6 +46,7 @@ class PagerLayer:
     C: int
     E: int
     policy: int = LRU
+    wave_order: int = ASCENDING
     pi: dict = field(default_factory=dict)        # expert -> slot
     pi_inv: list = field(default_factory=list)    # slot -> expert or None
     tau: list = field(default_factory=list)       # per-slot LRU tick
@@ -70,6 +76,8 @@ class PagerLayer:
         R = sorted(set(int(e) for e in routed))
         if not R:
             return []                                   # n_tokens = 0: no-op, no tick (G23)
+        if self.wave_order == HITS_FIRST and len(R) > self.C:      # G25
+            R = [e for e in R if e in self.pi] + [e for e in R if e not in self.pi]
         events: list[Event] = []
         step_no = self.steps
         for wv, lo in enumerate(range(0, len(R), self.C)):
@@ -99,7 +107,7 @@ class PagerLayer:
             self.hits += len(hit_set)
             self.misses += len(M)
             self.references += len(Rw)
-            for e in Rw:                                 # ascending expert id within the wave
+            for e in Rw:                                 # wave order (ascending expert id under G5)
                 if e in assign:
                     events.append(Event(step_no, wv, e, assign[e][0], assign[e][1], MISS))
                 else:

@@ -5,7 +5,7 @@ import pytest
 
 from golden_util import num, read_golden
 from oracle import mvwsa
-from oracle.paging import HIT, LFU, LRU, MISS, RESIZE_DROP, RESIZE_MOVE, PagerLayer
+from oracle.paging import ASCENDING, HITS_FIRST, HIT, LFU, LRU, MISS, RESIZE_DROP, RESIZE_MOVE, PagerLayer
 
 TR = read_golden("hand_paging_trace.txt")
 STEPS = [{1, 4}, {1, 2}, {3, 5}, {1, 2}, {2, 3}, {0, 4}]
@@ -52,6 +52,67 @@ def test_p4_overflow_waves():
     ev = p.step([3, 5])
     _, sl, ta = _parse_step(sec["step1"])
     assert sum(e.kind == HIT for e in ev) == num(sec["step1_hits"]) and p.slots() == sl and p.tau == ta
+
+
+def test_g25_hits_first_hand_trace():
+    """G25, stepped by hand in tests/golden/hand_paging_trace.txt [hits_first]."""
+    sec = TR["hits_first"]
+    steps = [{4, 5}, {0, 1, 5}, {1, 5}]
+    p = PagerLayer(C=2, E=6, policy=LRU, wave_order=HITS_FIRST)
+    for i, R in enumerate(steps):
+        ev = p.step(R)
+        m, sl, ta = _parse_step(sec[f"step{i}"])
+        assert [(e.expert, e.slot, e.evicted) for e in ev if e.kind == MISS] == m
+        assert p.slots() == sl and p.tau == ta
+        if i == 1:
+            assert [e.expert for e in ev] == [int(t) for t in sec["step1_order"].split()]
+            assert [e.wave for e in ev] == [int(t) for t in sec["step1_waves"].split()]
+        p.check_invariants()
+    assert p.hits == num(sec["hits"]) and p.misses == num(sec["misses"])
+    q = PagerLayer(C=2, E=6, policy=LRU, wave_order=ASCENDING)
+    for i, R in enumerate(steps):
+        ev = q.step(R)
+        if i == 1:
+            m, sl, ta = _parse_step(sec["ascending_step1"])
+            assert [(e.expert, e.slot, e.evicted) for e in ev if e.kind == MISS] == m
+            assert q.slots() == sl and q.tau == ta
+    assert q.hits == num(sec["ascending_hits"]) and q.misses == num(sec["ascending_misses"])
+
+
+@pytest.mark.parametrize("policy", [LRU, LFU])
+def test_g25_hits_first_closed_form_random_streams(policy):
+    """Under HITS_FIRST the faults of a step are exactly R minus the residents at step start (set arithmetic,
+    not the oracle's loop); ASCENDING can only fault more on the same state; |R| <= C gives the same trace."""
+    rng = random.Random(11)
+    for trial in range(40):
+        E = rng.randint(3, 40)
+        C = rng.randint(1, E)
+        k = rng.randint(1, min(E, 12))
+        hf = PagerLayer(C=C, E=E, policy=policy, wave_order=HITS_FIRST)
+        for t in range(50):
+            R = set(rng.sample(range(E), rng.randint(1, k)))
+            resident = set(hf.pi)
+            asc = PagerLayer(C=C, E=E, policy=policy)          # same state, ascending order, one step
+            asc.pi, asc.pi_inv, asc.tau, asc.f, asc.c, asc.steps = dict(hf.pi), list(hf.pi_inv), list(hf.tau), list(hf.f), hf.c, hf.steps
+            ev = hf.step(R)
+            ev_a = asc.step(R)
+            assert sorted(e.expert for e in ev) == sorted(R)
+            assert {e.expert for e in ev if e.kind == MISS} == R - resident
+            assert {e.expert for e in ev if e.kind == HIT} == R & resident
+            assert sum(e.kind == MISS for e in ev_a) >= len(R - resident)
+            if len(R) <= C:
+                assert [e.key() for e in ev] == [e.key() for e in ev_a]
+            else:
+                n_res = len(R & resident)
+                assert [e.expert for e in ev] == sorted(R & resident) + sorted(R - resident)
+                assert all(e.wave == 0 for e in ev[:n_res])
+            for wv in set(e.wave for e in ev):
+                sl = [e.slot for e in ev if e.wave == wv]
+                assert len(set(sl)) == len(sl) <= C
+                evicted = {e.evicted for e in ev if e.wave == wv and e.evicted >= 0}
+                assert not evicted & {e.expert for e in ev if e.wave == wv}
+            hf.check_invariants()
+        assert hf.hits + hf.misses == hf.references
 
 
 def test_p3_fig4_printed_fault_counts():
