@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--budget-gib", type=float, default=0.0, help="expert-pool budget (0 = the config's)")
     ap.add_argument("--batch", type=int, default=1)
     ap.add_argument("--policy", default="lru", choices=["lru", "lfu"])
+    ap.add_argument("--wave-order", default="ascending", choices=["ascending", "hits-first"],
+                    help="overflow wave order (wisp_set_wave_order, DESIGN.md G25); only matters when |R| > C")
     ap.add_argument("--fetch", default="fused", choices=["fused", "zerocopy", "memcpy"],
                     help="miss path: fused = persistent decode kernel whose TMA producer reads misses from the mapped master")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -163,6 +165,8 @@ def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=N
                   policy=wp.WISP_LFU if args.policy == "lfu" else wp.WISP_LRU,
                   fetch={"memcpy": wp.WISP_FETCH_MEMCPY, "zerocopy": wp.WISP_FETCH_ZEROCOPY, "fused": wp.WISP_FETCH_FUSED}[fetch or args.fetch],
                   ring_stages=getattr(args, "ring_stages", 0))
+    if getattr(args, "wave_order", "ascending") == "hits-first":
+        ctx.set_wave_order(wp.WISP_WAVES_HITS_FIRST)
     staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
     for l in (register_layers if register_layers is not None else range(shape.n_layers)):
         si.gen_layer_experts(shape, l, gen_device, out=staging)
@@ -688,7 +692,7 @@ def main_ours(args):
             "vs_baseline": None, "dtype": "bf16" if shape.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": f"{shape.name} decode, batch {B}, {shape.n_layers} layers, E={shape.n_experts}, top-{shape.top_k}, "
                                    f"d={shape.d_model}, d_ff={shape.d_ff}, expert pool {budget / GIB:.3f} GiB -> C={C} slots/layer, "
-                                   f"{args.policy.upper()}, fetch={args.fetch}",
+                                   f"{args.policy.upper()}, fetch={args.fetch}" + (", waves=hits-first" if args.wave_order == "hits-first" else ""),
                        "api": "wisp_moe_forward per layer" if args.per_layer_api else ("wisp_stack_forward (one persistent cooperative kernel per token)" if args.fetch == "fused" else "wisp_stack_forward (CUDA graph per token)"),
                        "l2": f"weights streamed per step {avg_R * shape.n_layers * shape.expert_bytes / GIB:.2f} GiB >> 126 MB L2 (no flush needed)",
                        "layers_reduced_for_host_ram": reduced, "full_config_layers": full_layers, "parallelism": "replicas" if world > 1 else "single"},

@@ -55,6 +55,12 @@ typedef enum { WISP_LRU = 0, WISP_LFU = 1 } wisp_policy;
  * pinned master, computes on them and writes them into the victim slot (same bytes, same summation order as
  * a hit, so outputs stay byte-identical).  Prefill calls (n_tokens > 8) under FUSED use the ZEROCOPY kernel. */
 typedef enum { WISP_FETCH_MEMCPY = 0, WISP_FETCH_ZEROCOPY = 1, WISP_FETCH_FUSED = 2 } wisp_fetch;
+/* Order in which an overflowing step (|R| > C) is cut into waves of at most C experts (PAPER.md:112 leaves overflow
+ * handling to the implementation; G5 / G25).  ASCENDING (default) = ascending expert id.  HITS_FIRST = the
+ * members of R resident when the step begins (ascending id) come first, then the faults (ascending id): a resident
+ * member is never evicted by an earlier wave of its own step, so the step faults exactly |R \ dom(pi)| times.
+ * Steps with |R| <= C are identical under both.  Outputs never depend on the order. */
+typedef enum { WISP_WAVES_ASCENDING = 0, WISP_WAVES_HITS_FIRST = 1 } wisp_wave_order;
 
 typedef struct {
   int32_t n_layers;   /* L */
@@ -104,7 +110,8 @@ enum { WISP_K_ROUTER = 0, WISP_K_TOPK = 1, WISP_K_RESIDENCY = 2, WISP_K_FETCH = 
        WISP_N_KERNEL_CLASSES = 12 };
 
 /* kind: 0 hit, 1 miss, 2 resize-drop, 3 resize-move (for a move `evicted` carries the source slot).
- * Events of one wave are emitted in ascending expert id; waves in order; layers/steps in call order. */
+ * Events of one wave are emitted in wave order (ascending expert id; under WISP_WAVES_HITS_FIRST an overflowing step
+ * lists residents, then faults, each ascending); waves in order; layers/steps in call order. */
 typedef struct {
   uint64_t step;   /* per-layer step counter (0-based) */
   uint32_t layer;
@@ -188,6 +195,9 @@ int wisp_residual_add(wisp_ctx* ctx, const void* x, const void* y, void* out, in
 int wisp_layer_stats_read(wisp_ctx* ctx, int32_t layer, wisp_layer_stats* out);
 /* Trace ring: when on, every reference / resize action appends one wisp_trace_event. */
 int wisp_trace_enable(wisp_ctx* ctx, int32_t on);
+/* Select the overflow wave order (wisp_wave_order) for all later forwards.  Synchronises the device; residency state,
+ * counters and slot contents are kept.  Errors: EINVAL (NULL ctx or unknown order; state unchanged). */
+int wisp_set_wave_order(wisp_ctx* ctx, int32_t order);
 /* Drain up to `cap` events into host `buf` (oldest first); *n_out = number written.  Synchronises. */
 int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t* n_out);
 /* Routing of the most recent forward of `layer`: host ids [n_tokens, k] (rank order) and w [n_tokens, k].

@@ -11,6 +11,7 @@ _LIB = None
 WISP_F32, WISP_BF16 = 0, 1
 WISP_LRU, WISP_LFU = 0, 1
 WISP_FETCH_MEMCPY, WISP_FETCH_ZEROCOPY, WISP_FETCH_FUSED = 0, 1, 2
+WISP_WAVES_ASCENDING, WISP_WAVES_HITS_FIRST = 0, 1
 KERNEL_CLASSES = ("router", "topk", "residency", "fetch", "gate_up", "down", "combine", "prefill_gate_up",
                   "prefill_down", "other", "gate_up_miss", "down_miss")
 N_KERNEL_CLASSES = len(KERNEL_CLASSES)
@@ -67,6 +68,7 @@ _SIGS = {
     "wisp_residual_add": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]),
     "wisp_layer_stats_read": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(WispLayerStats)]),
     "wisp_trace_enable": (C.c_int, [C.c_void_p, C.c_int32]),
+    "wisp_set_wave_order": (C.c_int, [C.c_void_p, C.c_int32]),
     "wisp_trace_read": (C.c_int, [C.c_void_p, C.POINTER(WispTraceEvent), C.c_uint64, C.POINTER(C.c_uint64)]),
     "wisp_last_topk": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]),
     "wisp_last_logits": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32]),
@@ -165,6 +167,9 @@ class Wisp:
 
     def trace_enable(self, on=True):
         self._ck(self.L.wisp_trace_enable(self.ctx, int(on)), "wisp_trace_enable")
+
+    def set_wave_order(self, order):
+        self._ck(self.L.wisp_set_wave_order(self.ctx, int(order)), "wisp_set_wave_order")
 
     def trace_read(self, cap=1 << 20):
         buf = (WispTraceEvent * cap)()

@@ -32,6 +32,7 @@ constexpr unsigned kGridBarrierSpinLimit = 1u << 26;
 
 struct PersistArgs {
   int L, E, k, d, dff, T, C, policy;
+  int wave_order;               // wisp_wave_order (G25)
   int layer_lo, layer_hi;
   int residual;                 // 1: x_{l+1} = x_l + y_l chained through xbuf, `out` = x_hi; 0: out = y (one layer)
   int fused;                    // misses are read from the mapped master by the FFN producer
@@ -239,7 +240,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) decode_persistent_kernel(co
       pa.ids = s_ids; pa.n_pairs = T_ * k; pa.E = E; pa.C = C; pa.policy = a.policy; pa.layer = l;
       pa.st = st; pa.plan = pp; pa.host_plan = nullptr;
       pa.trace = a.trace; pa.trace_ctr = a.trace_ctr; pa.trace_cap = a.trace_cap; pa.trace_on = a.trace_on;
-      pa.track = a.track; pa.build_pairs = 1;
+      pa.track = a.track; pa.build_pairs = 1; pa.wave_order = a.wave_order;
       plan_compute<kPersistMaxExperts>(pa, sh, writer, 1);
     }
     if (tid == 0) mbar_arrive(smem_u32(&s_plan_ready));                      // the producer may start streaming

@@ -4,7 +4,8 @@
 //
 // Readings: G1 M = R \ dom(pi); G2 ties -> lower slot; G3 M ascending id <-> U in key order;
 // G4 empty slots (tau = 0) first; G5 waves of <= C ascending ids; G6 LFU key (f, tau, slot), empty f = -1;
-// G24 one tick per wave.
+// G24 one tick per wave; G25 wave order: WISP_WAVES_HITS_FIRST lists R as (residents at step start, ascending id)
+// then (faults, ascending id) when |R| > C (overflow handling is an implementation detail).
 #pragma once
 #include "common.cuh"
 
@@ -25,6 +26,7 @@ struct PlanArgs {
   int trace_on;
   int track;                      // MV-WSA reuse-distance tracking
   int build_pairs;                // build pair_list here (small n_pairs) or leave it to group_pairs_kernel
+  int wave_order;                 // wisp_wave_order (G25)
 };
 
 // ---- Algorithm 1 as a device function, usable by a standalone CTA (NT = 1024 threads) and by every CTA of the
@@ -169,6 +171,16 @@ __device__ __forceinline__ void plan_compute(const PlanArgs& a, PlanShared<NT>& 
     plan_sync<NT>(bar);
     if (tid < nR) a.st.last_pos[sh.R[tid]] = base + 1 + tid;
     if (tid == 0) a.st.scal[6] = base + nR;
+    plan_sync<NT>(bar);
+  }
+
+  // ---- G25: hits-first listing of R (only when the step overflows; one wave gives the same plan either way) ----
+  if (a.wave_order == WISP_WAVES_HITS_FIRST && nR > C) {
+    const int e = tid < nR ? sh.R[tid] : -1;
+    const int res = (e >= 0 && sh.pi[e] >= 0) ? 1 : 0;
+    int n_res;
+    const int ri = block_excl_scan<NT>(res, sh.ws, n_res, bar);   // ends with a barrier: every R[tid] has been read
+    if (e >= 0) sh.R[res ? ri : n_res + (tid - ri)] = e;
     plan_sync<NT>(bar);
   }
 

@@ -63,6 +63,7 @@ struct wisp_ctx {
   u64* trace_ctr = nullptr;        // device [2]
   u64 trace_cap = 0;
   int trace_on = 0;
+  int wave_order = WISP_WAVES_ASCENDING;   // G25
   int track = 0;
   std::vector<double> host_hist;
 
@@ -238,6 +239,7 @@ int launch_plan(wisp_ctx* ctx, int layer, const int* ids, int n_pairs, bool want
   a.trace_ctr = ctx->trace_ctr;
   a.trace_cap = ctx->trace_cap;
   a.trace_on = ctx->trace_on;
+  a.wave_order = ctx->wave_order;
   a.track = ctx->track;
   a.build_pairs = n_pairs <= 256;
   {
@@ -501,6 +503,7 @@ int launch_persistent(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void
   pa.x_in = x; pa.xbuf[0] = ctx->xbuf[0]; pa.xbuf[1] = ctx->xbuf[1]; pa.out = out;
   pa.gbar = ctx->gbar; pa.err = ctx->dev_err;
   pa.trace = ctx->trace; pa.trace_ctr = ctx->trace_ctr; pa.trace_cap = ctx->trace_cap; pa.trace_on = ctx->trace_on;
+  pa.wave_order = ctx->wave_order;
   pa.track = ctx->track;
   pa.phase_ns = ctx->timing_level >= 2 ? ctx->phase_ns : nullptr;
   int rc;
@@ -949,6 +952,16 @@ int wisp_trace_enable(wisp_ctx* ctx, int32_t on) {
   return WISP_OK;
 }
 
+int wisp_set_wave_order(wisp_ctx* ctx, int32_t order) {
+  if (!ctx) return WISP_EINVAL;
+  if (order != WISP_WAVES_ASCENDING && order != WISP_WAVES_HITS_FIRST)
+    return fail(ctx, WISP_EINVAL, "wisp_set_wave_order: order must be WISP_WAVES_ASCENDING or WISP_WAVES_HITS_FIRST");
+  CK(cudaDeviceSynchronize());
+  ctx->wave_order = order;
+  drop_graphs(ctx);   // kernel argument baked into captured graphs
+  return WISP_OK;
+}
+
 int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t* n_out) {
   if (!ctx || !n_out || (cap && !buf)) return fail(ctx, WISP_EINVAL, "bad argument");
   CK(cudaDeviceSynchronize());
@@ -1005,7 +1018,7 @@ int wisp_debug_step_routing(wisp_ctx* ctx, int32_t layer, const int32_t* ids, in
   a.ids = ctx->dbg_ids; a.n_pairs = n_ids; a.E = ctx->cfg.n_experts; a.C = ctx->C; a.policy = ctx->cfg.policy; a.layer = layer;
   a.st = layer_state(ctx, layer); a.plan = ctx->plan; a.host_plan = ctx->host_plan;
   a.trace = ctx->trace; a.trace_ctr = ctx->trace_ctr; a.trace_cap = ctx->trace_cap; a.trace_on = ctx->trace_on;
-  a.track = ctx->track; a.build_pairs = 0;
+  a.track = ctx->track; a.build_pairs = 0; a.wave_order = ctx->wave_order;
   residency_plan_kernel<<<1, kPlanThreads>>>(a);
   CK(cudaGetLastError());
   CK(cudaDeviceSynchronize());

@@ -17,7 +17,7 @@ def model(shape):
 
 
 def make_ctx(shape, slots=None, *, budget=None, policy=0, fetch=1, max_tokens=8, kv_block_bytes=0, kv_floor_blocks=0,
-             trace=True, trace_capacity=0):
+             trace=True, trace_capacity=0, wave_order=0):
     import paper_2606_21868_b200 as wp
     if budget is None:
         budget = slots * shape.slot_unit_bytes + kv_floor_blocks * kv_block_bytes
@@ -30,6 +30,8 @@ def make_ctx(shape, slots=None, *, budget=None, policy=0, fetch=1, max_tokens=8,
         ctx.register_host_experts(l, experts[l], routers[l][0], routers[l][1])
     if trace:
         ctx.trace_enable(True)
+    if wave_order:
+        ctx.set_wave_order(wave_order)
     return ctx
 
 
@@ -72,11 +74,11 @@ def run_stack(ctx, shape, hidden):
     return outs
 
 
-def sim_trace(shape, slots, policy, routed_per_step_layer, resize_at=None):
+def sim_trace(shape, slots, policy, routed_per_step_layer, resize_at=None, wave_order=0):
     """Oracle O4 simulation fed the GPU's routing.  routed_per_step_layer[t][l] = iterable of ids.
     Returns events as tuples matching Wisp.trace_read()."""
     from oracle.paging import PagerLayer
-    pagers = [PagerLayer(C=slots, E=shape.n_experts, policy=policy) for _ in range(shape.n_layers)]
+    pagers = [PagerLayer(C=slots, E=shape.n_experts, policy=policy, wave_order=wave_order) for _ in range(shape.n_layers)]
     ev = []
     for t, per in enumerate(routed_per_step_layer):
         for l, ids in enumerate(per):

@@ -76,6 +76,24 @@ def test_qwen3_shape_batch4_decode():
         else:
             assert_same_bytes(ref, res)
         ctx.close()
+    # G25: hits-first waves at the same shape (C = 9 < |R|), multi-kernel path and persistent kernel
+    want, pagers = sim_trace(shape, 9, 0, routed, wave_order=1)
+    _, asc = sim_trace(shape, 9, 0, routed)
+    assert sum(p.misses for p in pagers) < sum(p.misses for p in asc)
+    ctx = make_ctx(shape, 9, fetch=2, max_tokens=4, wave_order=1)
+    assert_same_bytes(ref, run_chain(ctx, shape, hidden))
+    assert ctx.trace_read() == want
+    ctx.close()
+    ctx = make_ctx(shape, 128, fetch=2, max_tokens=4, trace=False)
+    ref_stack = run_stack(ctx, shape, hidden)
+    ctx.close()
+    ctx = make_ctx(shape, 9, fetch=2, max_tokens=4, wave_order=1)
+    got = run_stack(ctx, shape, hidden)
+    assert all(torch.equal(a.view(torch.uint8), b.view(torch.uint8)) for a, b in zip(ref_stack, got))
+    assert ctx.trace_read() == want
+    for l in range(shape.n_layers):
+        assert ctx.debug_verify_pool(l) == 0
+    ctx.close()
 
 
 def test_qwen3_shape_prefill_sampled_tokens():

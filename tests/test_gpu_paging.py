@@ -48,6 +48,48 @@ def test_adversarial_routing_trace_and_state(C, policy, fetch):
         ctx.close()
 
 
+@pytest.mark.parametrize("C", [1, 2, 6, 15])
+@pytest.mark.parametrize("policy", [0, 1])
+@pytest.mark.parametrize("fetch", [0, 2])
+def test_hits_first_wave_order_trace_and_state(C, policy, fetch):
+    """G25 (SURVEY.md 8(f) f1): wisp_set_wave_order(HITS_FIRST) against the oracle's hits-first simulation, bit-exact;
+    the step's faults are exactly R minus the residents at step start."""
+    E = SH.n_experts
+    for name, steps in streams(E, C, 3):
+        ctx = make_ctx(SH, C, policy=policy, fetch=fetch, wave_order=1)
+        pager = PagerLayer(C=C, E=E, policy=policy, wave_order=1)
+        want, closed_form_misses = [], 0
+        for R in steps:
+            closed_form_misses += len(set(R) - set(pager.pi))
+            ctx.debug_step_routing(1, R)
+            want += [(1, e.step, e.wave, e.expert, e.slot, e.evicted, e.kind) for e in pager.step(R)]
+        assert ctx.trace_read() == want, name
+        pi_inv, tau, freq, clock = ctx.debug_residency(1)
+        assert pi_inv.tolist() == [-1 if e is None else e for e in pager.pi_inv]
+        assert tau.tolist() == pager.tau and freq.tolist() == pager.f and clock == pager.c
+        assert ctx.debug_verify_pool(1) == 0, name
+        s = ctx.layer_stats(1)
+        assert (s.hits, s.misses, s.evictions, s.references, s.steps) == (pager.hits, pager.misses, pager.evictions, pager.references, pager.steps)
+        assert s.misses == closed_form_misses
+        ctx.close()
+
+
+def test_set_wave_order_errors_and_switch_back():
+    ctx = make_ctx(SH, 2)
+    import paper_2606_21868_b200 as wp
+    with pytest.raises(wp.WispError):
+        ctx.set_wave_order(7)
+    pager = PagerLayer(C=2, E=SH.n_experts)
+    want = []
+    for order, R in ((1, [4, 5]), (1, [0, 1, 5]), (0, [0, 1, 5, 7]), (1, [2, 5, 7])):
+        ctx.set_wave_order(order)
+        pager.wave_order = order
+        ctx.debug_step_routing(0, R)
+        want += [(0, e.step, e.wave, e.expert, e.slot, e.evicted, e.kind) for e in pager.step(R)]
+    assert ctx.trace_read() == want
+    ctx.close()
+
+
 @pytest.mark.parametrize("policy", [0, 1])
 def test_resize_cycle_outputs_unchanged_and_trace(policy):
     """PAPER.md:261 (D2): shrink/grow cycle leaves outputs byte-identical; trace == simulation of the same resize."""

@@ -109,6 +109,55 @@ def test_batch_decode_overflow_waves(T):
         ctx.close()
 
 
+@pytest.mark.parametrize("T", [4, 8])
+def test_hits_first_waves_outputs_unchanged(T):
+    """G25: the wave order never changes outputs, the trace equals the hits-first simulation, and an
+    overflowing workload faults no more than under ascending waves.  Multi-kernel path and persistent kernel."""
+    shape = si.TINY
+    hidden = si.gen_decode_hidden(shape, 12, T)
+    ctx = make_ctx(shape, 16, max_tokens=T)
+    ref = run_chain(ctx, shape, hidden)
+    ctx.close()
+    ctx = make_ctx(shape, 16, max_tokens=T, fetch=2)
+    ref_stack = run_stack(ctx, shape, hidden)
+    ctx.close()
+    routed = [[rec["ids"].flatten().tolist() for rec in per] for per in ref]
+    for slots, fetch in ((5, 1), (5, 2), (1, 2), (3, 0)):
+        want, pagers = sim_trace(shape, slots, 0, routed, wave_order=1)
+        _, asc = sim_trace(shape, slots, 0, routed)
+        assert sum(p.misses for p in pagers) <= sum(p.misses for p in asc)
+        ctx = make_ctx(shape, slots, max_tokens=T, fetch=fetch, wave_order=1)
+        assert_same_bytes(ref, run_chain(ctx, shape, hidden))
+        assert ctx.trace_read() == want
+        for l in range(shape.n_layers):
+            assert ctx.debug_verify_pool(l) == 0
+        ctx.close()
+        ctx = make_ctx(shape, slots, max_tokens=T, fetch=fetch, wave_order=1)
+        got = run_stack(ctx, shape, hidden)
+        assert all(torch.equal(a.view(torch.uint8), b.view(torch.uint8)) for a, b in zip(ref_stack, got))
+        assert ctx.trace_read() == want
+        ctx.close()
+
+
+def test_hits_first_prefill_outputs_unchanged():
+    shape, T = MED, 96
+    hidden = si.gen_prefill_hidden(shape, T).view(1, T, shape.d_model)
+    ctx = make_ctx(shape, shape.n_experts, max_tokens=T)
+    ref = run_chain(ctx, shape, hidden)
+    ctx.close()
+    routed = [[rec["ids"].flatten().tolist() for rec in per] for per in ref]
+    for slots, fetch in ((5, 1), (3, 2)):
+        # two passes over the same batch: the second starts with residents, where the two orders differ
+        ctx = make_ctx(shape, slots, fetch=fetch, max_tokens=T, wave_order=1)
+        assert_same_bytes(ref, run_chain(ctx, shape, hidden))
+        assert_same_bytes(ref, run_chain(ctx, shape, hidden))
+        want, pagers = sim_trace(shape, slots, 0, routed + routed, wave_order=1)
+        _, asc = sim_trace(shape, slots, 0, routed + routed)
+        assert ctx.trace_read() == want
+        assert sum(p.misses for p in pagers) < sum(p.misses for p in asc)
+        ctx.close()
+
+
 @pytest.mark.parametrize("shape,T", [(si.TINY, 40), (MED, 96)])
 def test_prefill_grouped_path(shape, T):
     hidden = si.gen_prefill_hidden(shape, T).view(1, T, shape.d_model)
