@@ -457,6 +457,8 @@ def main_mvwsa(args):
     ctx = wp.Wisp(B, n_layers=shape.n_layers, n_experts=shape.n_experts, top_k=shape.top_k, d_model=shape.d_model, d_ff=shape.d_ff,
                   max_tokens=2048, dtype=wp.WISP_BF16, policy=wp.WISP_LRU, fetch=wp.WISP_FETCH_FUSED, kv_block_bytes=b,
                   kv_floor_blocks=floor_blocks)
+    if args.wave_order == "hits-first":
+        ctx.set_wave_order(wp.WISP_WAVES_HITS_FIRST)
     staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
     for l in range(shape.n_layers):
         si.gen_layer_experts(shape, l, "cuda", out=staging)
@@ -478,7 +480,8 @@ def main_mvwsa(args):
     line = {"metric": "mvwsa_e2e_seconds", "value": live["e2e_s"] if live else None, "unit": "s", "n_gpus": 1, "higher_is_better": False,
             "dtype": "bf16", "data": "synthetic",
             "config": {"workload": f"config 5: {shape.name}, {shape.n_layers} layers, B = 12 GiB shared by expert slots and KV reservations, "
-                                   f"4 requests, prompts {prompts}, {n_decode} decode steps each, KV floor {floor_blocks} blocks"},
+                                   f"4 requests, prompts {prompts}, {n_decode} decode steps each, KV floor {floor_blocks} blocks"
+                                   + (", waves=hits-first" if args.wave_order == "hits-first" else "")},
             "live_vs_fixed_50": round(base["e2e_s"] / live["e2e_s"], 3) if base and live else None, "arms": arms}
     print(json.dumps(line))
 
