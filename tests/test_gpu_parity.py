@@ -109,8 +109,9 @@ def test_batch_decode_overflow_waves(T):
         ctx.close()
 
 
+@pytest.mark.parametrize("policy", [0, 1])
 @pytest.mark.parametrize("T", [4, 8])
-def test_hits_first_waves_outputs_unchanged(T):
+def test_hits_first_waves_outputs_unchanged(T, policy):
     """G25: the wave order never changes outputs, the trace equals the hits-first simulation, and an
     overflowing workload faults no more than under ascending waves.  Multi-kernel path and persistent kernel."""
     shape = si.TINY
@@ -123,16 +124,17 @@ def test_hits_first_waves_outputs_unchanged(T):
     ctx.close()
     routed = [[rec["ids"].flatten().tolist() for rec in per] for per in ref]
     for slots, fetch in ((5, 1), (5, 2), (1, 2), (3, 0)):
-        want, pagers = sim_trace(shape, slots, 0, routed, wave_order=1)
-        _, asc = sim_trace(shape, slots, 0, routed)
-        assert sum(p.misses for p in pagers) <= sum(p.misses for p in asc)
-        ctx = make_ctx(shape, slots, max_tokens=T, fetch=fetch, wave_order=1)
+        want, pagers = sim_trace(shape, slots, policy, routed, wave_order=1)
+        if policy == 0:     # per step from the same state this is a theorem; over this seeded LRU trajectory it is checked as measured
+            _, asc = sim_trace(shape, slots, policy, routed)
+            assert sum(p.misses for p in pagers) <= sum(p.misses for p in asc)
+        ctx = make_ctx(shape, slots, max_tokens=T, fetch=fetch, wave_order=1, policy=policy)
         assert_same_bytes(ref, run_chain(ctx, shape, hidden))
         assert ctx.trace_read() == want
         for l in range(shape.n_layers):
             assert ctx.debug_verify_pool(l) == 0
         ctx.close()
-        ctx = make_ctx(shape, slots, max_tokens=T, fetch=fetch, wave_order=1)
+        ctx = make_ctx(shape, slots, max_tokens=T, fetch=fetch, wave_order=1, policy=policy)
         got = run_stack(ctx, shape, hidden)
         assert all(torch.equal(a.view(torch.uint8), b.view(torch.uint8)) for a, b in zip(ref_stack, got))
         assert ctx.trace_read() == want
