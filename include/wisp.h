@@ -14,14 +14,20 @@
  *
  * Conventions
  *   - Every call returns a wisp_status (0 = OK, negative = error); on error the context is unchanged.
+ *     One asynchronous failure exists: if a grid-wide barrier of the fused decode kernel times out (a CTA died),
+ *     the kernel abandons the forward, and the NEXT call that synchronises or launches on the context
+ *     (wisp_moe_forward, wisp_stack_forward, wisp_stats, wisp_trace_read, wisp_last_topk, wisp_last_logits)
+ *     returns WISP_ECUDA once, with wisp_last_error naming it; the outputs of the abandoned forward are invalid.
  *     wisp_last_error() gives a human-readable message for the last failing call on that context.
  *   - "host" / "device" on a pointer says where the memory lives.  The library never takes or returns
  *     framework (torch) types.  `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
  *   - One context is used from one thread at a time.  No CPU fallback exists: without a CUDA device
  *     wisp_create fails with WISP_ECUDA.
- *   - Canonical expert blob (one expert, M_e = 3*d_model*d_ff*sizeof(dtype) bytes),
- *     row-major out x in:  [ gate (d_ff x d_model) | up (d_ff x d_model) | down (d_model x d_ff) ].
- *     Slot bytes == master bytes (the exactness invariant).
+ *   - Canonical expert blob as the CALLER supplies it (one expert, M_e = 3*d_model*d_ff*sizeof(dtype) bytes,
+ *     PAPER.md:102), row-major out x in:  [ gate (d_ff x d_model) | up (d_ff x d_model) | down (d_model x d_ff) ].
+ *     wisp_register_host_experts re-tiles it once into the library's in-slot layout (8-row x 16-byte core
+ *     matrices, csrc/common.cuh) in its own pinned master; slot bytes == master bytes from then on (the
+ *     exactness invariant).
  *   - Arena: one device allocation of `budget_bytes`.  Expert slot s of layer l lives at byte offset
  *     (s*L + l)*M_e  (slot-major, so growing C by one appends a = L*M_e bytes); the KV
  *     pool is the top kappa*b bytes and is modelled as block reservations (BASELINE.json config 5).
@@ -72,7 +78,10 @@ typedef struct {
   int32_t dtype;      /* wisp_dtype: dtype of weights, hidden and out */
   int32_t policy;     /* wisp_policy */
   int32_t fetch;      /* wisp_fetch */
-  int32_t ring_stages; /* shared-memory ring depth of the decode FFN kernels, 2..8; 0 = library default (3 in the persistent kernel) */
+  int32_t ring_stages; /* shared-memory ring depth (parts of <= 32 KiB) of the decode FFN kernels, 2..8; 0 = as many as fit */
+  int32_t unit_rows;   /* act rows per decode FFN work unit: multiple of 8 dividing d_ff with d_ff/unit_rows a multiple of 8;
+                          0 = library default (8 for calls of <= 2 tokens, 16 for 3..8 tokens).  Outputs are byte-identical across
+                          budgets, policies and fetch paths for a GIVEN unit size; changing it regroups the fp32 partial sums. */
   uint64_t kv_block_bytes;  /* b: bytes per KV block summed over layers; 0 = no KV accounting */
   uint64_t kv_floor_blocks; /* kappa_min of Eq. 4; wisp_set_split refuses to go below it */
   uint64_t trace_capacity;  /* trace ring capacity in events; 0 = library default (1<<20) */
@@ -103,11 +112,13 @@ typedef struct {
   uint64_t kernel_launches;      /* library kernels launched so far (graph replays count their kernel nodes) */
 } wisp_stats_t;
 
-/* Kernel classes of wisp_timing_read. */
-enum { WISP_K_ROUTER = 0, WISP_K_TOPK = 1, WISP_K_RESIDENCY = 2, WISP_K_FETCH = 3, WISP_K_GATE_UP = 4, WISP_K_DOWN = 5,
+/* Kernel classes of wisp_timing_read.  Decode (n_tokens <= 8): ROUTER = logits + top-k, RESIDENCY = Algorithm 1, FFN = the fused
+ * gate/up/SwiGLU/down stream of layer calls without a miss (inside the fused kernel: including the grid barrier that ends it),
+ * FFN_MISS = the same for layer calls with >= 1 miss, COMBINE = ordered combine + residual + next layer's partial logits.
+ * Prefill: ROUTER, TOPK, RESIDENCY, FETCH, PREFILL_GATE_UP, PREFILL_DOWN, COMBINE, OTHER (gather, work lists). */
+enum { WISP_K_ROUTER = 0, WISP_K_TOPK = 1, WISP_K_RESIDENCY = 2, WISP_K_FETCH = 3, WISP_K_FFN = 4, WISP_K_FFN_MISS = 5,
        WISP_K_COMBINE = 6, WISP_K_PREFILL_GATE_UP = 7, WISP_K_PREFILL_DOWN = 8, WISP_K_OTHER = 9,
-       WISP_K_GATE_UP_MISS = 10, WISP_K_DOWN_MISS = 11,   /* decode FFN phases of layer calls that had >= 1 miss (fused path) */
-       WISP_N_KERNEL_CLASSES = 12 };
+       WISP_N_KERNEL_CLASSES = 10 };
 
 /* kind: 0 hit, 1 miss, 2 resize-drop, 3 resize-move (for a move `evicted` carries the source slot).
  * Events of one wave are emitted in wave order (ascending expert id; under WISP_WAVES_HITS_FIRST an overflowing step

@@ -12,8 +12,8 @@ WISP_F32, WISP_BF16 = 0, 1
 WISP_LRU, WISP_LFU = 0, 1
 WISP_FETCH_MEMCPY, WISP_FETCH_ZEROCOPY, WISP_FETCH_FUSED = 0, 1, 2
 WISP_WAVES_ASCENDING, WISP_WAVES_HITS_FIRST = 0, 1
-KERNEL_CLASSES = ("router", "topk", "residency", "fetch", "gate_up", "down", "combine", "prefill_gate_up",
-                  "prefill_down", "other", "gate_up_miss", "down_miss")
+KERNEL_CLASSES = ("router", "topk", "residency", "fetch", "ffn", "ffn_miss", "combine", "prefill_gate_up",
+                  "prefill_down", "other")
 N_KERNEL_CLASSES = len(KERNEL_CLASSES)
 STATUS_NAMES = {0: "WISP_OK", -1: "WISP_EINVAL", -2: "WISP_ENOMEM", -3: "WISP_ECUDA", -4: "WISP_ESTATE", -5: "WISP_EBUDGET"}
 
@@ -21,7 +21,7 @@ STATUS_NAMES = {0: "WISP_OK", -1: "WISP_EINVAL", -2: "WISP_ENOMEM", -3: "WISP_EC
 class WispConfig(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("n_experts", C.c_int32), ("top_k", C.c_int32), ("d_model", C.c_int32),
                 ("d_ff", C.c_int32), ("max_tokens", C.c_int32), ("dtype", C.c_int32), ("policy", C.c_int32),
-                ("fetch", C.c_int32), ("ring_stages", C.c_int32), ("kv_block_bytes", C.c_uint64),
+                ("fetch", C.c_int32), ("ring_stages", C.c_int32), ("unit_rows", C.c_int32), ("kv_block_bytes", C.c_uint64),
                 ("kv_floor_blocks", C.c_uint64), ("trace_capacity", C.c_uint64)]
 
 
@@ -111,9 +111,9 @@ class Wisp:
     """Holder of one wisp_ctx.  Methods mirror the C entry points one to one."""
 
     def __init__(self, budget_bytes: int, *, n_layers, n_experts, top_k, d_model, d_ff, max_tokens, dtype, policy=WISP_LRU,
-                 fetch=WISP_FETCH_ZEROCOPY, kv_block_bytes=0, kv_floor_blocks=0, trace_capacity=0, ring_stages=0):
+                 fetch=WISP_FETCH_ZEROCOPY, kv_block_bytes=0, kv_floor_blocks=0, trace_capacity=0, ring_stages=0, unit_rows=0):
         self.L = lib()
-        self.cfg = WispConfig(n_layers, n_experts, top_k, d_model, d_ff, max_tokens, dtype, policy, fetch, ring_stages,
+        self.cfg = WispConfig(n_layers, n_experts, top_k, d_model, d_ff, max_tokens, dtype, policy, fetch, ring_stages, unit_rows,
                               kv_block_bytes, kv_floor_blocks, trace_capacity)
         self.ctx = C.c_void_p()
         rc = self.L.wisp_create(budget_bytes, C.byref(self.cfg), C.byref(self.ctx))

@@ -12,6 +12,7 @@
 #include <stdint.h>
 
 #include "../../include/wisp.h"
+#include "ptx.cuh"
 
 namespace wisp {
 
@@ -75,6 +76,24 @@ template <typename T> __device__ __forceinline__ T from_f32(float v);
 template <> __device__ __forceinline__ float from_f32<float>(float v) { return v; }
 template <> __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
 
+__device__ __forceinline__ float silu_f(float v) { return v / (1.0f + expf(-v)); }
+
+// ---- in-slot weight layout ("core-matrix tiled") ------------------------------------------
+// The library re-tiles the caller's canonical blob [gate | up | down] (row-major out x in) once, at registration, into
+// 8-row x 16-byte core matrices (128 contiguous bytes each; kc = 16 / sizeof(dtype) elements per row of a core):
+//   gate, up  [d_ff x d]   : core (r/8, k/kc)  at ((r/8) * (d/kc)  + k/kc) * 128 B   -> 8 act rows x all of d are contiguous
+//   down      [d x d_ff]   : core (j/8, i/kc)  at ((i/kc) * (d/8)  + j/8 ) * 128 B   -> 8 act columns x all of d are contiguous
+// inside a core: row (r%8 | j%8) at 16 B * row, element (k%kc | i%kc).  One decode work unit (8 act rows: their gate rows, up
+// rows and down columns) is then three contiguous pieces that 1-D TMA bulk copies fetch whole, ldmatrix reads without bank
+// conflicts, and the prefill tcgen05 kernel consumes as the canonical no-swizzle K-major operand layout.  Master bytes == slot
+// bytes: the same tiling lives in the pinned master and in every slot.
+__host__ __device__ __forceinline__ size_t tiled_gu_index(int r, int k, int d, int kc) {
+  return ((size_t)(r >> 3) * (d / kc) + k / kc) * (8 * kc) + (size_t)(r & 7) * kc + k % kc;
+}
+__host__ __device__ __forceinline__ size_t tiled_down_index(int j, int i, int d, int kc) {
+  return ((size_t)(i / kc) * (d >> 3) + (j >> 3)) * (8 * kc) + (size_t)(j & 7) * kc + i % kc;
+}
+
 // ---- the per-forward plan written by the residency kernel ------------------------------------------
 // hdr[0] = n_waves, hdr[1] = n_ref (|R|), hdr[2] = n_miss, hdr[3] = n_pairs.  Entries are in wave order
 // (ascending expert id; wave w = entries [w*C, min(n_ref, (w+1)*C)) ).
@@ -86,6 +105,9 @@ struct PlanPtrs {
   int* exp_count;      // [E]  (token, rank) pairs routed to expert e
   int* exp_offset;     // [E+1] exclusive prefix of exp_count over ascending e
   int* pair_list;      // [n_pairs] pair indices (t*k + rank) grouped by expert, ascending inside a group
+  // decode path only (nullable): the order in which the FFN takes the entries of a wave, and the inverse of pair_list
+  int* unit_entry;     // [E]  per wave segment [w*C, ...): entry indices, this step's misses first (their host reads start at once)
+  int* pair_pos;       // [n_pairs] pair_pos[pair_list[p]] = p: position of a (token, rank) pair in the expert-sorted order
 };
 
 // Host-visible copy of the plan for the MEMCPY miss path (mapped pinned memory).

@@ -1,0 +1,102 @@
+// decode_combine.cuh -- the reduce-scatter half of a decode layer: ordered combine (+ residual) of the FFN chunk partials
+// and the NEXT layer's router logits, both distributed over the grid in 16-column slices of the hidden state.
+//
+//   y_{t,i}[j]  = sum_{c = 0..NC-1} P[pos(t,i)][c][j]      8 groups of NC/8 consecutive chunks: inside a group ascending c
+//                                                           (fp32 add chain from the first partial), then the 8 group sums
+//                                                           ascending
+//   out_t[j]    = sum_{i = 0..k-1} w[t,i] * y_{t,i}[j]      fmaf in rank order from 0.f, stored in the model dtype (a4, G21)
+//   x'_t[j]     = x_t[j] + out_t[j]                         fp32 add of the two model-dtype values, stored in the model dtype (O3)
+//   z_e        += sum_{j in slice} W_r[e][j] * x'_t[j]      fmaf in ascending j from 0.f per slice, then added to the logit
+//                                                           accumulator as a 2^-40 fixed-point integer (a1)
+// The logit accumulator is an int64 per (token, expert): integer addition is associative, so the all-reduce of the
+// 16-column partial logits over the grid is bit-reproducible whatever order the CTAs' `red.add.u64` arrive in, and it needs
+// no second grid-wide exchange: after one barrier every CTA reads E words per token.  (A logit partial is O(1); 2^-40
+// resolution is five orders of magnitude below fp32 rounding of the logit itself.)
+#pragma once
+#include "common.cuh"
+
+namespace wisp {
+
+constexpr int kSliceCols = 16;
+constexpr float kLogitFixScale = 1099511627776.f;        // 2^40
+constexpr double kLogitFixInv = 1.0 / 1099511627776.0;
+
+__device__ __forceinline__ long long logit_to_fix(float v) {
+  const float s = v * kLogitFixScale;
+  if (!(fabsf(s) < 4.0e18f)) return s > 0.f ? (1ll << 62) : -(1ll << 62);   // non-finite input (G23): saturate, stay defined
+  return __float2ll_rn(s);
+}
+__device__ __forceinline__ float logit_from_fix(long long f, float bias) { return (float)((double)f * kLogitFixInv) + bias; }
+
+// Partial logits of one 16-column slice of token t's hidden state (xn[16], fp32 images of the model-dtype values) for all
+// experts, added into zfix[t][e].  wrt: this layer's router weights TRANSPOSED, [d][E] in the model dtype.
+template <typename T>
+__device__ __forceinline__ void slice_logits(const T* __restrict__ wrt, const float* xn, int j0, int E, long long* zfix_t, int tid, int nthr) {
+  for (int e = tid; e < E; e += nthr) {
+    float zp = 0.f;
+#pragma unroll
+    for (int jj = 0; jj < kSliceCols; ++jj) zp = fmaf(to_f32<T>(wrt[(size_t)(j0 + jj) * E + e]), xn[jj], zp);
+    atomicAdd(reinterpret_cast<unsigned long long*>(zfix_t + e), (unsigned long long)logit_to_fix(zp));
+  }
+}
+
+struct CombineArgs {
+  const float* partial;      // P [pair position][NC][d]
+  int n_chunks, d, k;
+  const float* topw;         // [T][k] routing weights (rank order)
+  const int* pair_pos;       // [T][k] position of pair (t, rank) in the expert-sorted order
+};
+
+// One slice (token t, columns j0 .. j0+15) by 256 threads synchronising on named barrier `bar`.
+//   x_row  : token t's current hidden state (model dtype) or nullptr (no residual: the result is out_t itself)
+//   dst_row: where the result row goes (global, model dtype)
+//   s_yg   : 8 * 8 * 16 floats, s_y: kMaxTopK * 16 floats, s_xn: 16 floats (receives the fp32 image of the stored result)
+template <typename T>
+__device__ __forceinline__ void combine_slice(const CombineArgs& a, int t, int j0, const T* x_row, T* dst_row, float* s_yg, float* s_y,
+                                              float* s_xn, int bar) {
+  const int tid = threadIdx.x, grp = tid >> 5, lane = tid & 31, ri = lane >> 2, j4 = (lane & 3) * 4;
+  const int per = a.n_chunks >> 3;
+  for (int i0 = 0; i0 < a.k; i0 += 8) {
+    const int rank = i0 + ri;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (rank < a.k) {
+      const int pos = a.pair_pos[t * a.k + rank];
+      const float* src = a.partial + ((size_t)pos * a.n_chunks + (size_t)grp * per) * a.d + j0 + j4;
+      for (int c0 = 0; c0 < per; c0 += 16) {                 // up to 16 independent L2 reads in flight, added in ascending c
+        float4 v[16];
+#pragma unroll
+        for (int u = 0; u < 16; ++u)
+          if (c0 + u < per) v[u] = __ldcg(reinterpret_cast<const float4*>(src + (size_t)(c0 + u) * a.d));
+#pragma unroll
+        for (int u = 0; u < 16; ++u)
+          if (c0 + u < per) {
+            if (c0 + u == 0) acc = v[0];
+            else { acc.x += v[u].x; acc.y += v[u].y; acc.z += v[u].z; acc.w += v[u].w; }
+          }
+      }
+    }
+    *reinterpret_cast<float4*>(s_yg + (grp * 8 + ri) * kSliceCols + j4) = acc;
+    asm volatile("bar.sync %0, 256;" ::"r"(bar) : "memory");
+    if (tid < 32 && rank < a.k) {
+      float4 y = *reinterpret_cast<const float4*>(s_yg + ri * kSliceCols + j4);
+#pragma unroll
+      for (int g = 1; g < 8; ++g) {
+        const float4 v = *reinterpret_cast<const float4*>(s_yg + (g * 8 + ri) * kSliceCols + j4);
+        y.x += v.x; y.y += v.y; y.z += v.z; y.w += v.w;
+      }
+      *reinterpret_cast<float4*>(s_y + rank * kSliceCols + j4) = y;
+    }
+    asm volatile("bar.sync %0, 256;" ::"r"(bar) : "memory");
+  }
+  if (tid < kSliceCols) {
+    float acc = 0.f;
+    for (int i = 0; i < a.k; ++i) acc = fmaf(a.topw[t * a.k + i], s_y[i * kSliceCols + tid], acc);
+    T o = from_f32<T>(acc);
+    if (x_row) o = from_f32<T>(to_f32<T>(x_row[j0 + tid]) + to_f32<T>(o));
+    dst_row[j0 + tid] = o;
+    s_xn[tid] = to_f32<T>(o);
+  }
+  asm volatile("bar.sync %0, 256;" ::"r"(bar) : "memory");
+}
+
+}  // namespace wisp

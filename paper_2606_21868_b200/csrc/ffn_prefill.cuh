@@ -5,7 +5,6 @@
 //   ystage[pair, j] = <D[j], act[pair]>                   fp32
 #pragma once
 #include "common.cuh"
-#include "ffn_stream.cuh"
 
 namespace wisp {
 
@@ -31,8 +30,11 @@ __global__ void __launch_bounds__(256) prefill_ffn_kernel(PlanPtrs plan, int wav
   const int K = MODE == 0 ? d : d_ff;
   const int r0 = blockIdx.x * kPfTile;
   const T* blob = pool + ((size_t)plan.entry_slot[i] * L + layer) * blob_elems;
-  const T* w0 = MODE == 0 ? blob + (size_t)r0 * d : blob + 2 * (size_t)d_ff * d + (size_t)r0 * d_ff;
-  const T* w1 = w0 + (size_t)d_ff * d;   // up rows (MODE 0 only)
+  // weights are read through the tiled in-slot layout (common.cuh): gate / up rows r0.., or down rows (outputs j) r0..
+  constexpr int kc = 16 / (int)sizeof(T);
+  const T* wg = blob;
+  const T* wu = blob + (size_t)d_ff * d;
+  const T* wd = blob + 2 * (size_t)d_ff * d;
 
   __shared__ float sA[kPfK][kPfTile + 1];
   __shared__ float sW0[kPfK][kPfTile + 1];
@@ -51,8 +53,13 @@ __global__ void __launch_bounds__(256) prefill_ffn_kernel(PlanPtrs plan, int wav
       float av = 0.f;
       if (pr >= 0) av = MODE == 0 ? to_f32<T>(x[(size_t)(pr / k) * d + k0 + kk]) : to_f32<T>(act[(size_t)pr * d_ff + k0 + kk]);
       sA[kk][row] = av;
-      sW0[kk][row] = to_f32<T>(w0[(size_t)row * K + k0 + kk]);
-      if (MODE == 0) sW1[kk][row] = to_f32<T>(w1[(size_t)row * K + k0 + kk]);
+      if (MODE == 0) {
+        const size_t wi = tiled_gu_index(r0 + row, k0 + kk, d, kc);
+        sW0[kk][row] = to_f32<T>(wg[wi]);
+        sW1[kk][row] = to_f32<T>(wu[wi]);
+      } else {
+        sW0[kk][row] = to_f32<T>(wd[tiled_down_index(r0 + row, k0 + kk, d, kc)]);
+      }
     }
     __syncthreads();
 #pragma unroll 8
@@ -81,6 +88,23 @@ __global__ void __launch_bounds__(256) prefill_ffn_kernel(PlanPtrs plan, int wav
       else ystage[(size_t)pr * d + r] = c0[p][q];
     }
   }
+}
+
+// out[t, j] = sum_i w[t,i] * ystage[t*k+i, j] in rank order (fmaf from 0.f, fp32), stored in the model dtype; the optional
+// residual successor x_next = x + out uses the rounding of DESIGN.md O3.  Prefill / overflow staging path (a5): the grouped
+// GEMMs leave y per (token, rank) pair in ystage [T*k][d].
+template <typename T>
+__global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ ystage, const float* __restrict__ w,
+                                                      T* __restrict__ out, const T* __restrict__ x_res,
+                                                      T* __restrict__ x_next, int n_tokens, int d, int k) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)n_tokens * d) return;
+  const int t = (int)(idx / d), j = (int)(idx % d);
+  float acc = 0.f;
+  for (int i = 0; i < k; ++i) acc = fmaf(w[(size_t)t * k + i], ystage[((size_t)t * k + i) * d + j], acc);
+  const T o = from_f32<T>(acc);
+  out[idx] = o;
+  if (x_res) x_next[idx] = from_f32<T>(to_f32<T>(x_res[idx]) + to_f32<T>(o));
 }
 
 }  // namespace wisp

@@ -8,8 +8,11 @@
 //                     act[pos, r] = silu(Hg[r, pos]) * Hu[r, pos]   (bf16, sorted-pair order, G21)
 //   GEMM 2 (MODE 1):  Y = D_s act_e^T                   [128 rows x NT tokens], K = d_ff  -> ystage[pair, r] fp32
 // "Swap AB": the weight rows are the MMA M dimension (always 128 full rows), the ragged token count is N.
-// Operands are K-major; A tiles come straight from the slot through a 3-D tensor map over the arena
-// (K, row, blob index = slot*L + layer), B tiles from the gathered token rows xg / the act buffer.
+// Operands are K-major.  A tiles come straight from the slot: the in-slot layout (common.cuh) stores every matrix as
+// 8-row x 16-byte core matrices of 128 contiguous bytes, which is the canonical NO-SWIZZLE K-major UMMA operand layout, so a
+// 4-D tensor map (64 elements of a core, core column, core row, blob index = slot*L + layer) drops a 128 x 64 tile into shared
+// memory ready for the descriptor (gate/up: cores of a row group adjacent along K; down: cores of an act-column block
+// adjacent along M).  B tiles come from the gathered token rows xg / the act buffer with the 128-byte swizzle.
 // Warp roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer, warps 2..5 = epilogue.
 // Determinism (parity (b)): a column (token) of the accumulator depends only on that token's row and the weight
 // tile, the K order is fixed, and nothing depends on the slot, the wave or the other tokens of the tile.
@@ -17,7 +20,6 @@
 #include <cuda.h>
 
 #include "common.cuh"
-#include "ffn_stream.cuh"
 
 namespace wisp {
 
@@ -67,6 +69,10 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm,
   asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
                ::"r"(dst), "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+               ::"r"(dst), "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t cols) {
   asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(cols) : "memory");
   asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -108,6 +114,17 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
   desc |= (uint64_t)(1024u >> 4) << 32;                      // stride byte offset
   desc |= (uint64_t)1 << 46;                                 // version
   desc |= (uint64_t)2 << 61;                                 // SWIZZLE_128B
+  return desc;
+}
+// Shared-memory matrix descriptor of a K-major tile stored as plain (unswizzled) core matrices of 8 rows x 16 bytes, 128
+// contiguous bytes each: lbo = bytes between the two core matrices of one MMA along K, sbo = bytes between core matrices
+// that are adjacent along M.  Layout type 0 = SWIZZLE_NONE ("interleave").
+__device__ __forceinline__ uint64_t umma_desc_cores(uint32_t smem_addr, uint32_t lbo, uint32_t sbo) {
+  uint64_t desc = 0;
+  desc |= (uint64_t)((smem_addr >> 4) & 0x3fffu);
+  desc |= (uint64_t)((lbo >> 4) & 0x3fffu) << 16;
+  desc |= (uint64_t)((sbo >> 4) & 0x3fffu) << 32;
+  desc |= (uint64_t)1 << 46;                                 // version
   return desc;
 }
 // Instruction descriptor: D fp32, A and B bf16, both K-major, M x N tile.
@@ -184,8 +201,14 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
           const uint32_t bar = smem_u32(&s_full[s]);
           mbar_expect_tx(bar, kStage);
           const uint32_t base = smem0 + s * kStage;
-          tma_load_3d(base, &tm_w, kb * kMmaBK, r0, blob, bar);
-          if (MODE == 0) tma_load_3d(base + kMmaTileBytes, &tm_w, kb * kMmaBK, a.dff + r0, blob, bar);
+          if (MODE == 0) {          // (core, core column = K block, core row = row group, blob): gate then up
+            tma_load_4d(base, &tm_w, 0, kb * (kMmaBK / 8), r0 / 8, blob, bar);
+            tma_load_4d(base + kMmaTileBytes, &tm_w, 0, kb * (kMmaBK / 8), (a.dff + r0) / 8, blob, bar);
+          } else if (MODE == 1) {   // (core, output group j/8, act-column block i/8, blob)
+            tma_load_4d(base, &tm_w, 0, r0 / 8, kb * (kMmaBK / 8), blob, bar);
+          } else {
+            tma_load_3d(base, &tm_w, kb * kMmaBK, r0, blob, bar);
+          }
           tma_load_2d(base + NA * kMmaTileBytes, &tm_x, kb * kMmaBK, pos0, bar);
           if (++s == n_stages) { s = 0; ph ^= 1u; }
         }
@@ -206,13 +229,19 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
           mbar_wait(smem_u32(&s_full[s]), ph);
           tc_fence_after();
           const uint32_t base = smem0 + s * kStage;
-          const uint64_t da0 = umma_desc_sw128(base), da1 = umma_desc_sw128(base + kMmaTileBytes);
+          // A: MODE 0 tile = [16 row groups][8 K cores][128 B]  (K-adjacent cores 128 B apart, row groups 1 KiB apart; 16 K
+          //                   elements = 2 cores = 256 B per MMA);
+          //    MODE 1 tile = [8 K blocks][16 output groups][128 B] (K-adjacent cores 2 KiB apart, output groups 128 B apart;
+          //                   4 KiB per MMA);  MODE 2 (router rows, row-major in global memory) = 128-byte swizzle
+          const uint64_t da0 = MODE == 0 ? umma_desc_cores(base, 128u, 1024u) : MODE == 1 ? umma_desc_cores(base, 2048u, 128u) : umma_desc_sw128(base);
+          const uint64_t da1 = umma_desc_cores(base + kMmaTileBytes, 128u, 1024u);
+          const uint32_t a_step = MODE == 0 ? 256u >> 4 : MODE == 1 ? 4096u >> 4 : 2u;
           const uint64_t db = umma_desc_sw128(base + NA * kMmaTileBytes);
 #pragma unroll
-          for (int k4 = 0; k4 < kMmaBK / 16; ++k4) {          // UMMA_K = 16 bf16 = 32 bytes = 2 sixteen-byte units
+          for (int k4 = 0; k4 < kMmaBK / 16; ++k4) {          // UMMA_K = 16 bf16
             const uint32_t acc = (kb | k4) != 0;
-            umma_bf16(acc_base, da0 + 2 * k4, db + 2 * k4, idesc, acc);
-            if (MODE == 0) umma_bf16(acc_base + 128, da1 + 2 * k4, db + 2 * k4, idesc, acc);
+            umma_bf16(acc_base, da0 + a_step * k4, db + 2 * k4, idesc, acc);
+            if (MODE == 0) umma_bf16(acc_base + 128, da1 + a_step * k4, db + 2 * k4, idesc, acc);
           }
           umma_commit(smem_u32(&s_empty[s]));                 // frees the stage once these MMAs have read it
           if (++s == n_stages) { s = 0; ph ^= 1u; }

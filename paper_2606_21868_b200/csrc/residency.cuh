@@ -258,6 +258,19 @@ __device__ __forceinline__ void plan_compute(const PlanArgs& a, PlanShared<NT>& 
     plan_sync<NT>(bar);
   }
   if (tid == 0) { a.plan.hdr[0] = n_waves; a.plan.hdr[1] = nR; a.plan.hdr[2] = miss_total; a.plan.hdr[3] = a.n_pairs; }
+  // decode path: unit order of every wave (misses first, each group in wave order) and the inverse pair permutation
+  if (a.plan.unit_entry != nullptr && tid < nR) {
+    const int lo = (tid / C) * C, nw = min(C, nR - lo);
+    const int mine = a.plan.entry_miss[tid];
+    int miss_before = 0, hit_before = 0, miss_all = 0;
+    for (int o = 0; o < nw; ++o) {
+      const int m = a.plan.entry_miss[lo + o];
+      miss_all += m;
+      if (lo + o < tid) { miss_before += m; hit_before += 1 - m; }
+    }
+    a.plan.unit_entry[lo + (mine ? miss_before : miss_all + hit_before)] = tid;
+  }
+  if (a.plan.pair_pos != nullptr && a.build_pairs && tid < a.n_pairs) a.plan.pair_pos[a.plan.pair_list[tid]] = tid;
 
   // ---- write back ----
   if (writer) {
@@ -282,6 +295,88 @@ __device__ __forceinline__ void plan_compute(const PlanArgs& a, PlanShared<NT>& 
     }
   }
   plan_sync<NT>(bar);
+}
+
+// Hit fast path of WISPLAYER.STEP(R) for decode-sized calls, run by ONE warp (lanes of warp 0 of the caller): when every
+// member of R is already resident and |R| <= C, Algorithm 1 has no fault to assign (lines 2-8 are empty) and the step is
+// just the tick of line 9: c <- c+1, tau[pi(e)] <- c, f[e] += 1 for e in R (G24).  Builds the same plan
+// plan_compute would (entries in ascending id, pairs grouped by expert) and returns true; returns false -- touching nothing
+// but its scratch -- when the step has a fault, overflows, is being tracked for MV-WSA or has more than 64 pairs, and the
+// caller then runs plan_compute.  `sh` holds the layer's state as loaded by plan_load.
+template <int NT>
+__device__ __forceinline__ bool plan_fast_warp(const PlanArgs& a, PlanShared<NT>& sh, bool writer, int lane) {
+  const int E = a.E, n_pairs = a.n_pairs;
+  if (a.track || n_pairs > 64 || E > 256) return false;
+  if (lane < 8) sh.bitmap[lane] = 0u;
+  __syncwarp();
+  const int e0 = lane < n_pairs ? a.ids[lane] : -1, e1 = lane + 32 < n_pairs ? a.ids[lane + 32] : -1;
+  if (e0 >= 0) atomicOr(&sh.bitmap[e0 >> 5], 1u << (e0 & 31));
+  if (e1 >= 0) atomicOr(&sh.bitmap[e1 >> 5], 1u << (e1 & 31));
+  __syncwarp();
+  unsigned word = lane < 8 ? sh.bitmap[lane] : 0u;
+  int inc = __popc(word);
+#pragma unroll
+  for (int o = 1; o < 8; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+  const int nR = __shfl_sync(0xffffffffu, inc, 7);
+  int pos = inc - __popc(word);
+  while (word) { const int b = __ffs(word) - 1; word &= word - 1; sh.R[pos++] = lane * 32 + b; }   // R ascending
+  __syncwarp();
+  bool ok = nR <= a.C;
+  for (int i = lane; i < nR; i += 32) ok = ok && sh.pi[sh.R[i]] >= 0;
+  if (!__all_sync(0xffffffffu, ok)) return false;
+  // pairs grouped by expert: counts, offsets (ascending id == ascending entry), stable lists
+  int run = 0;
+  for (int i0 = 0; i0 < nR; i0 += 32) {
+    const int i = i0 + lane;
+    const int e = i < nR ? sh.R[i] : -1;
+    int cnt = 0;
+    for (int p = 0; p < n_pairs; ++p) cnt += (a.ids[p] == e);
+    if (e < 0) cnt = 0;
+    int sc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, sc, o); if (lane >= o) sc += v; }
+    const int off = run + sc - cnt;
+    if (e >= 0) {
+      const int slot = sh.pi[e];
+      a.plan.entry_expert[i] = e; a.plan.entry_slot[i] = slot; a.plan.entry_miss[i] = 0;
+      a.plan.exp_count[e] = cnt; a.plan.exp_offset[e] = off;
+      if (a.plan.unit_entry) a.plan.unit_entry[i] = i;
+      int j = 0;
+      for (int p = 0; p < n_pairs; ++p)
+        if (a.ids[p] == e) { a.plan.pair_list[off + j] = p; if (a.plan.pair_pos) a.plan.pair_pos[p] = off + j; ++j; }
+      if (writer) {                                                // line 9: the tick
+        a.st.tau[slot] = sh.clock + 1ull;
+        a.st.freq[e] = sh.freq[e] + 1ull;
+        if (a.trace_on) {
+          const u64 base = a.trace_ctr[0];
+          if (base + (u64)nR <= a.trace_cap) {
+            wisp_trace_event ev;
+            ev.step = sh.scal[1]; ev.layer = (uint32_t)a.layer; ev.wave = 0u; ev.expert = e; ev.slot = slot; ev.evicted = -1; ev.kind = 0u;
+            a.trace[base + i] = ev;
+          }
+        }
+      }
+    }
+    run += __shfl_sync(0xffffffffu, sc, 31);
+  }
+  __syncwarp();
+  if (lane == 0) {
+    a.plan.hdr[0] = nR > 0 ? 1 : 0; a.plan.hdr[1] = nR; a.plan.hdr[2] = 0; a.plan.hdr[3] = n_pairs;
+    a.plan.exp_offset[E] = n_pairs;
+    if (writer) {
+      a.st.scal[0] = sh.clock + 1ull;
+      if (nR > 0) a.st.scal[1] = sh.scal[1] + 1ull;
+      a.st.scal[2] = sh.scal[2] + (u64)nR;
+      a.st.scal[5] = sh.scal[5] + (u64)nR;
+      if (a.trace_on) {
+        const u64 base = a.trace_ctr[0];
+        if (base + (u64)nR <= a.trace_cap) a.trace_ctr[0] = base + (u64)nR;
+        else a.trace_ctr[1] += (u64)nR;
+      }
+    }
+  }
+  __syncwarp();
+  return true;
 }
 
 __global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a) {

@@ -62,57 +62,62 @@ __global__ void __launch_bounds__(256) router_logits_kernel(const T* __restrict_
   router_row_warp<T>(x, w_r + (size_t)e * d, bias ? bias[e] : 0.f, z, e, t0, min(kRouterTokTile, n_tokens - t0), E, d, lane);
 }
 
-// Top-k + softmax of n_tokens rows of logits held in shared memory (z [n_tokens][E], read only), by `nthr` threads
-// (threadIdx.x < nthr) that synchronise through named barrier `bar`.  Selection by rank counting, which IS the
-// definition (G7): rank(e) = #{j : z_j > z_e or (z_j == z_e and j < e)}; the experts of rank < k are the top-k in
-// (z desc, id asc) order.  w_i = exp(z_i - z_0) / sum_j exp(z_j - z_0), the sum taken in rank order j = 0..k-1.
-// ids_out / w_out: [n_tokens][k] (any address space); selz: [n_tokens][k] floats of shared scratch.
-__device__ __forceinline__ void topk_softmax_block(const float* z, int n_tokens, int E, int k, int* ids_out, float* w_out,
-                                                   float* selz, int nthr, int bar) {
-  const int tid = threadIdx.x;
-  for (int idx = tid; idx < n_tokens * E; idx += nthr) {
-    const int t = idx / E, e = idx % E;
-    const float* row = z + (size_t)t * E;
-    const float ze = row[e];
-    int rank = 0;
-    if ((E & 3) == 0 && (((size_t)row) & 15) == 0) {       // all lanes read the same address: shared-memory broadcast
-      const float4* row4 = reinterpret_cast<const float4*>(row);
-#pragma unroll 4
-      for (int j4 = 0; j4 < E / 4; ++j4) {
-        const float4 v = row4[j4];
-        const int j = j4 * 4;
-        rank += (v.x > ze) || (v.x == ze && j < e);
-        rank += (v.y > ze) || (v.y == ze && j + 1 < e);
-        rank += (v.z > ze) || (v.z == ze && j + 2 < e);
-        rank += (v.w > ze) || (v.w == ze && j + 3 < e);
-      }
-    } else {
-      for (int j = 0; j < E; ++j) {
-        const float zj = row[j];
-        rank += (zj > ze) || (zj == ze && j < e);
-      }
+// Top-k + softmax of ONE token's logits by ONE warp ("warp-shuffle softmax and top-k", BASELINE.json north_star; G7).
+// Lane l owns the logits of experts l, l+32, ... as 64-bit keys (order-preserving image of z << 32 | ~id), so the warp
+// arg-max of a key is the largest logit with ties going to the LOWER id; k rounds give ids in (z desc, id asc) order.
+// -0 compares equal to +0 and a NaN ranks with -inf (it can never corrupt an id: every selected id is a real expert).
+// w_i = exp(z_i - z_0) / sum_j exp(z_j - z_0), the sum taken in rank order j = 0..k-1 (every lane computes the same chain).
+// EPL = logits per lane (E <= 32 * EPL); zf(e) returns the logit of expert e.  ids_out / w_out: [k].
+__device__ __forceinline__ unsigned long long topk_key(float z, int e) {
+  z += 0.0f;                                            // -0 -> +0
+  unsigned u = __float_as_uint(z);
+  if (z != z) u = 0xff800000u;                          // NaN -> -inf
+  u = (u & 0x80000000u) ? ~u : (u | 0x80000000u);       // unsigned order == float order
+  return ((unsigned long long)u << 32) | (unsigned)(0xffffffffu - (unsigned)e);
+}
+__device__ __forceinline__ float topk_key_logit(unsigned long long key) {
+  unsigned u = (unsigned)(key >> 32);
+  u = (u & 0x80000000u) ? (u & 0x7fffffffu) : ~u;
+  return __uint_as_float(u);
+}
+template <int EPL, typename ZF>
+__device__ __forceinline__ void topk_softmax_warp(ZF zf, int E, int k, int* ids_out, float* w_out, int lane) {
+  unsigned long long key[EPL];
+#pragma unroll
+  for (int j = 0; j < EPL; ++j) {
+    const int e = lane + 32 * j;
+    key[j] = e < E ? topk_key(zf(e), e) : 0ull;          // 0 = absent / already taken (every live key is > 0)
+  }
+  float my_z = 0.f;                                     // lane r keeps the logit of rank r
+  for (int r = 0; r < k; ++r) {
+    unsigned long long best = 0ull;
+#pragma unroll
+    for (int j = 0; j < EPL; ++j) best = key[j] > best ? key[j] : best;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
+      best = other > best ? other : best;
     }
-    if (rank < k) { ids_out[t * k + rank] = e; selz[t * k + rank] = ze; }
+    const int e = (int)(0xffffffffu - (unsigned)(best & 0xffffffffu));
+#pragma unroll
+    for (int j = 0; j < EPL; ++j)
+      if (e == lane + 32 * j) key[j] = 0ull;
+    if (lane == r) { my_z = topk_key_logit(best); ids_out[r] = e; }
   }
-  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthr) : "memory");
-  for (int idx = tid; idx < n_tokens * k; idx += nthr) {
-    const int t = idx / k;
-    const float z0 = selz[t * k];
-    float den = 0.f;
-    for (int j = 0; j < k; ++j) den += expf(selz[t * k + j] - z0);   // fixed order
-    w_out[idx] = expf(selz[idx] - z0) / den;
-  }
-  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthr) : "memory");
+  const float z0 = __shfl_sync(0xffffffffu, my_z, 0);
+  float den = 0.f;
+  for (int j = 0; j < k; ++j) den += expf(__shfl_sync(0xffffffffu, my_z, j) - z0);   // fixed order
+  if (lane < k) w_out[lane] = expf(my_z - z0) / den;
 }
 
-// 4 tokens per block of 128 threads.  smem: 4 * E floats (logits) + 4 * k floats.
+// Prefill / multi-kernel path: one warp per token, 4 tokens per block of 128 threads; z [n_tokens][E] in global memory.
+template <int EPL>
 __global__ void __launch_bounds__(128) topk_softmax_kernel(const float* __restrict__ z, int* __restrict__ ids,
                                                            float* __restrict__ w, int n_tokens, int E, int k) {
-  extern __shared__ float sz[];
-  const int t0 = blockIdx.x * 4, nt = min(4, n_tokens - t0);
-  for (int i = threadIdx.x; i < nt * E; i += 128) sz[i] = z[(size_t)t0 * E + i];
-  __syncthreads();
-  topk_softmax_block(sz, nt, E, k, ids + (size_t)t0 * k, w + (size_t)t0 * k, sz + 4 * E, 128, 0);
+  const int t = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (t >= n_tokens) return;
+  const float* row = z + (size_t)t * E;
+  topk_softmax_warp<EPL>([&](int e) { return row[e]; }, E, k, ids + (size_t)t * k, w + (size_t)t * k, lane);
 }
 
 }  // namespace wisp

@@ -1,6 +1,6 @@
 // wisp.cu -- context, C ABI (include/wisp.h) and launch orchestration of libwisp (sm_100a).
 // Host code only enqueues work; every step of the hot path (router, residency, fetch, FFN, combine)
-// runs in the kernels of router.cuh / residency.cuh / fetch.cuh / ffn_decode.cuh / ffn_prefill.cuh.
+// runs in the kernels of router.cuh / residency.cuh / fetch.cuh / decode_*.cuh / ffn_prefill*.cuh.
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
@@ -10,16 +10,17 @@
 #include <vector>
 
 #include "common.cuh"
-#include "decode_persistent.cuh"
+#include "decode_kernels.cuh"
 #include "fetch.cuh"
 #include "ffn_prefill.cuh"
 #include "ffn_prefill_mma.cuh"
-#include "ffn_stream.cuh"
 #include "mvwsa.h"
 #include "residency.cuh"
 #include "router.cuh"
 
 using namespace wisp;
+
+static_assert(sizeof(wisp_config) == 72 && sizeof(wisp_trace_event) == 32, "C ABI struct layout (tests/test_library_abi.py mirrors it)");
 
 struct wisp_ctx {
   wisp_config cfg{};
@@ -31,9 +32,10 @@ struct wisp_ctx {
   int num_sms = 0;
 
   char* arena = nullptr;
-  std::vector<void*> master;       // pinned, mapped; one allocation per layer
+  std::vector<void*> master;       // pinned, mapped; one allocation per layer, blobs in the tiled in-slot layout
   std::vector<char> registered;
-  char* router_w = nullptr;        // device [L][E][d]
+  char* router_w = nullptr;        // device [L][E][d]   (prefill router GEMM)
+  char* router_wt = nullptr;       // device [L][d][E]   (decode: 16-column slices of the hidden state)
   float* router_bias = nullptr;    // device [L][E]
 
   // per-layer residency state (device), each [L][...]
@@ -49,9 +51,8 @@ struct wisp_ctx {
   int* plan_mem = nullptr;
   PlanPtrs plan{};
   HostPlan* host_plan = nullptr;   // mapped pinned
-  float* act_f32 = nullptr;        // [kDecodeMaxTokens*k][d_ff]
   char* act_T = nullptr;           // [maxT*k][d_ff] model dtype (prefill)
-  float* ystage = nullptr;         // [maxT*k][d]
+  float* ystage = nullptr;         // [maxT*k][d] (prefill)
   char* xbuf[2] = {nullptr, nullptr};
   char* ybuf = nullptr;
   int* dbg_ids = nullptr;
@@ -78,14 +79,18 @@ struct wisp_ctx {
   u64 launches = 0;
   std::map<int, u64> graph_nodes;
 
-  std::map<int, cudaGraphExec_t> graphs;
+  std::map<int, cudaGraphExec_t> graphs;   // decode-sized stacks only (n_tokens <= kDecodeMaxTokens)
   int grid_fetch = 0;
-  StreamGeom geom_gu[2]{}, geom_dn[2]{};   // decode FFN stream geometry (gate/up, down); [0]: <= 2 tokens (16 rows per thread per stage), [1]: more (8)
-  // persistent decode kernel (decode_persistent.cuh)
+  // decode path (decode_*.cuh)
+  DecodeGeom dgeom[2]{};             // [0]: calls of at most 2 tokens, [1]: 3..8 tokens (larger work units: fewer chunk partials)
+  float* partial = nullptr;          // chunk partials P [pair position][NC][d]
+  long long* zfix = nullptr;         // [2][kDecodeMaxTokens][E] int64 logit accumulators (zero between launches)
+  unsigned* dsync = nullptr;         // [0] grid barrier counter, [1..2] unit tickets
   const char** d_masters = nullptr;  // device [L]: mapped master pointers
-  unsigned* gbar = nullptr;          // grid barrier counter
-  int* dev_err = nullptr;            // device error flag (grid barrier timeout)
-  u64* phase_ns = nullptr;           // device [kPersistPhases]
+  int* host_err = nullptr;           // mapped pinned flag: a grid barrier of the fused kernel timed out
+  int* dev_err = nullptr;            // its device alias
+  u64* phase_ns = nullptr;           // device [kDecPhases + 2]
+  size_t fused_smem = 0, ffn_smem = 0;   // dynamic shared memory available to the fused / split ffn kernel on this device
   int persist_enabled = 1;
   // tcgen05 prefill path (ffn_prefill_mma.cuh): TMA tensor maps over the arena / the B-operand buffers
   bool mma_ok = false;
@@ -93,14 +98,11 @@ struct wisp_ctx {
   void* encode_fn = nullptr;         // cuTensorMapEncodeTiled (per-call map over the caller's hidden states)
   char* xg = nullptr;                // [maxT*k][d] gathered token rows (bf16)
   int* mma_work = nullptr;           // work list of the current wave: (entry, first pair) items + count
-  u64 persist_layers_timed = 0;
-  bool use_persistent(int T_) const {
+  u64 fused_layers_timed = 0;
+  bool use_fused(int T_) const {
     return persist_enabled && cfg.fetch == WISP_FETCH_FUSED && T_ <= kDecodeMaxTokens && cfg.n_experts <= kPersistMaxExperts;
   }
   std::string err;
-  // programmatic dependent launch between the kernels of a layer (not with host-driven copies or event timing)
-  int use_pdl() const { return cfg.fetch != WISP_FETCH_MEMCPY && timing_level == 0 && pdl_enabled; }
-  int pdl_enabled = 1;
 };
 
 namespace {
@@ -183,11 +185,11 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 bool make_tmap(EncodeTiledFn fn, CUtensorMap* tm, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides_bytes,
-               const cuuint32_t* box) {
-  cuuint32_t estr[3] = {1, 1, 1};
+               const cuuint32_t* box, bool swizzle128) {
+  cuuint32_t estr[4] = {1, 1, 1, 1};
   return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, base, dims, strides_bytes, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+            CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 template <typename T>
@@ -201,7 +203,7 @@ int launch_router(wisp_ctx* ctx, int layer, const void* x, int T_, cudaStream_t 
     CUtensorMap tm_x;
     const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)T_}, str[1] = {(cuuint64_t)d * 2};
     const cuuint32_t box2[2] = {kMmaBK, kMmaNT};
-    if (!make_tmap(reinterpret_cast<EncodeTiledFn>(ctx->encode_fn), &tm_x, const_cast<void*>(x), 2, dims, str, box2))
+    if (!make_tmap(reinterpret_cast<EncodeTiledFn>(ctx->encode_fn), &tm_x, const_cast<void*>(x), 2, dims, str, box2, true))
       return fail(ctx, WISP_ECUDA, "tensor map over the hidden states failed (16-byte aligned rows required)");
     MmaArgs m{};
     m.L = cfg.n_layers; m.layer = layer; m.d = d; m.dff = cfg.d_ff; m.k = k;
@@ -217,8 +219,8 @@ int launch_router(wisp_ctx* ctx, int layer, const void* x, int T_, cudaStream_t 
   const size_t off = (size_t)layer * cfg.max_tokens * k;
   {
     Span sp(ctx, WISP_K_TOPK, st);
-    topk_softmax_kernel<<<(T_ + 3) / 4, 128, 4 * (E + k) * sizeof(float), st>>>(ctx->logits, ctx->ids + off, ctx->topw + off,
-                                                                          T_, E, k);
+    if (E <= 256) topk_softmax_kernel<8><<<(T_ + 3) / 4, 128, 0, st>>>(ctx->logits, ctx->ids + off, ctx->topw + off, T_, E, k);
+    else topk_softmax_kernel<kMaxExperts / 32><<<(T_ + 3) / 4, 128, 0, st>>>(ctx->logits, ctx->ids + off, ctx->topw + off, T_, E, k);
   }
   CK(cudaGetLastError());
   return WISP_OK;
@@ -290,97 +292,169 @@ int fetch_wave(wisp_ctx* ctx, int layer, int wave, bool host_known, cudaStream_t
   return WISP_OK;
 }
 
-constexpr size_t kStreamSmemMax = 216u << 10;   // dynamic shared memory ceiling of the ring (227 KiB per CTA minus static)
-
-// ---- decode FFN (ffn_stream.cuh) -------------------------------------------------------------------------
-StreamGeom make_geom(int K, int rows, int n_mats, size_t elem, size_t off0, size_t off1, int want_stages, int vals) {
-  StreamGeom g{};
-  g.K = K; g.rows = rows; g.n_mats = n_mats;
-  g.mat_off[0] = off0; g.mat_off[1] = off1;
-  g.row_bytes = (int)(K * elem);
-  const int n_chunks = g.row_bytes / 16;            // multiple of 32 (K is a multiple of 256)
-  int q = 8;                                        // segment = 32*q chunks, the largest divisor of the row that fits 256 threads
-  while ((n_chunks / 32) % q) --q;
-  g.P = 32 * q;
-  g.NSEG = n_chunks / g.P;
-  g.G = kStreamConsumers / g.P;
-  g.RB = (vals / n_mats) * g.G;
-  g.seg_bytes = g.P * 16;
-  g.stage_bytes = n_mats * g.RB * g.seg_bytes;
-  g.upe = rows / g.RB;
-  g.n_active = g.G * g.P;
-  int ns = want_stages > 0 ? want_stages : kStreamMaxStages;
-  ns = std::min(ns, (int)(kStreamSmemMax / g.stage_bytes));
-  g.n_stages = std::max(2, std::min(ns, kStreamMaxStages));
+// ---- decode path (decode_*.cuh) --------------------------------------------------------------------------------
+// Geometry of the fused FFN stream: slab = the largest multiple-of-256 divisor of d whose 8-row part fits 32 KiB.
+DecodeGeom make_decode_geom(int d, int dff, size_t elem, int rows_unit) {
+  DecodeGeom g{};
+  g.d = d; g.dff = dff; g.elem = (int)elem; g.kc = (int)(16 / elem);
+  int m = (int)(kDecMaxPartBytes / (8 * elem)) / 256;
+  const int q = d / 256;
+  while (q % m) --m;
+  g.slab = 256 * m;
+  g.n_slab = d / g.slab;
+  g.part_bytes = 8 * g.slab * (int)elem;
+  g.rows_unit = rows_unit;
+  g.n_sb = rows_unit / 8;
+  g.n_chunks = dff / rows_unit;
+  g.parts_unit = 3 * g.n_sb * g.n_slab;
+  g.steps = g.slab / 128;
+  g.down_pieces = 8 / g.kc;
+  g.up_off = (unsigned long long)dff * d * elem;
+  g.down_off = 2 * g.up_off;
+  g.group_bytes = 8ull * d * elem;
   return g;
 }
 
-template <typename T, int MODE, int NP>
-int launch_stream(wisp_ctx* ctx, const StreamArgs& a, const StreamGeom& g, cudaStream_t st) {
-  auto kern = ffn_stream_kernel<T, MODE, NP>;
-  const size_t smem = (size_t)g.n_stages * g.stage_bytes;
-  static bool attr_done = false;                    // per instantiation
-  if (!attr_done) {
-    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStreamSmemMax));
-    attr_done = true;
-  }
-  cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(ctx->num_sms);
-  cfg.blockDim = dim3(kStreamThreads);
-  cfg.dynamicSmemBytes = smem;
-  cfg.stream = st;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at;
-  cfg.numAttrs = a.pdl ? 1 : 0;
-  CK(cudaLaunchKernelEx(&cfg, kern, a, g));
+struct DecodeSmem { int n_slots, xs_pitch, xs_bytes; size_t bytes; };
+// Shared-memory carve-up of a decode CTA: [hidden states, rows padded by 16 B][ring of n_slots parts].
+int decode_smem(wisp_ctx* ctx, const DecodeGeom& g, int T_, size_t avail, DecodeSmem* out) {
+  out->xs_pitch = g.d + g.kc;
+  out->xs_bytes = (int)(((size_t)T_ * out->xs_pitch * g.elem + 127) & ~(size_t)127);
+  if ((size_t)out->xs_bytes + 2 * (size_t)g.part_bytes > avail) return fail(ctx, WISP_EINVAL, "decode kernel: shared memory too small for this shape");
+  int n = (int)std::min<size_t>(kDecMaxSlots, (avail - out->xs_bytes) / g.part_bytes);
+  if (ctx->cfg.ring_stages > 0) n = std::min(n, std::max(2, (int)ctx->cfg.ring_stages));
+  out->n_slots = n;
+  out->bytes = (size_t)out->xs_bytes + (size_t)n * g.part_bytes;
   return WISP_OK;
 }
 
-template <typename T, int MODE>
-int launch_stream_np(wisp_ctx* ctx, const StreamArgs& a, const StreamGeom& g, int T_, cudaStream_t st) {
-  if (T_ <= 1) return launch_stream<T, MODE, 1>(ctx, a, g, st);
-  if (T_ <= 2) return launch_stream<T, MODE, 2>(ctx, a, g, st);
-  if (T_ <= 4) return launch_stream<T, MODE, 4>(ctx, a, g, st);
-  return launch_stream<T, MODE, 8>(ctx, a, g, st);
+// A grid barrier of the fused kernel timed out in an earlier launch: report it once, put the device-side protocol state back.
+int check_dev_err(wisp_ctx* ctx) {
+  if (!ctx->host_err || !*reinterpret_cast<volatile int*>(ctx->host_err)) return WISP_OK;
+  cudaDeviceSynchronize();
+  *reinterpret_cast<volatile int*>(ctx->host_err) = 0;
+  cudaMemset(ctx->zfix, 0, 2 * (size_t)kDecodeMaxTokens * ctx->cfg.n_experts * sizeof(long long));
+  cudaMemset(ctx->dsync, 0, 4 * sizeof(unsigned));
+  return fail(ctx, WISP_ECUDA, "fused decode kernel: a grid-wide barrier timed out; the outputs of that forward are invalid");
 }
 
 template <typename T>
-int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, cudaStream_t st) {
+int launch_fused(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out, bool residual, cudaStream_t st) {
+  const auto& cfg = ctx->cfg;
+  DecodeArgs pa{};
+  pa.L = cfg.n_layers; pa.E = cfg.n_experts; pa.k = cfg.top_k; pa.d = cfg.d_model; pa.dff = cfg.d_ff; pa.T = T_; pa.C = ctx->C;
+  pa.policy = cfg.policy; pa.wave_order = ctx->wave_order; pa.layer_lo = lo; pa.layer_hi = hi; pa.residual = residual ? 1 : 0;
+  pa.pool = ctx->arena; pa.masters = reinterpret_cast<const char* const*>(ctx->d_masters); pa.blob_bytes = ctx->Me;
+  pa.router_wt = ctx->router_wt; pa.router_bias = ctx->router_bias;
+  pa.pi = ctx->pi; pa.pi_inv = ctx->pi_inv; pa.tau = ctx->tau; pa.freq = ctx->freq; pa.scal = ctx->scal;
+  pa.last_pos = ctx->last_pos; pa.hist = ctx->hist;
+  pa.logits = ctx->logits; pa.ids = ctx->ids; pa.topw = ctx->topw; pa.max_tokens = cfg.max_tokens;
+  pa.partial = ctx->partial; pa.zfix = ctx->zfix; pa.sync = ctx->dsync;
+  pa.x_in = x; pa.xbuf[0] = ctx->xbuf[0]; pa.xbuf[1] = ctx->xbuf[1]; pa.out = out;
+  pa.err = ctx->dev_err;
+  pa.trace = ctx->trace; pa.trace_ctr = ctx->trace_ctr; pa.trace_cap = ctx->trace_cap; pa.trace_on = ctx->trace_on;
+  pa.track = ctx->track;
+  pa.phase_ns = ctx->timing_level >= 2 ? ctx->phase_ns : nullptr;
+  DecodeGeom g = ctx->dgeom[T_ <= 2 ? 0 : 1];
+  DecodeSmem sm;
+  int rc = decode_smem(ctx, g, T_, ctx->fused_smem, &sm);
+  if (rc) return rc;
+  CK(cudaMemsetAsync(ctx->dsync, 0, 4 * sizeof(unsigned), st));
+  void* args[] = {&pa, &g, &sm.n_slots, &sm.xs_pitch, &sm.xs_bytes};
+  CK(cudaLaunchCooperativeKernel((const void*)decode_fused_kernel<T>, dim3(ctx->num_sms), dim3(kDecThreads), args, sm.bytes, st));
+  ++ctx->launches;
+  for (int l = lo; l < hi; ++l) ctx->last_T[l] = T_;
+  ctx->last_layer = hi - 1;
+  if (ctx->timing_level >= 2) ctx->fused_layers_timed += (u64)(hi - lo);
+  return WISP_OK;
+}
+
+int launch_fused_any(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out, bool residual, cudaStream_t st) {
+  return ctx->cfg.dtype == WISP_F32 ? launch_fused<float>(ctx, lo, hi, x, T_, out, residual, st)
+                                    : launch_fused<__nv_bfloat16>(ctx, lo, hi, x, T_, out, residual, st);
+}
+
+// Split form of one decode layer (MEMCPY / ZEROCOPY contexts, E > 256): logits, plan, per wave (fetch, ffn), combine -- the
+// same device functions as the fused kernel, so both give the same bits.  x_next != nullptr: residual successor instead of y.
+template <typename T>
+int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
+  const auto& cfg = ctx->cfg;
+  const int k = cfg.top_k, E = cfg.n_experts, d = cfg.d_model, L = cfg.n_layers;
+  const int n_pairs = T_ * k, n_slices = T_ * (d / kSliceCols);
+  const size_t off = (size_t)layer * cfg.max_tokens * k;
+  const bool memcpy_path = cfg.fetch == WISP_FETCH_MEMCPY;
+  const T* wrt = reinterpret_cast<const T*>(ctx->router_wt) + (size_t)layer * d * E;
+  {
+    Span sp(ctx, WISP_K_ROUTER, st);
+    decode_logits_kernel<T><<<std::min(n_slices, 4 * ctx->num_sms), 256, 0, st>>>(reinterpret_cast<const T*>(x), wrt, ctx->zfix, T_, E, d);
+  }
+  {
+    PlanArgs a;
+    a.ids = nullptr; a.n_pairs = n_pairs; a.E = E; a.C = ctx->C; a.policy = cfg.policy; a.layer = layer;
+    a.st = layer_state(ctx, layer); a.plan = ctx->plan; a.host_plan = memcpy_path ? ctx->host_plan : nullptr;
+    a.trace = ctx->trace; a.trace_ctr = ctx->trace_ctr; a.trace_cap = ctx->trace_cap; a.trace_on = ctx->trace_on;
+    a.wave_order = ctx->wave_order; a.track = ctx->track; a.build_pairs = 1;
+    Span sp(ctx, WISP_K_RESIDENCY, st);
+    const float* bias = ctx->router_bias + (size_t)layer * E;
+    if (E <= 256) decode_plan_kernel<256><<<1, 256, 0, st>>>(a, ctx->zfix, bias, ctx->logits, ctx->ids + off, ctx->topw + off, T_, k);
+    else decode_plan_kernel<kPlanThreads><<<1, kPlanThreads, 0, st>>>(a, ctx->zfix, bias, ctx->logits, ctx->ids + off, ctx->topw + off, T_, k);
+  }
+  CK(cudaGetLastError());
+  int n_waves;
+  if (memcpy_path) {
+    CK(cudaEventRecord(ctx->ev_plan, st));
+    CK(cudaEventSynchronize(ctx->ev_plan));      // the host must see the miss list
+    n_waves = ctx->host_plan->n_waves;
+  } else {
+    n_waves = (std::min(E, n_pairs) + ctx->C - 1) / ctx->C;   // worst case; empty waves exit at once
+  }
+  const DecodeGeom g = ctx->dgeom[T_ <= 2 ? 0 : 1];
+  DecodeSmem sm;
+  int rc = decode_smem(ctx, g, T_, ctx->ffn_smem, &sm);
+  if (rc) return rc;
+  DecodeFfnArgs fa{};
+  fa.pool = ctx->arena; fa.blob_bytes = ctx->Me; fa.L = L; fa.layer = layer; fa.k = k; fa.partial = ctx->partial;
+  fa.master = cfg.fetch == WISP_FETCH_FUSED ? static_cast<const char*>(ctx->master[layer]) : nullptr;
+  fa.ticket = ctx->dsync + 1;
+  for (int w = 0; w < n_waves; ++w) {
+    if (cfg.fetch != WISP_FETCH_FUSED) {
+      rc = fetch_wave(ctx, layer, w, memcpy_path, st);
+      if (rc) return rc;
+    }
+    CK(cudaMemsetAsync(ctx->dsync + 1, 0, sizeof(unsigned), st));
+    Span sp(ctx, WISP_K_FFN, st);
+    decode_ffn_kernel<T><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, w, ctx->C, E, T_, reinterpret_cast<const T*>(x),
+                                                                     sm.n_slots, sm.xs_pitch, sm.xs_bytes);
+  }
+  {
+    CombineArgs ca;
+    ca.partial = ctx->partial; ca.n_chunks = g.n_chunks; ca.d = d; ca.k = k; ca.topw = ctx->topw + off; ca.pair_pos = ctx->plan.pair_pos;
+    Span sp(ctx, WISP_K_COMBINE, st);
+    decode_combine_kernel<T><<<std::min(n_slices, 4 * ctx->num_sms), 256, 0, st>>>(
+        ca, x_next ? reinterpret_cast<const T*>(x) : nullptr, reinterpret_cast<T*>(x_next ? x_next : out), T_);
+  }
+  CK(cudaGetLastError());
+  ctx->last_T[layer] = T_;
+  ctx->last_layer = layer;
+  return WISP_OK;
+}
+
+// ---- prefill path: grouped GEMM per wave (n_tokens > kDecodeMaxTokens) ----------------------------------------------
+template <typename T>
+int launch_prefill_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, cudaStream_t st) {
   const auto& cfg = ctx->cfg;
   const int d = cfg.d_model, dff = cfg.d_ff, k = cfg.top_k, L = cfg.n_layers;
   const T* pool = reinterpret_cast<const T*>(ctx->arena);
-  if (T_ <= kDecodeMaxTokens) {
-    StreamArgs a{};
-    a.plan = ctx->plan; a.wave = wave; a.C = ctx->C;
-    a.pool = ctx->arena;
-    a.master = cfg.fetch == WISP_FETCH_FUSED ? static_cast<const char*>(ctx->master[layer]) : nullptr;
-    a.blob_bytes = ctx->Me; a.L = L; a.layer = layer; a.k = k;
-    a.pdl = ctx->use_pdl();
-    int rc;
-    {
-      Span sp(ctx, WISP_K_GATE_UP, st);
-      a.operand = x; a.result = ctx->act_f32; a.out_ld = dff;
-      rc = launch_stream_np<T, 0>(ctx, a, ctx->geom_gu[T_ <= 2 ? 0 : 1], T_, st);
-    }
-    if (rc) return rc;
-    {
-      Span sp(ctx, WISP_K_DOWN, st);
-      a.operand = ctx->act_f32; a.result = ctx->ystage; a.out_ld = d;
-      rc = launch_stream_np<T, 1>(ctx, a, ctx->geom_dn[T_ <= 2 ? 0 : 1], T_, st);
-    }
-    if (rc) return rc;
-  } else if (ctx->mma_ok) {
-    // tcgen05 grouped GEMM (bf16): xg was gathered once per forward (forward_layer); 4 / 6 ring stages of 48 / 32 KiB
+  if (ctx->mma_ok) {
+    // tcgen05 grouped GEMM (bf16): xg was gathered once per forward (forward_layer_prefill); 4 / 6 ring stages of 48 / 32 KiB
     MmaArgs m{};
     m.plan = ctx->plan; m.wave = wave; m.C = ctx->C; m.L = L; m.layer = layer; m.d = d; m.dff = dff; m.k = k;
     m.act = reinterpret_cast<__nv_bfloat16*>(ctx->act_T); m.ystage = ctx->ystage;
+    int* n_work = ctx->mma_work + 2 * (cfg.n_experts + cfg.max_tokens * k / kMmaNT + 1);
     {
       Span sp(ctx, WISP_K_OTHER, st);
-      build_work_kernel<<<1, 32, 0, st>>>(ctx->plan, wave, ctx->C, ctx->mma_work, ctx->mma_work + 2 * (cfg.n_experts + cfg.max_tokens * k / kMmaNT + 1));
+      build_work_kernel<<<1, 32, 0, st>>>(ctx->plan, wave, ctx->C, ctx->mma_work, n_work);
     }
-    const int* n_work = ctx->mma_work + 2 * (cfg.n_experts + cfg.max_tokens * k / kMmaNT + 1);
     {
       Span sp(ctx, WISP_K_PREFILL_GATE_UP, st);
       const int ns = 4;
@@ -411,9 +485,9 @@ int launch_ffn_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, c
   return WISP_OK;
 }
 
-// ---- tcgen05 prefill path: tensor maps -----------------------------------------------------------------------
-// K-major bf16 operands in boxes of [64 K-elements][128 rows]: weights through a 3-D view of the arena
-// (K, weight row, blob = slot*L + layer), tokens / activations through 2-D views of xg and act.
+// Tensor maps of the tcgen05 prefill path.  Weights: 4-D views of the arena in the tiled in-slot layout (common.cuh),
+// (64 elements of a core matrix, core column, core row, blob = slot*L + layer), no swizzle; tokens / activations: 2-D
+// K-major views of xg and act with the 128-byte swizzle; router rows: 3-D row-major view with the 128-byte swizzle.
 bool setup_mma_path(wisp_ctx* ctx) {
   const auto& cfg = ctx->cfg;
   if (cfg.dtype != WISP_BF16 || cfg.max_tokens <= kDecodeMaxTokens) return false;
@@ -426,26 +500,30 @@ bool setup_mma_path(wisp_ctx* ctx) {
   if (n_blobs < 1) return false;
   const cuuint32_t box3[3] = {kMmaBK, kMmaM, 1}, box2[2] = {kMmaBK, kMmaNT};
   {
-    const cuuint64_t dims[3] = {d, 2 * dff, n_blobs}, str[2] = {d * 2, ctx->Me};
-    if (!make_tmap(fn, &ctx->tm_gu, ctx->arena, 3, dims, str, box3)) return false;
+    // gate then up: core (r/8, k/8) at ((r/8)*(d/8) + k/8) * 128 B; a tile = 16 row groups x 8 K cores
+    const cuuint64_t dims[4] = {64, d / 8, 2 * dff / 8, n_blobs}, str[3] = {128, d * 16, ctx->Me};
+    const cuuint32_t box[4] = {64, kMmaBK / 8, kMmaM / 8, 1};
+    if (!make_tmap(fn, &ctx->tm_gu, ctx->arena, 4, dims, str, box, false)) return false;
   }
   {
-    const cuuint64_t dims[3] = {dff, d, n_blobs}, str[2] = {dff * 2, ctx->Me};
-    if (!make_tmap(fn, &ctx->tm_dn, ctx->arena + 2 * d * dff * 2, 3, dims, str, box3)) return false;
+    // down: core (j/8, i/8) at ((i/8)*(d/8) + j/8) * 128 B; a tile = 8 act-column blocks x 16 output groups
+    const cuuint64_t dims[4] = {64, d / 8, dff / 8, n_blobs}, str[3] = {128, d * 16, ctx->Me};
+    const cuuint32_t box[4] = {64, kMmaM / 8, kMmaBK / 8, 1};
+    if (!make_tmap(fn, &ctx->tm_dn, ctx->arena + 2 * d * dff * 2, 4, dims, str, box, false)) return false;
   }
   if (cudaMalloc(&ctx->xg, rows * d * 2) != cudaSuccess) return false;
   if (cudaMalloc(&ctx->mma_work, (2 * (size_t)(cfg.n_experts + cfg.max_tokens * cfg.top_k / kMmaNT + 1) + 1) * sizeof(int)) != cudaSuccess) return false;
   {
     const cuuint64_t dims[2] = {d, rows}, str[1] = {d * 2};
-    if (!make_tmap(fn, &ctx->tm_xg, ctx->xg, 2, dims, str, box2)) return false;
+    if (!make_tmap(fn, &ctx->tm_xg, ctx->xg, 2, dims, str, box2, true)) return false;
   }
   {
     const cuuint64_t dims[2] = {dff, rows}, str[1] = {dff * 2};
-    if (!make_tmap(fn, &ctx->tm_act, ctx->act_T, 2, dims, str, box2)) return false;
+    if (!make_tmap(fn, &ctx->tm_act, ctx->act_T, 2, dims, str, box2, true)) return false;
   }
   if (cfg.n_experts % kMmaM == 0) {   // router weights [L][E][d] as (K, expert row, layer)
     const cuuint64_t dims[3] = {d, (cuuint64_t)cfg.n_experts, (cuuint64_t)cfg.n_layers}, str[2] = {d * 2, (cuuint64_t)cfg.n_experts * d * 2};
-    if (!make_tmap(fn, &ctx->tm_rw, ctx->router_w, 3, dims, str, box3)) return false;
+    if (!make_tmap(fn, &ctx->tm_rw, ctx->router_w, 3, dims, str, box3, true)) return false;
   }
   for (int mode = 0; mode < 3; ++mode) {
     const void* k = mode == 0 ? (const void*)prefill_mma_kernel<0> : mode == 1 ? (const void*)prefill_mma_kernel<1> : (const void*)prefill_mma_kernel<2>;
@@ -454,79 +532,9 @@ bool setup_mma_path(wisp_ctx* ctx) {
   return true;
 }
 
-// ---- persistent decode kernel: layers [lo, hi) of one token batch in one cooperative launch ----------------------
-template <typename T, int NP>
-int launch_persistent_np(wisp_ctx* ctx, PersistArgs& pa, cudaStream_t st) {
-  auto kern = decode_persistent_kernel<T, NP>;
-  static int n_stages = 0, stride = 0;
-  static size_t smem = 0;
-  if (!n_stages) {                                  // per instantiation (geometry is per context shape: recomputed below if it changes)
-    cudaFuncAttributes fa;
-    CK(cudaFuncGetAttributes(&fa, kern));
-    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((227u << 10) - fa.sharedSizeBytes)));
-    smem = (227u << 10) - fa.sharedSizeBytes;
-  }
-  const int gi = pa.T <= 2 ? 0 : 1;
-  stride = std::max(ctx->geom_gu[gi].stage_bytes, ctx->geom_dn[gi].stage_bytes);
-  int xs_bytes = (int)(((size_t)pa.T * pa.d * ctx->elem + 1023) & ~(size_t)1023);   // hidden state copy per CTA
-  const int rows_per_cta = (pa.E + ctx->num_sms - 1) / ctx->num_sms;               // router rows staged per CTA
-  int rw_bytes = (int)(((size_t)rows_per_cta * pa.d * ctx->elem + 1023) & ~(size_t)1023);
-  xs_bytes += 0;
-  if ((size_t)xs_bytes + rw_bytes + 2 * (size_t)stride > smem) return fail(ctx, WISP_EINVAL, "persistent decode kernel: shared memory too small");
-  n_stages = (int)std::min<size_t>(kStreamMaxStages, (smem - xs_bytes - rw_bytes) / stride);
-  // Measured on B200 (Qwen3 shape, all-resident, 12 layers): 2 / 3 / 4 / 5 / 6 stages -> 0.581 / 0.577 / 0.578 / 0.593 / 0.597 ms
-  // per token at batch 1 and 1.09 vs 1.24 ms (3 vs 6) at batch 4; no difference at the Mixtral shape.  A deeper ring lets
-  // the producer run further into the down tiles while gate/up is still streaming, which costs more than it hides.
-  n_stages = std::min(n_stages, ctx->cfg.ring_stages > 0 ? (int)ctx->cfg.ring_stages : (gi == 0 ? 2 : 3));
-  if (n_stages < 2) return fail(ctx, WISP_EINVAL, "persistent decode kernel: ring does not fit shared memory");
-  CK(cudaMemsetAsync(ctx->gbar, 0, sizeof(unsigned), st));
-  StreamGeom ggu = ctx->geom_gu[gi], gdn = ctx->geom_dn[gi];
-  void* args[] = {&pa, &ggu, &gdn, &n_stages, &stride, &xs_bytes, &rw_bytes};
-  CK(cudaLaunchCooperativeKernel((const void*)kern, dim3(ctx->num_sms), dim3(kStreamThreads), args,
-                                 (size_t)xs_bytes + rw_bytes + (size_t)n_stages * stride, st));
-  ++ctx->launches;
-  return WISP_OK;
-}
-
+// One prefill MoE layer: router -> residency -> per wave (fetch, grouped GEMMs into ystage [T,k,d]) -> ordered combine (a5).
 template <typename T>
-int launch_persistent(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out, bool residual, cudaStream_t st) {
-  const auto& cfg = ctx->cfg;
-  PersistArgs pa{};
-  pa.L = cfg.n_layers; pa.E = cfg.n_experts; pa.k = cfg.top_k; pa.d = cfg.d_model; pa.dff = cfg.d_ff; pa.T = T_; pa.C = ctx->C;
-  pa.policy = cfg.policy; pa.layer_lo = lo; pa.layer_hi = hi; pa.residual = residual ? 1 : 0; pa.fused = 1;
-  pa.pool = ctx->arena; pa.masters = reinterpret_cast<const char* const*>(ctx->d_masters); pa.blob_bytes = ctx->Me;
-  pa.router_w = ctx->router_w; pa.router_bias = ctx->router_bias;
-  pa.pi = ctx->pi; pa.pi_inv = ctx->pi_inv; pa.tau = ctx->tau; pa.freq = ctx->freq; pa.scal = ctx->scal;
-  pa.last_pos = ctx->last_pos; pa.hist = ctx->hist;
-  pa.logits = ctx->logits; pa.ids = ctx->ids; pa.topw = ctx->topw; pa.max_tokens = cfg.max_tokens;
-  pa.act = ctx->act_f32; pa.ystage = ctx->ystage;
-  pa.x_in = x; pa.xbuf[0] = ctx->xbuf[0]; pa.xbuf[1] = ctx->xbuf[1]; pa.out = out;
-  pa.gbar = ctx->gbar; pa.err = ctx->dev_err;
-  pa.trace = ctx->trace; pa.trace_ctr = ctx->trace_ctr; pa.trace_cap = ctx->trace_cap; pa.trace_on = ctx->trace_on;
-  pa.wave_order = ctx->wave_order;
-  pa.track = ctx->track;
-  pa.phase_ns = ctx->timing_level >= 2 ? ctx->phase_ns : nullptr;
-  int rc;
-  if (T_ <= 1) rc = launch_persistent_np<T, 1>(ctx, pa, st);
-  else if (T_ <= 2) rc = launch_persistent_np<T, 2>(ctx, pa, st);
-  else if (T_ <= 4) rc = launch_persistent_np<T, 4>(ctx, pa, st);
-  else rc = launch_persistent_np<T, 8>(ctx, pa, st);
-  if (rc) return rc;
-  for (int l = lo; l < hi; ++l) ctx->last_T[l] = T_;
-  ctx->last_layer = hi - 1;
-  if (ctx->timing_level >= 2) ctx->persist_layers_timed += (u64)(hi - lo);
-  return WISP_OK;
-}
-
-int launch_persistent_any(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out, bool residual, cudaStream_t st) {
-  return ctx->cfg.dtype == WISP_F32 ? launch_persistent<float>(ctx, lo, hi, x, T_, out, residual, st)
-                                    : launch_persistent<__nv_bfloat16>(ctx, lo, hi, x, T_, out, residual, st);
-}
-
-// One MoE layer: router -> residency -> per wave (fetch, FFN) -> combine.  x_next != nullptr also writes
-// the residual successor (stack helper).
-template <typename T>
-int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
+int forward_layer_prefill(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
   const auto& cfg = ctx->cfg;
   const int k = cfg.top_k, E = cfg.n_experts;
   const int n_pairs = T_ * k;
@@ -544,18 +552,15 @@ int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, vo
   } else {
     n_waves = (std::min(E, n_pairs) + ctx->C - 1) / ctx->C;   // worst case; empty waves exit at once
   }
-  if (T_ > kDecodeMaxTokens && ctx->mma_ok) {      // B operand of GEMM 1: token rows in sorted-pair order
+  if (ctx->mma_ok) {                               // B operand of GEMM 1: token rows in sorted-pair order
     Span sp(ctx, WISP_K_OTHER, st);
     gather_tokens_kernel<<<std::min(n_pairs, 4 * ctx->num_sms), 256, 0, st>>>(ctx->plan.pair_list, n_pairs, k, cfg.d_model * 2 / 16,
                                                                              reinterpret_cast<const uint4*>(x), reinterpret_cast<uint4*>(ctx->xg));
   }
-  const bool fused_fill = cfg.fetch == WISP_FETCH_FUSED && T_ <= kDecodeMaxTokens;   // the FFN kernels fetch their own misses
   for (int w = 0; w < n_waves; ++w) {
-    if (!fused_fill) {
-      rc = fetch_wave(ctx, layer, w, memcpy_path, st);
-      if (rc) return rc;
-    }
-    rc = launch_ffn_wave<T>(ctx, layer, w, x, T_, st);
+    rc = fetch_wave(ctx, layer, w, memcpy_path, st);   // prefill under FUSED uses the zero-copy kernel
+    if (rc) return rc;
+    rc = launch_prefill_wave<T>(ctx, layer, w, x, T_, st);
     if (rc) return rc;
   }
   const size_t n = (size_t)T_ * cfg.d_model;
@@ -563,7 +568,7 @@ int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, vo
     Span sp(ctx, WISP_K_COMBINE, st);
     combine_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(ctx->ystage, ctx->topw + off, reinterpret_cast<T*>(out),
                                                                    x_next ? reinterpret_cast<const T*>(x) : nullptr,
-                                                                   reinterpret_cast<T*>(x_next), T_, cfg.d_model, k, 0);
+                                                                   reinterpret_cast<T*>(x_next), T_, cfg.d_model, k);
   }
   CK(cudaGetLastError());
   ctx->last_T[layer] = T_;
@@ -572,8 +577,12 @@ int forward_layer(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, vo
 }
 
 int forward_layer_any(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
-  return ctx->cfg.dtype == WISP_F32 ? forward_layer<float>(ctx, layer, x, T_, out, x_next, st)
-                                    : forward_layer<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st);
+  const bool f32 = ctx->cfg.dtype == WISP_F32;
+  if (T_ <= kDecodeMaxTokens)
+    return f32 ? forward_layer_decode<float>(ctx, layer, x, T_, out, x_next, st)
+               : forward_layer_decode<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st);
+  return f32 ? forward_layer_prefill<float>(ctx, layer, x, T_, out, x_next, st)
+             : forward_layer_prefill<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st);
 }
 
 int check_forward_args(wisp_ctx* ctx, int layer_lo, int layer_hi, const void* hidden, int n_tokens, void* out) {
@@ -594,18 +603,53 @@ int occupancy_grid(wisp_ctx* ctx, F kernel, int threads, int cap_per_sm) {
   return ctx->num_sms * std::min(nb, cap_per_sm);
 }
 
+
+// Re-tile the caller's canonical blobs ([gate | up | down], row-major out x in) into the in-slot layout of common.cuh:
+// 8-row x 16-byte core matrices, gate/up cores ordered (row group, K), down cores ordered (act-column block, output group).
+// Pure byte movement in 16-byte pieces, spread over host threads (a layer is 1-3 GiB).
+void retile_layer(const char* src, char* dst, size_t E, size_t d, size_t dff, size_t elem) {
+  const size_t kc = 16 / elem, Me = 3 * d * dff * elem, mat = d * dff * elem;
+  const size_t gu_items = E * 2 * (dff / 8);                 // (expert, gate|up, row group)
+  const size_t ib_per = dff / kc, line_ib = std::max<size_t>(1, 64 / 16);   // down: 4 act-column blocks share a 64-byte line
+  const size_t dn_items = E * ((ib_per + line_ib - 1) / line_ib);
+  const size_t total = gu_items + dn_items;
+  const unsigned hw = std::thread::hardware_concurrency();
+  const size_t nthr = std::min<size_t>(32, std::max<size_t>(4, hw ? hw : 8));
+  auto work = [=](size_t lo, size_t hi) {
+    for (size_t it = lo; it < hi; ++it) {
+      if (it < gu_items) {
+        const size_t e = it / (2 * (dff / 8)), rem = it % (2 * (dff / 8)), m = rem / (dff / 8), rg = rem % (dff / 8);
+        const char* s0 = src + e * Me + m * mat + rg * 8 * d * elem;
+        char* o = dst + e * Me + m * mat + rg * 8 * d * elem;
+        for (size_t kb = 0; kb < d / kc; ++kb)
+          for (size_t r = 0; r < 8; ++r) std::memcpy(o + (kb * 8 + r) * 16, s0 + r * d * elem + kb * 16, 16);
+      } else {
+        const size_t q = it - gu_items, groups = (ib_per + line_ib - 1) / line_ib, e = q / groups, ib0 = (q % groups) * line_ib;
+        const size_t nib = std::min(line_ib, ib_per - ib0);
+        const char* s0 = src + e * Me + 2 * mat;             // down [d][dff]
+        char* o = dst + e * Me + 2 * mat;
+        for (size_t j = 0; j < d; ++j)
+          for (size_t b = 0; b < nib; ++b)
+            std::memcpy(o + (((ib0 + b) * (d / 8) + j / 8) * 8 + (j & 7)) * 16, s0 + (j * dff + (ib0 + b) * kc) * elem, 16);
+      }
+    }
+  };
+  std::vector<std::thread> th;
+  const size_t per = (total + nthr - 1) / nthr;
+  for (size_t i = 0; i < nthr; ++i) {
+    const size_t lo = i * per, hi = std::min(total, lo + per);
+    if (lo >= hi) break;
+    th.emplace_back(work, lo, hi);
+  }
+  for (auto& t : th) t.join();
+}
+
 }  // namespace
 
 extern "C" {
 
 const char* wisp_version(void) { return kVersion; }
 
-#ifdef WISP_PROBE_TIMELINE
-int wisp_debug_probe_read(wisp_ctx* ctx, unsigned long long* out, int n) {   // profiling probe builds only
-  cudaDeviceSynchronize();
-  return cudaMemcpy(out, ctx->phase_ns + 16, (size_t)n * sizeof(u64), cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -3;
-}
-#endif
 
 const char* wisp_last_error(wisp_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
@@ -617,7 +661,8 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
       cfg->d_ff < 256 || cfg->d_ff % 256 || cfg->max_tokens < 1 ||
       (cfg->dtype != WISP_F32 && cfg->dtype != WISP_BF16) || (cfg->policy != WISP_LRU && cfg->policy != WISP_LFU) ||
       (cfg->fetch != WISP_FETCH_MEMCPY && cfg->fetch != WISP_FETCH_ZEROCOPY && cfg->fetch != WISP_FETCH_FUSED) ||
-      cfg->ring_stages < 0 || cfg->ring_stages > kStreamMaxStages)
+      cfg->ring_stages < 0 || cfg->ring_stages > kDecMaxSlots || cfg->unit_rows < 0 || cfg->unit_rows % 8 ||
+      (cfg->unit_rows > 0 && (cfg->d_ff % cfg->unit_rows || (cfg->d_ff / cfg->unit_rows) % 8)))
     return WISP_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return WISP_ECUDA;   // no CPU fallback
@@ -660,6 +705,7 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   ctx->num_sms = prop.multiProcessorCount;
   CKC(cudaMalloc(&ctx->arena, budget_bytes));
   CKC(cudaMalloc(&ctx->router_w, (size_t)L * E * d * ctx->elem));
+  CKC(cudaMalloc(&ctx->router_wt, (size_t)L * E * d * ctx->elem));
   CKC(cudaMalloc(&ctx->router_bias, (size_t)L * E * sizeof(float)));
   CKC(cudaMalloc(&ctx->pi, (size_t)L * E * sizeof(int)));
   CKC(cudaMalloc(&ctx->pi_inv, (size_t)L * E * sizeof(int)));
@@ -677,9 +723,10 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   CKC(cudaMemset(ctx->hist, 0, (size_t)L * (E + 2) * sizeof(u64)));
   CKC(cudaMalloc(&ctx->logits, maxT * E * sizeof(float)));
   CKC(cudaMalloc(&ctx->ids, (size_t)L * maxT * k * sizeof(int)));
+  CKC(cudaMemset(ctx->ids, 0, (size_t)L * maxT * k * sizeof(int)));
   CKC(cudaMalloc(&ctx->topw, (size_t)L * maxT * k * sizeof(float)));
   {
-    const size_t n_int = 4 + 3 * (size_t)E + E + (E + 1) + maxT * k;
+    const size_t n_int = 4 + 3 * (size_t)E + E + (E + 1) + 2 * maxT * k + E;
     CKC(cudaMalloc(&ctx->plan_mem, n_int * sizeof(int)));
     CKC(cudaMemset(ctx->plan_mem, 0, n_int * sizeof(int)));
     int* p = ctx->plan_mem;
@@ -689,11 +736,12 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
     ctx->plan.entry_miss = p; p += E;
     ctx->plan.exp_count = p; p += E;
     ctx->plan.exp_offset = p; p += E + 1;
-    ctx->plan.pair_list = p;
+    ctx->plan.pair_list = p; p += maxT * k;
+    ctx->plan.pair_pos = p; p += maxT * k;
+    ctx->plan.unit_entry = p;
   }
   CKC(cudaHostAlloc(&ctx->host_plan, sizeof(HostPlan), cudaHostAllocMapped));
   std::memset(ctx->host_plan, 0, sizeof(HostPlan));
-  CKC(cudaMalloc(&ctx->act_f32, (size_t)kDecodeMaxTokens * k * dff * sizeof(float)));
   CKC(cudaMalloc(&ctx->act_T, maxT * k * dff * ctx->elem));
   CKC(cudaMalloc(&ctx->ystage, maxT * k * d * sizeof(float)));
   CKC(cudaMalloc(&ctx->xbuf[0], maxT * d * ctx->elem));
@@ -706,24 +754,42 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   CKC(cudaMemset(ctx->trace_ctr, 0, 2 * sizeof(u64)));
   CKC(cudaMalloc(&ctx->d_masters, (size_t)L * sizeof(char*)));
   CKC(cudaMemset(ctx->d_masters, 0, (size_t)L * sizeof(char*)));
-  CKC(cudaMalloc(&ctx->gbar, sizeof(unsigned)));
-  CKC(cudaMalloc(&ctx->dev_err, sizeof(int)));
-  CKC(cudaMemset(ctx->dev_err, 0, sizeof(int)));
-  CKC(cudaMalloc(&ctx->phase_ns, (16 + 8 * 256) * sizeof(u64)));   // phases, 2 counters, (probe builds) per-CTA times
-  CKC(cudaMemset(ctx->phase_ns, 0, (16 + 8 * 256) * sizeof(u64)));
+  CKC(cudaMalloc(&ctx->dsync, 4 * sizeof(unsigned)));
+  CKC(cudaMemset(ctx->dsync, 0, 4 * sizeof(unsigned)));
+  CKC(cudaMalloc(&ctx->zfix, 2 * (size_t)kDecodeMaxTokens * E * sizeof(long long)));
+  CKC(cudaMemset(ctx->zfix, 0, 2 * (size_t)kDecodeMaxTokens * E * sizeof(long long)));
+  CKC(cudaHostAlloc(&ctx->host_err, sizeof(int), cudaHostAllocMapped));
+  *ctx->host_err = 0;
+  CKC(cudaHostGetDevicePointer(reinterpret_cast<void**>(&ctx->dev_err), ctx->host_err, 0));
+  CKC(cudaMalloc(&ctx->phase_ns, (kDecPhases + 2) * sizeof(u64)));
+  CKC(cudaMemset(ctx->phase_ns, 0, (kDecPhases + 2) * sizeof(u64)));
+  {
+    // Work-unit size of the decode FFN: 8 act rows (96 KiB of weights at the Qwen3 shape) for calls of at most 2 tokens, 16
+    // for 3..8 tokens, where more experts are in flight and every routed pair writes its own chunk partials.  fp32 models
+    // (config 1, parity only) always use 8.
+    const int r0 = cfg->unit_rows > 0 && cfg->dtype != WISP_F32 ? cfg->unit_rows : 8;
+    const int r1 = cfg->dtype == WISP_F32 ? 8 : cfg->unit_rows > 0 ? cfg->unit_rows : 16;
+    ctx->dgeom[0] = make_decode_geom(d, dff, ctx->elem, r0);
+    ctx->dgeom[1] = make_decode_geom(d, dff, ctx->elem, r1);
+    const size_t t_dec = std::min<size_t>(maxT, kDecodeMaxTokens);
+    const size_t pairs0 = std::min<size_t>(t_dec, 2) * k, pairs1 = t_dec * k;
+    const size_t n_part = std::max(pairs0 * ctx->dgeom[0].n_chunks, pairs1 * ctx->dgeom[1].n_chunks) * d;
+    CKC(cudaMalloc(&ctx->partial, n_part * sizeof(float)));
+    cudaFuncAttributes fa;
+    const void* kf = cfg->dtype == WISP_F32 ? (const void*)decode_fused_kernel<float> : (const void*)decode_fused_kernel<__nv_bfloat16>;
+    const void* kn = cfg->dtype == WISP_F32 ? (const void*)decode_ffn_kernel<float> : (const void*)decode_ffn_kernel<__nv_bfloat16>;
+    CKC(cudaFuncGetAttributes(&fa, kf));
+    ctx->fused_smem = (227u << 10) - fa.sharedSizeBytes;
+    CKC(cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->fused_smem));
+    CKC(cudaFuncGetAttributes(&fa, kn));
+    ctx->ffn_smem = (227u << 10) - fa.sharedSizeBytes;
+    CKC(cudaFuncSetAttribute(kn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->ffn_smem));
+  }
   CKC(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
   CKC(cudaEventCreateWithFlags(&ctx->ev_plan, cudaEventDisableTiming));
   CKC(cudaEventCreateWithFlags(&ctx->ev_compute, cudaEventDisableTiming));
   CKC(cudaEventCreateWithFlags(&ctx->ev_copy, cudaEventDisableTiming));
 #undef CKC
-  {
-    const size_t gu = (size_t)d * dff * ctx->elem;
-    for (int gi = 0; gi < 2; ++gi) {
-      const int vals = stream_vals_for_tokens(gi == 0 ? 1 : kDecodeMaxTokens);
-      ctx->geom_gu[gi] = make_geom(d, dff, 2, ctx->elem, 0, gu, cfg->ring_stages, vals);
-      ctx->geom_dn[gi] = make_geom(dff, d, 1, ctx->elem, 2 * gu, 0, cfg->ring_stages, vals);
-    }
-  }
   ctx->grid_fetch = ctx->num_sms * 2;
   ctx->mma_ok = setup_mma_path(ctx);
   if (cfg->dtype == WISP_BF16 && cfg->max_tokens > kDecodeMaxTokens && !ctx->mma_ok) {
@@ -743,12 +809,13 @@ int wisp_destroy(wisp_ctx* ctx) {
     if (m) cudaFreeHost(m);
   void* dev_ptrs[] = {ctx->arena,    ctx->router_w, ctx->router_bias, ctx->pi,      ctx->pi_inv,  ctx->tau,
                       ctx->freq,     ctx->scal,     ctx->last_pos,    ctx->hist,    ctx->logits,  ctx->ids,
-                      ctx->topw,     ctx->plan_mem, ctx->act_f32,     ctx->act_T,   ctx->ystage,  ctx->xbuf[0],
+                      ctx->topw,     ctx->plan_mem, ctx->router_wt,   ctx->act_T,   ctx->ystage,  ctx->xbuf[0],
                       ctx->xbuf[1],  ctx->ybuf,     ctx->dbg_ids,     ctx->moves,   ctx->bad_slots, ctx->trace,
-                      ctx->trace_ctr, ctx->d_masters, ctx->gbar, ctx->dev_err, ctx->phase_ns, ctx->xg, ctx->mma_work};
+                      ctx->trace_ctr, ctx->d_masters, ctx->dsync, ctx->zfix, ctx->partial, ctx->phase_ns, ctx->xg, ctx->mma_work};
   for (void* p : dev_ptrs)
     if (p) cudaFree(p);
   if (ctx->host_plan) cudaFreeHost(ctx->host_plan);
+  if (ctx->host_err) cudaFreeHost(ctx->host_err);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   for (cudaEvent_t e : {ctx->ev_plan, ctx->ev_compute, ctx->ev_copy})
     if (e) cudaEventDestroy(e);
@@ -768,19 +835,17 @@ int wisp_register_host_experts(wisp_ctx* ctx, int32_t layer, const void* experts
   const size_t E = ctx->cfg.n_experts, d = ctx->cfg.d_model;
   void* m = nullptr;
   CK(cudaHostAlloc(&m, E * ctx->Me, cudaHostAllocMapped | cudaHostAllocPortable));
-  {  // parallel host copy: 1 GiB-class blobs per layer, one memcpy thread is far below DRAM bandwidth
-    const size_t total = E * ctx->Me, nthr = 8, part = (total / nthr + 4095) & ~(size_t)4095;
-    std::vector<std::thread> th;
-    for (size_t i = 0; i < nthr; ++i) {
-      const size_t lo = i * part, hi = std::min(total, lo + part);
-      if (lo >= hi) break;
-      th.emplace_back([=] { std::memcpy(static_cast<char*>(m) + lo, static_cast<const char*>(experts) + lo, hi - lo); });
-    }
-    for (auto& t : th) t.join();
-  }
+  retile_layer(static_cast<const char*>(experts), static_cast<char*>(m), E, d, ctx->cfg.d_ff, ctx->elem);
   ctx->master[layer] = m;
   CK(cudaMemcpy(ctx->d_masters + layer, &m, sizeof(char*), cudaMemcpyHostToDevice));
   CK(cudaMemcpy(ctx->router_w + (size_t)layer * E * d * ctx->elem, router_w, E * d * ctx->elem, cudaMemcpyHostToDevice));
+  {  // transposed copy [d][E] for the decode path's 16-column logit slices
+    std::vector<char> wt(E * d * ctx->elem);
+    const char* w = static_cast<const char*>(router_w);
+    for (size_t e = 0; e < E; ++e)
+      for (size_t j = 0; j < d; ++j) std::memcpy(wt.data() + (j * E + e) * ctx->elem, w + (e * d + j) * ctx->elem, ctx->elem);
+    CK(cudaMemcpy(ctx->router_wt + (size_t)layer * E * d * ctx->elem, wt.data(), wt.size(), cudaMemcpyHostToDevice));
+  }
   if (router_bias) CK(cudaMemcpy(ctx->router_bias + (size_t)layer * E, router_bias, E * sizeof(float), cudaMemcpyHostToDevice));
   else CK(cudaMemset(ctx->router_bias + (size_t)layer * E, 0, E * sizeof(float)));
   ctx->registered[layer] = 1;
@@ -791,8 +856,9 @@ int wisp_moe_forward(wisp_ctx* ctx, int32_t layer, const void* hidden, int32_t n
   int rc = check_forward_args(ctx, layer, layer + 1, hidden, n_tokens, out);
   if (rc) return rc;
   if (n_tokens == 0) return WISP_OK;
-  if (ctx->use_persistent(n_tokens))
-    return launch_persistent_any(ctx, layer, layer + 1, hidden, n_tokens, out, false, static_cast<cudaStream_t>(cuda_stream));
+  if ((rc = check_dev_err(ctx))) return rc;
+  if (ctx->use_fused(n_tokens))
+    return launch_fused_any(ctx, layer, layer + 1, hidden, n_tokens, out, false, static_cast<cudaStream_t>(cuda_stream));
   return forward_layer_any(ctx, layer, hidden, n_tokens, out, nullptr, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -802,7 +868,8 @@ int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void
   if (n_tokens == 0) return WISP_OK;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const int L = ctx->cfg.n_layers;
-  if (ctx->use_persistent(n_tokens)) return launch_persistent_any(ctx, 0, L, hidden, n_tokens, hidden_out, true, st);
+  if ((rc = check_dev_err(ctx))) return rc;
+  if (ctx->use_fused(n_tokens)) return launch_fused_any(ctx, 0, L, hidden, n_tokens, hidden_out, true, st);
   const size_t bytes = (size_t)n_tokens * ctx->cfg.d_model * ctx->elem;
   CK(cudaMemcpyAsync(ctx->xbuf[0], hidden, bytes, cudaMemcpyDeviceToDevice, st));
   auto chain = [&](cudaStream_t s) -> int {
@@ -812,7 +879,7 @@ int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void
     }
     return WISP_OK;
   };
-  if (ctx->cfg.fetch != WISP_FETCH_MEMCPY && ctx->timing_level == 0 && st != nullptr) {
+  if (ctx->cfg.fetch != WISP_FETCH_MEMCPY && ctx->timing_level == 0 && st != nullptr && n_tokens <= kDecodeMaxTokens) {
     auto it = ctx->graphs.find(n_tokens);
     if (it == ctx->graphs.end()) {
       cudaGraph_t g = nullptr;
@@ -914,9 +981,8 @@ int wisp_stats(wisp_ctx* ctx, wisp_stats_t* out) {
   std::vector<u64> s((size_t)L * 8);
   CK(cudaDeviceSynchronize());
   {
-    int derr = 0;
-    CK(cudaMemcpy(&derr, ctx->dev_err, sizeof(int), cudaMemcpyDeviceToHost));
-    if (derr) return fail(ctx, WISP_ECUDA, "persistent decode kernel: grid barrier timed out");
+    const int rc = check_dev_err(ctx);
+    if (rc) return rc;
   }
   CK(cudaMemcpy(s.data(), ctx->scal, s.size() * sizeof(u64), cudaMemcpyDeviceToHost));
   for (int l = 0; l < L; ++l) {
@@ -965,6 +1031,7 @@ int wisp_set_wave_order(wisp_ctx* ctx, int32_t order) {
 int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t* n_out) {
   if (!ctx || !n_out || (cap && !buf)) return fail(ctx, WISP_EINVAL, "bad argument");
   CK(cudaDeviceSynchronize());
+  { const int rc_ = check_dev_err(ctx); if (rc_) return rc_; }
   u64 tc[2];
   CK(cudaMemcpy(tc, ctx->trace_ctr, sizeof(tc), cudaMemcpyDeviceToHost));
   const u64 n = std::min<u64>(cap, tc[0]);
@@ -984,6 +1051,7 @@ int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t
 int wisp_last_topk(wisp_ctx* ctx, int32_t layer, int32_t* ids, float* w, int32_t* n_tokens_out) {
   if (!ctx || layer < 0 || layer >= ctx->cfg.n_layers) return fail(ctx, WISP_EINVAL, "bad argument");
   CK(cudaDeviceSynchronize());
+  { const int rc_ = check_dev_err(ctx); if (rc_) return rc_; }
   const int T_ = ctx->last_T[layer];
   const size_t off = (size_t)layer * ctx->cfg.max_tokens * ctx->cfg.top_k, n = (size_t)T_ * ctx->cfg.top_k;
   if (ids && n) CK(cudaMemcpy(ids, ctx->ids + off, n * sizeof(int), cudaMemcpyDeviceToHost));
@@ -995,6 +1063,7 @@ int wisp_last_topk(wisp_ctx* ctx, int32_t layer, int32_t* ids, float* w, int32_t
 int wisp_last_logits(wisp_ctx* ctx, float* z, int32_t n_tokens) {
   if (!ctx || !z || n_tokens < 0 || n_tokens > ctx->cfg.max_tokens) return fail(ctx, WISP_EINVAL, "bad argument");
   CK(cudaDeviceSynchronize());
+  { const int rc_ = check_dev_err(ctx); if (rc_) return rc_; }
   if (n_tokens) CK(cudaMemcpy(z, ctx->logits, (size_t)n_tokens * ctx->cfg.n_experts * sizeof(float), cudaMemcpyDeviceToHost));
   return WISP_OK;
 }
@@ -1070,25 +1139,17 @@ int wisp_timing_read(wisp_ctx* ctx, double* ms, uint64_t* launches, int32_t rese
   if (!ctx || !ms || !launches) return fail(ctx, WISP_EINVAL, "bad argument");
   CK(cudaDeviceSynchronize());
   harvest_timing(ctx, true);
-  if (ctx->persist_layers_timed) {   // phases of the persistent decode kernel, stamped with %globaltimer by CTA 0
-    u64 ns[kPersistPhases];
+  if (ctx->fused_layers_timed) {   // phases of the fused decode kernel, stamped with %globaltimer by CTA 0
+    u64 ns[kDecPhases + 2];         // + layer calls without a miss, with a miss
     CK(cudaMemcpy(ns, ctx->phase_ns, sizeof(ns), cudaMemcpyDeviceToHost));
     CK(cudaMemset(ctx->phase_ns, 0, sizeof(ns)));
-    const int cls[kPersistPhases] = {WISP_K_ROUTER, WISP_K_TOPK, WISP_K_RESIDENCY, WISP_K_OTHER, WISP_K_GATE_UP, WISP_K_DOWN,
-                                     WISP_K_COMBINE, WISP_K_GATE_UP_MISS, WISP_K_DOWN_MISS};
-    u64 cnt[2];                       // [0] layer calls without a miss, [1] with
-    CK(cudaMemcpy(cnt, ctx->phase_ns + kPersistPhases, sizeof(cnt), cudaMemcpyDeviceToHost));
-    CK(cudaMemset(ctx->phase_ns + kPersistPhases, 0, sizeof(cnt)));
-    for (int i = 0; i < kPersistPhases; ++i) {
+    const int cls[kDecPhases] = {WISP_K_ROUTER, WISP_K_RESIDENCY, WISP_K_OTHER, WISP_K_FFN, WISP_K_FFN_MISS, WISP_K_COMBINE};
+    const u64 n_hit = ns[kDecPhases], n_miss = ns[kDecPhases + 1];
+    for (int i = 0; i < kDecPhases; ++i) {
       ctx->class_ms[cls[i]] += (double)ns[i] * 1e-6;
-#ifdef WISP_PROBE_TIMELINE
-      ctx->class_n[cls[i]] += cnt[0];
-      continue;
-#endif
-      ctx->class_n[cls[i]] += cls[i] == WISP_K_GATE_UP || cls[i] == WISP_K_DOWN ? cnt[0]
-                              : cls[i] == WISP_K_GATE_UP_MISS || cls[i] == WISP_K_DOWN_MISS ? cnt[1] : cnt[0] + cnt[1];
+      ctx->class_n[cls[i]] += cls[i] == WISP_K_FFN ? n_hit : cls[i] == WISP_K_FFN_MISS ? n_miss : n_hit + n_miss;
     }
-    ctx->persist_layers_timed = 0;
+    ctx->fused_layers_timed = 0;
   }
   for (int i = 0; i < WISP_N_KERNEL_CLASSES; ++i) { ms[i] = ctx->class_ms[i]; launches[i] = ctx->class_n[i]; }
   if (reset)
