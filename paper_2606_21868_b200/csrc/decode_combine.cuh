@@ -29,13 +29,14 @@ __device__ __forceinline__ long long logit_to_fix(float v) {
 __device__ __forceinline__ float logit_from_fix(long long f, float bias) { return (float)((double)f * kLogitFixInv) + bias; }
 
 // Partial logits of one 16-column slice of token t's hidden state (xn[16], fp32 images of the model-dtype values) for all
-// experts, added into zfix[t][e].  wrt: this layer's router weights TRANSPOSED, [d][E] in the model dtype.
+// experts, added into zfix[t][e].  w16: rows j0 .. j0+15 of this layer's router weights TRANSPOSED ([d][E], model dtype), in
+// global memory or staged in shared memory.
 template <typename T>
-__device__ __forceinline__ void slice_logits(const T* __restrict__ wrt, const float* xn, int j0, int E, long long* zfix_t, int tid, int nthr) {
+__device__ __forceinline__ void slice_logits(const T* w16, const float* xn, int E, long long* zfix_t, int tid, int nthr) {
   for (int e = tid; e < E; e += nthr) {
     float zp = 0.f;
 #pragma unroll
-    for (int jj = 0; jj < kSliceCols; ++jj) zp = fmaf(to_f32<T>(wrt[(size_t)(j0 + jj) * E + e]), xn[jj], zp);
+    for (int jj = 0; jj < kSliceCols; ++jj) zp = fmaf(to_f32<T>(w16[(size_t)jj * E + e]), xn[jj], zp);
     atomicAdd(reinterpret_cast<unsigned long long*>(zfix_t + e), (unsigned long long)logit_to_fix(zp));
   }
 }

@@ -15,17 +15,20 @@
 // handed out DYNAMICALLY (one atomic ticket per unit): the two dies of a B200 stream at different rates and a static
 // split leaves the faster one idle at the barrier.
 //
-// Data path per CTA (288 threads): a producer warp takes tickets and streams each unit's parts (8 rows x one slab of at most
-// 32 KiB) through a shared-memory ring with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx); 8 consumer warps
-// compute.  bf16: the products run on the tensor cores through mma.sync.m16n8k16 (the 8 MMA columns are the tokens routed
-// to the expert; A fragments come straight from the ring with ldmatrix, each core matrix being 128 contiguous bytes), so
-// the arithmetic leaves the FMA pipes and the kernel stays a pure HBM stream at 1..8 tokens (1 flop/byte: this is an ALU
-// offload of a memory-bound kernel, not a GEMM -- units of 96 KiB are far too small for tcgen05's 128-row tiles).
-// fp32 (config 1, parity only): plain FMA with the same data flow and the same reduction tree.
-//   gate/up of a sub-block of 8 act rows: warp w owns the K range [w, w+1) * slab/8 of every slab; its 16 x 8 partial tile
-//     goes to shared memory, warp 0 adds the 8 warps' partials in ascending warp order, applies SwiGLU, and publishes
-//     a[8 rows][8 tokens] (bf16 for bf16 models, G21);
-//   down: warp w owns the outputs j in [w, w+1) * slab/8 of every slab and accumulates over the chunk's rows in registers.
+// Data path per CTA (320 threads), a dataflow of four roles that talk through mbarriers only (no block-wide barrier):
+//   producer warp (one lane): takes unit tickets and streams each unit's parts (8 rows x one slab of at most 32 KiB) through
+//     a shared-memory ring with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx), in the order
+//     gate/up(unit i+1), down(unit i), ... so the down parts of a unit arrive while its SwiGLU is being reduced;
+//   8 consumer warps: gate/up of a sub-block of 8 act rows -- warp w owns the K range [w, w+1) * slab/8 of every slab and
+//     leaves its 16 x 8 partial tile (rows 0-7 gate, 8-15 up; columns = the tokens routed to the expert) in shared memory;
+//     down -- warp w owns the outputs j in [w, w+1) * slab/8 of every slab, accumulates over the chunk's rows in registers
+//     and stores the chunk partial.  Each warp runs at its own pace; a ring slot is free when all 8 warps have read it;
+//   reducer warp: adds the 8 warps' gate/up partials in ascending warp order, applies SwiGLU, publishes
+//     a[8 rows][8 tokens] (bf16 for bf16 models, G21) for the down parts.
+// bf16: the products run on the tensor cores through mma.sync.m16n8k16 (A fragments come straight from the ring with
+// ldmatrix, each core matrix being 128 contiguous bytes), so the arithmetic leaves the FMA pipes and the kernel stays a pure
+// HBM stream at 1..8 tokens (1 flop/byte: this is an ALU offload of a memory-bound kernel, not a GEMM -- units of 96 KiB are
+// far too small for tcgen05's 128-row tiles).  fp32 (config 1, parity only): plain FMA, same data flow, same reduction tree.
 // Fused miss path (WISP_FETCH_FUSED): the parts of an entry marked as a miss are read from the mapped pinned master
 // (Alg. 1 line 6) and consumer warp 0 stores each landed part into the victim slot with a bulk shared->global
 // copy: same bytes, same order of arithmetic as a hit.
@@ -36,10 +39,9 @@ namespace wisp {
 
 constexpr int kDecConsumers = 256;                      // 8 consumer warps
 constexpr int kDecWarps = kDecConsumers / 32;
-constexpr int kDecThreads = kDecConsumers + 32;         // + 1 producer warp
+constexpr int kDecThreads = kDecConsumers + 64;         // + producer warp + reducer warp
 constexpr int kDecMaxSlots = 8;
 constexpr int kDecMaxSteps = 16;                        // MMA steps per warp per part: slab / 128 <= 16
-constexpr int kDecUnitQueue = 8;                        // unit ids in flight between producer and consumers
 constexpr int kDecMaxPartBytes = 32 << 10;
 
 // Geometry, computed on the host once per context and token class (make_decode_geom in wisp.cu).
@@ -65,6 +67,7 @@ struct DecodeFfnArgs {
   const char* master;     // mapped pinned master of this layer (fused miss path) or nullptr
   unsigned long long blob_bytes;
   int L, layer, k;
+  float inv_k;            // 1.0f / k (token of pair p = floor((p + 0.5) / k), exact for p < 256)
   float* partial;         // P [pair position][NC][d] fp32
   unsigned* ticket;       // unit ticket counter of this wave (zero when the wave starts)
 };
@@ -86,17 +89,11 @@ __device__ __forceinline__ void ring_init(const DecRing& r) {   // full: the pro
   mbar_fence_init();
 }
 
-// Part p of a unit (chunk c): which matrix, sub-block and slab.  Order: every gate/up part first (sub-block major, slab
-// minor, gate before up), then the down parts (slab major, sub-block minor) -- so a[] of all sub-blocks exists before the
-// first down part and one set of down accumulators serves one slab at a time.
+// One ring part: matrix (0 gate, 1 up, 2 down), sub-block of 8 act rows inside the unit, slab of d.
 struct DecPart { int mat, sb, slab; };
-__device__ __forceinline__ DecPart dec_part(const DecodeGeom& g, int p) {
-  DecPart r;
-  const int n_gu = 2 * g.n_sb * g.n_slab;
-  if (p < n_gu) { r.sb = p / (2 * g.n_slab); const int rem = p % (2 * g.n_slab); r.slab = rem >> 1; r.mat = rem & 1; }
-  else { const int q = p - n_gu; r.slab = q / g.n_sb; r.sb = q % g.n_sb; r.mat = 2; }
-  return r;
-}
+// What the producer tells the consumers about the part in a ring slot (one int per slot).
+constexpr int kPartEnd = 3;
+__device__ __forceinline__ int part_meta(int kind, int sb, int slab, int c, int q) { return kind | (sb << 2) | (slab << 4) | (c << 8) | (q << 20); }
 // Byte offset inside the blob of piece `piece` of that part.
 __device__ __forceinline__ unsigned long long dec_part_offset(const DecodeGeom& g, int c, const DecPart& p, int piece) {
   const unsigned long long grp = (unsigned long long)(c * g.n_sb + p.sb);
@@ -105,42 +102,93 @@ __device__ __forceinline__ unsigned long long dec_part_offset(const DecodeGeom& 
   return g.down_off + (grp * g.down_pieces + piece) * (g.group_bytes / g.down_pieces) + (unsigned long long)p.slab * pb;
 }
 
+// ---- per-CTA dataflow state (shared memory) -----------------------------------------------------------------------
+struct DecFfnShared {
+  unsigned long long full[kDecMaxSlots], empty[kDecMaxSlots];
+  unsigned long long red_full[2][2];     // [unit parity][sub-block]: the 8 consumer warps' gate/up partials are in place
+  unsigned long long act_ready[2];       // [unit parity]: the reducer has published a[] of every sub-block of the unit
+  int meta[kDecMaxSlots];                // part_meta of the part in each ring slot
+  volatile int units_total;              // units this CTA's producer has queued so far (all waves of the launch)
+  volatile int final;                    // the consumers have finished the last wave of the launch
+  int abort;                             // a grid barrier timed out: everybody leaves
+  alignas(16) float red[2][2][kDecWarps * 128];   // gate/up partial tiles; also the combine's scratch between waves
+  alignas(16) float act[2][2][64];       // a[token column][act row] per (unit parity, sub-block), bf16 or fp32
+};
+
+__device__ __forceinline__ void dec_ffn_shared_init(DecFfnShared& fs, const DecRing& ring) {   // one thread, before a CTA-wide sync
+  ring_init(ring);
+  for (int p = 0; p < 2; ++p) {
+    mbar_init(smem_u32(&fs.act_ready[p]), 1);
+    for (int sb = 0; sb < 2; ++sb) mbar_init(smem_u32(&fs.red_full[p][sb]), kDecWarps);
+  }
+  mbar_fence_init();
+  fs.units_total = 0; fs.final = 0; fs.abort = 0;
+}
+
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile("{\n.reg .pred P1;\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\nselp.u32 %0, 1, 0, P1;\n}"
+               : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  return done != 0;
+}
+// mbarrier wait that gives up when the CTA aborted (a grid barrier timed out)
+__device__ __forceinline__ bool mbar_wait_or_abort(uint32_t bar, uint32_t parity, const int* s_abort) {
+  while (!mbar_try_wait(bar, parity))
+    if (*reinterpret_cast<const volatile int*>(s_abort)) return false;
+  return true;
+}
+
 // ---- producer: one lane takes unit tickets and issues the bulk loads --------------------------------------------
 // Units of the wave whose plan entries are [lo, lo + nw): u in [0, nw * NC), entry = unit_entry[lo + u / NC], chunk = u % NC.
 // The first unit of CTA b is b (no atomic on the critical path of a phase start), later ones come from the ticket counter.
-__device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const DecodeGeom& g, const PlanPtrs& plan, const DecRing& ring,
-                                               DecRingPos& rp, int& useq, int* s_unit, int lo, int nw, uint64_t pol) {
+// Part order in the ring: gate/up parts of unit i+1 (sub-block major, slab minor, gate before up), then the down parts of
+// unit i (slab major, sub-block minor), ..., the down parts of the last unit, an END marker.
+__device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const DecodeGeom& g, const PlanPtrs& plan, DecFfnShared& fs,
+                                               const DecRing& ring, DecRingPos& rp, int lo, int nw, uint64_t pol) {
   const int n_units = nw * g.n_chunks;
-  int u = (int)blockIdx.x;
-  while (true) {
-    if (u >= n_units) {                                        // sentinel: tells the consumers that this wave is over
-      mbar_wait(ring.empty0 + 8u * rp.s, rp.ph ^ 1u);
-      s_unit[useq & (kDecUnitQueue - 1)] = -1;
-      mbar_arrive(ring.full0 + 8u * rp.s);
-      ring_advance(ring, rp);
-      ++useq;
-      return;
-    }
+  auto emit = [&](const char* blob, int q, int c, const DecPart& pt) -> bool {
+    if (!mbar_wait_or_abort(ring.empty0 + 8u * rp.s, rp.ph ^ 1u, &fs.abort)) return false;
+    fs.meta[rp.s] = part_meta(pt.mat, pt.sb, pt.slab, c, q);
+    const uint32_t bar = ring.full0 + 8u * rp.s, dst = ring.slot0 + (uint32_t)rp.s * ring.stride;
+    mbar_expect_tx(bar, (uint32_t)g.part_bytes);
+    const int np = pt.mat == 2 ? g.down_pieces : 1;
+    const uint32_t pb = (uint32_t)g.part_bytes / np;
+    for (int piece = 0; piece < np; ++piece) bulk_g2s(dst + piece * pb, blob + dec_part_offset(g, c, pt, piece), pb, bar, pol);
+    ring_advance(ring, rp);
+    return true;
+  };
+  auto blob_of = [&](int q) {
+    const bool from_host = a.master != nullptr && plan.entry_miss[q] != 0;
+    return from_host ? a.master + (size_t)plan.entry_expert[q] * a.blob_bytes
+                     : a.pool + ((size_t)plan.entry_slot[q] * a.L + a.layer) * a.blob_bytes;
+  };
+  auto emit_down = [&](int q, int c) -> bool {
+    const char* blob = blob_of(q);
+    for (int s = 0; s < g.n_slab; ++s)
+      for (int sb = 0; sb < g.n_sb; ++sb)
+        if (!emit(blob, q, c, DecPart{2, sb, s})) return false;
+    return true;
+  };
+  int u = (int)blockIdx.x, pq = -1, pc = 0, count = 0;
+  while (u < n_units) {
     const unsigned t = atomicAdd(a.ticket, 1u);                // next unit: its latency hides behind this unit's copies
     const int q = plan.unit_entry[lo + u / g.n_chunks], c = u % g.n_chunks;
-    const bool from_host = a.master != nullptr && plan.entry_miss[q] != 0;
-    const char* blob = from_host ? a.master + (size_t)plan.entry_expert[q] * a.blob_bytes
-                                 : a.pool + ((size_t)plan.entry_slot[q] * a.L + a.layer) * a.blob_bytes;
-    for (int p = 0; p < g.parts_unit; ++p) {
-      const DecPart pt = dec_part(g, p);
-      mbar_wait(ring.empty0 + 8u * rp.s, rp.ph ^ 1u);
-      if (p == 0) s_unit[useq & (kDecUnitQueue - 1)] = u;
-      const uint32_t bar = ring.full0 + 8u * rp.s, dst = ring.slot0 + (uint32_t)rp.s * ring.stride;
-      mbar_expect_tx(bar, (uint32_t)g.part_bytes);
-      const int np = pt.mat == 2 ? g.down_pieces : 1;
-      const uint32_t pb = (uint32_t)g.part_bytes / np;
-      for (int piece = 0; piece < np; ++piece)
-        bulk_g2s(dst + piece * pb, blob + dec_part_offset(g, c, pt, piece), pb, bar, pol);
-      ring_advance(ring, rp);
-    }
-    ++useq;
+    const char* blob = blob_of(q);
+    for (int sb = 0; sb < g.n_sb; ++sb)
+      for (int s = 0; s < g.n_slab; ++s) {
+        if (!emit(blob, q, c, DecPart{0, sb, s})) return;
+        if (!emit(blob, q, c, DecPart{1, sb, s})) return;
+      }
+    if (pq >= 0 && !emit_down(pq, pc)) return;
+    pq = q; pc = c; ++count;
     u = (int)gridDim.x + (int)t;
   }
+  if (pq >= 0 && !emit_down(pq, pc)) return;
+  if (!mbar_wait_or_abort(ring.empty0 + 8u * rp.s, rp.ph ^ 1u, &fs.abort)) return;   // END marker: this wave is over
+  fs.meta[rp.s] = kPartEnd;
+  mbar_arrive(ring.full0 + 8u * rp.s);
+  ring_advance(ring, rp);
+  fs.units_total = fs.units_total + count;
 }
 
 // C-fragment position of element (row, col) of a 16 x 8 tile inside a warp's 128-float partial (index lane * 4 + reg).
@@ -149,45 +197,77 @@ __device__ __forceinline__ int cfrag_index(int row, int col) { return ((row & 7)
 template <typename T> struct ActT { typedef float type; };
 template <> struct ActT<__nv_bfloat16> { typedef __nv_bfloat16 type; };
 
-// ---- consumers: the 8 warps (tid 0..255) process the units the producer queued, until the sentinel ---------------
-// xs: the call's hidden states in shared memory, [T][xs_pitch] elements of T (rows padded by 16 bytes).
-// s_red: 8 * 128 floats; s_act: 2 * 64 elements of ActT (a[sub-block][token column][act row]).
+// ---- reducer warp: SwiGLU of every unit the consumers push, until the launch is over ------------------------------
+// a[n][r] = silu(sum_w gate_w[r][n]) * (sum_w up_w[r][n]), the 8 warp partials added in ascending warp order.
 template <typename T>
-__device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const DecodeGeom& g, const PlanPtrs& plan, const DecRing& ring,
-                                               DecRingPos& rp, int& useq, const int* s_unit, int lo, const T* xs, int xs_pitch,
-                                               float* s_red, void* s_act_raw) {
+__device__ __forceinline__ void decode_reduce(const DecodeGeom& g, DecFfnShared& fs, int lane) {
+  typedef typename ActT<T>::type AT;
+  const int col = lane >> 2, kq = (lane & 3) * 2;
+  for (unsigned i = 0;; ++i) {
+    const unsigned par = i & 1u, ph = (i >> 1) & 1u;
+    for (int sb = 0; sb < g.n_sb; ++sb) {
+      const uint32_t bar = smem_u32(&fs.red_full[par][sb]);
+      while (!mbar_try_wait(bar, ph))
+        if (fs.abort || (fs.final && (int)i >= fs.units_total)) return;
+      const float* red = fs.red[par][sb];
+      float4 tot = *reinterpret_cast<const float4*>(red + lane * 4);
+#pragma unroll
+      for (int w = 1; w < kDecWarps; ++w) {
+        const float4 v = *reinterpret_cast<const float4*>(red + w * 128 + lane * 4);
+        tot.x += v.x; tot.y += v.y; tot.z += v.z; tot.w += v.w;
+      }
+      // this lane holds gate (x, y) and up (z, w) of act row lane/4 for the token columns kq, kq+1
+      AT* dst = reinterpret_cast<AT*>(fs.act[par][sb]);
+      if constexpr (sizeof(T) == 2) {
+        dst[kq * 8 + col] = __float2bfloat16_rn(silu_f(tot.x) * tot.z);
+        dst[(kq + 1) * 8 + col] = __float2bfloat16_rn(silu_f(tot.y) * tot.w);
+      } else {
+        dst[kq * 8 + col] = silu_f(tot.x) * tot.z;
+        dst[(kq + 1) * 8 + col] = silu_f(tot.y) * tot.w;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&fs.act_ready[par]));
+  }
+}
+
+// ---- consumers: the 8 warps (tid 0..255) process the parts the producer queued, until the END marker ---------------
+// xs: the call's hidden states in shared memory, [T][xs_pitch] elements of T (rows padded by 16 bytes).
+// gu_seq / d_seq: units whose gate/up / down this warp has finished so far in the launch (select the parity buffers).
+template <typename T>
+__device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const DecodeGeom& g, const PlanPtrs& plan, DecFfnShared& fs,
+                                               const DecRing& ring, DecRingPos& rp, unsigned& gu_seq, unsigned& d_seq, const T* xs,
+                                               int xs_pitch) {
   typedef typename ActT<T>::type AT;
   constexpr bool kMma = sizeof(T) == 2;
-  AT* s_act = reinterpret_cast<AT*>(s_act_raw);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int col = lane >> 2, kq = (lane & 3) * 2;             // MMA fragment coordinates of this lane
   while (true) {
     mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
-    const int u = s_unit[useq & (kDecUnitQueue - 1)];
-    ++useq;
-    if (u < 0) {                                              // sentinel slot: hand it back and stop
+    const int meta = fs.meta[rp.s];
+    const int kind = meta & 3;
+    if (kind == kPartEnd) {                                   // hand the marker's slot back and stop
       __syncwarp();
       if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);
       ring_advance(ring, rp);
       break;
     }
-    const int q = plan.unit_entry[lo + u / g.n_chunks], c = u % g.n_chunks;
+    // The part opens a GROUP of parts of the same unit: kind 0 = the gate/up parts of sub-block sb0 (n_slab pairs), kind 2 =
+    // the down parts of slab s0 (n_sb parts).  The accumulators of a group live only inside it.
+    const int sb0 = (meta >> 2) & 3, s0 = (meta >> 4) & 15, c = (meta >> 8) & 0xfff, q = (meta >> 20) & 0x3ff;
     const int e = plan.entry_expert[q];
     const int cnt = min(plan.exp_count[e], kDecodeMaxTokens);
     const int pos0 = plan.exp_offset[e];
     const int* pl = plan.pair_list + pos0;
     const bool fill = a.master != nullptr && plan.entry_miss[q] != 0;
     char* slot_blob = const_cast<char*>(a.pool) + ((size_t)plan.entry_slot[q] * a.L + a.layer) * a.blob_bytes;
-    int part = 0;
-    // hand a consumed ring slot back (after, on a miss, warp 0 has stored it into the victim slot)
+    // on a miss, warp 0 stores the landed part into the victim slot before the ring slot is handed back
     auto store_part = [&](const DecPart& pt) {
-      if (fill && warp == 0) {
-        if (lane == 0) {
-          const int np = pt.mat == 2 ? g.down_pieces : 1;
-          const uint32_t pb = (uint32_t)g.part_bytes / np, src = ring.slot0 + (uint32_t)rp.s * ring.stride;
-          for (int piece = 0; piece < np; ++piece) bulk_s2g(slot_blob + dec_part_offset(g, c, pt, piece), src + piece * pb, pb);
-          bulk_commit();
-        }
+      if (fill && warp == 0 && lane == 0) {
+        const int np = pt.mat == 2 ? g.down_pieces : 1;
+        const uint32_t pb = (uint32_t)g.part_bytes / np, src = ring.slot0 + (uint32_t)rp.s * ring.stride;
+        for (int piece = 0; piece < np; ++piece) bulk_s2g(slot_blob + dec_part_offset(g, c, pt, piece), src + piece * pb, pb);
+        bulk_commit();
       }
     };
     auto release = [&]() {
@@ -196,148 +276,146 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
       if (lane == 0) mbar_arrive(ring.empty0 + 8u * rp.s);
       ring_advance(ring, rp);
     };
-    const int tok = col < cnt ? pl[col] / a.k : -1;            // token of MMA column `col` (-1: unused column, operand 0)
 
-    // ================= gate/up + SwiGLU, sub-block by sub-block =================
-    for (int sb = 0; sb < g.n_sb; ++sb) {
-      float cacc[4] = {0.f, 0.f, 0.f, 0.f};                    // MMA: this warp's 16 x 8 partial tile (rows 0-7 gate, 8-15 up)
+    if (kind == 0) {
+      // ================= gate/up group of sub-block sb (each gate part is followed by its up part) =================
+      // the warp's 16 x 8 partial tile (rows 0-7 gate, 8-15 up) as FOUR independent accumulator chains (k-step t feeds chain
+      // t % 4), added as (0 + 1) + (2 + 3) when the last slab is done
+      const int sb = sb0;
+      float c4[4][4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { c4[j][0] = 0.f; c4[j][1] = 0.f; c4[j][2] = 0.f; c4[j][3] = 0.f; }
+      const unsigned par = gu_seq & 1u;
+      float* red = fs.red[par][sb] + warp * 128;
       for (int s = 0; s < g.n_slab; ++s) {
-        // ring slots of the gate part and of the up part
-        if (part > 0) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
-        const uint32_t gbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
-        const DecPart ptg = dec_part(g, part);
-        store_part(ptg);
-        DecRingPos rpu = rp;
-        ring_advance(ring, rpu);
-        mbar_wait(ring.full0 + 8u * rpu.s, rpu.ph);
-        const uint32_t ubase = ring.slot0 + (uint32_t)rpu.s * ring.stride;
-        const int k_lo = s * g.slab + warp * (g.slab >> 3);    // this warp's K range of the slab
-        if constexpr (kMma) {
-          const uint32_t abase = ((lane >> 3) & 1 ? ubase : gbase) + (uint32_t)(lane & 7) * 16u + (uint32_t)(lane >> 4) * 128u +
-                                 (uint32_t)(warp * g.steps) * 256u;
-          const T* xrow = xs + (size_t)max(tok, 0) * xs_pitch + k_lo + kq;
-#pragma unroll
-          for (int t = 0; t < kDecMaxSteps; ++t) {
-            if (t < g.steps) {
-              uint32_t a0, a1, a2, a3;
-              ldmatrix_x4(a0, a1, a2, a3, abase + (uint32_t)t * 256u);
-              uint32_t b0 = 0u, b1 = 0u;
-              if (tok >= 0) {
-                b0 = *reinterpret_cast<const uint32_t*>(xrow + t * 16);
-                b1 = *reinterpret_cast<const uint32_t*>(xrow + t * 16 + 8);
-              }
-              mma_bf16_16816(cacc, a0, a1, a2, a3, b0, b1);
-            }
-          }
-        } else {
-          // fp32: lane l owns the 16-byte chunks l, l+32, ... of the warp's K range; one token column at a time
-          const int n_chunk = (g.slab >> 3) / g.kc;
-          for (int n = 0; n < cnt; ++n) {
-            const T* xrow = xs + (size_t)(pl[n] / a.k) * xs_pitch + k_lo;
-            for (int r = 0; r < 16; ++r) {
-              const uint32_t base = (r < 8 ? gbase : ubase) + (uint32_t)(r & 7) * 16u + (uint32_t)(warp * n_chunk) * 128u;
-              float acc = 0.f;
-              for (int ch = lane; ch < n_chunk; ch += 32) {
-                float wv[4];
-                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(wv[0]), "=f"(wv[1]), "=f"(wv[2]), "=f"(wv[3]) : "r"(base + (uint32_t)ch * 128u));
-#pragma unroll
-                for (int j = 0; j < 4; ++j) acc = fmaf(wv[j], to_f32<T>(xrow[ch * 4 + j]), acc);
-              }
-              acc = warp_sum(acc);
-              if (lane == 0) {                                  // accumulates over the slabs of the sub-block
-                float* dst = s_red + warp * 128 + cfrag_index(r, n);
-                *dst = (s == 0 ? 0.f : *dst) + acc;
-              }
-            }
-          }
-        }
-        release();                       // gate part
-        const DecPart ptu = dec_part(g, part + 1);
-        store_part(ptu);
-        release();                       // up part
-        part += 2;
-      }
-      // ---- cross-warp reduction (ascending warp order) + SwiGLU, by warp 0 ----
+      if (s > 0) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
+      const uint32_t gbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
+      store_part(DecPart{0, sb, s});
+      DecRingPos rpu = rp;
+      ring_advance(ring, rpu);
+      mbar_wait(ring.full0 + 8u * rpu.s, rpu.ph);
+      const uint32_t ubase = ring.slot0 + (uint32_t)rpu.s * ring.stride;
+      const int k_lo = s * g.slab + warp * (g.slab >> 3);     // this warp's K range of the slab
       if constexpr (kMma) {
-        *reinterpret_cast<float4*>(s_red + warp * 128 + lane * 4) = make_float4(cacc[0], cacc[1], cacc[2], cacc[3]);
-      }
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      if (warp == 0) {
-        float4 tot = *reinterpret_cast<const float4*>(s_red + lane * 4);
+        const int tok = col < cnt ? (int)(((float)pl[col] + 0.5f) * a.inv_k) : -1;   // token of MMA column `col` (-1: operand 0)
+        const uint32_t abase = ((lane >> 3) & 1 ? ubase : gbase) + (uint32_t)(lane & 7) * 16u + (uint32_t)(lane >> 4) * 128u +
+                               (uint32_t)(warp * g.steps) * 256u;
+        const T* xrow = xs + (size_t)max(tok, 0) * xs_pitch + k_lo + kq;
 #pragma unroll
-        for (int w = 1; w < kDecWarps; ++w) {
-          const float4 v = *reinterpret_cast<const float4*>(s_red + w * 128 + lane * 4);
-          tot.x += v.x; tot.y += v.y; tot.z += v.z; tot.w += v.w;
+        for (int t0 = 0; t0 < kDecMaxSteps; t0 += 4) {
+          if (t0 < g.steps) {
+            uint32_t af[4][4], bf[4][2];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              if (t0 + j < g.steps) {
+                ldmatrix_x4(af[j][0], af[j][1], af[j][2], af[j][3], abase + (uint32_t)(t0 + j) * 256u);
+                bf[j][0] = tok >= 0 ? *reinterpret_cast<const uint32_t*>(xrow + (t0 + j) * 16) : 0u;
+                bf[j][1] = tok >= 0 ? *reinterpret_cast<const uint32_t*>(xrow + (t0 + j) * 16 + 8) : 0u;
+              }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              if (t0 + j < g.steps) mma_bf16_16816(c4[j], af[j][0], af[j][1], af[j][2], af[j][3], bf[j][0], bf[j][1]);
+          }
         }
-        // lane holds gate (x, y) and up (z, w) of act row lane/4 for token columns kq, kq+1
-        AT* dst = s_act + (sb * 8) * 8;
-        if constexpr (kMma) {
-          dst[(kq) * 8 + col] = __float2bfloat16_rn(silu_f(tot.x) * tot.z);
-          dst[(kq + 1) * 8 + col] = __float2bfloat16_rn(silu_f(tot.y) * tot.w);
-        } else {
-          dst[(kq) * 8 + col] = silu_f(tot.x) * tot.z;
-          dst[(kq + 1) * 8 + col] = silu_f(tot.y) * tot.w;
+        if (s == g.n_slab - 1)
+          *reinterpret_cast<float4*>(red + lane * 4) =
+              make_float4((c4[0][0] + c4[1][0]) + (c4[2][0] + c4[3][0]), (c4[0][1] + c4[1][1]) + (c4[2][1] + c4[3][1]),
+                          (c4[0][2] + c4[1][2]) + (c4[2][2] + c4[3][2]), (c4[0][3] + c4[1][3]) + (c4[2][3] + c4[3][3]));
+      } else {
+        // fp32: lane l owns the 16-byte chunks l, l+32, ... of the warp's K range; one token column at a time; the warp's tile
+        // entry accumulates over the slabs in shared memory (warp-private)
+        const int n_chunk = (g.slab >> 3) / g.kc;
+        for (int n = 0; n < cnt; ++n) {
+          const T* xrow = xs + (size_t)(int)(((float)pl[n] + 0.5f) * a.inv_k) * xs_pitch + k_lo;
+          for (int r = 0; r < 16; ++r) {
+            const uint32_t base = (r < 8 ? gbase : ubase) + (uint32_t)(r & 7) * 16u + (uint32_t)(warp * n_chunk) * 128u;
+            float acc = 0.f;
+            for (int ch = lane; ch < n_chunk; ch += 32) {
+              float wv[4];
+              asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(wv[0]), "=f"(wv[1]), "=f"(wv[2]), "=f"(wv[3]) : "r"(base + (uint32_t)ch * 128u));
+#pragma unroll
+              for (int j = 0; j < 4; ++j) acc = fmaf(wv[j], to_f32<T>(xrow[ch * 4 + j]), acc);
+            }
+            acc = warp_sum(acc);
+            if (lane == 0) {
+              float* dst = red + cfrag_index(r, n);
+              *dst = (s == 0 ? 0.f : *dst) + acc;
+            }
+          }
         }
       }
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-    }
-
-    // ================= down: P[pair][c][j] = sum_i a_i * D[j][i], slab by slab =================
-    for (int s = 0; s < g.n_slab; ++s) {
-      float yacc[kMma ? kDecMaxSteps : 1][4];
+      release();                                               // gate part
+      store_part(DecPart{1, sb, s});
+      release();                                               // up part
+      }
+      __syncwarp();                                            // the sub-block's partial tile is complete: tell the reducer
+      if (lane == 0) mbar_arrive(smem_u32(&fs.red_full[par][sb]));
+      if (sb == g.n_sb - 1) ++gu_seq;
+    } else {
+      // ================= down group of slab s: P[pair][c][j] = sum_{i in chunk} a_i * D[j][i] for the outputs j of the slab =================
+      const int s = s0;
+      const unsigned par = d_seq & 1u;
+      if (s == 0) mbar_wait(smem_u32(&fs.act_ready[par]), (d_seq >> 1) & 1u);   // a[] of this unit is published
+      float yacc[kMma ? kDecMaxSteps : 1][4];                  // outputs j of this warp x token columns
       if constexpr (kMma) {
 #pragma unroll
         for (int t = 0; t < kDecMaxSteps; ++t) { yacc[t][0] = 0.f; yacc[t][1] = 0.f; yacc[t][2] = 0.f; yacc[t][3] = 0.f; }
       }
       for (int sb = 0; sb < g.n_sb; ++sb) {
-        mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
-        const uint32_t dbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
-        const DecPart ptd = dec_part(g, part);
-        store_part(ptd);
-        if constexpr (kMma) {
-          // A[j][i]: 16 outputs j x (8 act columns i, upper half of K zero); B[i][n] = a[n][i]
-          const uint32_t b0 = *reinterpret_cast<const uint32_t*>(s_act + (sb * 8 + col) * 8 + kq);
-          const uint32_t abase = dbase + (uint32_t)(lane & 7) * 16u + (uint32_t)((lane >> 3) & 1) * 128u + (uint32_t)(warp * g.steps) * 256u;
+      if (sb > 0) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
+      const uint32_t dbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
+      store_part(DecPart{2, sb, s});
+      const AT* act = reinterpret_cast<const AT*>(fs.act[par][sb]);
+      if constexpr (kMma) {
+        // A[j][i]: 16 outputs j x (8 act columns i, upper half of K zero); B[i][n] = a[n][i]
+        const uint32_t b0 = *reinterpret_cast<const uint32_t*>(act + col * 8 + kq);
+        const uint32_t abase = dbase + (uint32_t)(lane & 7) * 16u + (uint32_t)((lane >> 3) & 1) * 128u + (uint32_t)(warp * g.steps) * 256u;
 #pragma unroll
-          for (int t = 0; t < kDecMaxSteps; ++t) {
-            if (t < g.steps) {
-              uint32_t a0, a1;
-              ldmatrix_x2(a0, a1, abase + (uint32_t)t * 256u);
-              mma_bf16_16816(yacc[t], a0, a1, 0u, 0u, b0, 0u);
-            }
-          }
-        } else {
-          // fp32: thread owns outputs j = tid, tid + 256, ... of the slab; n_sb == 1 for fp32 models, so the sum over the 8 act
-          // columns is complete here: i ascending, fmaf from 0.f
-          const uint32_t half = (uint32_t)g.part_bytes / 2;
-          for (int jj = tid; jj < g.slab; jj += kDecConsumers) {
-            float wv[8];
-            const uint32_t addr = dbase + (uint32_t)(jj >> 3) * 128u + (uint32_t)(jj & 7) * 16u;
-            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(wv[0]), "=f"(wv[1]), "=f"(wv[2]), "=f"(wv[3]) : "r"(addr));
-            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(wv[4]), "=f"(wv[5]), "=f"(wv[6]), "=f"(wv[7]) : "r"(addr + half));
-            for (int n = 0; n < cnt; ++n) {
-              float acc = 0.f;
+        for (int t0 = 0; t0 < kDecMaxSteps; t0 += 4) {        // four output tiles per batch: loads first, then the MMAs
+          if (t0 < g.steps) {
+            uint32_t af[4][2];
 #pragma unroll
-              for (int i = 0; i < 8; ++i) acc = fmaf(wv[i], to_f32<AT>(s_act[(sb * 8 + n) * 8 + i]), acc);
-              a.partial[((size_t)(pos0 + n) * g.n_chunks + c) * g.d + s * g.slab + jj] = acc;
-            }
+            for (int j = 0; j < 4; ++j)
+              if (t0 + j < g.steps) ldmatrix_x2(af[j][0], af[j][1], abase + (uint32_t)(t0 + j) * 256u);
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              if (t0 + j < g.steps) mma_bf16_16816(yacc[t0 + j], af[j][0], af[j][1], 0u, 0u, b0, 0u);
           }
         }
         release();
-        ++part;
-      }
-      if constexpr (kMma) {
-        const int j0 = s * g.slab + warp * (g.slab >> 3) + col;
-        float* p0 = a.partial + ((size_t)(pos0 + kq) * g.n_chunks + c) * g.d + j0;
-        float* p1 = p0 + (size_t)g.n_chunks * g.d;
+        if (sb == g.n_sb - 1) {
+          const int j0 = s * g.slab + warp * (g.slab >> 3) + col;
+          float* p0 = a.partial + ((size_t)(pos0 + kq) * g.n_chunks + c) * g.d + j0;
+          float* p1 = p0 + (size_t)g.n_chunks * g.d;
 #pragma unroll
-        for (int t = 0; t < kDecMaxSteps; ++t) {
-          if (t < g.steps) {
-            if (kq < cnt) { p0[t * 16] = yacc[t][0]; p0[t * 16 + 8] = yacc[t][2]; }
-            if (kq + 1 < cnt) { p1[t * 16] = yacc[t][1]; p1[t * 16 + 8] = yacc[t][3]; }
+          for (int t = 0; t < kDecMaxSteps; ++t) {
+            if (t < g.steps) {
+              if (kq < cnt) { p0[t * 16] = yacc[t][0]; p0[t * 16 + 8] = yacc[t][2]; }
+              if (kq + 1 < cnt) { p1[t * 16] = yacc[t][1]; p1[t * 16 + 8] = yacc[t][3]; }
+            }
           }
         }
+      } else {
+        // fp32: thread owns outputs j = tid, tid + 256, ... of the slab; fp32 models use one sub-block per unit, so the sum over
+        // the 8 act columns is complete here: i ascending, fmaf from 0.f
+        const uint32_t half = (uint32_t)g.part_bytes / 2;
+        for (int jj = tid; jj < g.slab; jj += kDecConsumers) {
+          float wv[8];
+          const uint32_t addr = dbase + (uint32_t)(jj >> 3) * 128u + (uint32_t)(jj & 7) * 16u;
+          asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(wv[0]), "=f"(wv[1]), "=f"(wv[2]), "=f"(wv[3]) : "r"(addr));
+          asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(wv[4]), "=f"(wv[5]), "=f"(wv[6]), "=f"(wv[7]) : "r"(addr + half));
+          for (int n = 0; n < cnt; ++n) {
+            float acc = 0.f;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) acc = fmaf(wv[i], to_f32<AT>(act[n * 8 + i]), acc);
+            a.partial[((size_t)(pos0 + n) * g.n_chunks + c) * g.d + s * g.slab + jj] = acc;
+          }
+        }
+        release();
       }
+      }
+      if (s == g.n_slab - 1) ++d_seq;
     }
   }
   if (a.master != nullptr && tid == 0) bulk_wait0();     // this CTA's slot fills are complete before the next grid-wide barrier

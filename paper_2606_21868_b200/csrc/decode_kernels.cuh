@@ -105,25 +105,10 @@ __device__ __forceinline__ bool grid_barrier(unsigned* ctr, unsigned& gen, volat
   return *reinterpret_cast<volatile int*>(s_abort) == 0;
 }
 
-// mbarrier wait of the producer lane that gives up when the consumers aborted
-__device__ __forceinline__ bool mbar_wait_or_abort(uint32_t bar, uint32_t parity, const int* s_abort) {
-  while (true) {
-    uint32_t done;
-    asm volatile(
-        "{\n.reg .pred P1;\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\nselp.u32 %0, 1, 0, P1;\n}"
-        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-    if (done) return true;
-    if (*reinterpret_cast<const volatile int*>(s_abort)) return false;
-  }
-}
-
-// Shared state of one decode CTA (static shared memory of the fused and of the split ffn kernel).
+// Shared state of one decode CTA besides the FFN dataflow (static shared memory of the fused kernel).
 struct DecShared {
-  unsigned long long full[kDecMaxSlots], empty[kDecMaxSlots], go;
-  int unit[kDecUnitQueue];
-  int abort;
-  alignas(16) float red[kDecWarps * 128];                 // gate/up warp partials | the combine's 8 x 8 x 16 group sums
-  alignas(16) float act[2 * 64];                          // a[sub-block][token column][act row] (bf16 or fp32)
+  unsigned long long go;                                  // the plan of the next wave exists: the producer may stream
+  unsigned long long wpre;                                // the next layer's router-weight slice has landed in shared memory
   alignas(16) float y[kMaxTopK * kSliceCols];
   float xn[kSliceCols];
   int ids[kDecodeMaxTokens * kMaxTopK];
@@ -133,28 +118,32 @@ struct DecShared {
 
 template <typename T>
 __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const DecodeArgs a, const DecodeGeom g, int n_slots, int xs_pitch,
-                                                                      int xs_bytes) {
+                                                                      int pre_off, int ring_off) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(16) DecShared ds;
+  __shared__ __align__(16) DecFfnShared fs;
   __shared__ PlanShared<kPersistMaxExperts> sh;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   DecRing ring;
-  ring.slot0 = smem_u32(smem_raw) + (uint32_t)xs_bytes; ring.full0 = smem_u32(ds.full); ring.empty0 = smem_u32(ds.empty);
+  ring.slot0 = smem_u32(smem_raw) + (uint32_t)ring_off; ring.full0 = smem_u32(fs.full); ring.empty0 = smem_u32(fs.empty);
   ring.n_slots = n_slots; ring.stride = g.part_bytes;
   if (tid == 0) {
     mbar_init(smem_u32(&ds.go), 1);
-    ring_init(ring);
-    ds.abort = 0;
+    mbar_init(smem_u32(&ds.wpre), 1);
+    dec_ffn_shared_init(fs, ring);
   }
   __syncthreads();
   DecRingPos rp{0, 0u};
-  int useq = 0;
   const int E = a.E, k = a.k, d = a.d, T_ = a.T, C = a.C;
   const PlanPtrs pp = plan_ptrs_of(ds.pl);
   DecodeFfnArgs fa{};
-  fa.pool = a.pool; fa.blob_bytes = a.blob_bytes; fa.L = a.L; fa.k = k; fa.partial = a.partial;
+  fa.pool = a.pool; fa.blob_bytes = a.blob_bytes; fa.L = a.L; fa.k = k; fa.inv_k = 1.0f / (float)k; fa.partial = a.partial;
 
+  if (warp == kDecWarps + 1) {                           // ===================== reducer warp =====================
+    decode_reduce<T>(g, fs, lane);
+    return;
+  }
   if (warp == kDecWarps) {
     // ===================== producer warp (one lane): streams every wave's units as soon as its plan exists ==========
     if (lane != 0) return;
@@ -165,11 +154,12 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
       fa.master = a.masters[l];
       int n_waves = 1;
       for (int w = 0; w < n_waves; ++w, ++qseq) {
-        if (!mbar_wait_or_abort(smem_u32(&ds.go), qseq & 1u, &ds.abort)) return;
+        if (!mbar_wait_or_abort(smem_u32(&ds.go), qseq & 1u, &fs.abort)) return;
         n_waves = ds.pl.hdr[0];
         const int nR = ds.pl.hdr[1], lo = w * C, nw = min(nR, lo + C) - lo;
         fa.ticket = a.sync + 1 + (qseq & 1u);
-        decode_produce(fa, g, pp, ring, rp, useq, ds.unit, lo, nw, pol);
+        decode_produce(fa, g, pp, fs, ring, rp, lo, nw, pol);
+        if (fs.abort) return;
       }
     }
     return;
@@ -182,7 +172,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
   auto stamp = [&](int phase) {
     if (timing) { const u64 t = globaltimer_ns(); a.phase_ns[phase] += t - t_prev; t_prev = t; }
   };
-  unsigned gen = 0, qseq = 0;
+  unsigned gen = 0, qseq = 0, gu_seq = 0, d_seq = 0, n_pre = 0;
   T* xs = reinterpret_cast<T*>(smem_raw);               // current hidden state, [T][xs_pitch], in EVERY CTA
   auto load_xs = [&](const void* src_) {
     const int vec_row = d * (int)sizeof(T) / 16;
@@ -202,11 +192,11 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
       const int t = sl / (d / kSliceCols), j0 = (sl % (d / kSliceCols)) * kSliceCols;
       if (tid < kSliceCols) ds.xn[tid] = to_f32<T>(xs[(size_t)t * xs_pitch + j0 + tid]);
       asm volatile("bar.sync 1, 256;" ::: "memory");
-      slice_logits<T>(wrt, ds.xn, j0, E, a.zfix + ((size_t)(a.layer_lo & 1) * kDecodeMaxTokens + t) * E, tid, kDecConsumers);
+      slice_logits<T>(wrt + (size_t)j0 * E, ds.xn, E, a.zfix + ((size_t)(a.layer_lo & 1) * kDecodeMaxTokens + t) * E, tid, kDecConsumers);
       asm volatile("bar.sync 1, 256;" ::: "memory");
     }
   }
-  if (!grid_barrier(a.sync, gen, a.err, &ds.abort)) return;
+  if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;
 
   for (int l = a.layer_lo; l < a.layer_hi; ++l) {
     const LayerState st = layer_state_of(a, l);
@@ -247,9 +237,18 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     }
     const int n_waves = ds.pl.hdr[0];
     const int miss_cls = ds.pl.hdr[2] > 0 ? 1 : 0;             // layers with misses are timed apart
+    // this CTA's first combine slice is known now: its 16 rows of the NEXT layer's router weights (one contiguous block of
+    // [d][E]) are staged in shared memory by a bulk copy while the FFN streams
+    const bool pre = !last && (int)blockIdx.x < n_slices;
     if (tid == 0) {
       if (writer) a.sync[1 + ((qseq + 1) & 1u)] = 0u;          // ticket counter of the NEXT wave (idle since the wave before this one)
       mbar_arrive(smem_u32(&ds.go));                           // the producer may start streaming
+      if (pre) {
+        const uint32_t bytes = (uint32_t)(kSliceCols * E * sizeof(T));
+        const T* src = reinterpret_cast<const T*>(a.router_wt) + ((size_t)(l + 1) * d + (size_t)((int)blockIdx.x % (d / kSliceCols)) * kSliceCols) * E;
+        mbar_expect_tx(smem_u32(&ds.wpre), bytes);
+        bulk_g2s_nohint(smem_u32(smem_raw) + (uint32_t)pre_off, src, bytes, smem_u32(&ds.wpre));
+      }
     }
     stamp(1);
     if (!last) plan_load<kPersistMaxExperts>(sh, layer_state_of(a, l + 1), E, C);   // stable until that layer's own plan
@@ -261,17 +260,17 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     fa.master = a.masters[l];
     for (int w = 0; w < n_waves; ++w, ++qseq) {
       if (w > 0) {
-        if (!grid_barrier(a.sync, gen, a.err, &ds.abort)) return;   // the previous wave's slots may now be refilled
+        if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;   // the previous wave's slots may now be refilled
         if (tid == 0) {
           if (writer) a.sync[1 + ((qseq + 1) & 1u)] = 0u;
           mbar_arrive(smem_u32(&ds.go));
         }
       }
       fa.ticket = a.sync + 1 + (qseq & 1u);
-      decode_consume<T>(fa, g, pp, ring, rp, useq, ds.unit, w * C, xs, xs_pitch, ds.red, ds.act);
+      decode_consume<T>(fa, g, pp, fs, ring, rp, gu_seq, d_seq, xs, xs_pitch);
     }
     if (n_waves == 0) ++qseq;                                  // (cannot happen: n_tokens >= 1) keeps the producer in step
-    if (!grid_barrier(a.sync, gen, a.err, &ds.abort)) return;  // C: every chunk partial of this layer is in place
+    if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;  // C: every chunk partial of this layer is in place
     stamp(3 + miss_cls);
 
     // ---- combine (+ residual) and the next layer's logits, 16-column slices over the grid ----
@@ -284,17 +283,26 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
       long long* zf_n = a.zfix + (size_t)((l + 1) & 1) * kDecodeMaxTokens * E;
       for (int sl = blockIdx.x; sl < n_slices; sl += gridDim.x) {
         const int t = sl / (d / kSliceCols), j0 = (sl % (d / kSliceCols)) * kSliceCols;
-        combine_slice<T>(ca, t, j0, a.residual ? xs + (size_t)t * xs_pitch : nullptr, xg + (size_t)t * d, ds.red, ds.y, ds.xn, 1);
-        if (!last) slice_logits<T>(wrt, ds.xn, j0, E, zf_n + (size_t)t * E, tid, kDecConsumers);
+        combine_slice<T>(ca, t, j0, a.residual ? xs + (size_t)t * xs_pitch : nullptr, xg + (size_t)t * d, fs.red[0][0], ds.y, ds.xn, 1);
+        if (!last) {
+          const T* w16 = wrt + (size_t)j0 * E;
+          if (sl == (int)blockIdx.x) {                         // the staged slice
+            mbar_wait(smem_u32(&ds.wpre), n_pre & 1u);
+            ++n_pre;
+            w16 = reinterpret_cast<const T*>(smem_raw + pre_off);
+          }
+          slice_logits<T>(w16, ds.xn, E, zf_n + (size_t)t * E, tid, kDecConsumers);
+        }
       }
       if (!last) {
-        if (!grid_barrier(a.sync, gen, a.err, &ds.abort)) return;   // E: x_{l+1} and its logits are complete
+        if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;   // E: x_{l+1} and its logits are complete
         load_xs(xg);
         asm volatile("bar.sync 1, 256;" ::: "memory");
       }
     }
     stamp(5);
   }
+  if (tid == 0) fs.final = 1;                                   // lets the reducer warp leave
 }
 
 // ===================== split form: the same steps as separate launches =====================
@@ -309,7 +317,7 @@ __global__ void __launch_bounds__(256) decode_logits_kernel(const T* __restrict_
     const int t = sl / (d / kSliceCols), j0 = (sl % (d / kSliceCols)) * kSliceCols;
     if (threadIdx.x < kSliceCols) s_xn[threadIdx.x] = to_f32<T>(x[(size_t)t * d + j0 + threadIdx.x]);
     __syncthreads();
-    slice_logits<T>(wrt, s_xn, j0, E, zfix + (size_t)t * E, threadIdx.x, 256);
+    slice_logits<T>(wrt + (size_t)j0 * E, s_xn, E, zfix + (size_t)t * E, threadIdx.x, 256);
     __syncthreads();
   }
 }
@@ -352,23 +360,24 @@ __global__ void __launch_bounds__(NT) decode_plan_kernel(PlanArgs a, long long* 
 template <typename T>
 __global__ void __launch_bounds__(kDecThreads, 1) decode_ffn_kernel(DecodeFfnArgs fa, const DecodeGeom g, PlanPtrs gp, int wave, int C, int E,
                                                                     int n_tokens, const T* __restrict__ x, int n_slots, int xs_pitch,
-                                                                    int xs_bytes) {
+                                                                    int ring_off) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  __shared__ __align__(16) DecShared ds;
+  __shared__ __align__(16) DecFfnShared fs;
+  __shared__ DecPlan spl;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (wave >= gp.hdr[0]) return;
   DecRing ring;
-  ring.slot0 = smem_u32(smem_raw) + (uint32_t)xs_bytes; ring.full0 = smem_u32(ds.full); ring.empty0 = smem_u32(ds.empty);
+  ring.slot0 = smem_u32(smem_raw) + (uint32_t)ring_off; ring.full0 = smem_u32(fs.full); ring.empty0 = smem_u32(fs.empty);
   ring.n_slots = n_slots; ring.stride = g.part_bytes;
-  if (tid == 0) ring_init(ring);
-  // the plan -> shared memory (the consumers index it per unit)
+  if (tid == 0) dec_ffn_shared_init(fs, ring);
+  // the plan -> shared memory (the consumers index it per part)
   const int nR = gp.hdr[1], n_pairs = gp.hdr[3];
   for (int i = tid; i < nR; i += kDecThreads) {
-    ds.pl.entry_expert[i] = gp.entry_expert[i]; ds.pl.entry_slot[i] = gp.entry_slot[i]; ds.pl.entry_miss[i] = gp.entry_miss[i];
-    ds.pl.unit_entry[i] = gp.unit_entry[i];
+    spl.entry_expert[i] = gp.entry_expert[i]; spl.entry_slot[i] = gp.entry_slot[i]; spl.entry_miss[i] = gp.entry_miss[i];
+    spl.unit_entry[i] = gp.unit_entry[i];
   }
-  for (int i = tid; i < n_pairs; i += kDecThreads) ds.pl.pair_list[i] = gp.pair_list[i];
-  PlanPtrs pp = plan_ptrs_of(ds.pl);
+  for (int i = tid; i < n_pairs; i += kDecThreads) spl.pair_list[i] = gp.pair_list[i];
+  PlanPtrs pp = plan_ptrs_of(spl);
   pp.exp_count = gp.exp_count; pp.exp_offset = gp.exp_offset;     // indexed by expert id (E may exceed the shared capacity)
   T* xs = reinterpret_cast<T*>(smem_raw);
   {
@@ -378,12 +387,17 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_ffn_kernel(DecodeFfnArg
   }
   __syncthreads();
   DecRingPos rp{0, 0u};
-  int useq = 0;
+  fa.inv_k = 1.0f / (float)fa.k;
   const int lo = wave * C, nw = min(nR, lo + C) - lo;
-  if (warp == kDecWarps) {
-    if (lane == 0) decode_produce(fa, g, pp, ring, rp, useq, ds.unit, lo, nw, l2_evict_first_policy());
+  if (warp == kDecWarps + 1) {
+    decode_reduce<T>(g, fs, lane);
+  } else if (warp == kDecWarps) {
+    if (lane == 0) decode_produce(fa, g, pp, fs, ring, rp, lo, nw, l2_evict_first_policy());
   } else {
-    decode_consume<T>(fa, g, pp, ring, rp, useq, ds.unit, lo, xs, xs_pitch, ds.red, ds.act);
+    unsigned gu_seq = 0, d_seq = 0;
+    decode_consume<T>(fa, g, pp, fs, ring, rp, gu_seq, d_seq, xs, xs_pitch);
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (tid == 0) fs.final = 1;
   }
 }
 

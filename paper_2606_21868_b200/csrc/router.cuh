@@ -63,46 +63,43 @@ __global__ void __launch_bounds__(256) router_logits_kernel(const T* __restrict_
 }
 
 // Top-k + softmax of ONE token's logits by ONE warp ("warp-shuffle softmax and top-k", BASELINE.json north_star; G7).
-// Lane l owns the logits of experts l, l+32, ... as 64-bit keys (order-preserving image of z << 32 | ~id), so the warp
-// arg-max of a key is the largest logit with ties going to the LOWER id; k rounds give ids in (z desc, id asc) order.
-// -0 compares equal to +0 and a NaN ranks with -inf (it can never corrupt an id: every selected id is a real expert).
+// Lane l owns the logits of experts l, l+32, ... as order-preserving 32-bit keys.  One round = the warp maximum of the keys
+// (redux.sync.max), then the LOWEST expert id among the lanes that hold that maximum (redux.sync.min): the largest logit
+// with ties going to the lower id; k rounds give ids in (z desc, id asc) order.  -0 compares equal to +0 and a NaN ranks
+// with -inf (it can never corrupt an id: every selected id is a real expert).
 // w_i = exp(z_i - z_0) / sum_j exp(z_j - z_0), the sum taken in rank order j = 0..k-1 (every lane computes the same chain).
 // EPL = logits per lane (E <= 32 * EPL); zf(e) returns the logit of expert e.  ids_out / w_out: [k].
-__device__ __forceinline__ unsigned long long topk_key(float z, int e) {
+__device__ __forceinline__ unsigned topk_key(float z) {
   z += 0.0f;                                            // -0 -> +0
   unsigned u = __float_as_uint(z);
   if (z != z) u = 0xff800000u;                          // NaN -> -inf
-  u = (u & 0x80000000u) ? ~u : (u | 0x80000000u);       // unsigned order == float order
-  return ((unsigned long long)u << 32) | (unsigned)(0xffffffffu - (unsigned)e);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);    // unsigned order == float order; every key is > 0
 }
-__device__ __forceinline__ float topk_key_logit(unsigned long long key) {
-  unsigned u = (unsigned)(key >> 32);
+__device__ __forceinline__ float topk_key_logit(unsigned u) {
   u = (u & 0x80000000u) ? (u & 0x7fffffffu) : ~u;
   return __uint_as_float(u);
 }
 template <int EPL, typename ZF>
 __device__ __forceinline__ void topk_softmax_warp(ZF zf, int E, int k, int* ids_out, float* w_out, int lane) {
-  unsigned long long key[EPL];
+  unsigned key[EPL];
 #pragma unroll
   for (int j = 0; j < EPL; ++j) {
     const int e = lane + 32 * j;
-    key[j] = e < E ? topk_key(zf(e), e) : 0ull;          // 0 = absent / already taken (every live key is > 0)
+    key[j] = e < E ? topk_key(zf(e)) : 0u;               // 0 = absent / already taken
   }
   float my_z = 0.f;                                     // lane r keeps the logit of rank r
   for (int r = 0; r < k; ++r) {
-    unsigned long long best = 0ull;
+    unsigned best = 0u;
+    int best_j = 0;
 #pragma unroll
-    for (int j = 0; j < EPL; ++j) best = key[j] > best ? key[j] : best;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
-      best = other > best ? other : best;
-    }
-    const int e = (int)(0xffffffffu - (unsigned)(best & 0xffffffffu));
+    for (int j = EPL - 1; j >= 0; --j)                   // descending j with >= : among equal keys the lowest id of the lane wins
+      if (key[j] >= best) { best = key[j]; best_j = j; }
+    const unsigned top = __reduce_max_sync(0xffffffffu, best);
+    const unsigned e = __reduce_min_sync(0xffffffffu, best == top ? (unsigned)(lane + 32 * best_j) : 0xffffffffu);
 #pragma unroll
     for (int j = 0; j < EPL; ++j)
-      if (e == lane + 32 * j) key[j] = 0ull;
-    if (lane == r) { my_z = topk_key_logit(best); ids_out[r] = e; }
+      if ((int)e == lane + 32 * j) key[j] = 0u;
+    if (lane == r) { my_z = topk_key_logit(top); ids_out[r] = (int)e; }
   }
   const float z0 = __shfl_sync(0xffffffffu, my_z, 0);
   float den = 0.f;

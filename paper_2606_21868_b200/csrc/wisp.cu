@@ -315,16 +315,19 @@ DecodeGeom make_decode_geom(int d, int dff, size_t elem, int rows_unit) {
   return g;
 }
 
-struct DecodeSmem { int n_slots, xs_pitch, xs_bytes; size_t bytes; };
-// Shared-memory carve-up of a decode CTA: [hidden states, rows padded by 16 B][ring of n_slots parts].
-int decode_smem(wisp_ctx* ctx, const DecodeGeom& g, int T_, size_t avail, DecodeSmem* out) {
+struct DecodeSmem { int n_slots, xs_pitch, pre_off, ring_off; size_t bytes; };
+// Shared-memory carve-up of a decode CTA: [hidden states, rows padded by 16 B][staged router-weight slice (fused kernel)]
+// [ring of n_slots parts].
+int decode_smem(wisp_ctx* ctx, const DecodeGeom& g, int T_, size_t avail, bool fused, DecodeSmem* out) {
   out->xs_pitch = g.d + g.kc;
-  out->xs_bytes = (int)(((size_t)T_ * out->xs_pitch * g.elem + 127) & ~(size_t)127);
-  if ((size_t)out->xs_bytes + 2 * (size_t)g.part_bytes > avail) return fail(ctx, WISP_EINVAL, "decode kernel: shared memory too small for this shape");
-  int n = (int)std::min<size_t>(kDecMaxSlots, (avail - out->xs_bytes) / g.part_bytes);
+  out->pre_off = (int)(((size_t)T_ * out->xs_pitch * g.elem + 127) & ~(size_t)127);
+  const size_t pre = fused ? (((size_t)kSliceCols * ctx->cfg.n_experts * g.elem + 127) & ~(size_t)127) : 0;
+  out->ring_off = out->pre_off + (int)pre;
+  if ((size_t)out->ring_off + 2 * (size_t)g.part_bytes > avail) return fail(ctx, WISP_EINVAL, "decode kernel: shared memory too small for this shape");
+  int n = (int)std::min<size_t>(kDecMaxSlots, (avail - out->ring_off) / g.part_bytes);
   if (ctx->cfg.ring_stages > 0) n = std::min(n, std::max(2, (int)ctx->cfg.ring_stages));
   out->n_slots = n;
-  out->bytes = (size_t)out->xs_bytes + (size_t)n * g.part_bytes;
+  out->bytes = (size_t)out->ring_off + (size_t)n * g.part_bytes;
   return WISP_OK;
 }
 
@@ -357,10 +360,10 @@ int launch_fused(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out
   pa.phase_ns = ctx->timing_level >= 2 ? ctx->phase_ns : nullptr;
   DecodeGeom g = ctx->dgeom[T_ <= 2 ? 0 : 1];
   DecodeSmem sm;
-  int rc = decode_smem(ctx, g, T_, ctx->fused_smem, &sm);
+  int rc = decode_smem(ctx, g, T_, ctx->fused_smem, true, &sm);
   if (rc) return rc;
   CK(cudaMemsetAsync(ctx->dsync, 0, 4 * sizeof(unsigned), st));
-  void* args[] = {&pa, &g, &sm.n_slots, &sm.xs_pitch, &sm.xs_bytes};
+  void* args[] = {&pa, &g, &sm.n_slots, &sm.xs_pitch, &sm.pre_off, &sm.ring_off};
   CK(cudaLaunchCooperativeKernel((const void*)decode_fused_kernel<T>, dim3(ctx->num_sms), dim3(kDecThreads), args, sm.bytes, st));
   ++ctx->launches;
   for (int l = lo; l < hi; ++l) ctx->last_T[l] = T_;
@@ -410,7 +413,7 @@ int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* 
   }
   const DecodeGeom g = ctx->dgeom[T_ <= 2 ? 0 : 1];
   DecodeSmem sm;
-  int rc = decode_smem(ctx, g, T_, ctx->ffn_smem, &sm);
+  int rc = decode_smem(ctx, g, T_, ctx->ffn_smem, false, &sm);
   if (rc) return rc;
   DecodeFfnArgs fa{};
   fa.pool = ctx->arena; fa.blob_bytes = ctx->Me; fa.L = L; fa.layer = layer; fa.k = k; fa.partial = ctx->partial;
@@ -424,7 +427,7 @@ int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* 
     CK(cudaMemsetAsync(ctx->dsync + 1, 0, sizeof(unsigned), st));
     Span sp(ctx, WISP_K_FFN, st);
     decode_ffn_kernel<T><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, w, ctx->C, E, T_, reinterpret_cast<const T*>(x),
-                                                                     sm.n_slots, sm.xs_pitch, sm.xs_bytes);
+                                                                     sm.n_slots, sm.xs_pitch, sm.ring_off);
   }
   {
     CombineArgs ca;
