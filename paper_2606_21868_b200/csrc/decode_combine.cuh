@@ -19,14 +19,15 @@ namespace wisp {
 
 constexpr int kSliceCols = 16;
 constexpr float kLogitFixScale = 1099511627776.f;        // 2^40
-constexpr double kLogitFixInv = 1.0 / 1099511627776.0;
+constexpr float kLogitFixInv = 1.0f / 1099511627776.f;    // 2^-40 (exact)
 
 __device__ __forceinline__ long long logit_to_fix(float v) {
   const float s = v * kLogitFixScale;
   if (!(fabsf(s) < 4.0e18f)) return s > 0.f ? (1ll << 62) : -(1ll << 62);   // non-finite input (G23): saturate, stay defined
   return __float2ll_rn(s);
 }
-__device__ __forceinline__ float logit_from_fix(long long f, float bias) { return (float)((double)f * kLogitFixInv) + bias; }
+// one rounding (int64 -> fp32), an exact scaling, one fp32 add; no fp64 on the routing chain
+__device__ __forceinline__ float logit_from_fix(long long f, float bias) { return __ll2float_rn(f) * kLogitFixInv + bias; }
 
 // Partial logits of one 16-column slice of token t's hidden state (xn[16], fp32 images of the model-dtype values) for all
 // experts, added into zfix[t][e].  w16: rows j0 .. j0+15 of this layer's router weights TRANSPOSED ([d][E], model dtype), in

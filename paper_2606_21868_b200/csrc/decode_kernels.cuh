@@ -207,9 +207,13 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     if (warp < T_) {
       const float* bias = a.router_bias + (size_t)l * E;
       const long long* zt = zf_l + (size_t)warp * E;
-      auto zf = [&](int e) { return logit_from_fix(__ldcg(zt + e), bias[e]); };
+      float* zout = writer ? a.logits + (size_t)warp * E : nullptr;     // test surface: wisp_last_logits
+      auto zf = [&](int e) {
+        const float z = logit_from_fix(__ldcg(zt + e), bias[e]);
+        if (zout) zout[e] = z;
+        return z;
+      };
       topk_softmax_warp<kPersistMaxExperts / 32>(zf, E, k, ds.ids + warp * k, ds.w + warp * k, lane);
-      if (writer) for (int e = lane; e < E; e += 32) a.logits[(size_t)warp * E + e] = zf(e);
     }
     asm volatile("bar.sync 1, 256;" ::: "memory");
     stamp(0);

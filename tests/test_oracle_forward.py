@@ -136,3 +136,36 @@ def test_stack_residual_chain_and_paging_independence():
     x1 = (per[0]["x"].float() + per[0]["out"].to(shape.torch_dtype).float()).to(shape.torch_dtype)
     assert torch.equal(per[1]["x"], x1)
     assert torch.equal(per[0]["x"], h.to(shape.torch_dtype))
+
+
+def test_p1b_router_logits_hand_case_nonzero_rows_and_bias():
+    """Pins the W_r.x term of O1 (orientation, bias add) on hand arithmetic (tests/golden/hand_router_ffn.txt P1b)."""
+    x = torch.tensor([[1.0, 2.0]], dtype=F64)
+    w_r = torch.tensor([[1.0, -0.5], [0.5, 1.0], [-1.0, 1.0], [2.0, -1.5]], dtype=F64)
+    bias = torch.tensor([1.0, 0.5, 1.0, 1.0])
+    z = mf.router_logits(x, w_r, bias)
+    assert z[0].tolist() == [G["p1b_z0"], G["p1b_z1"], G["p1b_z2"], G["p1b_z3"]]
+    ids, w = mf.topk_softmax(z, 2)
+    assert ids.tolist() == [[G["p1_id0"], G["p1_id1"]]]
+    assert w[0].tolist() == pytest.approx([G["p1_w0"], G["p1_w1"]], abs=1e-9)
+    # square W_r: a transposed product passes the shape check but not the numbers
+    z2 = mf.router_logits(x, torch.tensor([[1.0, 2.0], [3.0, 4.0]], dtype=F64), torch.tensor([0.5, -0.5]))
+    assert z2[0].tolist() == [G["p1b_sq_z0"], G["p1b_sq_z1"]]
+    # two tokens: rows of x map to rows of z
+    z3 = mf.router_logits(torch.tensor([[1.0, 2.0], [2.0, 4.0]], dtype=F64), w_r, bias)
+    assert z3[1].tolist() == [1.0, 5.5, 3.0, -1.0]            # 2 * (W_r x) + bias, by hand
+
+
+def test_p1c_bf16_inputs_are_widened_exactly_before_the_product():
+    """O1: 'fp64 from the stored values'.  With the product rounded to bf16 the winner flips (golden P1c)."""
+    x = torch.tensor([[1.0 + 2.0 ** -7]], dtype=torch.bfloat16)
+    w_r = torch.tensor([[1.0 + 2.0 ** -7], [1.0]], dtype=torch.bfloat16)
+    bias = torch.tensor([0.0, 0.00785], dtype=torch.float32)
+    assert x.double().item() == 1.0078125 and w_r.double()[0, 0].item() == 1.0078125   # both are bf16 values
+    z = mf.router_logits(x, w_r, bias)
+    assert z[0, 0].item() == G["p1c_z0"]                        # exact: (1 + 2^-7)^2
+    ids, _ = mf.topk_softmax(z, 1)
+    assert ids.tolist() == [[G["p1c_top1"]]]
+    # the mistake this pins: rounding the product to bf16 first gives 1.015625 < z1
+    wrong = (x * w_r[0]).double().item()
+    assert wrong == 1.015625 and wrong + 0.0 < z[0, 1].item() < z[0, 0].item()

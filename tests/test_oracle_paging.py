@@ -211,3 +211,65 @@ def test_resize_shrink_grow_cycle():
 def test_empty_step_is_noop():
     p = PagerLayer(C=2, E=4)
     assert p.step([]) == [] and p.c == 0 and p.steps == 0
+
+
+def _parse_resize(spec):
+    """'drop:2@1 move:3@1<2' -> [(expert, slot, evicted_or_source, kind)]"""
+    out = []
+    for tok in spec.split():
+        kind, rest = tok.split(":")
+        e, rest = rest.split("@")
+        if kind == "drop":
+            out.append((int(e), int(rest), -1, RESIZE_DROP))
+        else:
+            dst, src = rest.split("<")
+            out.append((int(e), int(dst), int(src), RESIZE_MOVE))
+    return out
+
+
+def _lfu_state(steps):
+    p = PagerLayer(C=3, E=8, policy=LFU)
+    for R in steps:
+        p.step(R)
+    return p
+
+
+def test_lfu_resize_hand_trace():
+    """O4 resize rule under LFU, keep order (f desc, tau desc, slot asc): hand-stepped (golden [lfu_resize])."""
+    import copy
+    g = read_golden("hand_paging_trace.txt")["lfu_resize"]
+    ints = lambda v: [int(t) for t in v.split()]
+    base = _lfu_state([[1, 2, 3], [3], [3], [1]])
+    assert base.slots() == ints(g["state_slots"]) and base.tau == ints(g["state_tau"])
+    assert (base.f[1], base.f[2], base.f[3]) == (2, 1, 3)
+    p = copy.deepcopy(base)
+    ev = [(e.expert, e.slot, e.evicted, e.kind) for e in p.resize(2)]
+    assert ev == _parse_resize(g["shrink2_events"]) and p.slots() == ints(g["shrink2_slots"]) and p.tau == ints(g["shrink2_tau"])
+    p.check_invariants()
+    p = copy.deepcopy(base)
+    ev = [(e.expert, e.slot, e.evicted, e.kind) for e in p.resize(1)]
+    assert ev == _parse_resize(g["shrink1_lfu_events"]) and p.slots() == ints(g["shrink1_lfu_slots"]) and p.tau == ints(g["shrink1_lfu_tau"])
+    # the same state under LRU keeps a different survivor (the most recent, not the most frequent)
+    q = copy.deepcopy(base)
+    q.policy = LRU
+    ev = [(e.expert, e.slot, e.evicted, e.kind) for e in q.resize(1)]
+    assert ev == _parse_resize(g["shrink1_lru_events"]) and q.slots() == ints(g["shrink1_lru_slots"])
+    # f ties fall back to tau descending
+    t = _lfu_state([[1, 2], [1], [1], [3]])
+    assert t.tau == ints(g["tie_state_tau"])
+    ev = [(e.expert, e.slot, e.evicted, e.kind) for e in t.resize(2)]
+    assert ev == _parse_resize(g["tie_shrink2_events"]) and t.slots() == ints(g["tie_shrink2_slots"]) and t.tau == ints(g["tie_shrink2_tau"])
+    t.check_invariants()
+
+
+def test_decay_and_miss_curve_two_period_hand_case():
+    """PAPER.md:152 'decayed' histograms: bins of period 1 times lambda, plus period 2 (golden [decay])."""
+    from oracle import mvwsa
+    g = read_golden("hand_paging_trace.txt")["decay"]
+    d_all = mvwsa.stack_distances(list("abab" "bc"))          # the LRU stack carries over between the periods
+    h1 = mvwsa.histogram(d_all[:3], 2)
+    h = mvwsa.decay(h1, 0.5)
+    h2 = mvwsa.histogram(d_all[3:], 2)
+    tot = [a + b for a, b in zip(h, h2)]
+    assert tot[1:] == [float(v) for v in g["bins_after"].split()]
+    assert mvwsa.miss_curve_from_hist(tot, 2) == [float(g["m0"]), float(g["m1"]), float(g["m2"])]
