@@ -48,8 +48,10 @@ def parse():
     ap.add_argument("--policy", default="lru", choices=["lru", "lfu"])
     ap.add_argument("--wave-order", default="ascending", choices=["ascending", "hits-first"],
                     help="overflow wave order (wisp_set_wave_order, DESIGN.md G25); only matters when |R| > C")
-    ap.add_argument("--fetch", default="fused", choices=["fused", "zerocopy", "memcpy"],
-                    help="miss path: fused = persistent decode kernel whose TMA producer reads misses from the mapped master")
+    ap.add_argument("--fetch", default="fused", choices=["fused", "zerocopy", "memcpy", "static"],
+                    help="miss path: fused = persistent decode kernel whose TMA producer reads misses from the mapped master; "
+                         "static = the static layer-offload comparison arm (PAPER.md:21, 207): no residency cache, every layer call "
+                         "streams its experts from the host master again")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-miss-path", action="store_true")
     ap.add_argument("--no-prefill", action="store_true")
@@ -58,6 +60,11 @@ def parse():
                     help="extra, clearly labelled locality stress (never the headline): router bias x 0.25 and AR(1) coefficient 0.5 "
                          "(same stationary variance) -> adjacent-step carry-over near the paper's 0.44-0.48 (PAPER.md:187)")
     ap.add_argument("--per-layer-api", action="store_true", help="drive wisp_moe_forward per layer instead of wisp_stack_forward")
+    ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed arm, each from an empty pool (median and best are reported)")
+    ap.add_argument("--unit-rows", type=int, default=0, help="act rows per decode FFN work unit (0 = library default)")
+    ap.add_argument("--no-micro", action="store_true", help="skip the m1 (FFN-only replay) and m3 (router/top-k/plan) microbenchmarks")
+    ap.add_argument("--verify", default="", help="full-depth parity run instead of a bench line: comma list of 2,3,4 (BASELINE.json configs)")
+    ap.add_argument("--verify-steps", type=int, default=256)
     return ap.parse_args()
 
 
@@ -147,13 +154,13 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(kernel):
-    """dram read+write bytes per launch of `kernel` from the committed ncu capture, or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+def profile_traffic(kernel):
+    """dram read+write bytes per launch of `kernel` from the committed ncu capture (profiles/r02_traffic.json), with the
+    capture it came from: NOT measured in this run (ncu is not available inside a bench run)."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
     if os.path.exists(p):
         with open(p) as fh:
-            v = json.load(fh).get(kernel)
-            return v.get("traffic") if isinstance(v, dict) else v
+            return json.load(fh).get(kernel)
     return None
 
 
@@ -163,8 +170,9 @@ def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=N
     ctx = wp.Wisp(budget, n_layers=shape.n_layers, n_experts=shape.n_experts, top_k=shape.top_k, d_model=shape.d_model,
                   d_ff=shape.d_ff, max_tokens=max_tokens, dtype=wp.WISP_F32 if shape.dtype == "f32" else wp.WISP_BF16,
                   policy=wp.WISP_LFU if args.policy == "lfu" else wp.WISP_LRU,
-                  fetch={"memcpy": wp.WISP_FETCH_MEMCPY, "zerocopy": wp.WISP_FETCH_ZEROCOPY, "fused": wp.WISP_FETCH_FUSED}[fetch or args.fetch],
-                  ring_stages=getattr(args, "ring_stages", 0))
+                  fetch={"memcpy": wp.WISP_FETCH_MEMCPY, "zerocopy": wp.WISP_FETCH_ZEROCOPY, "fused": wp.WISP_FETCH_FUSED,
+                         "static": wp.WISP_FETCH_FUSED}[fetch or args.fetch],
+                  ring_stages=getattr(args, "ring_stages", 0), unit_rows=getattr(args, "unit_rows", 0))
     if getattr(args, "wave_order", "ascending") == "hits-first":
         ctx.set_wave_order(wp.WISP_WAVES_HITS_FIRST)
     staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
@@ -314,67 +322,6 @@ def prefill_bench(shape, args, n_layers=8, T=2048):
     return out
 
 
-class KvSched:
-    """Harness-level KV-reservation scheduler of BASELINE.json config 5 (G12/G14/G15): FCFS admission on
-    block reservations, a request holds ceil((P+g)/16) blocks, the most recently admitted request is preempted when a
-    block is needed and none is free (it re-prefills P+g tokens).  Reservations go through wisp_kv_reserve."""
-
-    def __init__(self, ctx, prompts, target):
-        self.ctx, self.target = ctx, target
-        self.waiting = [dict(rid=i, prompt=p, gen=0, blocks=0, t_first=None) for i, p in enumerate(prompts)]
-        self.running, self.done = [], []
-        self.preemptions = self.reprefill = 0
-
-    def kappa(self):
-        return self.ctx.stats().kv_blocks
-
-    def used(self):
-        return sum(r["blocks"] for r in self.running)
-
-    def admit(self):
-        out = []
-        while self.waiting:
-            r = self.waiting[0]
-            n = -(-(r["prompt"] + r["gen"]) // 16)
-            if self.used() + n > self.kappa():
-                break
-            self.waiting.pop(0)
-            self.ctx.kv_reserve(n)
-            r["blocks"] = n
-            self.running.append(r)
-            out.append(r)
-        return out
-
-    def grow_for_decode(self):
-        i = 0
-        while i < len(self.running):
-            r = self.running[i]
-            n = -(-(r["prompt"] + r["gen"] + 1) // 16)
-            evicted_self = False
-            while n > r["blocks"] and self.used() + (n - r["blocks"]) > self.kappa() and len(self.running) > 1:
-                v = self.running.pop()
-                self.ctx.kv_reserve(-v["blocks"])
-                v["blocks"] = 0
-                self.preemptions += 1
-                self.reprefill += v["prompt"] + v["gen"]
-                self.waiting.insert(0, v)
-                if v is r:
-                    evicted_self = True
-                    break
-            if evicted_self:
-                continue
-            if n > r["blocks"]:
-                self.ctx.kv_reserve(n - r["blocks"])
-                r["blocks"] = n
-            i += 1
-
-    def finish(self):
-        for r in [x for x in self.running if x["gen"] >= self.target]:
-            self.ctx.kv_reserve(-r["blocks"])
-            self.running.remove(r)
-            self.done.append(r)
-
-
 def mvwsa_arm(shape, args, arm, prompts, n_decode, ctx, streams):
     """One arm of config 5 on an existing context: arm = "live" or a fixed expert fraction.  Returns the arm's report."""
     B = 12 * GIB
@@ -382,65 +329,68 @@ def mvwsa_arm(shape, args, arm, prompts, n_decode, ctx, streams):
     floor_blocks = -(-(16384 + n_decode) // 16)
     frac = 0.5 if arm == "live" else float(arm)
     C0 = max(1, int(B * frac) // a)
-    ctx.set_split(a, (B - a) // b * b)                                # shrink to one slot first: every arm starts (almost) cold
     ctx.set_split(C0 * a, (B - C0 * a) // b * b)
+    ctx.debug_reset_pool()                                            # every arm starts from an empty pool
     ctx.mvwsa_track(arm == "live")
-    sched = KvSched(ctx, prompts, n_decode)
+    from paper_2606_21868_b200.kv_sched import KvRequest, KvReservationScheduler
+    # the ONE harness scheduler (tests/test_kv_sched.py checks it against the oracle's model and a hand-stepped case);
+    # kappa is cached and refreshed only after a successful wisp_set_split; p of Eq. 6 is the scheduler's window peak
+    sched = KvReservationScheduler(ctx.stats().kv_blocks, [KvRequest(i, p, n_decode) for i, p in enumerate(prompts)], reserve=ctx.kv_reserve)
     stream = torch.cuda.Stream()
     T = 2048
     xin = torch.empty((T, shape.d_model), dtype=shape.torch_dtype, device="cuda")
     xout = torch.empty_like(xin)
-    splits = [(0, C0, ctx.stats().kv_blocks)]
+    splits = [(0, C0, sched.kappa)]
     st0 = ctx.stats()
     t_prefill = t_decode = 0.0
     decode_iters = 0
     t_start = time.perf_counter()
+    sched.reset_window()
     with torch.cuda.stream(stream):
         while sched.waiting or sched.running:
-            for r in sched.admit():                                   # prefill (or re-prefill) in chunks of 2048 tokens
-                n_tok = r["prompt"] + r["gen"]
+            for r, n_tok in sched.admit():                            # prefill (or re-prefill) in chunks of 2048 tokens
                 t0 = time.perf_counter()
                 for c0 in range(0, n_tok, T):
                     n = min(T, n_tok - c0)
-                    ctx.stack_forward(streams["prefill"][r["rid"]][:n], xout[:n], stream.cuda_stream)
+                    ctx.stack_forward(streams["prefill"][r.rid][:n], xout[:n], stream.cuda_stream)
                 stream.synchronize()
                 t_prefill += time.perf_counter() - t0
-                if r["t_first"] is None:
-                    r["t_first"] = time.perf_counter() - t_start
+                if r.t_first is None:
+                    r.t_first = time.perf_counter() - t_start
             if not sched.running:
                 if sched.waiting:
                     raise RuntimeError("KV pool too small for the head request (admission floor violated)")
                 break
-            sched.grow_for_decode()
-            nb = len(sched.running)
+            running = sched.grow_for_decode()
+            nb = len(running)
             t0 = time.perf_counter()
-            for i, r in enumerate(sched.running):
-                xin[i].copy_(streams["decode"][r["rid"]][r["gen"]], non_blocking=True)
+            for i, r in enumerate(running):
+                xin[i].copy_(streams["decode"][r.rid][r.gen], non_blocking=True)
             ctx.stack_forward(xin[:nb], xout[:nb], stream.cuda_stream)
             stream.synchronize()
             t_decode += time.perf_counter() - t0
-            for r in sched.running:
-                r["gen"] += 1
-            sched.finish()
+            sched.finish_tick()
             decode_iters += 1
             if arm == "live" and decode_iters % 64 == 0:              # G16: Eq. 6-8 every 64 decode steps, between forwards
-                eb, kb, moved = ctx.mvwsa_propose(mode=0, c_min=shape.top_k, c_max=0, dead_zone=1, headroom=0.2)
+                eb, kb, moved = ctx.mvwsa_propose(mode=0, c_min=shape.top_k, c_max=0, dead_zone=1, headroom=0.2,
+                                                  kv_peak_blocks=sched.window_peak)
                 ctx.mvwsa_miss_curve(shape.n_experts + 1, decay=0.5)
                 if moved:
                     try:
                         ctx.set_split(eb, kb)
+                        sched.set_kappa(kb // b)
                         splits.append((decode_iters, eb // a, kb // b))
                     except Exception:
                         pass                                          # refused resize: the previous split stays
-                ctx.stats()                                           # resets the KV peak window
+                sched.reset_window()
     wall = time.perf_counter() - t_start
     st1 = ctx.stats()
     refs = st1.total.references - st0.total.references
     miss = st1.total.misses - st0.total.misses
-    ttft = sorted(r["t_first"] for r in sched.done)
+    ttft = sorted(r.t_first for r in sched.done)
     return {"arm": arm, "e2e_s": round(wall, 2), "ttft_median_s": round(ttft[len(ttft) // 2], 2), "prefill_s": round(t_prefill, 2),
             "decode_s": round(t_decode, 2), "decode_tokens_per_s": round(len(prompts) * n_decode / max(t_decode, 1e-9), 1),
-            "preemptions": sched.preemptions, "reprefilled_tokens": sched.reprefill, "splits_step_C_kappa": splits,
+            "preemptions": sched.preemptions, "reprefilled_tokens": sched.reprefill_tokens, "splits_step_C_kappa": splits,
             "hit_rate": round(1 - miss / max(1, refs), 4), "miss_gib": round(miss * shape.expert_bytes / GIB, 1),
             "kv_floor_blocks": floor_blocks}
 
@@ -546,9 +496,135 @@ def main_reference(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{shape.name} decode batch {args.batch}, all experts resident (oracle has no pool)",
                        "sample": sample},
-            "cpu_baseline": {"value": val, "unit": "tokens/s", "cores": torch.get_num_threads(), "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "tokens/s", "cores": os.cpu_count(), "torch_threads": torch.get_num_threads(),
+                             "kind": "oracle (oracle/moe_forward.py: PyTorch CPU ops in fp64, as it stands)", "sample": sample},
             "e2e": {"value": val, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
+
+
+def ffn_microbench(shape, args, batches=(1, 4), n_steps=24):
+    """m1: the decode FFN kernel alone (decode_ffn_kernel: the same device code the fused kernel runs between its barriers).
+    One layer, every expert resident; the routing of `n_steps` AR(1) decode steps is recorded with the full path, then
+    replayed: wisp_debug_step_routing rebuilds the plan (untimed), the L2 is flushed (untimed), and ONE
+    wisp_debug_ffn_launch is timed with CUDA events.  Algorithmic bytes = |R| * M_e."""
+    import paper_2606_21868_b200 as wp
+    hbm_peak, _ = measured_peaks()
+    one = shape.with_layers(1)
+    out = {}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for B in batches:
+        ctx = wp.Wisp(one.n_experts * one.slot_unit_bytes, n_layers=1, n_experts=one.n_experts, top_k=one.top_k, d_model=one.d_model,
+                      d_ff=one.d_ff, max_tokens=B, dtype=wp.WISP_BF16 if one.dtype == "bf16" else wp.WISP_F32, fetch=wp.WISP_FETCH_ZEROCOPY,
+                      unit_rows=getattr(args, "unit_rows", 0))
+        blob = si.gen_layer_experts(one, 0, "cuda")
+        w_r, bias = si.gen_router(one, 0)
+        ctx.register_host_experts(0, blob, w_r, bias)
+        del blob
+        x = si.gen_decode_hidden(one, n_steps, B).to(one.torch_dtype).cuda()
+        y = torch.empty_like(x[0])
+        st = torch.cuda.current_stream().cuda_stream
+        routed = []
+        for t in range(n_steps):
+            ctx.moe_forward(0, x[t], y, st)
+            routed.append([int(v) for v in ctx.last_topk(0)[0].flatten()])
+        tot_ms, tot_bytes, best = 0.0, 0, 0.0
+        for rep in range(2):
+            for t in range(n_steps):
+                ctx.debug_step_routing(0, routed[t])
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); ctx.debug_ffn_launch(0, x[t], st); e1.record(); torch.cuda.synchronize()
+                if rep == 0:
+                    continue                                   # first pass: warm-up (instruction cache, first touches)
+                nbytes = len(set(routed[t])) * one.expert_bytes
+                ms = e0.elapsed_time(e1)
+                tot_ms += ms; tot_bytes += nbytes
+                best = max(best, nbytes / (ms * 1e-3) / 1e9)
+        gbs = tot_bytes / (tot_ms * 1e-3) / 1e9
+        out[f"batch{B}"] = {"avg_us": round(tot_ms / n_steps * 1e3, 2), "avg_experts": round(tot_bytes / one.expert_bytes / n_steps, 2),
+                            "gbs": round(gbs, 1), "frac_of_hbm_peak": round(gbs / hbm_peak, 4), "best_gbs": round(best, 1)}
+        ctx.close()
+    out["how"] = ("decode_ffn_kernel alone, one launch per CUDA-event pair (launch latency included), L2 flushed by a 256 MiB write before "
+                  "every launch, routing recorded from the full path and replayed")
+    return out
+
+
+def route_microbench(shape, args):
+    """m3: router + top-k + residency lookup alone, microseconds per layer call at T = 1, 4 (decode kernels of the split form:
+    logits slices, then one plan CTA = top-k + Algorithm 1) and T = 2048 (prefill: tcgen05 router GEMM, warp top-k, plan +
+    pair grouping), CUDA events around each launch, every expert resident."""
+    import paper_2606_21868_b200 as wp
+    one = shape.with_layers(1)
+    T_max = 2048
+    ctx = wp.Wisp(one.n_experts * one.slot_unit_bytes, n_layers=1, n_experts=one.n_experts, top_k=one.top_k, d_model=one.d_model,
+                  d_ff=one.d_ff, max_tokens=T_max, dtype=wp.WISP_BF16 if one.dtype == "bf16" else wp.WISP_F32, fetch=wp.WISP_FETCH_ZEROCOPY)
+    blob = si.gen_layer_experts(one, 0, "cuda")
+    w_r, bias = si.gen_router(one, 0)
+    ctx.register_host_experts(0, blob, w_r, bias)
+    del blob
+    st = torch.cuda.current_stream().cuda_stream
+    out = {}
+    for T in (1, 4, T_max):
+        x = (si.gen_prefill_hidden(one, T) if T > 8 else si.gen_decode_hidden(one, 1, T)[0]).to(one.torch_dtype).cuda()
+        y = torch.empty_like(x)
+        for _ in range(3):
+            ctx.moe_forward(0, x, y, st)
+        torch.cuda.synchronize()
+        ctx.timing_enable(2); ctx.timing_read(reset=True)
+        reps = 10
+        for _ in range(reps):
+            ctx.moe_forward(0, x, y, st)
+        torch.cuda.synchronize()
+        kt = ctx.timing_read(); ctx.timing_enable(0)
+        row = {k: round(kt[k][0] / reps * 1e3, 2) for k in ("router", "topk", "residency") if kt[k][1]}
+        row["sum_us"] = round(sum(row.values()), 2)
+        out[f"T{T}"] = row
+    ctx.close()
+    out["how"] = ("CUDA events around each launch of the split form (one layer, all experts resident): router = logits, topk = prefill top-k "
+                  "kernel (decode: inside the plan launch), residency = plan (+ pair grouping at T = 2048)")
+    return out
+
+
+POOL_WARM_STEPS = 16          # SURVEY.md 8(d) protocol: "warm" = the steps after the first 16 from an empty pool
+
+
+def decode_arm(ctx, shape, x_dev, y_dev, stream, args, n_warm, scratch, host_io=None):
+    """ONE repetition of the timed arm, from an EMPTY pool (wisp_debug_reset_pool): the first n_warm steps (cold segment), then
+    exactly args.steps timed steps (warm segment), each segment bracketed by CUDA events on the launching stream.
+    host_io = (h_in pinned [K, B, d], h_out pinned, xin, xout): the warm segment goes through host buffers (e2e).
+    Returns dict(cold_ms, warm_ms, misses_cold, misses_warm, refs_warm, launches)."""
+    K = args.steps
+    ctx.debug_reset_pool()
+    st0 = ctx.stats()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ev[0].record(stream)
+    run_steps(ctx, shape, x_dev[:n_warm], y_dev[:n_warm], stream, args.per_layer_api, scratch)
+    ev[1].record(stream)
+    stream.synchronize()
+    st1 = ctx.stats()
+    torch.cuda.synchronize()
+    ev[2].record(stream)
+    if host_io is None:
+        run_steps(ctx, shape, x_dev[n_warm:n_warm + K], y_dev[n_warm:n_warm + K], stream, args.per_layer_api, scratch)
+    else:
+        h_in, h_out, xin, xout = host_io
+        for t in range(K):
+            xin.copy_(h_in[t], non_blocking=True)
+            run_steps(ctx, shape, xin[None], xout[None], stream, args.per_layer_api, scratch)
+            h_out[t].copy_(xout, non_blocking=True)
+            stream.synchronize()                       # the caller consumes each token's result before the next step
+    ev[3].record(stream)
+    torch.cuda.synchronize()
+    st2 = ctx.stats()
+    return {"cold_ms": ev[0].elapsed_time(ev[1]), "warm_ms": ev[2].elapsed_time(ev[3]),
+            "misses_cold": int(st1.total.misses - st0.total.misses), "misses_warm": int(st2.total.misses - st1.total.misses),
+            "refs_warm": int(st2.total.references - st1.total.references),
+            "launches": int(st2.kernel_launches - st1.kernel_launches)}
+
+
+def median(xs):
+    s = sorted(xs)
+    return s[len(s) // 2] if len(s) % 2 else 0.5 * (s[len(s) // 2 - 1] + s[len(s) // 2])
 
 
 def main_ours(args):
@@ -575,13 +651,14 @@ def main_ours(args):
         budget = budget // shape.n_layers * nl
         shape = shape.with_layers(nl)
         reduced = True
-    B = args.batch
+    B, K = args.batch, args.steps
+    n_warm = max(args.warmup, POOL_WARM_STEPS)
     t_setup = time.time()
     ctx, staging = build_context(shape, budget, args, max(B, 1))
     del staging
     t_setup = time.time() - t_setup
     C = ctx.stats().slots_per_layer
-    n_all = args.warmup + args.steps
+    n_all = n_warm + K
     if args.stress:
         hidden = si.gen_decode_hidden(shape, n_all, B, rho=0.5, noise=math.sqrt(0.01 / 0.19 * 0.75)).to(shape.torch_dtype)
     else:
@@ -596,128 +673,135 @@ def main_ours(args):
             dist.barrier()
 
     with torch.cuda.stream(stream):
-        run_steps(ctx, shape, x_dev[:args.warmup], y_dev[:args.warmup], stream, args.per_layer_api, scratch)
-        stream.synchronize()
-        st0 = ctx.stats()
+        # untimed: one full pass so that instruction caches, the pinned master's first touches and the CUDA context are warm
+        decode_arm(ctx, shape, x_dev, y_dev, stream, args, n_warm, scratch)
         sampler = ClockSampler(local)
         barrier(); torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        run_steps(ctx, shape, x_dev[args.warmup:], y_dev[args.warmup:], stream, args.per_layer_api, scratch)
-        e1.record(stream)
+        reps, ref_bytes, reps_identical = [], None, True
+        for r in range(max(1, args.reps)):
+            res = decode_arm(ctx, shape, x_dev, y_dev, stream, args, n_warm, scratch)
+            reps.append(res)
+            out_bytes = y_dev.view(torch.uint8).cpu()
+            if ref_bytes is None:
+                ref_bytes = out_bytes
+            elif not torch.equal(ref_bytes, out_bytes) or (res["misses_cold"], res["misses_warm"]) != (reps[0]["misses_cold"], reps[0]["misses_warm"]):
+                reps_identical = False
         torch.cuda.synchronize(); barrier()
         clocks = sampler.stop()
-        ms = e0.elapsed_time(e1)
-        st1 = ctx.stats()
-        ms = max_over_ranks(ms, dist, "cuda")
-        value = replica_throughput(args.steps * B, world, ms)
+        warm_ms = max_over_ranks(median([r["warm_ms"] for r in reps]), dist, "cuda")
+        best_ms = max_over_ranks(min(r["warm_ms"] for r in reps), dist, "cuda")
+        cold_ms = max_over_ranks(median([r["cold_ms"] + r["warm_ms"] for r in reps]), dist, "cuda")
+        value = replica_throughput(K * B, world, warm_ms)
+        r0 = reps[0]
 
-        # ---- e2e: host buffers, H2D + D2H inside the timed region, through the public call ----
-        h_in = hidden[args.warmup:].contiguous().pin_memory()
+        # ---- e2e: the same arm, from the same pool state, with the timed steps going through HOST buffers ----
+        h_in = hidden[n_warm:].contiguous().pin_memory()
         h_out = torch.empty_like(h_in).pin_memory()
         xin = torch.empty((B, shape.d_model), dtype=shape.torch_dtype, device="cuda")
         xout = torch.empty_like(xin)
         barrier(); torch.cuda.synchronize()
-        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e2.record(stream)
-        for t in range(args.steps):
-            xin.copy_(h_in[t], non_blocking=True)
-            run_steps(ctx, shape, xin[None], xout[None], stream, args.per_layer_api, scratch)
-            h_out[t].copy_(xout, non_blocking=True)
-            stream.synchronize()                       # the caller consumes each token's result before the next step
-        e3.record(stream)
-        torch.cuda.synchronize(); barrier()
-        ms_e2e = e2.elapsed_time(e3)
-        ms_e2e = max_over_ranks(ms_e2e, dist, "cuda")
+        e2e_reps = [decode_arm(ctx, shape, x_dev, y_dev, stream, args, n_warm, scratch, host_io=(h_in, h_out, xin, xout))
+                    for _ in range(max(1, min(3, args.reps)))]
+        ms_e2e = max_over_ranks(median([r["warm_ms"] for r in e2e_reps]), dist, "cuda")
         io_bytes = B * shape.d_model * shape.elem_bytes
-        same = torch.equal(h_out.view(torch.uint8), y_dev[args.warmup:].cpu().view(torch.uint8))
+        same = torch.equal(h_out.view(torch.uint8), ref_bytes[n_warm:])
 
-        # ---- per-kernel durations over the same steps (CUDA events on the launching stream; no graph) ----
-        n_prof = min(args.steps, 32)
+        # ---- phase durations over the same arm (fused path: %globaltimer stamps of CTA 0; split form: CUDA events per launch) ----
+        ctx.debug_reset_pool()
+        run_steps(ctx, shape, x_dev[:n_warm], y_dev[:n_warm], stream, args.per_layer_api, scratch)
+        stream.synchronize()
         ctx.timing_enable(2)
         ctx.timing_read(reset=True)
-        run_steps(ctx, shape, x_dev[args.warmup:args.warmup + n_prof], y_dev[args.warmup:args.warmup + n_prof], stream,
-                  args.per_layer_api, scratch)
+        run_steps(ctx, shape, x_dev[n_warm:], y_dev[n_warm:], stream, args.per_layer_api, scratch)
         stream.synchronize()
         kt = ctx.timing_read()
         ctx.timing_enable(0)
-
     hbm_peak, peak_how = measured_peaks()
-    refs = st1.total.references - st0.total.references
-    misses = st1.total.misses - st0.total.misses
-    # algorithmic bytes of one gate_up launch = experts of the wave x (gate + up) bytes
-    avg_R = refs / max(1, args.steps * shape.n_layers)
-    gu_bytes = avg_R * 2 * shape.d_model * shape.d_ff * shape.elem_bytes
-    dn_bytes = avg_R * shape.d_model * shape.d_ff * shape.elem_bytes
+    refs, misses = r0["refs_warm"], r0["misses_warm"]
+    avg_R = refs / max(1, K * shape.n_layers)                    # routed experts per layer call
+    ffn_bytes = avg_R * shape.expert_bytes                       # algorithmic bytes of one layer's FFN
     kern = {}
     for name, (tot_ms, n) in kt.items():
         if n:
             kern[name] = {"avg_us": round(tot_ms / n * 1e3, 3), "launches": int(n)}
-    step_us = sum(v["avg_us"] * v["launches"] for v in kern.values()) / max(1, n_prof)
-    for name in kern:
-        kern[name]["share_of_kernel_time"] = round(kern[name]["avg_us"] * kern[name]["launches"] / max(1e-9, step_us * n_prof), 4)
     roof = None
-    fused = args.fetch == "fused"
-    if "gate_up" in kern:
-        # FFN phases (fused path: %globaltimer stamps of CTA 0 inside the persistent kernel, layer calls WITHOUT a miss only,
-        # each phase including the grid barrier that ends it; other paths: CUDA events around each launch)
-        ach = gu_bytes / (kern["gate_up"]["avg_us"] * 1e-6) / 1e9
-        ffn = {"gate_up": {"achieved": round(ach, 1), "frac": round(ach / hbm_peak, 4), "bytes": int(gu_bytes), "avg_us": kern["gate_up"]["avg_us"]}}
-        if "down" in kern:
-            ach_d = dn_bytes / (kern["down"]["avg_us"] * 1e-6) / 1e9
-            ffn["down"] = {"achieved": round(ach_d, 1), "frac": round(ach_d / hbm_peak, 4), "bytes": int(dn_bytes), "avg_us": kern["down"]["avg_us"]}
-        ffn_us = kern["gate_up"]["avg_us"] + kern.get("down", {"avg_us": 0})["avg_us"]
-        ffn_gbs = (gu_bytes + dn_bytes) / (ffn_us * 1e-6) / 1e9
-        ffn["ffn_gbs"] = round(ffn_gbs, 1)
-        ffn["ffn_frac"] = round(ffn_gbs / hbm_peak, 4)
+    fused = args.fetch in ("fused", "static") and B <= 8 and shape.n_experts <= 256 and not args.per_layer_api
+    if "ffn" in kern:
+        # FFN phase (fused kernel: %globaltimer stamps of CTA 0 over layer calls WITHOUT a miss, from the release of the
+        # producer to the grid barrier that ends the phase, barrier included; split form: CUDA events around each launch)
+        ach = ffn_bytes / (kern["ffn"]["avg_us"] * 1e-6) / 1e9
+        ffn = {"ffn": {"achieved": round(ach, 1), "frac": round(ach / hbm_peak, 4), "bytes": int(ffn_bytes), "avg_us": kern["ffn"]["avg_us"]},
+               "ffn_gbs": round(ach, 1), "ffn_frac": round(ach / hbm_peak, 4)}
+        layer_us = sum(kern[k]["avg_us"] for k in ("router", "residency", "other", "ffn", "combine") if k in kern)
+        ffn["hit_layer_us"] = round(layer_us, 2)
+        ffn["hit_layer_frac_of_hbm_time"] = round((ffn_bytes + shape.n_experts * shape.d_model * shape.elem_bytes) / (hbm_peak * 1e9) * 1e6 / layer_us, 4)
+        launch_bytes = avg_R * shape.n_layers * shape.expert_bytes + shape.n_layers * shape.n_experts * shape.d_model * shape.elem_bytes
         if fused:
-            # dominant kernel = the persistent decode kernel, ONE launch per step: algorithmic bytes of the launch
-            # (expert bytes of the routed experts + router weights) / the launch duration measured
-            # over the timed region (back-to-back launches on the timed stream)
-            launch_bytes = avg_R * shape.n_layers * shape.expert_bytes + shape.n_layers * shape.n_experts * shape.d_model * shape.elem_bytes
-            launch_us = ms / args.steps * 1e3
+            # dominant kernel = the fused decode kernel, ONE launch per step: algorithmic bytes of the launch (expert bytes of the
+            # routed experts + router weights) / the launch duration measured over the timed region (back-to-back launches)
+            launch_us = warm_ms / K * 1e3
             ach_l = launch_bytes / (launch_us * 1e-6) / 1e9
-            link_s = misses * shape.expert_bytes / args.steps / 55.5e9
-            roof = {"bound": "hbm", "kernel": "decode_persistent_kernel", "achieved": round(ach_l, 1), "peak": hbm_peak, "unit": "GB/s",
-                    "frac": round(ach_l / hbm_peak, 4), "traffic": ncu_traffic("decode_persistent_kernel"),
+            roof = {"bound": "hbm", "kernel": "decode_fused_kernel", "achieved": round(ach_l, 1), "peak": hbm_peak, "unit": "GB/s",
+                    "frac": round(ach_l / hbm_peak, 4), "traffic": None, "traffic_from_profile": profile_traffic("decode_fused_kernel"),
                     "bytes_per_launch": int(launch_bytes), "avg_launch_us": round(launch_us, 2), "peak_source": peak_how,
-                    "frac_of_nominal_8TBs": round(ach_l / 8000.0, 4),
-                    "step_lower_bound_us": round(max(launch_bytes / (hbm_peak * 1e9), link_s) * 1e6, 1),
-                    "host_link_us_per_step": round(link_s * 1e6, 1), "ffn_phases_hit_only": ffn}
+                    "frac_of_nominal_8TBs": round(ach_l / 8000.0, 4), "ffn_phases_hit_only": ffn}
         else:
-            roof = {"bound": "hbm", "kernel": "ffn_stream_kernel<gate_up>", "achieved": round(ach, 1), "peak": hbm_peak, "unit": "GB/s",
-                    "frac": round(ach / hbm_peak, 4), "traffic": ncu_traffic("ffn_stream_kernel"),
-                    "bytes_per_launch": int(gu_bytes), "avg_launch_us": kern["gate_up"]["avg_us"], "peak_source": peak_how,
+            roof = {"bound": "hbm", "kernel": "decode_ffn_kernel", "achieved": round(ach, 1), "peak": hbm_peak, "unit": "GB/s",
+                    "frac": round(ach / hbm_peak, 4), "traffic": None, "traffic_from_profile": profile_traffic("decode_ffn_kernel"),
+                    "bytes_per_launch": int(ffn_bytes), "avg_launch_us": kern["ffn"]["avg_us"], "peak_source": peak_how,
                     "frac_of_nominal_8TBs": round(ach / 8000.0, 4), "ffn_phases": ffn}
 
-    line = {"metric": "decode_tokens_per_s", "value": value, "unit": "tokens/s", "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+    line = {"metric": "decode_tokens_per_s", "value": value, "unit": "tokens/s", "n_gpus": world, "steps": K,
+            "warmup": args.warmup, "ms_per_step": warm_ms / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16" if shape.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": f"{shape.name} decode, batch {B}, {shape.n_layers} layers, E={shape.n_experts}, top-{shape.top_k}, "
                                    f"d={shape.d_model}, d_ff={shape.d_ff}, expert pool {budget / GIB:.3f} GiB -> C={C} slots/layer, "
                                    f"{args.policy.upper()}, fetch={args.fetch}" + (", waves=hits-first" if args.wave_order == "hits-first" else ""),
-                       "api": "wisp_moe_forward per layer" if args.per_layer_api else ("wisp_stack_forward (one persistent cooperative kernel per token)" if args.fetch == "fused" else "wisp_stack_forward (CUDA graph per token)"),
+                       "api": "wisp_moe_forward per layer" if args.per_layer_api else ("wisp_stack_forward (one fused cooperative kernel per token)" if fused else "wisp_stack_forward (CUDA graph per token)"),
+                       "protocol": f"every repetition starts from an EMPTY pool (wisp_debug_reset_pool): {n_warm} untimed steps "
+                                   f"({'--warmup' if args.warmup >= POOL_WARM_STEPS else f'--warmup {args.warmup} raised to the {POOL_WARM_STEPS} pool warm-up steps of SURVEY.md 8(d)'}), "
+                                   f"then exactly {K} timed steps; value = median of {len(reps)} repetitions (warm rate); e2e repeats the same arm "
+                                   "from the same pool state with the timed steps going through pinned host buffers",
                        "l2": f"weights streamed per step {avg_R * shape.n_layers * shape.expert_bytes / GIB:.2f} GiB >> 126 MB L2 (no flush needed)",
                        "layers_reduced_for_host_ram": reduced, "full_config_layers": full_layers, "parallelism": "replicas" if world > 1 else "single"},
             "clocks": clocks,
-            "e2e": {"value": args.steps * B * world / (ms_e2e * 1e-3), "unit": "tokens/s", "h2d_bytes_per_step": io_bytes,
-                    "d2h_bytes_per_step": io_bytes, "outputs_equal_device_run": bool(same)},
-            "gpu_launches": int(st1.kernel_launches - st0.kernel_launches),
+            "e2e": {"value": K * B * world / (ms_e2e * 1e-3), "unit": "tokens/s", "h2d_bytes_per_step": io_bytes,
+                    "d2h_bytes_per_step": io_bytes, "outputs_equal_device_run": bool(same),
+                    "misses_in_timed_steps": e2e_reps[0]["misses_warm"]},
+            "gpu_launches": r0["launches"],
             "roofline": roof,
+            "rates": {"warm_tokens_per_s_median": value, "warm_tokens_per_s_best": replica_throughput(K * B, world, best_ms),
+                      "cold_tokens_per_s_median": replica_throughput((n_warm + K) * B, world, cold_ms),
+                      "misses_cold_segment": r0["misses_cold"], "misses_warm_segment": misses, "repetitions": len(reps),
+                      "repetitions_identical_outputs_and_misses": bool(reps_identical),
+                      "warm_ms_per_rep": [round(r["warm_ms"], 3) for r in reps]},
             "paging": {"hit_rate": round(1 - misses / max(1, refs), 5), "misses": int(misses), "references": int(refs),
-                       "miss_bytes_per_step": misses * shape.expert_bytes / args.steps,
-                       "hbm_bound_tokens_per_s": round(hbm_peak * 1e9 / max(1.0, avg_R * shape.n_layers * shape.expert_bytes), 1)},
+                       "miss_bytes_per_step": misses * shape.expert_bytes / K,
+                       "hbm_bound_tokens_per_s": round(hbm_peak * 1e9 * B / max(1.0, avg_R * shape.n_layers * shape.expert_bytes), 1)},
             "kernels": kern, "setup_s": round(t_setup, 1)}
+    ctx.close()
+    del ctx
     if rank == 0 and world == 1 and not args.no_miss_path:
         try:
             line["miss_path"] = miss_path_microbench(shape, args)
-            if roof and "host_link_us_per_step" in roof:            # restate the link bound with the peak measured just now
-                link_s = misses * shape.expert_bytes / args.steps / (line["miss_path"]["link_peak_gbs"] * 1e9)
+            if roof and "bytes_per_launch" in roof and fused:       # "the slower of the two" (north_star), with the link peak measured just now
+                link_s = misses * shape.expert_bytes / K / (line["miss_path"]["link_peak_gbs"] * 1e9)
                 roof["host_link_us_per_step"] = round(link_s * 1e6, 1)
                 roof["step_lower_bound_us"] = round(max(roof["bytes_per_launch"] / (hbm_peak * 1e9), link_s) * 1e6, 1)
                 roof["frac_of_step_lower_bound"] = round(roof["step_lower_bound_us"] / roof["avg_launch_us"], 4)
-        except Exception as ex:                        # the microbenchmark must never take the headline down
+        except Exception as ex:                        # a microbenchmark must never take the headline down
             line["miss_path"] = {"error": repr(ex)[:200]}
+    if rank == 0 and world == 1 and not args.no_micro and shape.dtype == "bf16":
+        try:
+            line["ffn_only"] = {"this_shape": ffn_microbench(shape, args)}
+            other = si.MIXTRAL if shape.name.startswith("qwen3") else si.QWEN3
+            line["ffn_only"][other.name] = ffn_microbench(other, args, n_steps=8)
+        except Exception as ex:
+            line["ffn_only"] = {"error": repr(ex)[:300]}
+        try:
+            line["route_only"] = route_microbench(shape, args)
+        except Exception as ex:
+            line["route_only"] = {"error": repr(ex)[:300]}
     if rank == 0 and world == 1 and not args.no_prefill and shape.dtype == "bf16":
         try:
             line["prefill"] = prefill_bench(shape, args)
@@ -731,7 +815,7 @@ def main_ours(args):
         routers = [si.gen_router(shape, l) for l in range(nl)]
         tot, done, toks = 0.0, 0, 0
         while tot < 12.0 and toks < 4096:
-            x = hidden[(args.warmup + toks) % n_all].to(shape.torch_dtype)
+            x = hidden[(n_warm + toks) % n_all].to(shape.torch_dtype)
             t0 = time.perf_counter()
             for l in range(nl):
                 out, *_ = mf.moe_layer(x, blobs[l], routers[l][0], routers[l][1], shape.top_k, shape.d_ff)
@@ -739,10 +823,11 @@ def main_ours(args):
             tot += time.perf_counter() - t0
             done += nl
             toks += 1
-        line["cpu_baseline"] = {"value": (done / shape.n_layers) * B / tot, "unit": "tokens/s", "cores": torch.get_num_threads(),
-                                "kind": "oracle", "sample": f"{toks} decode tokens x first {nl} of {shape.n_layers} layers, "
+        line["cpu_baseline"] = {"value": (done / shape.n_layers) * B / tot, "unit": "tokens/s", "cores": os.cpu_count(),
+                                "torch_threads": torch.get_num_threads(),
+                                "kind": "oracle (oracle/moe_forward.py: PyTorch CPU ops in fp64, as it stands, all experts resident)",
+                                "sample": f"{toks} decode tokens x first {nl} of {shape.n_layers} layers, "
                                 f"tokens/s scaled by layers done / {shape.n_layers} ({tot:.1f} s of CPU work)"}
-    ctx.close()
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:

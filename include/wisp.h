@@ -219,6 +219,14 @@ int wisp_last_logits(wisp_ctx* ctx, float* z, int32_t n_tokens);
 /* Drive the pager with a given routed-id list (host, n_ids ids, repeats allowed): runs the residency
  * lookup and the demand fetch of one step of `layer`, no router and no FFN.  Synchronises. */
 int wisp_debug_step_routing(wisp_ctx* ctx, int32_t layer, const int32_t* ids, int32_t n_ids);
+/* Empty the expert pool of every layer and zero the paging state and counters (pi, pi^-1, tau, f, clock, steps, hits, misses,
+ * evictions, references; reuse-distance histograms): the context is as cold as after registration.  Slot contents, the split
+ * and KV reservations are kept.  Measurement / verification helper: every timed arm starts from this state.  Synchronises. */
+int wisp_debug_reset_pool(wisp_ctx* ctx);
+/* FFN-only replay (microbenchmark m1): launches the decode FFN kernel for wave 0 of the plan left by the most recent
+ * wisp_debug_step_routing(layer, ids) -- ids given in (token, rank) order, n_tokens*top_k of them, every expert resident after
+ * that call -- on `hidden` (device, [n_tokens, d_model]); no router, no lookup, no combine.  n_tokens <= 8.  Asynchronous. */
+int wisp_debug_ffn_launch(wisp_ctx* ctx, int32_t layer, const void* hidden, int32_t n_tokens, void* cuda_stream);
 /* Residency state of `layer`: host pi_inv [C] (expert per slot, -1 empty), tau [C], freq [E], *clock.
  * Any pointer may be NULL.  Synchronises. */
 int wisp_debug_residency(wisp_ctx* ctx, int32_t layer, int32_t* pi_inv, uint64_t* tau, uint64_t* freq,

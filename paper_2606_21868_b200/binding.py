@@ -73,6 +73,8 @@ _SIGS = {
     "wisp_last_topk": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]),
     "wisp_last_logits": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32]),
     "wisp_debug_step_routing": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_int32]),
+    "wisp_debug_reset_pool": (C.c_int, [C.c_void_p]),
+    "wisp_debug_ffn_launch": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]),
     "wisp_debug_residency": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "wisp_debug_verify_pool": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_int32)]),
     "wisp_timing_enable": (C.c_int, [C.c_void_p, C.c_int32]),
@@ -196,6 +198,12 @@ class Wisp:
     def debug_step_routing(self, layer, ids):
         arr = (C.c_int32 * len(ids))(*[int(i) for i in ids])
         self._ck(self.L.wisp_debug_step_routing(self.ctx, layer, arr, len(ids)), "wisp_debug_step_routing")
+
+    def debug_reset_pool(self):
+        self._ck(self.L.wisp_debug_reset_pool(self.ctx), "wisp_debug_reset_pool")
+
+    def debug_ffn_launch(self, layer, hidden, stream):
+        self._ck(self.L.wisp_debug_ffn_launch(self.ctx, layer, _ptr(hidden), hidden.shape[0], C.c_void_p(stream)), "wisp_debug_ffn_launch")
 
     def debug_residency(self, layer):
         import numpy as np

@@ -1090,7 +1090,7 @@ int wisp_debug_step_routing(wisp_ctx* ctx, int32_t layer, const int32_t* ids, in
   a.ids = ctx->dbg_ids; a.n_pairs = n_ids; a.E = ctx->cfg.n_experts; a.C = ctx->C; a.policy = ctx->cfg.policy; a.layer = layer;
   a.st = layer_state(ctx, layer); a.plan = ctx->plan; a.host_plan = ctx->host_plan;
   a.trace = ctx->trace; a.trace_ctr = ctx->trace_ctr; a.trace_cap = ctx->trace_cap; a.trace_on = ctx->trace_on;
-  a.track = ctx->track; a.build_pairs = 0; a.wave_order = ctx->wave_order;
+  a.track = ctx->track; a.build_pairs = n_ids <= std::min<int>(kDecodeMaxTokens, ctx->cfg.max_tokens) * ctx->cfg.top_k ? 1 : 0; a.wave_order = ctx->wave_order;
   residency_plan_kernel<<<1, kPlanThreads>>>(a);
   CK(cudaGetLastError());
   CK(cudaDeviceSynchronize());
@@ -1100,6 +1100,47 @@ int wisp_debug_step_routing(wisp_ctx* ctx, int32_t layer, const int32_t* ids, in
     if (rc) return rc;
     CK(cudaDeviceSynchronize());   // wave w+1 may overwrite slots of wave w: keep them serial
   }
+  return WISP_OK;
+}
+
+int wisp_debug_reset_pool(wisp_ctx* ctx) {
+  if (!ctx) return WISP_EINVAL;
+  CK(cudaDeviceSynchronize());
+  const size_t L = ctx->cfg.n_layers, E = ctx->cfg.n_experts;
+  CK(cudaMemset(ctx->pi, 0xff, L * E * sizeof(int)));
+  CK(cudaMemset(ctx->pi_inv, 0xff, L * E * sizeof(int)));
+  CK(cudaMemset(ctx->tau, 0, L * E * sizeof(u64)));
+  CK(cudaMemset(ctx->freq, 0, L * E * sizeof(u64)));
+  CK(cudaMemset(ctx->scal, 0, L * 8 * sizeof(u64)));
+  CK(cudaMemset(ctx->last_pos, 0, L * E * sizeof(u64)));
+  CK(cudaMemset(ctx->hist, 0, L * (E + 2) * sizeof(u64)));
+  std::fill(ctx->host_hist.begin(), ctx->host_hist.end(), 0.0);
+  CK(cudaDeviceSynchronize());
+  return WISP_OK;
+}
+
+int wisp_debug_ffn_launch(wisp_ctx* ctx, int32_t layer, const void* hidden, int32_t n_tokens, void* cuda_stream) {
+  if (!ctx || !hidden || layer < 0 || layer >= ctx->cfg.n_layers || n_tokens < 1 || n_tokens > kDecodeMaxTokens ||
+      n_tokens > ctx->cfg.max_tokens)
+    return fail(ctx, WISP_EINVAL, "bad argument");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const DecodeGeom g = ctx->dgeom[n_tokens <= 2 ? 0 : 1];
+  DecodeSmem sm;
+  int rc = decode_smem(ctx, g, n_tokens, ctx->ffn_smem, false, &sm);
+  if (rc) return rc;
+  DecodeFfnArgs fa{};
+  fa.pool = ctx->arena; fa.blob_bytes = ctx->Me; fa.L = ctx->cfg.n_layers; fa.layer = layer; fa.k = ctx->cfg.top_k;
+  fa.partial = ctx->partial; fa.master = nullptr; fa.ticket = ctx->dsync + 1;
+  CK(cudaMemsetAsync(ctx->dsync + 1, 0, sizeof(unsigned), st));
+  ++ctx->launches;
+  if (ctx->cfg.dtype == WISP_F32)
+    decode_ffn_kernel<float><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, 0, ctx->C, ctx->cfg.n_experts, n_tokens,
+                                                                         static_cast<const float*>(hidden), sm.n_slots, sm.xs_pitch, sm.ring_off);
+  else
+    decode_ffn_kernel<__nv_bfloat16><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, 0, ctx->C, ctx->cfg.n_experts, n_tokens,
+                                                                                 static_cast<const __nv_bfloat16*>(hidden), sm.n_slots,
+                                                                                 sm.xs_pitch, sm.ring_off);
+  CK(cudaGetLastError());
   return WISP_OK;
 }
 
