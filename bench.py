@@ -585,6 +585,144 @@ def route_microbench(shape, args):
     return out
 
 
+def verify_stack(shape, runs, *, steps, batches, prefill_tokens=0, samples=((0, 0),), policies=("lru",), log=None):
+    """Full-depth parity of one BASELINE.json stack through the launch configuration the bench times (wisp_stack_forward, fused
+    fetch).  ONE context sized for the all-resident pool; each run re-splits it (wisp_set_split) and starts from an empty pool.
+      (a) the trace of every run == oracle/paging.py fed the GPU's ids;   (b) every step's x_L is byte-identical to the
+      all-resident run's;   (c)/(d) teacher-forced against oracle/moe_forward.py on the sampled (step, layer) pairs.
+    runs: list of (label, slots) -- the first must be the all-resident reference.  Returns the summary dict."""
+    import paper_2606_21868_b200 as wp
+    from oracle import moe_forward as mf
+    from oracle.paging import LFU, LRU, PagerLayer
+    L, E, k, d = shape.n_layers, shape.n_experts, shape.top_k, shape.d_model
+    a = shape.slot_unit_bytes
+    max_tokens = max(max(batches), prefill_tokens, 1)
+    ctx = wp.Wisp(E * a, n_layers=L, n_experts=E, top_k=k, d_model=d, d_ff=shape.d_ff, max_tokens=max_tokens,
+                  dtype=wp.WISP_F32 if shape.dtype == "f32" else wp.WISP_BF16, fetch=wp.WISP_FETCH_FUSED, trace_capacity=1 << 23)
+    staging = torch.empty((E, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
+    for l in range(L):
+        si.gen_layer_experts(shape, l, "cuda", out=staging)
+        w_r, bias = si.gen_router(shape, l)
+        ctx.register_host_experts(l, staging, w_r, bias)
+    del staging
+    ctx.trace_enable(True)
+    stream = torch.cuda.Stream()
+    summary = {"shape": shape.name, "layers": L, "steps": steps, "batches": list(batches), "prefill_tokens": prefill_tokens,
+               "runs": [], "trace_events": 0, "byte_identical": True, "trace_equal": True}
+    xp = si.gen_prefill_hidden(shape, prefill_tokens).to(shape.torch_dtype).cuda() if prefill_tokens else None
+    for B in batches:
+        x = si.gen_decode_hidden(shape, steps, B).to(shape.torch_dtype).cuda()
+        ref = None                                   # (prefill out bytes, decode out bytes, routed ids per forward per layer)
+        for policy in policies:
+            ctx.set_policy(wp.WISP_LFU if policy == "lfu" else wp.WISP_LRU)
+            for label, slots in runs:
+                ctx.set_split(slots * a, 0)
+                ctx.debug_reset_pool()
+                ctx.trace_read()                     # drain
+                y = torch.empty_like(x)
+                yp = torch.empty_like(xp) if xp is not None else None
+                routed = []                          # per forward: list over layers of id lists
+                with torch.cuda.stream(stream):
+                    if xp is not None:
+                        ctx.stack_forward(xp, yp, stream.cuda_stream)
+                        stream.synchronize()
+                        if ref is None:
+                            routed.append([ctx.last_topk(l)[0].flatten().tolist() for l in range(L)])
+                    for t in range(steps):
+                        ctx.stack_forward(x[t], y[t], stream.cuda_stream)
+                        if ref is None:              # ids are read in the reference run only: identical bytes imply identical routing
+                            stream.synchronize()
+                            routed.append([ctx.last_topk(l)[0].flatten().tolist() for l in range(L)])
+                    stream.synchronize()
+                got = ctx.trace_read(cap=1 << 23)
+                st = ctx.stats()
+                if ref is None:
+                    ref = (yp.view(torch.uint8).cpu() if yp is not None else None, y.view(torch.uint8).cpu(), routed)
+                same = torch.equal(y.view(torch.uint8).cpu(), ref[1]) and (yp is None or torch.equal(yp.view(torch.uint8).cpu(), ref[0]))
+                pagers = [PagerLayer(C=slots, E=E, policy=LFU if policy == "lfu" else LRU) for _ in range(L)]
+                want = []
+                for per in ref[2]:
+                    for l, ids in enumerate(per):
+                        want += [(l, e.step, e.wave, e.expert, e.slot, e.evicted, e.kind) for e in pagers[l].step(ids)]
+                trace_ok = got == want and st.trace_dropped == 0
+                bad_slots = sum(ctx.debug_verify_pool(l) for l in range(L))
+                run = {"pool": label, "slots": slots, "policy": policy, "batch": B, "trace_events": len(got), "trace_equal": trace_ok,
+                       "byte_identical": bool(same), "misses": int(st.total.misses), "hits": int(st.total.hits),
+                       "oracle_misses": sum(p.misses for p in pagers), "pool_bytes_equal_master": bad_slots == 0}
+                summary["runs"].append(run)
+                summary["trace_events"] += len(got)
+                summary["byte_identical"] &= bool(same) and bad_slots == 0
+                summary["trace_equal"] &= trace_ok
+                if log:
+                    log(run)
+        # ---- (c)/(d): teacher-forced oracle check on sampled (step, layer) pairs, per-layer API on the all-resident pool ----
+        ctx.set_policy(wp.WISP_LRU)
+        ctx.set_split(runs[0][1] * a, 0)
+        ctx.debug_reset_pool()
+        worst, n_ids, tol = 0.0, 0, (1e-5 if shape.dtype == "f32" else 2e-2)
+        st_ = torch.cuda.current_stream().cuda_stream
+        for t in sorted({s for s, _ in samples if s < steps}):
+            want_layers = {l for s, l in samples if s == t and l < L}
+            xi = x[t].clone()
+            for l in range(L):
+                out = torch.empty_like(xi)
+                ctx.moe_forward(l, xi, out, st_)
+                xn = torch.empty_like(xi)
+                ctx.residual_add(xi, out, xn, st_)
+                if l in want_layers:
+                    torch.cuda.synchronize()
+                    ids, w = ctx.last_topk(l)
+                    blob = si.gen_layer_experts(shape, l, "cuda")
+                    w_r, bias = si.gen_router(shape, l)
+                    o_ref, o_ids, o_w, z = mf.moe_layer(xi.cpu(), blob, w_r, bias, k, shape.d_ff)
+                    zs = torch.sort(z, dim=1, descending=True).values
+                    clear = (zs[:, k - 1] - zs[:, k]) > 1e-4 if k < E else torch.ones(z.shape[0], dtype=torch.bool)
+                    gid = torch.from_numpy(ids).long()
+                    assert torch.equal(gid[clear], o_ids[clear]), f"parity (c): step {t} layer {l}"
+                    if not bool(clear.all()):
+                        o_ref, _, o_w, _ = mf.moe_layer(xi.cpu(), blob, w_r, bias, k, shape.d_ff, ids=gid)
+                    err = (out.cpu().double() - o_ref).abs().max().item() / o_ref.abs().max().item()
+                    assert err <= tol, f"parity (d): step {t} layer {l}: {err}"
+                    worst = max(worst, err)
+                    n_ids += int(clear.sum())
+                    del blob
+                xi = xn
+            torch.cuda.synchronize()
+            # the per-layer chain ends in the same bytes as the stack call the bench times
+            assert torch.equal(xi.view(torch.uint8).cpu(), ref[1][t]), f"per-layer chain != wisp_stack_forward at step {t}"
+        summary.setdefault("max_rel_err", 0.0)
+        summary["max_rel_err"] = max(summary["max_rel_err"], worst)
+        summary["oracle_samples"] = summary.get("oracle_samples", 0) + len([1 for s, l in samples if s < steps and l < L])
+        summary["ids_checked"] = summary.get("ids_checked", 0) + n_ids
+    ctx.close()
+    return summary
+
+
+def main_verify(args):
+    """bench.py --verify 2,3,4: BASELINE.json configs 2-4 at full depth (byte-identical at every cap)."""
+    out = {}
+    steps = args.verify_steps
+    log = lambda r: print(json.dumps(r), file=sys.stderr, flush=True)
+    q = si.QWEN3 if args.layers <= 0 else si.QWEN3.with_layers(args.layers)
+    m = si.MIXTRAL if args.layers <= 0 else si.MIXTRAL.with_layers(args.layers)
+    slots_of = lambda shape, gib: max(1, min(shape.n_experts, int(gib * GIB) // si.QWEN3.slot_unit_bytes if shape.name.startswith("qwen3") else int(gib * GIB) // si.MIXTRAL.slot_unit_bytes))
+    samp = lambda shape: tuple((s, l) for s in (0, steps // 2, steps - 1) for l in (0, shape.n_layers // 2, shape.n_layers - 1))
+    for cfg in [c.strip() for c in args.verify.split(",") if c.strip()]:
+        if cfg == "2":      # 8 GiB, LRU vs LFU, batch 1
+            out["config2"] = verify_stack(q, [("all-resident", q.n_experts), ("8 GiB", slots_of(q, 8))], steps=steps, batches=(1,),
+                                          samples=samp(q), policies=("lru", "lfu"), log=log)
+        elif cfg == "3":    # prefill 2048 + decode at batch 1 and 4, budgets 4/8/16/32 GiB + all-resident
+            runs = [("all-resident", q.n_experts)] + [(f"{g} GiB", slots_of(q, g)) for g in (32, 16, 8, 4)]
+            out["config3"] = verify_stack(q, runs, steps=steps, batches=(1, 4), prefill_tokens=2048, samples=samp(q), log=log)
+        elif cfg == "4":    # Mixtral shape, 24 GiB -> C = 2, batch 1 and 4
+            out["config4"] = verify_stack(m, [("all-resident", m.n_experts), ("24 GiB", slots_of(m, 24))], steps=steps, batches=(1, 4),
+                                          samples=samp(m), log=log)
+    ok = all(v["byte_identical"] and v["trace_equal"] for v in out.values())
+    print(json.dumps({"verify": out, "ok": ok}))
+    if not ok:
+        raise SystemExit(1)
+
+
 POOL_WARM_STEPS = 16          # SURVEY.md 8(d) protocol: "warm" = the steps after the first 16 from an empty pool
 
 
@@ -836,7 +974,9 @@ def main_ours(args):
 
 if __name__ == "__main__":
     a = parse()
-    if a.workload == "mvwsa":
+    if a.verify:
+        main_verify(a)
+    elif a.workload == "mvwsa":
         main_mvwsa(a)
     elif a.impl == "reference":
         main_reference(a)

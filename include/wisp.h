@@ -209,6 +209,9 @@ int wisp_trace_enable(wisp_ctx* ctx, int32_t on);
 /* Select the overflow wave order (wisp_wave_order) for all later forwards.  Synchronises the device; residency state,
  * counters and slot contents are kept.  Errors: EINVAL (NULL ctx or unknown order; state unchanged). */
 int wisp_set_wave_order(wisp_ctx* ctx, int32_t order);
+/* Select the eviction policy (wisp_policy) for all later forwards; tau and f are kept (both are maintained under either
+ * policy), so a switch is usually followed by wisp_debug_reset_pool.  Synchronises.  Errors: EINVAL. */
+int wisp_set_policy(wisp_ctx* ctx, int32_t policy);
 /* Drain up to `cap` events into host `buf` (oldest first); *n_out = number written.  Synchronises. */
 int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t* n_out);
 /* Routing of the most recent forward of `layer`: host ids [n_tokens, k] (rank order) and w [n_tokens, k].

@@ -69,6 +69,7 @@ _SIGS = {
     "wisp_layer_stats_read": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(WispLayerStats)]),
     "wisp_trace_enable": (C.c_int, [C.c_void_p, C.c_int32]),
     "wisp_set_wave_order": (C.c_int, [C.c_void_p, C.c_int32]),
+    "wisp_set_policy": (C.c_int, [C.c_void_p, C.c_int32]),
     "wisp_trace_read": (C.c_int, [C.c_void_p, C.POINTER(WispTraceEvent), C.c_uint64, C.POINTER(C.c_uint64)]),
     "wisp_last_topk": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]),
     "wisp_last_logits": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32]),
@@ -172,6 +173,9 @@ class Wisp:
 
     def set_wave_order(self, order):
         self._ck(self.L.wisp_set_wave_order(self.ctx, int(order)), "wisp_set_wave_order")
+
+    def set_policy(self, policy):
+        self._ck(self.L.wisp_set_policy(self.ctx, int(policy)), "wisp_set_policy")
 
     def trace_read(self, cap=1 << 20):
         buf = (WispTraceEvent * cap)()

@@ -1031,6 +1031,15 @@ int wisp_set_wave_order(wisp_ctx* ctx, int32_t order) {
   return WISP_OK;
 }
 
+int wisp_set_policy(wisp_ctx* ctx, int32_t policy) {
+  if (!ctx) return WISP_EINVAL;
+  if (policy != WISP_LRU && policy != WISP_LFU) return fail(ctx, WISP_EINVAL, "wisp_set_policy: policy must be WISP_LRU or WISP_LFU");
+  CK(cudaDeviceSynchronize());
+  ctx->cfg.policy = policy;
+  drop_graphs(ctx);   // kernel argument baked into captured graphs
+  return WISP_OK;
+}
+
 int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t* n_out) {
   if (!ctx || !n_out || (cap && !buf)) return fail(ctx, WISP_EINVAL, "bad argument");
   CK(cudaDeviceSynchronize());
