@@ -675,8 +675,16 @@ def verify_stack(shape, runs, *, steps, batches, prefill_tokens=0, samples=((0, 
                     blob = si.gen_layer_experts(shape, l, "cuda")
                     w_r, bias = si.gen_router(shape, l)
                     o_ref, o_ids, o_w, z = mf.moe_layer(xi.cpu(), blob, w_r, bias, k, shape.d_ff)
+                    if not bool(torch.isfinite(o_ref).all()):          # G23: the recipe's hidden state left the finite range
+                        summary["samples_skipped_nonfinite"] = summary.get("samples_skipped_nonfinite", 0) + 1
+                        del blob
+                        xi = xn
+                        continue
                     zs = torch.sort(z, dim=1, descending=True).values
-                    clear = (zs[:, k - 1] - zs[:, k]) > 1e-4 if k < E else torch.ones(z.shape[0], dtype=torch.bool)
+                    # (c) binds where the k-th / (k+1)-th logit gap exceeds 1e-4 (north_star) AND what fp32 can resolve at this
+                    # logit magnitude (2^-16 relative: 128 ulp of slack for a d-term fp32 dot product; only matters once |z| >> 1)
+                    margin = torch.clamp(z.abs().max(dim=1).values * 2.0 ** -16, min=1e-4)
+                    clear = (zs[:, k - 1] - zs[:, k]) > margin if k < E else torch.ones(z.shape[0], dtype=torch.bool)
                     gid = torch.from_numpy(ids).long()
                     assert torch.equal(gid[clear], o_ids[clear]), f"parity (c): step {t} layer {l}"
                     if not bool(clear.all()):
@@ -715,8 +723,12 @@ def main_verify(args):
             runs = [("all-resident", q.n_experts)] + [(f"{g} GiB", slots_of(q, g)) for g in (32, 16, 8, 4)]
             out["config3"] = verify_stack(q, runs, steps=steps, batches=(1, 4), prefill_tokens=2048, samples=samp(q), log=log)
         elif cfg == "4":    # Mixtral shape, 24 GiB -> C = 2, batch 1 and 4
+            # Under BASELINE.json's recipe (N(0, 0.02) weights, d_ff = 14336, no normalisation) this stack's hidden state grows
+            # doubly exponentially with depth (|x| ~ 1e2 at layer 13, 1e7 at layer 15, inf soon after): (a) and (b) are checked
+            # at full depth regardless; the oracle samples sit in the layers where the values are still O(1).
+            samp4 = tuple((s, l) for s in (0, steps // 2, steps - 1) for l in (0, 4, 9))
             out["config4"] = verify_stack(m, [("all-resident", m.n_experts), ("24 GiB", slots_of(m, 24))], steps=steps, batches=(1, 4),
-                                          samples=samp(m), log=log)
+                                          samples=samp4, log=log)
     ok = all(v["byte_identical"] and v["trace_equal"] for v in out.values())
     print(json.dumps({"verify": out, "ok": ok}))
     if not ok:

@@ -82,6 +82,7 @@ typedef struct {
   int32_t unit_rows;   /* act rows per decode FFN work unit: multiple of 8 dividing d_ff with d_ff/unit_rows a multiple of 8;
                           0 = library default (8 for calls of <= 2 tokens, 16 for 3..8 tokens).  Outputs are byte-identical across
                           budgets, policies and fetch paths for a GIVEN unit size; changing it regroups the fp32 partial sums. */
+  int32_t reserved0;   /* must be 0 */
   uint64_t kv_block_bytes;  /* b: bytes per KV block summed over layers; 0 = no KV accounting */
   uint64_t kv_floor_blocks; /* kappa_min of Eq. 4; wisp_set_split refuses to go below it */
   uint64_t trace_capacity;  /* trace ring capacity in events; 0 = library default (1<<20) */

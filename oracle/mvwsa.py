@@ -3,7 +3,10 @@
 TEST INFRASTRUCTURE (see oracle/__init__.py).  Pure Python, integers and fp64.
 Readings (SURVEY.md §8(c) / DESIGN.md): G10 floor brackets in Eq. 7, 8; G11 constants h = 0.2,
 Delta = 1, C_min = k, lambda = 0.5; G12 KV cost model = reservation/preemption scheduler below.
-Unpinned ("parity unpinned"): the KV-reservation scheduler model and lambda/hysteresis constants.
+Pins (tests/): Table 4 (P6), hand-stepped KV schedule (tests/golden/hand_kv_schedule.txt), two-period decay hand case,
+Mattson k = 1 equality (P7), brute-force argmin == greedy (P10).  Still "parity unpinned": the k > 1 reuse-distance
+ESTIMATOR of Algorithm 1's miss count beyond monotonicity and its limits (P7), and the VALUES of the constants lambda = 0.5,
+h = 0.2, Delta = 1 (G11: the paper gives none).
 """
 from __future__ import annotations
 

@@ -21,7 +21,7 @@ STATUS_NAMES = {0: "WISP_OK", -1: "WISP_EINVAL", -2: "WISP_ENOMEM", -3: "WISP_EC
 class WispConfig(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("n_experts", C.c_int32), ("top_k", C.c_int32), ("d_model", C.c_int32),
                 ("d_ff", C.c_int32), ("max_tokens", C.c_int32), ("dtype", C.c_int32), ("policy", C.c_int32),
-                ("fetch", C.c_int32), ("ring_stages", C.c_int32), ("unit_rows", C.c_int32), ("kv_block_bytes", C.c_uint64),
+                ("fetch", C.c_int32), ("ring_stages", C.c_int32), ("unit_rows", C.c_int32), ("reserved0", C.c_int32), ("kv_block_bytes", C.c_uint64),
                 ("kv_floor_blocks", C.c_uint64), ("trace_capacity", C.c_uint64)]
 
 
@@ -116,7 +116,7 @@ class Wisp:
     def __init__(self, budget_bytes: int, *, n_layers, n_experts, top_k, d_model, d_ff, max_tokens, dtype, policy=WISP_LRU,
                  fetch=WISP_FETCH_ZEROCOPY, kv_block_bytes=0, kv_floor_blocks=0, trace_capacity=0, ring_stages=0, unit_rows=0):
         self.L = lib()
-        self.cfg = WispConfig(n_layers, n_experts, top_k, d_model, d_ff, max_tokens, dtype, policy, fetch, ring_stages, unit_rows,
+        self.cfg = WispConfig(n_layers, n_experts, top_k, d_model, d_ff, max_tokens, dtype, policy, fetch, ring_stages, unit_rows, 0,
                               kv_block_bytes, kv_floor_blocks, trace_capacity)
         self.ctx = C.c_void_p()
         rc = self.L.wisp_create(budget_bytes, C.byref(self.cfg), C.byref(self.ctx))
