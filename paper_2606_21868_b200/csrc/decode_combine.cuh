@@ -67,8 +67,8 @@ __device__ __forceinline__ void combine_slice(const CombineArgs& a, int t, int j
       for (int c0 = 0; c0 < per; c0 += 16) {                 // up to 16 independent L2 reads in flight, added in ascending c
         float4 v[16];
 #pragma unroll
-        for (int u = 0; u < 16; ++u)
-          if (c0 + u < per) v[u] = __ldcg(reinterpret_cast<const float4*>(src + (size_t)(c0 + u) * a.d));
+        for (int u = 0; u < 16; ++u)                           // unpredicated (index clamped) so that all 16 loads issue before the first add
+          v[u] = __ldcg(reinterpret_cast<const float4*>(src + (size_t)min(c0 + u, per - 1) * a.d));
 #pragma unroll
         for (int u = 0; u < 16; ++u)
           if (c0 + u < per) {

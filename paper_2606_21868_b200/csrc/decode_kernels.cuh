@@ -58,7 +58,7 @@ struct DecodeArgs {
   u64* trace_ctr;
   u64 trace_cap;
   int trace_on, track;
-  u64* phase_ns;                // nullable: [kDecPhases + 2] globaltimer ns summed by CTA 0, then counts of hit / miss layers
+  u64* phase_ns;                // nullable: [kDecPhases + 2] globaltimer ns summed by the last CTA, then counts of hit / miss layers
 };
 
 // The per-layer plan in shared memory (same fields as PlanPtrs).
@@ -167,12 +167,13 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
 
   // ===================== consumer warps =====================
   const bool writer = blockIdx.x == 0;
-  const bool timing = writer && tid == 0 && a.phase_ns != nullptr;
+  const bool timing = blockIdx.x == gridDim.x - 1 && tid == 0 && a.phase_ns != nullptr;   // a CTA that is not the writer
   u64 t_prev = timing ? globaltimer_ns() : 0ull;
   auto stamp = [&](int phase) {
     if (timing) { const u64 t = globaltimer_ns(); a.phase_ns[phase] += t - t_prev; t_prev = t; }
   };
-  unsigned gen = 0, qseq = 0, gu_seq = 0, d_seq = 0, n_pre = 0;
+  unsigned gen = 0, qseq = 0, gu_seq = 0, d_seq = 0;
+  const uint32_t w_off = (uint32_t)((E * sizeof(float) + 127) & ~(size_t)127);   // staged region: [router bias of the next layer][weight slice]
   T* xs = reinterpret_cast<T*>(smem_raw);               // current hidden state, [T][xs_pitch], in EVERY CTA
   auto load_xs = [&](const void* src_) {
     const int vec_row = d * (int)sizeof(T) / 16;
@@ -203,17 +204,44 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     const bool last = l == a.layer_hi - 1;
     long long* zf_l = a.zfix + (size_t)(l & 1) * kDecodeMaxTokens * E;
 
-    // ---- route: logits -> top-k (one warp per token) ----
-    if (warp < T_) {
+    // ---- route: logits -> top-k (one warp per token); the other threads' loads of x_l (written by the previous layer's
+    // combine) are in flight meanwhile ----
+    constexpr int kXsRegs = 8;
+    const int xs_vec = T_ * (d * (int)sizeof(T) / 16);
+    const bool reload = l > a.layer_lo, reload_regs = xs_vec <= kXsRegs * kDecConsumers;
+    const void* x_src = a.xbuf[(l - 1 - a.layer_lo) & 1];
+    uint4 xr[kXsRegs];
+    if (reload && reload_regs) {
+#pragma unroll
+      for (int i = 0; i < kXsRegs; ++i)
+        if (i * kDecConsumers < xs_vec) xr[i] = __ldcg(reinterpret_cast<const uint4*>(x_src) + min(tid + i * kDecConsumers, xs_vec - 1));
+    }
+    {
       const float* bias = a.router_bias + (size_t)l * E;
-      const long long* zt = zf_l + (size_t)warp * E;
-      float* zout = writer ? a.logits + (size_t)warp * E : nullptr;     // test surface: wisp_last_logits
-      auto zf = [&](int e) {
-        const float z = logit_from_fix(__ldcg(zt + e), bias[e]);
-        if (zout) zout[e] = z;
+      if (reload) {                                            // staged in shared memory during the previous layer's FFN
+        mbar_wait(smem_u32(&ds.wpre), (unsigned)(l - 1 - a.layer_lo) & 1u);
+        bias = reinterpret_cast<const float*>(smem_raw + pre_off);
+      }
+      float* zout = writer ? a.logits : nullptr;               // test surface: wisp_last_logits
+      auto zf = [&](int t, int e) {
+        const float z = logit_from_fix(__ldcg(zf_l + (size_t)t * E + e), bias[e]);
+        if (zout) zout[(size_t)t * E + e] = z;
         return z;
       };
-      topk_softmax_warp<kPersistMaxExperts / 32>(zf, E, k, ds.ids + warp * k, ds.w + warp * k, lane);
+      // (T * k <= 256 pairs: kDecodeMaxTokens * kMaxTopK; the FFN dataflow's scratch is idle between waves)
+      topk_softmax_block(zf, T_, E, k, ds.ids, ds.w, reinterpret_cast<unsigned*>(&fs.red[0][0][0]), tid, kDecConsumers, 1);
+    }
+    if (reload) {
+      if (reload_regs) {
+        const int vec_row = d * (int)sizeof(T) / 16;
+#pragma unroll
+        for (int i = 0; i < kXsRegs; ++i) {
+          const int v = tid + i * kDecConsumers;
+          if (v < xs_vec) reinterpret_cast<uint4*>(xs + (size_t)(v / vec_row) * xs_pitch)[v % vec_row] = xr[i];
+        }
+      } else {
+        load_xs(x_src);
+      }
     }
     asm volatile("bar.sync 1, 256;" ::: "memory");
     stamp(0);
@@ -247,11 +275,14 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     if (tid == 0) {
       if (writer) a.sync[1 + ((qseq + 1) & 1u)] = 0u;          // ticket counter of the NEXT wave (idle since the wave before this one)
       mbar_arrive(smem_u32(&ds.go));                           // the producer may start streaming
-      if (pre) {
-        const uint32_t bytes = (uint32_t)(kSliceCols * E * sizeof(T));
-        const T* src = reinterpret_cast<const T*>(a.router_wt) + ((size_t)(l + 1) * d + (size_t)((int)blockIdx.x % (d / kSliceCols)) * kSliceCols) * E;
-        mbar_expect_tx(smem_u32(&ds.wpre), bytes);
-        bulk_g2s_nohint(smem_u32(smem_raw) + (uint32_t)pre_off, src, bytes, smem_u32(&ds.wpre));
+      if (!last) {                                             // + the next layer's router bias (every CTA routes)
+        const uint32_t wbytes = pre ? (uint32_t)(kSliceCols * E * sizeof(T)) : 0u, bbytes = (uint32_t)(E * sizeof(float));
+        mbar_expect_tx(smem_u32(&ds.wpre), wbytes + bbytes);
+        bulk_g2s_nohint(smem_u32(smem_raw) + (uint32_t)pre_off, a.router_bias + (size_t)(l + 1) * E, bbytes, smem_u32(&ds.wpre));
+        if (pre) {
+          const T* src = reinterpret_cast<const T*>(a.router_wt) + ((size_t)(l + 1) * d + (size_t)((int)blockIdx.x % (d / kSliceCols)) * kSliceCols) * E;
+          bulk_g2s_nohint(smem_u32(smem_raw) + (uint32_t)pre_off + w_off, src, wbytes, smem_u32(&ds.wpre));
+        }
       }
     }
     stamp(1);
@@ -291,17 +322,14 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
         if (!last) {
           const T* w16 = wrt + (size_t)j0 * E;
           if (sl == (int)blockIdx.x) {                         // the staged slice
-            mbar_wait(smem_u32(&ds.wpre), n_pre & 1u);
-            ++n_pre;
-            w16 = reinterpret_cast<const T*>(smem_raw + pre_off);
+            mbar_wait(smem_u32(&ds.wpre), (unsigned)(l - a.layer_lo) & 1u);
+            w16 = reinterpret_cast<const T*>(smem_raw + pre_off + w_off);
           }
           slice_logits<T>(w16, ds.xn, E, zf_n + (size_t)t * E, tid, kDecConsumers);
         }
       }
       if (!last) {
-        if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;   // E: x_{l+1} and its logits are complete
-        load_xs(xg);
-        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;   // E: x_{l+1} and its logits are complete (reloaded by the route step)
       }
     }
     stamp(5);

@@ -306,58 +306,80 @@ __device__ __forceinline__ void plan_compute(const PlanArgs& a, PlanShared<NT>& 
 template <int NT>
 __device__ __forceinline__ bool plan_fast_warp(const PlanArgs& a, PlanShared<NT>& sh, bool writer, int lane) {
   const int E = a.E, n_pairs = a.n_pairs;
-  if (a.track || n_pairs > 64 || E > 256) return false;
-  if (lane < 8) sh.bitmap[lane] = 0u;
-  __syncwarp();
-  const int e0 = lane < n_pairs ? a.ids[lane] : -1, e1 = lane + 32 < n_pairs ? a.ids[lane + 32] : -1;
-  if (e0 >= 0) atomicOr(&sh.bitmap[e0 >> 5], 1u << (e0 & 31));
-  if (e1 >= 0) atomicOr(&sh.bitmap[e1 >> 5], 1u << (e1 & 31));
-  __syncwarp();
-  unsigned word = lane < 8 ? sh.bitmap[lane] : 0u;
-  int inc = __popc(word);
+  if (a.track || n_pairs > 64 || E > NT) return false;
+  // Lane l holds pairs l and l + 32.  One pass of warp shuffles gives every pair its position in the expert-sorted pair
+  // order (pairs ordered by (expert id, pair index)), its expert's pair count and whether it is the first pair of its expert.
+  const int n_hi = n_pairs > 32 ? n_pairs - 32 : 0;
+  int e[2] = {lane < n_pairs ? a.ids[lane] : 0x7fffffff, lane < n_hi ? a.ids[lane + 32] : 0x7fffffff};
+  int pos[2] = {0, 0}, cnt[2] = {0, 0};
+  bool first[2] = {true, true};
+  const int n_lo = min(n_pairs, 32);
+  for (int q = 0; q < n_lo; ++q) {
+    const int eq = __shfl_sync(0xffffffffu, e[0], q);
 #pragma unroll
-  for (int o = 1; o < 8; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-  const int nR = __shfl_sync(0xffffffffu, inc, 7);
-  int pos = inc - __popc(word);
-  while (word) { const int b = __ffs(word) - 1; word &= word - 1; sh.R[pos++] = lane * 32 + b; }   // R ascending
-  __syncwarp();
+    for (int h = 0; h < 2; ++h) {
+      const int me = lane + 32 * h;
+      pos[h] += (eq < e[h]) || (eq == e[h] && q < me);
+      cnt[h] += (eq == e[h]);
+      first[h] = first[h] && !(eq == e[h] && q < me);
+    }
+  }
+  for (int q = 0; q < n_hi; ++q) {
+    const int eq = __shfl_sync(0xffffffffu, e[1], q);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int me = lane + 32 * h;
+      pos[h] += (eq < e[h]) || (eq == e[h] && q + 32 < me);
+      cnt[h] += (eq == e[h]);
+      first[h] = first[h] && !(eq == e[h] && q + 32 < me);
+    }
+  }
+  const bool live[2] = {lane < n_pairs, lane < n_hi};
+  // entry index of an expert = number of distinct smaller ids = first-pairs that sort before it
+  const unsigned lead0 = __ballot_sync(0xffffffffu, live[0] && first[0]), lead1 = __ballot_sync(0xffffffffu, live[1] && first[1]);
+  const int nR = __popc(lead0) + __popc(lead1);
+  int slot[2] = {-1, -1}, ent[2] = {0, 0};
   bool ok = nR <= a.C;
-  for (int i = lane; i < nR; i += 32) ok = ok && sh.pi[sh.R[i]] >= 0;
-  if (!__all_sync(0xffffffffu, ok)) return false;
-  // pairs grouped by expert: counts, offsets (ascending id == ascending entry), stable lists
-  int run = 0;
-  for (int i0 = 0; i0 < nR; i0 += 32) {
-    const int i = i0 + lane;
-    const int e = i < nR ? sh.R[i] : -1;
-    int cnt = 0;
-    for (int p = 0; p < n_pairs; ++p) cnt += (a.ids[p] == e);
-    if (e < 0) cnt = 0;
-    int sc = cnt;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, sc, o); if (lane >= o) sc += v; }
-    const int off = run + sc - cnt;
-    if (e >= 0) {
-      const int slot = sh.pi[e];
-      a.plan.entry_expert[i] = e; a.plan.entry_slot[i] = slot; a.plan.entry_miss[i] = 0;
-      a.plan.exp_count[e] = cnt; a.plan.exp_offset[e] = off;
-      if (a.plan.unit_entry) a.plan.unit_entry[i] = i;
-      int j = 0;
-      for (int p = 0; p < n_pairs; ++p)
-        if (a.ids[p] == e) { a.plan.pair_list[off + j] = p; if (a.plan.pair_pos) a.plan.pair_pos[p] = off + j; ++j; }
-      if (writer) {                                                // line 9: the tick
-        a.st.tau[slot] = sh.clock + 1ull;
-        a.st.freq[e] = sh.freq[e] + 1ull;
-        if (a.trace_on) {
-          const u64 base = a.trace_ctr[0];
-          if (base + (u64)nR <= a.trace_cap) {
-            wisp_trace_event ev;
-            ev.step = sh.scal[1]; ev.layer = (uint32_t)a.layer; ev.wave = 0u; ev.expert = e; ev.slot = slot; ev.evicted = -1; ev.kind = 0u;
-            a.trace[base + i] = ev;
-          }
+  for (int h = 0; h < 2; ++h) {
+    if (live[h] && first[h]) {
+      slot[h] = sh.pi[e[h]];
+      ok = ok && slot[h] >= 0;
+    }
+  }
+  if (!__all_sync(0xffffffffu, ok)) return false;
+  // position of every first-pair among the first-pairs in sorted order: pairs are scattered by pos through shared scratch
+  if (lane < 2) sh.bitmap[lane] = 0u;
+  __syncwarp();
+#pragma unroll
+  for (int h = 0; h < 2; ++h)
+    if (live[h] && first[h]) atomicOr(&sh.bitmap[pos[h] >> 5], 1u << (pos[h] & 31));
+  __syncwarp();
+  const unsigned b0 = sh.bitmap[0], b1 = sh.bitmap[1];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    if (!live[h]) continue;
+    const int p = lane + 32 * h;
+    a.plan.pair_list[pos[h]] = p;
+    if (a.plan.pair_pos) a.plan.pair_pos[p] = pos[h];
+    if (!first[h]) continue;
+    ent[h] = pos[h] < 32 ? __popc(b0 & ((1u << pos[h]) - 1u)) : __popc(b0) + __popc(b1 & ((1u << (pos[h] - 32)) - 1u));
+    const int i = ent[h];
+    a.plan.entry_expert[i] = e[h]; a.plan.entry_slot[i] = slot[h]; a.plan.entry_miss[i] = 0;
+    a.plan.exp_count[e[h]] = cnt[h]; a.plan.exp_offset[e[h]] = pos[h];
+    if (a.plan.unit_entry) a.plan.unit_entry[i] = i;
+    if (writer) {                                                  // line 9: the tick
+      a.st.tau[slot[h]] = sh.clock + 1ull;
+      a.st.freq[e[h]] = sh.freq[e[h]] + 1ull;
+      if (a.trace_on) {
+        const u64 base = a.trace_ctr[0];
+        if (base + (u64)nR <= a.trace_cap) {
+          wisp_trace_event ev;
+          ev.step = sh.scal[1]; ev.layer = (uint32_t)a.layer; ev.wave = 0u; ev.expert = e[h]; ev.slot = slot[h]; ev.evicted = -1; ev.kind = 0u;
+          a.trace[base + i] = ev;
         }
       }
     }
-    run += __shfl_sync(0xffffffffu, sc, 31);
   }
   __syncwarp();
   if (lane == 0) {

@@ -63,12 +63,14 @@ __global__ void __launch_bounds__(256) router_logits_kernel(const T* __restrict_
 }
 
 // Top-k + softmax of ONE token's logits by ONE warp ("warp-shuffle softmax and top-k", BASELINE.json north_star; G7).
-// Lane l owns the logits of experts l, l+32, ... as order-preserving 32-bit keys.  One round = the warp maximum of the keys
-// (redux.sync.max), then the LOWEST expert id among the lanes that hold that maximum (redux.sync.min): the largest logit
-// with ties going to the lower id; k rounds give ids in (z desc, id asc) order.  -0 compares equal to +0 and a NaN ranks
-// with -inf (it can never corrupt an id: every selected id is a real expert).
-// w_i = exp(z_i - z_0) / sum_j exp(z_j - z_0), the sum taken in rank order j = 0..k-1 (every lane computes the same chain).
-// EPL = logits per lane (E <= 32 * EPL); zf(e) returns the logit of expert e.  ids_out / w_out: [k].
+// Lane l owns the experts l, l+32, ... (coalesced logit reads) as order-preserving 32-bit keys.  One round = the warp maximum of
+// the lanes' best keys (redux.sync.max); if one lane holds it (ballot) that is the winner, and on a tie the LOWEST expert id
+// among the tied lanes wins (redux.sync.min, rare): the largest logit with ties going to the lower id; k rounds give ids in
+// (z desc, id asc) order.  -0 compares equal to +0 and a NaN ranks with -inf (it can never corrupt an id: every selected id
+// is a real expert).
+// w_i = exp(z_i - z_0) / sum_j exp(z_j - z_0), the sum taken in rank order j = 0..k-1.
+// EPL = compile-time bound of per (E <= 32 * EPL); zf(e) returns the logit of expert e.  ids_out / w_out: [k], shared or global;
+// w_out doubles as scratch for the selected logits.
 __device__ __forceinline__ unsigned topk_key(float z) {
   z += 0.0f;                                            // -0 -> +0
   unsigned u = __float_as_uint(z);
@@ -87,24 +89,77 @@ __device__ __forceinline__ void topk_softmax_warp(ZF zf, int E, int k, int* ids_
     const int e = lane + 32 * j;
     key[j] = e < E ? topk_key(zf(e)) : 0u;               // 0 = absent / already taken
   }
-  float my_z = 0.f;                                     // lane r keeps the logit of rank r
   for (int r = 0; r < k; ++r) {
     unsigned best = 0u;
     int best_j = 0;
 #pragma unroll
-    for (int j = EPL - 1; j >= 0; --j)                   // descending j with >= : among equal keys the lowest id of the lane wins
+    for (int j = EPL - 1; j >= 0; --j)                   // descending j with >= : among equal keys the lane's lowest id wins
       if (key[j] >= best) { best = key[j]; best_j = j; }
     const unsigned top = __reduce_max_sync(0xffffffffu, best);
-    const unsigned e = __reduce_min_sync(0xffffffffu, best == top ? (unsigned)(lane + 32 * best_j) : 0xffffffffu);
+    const unsigned tied = __ballot_sync(0xffffffffu, best == top);
+    int e = lane + 32 * best_j;
+    if (tied & (tied - 1u)) e = (int)__reduce_min_sync(0xffffffffu, best == top ? (unsigned)e : 0xffffffffu);   // several lanes: lowest id
+    else e = __shfl_sync(0xffffffffu, e, __ffs(tied) - 1);
+    if ((e & 31) == lane) {
+      ids_out[r] = e;
+      w_out[r] = topk_key_logit(top);
 #pragma unroll
-    for (int j = 0; j < EPL; ++j)
-      if ((int)e == lane + 32 * j) key[j] = 0u;
-    if (lane == r) { my_z = topk_key_logit(top); ids_out[r] = (int)e; }
+      for (int j = 0; j < EPL; ++j)
+        if (j == (e >> 5)) key[j] = 0u;
+    }
   }
-  const float z0 = __shfl_sync(0xffffffffu, my_z, 0);
+  __syncwarp();
+  const float z0 = w_out[0];
+  const float ex = lane < k ? expf(w_out[lane] - z0) : 0.f;
   float den = 0.f;
-  for (int j = 0; j < k; ++j) den += expf(__shfl_sync(0xffffffffu, my_z, j) - z0);   // fixed order
-  if (lane < k) w_out[lane] = expf(my_z - z0) / den;
+  for (int j = 0; j < k; ++j) den += __shfl_sync(0xffffffffu, ex, j);   // fixed order
+  __syncwarp();
+  if (lane < k) w_out[lane] = ex / den;
+}
+
+// The same selection by a whole thread block (the fused decode kernel: 256 threads, 1..8 tokens): rank counting, which IS the
+// definition (G7): rank(e) = #{j : z_j > z_e or (z_j == z_e and j < e)} on the same 32-bit keys; the experts of rank < k are
+// the top-k in (z desc, id asc) order.  One pass of independent compares instead of k dependent warp reductions.  The softmax
+// is the same chain as in topk_softmax_warp, so both give the same ids and the same weight bits.
+// zf(t, e) returns the logit; keys: n_tokens * E words of shared scratch; threads tid < nthr synchronise on named barrier `bar`.
+template <typename ZF>
+__device__ __forceinline__ void topk_softmax_block(ZF zf, int n_tokens, int E, int k, int* ids_out, float* w_out, unsigned* keys, int tid,
+                                                   int nthr, int bar) {
+  for (int idx = tid; idx < n_tokens * E; idx += nthr) keys[idx] = topk_key(zf(idx / E, idx % E));
+  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthr) : "memory");
+  for (int idx = tid; idx < n_tokens * E; idx += nthr) {
+    const int t = idx / E, e = idx % E;
+    const unsigned* row = keys + (size_t)t * E;
+    const unsigned me = row[e];
+    int rank = 0;
+    if ((E & 3) == 0 && (((size_t)row) & 15) == 0) {       // all lanes of a token read the same address: shared-memory broadcast
+      const uint4* row4 = reinterpret_cast<const uint4*>(row);
+#pragma unroll 4
+      for (int j4 = 0; j4 < E / 4; ++j4) {
+        const uint4 v = row4[j4];
+        const int j = j4 * 4;
+        rank += (v.x > me) || (v.x == me && j < e);
+        rank += (v.y > me) || (v.y == me && j + 1 < e);
+        rank += (v.z > me) || (v.z == me && j + 2 < e);
+        rank += (v.w > me) || (v.w == me && j + 3 < e);
+      }
+    } else {
+      for (int j = 0; j < E; ++j) rank += (row[j] > me) || (row[j] == me && j < e);
+    }
+    if (rank < k) { ids_out[t * k + rank] = e; w_out[t * k + rank] = topk_key_logit(me); }
+  }
+  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthr) : "memory");
+  float val = 0.f;
+  const bool mine = tid < n_tokens * k;
+  if (mine) {
+    const int t = tid / k;
+    const float z0 = w_out[t * k];
+    float den = 0.f;
+    for (int j = 0; j < k; ++j) den += expf(w_out[t * k + j] - z0);   // fixed order
+    val = expf(w_out[tid] - z0) / den;
+  }
+  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthr) : "memory");
+  if (mine) w_out[tid] = val;
 }
 
 // Prefill / multi-kernel path: one warp per token, 4 tokens per block of 128 threads; z [n_tokens][E] in global memory.

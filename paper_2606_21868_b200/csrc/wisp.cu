@@ -321,7 +321,8 @@ struct DecodeSmem { int n_slots, xs_pitch, pre_off, ring_off; size_t bytes; };
 int decode_smem(wisp_ctx* ctx, const DecodeGeom& g, int T_, size_t avail, bool fused, DecodeSmem* out) {
   out->xs_pitch = g.d + g.kc;
   out->pre_off = (int)(((size_t)T_ * out->xs_pitch * g.elem + 127) & ~(size_t)127);
-  const size_t pre = fused ? (((size_t)kSliceCols * ctx->cfg.n_experts * g.elem + 127) & ~(size_t)127) : 0;
+  const size_t pre = fused ? (((size_t)ctx->cfg.n_experts * sizeof(float) + 127) & ~(size_t)127) +
+                                 (((size_t)kSliceCols * ctx->cfg.n_experts * g.elem + 127) & ~(size_t)127) : 0;
   out->ring_off = out->pre_off + (int)pre;
   if ((size_t)out->ring_off + 2 * (size_t)g.part_bytes > avail) return fail(ctx, WISP_EINVAL, "decode kernel: shared memory too small for this shape");
   int n = (int)std::min<size_t>(kDecMaxSlots, (avail - out->ring_off) / g.part_bytes);
