@@ -59,8 +59,15 @@ typedef enum { WISP_LRU = 0, WISP_LFU = 1 } wisp_policy;
  * reads the mapped pinned master (no host round trip; the whole call is stream-ordered); FUSED = no separate
  * copy step in decode: the FFN kernels' TMA producer reads a missing expert's tiles straight from the mapped
  * pinned master, computes on them and writes them into the victim slot (same bytes, same summation order as
- * a hit, so outputs stay byte-identical).  Prefill calls (n_tokens > 8) under FUSED use the ZEROCOPY kernel. */
-typedef enum { WISP_FETCH_MEMCPY = 0, WISP_FETCH_ZEROCOPY = 1, WISP_FETCH_FUSED = 2 } wisp_fetch;
+ * a hit, so outputs stay byte-identical).  Prefill calls (n_tokens > 8) under FUSED use the ZEROCOPY kernel.
+ * STATIC is not a miss path of the method but its COMPARISON ARM: static layer-level offload, "which
+ * streams the whole expert layer" (Table 2).  No per-expert residency: the budget holds
+ * floor(B / (E*M_e)) - 2 whole layers resident plus a two-layer bounce region; every forward copies ALL E experts of every other
+ * layer from the pinned master into the bounce region again (cudaMemcpyAsync on the copy stream, the copy of layer l+1
+ * overlapping the compute of layer l inside wisp_stack_forward), then runs the same FFN kernels on it.  Decode-sized calls only
+ * (n_tokens <= 8); wisp_set_split, the trace and the pool checks do not apply (ESTATE).  wisp_stats reports the streamed bytes
+ * in total.bytes_fetched. */
+typedef enum { WISP_FETCH_MEMCPY = 0, WISP_FETCH_ZEROCOPY = 1, WISP_FETCH_FUSED = 2, WISP_FETCH_STATIC = 3 } wisp_fetch;
 /* Order in which an overflowing step (|R| > C) is cut into waves of at most C experts (PAPER.md:112 leaves overflow
  * handling to the implementation; G5 / G25).  ASCENDING (default) = ascending expert id.  HITS_FIRST = the
  * members of R resident when the step begins (ascending id) come first, then the faults (ascending id): a resident

@@ -160,3 +160,14 @@ class PagerLayer:
             else:
                 assert self.tau[s] == 0
         assert len(set(self.pi.values())) == len(self.pi)
+
+
+# -- static layer-level offload: the paper's comparison arm (Table 2) --------------
+def static_offload_bytes_per_forward(n_layers: int, n_experts: int, expert_bytes: int, budget_bytes: int) -> int:
+    """Bytes a static layer-offload engine moves over the host link for ONE forward of the stack: it "streams the whole
+    expert layer" for every layer the budget does not hold, whatever the routing.  Reading (G26):
+    the budget holds whole layers of E * M_e bytes, two of them are bounce buffers (layer l+1 streams while layer l
+    computes), the first floor(B / (E * M_e)) - 2 layers stay resident."""
+    layer_bytes = n_experts * expert_bytes
+    resident = max(0, min(n_layers, budget_bytes // layer_bytes - 2))
+    return (n_layers - resident) * layer_bytes

@@ -10,7 +10,7 @@ _LIB = None
 
 WISP_F32, WISP_BF16 = 0, 1
 WISP_LRU, WISP_LFU = 0, 1
-WISP_FETCH_MEMCPY, WISP_FETCH_ZEROCOPY, WISP_FETCH_FUSED = 0, 1, 2
+WISP_FETCH_MEMCPY, WISP_FETCH_ZEROCOPY, WISP_FETCH_FUSED, WISP_FETCH_STATIC = 0, 1, 2, 3
 WISP_WAVES_ASCENDING, WISP_WAVES_HITS_FIRST = 0, 1
 KERNEL_CLASSES = ("router", "topk", "residency", "fetch", "ffn", "ffn_miss", "combine", "prefill_gate_up",
                   "prefill_down", "other")

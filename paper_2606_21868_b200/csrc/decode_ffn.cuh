@@ -63,10 +63,11 @@ struct DecodeGeom {
 };
 
 struct DecodeFfnArgs {
-  const char* pool;       // arena base; slot s of layer l at ((size_t)s * L + l) * blob_bytes
+  const char* layer_base; // slot s of this layer at layer_base + s * slot_stride.  Paged pool: arena + layer * M_e with stride L * M_e
+  unsigned long long slot_stride;   //   (slot-major arena); static-offload arm: the layer's own region with stride M_e
   const char* master;     // mapped pinned master of this layer (fused miss path) or nullptr
   unsigned long long blob_bytes;
-  int L, layer, k;
+  int k;
   float inv_k;            // 1.0f / k (token of pair p = floor((p + 0.5) / k), exact for p < 256)
   float* partial;         // P [pair position][NC][d] fp32
   unsigned* ticket;       // unit ticket counter of this wave (zero when the wave starts)
@@ -160,7 +161,7 @@ __device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const Dec
   auto blob_of = [&](int q) {
     const bool from_host = a.master != nullptr && plan.entry_miss[q] != 0;
     return from_host ? a.master + (size_t)plan.entry_expert[q] * a.blob_bytes
-                     : a.pool + ((size_t)plan.entry_slot[q] * a.L + a.layer) * a.blob_bytes;
+                     : a.layer_base + (size_t)plan.entry_slot[q] * a.slot_stride;
   };
   auto emit_down = [&](int q, int c) -> bool {
     const char* blob = blob_of(q);
@@ -260,7 +261,7 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
     const int pos0 = plan.exp_offset[e];
     const int* pl = plan.pair_list + pos0;
     const bool fill = a.master != nullptr && plan.entry_miss[q] != 0;
-    char* slot_blob = const_cast<char*>(a.pool) + ((size_t)plan.entry_slot[q] * a.L + a.layer) * a.blob_bytes;
+    char* slot_blob = const_cast<char*>(a.layer_base) + (size_t)plan.entry_slot[q] * a.slot_stride;
     // on a miss, warp 0 stores the landed part into the victim slot before the ring slot is handed back
     auto store_part = [&](const DecPart& pt) {
       if (fill && warp == 0 && lane == 0) {

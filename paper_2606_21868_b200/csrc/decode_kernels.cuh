@@ -138,7 +138,8 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
   const int E = a.E, k = a.k, d = a.d, T_ = a.T, C = a.C;
   const PlanPtrs pp = plan_ptrs_of(ds.pl);
   DecodeFfnArgs fa{};
-  fa.pool = a.pool; fa.blob_bytes = a.blob_bytes; fa.L = a.L; fa.k = k; fa.inv_k = 1.0f / (float)k; fa.partial = a.partial;
+  fa.slot_stride = (unsigned long long)a.L * a.blob_bytes; fa.blob_bytes = a.blob_bytes; fa.k = k; fa.inv_k = 1.0f / (float)k;
+  fa.partial = a.partial;
 
   if (warp == kDecWarps + 1) {                           // ===================== reducer warp =====================
     decode_reduce<T>(g, fs, lane);
@@ -150,7 +151,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     const uint64_t pol = l2_evict_first_policy();
     unsigned qseq = 0;                                   // waves started so far (all layers)
     for (int l = a.layer_lo; l < a.layer_hi; ++l) {
-      fa.layer = l;
+      fa.layer_base = a.pool + (size_t)l * a.blob_bytes;
       fa.master = a.masters[l];
       int n_waves = 1;
       for (int w = 0; w < n_waves; ++w, ++qseq) {
@@ -291,7 +292,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     if (timing) a.phase_ns[kDecPhases + miss_cls] += 1;
 
     // ---- ffn, wave by wave ----
-    fa.layer = l;
+    fa.layer_base = a.pool + (size_t)l * a.blob_bytes;
     fa.master = a.masters[l];
     for (int w = 0; w < n_waves; ++w, ++qseq) {
       if (w > 0) {

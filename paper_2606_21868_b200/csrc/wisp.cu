@@ -92,6 +92,14 @@ struct wisp_ctx {
   u64* phase_ns = nullptr;           // device [kDecPhases + 2]
   size_t fused_smem = 0, ffn_smem = 0;   // dynamic shared memory available to the fused / split ffn kernel on this device
   int persist_enabled = 1;
+  // static layer-offload comparison arm (WISP_FETCH_STATIC): resident layers [0, static_pinned) at arena + l*E*M_e, then a
+  // two-layer bounce region; every other layer is streamed from its master on every forward
+  int static_pinned = 0;
+  char* bounce[2] = {nullptr, nullptr};
+  cudaEvent_t ev_buf_free[2] = {nullptr, nullptr}, ev_buf_ready[2] = {nullptr, nullptr};
+  bool buf_used[2] = {false, false};
+  u64 static_streamed = 0;         // bytes copied into the bounce region so far
+  bool is_static() const { return cfg.fetch == WISP_FETCH_STATIC; }
   // tcgen05 prefill path (ffn_prefill_mma.cuh): TMA tensor maps over the arena / the B-operand buffers
   bool mma_ok = false;
   CUtensorMap tm_gu{}, tm_dn{}, tm_xg{}, tm_act{}, tm_rw{};
@@ -381,7 +389,8 @@ int launch_fused_any(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void*
 // Split form of one decode layer (MEMCPY / ZEROCOPY contexts, E > 256): logits, plan, per wave (fetch, ffn), combine -- the
 // same device functions as the fused kernel, so both give the same bits.  x_next != nullptr: residual successor instead of y.
 template <typename T>
-int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
+int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st,
+                         const char* slot_base = nullptr) {
   const auto& cfg = ctx->cfg;
   const int k = cfg.top_k, E = cfg.n_experts, d = cfg.d_model, L = cfg.n_layers;
   const int n_pairs = T_ * k, n_slices = T_ * (d / kSliceCols);
@@ -417,11 +426,13 @@ int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* 
   int rc = decode_smem(ctx, g, T_, ctx->ffn_smem, false, &sm);
   if (rc) return rc;
   DecodeFfnArgs fa{};
-  fa.pool = ctx->arena; fa.blob_bytes = ctx->Me; fa.L = L; fa.layer = layer; fa.k = k; fa.partial = ctx->partial;
+  fa.layer_base = slot_base ? slot_base : ctx->arena + (size_t)layer * ctx->Me;
+  fa.slot_stride = slot_base ? ctx->Me : (u64)L * ctx->Me;
+  fa.blob_bytes = ctx->Me; fa.k = k; fa.partial = ctx->partial;
   fa.master = cfg.fetch == WISP_FETCH_FUSED ? static_cast<const char*>(ctx->master[layer]) : nullptr;
   fa.ticket = ctx->dsync + 1;
   for (int w = 0; w < n_waves; ++w) {
-    if (cfg.fetch != WISP_FETCH_FUSED) {
+    if (cfg.fetch != WISP_FETCH_FUSED && cfg.fetch != WISP_FETCH_STATIC) {
       rc = fetch_wave(ctx, layer, w, memcpy_path, st);
       if (rc) return rc;
     }
@@ -589,6 +600,42 @@ int forward_layer_any(wisp_ctx* ctx, int layer, const void* x, int T_, void* out
              : forward_layer_prefill<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st);
 }
 
+// ---- static layer-offload arm (comparison) --------------------------------------------------------
+// Copy of all E experts of `layer` into bounce buffer `layer & 1` on the copy stream, after the compute that last used the
+// buffer.  No residency cache: a streamed layer is copied again on every forward.
+int static_issue_copy(wisp_ctx* ctx, int layer) {
+  const int b = layer & 1;
+  const u64 layer_bytes = (u64)ctx->cfg.n_experts * ctx->Me;
+  if (ctx->buf_used[b]) CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_buf_free[b], 0));
+  CK(cudaMemcpyAsync(ctx->bounce[b], ctx->master[layer], layer_bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+  CK(cudaEventRecord(ctx->ev_buf_ready[b], ctx->copy_stream));
+  ctx->static_streamed += layer_bytes;
+  return WISP_OK;
+}
+
+// One layer of the static arm on stream st.  copy_issued: the caller already queued this layer's copy (stack helper, which
+// streams layer l+1 while layer l computes).
+int forward_layer_static(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st, bool copy_issued) {
+  const bool resident = layer < ctx->static_pinned;
+  const int b = layer & 1;
+  const char* base = resident ? ctx->arena + (u64)layer * ctx->cfg.n_experts * ctx->Me : ctx->bounce[b];
+  if (!resident) {
+    if (!copy_issued) {
+      int rc = static_issue_copy(ctx, layer);
+      if (rc) return rc;
+    }
+    CK(cudaStreamWaitEvent(st, ctx->ev_buf_ready[b], 0));
+  }
+  int rc = ctx->cfg.dtype == WISP_F32 ? forward_layer_decode<float>(ctx, layer, x, T_, out, x_next, st, base)
+                                      : forward_layer_decode<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st, base);
+  if (rc) return rc;
+  if (!resident) {
+    CK(cudaEventRecord(ctx->ev_buf_free[b], st));
+    ctx->buf_used[b] = true;
+  }
+  return WISP_OK;
+}
+
 int check_forward_args(wisp_ctx* ctx, int layer_lo, int layer_hi, const void* hidden, int n_tokens, void* out) {
   if (!ctx) return WISP_EINVAL;
   if (n_tokens < 0 || n_tokens > ctx->cfg.max_tokens) return fail(ctx, WISP_EINVAL, "n_tokens out of range");
@@ -664,7 +711,8 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
       cfg->top_k > kMaxTopK || cfg->top_k > cfg->n_experts || cfg->d_model < 256 || cfg->d_model % 256 ||
       cfg->d_ff < 256 || cfg->d_ff % 256 || cfg->max_tokens < 1 ||
       (cfg->dtype != WISP_F32 && cfg->dtype != WISP_BF16) || (cfg->policy != WISP_LRU && cfg->policy != WISP_LFU) ||
-      (cfg->fetch != WISP_FETCH_MEMCPY && cfg->fetch != WISP_FETCH_ZEROCOPY && cfg->fetch != WISP_FETCH_FUSED) ||
+      (cfg->fetch != WISP_FETCH_MEMCPY && cfg->fetch != WISP_FETCH_ZEROCOPY && cfg->fetch != WISP_FETCH_FUSED &&
+       cfg->fetch != WISP_FETCH_STATIC) ||
       cfg->ring_stages < 0 || cfg->ring_stages > kDecMaxSlots || cfg->unit_rows < 0 || cfg->unit_rows % 8 ||
       (cfg->unit_rows > 0 && (cfg->d_ff % cfg->unit_rows || (cfg->d_ff / cfg->unit_rows) % 8)))
     return WISP_EINVAL;
@@ -684,6 +732,16 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
     return WISP_EBUDGET;
   }
   ctx->C = (int)std::min<u64>(cfg->n_experts, (budget_bytes - kv0) / ctx->a_bytes);
+  if (cfg->fetch == WISP_FETCH_STATIC) {
+    // whole layers: floor(B / (E*M_e)) - 2 resident, 2 as bounce buffers; every expert of a layer is "resident" while it runs
+    const u64 layer_bytes = (u64)cfg->n_experts * ctx->Me;
+    if (kv0 != 0 || budget_bytes / layer_bytes < 2 || cfg->max_tokens > kDecodeMaxTokens) {
+      delete ctx;
+      return cfg->max_tokens > kDecodeMaxTokens ? WISP_EINVAL : WISP_EBUDGET;
+    }
+    ctx->static_pinned = (int)std::min<u64>(cfg->n_layers, budget_bytes / layer_bytes - 2);
+    ctx->C = cfg->n_experts;
+  }
   ctx->kappa = b ? (budget_bytes - (u64)ctx->C * ctx->a_bytes) / b : 0;
   const int L = cfg->n_layers, E = cfg->n_experts, k = cfg->top_k, d = cfg->d_model, dff = cfg->d_ff;
   const size_t maxT = cfg->max_tokens;
@@ -789,6 +847,19 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
     ctx->ffn_smem = (227u << 10) - fa.sharedSizeBytes;
     CKC(cudaFuncSetAttribute(kn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->ffn_smem));
   }
+  if (ctx->is_static()) {
+    // pi = pi^-1 = identity: slot e of a layer's region holds expert e
+    std::vector<int> ident((size_t)L * E);
+    for (size_t i = 0; i < ident.size(); ++i) ident[i] = (int)(i % E);
+    CKC(cudaMemcpy(ctx->pi, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice));
+    CKC(cudaMemcpy(ctx->pi_inv, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice));
+    const u64 layer_bytes = (u64)E * ctx->Me;
+    for (int b = 0; b < 2; ++b) {
+      ctx->bounce[b] = ctx->arena + ((u64)ctx->static_pinned + b) * layer_bytes;
+      CKC(cudaEventCreateWithFlags(&ctx->ev_buf_free[b], cudaEventDisableTiming));
+      CKC(cudaEventCreateWithFlags(&ctx->ev_buf_ready[b], cudaEventDisableTiming));
+    }
+  }
   CKC(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
   CKC(cudaEventCreateWithFlags(&ctx->ev_plan, cudaEventDisableTiming));
   CKC(cudaEventCreateWithFlags(&ctx->ev_compute, cudaEventDisableTiming));
@@ -821,7 +892,8 @@ int wisp_destroy(wisp_ctx* ctx) {
   if (ctx->host_plan) cudaFreeHost(ctx->host_plan);
   if (ctx->host_err) cudaFreeHost(ctx->host_err);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
-  for (cudaEvent_t e : {ctx->ev_plan, ctx->ev_compute, ctx->ev_copy})
+  for (cudaEvent_t e : {ctx->ev_plan, ctx->ev_compute, ctx->ev_copy, ctx->ev_buf_free[0], ctx->ev_buf_free[1], ctx->ev_buf_ready[0],
+                        ctx->ev_buf_ready[1]})
     if (e) cudaEventDestroy(e);
   for (auto& p : ctx->timing_pool) {
     cudaEventDestroy(p.a);
@@ -852,6 +924,8 @@ int wisp_register_host_experts(wisp_ctx* ctx, int32_t layer, const void* experts
   }
   if (router_bias) CK(cudaMemcpy(ctx->router_bias + (size_t)layer * E, router_bias, E * sizeof(float), cudaMemcpyHostToDevice));
   else CK(cudaMemset(ctx->router_bias + (size_t)layer * E, 0, E * sizeof(float)));
+  if (ctx->is_static() && layer < ctx->static_pinned)
+    CK(cudaMemcpy(ctx->arena + (u64)layer * E * ctx->Me, m, E * ctx->Me, cudaMemcpyHostToDevice));
   ctx->registered[layer] = 1;
   return WISP_OK;
 }
@@ -861,6 +935,7 @@ int wisp_moe_forward(wisp_ctx* ctx, int32_t layer, const void* hidden, int32_t n
   if (rc) return rc;
   if (n_tokens == 0) return WISP_OK;
   if ((rc = check_dev_err(ctx))) return rc;
+  if (ctx->is_static()) return forward_layer_static(ctx, layer, hidden, n_tokens, out, nullptr, static_cast<cudaStream_t>(cuda_stream), false);
   if (ctx->use_fused(n_tokens))
     return launch_fused_any(ctx, layer, layer + 1, hidden, n_tokens, out, false, static_cast<cudaStream_t>(cuda_stream));
   return forward_layer_any(ctx, layer, hidden, n_tokens, out, nullptr, static_cast<cudaStream_t>(cuda_stream));
@@ -874,6 +949,20 @@ int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void
   const int L = ctx->cfg.n_layers;
   if ((rc = check_dev_err(ctx))) return rc;
   if (ctx->use_fused(n_tokens)) return launch_fused_any(ctx, 0, L, hidden, n_tokens, hidden_out, true, st);
+  if (ctx->is_static()) {
+    // layer l+1 streams while layer l computes: its copy is queued before layer l's kernels
+    const size_t xb = (size_t)n_tokens * ctx->cfg.d_model * ctx->elem;
+    CK(cudaMemcpyAsync(ctx->xbuf[0], hidden, xb, cudaMemcpyDeviceToDevice, st));
+    int next_streamed = ctx->static_pinned;                          // first layer that needs a copy
+    if (next_streamed < L) { rc = static_issue_copy(ctx, next_streamed); if (rc) return rc; }
+    for (int l = 0; l < L; ++l) {
+      if (l >= ctx->static_pinned && l + 1 < L) { rc = static_issue_copy(ctx, l + 1); if (rc) return rc; }
+      rc = forward_layer_static(ctx, l, ctx->xbuf[l & 1], n_tokens, ctx->ybuf, ctx->xbuf[(l + 1) & 1], st, true);
+      if (rc) return rc;
+    }
+    CK(cudaMemcpyAsync(hidden_out, ctx->xbuf[L & 1], xb, cudaMemcpyDeviceToDevice, st));
+    return WISP_OK;
+  }
   const size_t bytes = (size_t)n_tokens * ctx->cfg.d_model * ctx->elem;
   CK(cudaMemcpyAsync(ctx->xbuf[0], hidden, bytes, cudaMemcpyDeviceToDevice, st));
   auto chain = [&](cudaStream_t s) -> int {
@@ -930,6 +1019,7 @@ int wisp_residual_add(wisp_ctx* ctx, const void* x, const void* y, void* out, in
 
 int wisp_set_split(wisp_ctx* ctx, uint64_t expert_bytes, uint64_t kv_bytes) {
   if (!ctx) return WISP_EINVAL;
+  if (ctx->is_static()) return fail(ctx, WISP_ESTATE, "static layer-offload arm: no expert/KV split to move");
   const u64 b = ctx->cfg.kv_block_bytes;
   const u64 Cn64 = std::min<u64>(ctx->cfg.n_experts, expert_bytes / ctx->a_bytes);
   const u64 kap = b ? kv_bytes / b : 0;
@@ -993,7 +1083,7 @@ int wisp_stats(wisp_ctx* ctx, wisp_stats_t* out) {
     out->total.steps += s[l * 8 + 1]; out->total.hits += s[l * 8 + 2]; out->total.misses += s[l * 8 + 3];
     out->total.evictions += s[l * 8 + 4]; out->total.references += s[l * 8 + 5];
   }
-  out->total.bytes_fetched = out->total.misses * ctx->Me;
+  out->total.bytes_fetched = ctx->is_static() ? ctx->static_streamed : out->total.misses * ctx->Me;
   u64 tc[2];
   CK(cudaMemcpy(tc, ctx->trace_ctr, sizeof(tc), cudaMemcpyDeviceToHost));
   harvest_timing(ctx, true);
@@ -1084,6 +1174,7 @@ int wisp_last_logits(wisp_ctx* ctx, float* z, int32_t n_tokens) {
 int wisp_debug_step_routing(wisp_ctx* ctx, int32_t layer, const int32_t* ids, int32_t n_ids) {
   if (!ctx || layer < 0 || layer >= ctx->cfg.n_layers || n_ids < 0 || (n_ids && !ids)) return fail(ctx, WISP_EINVAL, "bad argument");
   if (!ctx->registered[layer]) return fail(ctx, WISP_ESTATE, "layer not registered");
+  if (ctx->is_static()) return fail(ctx, WISP_ESTATE, "static layer-offload arm: no pager to drive");
   if (n_ids == 0) return WISP_OK;
   for (int i = 0; i < n_ids; ++i)
     if (ids[i] < 0 || ids[i] >= ctx->cfg.n_experts) return fail(ctx, WISP_EINVAL, "expert id out of range");
@@ -1117,8 +1208,11 @@ int wisp_debug_reset_pool(wisp_ctx* ctx) {
   if (!ctx) return WISP_EINVAL;
   CK(cudaDeviceSynchronize());
   const size_t L = ctx->cfg.n_layers, E = ctx->cfg.n_experts;
-  CK(cudaMemset(ctx->pi, 0xff, L * E * sizeof(int)));
-  CK(cudaMemset(ctx->pi_inv, 0xff, L * E * sizeof(int)));
+  if (!ctx->is_static()) {                                  // (the static arm's maps are the identity and stay)
+    CK(cudaMemset(ctx->pi, 0xff, L * E * sizeof(int)));
+    CK(cudaMemset(ctx->pi_inv, 0xff, L * E * sizeof(int)));
+  }
+  ctx->static_streamed = 0;
   CK(cudaMemset(ctx->tau, 0, L * E * sizeof(u64)));
   CK(cudaMemset(ctx->freq, 0, L * E * sizeof(u64)));
   CK(cudaMemset(ctx->scal, 0, L * 8 * sizeof(u64)));
@@ -1139,7 +1233,8 @@ int wisp_debug_ffn_launch(wisp_ctx* ctx, int32_t layer, const void* hidden, int3
   int rc = decode_smem(ctx, g, n_tokens, ctx->ffn_smem, false, &sm);
   if (rc) return rc;
   DecodeFfnArgs fa{};
-  fa.pool = ctx->arena; fa.blob_bytes = ctx->Me; fa.L = ctx->cfg.n_layers; fa.layer = layer; fa.k = ctx->cfg.top_k;
+  fa.layer_base = ctx->arena + (size_t)layer * ctx->Me; fa.slot_stride = (u64)ctx->cfg.n_layers * ctx->Me;
+  fa.blob_bytes = ctx->Me; fa.k = ctx->cfg.top_k;
   fa.partial = ctx->partial; fa.master = nullptr; fa.ticket = ctx->dsync + 1;
   CK(cudaMemsetAsync(ctx->dsync + 1, 0, sizeof(unsigned), st));
   ++ctx->launches;
@@ -1168,6 +1263,7 @@ int wisp_debug_residency(wisp_ctx* ctx, int32_t layer, int32_t* pi_inv, uint64_t
 int wisp_debug_verify_pool(wisp_ctx* ctx, int32_t layer, int32_t* mismatched_slots) {
   if (!ctx || !mismatched_slots || layer < 0 || layer >= ctx->cfg.n_layers) return fail(ctx, WISP_EINVAL, "bad argument");
   if (!ctx->registered[layer]) return fail(ctx, WISP_ESTATE, "layer not registered");
+  if (ctx->is_static()) return fail(ctx, WISP_ESTATE, "static layer-offload arm: no slot pool to verify");
   CK(cudaDeviceSynchronize());
   CK(cudaMemset(ctx->bad_slots, 0, (size_t)ctx->cfg.n_experts * sizeof(int)));
   dim3 g(32, ctx->C);

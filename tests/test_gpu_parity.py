@@ -212,3 +212,33 @@ def test_degenerate_inputs():
     ctx.moe_forward(0, x[:0], out[:0], st)           # n_tokens = 0: no-op, no tick (G23)
     assert ctx.layer_stats(0).steps == before
     ctx.close()
+
+
+@pytest.mark.parametrize("T", [1, 4])
+def test_static_layer_offload_arm(T):
+    """f2: the static layer-offload comparison arm streams whole expert layers and runs the SAME kernels:
+    outputs byte-identical to the paged pool, streamed bytes equal the oracle's byte model."""
+    import paper_2606_21868_b200 as wp
+    from oracle.paging import static_offload_bytes_per_forward
+    shape = si.TINY
+    hidden = si.gen_decode_hidden(shape, 6, T)
+    ctx = make_ctx(shape, 16, max_tokens=T)
+    ref = run_chain(ctx, shape, hidden)
+    ref_stack = run_stack(ctx, shape, hidden)
+    ctx.close()
+    layer_bytes = shape.n_experts * shape.expert_bytes
+    for n_layers_budget in (2, 3, 4):                       # 0, 1, 2 resident layers of 2
+        budget = n_layers_budget * layer_bytes
+        ctx = make_ctx(shape, budget=budget, fetch=wp.WISP_FETCH_STATIC, max_tokens=T, trace=False)
+        assert_same_bytes(ref, run_chain(ctx, shape, hidden))
+        per_fwd = static_offload_bytes_per_forward(shape.n_layers, shape.n_experts, shape.expert_bytes, budget)
+        assert ctx.stats().total.bytes_fetched == per_fwd * hidden.shape[0]
+        got = run_stack(ctx, shape, hidden)
+        assert all(torch.equal(a.view(torch.uint8), b.view(torch.uint8)) for a, b in zip(ref_stack, got))
+        st = ctx.stats()
+        assert st.total.bytes_fetched == 2 * per_fwd * hidden.shape[0] and st.total.misses == 0
+        with pytest.raises(wp.WispError):
+            ctx.set_split(layer_bytes, 0)
+        ctx.close()
+    with pytest.raises(wp.WispError):                       # less than the two bounce buffers
+        make_ctx(shape, budget=layer_bytes, fetch=wp.WISP_FETCH_STATIC, max_tokens=T, trace=False)

@@ -273,3 +273,18 @@ def test_decay_and_miss_curve_two_period_hand_case():
     tot = [a + b for a, b in zip(h, h2)]
     assert tot[1:] == [float(v) for v in g["bins_after"].split()]
     assert mvwsa.miss_curve_from_hist(tot, 2) == [float(g["m0"]), float(g["m1"]), float(g["m2"])]
+
+
+def test_static_offload_byte_model_closed_forms():
+    """f2: the static layer-offload arm's traffic.  Closed forms + the config 2 numbers by hand:
+    E * M_e = 128 * 9 MiB = 1152 MiB per layer; 8 GiB / 1152 MiB = 7 -> 5 resident + 2 bounce -> 43 layers streamed
+    = 43 * 1152 MiB = 48.375 GiB per token (vs 3.375 GiB * (1 - carry-over) for the paged pool, sec4_traffic.txt)."""
+    from oracle.paging import static_offload_bytes_per_forward as f
+    MIB = 1 << 20
+    L, E, Me = 48, 128, 9 * MIB
+    assert f(L, E, Me, 8 << 30) == 43 * 1152 * MIB == int(48.375 * (1 << 30))
+    assert f(L, E, Me, 2 * E * Me) == L * E * Me                     # two bounce buffers only: everything streams
+    assert f(L, E, Me, (L + 2) * E * Me) == 0                        # everything fits
+    assert f(L, E, Me, (L + 50) * E * Me) == 0
+    assert f(L, E, Me, 3 * E * Me + 5) == (L - 1) * E * Me
+    assert all(f(L, E, Me, (n + 2) * E * Me) - f(L, E, Me, (n + 3) * E * Me) == E * Me for n in range(L))   # one layer per E*M_e of budget
