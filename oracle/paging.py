@@ -23,7 +23,7 @@ from __future__ import annotations
 
 from dataclasses import dataclass, field
 
-HIT, MISS, RESIZE_DROP, RESIZE_MOVE = 0, 1, 2, 3
+HIT, MISS, RESIZE_DROP, RESIZE_MOVE, PREFETCH = 0, 1, 2, 3, 4
 LRU, LFU = 0, 1
 ASCENDING, HITS_FIRST = 0, 1
 
@@ -57,6 +57,7 @@ class PagerLayer:
     misses: int = 0
     evictions: int = 0
     references: int = 0
+    prefetches: int = 0
 
     def __post_init__(self):
         self.pi_inv = [None] * self.C
@@ -113,6 +114,35 @@ class PagerLayer:
                 else:
                     events.append(Event(step_no, wv, e, self.pi[e], -1, HIT))
         self.steps += 1
+        return events
+
+    # -- speculative prefetch ----------------------------------
+    def prefetch(self, experts) -> list[Event]:
+        """Bring the predicted experts (best first) into the pool BEFORE this layer's next step.  Reading (G27):
+        a resident expert is skipped; each other one takes the next victim in increasing policy key over ALL slots (no member
+        of R protects a slot: the layer is not running; slots filled by this call are not victims again); the slot's tau
+        becomes the current clock c (no tick: a prefetch is not a reference), f is untouched.  At a tight cap this can evict
+        an expert the next step still needs -- the effect the paper reports."""
+        events: list[Event] = []
+        taken = set()
+        for e in experts:
+            e = int(e)
+            if e in self.pi:
+                continue
+            free = [s for s in range(self.C) if s not in taken]
+            if not free:
+                break
+            s = min(free, key=self._victim_key)
+            old = self.pi_inv[s]
+            if old is not None:
+                del self.pi[old]
+                self.evictions += 1
+            self.pi[e] = s
+            self.pi_inv[s] = e
+            self.tau[s] = self.c
+            taken.add(s)
+            self.prefetches += 1
+            events.append(Event(self.steps, 0, e, s, -1 if old is None else old, PREFETCH))
         return events
 
     # -- resize (a7) ---------------------------------------------------------------------------
