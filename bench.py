@@ -63,6 +63,10 @@ def parse():
     ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed arm, each from an empty pool (median and best are reported)")
     ap.add_argument("--unit-rows", type=int, default=0, help="act rows per decode FFN work unit (0 = library default)")
     ap.add_argument("--no-micro", action="store_true", help="skip the m1 (FFN-only replay) and m3 (router/top-k/plan) microbenchmarks")
+    ap.add_argument("--prefetch", type=int, default=0, help="speculative prefetch of N experts per layer by the online co-activation "
+                    "predictor (wisp_set_prefetch; PAPER.md:175-189, App. E); needs --fetch zerocopy")
+    ap.add_argument("--prefetch-gamma", type=float, default=0.5)
+    ap.add_argument("--prefetch-window", type=int, default=1)
     ap.add_argument("--verify", default="", help="full-depth parity run instead of a bench line: comma list of 2,3,4 (BASELINE.json configs)")
     ap.add_argument("--verify-steps", type=int, default=256)
     return ap.parse_args()
@@ -175,6 +179,8 @@ def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=N
                   ring_stages=getattr(args, "ring_stages", 0), unit_rows=getattr(args, "unit_rows", 0))
     if getattr(args, "wave_order", "ascending") == "hits-first":
         ctx.set_wave_order(wp.WISP_WAVES_HITS_FIRST)
+    if getattr(args, "prefetch", 0) > 0 and (fetch or args.fetch) == "zerocopy":
+        ctx.set_prefetch(args.prefetch, args.prefetch_gamma, args.prefetch_window)
     staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
     for l in (register_layers if register_layers is not None else range(shape.n_layers)):
         si.gen_layer_experts(shape, l, gen_device, out=staging)
@@ -769,6 +775,7 @@ def decode_arm(ctx, shape, x_dev, y_dev, stream, args, n_warm, scratch, host_io=
     return {"cold_ms": ev[0].elapsed_time(ev[1]), "warm_ms": ev[2].elapsed_time(ev[3]),
             "misses_cold": int(st1.total.misses - st0.total.misses), "misses_warm": int(st2.total.misses - st1.total.misses),
             "refs_warm": int(st2.total.references - st1.total.references),
+            "prefetches_warm": int(st2.prefetches - st1.prefetches),
             "launches": int(st2.kernel_launches - st1.kernel_launches)}
 
 
@@ -916,7 +923,8 @@ def main_ours(args):
             "vs_baseline": None, "dtype": "bf16" if shape.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": f"{shape.name} decode, batch {B}, {shape.n_layers} layers, E={shape.n_experts}, top-{shape.top_k}, "
                                    f"d={shape.d_model}, d_ff={shape.d_ff}, expert pool {budget / GIB:.3f} GiB -> C={C} slots/layer, "
-                                   f"{args.policy.upper()}, fetch={args.fetch}" + (", waves=hits-first" if args.wave_order == "hits-first" else ""),
+                                   f"{args.policy.upper()}, fetch={args.fetch}" + (", waves=hits-first" if args.wave_order == "hits-first" else "")
+                                   + (f", speculative prefetch {args.prefetch}/layer" if args.prefetch > 0 else ""),
                        "api": "wisp_moe_forward per layer" if args.per_layer_api else ("wisp_stack_forward (one fused cooperative kernel per token)" if fused else
                                "wisp_stack_forward (static layer offload: whole layers streamed by cudaMemcpyAsync, split decode kernels)" if args.fetch == "static"
                                else "wisp_stack_forward (CUDA graph per token)"),
@@ -939,6 +947,9 @@ def main_ours(args):
                       "warm_ms_per_rep": [round(r["warm_ms"], 3) for r in reps]},
             "paging": {"hit_rate": round(1 - misses / max(1, refs), 5), "misses": int(misses), "references": int(refs),
                        "miss_bytes_per_step": misses * shape.expert_bytes / K,
+                       "prefetch": None if args.prefetch <= 0 else {"n_per_layer": args.prefetch, "gamma": args.prefetch_gamma,
+                                                                    "window": args.prefetch_window, "prefetches": r0["prefetches_warm"],
+                                                                    "prefetch_bytes_per_step": r0["prefetches_warm"] * shape.expert_bytes / K},
                        "hbm_bound_tokens_per_s": round(hbm_peak * 1e9 * B / max(1.0, avg_R * shape.n_layers * shape.expert_bytes), 1)},
             "kernels": kern, "setup_s": round(t_setup, 1)}
     ctx.close()

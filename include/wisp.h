@@ -118,6 +118,8 @@ typedef struct {
   uint64_t trace_dropped;        /* events lost because the ring was full */
   uint64_t fetch_ns;             /* event-timed busy time of the miss path (only while wisp_timing_enable >= 1) */
   uint64_t kernel_launches;      /* library kernels launched so far (graph replays count their kernel nodes) */
+  uint64_t prefetches;           /* experts brought in speculatively (wisp_set_prefetch); not counted as misses */
+  uint64_t prefetch_bytes;       /* prefetches * M_e: host-link bytes spent on speculation */
 } wisp_stats_t;
 
 /* Kernel classes of wisp_timing_read.  Decode (n_tokens <= 8): ROUTER = logits + top-k, RESIDENCY = Algorithm 1, FFN = the fused
@@ -128,7 +130,8 @@ enum { WISP_K_ROUTER = 0, WISP_K_TOPK = 1, WISP_K_RESIDENCY = 2, WISP_K_FETCH = 
        WISP_K_COMBINE = 6, WISP_K_PREFILL_GATE_UP = 7, WISP_K_PREFILL_DOWN = 8, WISP_K_OTHER = 9,
        WISP_N_KERNEL_CLASSES = 10 };
 
-/* kind: 0 hit, 1 miss, 2 resize-drop, 3 resize-move (for a move `evicted` carries the source slot).
+/* kind: 0 hit, 1 miss, 2 resize-drop, 3 resize-move (for a move `evicted` carries the source slot), 4 speculative prefetch
+ * (emitted between the events of layer l and those of layer l+1, best-scoring expert first; `step` = the target layer's next step).
  * Events of one wave are emitted in wave order (ascending expert id; under WISP_WAVES_HITS_FIRST an overflowing step
  * lists residents, then faults, each ascending); waves in order; layers/steps in call order. */
 typedef struct {
@@ -220,6 +223,14 @@ int wisp_set_wave_order(wisp_ctx* ctx, int32_t order);
 /* Select the eviction policy (wisp_policy) for all later forwards; tau and f are kept (both are maintained under either
  * policy), so a switch is usually followed by wisp_debug_reset_pool.  Synchronises.  Errors: EINVAL. */
 int wisp_set_policy(wisp_ctx* ctx, int32_t policy);
+/* Speculative expert prefetch driven by the online co-activation predictor of the paper's App. E (Section 4,
+ * PAPER.md:175-189 reports that it LOWERS single-stream decode throughput: the copies compete with demand traffic for the same
+ * link).  After layer l has routed, the n_per_layer best-scoring absent experts of layer l+1 (score s_{l+1}(e') = sum over the
+ * `window` previous layers of gamma^dist * sum_{e in R_l} P(e'|e), tables learned online from an empty start) are copied from the
+ * pinned master on a side stream into the victim slots of layer l+1 (increasing policy key; G27) while layer l's FFN
+ * runs.  Split decode form only: EINVAL unless cfg.fetch == WISP_FETCH_ZEROCOPY, 0 <= n_per_layer <= 32, 1 <= window <= 4,
+ * 0 < gamma <= 1.  n_per_layer = 0 switches it off; the tables are cleared on every call.  Outputs never change.  Synchronises. */
+int wisp_set_prefetch(wisp_ctx* ctx, int32_t n_per_layer, double gamma, int32_t window);
 /* Drain up to `cap` events into host `buf` (oldest first); *n_out = number written.  Synchronises. */
 int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t* n_out);
 /* Routing of the most recent forward of `layer`: host ids [n_tokens, k] (rank order) and w [n_tokens, k].

@@ -33,7 +33,7 @@ class WispStats(C.Structure):
     _fields_ = [("total", WispLayerStats), ("n_layers", C.c_int32), ("slots_per_layer", C.c_int32)] + [
         (n, C.c_uint64) for n in ("budget_bytes", "expert_bytes", "kv_bytes", "kv_blocks", "kv_blocks_reserved",
                                   "kv_blocks_peak", "resize_count", "failed_resize_count", "trace_dropped", "fetch_ns",
-                                  "kernel_launches")]
+                                  "kernel_launches", "prefetches", "prefetch_bytes")]
 
 
 class WispTraceEvent(C.Structure):
@@ -70,6 +70,7 @@ _SIGS = {
     "wisp_trace_enable": (C.c_int, [C.c_void_p, C.c_int32]),
     "wisp_set_wave_order": (C.c_int, [C.c_void_p, C.c_int32]),
     "wisp_set_policy": (C.c_int, [C.c_void_p, C.c_int32]),
+    "wisp_set_prefetch": (C.c_int, [C.c_void_p, C.c_int32, C.c_double, C.c_int32]),
     "wisp_trace_read": (C.c_int, [C.c_void_p, C.POINTER(WispTraceEvent), C.c_uint64, C.POINTER(C.c_uint64)]),
     "wisp_last_topk": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]),
     "wisp_last_logits": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32]),
@@ -173,6 +174,9 @@ class Wisp:
 
     def set_wave_order(self, order):
         self._ck(self.L.wisp_set_wave_order(self.ctx, int(order)), "wisp_set_wave_order")
+
+    def set_prefetch(self, n_per_layer, gamma=0.5, window=1):
+        self._ck(self.L.wisp_set_prefetch(self.ctx, int(n_per_layer), float(gamma), int(window)), "wisp_set_prefetch")
 
     def set_policy(self, policy):
         self._ck(self.L.wisp_set_policy(self.ctx, int(policy)), "wisp_set_policy")

@@ -15,6 +15,7 @@
 #include "ffn_prefill.cuh"
 #include "ffn_prefill_mma.cuh"
 #include "mvwsa.h"
+#include "prefetch.cuh"
 #include "residency.cuh"
 #include "router.cuh"
 
@@ -100,6 +101,14 @@ struct wisp_ctx {
   bool buf_used[2] = {false, false};
   u64 static_streamed = 0;         // bytes copied into the bounce region so far
   bool is_static() const { return cfg.fetch == WISP_FETCH_STATIC; }
+  // speculative prefetch (prefetch.cuh; wisp_set_prefetch)
+  int pf_n = 0, pf_window = 1;
+  double pf_gpow[kMaxWindow + 1] = {};
+  unsigned *pf_A = nullptr, *pf_row = nullptr;
+  int *pf_rlist = nullptr, *pf_rcount = nullptr, *pf_copy = nullptr;   // copy lists [L][1 + 2 * kMaxPrefetch]
+  cudaStream_t pf_stream = nullptr;
+  std::vector<cudaEvent_t> ev_pred, ev_copied;
+  std::vector<char> pf_pending;
   // tcgen05 prefill path (ffn_prefill_mma.cuh): TMA tensor maps over the arena / the B-operand buffers
   bool mma_ok = false;
   CUtensorMap tm_gu{}, tm_dn{}, tm_xg{}, tm_act{}, tm_rw{};
@@ -397,6 +406,10 @@ int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* 
   const size_t off = (size_t)layer * cfg.max_tokens * k;
   const bool memcpy_path = cfg.fetch == WISP_FETCH_MEMCPY;
   const T* wrt = reinterpret_cast<const T*>(ctx->router_wt) + (size_t)layer * d * E;
+  if (ctx->pf_n > 0 && ctx->pf_pending[layer]) {               // speculative copies into this layer's slots come first
+    CK(cudaStreamWaitEvent(st, ctx->ev_copied[layer], 0));
+    ctx->pf_pending[layer] = 0;
+  }
   {
     Span sp(ctx, WISP_K_ROUTER, st);
     decode_logits_kernel<T><<<std::min(n_slices, 4 * ctx->num_sms), 256, 0, st>>>(reinterpret_cast<const T*>(x), wrt, ctx->zfix, T_, E, d);
@@ -413,6 +426,31 @@ int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* 
     else decode_plan_kernel<kPlanThreads><<<1, kPlanThreads, 0, st>>>(a, ctx->zfix, bias, ctx->logits, ctx->ids + off, ctx->topw + off, T_, k);
   }
   CK(cudaGetLastError());
+  if (ctx->pf_n > 0) {
+    // f3: the predictor learns this layer's routing and prefetches for layer + 1 on the side stream while this layer computes
+    PredictArgs pa{};
+    pa.L = L; pa.E = E; pa.C = ctx->C; pa.policy = cfg.policy; pa.layer = layer; pa.window = ctx->pf_window; pa.n_prefetch = ctx->pf_n;
+    for (int i = 0; i <= kMaxWindow; ++i) pa.gpow[i] = ctx->pf_gpow[i];
+    pa.entry_expert = ctx->plan.entry_expert; pa.plan_hdr = ctx->plan.hdr;
+    pa.A = ctx->pf_A; pa.row = ctx->pf_row; pa.rlist = ctx->pf_rlist; pa.rcount = ctx->pf_rcount;
+    pa.st_next = layer_state(ctx, std::min(layer + 1, L - 1));
+    pa.copy_list = ctx->pf_copy + (size_t)layer * (1 + 2 * kMaxPrefetch);
+    pa.trace = ctx->trace; pa.trace_ctr = ctx->trace_ctr; pa.trace_cap = ctx->trace_cap; pa.trace_on = ctx->trace_on;
+    {
+      Span sp(ctx, WISP_K_OTHER, st);
+      predict_prefetch_kernel<<<1, kPredictThreads, 0, st>>>(pa);
+    }
+    if (layer + 1 < L) {
+      CK(cudaEventRecord(ctx->ev_pred[layer], st));
+      CK(cudaStreamWaitEvent(ctx->pf_stream, ctx->ev_pred[layer], 0));
+      prefetch_copy_kernel<<<32, 256, 0, ctx->pf_stream>>>(pa.copy_list, reinterpret_cast<const uint4*>(ctx->master[layer + 1]),
+                                                         reinterpret_cast<uint4*>(ctx->arena), ctx->Me / 16, L, layer + 1);
+      ++ctx->launches;
+      CK(cudaEventRecord(ctx->ev_copied[layer + 1], ctx->pf_stream));
+      ctx->pf_pending[layer + 1] = 1;
+    }
+    CK(cudaGetLastError());
+  }
   int n_waves;
   if (memcpy_path) {
     CK(cudaEventRecord(ctx->ev_plan, st));
@@ -891,6 +929,11 @@ int wisp_destroy(wisp_ctx* ctx) {
     if (p) cudaFree(p);
   if (ctx->host_plan) cudaFreeHost(ctx->host_plan);
   if (ctx->host_err) cudaFreeHost(ctx->host_err);
+  for (void* p : {(void*)ctx->pf_A, (void*)ctx->pf_row, (void*)ctx->pf_rlist, (void*)ctx->pf_rcount, (void*)ctx->pf_copy})
+    if (p) cudaFree(p);
+  if (ctx->pf_stream) cudaStreamDestroy(ctx->pf_stream);
+  for (cudaEvent_t e : ctx->ev_pred) cudaEventDestroy(e);
+  for (cudaEvent_t e : ctx->ev_copied) cudaEventDestroy(e);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   for (cudaEvent_t e : {ctx->ev_plan, ctx->ev_compute, ctx->ev_copy, ctx->ev_buf_free[0], ctx->ev_buf_free[1], ctx->ev_buf_ready[0],
                         ctx->ev_buf_ready[1]})
@@ -972,7 +1015,7 @@ int wisp_stack_forward(wisp_ctx* ctx, const void* hidden, int32_t n_tokens, void
     }
     return WISP_OK;
   };
-  if (ctx->cfg.fetch != WISP_FETCH_MEMCPY && ctx->timing_level == 0 && st != nullptr && n_tokens <= kDecodeMaxTokens) {
+  if (ctx->cfg.fetch != WISP_FETCH_MEMCPY && ctx->timing_level == 0 && st != nullptr && n_tokens <= kDecodeMaxTokens && ctx->pf_n == 0) {
     auto it = ctx->graphs.find(n_tokens);
     if (it == ctx->graphs.end()) {
       cudaGraph_t g = nullptr;
@@ -1100,6 +1143,8 @@ int wisp_stats(wisp_ctx* ctx, wisp_stats_t* out) {
   out->trace_dropped = tc[1];
   out->fetch_ns = (u64)(ctx->class_ms[WISP_K_FETCH] * 1e6);
   out->kernel_launches = ctx->launches;
+  for (int l = 0; l < L; ++l) out->prefetches += s[l * 8 + 7];
+  out->prefetch_bytes = out->prefetches * ctx->Me;
   ctx->kv_peak = ctx->kv_reserved;
   return WISP_OK;
 }
@@ -1128,6 +1173,43 @@ int wisp_set_policy(wisp_ctx* ctx, int32_t policy) {
   CK(cudaDeviceSynchronize());
   ctx->cfg.policy = policy;
   drop_graphs(ctx);   // kernel argument baked into captured graphs
+  return WISP_OK;
+}
+
+int wisp_set_prefetch(wisp_ctx* ctx, int32_t n_per_layer, double gamma, int32_t window) {
+  if (!ctx) return WISP_EINVAL;
+  if (ctx->cfg.fetch != WISP_FETCH_ZEROCOPY || n_per_layer < 0 || n_per_layer > kMaxPrefetch || window < 1 || window > kMaxWindow ||
+      !(gamma > 0.0 && gamma <= 1.0))
+    return fail(ctx, WISP_EINVAL, "wisp_set_prefetch: needs WISP_FETCH_ZEROCOPY, 0 <= n <= 32, 1 <= window <= 4, 0 < gamma <= 1");
+  CK(cudaDeviceSynchronize());
+  const size_t L = ctx->cfg.n_layers, E = ctx->cfg.n_experts;
+  for (void* p : {(void*)ctx->pf_A, (void*)ctx->pf_row, (void*)ctx->pf_rlist, (void*)ctx->pf_rcount, (void*)ctx->pf_copy})
+    if (p) cudaFree(p);
+  ctx->pf_A = ctx->pf_row = nullptr; ctx->pf_rlist = ctx->pf_rcount = ctx->pf_copy = nullptr;
+  ctx->pf_n = 0;
+  drop_graphs(ctx);
+  if (n_per_layer == 0) return WISP_OK;
+  CK(cudaMalloc(&ctx->pf_A, L * window * E * E * sizeof(unsigned)));
+  CK(cudaMalloc(&ctx->pf_row, L * window * E * sizeof(unsigned)));
+  CK(cudaMalloc(&ctx->pf_rlist, L * E * sizeof(int)));
+  CK(cudaMalloc(&ctx->pf_rcount, L * sizeof(int)));
+  CK(cudaMalloc(&ctx->pf_copy, L * (1 + 2 * kMaxPrefetch) * sizeof(int)));
+  CK(cudaMemset(ctx->pf_A, 0, L * window * E * E * sizeof(unsigned)));
+  CK(cudaMemset(ctx->pf_row, 0, L * window * E * sizeof(unsigned)));
+  CK(cudaMemset(ctx->pf_rcount, 0, L * sizeof(int)));
+  CK(cudaMemset(ctx->pf_copy, 0, L * (1 + 2 * kMaxPrefetch) * sizeof(int)));
+  if (!ctx->pf_stream) CK(cudaStreamCreateWithFlags(&ctx->pf_stream, cudaStreamNonBlocking));
+  while (ctx->ev_pred.size() < L) {
+    cudaEvent_t a, b;
+    CK(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+    ctx->ev_pred.push_back(a); ctx->ev_copied.push_back(b);
+  }
+  ctx->pf_pending.assign(L, 0);
+  ctx->pf_gpow[0] = 1.0;
+  for (int i = 1; i <= kMaxWindow; ++i) ctx->pf_gpow[i] = ctx->pf_gpow[i - 1] * gamma;   // running product, as in oracle/predictor.py
+  ctx->pf_window = window;
+  ctx->pf_n = n_per_layer;
   return WISP_OK;
 }
 
@@ -1213,6 +1295,13 @@ int wisp_debug_reset_pool(wisp_ctx* ctx) {
     CK(cudaMemset(ctx->pi_inv, 0xff, L * E * sizeof(int)));
   }
   ctx->static_streamed = 0;
+  if (ctx->pf_n > 0) {                                      // the predictor forgets too: every arm learns from an empty table
+    const size_t W = ctx->pf_window;
+    CK(cudaMemset(ctx->pf_A, 0, L * W * E * E * sizeof(unsigned)));
+    CK(cudaMemset(ctx->pf_row, 0, L * W * E * sizeof(unsigned)));
+    CK(cudaMemset(ctx->pf_rcount, 0, L * sizeof(int)));
+    ctx->pf_pending.assign(L, 0);
+  }
   CK(cudaMemset(ctx->tau, 0, L * E * sizeof(u64)));
   CK(cudaMemset(ctx->freq, 0, L * E * sizeof(u64)));
   CK(cudaMemset(ctx->scal, 0, L * 8 * sizeof(u64)));

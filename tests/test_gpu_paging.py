@@ -6,7 +6,7 @@ import pytest
 import torch
 
 import synth_inputs as si
-from harness import make_ctx, run_chain, sim_trace
+from harness import make_ctx, run_chain, run_stack, sim_trace
 from oracle import mvwsa
 from oracle.paging import PagerLayer
 
@@ -218,4 +218,53 @@ def test_mvwsa_device_histograms_and_proposals():
     assert eb == Cw * a and kb == ((B - Cw * a) // b) * b
     ctx.set_split(eb, kb)
     assert ctx.stats().slots_per_layer == Cw
+    ctx.close()
+
+
+@pytest.mark.parametrize("T,slots,n,window,policy", [(1, 5, 2, 1, 0), (4, 6, 3, 2, 0), (2, 4, 2, 2, 1), (1, 16, 2, 1, 0)])
+def test_speculative_prefetch_trace_and_outputs(T, slots, n, window, policy):
+    """f3 (App. E 402-414): with the online co-activation predictor prefetching n experts per layer, the
+    trace -- demand events AND prefetch events (kind 4) -- equals the oracle pager driven by the oracle predictor on the GPU's
+    ids, and outputs stay byte-identical to the run without prefetch."""
+    import paper_2606_21868_b200 as wp
+    from oracle.paging import PagerLayer
+    from oracle.predictor import CoActivationPredictor
+    shape = si.MoEShape("tiny4", 4, 16, 2, 256, 512, "f32", 1.1)
+    hidden = si.gen_decode_hidden(shape, 24, T, rho=0.5, noise=2.0)      # lively routing: the working set moves every step
+    ctx = make_ctx(shape, slots, max_tokens=T, fetch=wp.WISP_FETCH_ZEROCOPY, policy=policy)
+    ref = run_chain(ctx, shape, hidden)
+    ctx.close()
+    ctx = make_ctx(shape, slots, max_tokens=T, fetch=wp.WISP_FETCH_ZEROCOPY, policy=policy)
+    ctx.set_prefetch(n, 0.5, window)
+    res = run_chain(ctx, shape, hidden)
+    for pa, pb in zip(ref, res):
+        for a, b in zip(pa, pb):
+            assert torch.equal(a["out"].view(torch.uint8), b["out"].view(torch.uint8)) and torch.equal(a["ids"], b["ids"])
+    pagers = [PagerLayer(C=slots, E=shape.n_experts, policy=policy) for _ in range(shape.n_layers)]
+    pred = CoActivationPredictor(shape.n_layers, shape.n_experts, gamma=0.5, window=window)
+    want = []
+    for per in res:
+        pred.begin_pass()
+        for l, rec in enumerate(per):
+            ids = rec["ids"].flatten().tolist()
+            want += [(l, e.step, e.wave, e.expert, e.slot, e.evicted, e.kind) for e in pagers[l].step(ids)]
+            pred.observe(l, ids)
+            if l + 1 < shape.n_layers:
+                picks = pred.predict(l + 1, min(n, slots), resident=pagers[l + 1].pi.keys())
+                want += [(l + 1, e.step, e.wave, e.expert, e.slot, e.evicted, e.kind) for e in pagers[l + 1].prefetch(picks)]
+    got = ctx.trace_read()
+    assert got == want
+    st = ctx.stats()
+    assert st.prefetches == sum(p.prefetches for p in pagers) and st.total.misses == sum(p.misses for p in pagers)
+    assert st.prefetches > 0 or slots >= shape.n_experts
+    for l in range(shape.n_layers):
+        assert ctx.debug_verify_pool(l) == 0
+    # the stack helper takes the same path
+    ctx.debug_reset_pool()
+    ctx.trace_read()
+    fin = run_stack(ctx, shape, hidden)
+    for t in range(hidden.shape[0]):
+        last = res[t][-1]
+        assert torch.equal(fin[t].view(torch.uint8), (last["x"].float() + last["out"].float()).to(shape.torch_dtype).view(torch.uint8))
+    assert ctx.trace_read() == want
     ctx.close()

@@ -44,5 +44,5 @@ def test_no_cpu_fallback():
 def test_struct_sizes_match_header():
     from paper_2606_21868_b200 import binding as b
     assert ctypes.sizeof(b.WispConfig) == 72 and ctypes.sizeof(b.WispTraceEvent) == 32
-    assert ctypes.sizeof(b.WispLayerStats) == 48 and ctypes.sizeof(b.WispStats) == 48 + 8 + 11 * 8
+    assert ctypes.sizeof(b.WispLayerStats) == 48 and ctypes.sizeof(b.WispStats) == 48 + 8 + 13 * 8
     assert ctypes.sizeof(b.WispMvwsaIn) == 64
