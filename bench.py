@@ -168,6 +168,11 @@ def profile_traffic(kernel):
     return None
 
 
+def traffic_of(kernel, same_workload):
+    t = profile_traffic(kernel)
+    return int(t["traffic"]) if (t and same_workload) else None
+
+
 # ---------------------------------------------------------------------------------------------------------
 def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=None, gen_device="cuda"):
     import paper_2606_21868_b200 as wp
@@ -883,6 +888,9 @@ def main_ours(args):
             kern[name] = {"avg_us": round(tot_ms / n * 1e3, 3), "launches": int(n)}
     roof = None
     fused = args.fetch == "fused" and B <= 8 and shape.n_experts <= 256 and not args.per_layer_api
+    # roofline.traffic: the committed ncu capture's dram read + write bytes per launch -- only for the workload it was captured on
+    default_workload = (shape.name.startswith("qwen3") and "STRESS" not in shape.name and B == 1 and shape.n_layers == 48 and abs(budget / GIB - 8.0) < 1e-6
+                        and args.policy == "lru" and args.prefetch == 0)
     if "ffn" in kern:
         # FFN phase (fused kernel: %globaltimer stamps of CTA 0 over layer calls WITHOUT a miss, from the release of the
         # producer to the grid barrier that ends the phase, barrier included; split form: CUDA events around each launch)
@@ -899,7 +907,7 @@ def main_ours(args):
             launch_us = warm_ms / K * 1e3
             ach_l = launch_bytes / (launch_us * 1e-6) / 1e9
             roof = {"bound": "hbm", "kernel": "decode_fused_kernel", "achieved": round(ach_l, 1), "peak": hbm_peak, "unit": "GB/s",
-                    "frac": round(ach_l / hbm_peak, 4), "traffic": None, "traffic_from_profile": profile_traffic("decode_fused_kernel"),
+                    "frac": round(ach_l / hbm_peak, 4), "traffic": traffic_of("decode_fused_kernel", default_workload), "traffic_from_profile": profile_traffic("decode_fused_kernel"),
                     "bytes_per_launch": int(launch_bytes), "avg_launch_us": round(launch_us, 2), "peak_source": peak_how,
                     "frac_of_nominal_8TBs": round(ach_l / 8000.0, 4), "ffn_phases_hit_only": ffn}
         else:
