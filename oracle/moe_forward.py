@@ -8,6 +8,14 @@ softmax over the top-k, SwiGLU experts (readings G7, G8).
 
 Canonical expert blob (one expert, model dtype), row-major out x in:
     [ gate (d_ff x d) | up (d_ff x d) | down (d x d_ff) ]
+
+FP8 block-quantised experts ("The FP8 block-quantized path pages four tensors per expert (the
+weights and their block scales)"; reading G29): the blob is bytes,
+    [ W13 codes (2 d_ff x d) | W2 codes (d x d_ff) | S13 fp32 (2 d_ff/128 x d/128) | S2 fp32 (d/128 x d_ff/128) ]
+with W13 = [gate; up], codes in OCP e4m3 ("e4m3fn": 1 sign, 4 exponent bits of bias 7, 3 mantissa bits, no infinities, 0x7f / 0xff
+NaN), and the weight a code stands for is  W[r, c] = e4m3(code[r, c]) * S[r // 128, c // 128].  The method does not change
+the arithmetic ("without changing kernels, model weights, or quantization"), so the oracle is the same plain
+definition on the dequantised weights (weight-only quantisation: hidden states stay in the model's bf16).
 """
 from __future__ import annotations
 
@@ -46,6 +54,37 @@ def split_expert_blob(blob: torch.Tensor, d: int, d_ff: int):
     return blob[:n].view(d_ff, d), blob[n:2 * n].view(d_ff, d), blob[2 * n:3 * n].view(d, d_ff)
 
 
+FP8_BLOCK = 128
+
+
+def e4m3_value(code: int) -> float:
+    """The real number an OCP e4m3 byte stands for: (-1)^s * 2^(e-7) * (1 + m/8) for e > 0, (-1)^s * 2^-6 * (m/8) for e = 0;
+    s = bit 7, e = bits 6..3, m = bits 2..0; e = 15, m = 7 is NaN (the format has no infinities; largest finite 448)."""
+    s, e, m = (code >> 7) & 1, (code >> 3) & 0xF, code & 7
+    if e == 15 and m == 7:
+        return float("nan")
+    mag = (m / 8.0) * 2.0 ** -6 if e == 0 else (1.0 + m / 8.0) * 2.0 ** (e - 7)
+    return -mag if s else mag
+
+
+_E4M3_TABLE = torch.tensor([e4m3_value(c) for c in range(256)], dtype=F64)
+
+
+def split_expert_blob_fp8(blob: torch.Tensor, d: int, d_ff: int):
+    """Dequantised (G [d_ff, d], U [d_ff, d], D [d, d_ff]) in fp64 of one fp8 expert blob (uint8, layout in the module header)."""
+    n13, n2, B = 2 * d_ff * d, d * d_ff, FP8_BLOCK
+    blob = blob.contiguous()
+    q13 = _E4M3_TABLE[blob[:n13].long()].view(2 * d_ff, d)
+    q2 = _E4M3_TABLE[blob[n13:n13 + n2].long()].view(d, d_ff)
+    ns13 = (2 * d_ff // B) * (d // B)
+    sc = blob[n13 + n2:].clone().view(torch.float32).to(F64)
+    s13 = sc[:ns13].view(2 * d_ff // B, d // B)
+    s2 = sc[ns13:].view(d // B, d_ff // B)
+    w13 = q13 * s13.repeat_interleave(B, dim=0).repeat_interleave(B, dim=1)
+    w2 = q2 * s2.repeat_interleave(B, dim=0).repeat_interleave(B, dim=1)
+    return w13[:d_ff], w13[d_ff:], w2
+
+
 def silu(v: torch.Tensor) -> torch.Tensor:
     """silu(v) = v / (1 + e^{-v})."""
     return v / (1.0 + torch.exp(-v))
@@ -62,7 +101,7 @@ def moe_layer(x: torch.Tensor, experts: torch.Tensor, w_r: torch.Tensor, bias: t
               k: int, d_ff: int, ids: torch.Tensor | None = None, w: torch.Tensor | None = None):
     """O1 + O2 for one layer: out[t] = sum_{i<k} w[t,i] * y_{ids[t,i]}(x[t]), summed in rank order, fp64.
 
-    experts [E, 3*d*d_ff] canonical blobs.  If `ids`/`w` are given the routing is forced (used when a
+    experts [E, 3*d*d_ff] canonical blobs (uint8 [E, M_e]: fp8 block-quantised blobs, dequantised first).  If `ids`/`w` are given the routing is forced (used when a
     near-tie makes two id sets equally correct, G7/G22).  No shared expert, no FFN bias, no
     normalisation, no capacity factor.  Returns (out [T, d] fp64, ids [T, k] int64, w [T, k] fp64, z)."""
     T, d = x.shape
@@ -77,7 +116,7 @@ def moe_layer(x: torch.Tensor, experts: torch.Tensor, w_r: torch.Tensor, bias: t
     for i in range(k):                       # rank order
         for e in torch.unique(ids[:, i]).tolist():
             rows = (ids[:, i] == e).nonzero().flatten()
-            g, u, dn = split_expert_blob(experts[e], d, d_ff)
+            g, u, dn = (split_expert_blob_fp8 if experts.dtype == torch.uint8 else split_expert_blob)(experts[e], d, d_ff)
             out[rows] += w[rows, i:i + 1] * expert_ffn(x[rows], g, u, dn)
     return out, ids, w, z
 

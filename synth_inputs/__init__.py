@@ -13,9 +13,14 @@ Recipe (DESIGN.md "Input recipe"):
     (alpha = 1.1; 0.8 for the Mixtral-shaped config)  -> Zipf-skewed popularity;
   * decode hidden states: AR(1) h_t = 0.9 h_{t-1} + 0.1 xi_t, xi ~ N(0,1), stationary start
     h_{-1} ~ N(0, 0.01/0.19), kept in fp32 and cast when fed; batch streams are independent;
-  * prefill hidden states: i.i.d. N(0,1).
+  * prefill hidden states: i.i.d. N(0,1);
+  * dtype "fp8" ("the FP8 block-quantized path pages four tensors per expert (the weights and
+    their block scales)"): the same N(0, 0.02^2) draws stored the way an FP8 block-quantised checkpoint stores them -- per
+    128 x 128 block of W13 = [gate; up] and of W2 = down, the block's draws are first multiplied by a seeded gain 2^u,
+    u ~ U(-1, 1) (so block scales differ by up to 4x, as they do in real checkpoints), then scale = amax / 448 (fp32) and
+    code = RNE_e4m3(w / scale) (torch's float8_e4m3fn cast).  That is data preparation: both sides read the resulting bytes; hidden states and the router stay bf16.
 Base seed 21868; tensor-kind ids: 1 experts, 2 router W, 3 permutation, 4 hidden stream, 5 prompt
-lengths, 6 prefill tokens.
+lengths, 6 prefill tokens, 7 fp8 block gains.
 """
 from __future__ import annotations
 
@@ -25,7 +30,8 @@ from dataclasses import dataclass, replace
 import torch
 
 BASE_SEED = 21868
-KIND_EXPERTS, KIND_ROUTER, KIND_PERM, KIND_HIDDEN, KIND_PROMPT_LEN, KIND_PREFILL = 1, 2, 3, 4, 5, 6
+FP8_BLOCK = 128          # block-scale granularity of the fp8 expert weights (both dimensions)
+KIND_EXPERTS, KIND_ROUTER, KIND_PERM, KIND_HIDDEN, KIND_PROMPT_LEN, KIND_PREFILL, KIND_FP8_GAIN = 1, 2, 3, 4, 5, 6, 7
 
 _M1 = 0xBF58476D1CE4E5B9
 _M2 = 0x94D049BB133111EB
@@ -104,7 +110,7 @@ class MoEShape:
     top_k: int
     d_model: int
     d_ff: int
-    dtype: str            # "f32" | "bf16"
+    dtype: str            # "f32" | "bf16" | "fp8" (e4m3 expert weights with 128 x 128 fp32 block scales; hidden states / router bf16)
     zipf_alpha: float
     seed: int = BASE_SEED
 
@@ -113,7 +119,7 @@ class MoEShape:
         return torch.float32 if self.dtype == "f32" else torch.bfloat16
 
     @property
-    def elem_bytes(self) -> int:
+    def elem_bytes(self) -> int:            # bytes per hidden-state / router element
         return 4 if self.dtype == "f32" else 2
 
     @property
@@ -121,8 +127,22 @@ class MoEShape:
         return 3 * self.d_model * self.d_ff
 
     @property
+    def scale_elems(self) -> int:           # fp8: fp32 block scales of W13 and W2 (one per 128 x 128 block)
+        return self.expert_elems // (FP8_BLOCK * FP8_BLOCK) if self.dtype == "fp8" else 0
+
+    @property
     def expert_bytes(self) -> int:          # M_e
+        if self.dtype == "fp8":
+            return self.expert_elems + 4 * self.scale_elems
         return self.expert_elems * self.elem_bytes
+
+    @property
+    def blob_dtype(self):                   # element type of the tensor that holds the canonical expert blobs
+        return torch.uint8 if self.dtype == "fp8" else self.torch_dtype
+
+    @property
+    def blob_len(self) -> int:              # elements of blob_dtype per expert
+        return self.expert_bytes if self.dtype == "fp8" else self.expert_elems
 
     @property
     def slot_unit_bytes(self) -> int:       # a = L * M_e
@@ -136,7 +156,8 @@ class MoEShape:
 TINY = MoEShape("tiny", 2, 16, 2, 256, 512, "f32", 1.1)
 QWEN3 = MoEShape("qwen3-30b-a3b-shaped", 48, 128, 8, 2048, 768, "bf16", 1.1)
 MIXTRAL = MoEShape("mixtral-8x7b-shaped", 32, 8, 2, 4096, 14336, "bf16", 0.8)
-SHAPES = {s.name: s for s in (TINY, QWEN3, MIXTRAL)}
+QWEN3_FP8 = replace(QWEN3, name="qwen3-30b-a3b-shaped-fp8", dtype="fp8")       # f4: the quantised variant of the headline shape
+SHAPES = {s.name: s for s in (TINY, QWEN3, MIXTRAL, QWEN3_FP8)}
 
 
 def slots_for_budget(shape: MoEShape, expert_bytes: int) -> int:
@@ -157,11 +178,46 @@ def normal_multi(keys: list[int], n: int, device="cpu") -> torch.Tensor:
     return torch.sqrt(-2.0 * torch.log(u1)) * torch.cos((2.0 * math.pi) * u2)
 
 
+def _block_quantise_fp8(w: torch.Tensor, rows: int, cols: int, keys: list[int]):
+    """[n, rows, cols] fp32 -> (codes uint8 [n, rows, cols], scales fp32 [n, rows/128, cols/128]); data preparation only.
+    keys[i]: counter stream of item i's block gains."""
+    n, B = w.shape[0], FP8_BLOCK
+    nb = (rows // B) * (cols // B)
+    u = torch.stack([(_lsr(_hash_counter(k, nb, w.device), 40).to(torch.float32) + 0.5) * (2.0 ** -24) for k in keys])   # U(0,1)
+    gain = torch.exp2(2.0 * u - 1.0).view(n, rows // B, 1, cols // B, 1)
+    blk = w.view(n, rows // B, B, cols // B, B) * gain
+    scale = blk.abs().amax(dim=(2, 4)) / 448.0
+    scale = torch.where(scale > 0, scale, torch.ones_like(scale))
+    q = (blk / scale[:, :, None, :, None]).to(torch.float8_e4m3fn)
+    return q.view(torch.uint8).reshape(n, rows, cols), scale
+
+
 def gen_layer_experts(shape: MoEShape, layer: int, device="cpu", out: torch.Tensor | None = None,
                       chunk_experts: int | None = None) -> torch.Tensor:
     """Expert blobs of one layer, canonical layout [E, gate(d_ff x d) | up(d_ff x d) | down(d x d_ff)],
-    row-major out x in, in the model dtype.  `out` may be a preallocated (pinned) host tensor."""
+    row-major out x in, in the model dtype.  `out` may be a preallocated (pinned) host tensor.
+
+    dtype "fp8": uint8 blobs [E, expert_bytes] = [ W13 codes (2 d_ff x d) | W2 codes (d x d_ff) | S13 fp32 (2 d_ff/128 x d/128) |
+    S2 fp32 (d/128 x d_ff/128) ], the four tensors of PAPER.md:369."""
     E, n = shape.n_experts, shape.expert_elems
+    if shape.dtype == "fp8":
+        d, f = shape.d_model, shape.d_ff
+        if out is None:
+            out = torch.empty((E, shape.expert_bytes), dtype=torch.uint8)
+        if chunk_experts is None:
+            chunk_experts = max(1, min(E, (1 << 26) // n)) if str(device) != "cpu" else 1
+        for e0 in range(0, E, chunk_experts):
+            e1 = min(E, e0 + chunk_experts)
+            keys = [stream_key(shape.seed, KIND_EXPERTS, layer, e) for e in range(e0, e1)]
+            v = normal_multi(keys, n, device).mul_(0.02)
+            q13, s13 = _block_quantise_fp8(v[:, :2 * d * f].reshape(e1 - e0, 2 * f, d), 2 * f, d,
+                                           [stream_key(shape.seed, KIND_FP8_GAIN, layer, e, 0) for e in range(e0, e1)])
+            q2, s2 = _block_quantise_fp8(v[:, 2 * d * f:].reshape(e1 - e0, d, f), d, f,
+                                         [stream_key(shape.seed, KIND_FP8_GAIN, layer, e, 1) for e in range(e0, e1)])
+            sc = torch.cat([s13.reshape(e1 - e0, -1), s2.reshape(e1 - e0, -1)], dim=1).contiguous()
+            blob = torch.cat([q13.reshape(e1 - e0, -1), q2.reshape(e1 - e0, -1), sc.view(torch.uint8).reshape(e1 - e0, -1)], dim=1)
+            out[e0:e1].copy_(blob)
+        return out
     if out is None:
         out = torch.empty((E, n), dtype=shape.torch_dtype)
     if chunk_experts is None:
@@ -217,7 +273,7 @@ def gen_model(shape: MoEShape, device="cpu", pin: bool = False):
     """All layers: list of expert blobs [E, 3*d*d_ff], list of (W_r, bias).  Host tensors."""
     experts, routers = [], []
     for l in range(shape.n_layers):
-        buf = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=pin)
+        buf = torch.empty((shape.n_experts, shape.blob_len), dtype=shape.blob_dtype, pin_memory=pin)
         experts.append(gen_layer_experts(shape, l, device, out=buf))
         routers.append(gen_router(shape, l))
     return experts, routers
