@@ -52,7 +52,15 @@ typedef enum {
   WISP_EBUDGET = -5   /* split does not fit the budget / floor / reservations */
 } wisp_status;
 
-typedef enum { WISP_F32 = 0, WISP_BF16 = 1 } wisp_dtype;
+/* WISP_FP8_E4M3 ("The FP8 block-quantized path pages four tensors per expert (the weights and
+ * their block scales)"): expert weights are OCP e4m3 codes with one fp32 scale per 128 x 128 block, W[r][c] =
+ * e4m3(code[r][c]) * S[r/128][c/128]; hidden states, outputs and the router are bf16 (weight-only quantisation, G29).
+ * Canonical fp8 blob (bytes), M_e = 3*d*d_ff + 4 * 3*d*d_ff/16384:
+ *   [ W13 codes (2 d_ff x d_model; gate rows, then up rows) | W2 codes (d_model x d_ff) |
+ *     S13 fp32 (2 d_ff/128 x d_model/128) | S2 fp32 (d_model/128 x d_ff/128) ]
+ * Requires d_model a multiple of 1024 and d_ff a multiple of 256.  The products are exact (fp8 x bf16 on the tensor cores after
+ * an exact widening to f16 operands), accumulated in fp32 per 128-wide K block and scaled in fp32. */
+typedef enum { WISP_F32 = 0, WISP_BF16 = 1, WISP_FP8_E4M3 = 2 } wisp_dtype;
 typedef enum { WISP_LRU = 0, WISP_LFU = 1 } wisp_policy;
 /* Miss path (a3): MEMCPY = cudaMemcpyAsync per miss on a dedicated copy stream fenced with events (the
  * host reads the miss list: one host sync per layer call); ZEROCOPY = a device-initiated copy kernel that
@@ -82,7 +90,7 @@ typedef struct {
   int32_t d_model;    /* multiple of 256 */
   int32_t d_ff;       /* multiple of 256 */
   int32_t max_tokens; /* largest n_tokens passed to wisp_moe_forward (sizes staging buffers) */
-  int32_t dtype;      /* wisp_dtype: dtype of weights, hidden and out */
+  int32_t dtype;      /* wisp_dtype: dtype of weights, hidden and out (WISP_FP8_E4M3: fp8 expert weights, bf16 hidden / out / router) */
   int32_t policy;     /* wisp_policy */
   int32_t fetch;      /* wisp_fetch */
   int32_t ring_stages; /* shared-memory ring depth (parts of <= 32 KiB) of the decode FFN kernels, 2..8; 0 = as many as fit */
@@ -173,7 +181,7 @@ int wisp_destroy(wisp_ctx* ctx);
 
 /* Register one layer's full expert set: the "CPU master W^cpu" of Algorithm 1.
  *   experts     host, E canonical blobs, E*M_e bytes, in cfg.dtype.
- *   router_w    host, [E, d_model] row-major in cfg.dtype.
+ *   router_w    host, [E, d_model] row-major in cfg.dtype (bf16 for WISP_FP8_E4M3).
  *   router_bias host, [E] fp32, or NULL (zeros).
  * The library COPIES all three (experts into its own pinned, device-mapped host memory; router into
  * device memory, which is a fixed cost outside B); the caller may free its buffers on return.

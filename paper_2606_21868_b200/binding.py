@@ -8,7 +8,7 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
-WISP_F32, WISP_BF16 = 0, 1
+WISP_F32, WISP_BF16, WISP_FP8_E4M3 = 0, 1, 2
 WISP_LRU, WISP_LFU = 0, 1
 WISP_FETCH_MEMCPY, WISP_FETCH_ZEROCOPY, WISP_FETCH_FUSED, WISP_FETCH_STATIC = 0, 1, 2, 3
 WISP_WAVES_ASCENDING, WISP_WAVES_HITS_FIRST = 0, 1

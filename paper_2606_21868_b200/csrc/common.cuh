@@ -8,6 +8,7 @@
 // is what makes outputs byte-identical across budgets (parity (b)).
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 

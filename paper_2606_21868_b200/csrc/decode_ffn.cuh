@@ -29,6 +29,13 @@
 // ldmatrix, each core matrix being 128 contiguous bytes), so the arithmetic leaves the FMA pipes and the kernel stays a pure
 // HBM stream at 1..8 tokens (1 flop/byte: this is an ALU offload of a memory-bound kernel, not a GEMM -- units of 96 KiB are
 // far too small for tcgen05's 128-row tiles).  fp32 (config 1, parity only): plain FMA, same data flow, same reduction tree.
+// fp8 experts (WISP_FP8_E4M3, f4): the slot holds e4m3 codes in the same 8-row x 16-byte cores (16 K elements per row
+// of a gate/up core; down cores are 8 outputs x 8 act columns = 64 bytes) and the fp32 block scales at the blob's tail; every
+// part carries its slab/128 scales behind its data in the ring slot.  ldmatrix delivers 4 consecutive K codes per lane; since
+// the order of k inside one MMA is free as long as A and B agree, they feed the k slots {2q, 2q+1, 2q+8, 2q+9} of lane
+// quarter q directly -- no shuffles: two exact cvt.f16x2.e4m3x2 per register, the activations (hidden state, a) as f16 scaled
+// by an exact per-token power of two, f16 MMA with fp32 accumulation, one 128-wide K block per accumulator, block sums
+// scaled in fp32 (fmaf) in ascending block order.  Every product is exact; only the fp32 accumulation rounds.
 // Fused miss path (WISP_FETCH_FUSED): the parts of an entry marked as a miss are read from the mapped pinned master
 // (Alg. 1 line 6) and consumer warp 0 stores each landed part into the victim slot with a bulk shared->global
 // copy: same bytes, same order of arithmetic as a hit.
@@ -60,6 +67,12 @@ struct DecodeGeom {
   int down_pieces;       // 8 / kc: bulk copies per down part (the 8 act columns of a sub-block span 8/kc core columns)
   unsigned long long up_off, down_off;    // byte offsets of the up / down matrices inside a blob
   unsigned long long group_bytes;         // 8 * d * elem: one 8-row group of gate/up = the 8 act columns of down
+  // fp8 experts: fp32 block scales at the tail of the blob, S13 [2 d_ff / 128][d / 128] then S2 TRANSPOSED [d_ff / 128][d / 128]
+  int f8;                // 1: e4m3 weights with block scales
+  int act_elem;          // bytes per hidden-state element (2 for fp8 experts)
+  int scale_bytes;       // per part: 4 * slab / 128 (0 without scales)
+  int slot_bytes;        // ring slot = part_bytes + scale_bytes
+  unsigned long long s13_off, s2_off;
 };
 
 struct DecodeFfnArgs {
@@ -103,6 +116,14 @@ __device__ __forceinline__ unsigned long long dec_part_offset(const DecodeGeom& 
   return g.down_off + (grp * g.down_pieces + piece) * (g.group_bytes / g.down_pieces) + (unsigned long long)p.slab * pb;
 }
 
+// Byte offset inside the blob of the block scales of that part (fp8): the slab/128 scales of its K range (gate/up: row block of the
+// 8 rows) or of its output range (down: column block of the 8 act columns; S2 is stored transposed so they are contiguous).
+__device__ __forceinline__ unsigned long long dec_scale_offset(const DecodeGeom& g, int c, const DecPart& p) {
+  const int row0 = (c * g.n_sb + p.sb) * 8;
+  const unsigned long long blk = p.mat < 2 ? (unsigned long long)((p.mat * g.dff + row0) >> 7) : (unsigned long long)(row0 >> 7);
+  return (p.mat < 2 ? g.s13_off : g.s2_off) + 4ull * (blk * (unsigned long long)(g.d >> 7)) + (unsigned long long)p.slab * g.scale_bytes;
+}
+
 // ---- per-CTA dataflow state (shared memory) -----------------------------------------------------------------------
 struct DecFfnShared {
   unsigned long long full[kDecMaxSlots], empty[kDecMaxSlots];
@@ -113,7 +134,12 @@ struct DecFfnShared {
   volatile int final;                    // the consumers have finished the last wave of the launch
   int abort;                             // a grid barrier timed out: everybody leaves
   alignas(16) float red[2][2][kDecWarps * 128];   // gate/up partial tiles; also the combine's scratch between waves
-  alignas(16) float act[2][2][64];       // a[token column][act row] per (unit parity, sub-block), bf16 or fp32
+  alignas(16) float act[2][2][64];       // a[token column][act row] per (unit parity, sub-block), bf16 or fp32 (fp8 experts: scaled f16)
+  // fp8 experts: exact power-of-two scales of the f16 activation operands
+  float xscale[kDecodeMaxTokens];        // hidden state of token t = xh[t] * xscale[t]
+  unsigned xamax[kDecodeMaxTokens];      // scratch of stage_xh
+  float colscale[2][8];                  // [unit parity][MMA column]: xscale of the column's token (written by consumer warp 0)
+  float ascale[2][8];                    // [unit parity][MMA column]: a = act * ascale (written by the reducer)
 };
 
 __device__ __forceinline__ void dec_ffn_shared_init(DecFfnShared& fs, const DecRing& ring) {   // one thread, before a CTA-wide sync
@@ -124,6 +150,54 @@ __device__ __forceinline__ void dec_ffn_shared_init(DecFfnShared& fs, const DecR
   }
   mbar_fence_init();
   fs.units_total = 0; fs.final = 0; fs.abort = 0;
+}
+
+// Exact power-of-two factor that brings a non-negative fp32 maximum into [2^14, 2^15) (f16 range), and its inverse.
+__device__ __forceinline__ void f16_range_scale(float amax, float& mult, float& inv) {
+  const unsigned e = max(15u, (__float_as_uint(amax) >> 23) & 0xffu);
+  mult = __uint_as_float((268u - e) << 23);
+  inv = __uint_as_float((e - 14u) << 23);
+}
+
+// fp8 experts: the f16 copy of the call's hidden states, xh[t] = xs[t] * 2^p_t with the token's largest magnitude brought into
+// [2^14, 2^15) (exact: bf16 has fewer mantissa bits than f16; elements more than 2^29 below the token's maximum round to f16
+// subnormals, an absolute error below 2^-39 of that maximum).  Called by `nthreads` threads that `bar()` synchronises; xs must be
+// complete before the call, and the caller synchronises once more before xh / xscale are read.
+template <typename Bar>
+__device__ __forceinline__ void stage_xh(const __nv_bfloat16* xs, __half* xh, DecFfnShared& fs, int n_tokens, int d, int pitch, int tid,
+                                         int nthreads, Bar bar) {
+  if (tid < kDecodeMaxTokens) fs.xamax[tid] = 0u;
+  bar();
+  const int vec_row = d / 8, n_vec = n_tokens * vec_row;        // a warp's 32 consecutive vectors lie in one token (d % 256 == 0)
+  for (int i0 = 0; i0 < n_vec; i0 += nthreads) {
+    const int i = i0 + tid;
+    unsigned m = 0u;
+    if (i < n_vec) {
+      const uint4 v = *reinterpret_cast<const uint4*>(xs + (size_t)(i / vec_row) * pitch + (i % vec_row) * 8);
+      const unsigned w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) m = max(m, max(w[j] & 0x7fffu, (w[j] >> 16) & 0x7fffu));
+    }
+    m = __reduce_max_sync(0xffffffffu, m);
+    if ((tid & 31) == 0 && i < n_vec) atomicMax(&fs.xamax[i / vec_row], m);
+  }
+  bar();
+  for (int i = tid; i < n_vec; i += nthreads) {
+    const int t = i / vec_row;
+    float mult, inv;
+    f16_range_scale(__uint_as_float(fs.xamax[t] << 16), mult, inv);
+    if (i % vec_row == 0) fs.xscale[t] = inv;
+    const size_t off = (size_t)t * pitch + (i % vec_row) * 8;
+    const uint4 v = *reinterpret_cast<const uint4*>(xs + off);
+    const unsigned w[4] = {v.x, v.y, v.z, v.w};
+    unsigned o[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const __half2 h = __floats2half2_rn(__uint_as_float(w[j] << 16) * mult, __uint_as_float(w[j] & 0xffff0000u) * mult);
+      o[j] = *reinterpret_cast<const unsigned*>(&h);
+    }
+    *reinterpret_cast<uint4*>(xh + off) = make_uint4(o[0], o[1], o[2], o[3]);
+  }
 }
 
 __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
@@ -151,10 +225,11 @@ __device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const Dec
     if (!mbar_wait_or_abort(ring.empty0 + 8u * rp.s, rp.ph ^ 1u, &fs.abort)) return false;
     fs.meta[rp.s] = part_meta(pt.mat, pt.sb, pt.slab, c, q);
     const uint32_t bar = ring.full0 + 8u * rp.s, dst = ring.slot0 + (uint32_t)rp.s * ring.stride;
-    mbar_expect_tx(bar, (uint32_t)g.part_bytes);
+    mbar_expect_tx(bar, (uint32_t)g.slot_bytes);
     const int np = pt.mat == 2 ? g.down_pieces : 1;
     const uint32_t pb = (uint32_t)g.part_bytes / np;
     for (int piece = 0; piece < np; ++piece) bulk_g2s(dst + piece * pb, blob + dec_part_offset(g, c, pt, piece), pb, bar, pol);
+    if (g.scale_bytes) bulk_g2s(dst + (uint32_t)g.part_bytes, blob + dec_scale_offset(g, c, pt), (uint32_t)g.scale_bytes, bar, pol);
     ring_advance(ring, rp);
     return true;
   };
@@ -200,12 +275,13 @@ template <> struct ActT<__nv_bfloat16> { typedef __nv_bfloat16 type; };
 
 // ---- reducer warp: SwiGLU of every unit the consumers push, until the launch is over ------------------------------
 // a[n][r] = silu(sum_w gate_w[r][n]) * (sum_w up_w[r][n]), the 8 warp partials added in ascending warp order.
-template <typename T>
+template <typename T, bool F8>
 __device__ __forceinline__ void decode_reduce(const DecodeGeom& g, DecFfnShared& fs, int lane) {
   typedef typename ActT<T>::type AT;
   const int col = lane >> 2, kq = (lane & 3) * 2;
   for (unsigned i = 0;; ++i) {
     const unsigned par = i & 1u, ph = (i >> 1) & 1u;
+    float av[2][2];                                            // fp8: a of (sub-block, column kq / kq+1) until the unit's scale is known
     for (int sb = 0; sb < g.n_sb; ++sb) {
       const uint32_t bar = smem_u32(&fs.red_full[par][sb]);
       while (!mbar_try_wait(bar, ph))
@@ -219,13 +295,38 @@ __device__ __forceinline__ void decode_reduce(const DecodeGeom& g, DecFfnShared&
       }
       // this lane holds gate (x, y) and up (z, w) of act row lane/4 for the token columns kq, kq+1
       AT* dst = reinterpret_cast<AT*>(fs.act[par][sb]);
-      if constexpr (sizeof(T) == 2) {
+      if constexpr (F8) {
+        // the operands were xh = x / xscale: put the token's power of two back (exact), then a in the model's bf16 (G21)
+        const float c0 = fs.colscale[par][kq], c1 = fs.colscale[par][kq + 1];
+        av[sb & 1][0] = __bfloat162float(__float2bfloat16_rn(silu_f(tot.x * c0) * (tot.z * c0)));
+        av[sb & 1][1] = __bfloat162float(__float2bfloat16_rn(silu_f(tot.y * c1) * (tot.w * c1)));
+      } else if constexpr (sizeof(T) == 2) {
         dst[kq * 8 + col] = __float2bfloat16_rn(silu_f(tot.x) * tot.z);
         dst[(kq + 1) * 8 + col] = __float2bfloat16_rn(silu_f(tot.y) * tot.w);
       } else {
         dst[kq * 8 + col] = silu_f(tot.x) * tot.z;
         dst[(kq + 1) * 8 + col] = silu_f(tot.y) * tot.w;
       }
+    }
+    if constexpr (F8) {
+      // one scale per (unit, token column): the column's largest |a| over the unit's rows -> [2^14, 2^15); a is bf16, so the scaled
+      // f16 operand is exact
+      float m0 = fabsf(av[0][0]), m1 = fabsf(av[0][1]);
+      if (g.n_sb > 1) { m0 = fmaxf(m0, fabsf(av[1][0])); m1 = fmaxf(m1, fabsf(av[1][1])); }
+#pragma unroll
+      for (int o = 4; o < 32; o <<= 1) {
+        m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, o));
+        m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, o));
+      }
+      float mu0, in0, mu1, in1;
+      f16_range_scale(m0, mu0, in0);
+      f16_range_scale(m1, mu1, in1);
+      for (int sb = 0; sb < g.n_sb; ++sb) {
+        __half* dst = reinterpret_cast<__half*>(fs.act[par][sb]);
+        dst[kq * 8 + col] = __float2half_rn(av[sb & 1][0] * mu0);
+        dst[(kq + 1) * 8 + col] = __float2half_rn(av[sb & 1][1] * mu1);
+      }
+      if (col == 0) { fs.ascale[par][kq] = in0; fs.ascale[par][kq + 1] = in1; }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&fs.act_ready[par]));
@@ -235,12 +336,13 @@ __device__ __forceinline__ void decode_reduce(const DecodeGeom& g, DecFfnShared&
 // ---- consumers: the 8 warps (tid 0..255) process the parts the producer queued, until the END marker ---------------
 // xs: the call's hidden states in shared memory, [T][xs_pitch] elements of T (rows padded by 16 bytes).
 // gu_seq / d_seq: units whose gate/up / down this warp has finished so far in the launch (select the parity buffers).
-template <typename T>
+// fp8 experts: xh = the hidden states as f16 scaled per token (stage_xh), same pitch as xs.
+template <typename T, bool F8>
 __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const DecodeGeom& g, const PlanPtrs& plan, DecFfnShared& fs,
                                                const DecRing& ring, DecRingPos& rp, unsigned& gu_seq, unsigned& d_seq, const T* xs,
-                                               int xs_pitch) {
+                                               const __half* xh, int xs_pitch) {
   typedef typename ActT<T>::type AT;
-  constexpr bool kMma = sizeof(T) == 2;
+  constexpr bool kMma = sizeof(T) == 2 && !F8;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int col = lane >> 2, kq = (lane & 3) * 2;             // MMA fragment coordinates of this lane
   while (true) {
@@ -268,6 +370,7 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
         const int np = pt.mat == 2 ? g.down_pieces : 1;
         const uint32_t pb = (uint32_t)g.part_bytes / np, src = ring.slot0 + (uint32_t)rp.s * ring.stride;
         for (int piece = 0; piece < np; ++piece) bulk_s2g(slot_blob + dec_part_offset(g, c, pt, piece), src + piece * pb, pb);
+        if (g.scale_bytes) bulk_s2g(slot_blob + dec_scale_offset(g, c, pt), src + (uint32_t)g.part_bytes, (uint32_t)g.scale_bytes);
         bulk_commit();
       }
     };
@@ -286,8 +389,14 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
       float c4[4][4];
 #pragma unroll
       for (int j = 0; j < 4; ++j) { c4[j][0] = 0.f; c4[j][1] = 0.f; c4[j][2] = 0.f; c4[j][3] = 0.f; }
+      float tot8[4] = {0.f, 0.f, 0.f, 0.f};                    // fp8: the scaled block sums of this warp's K ranges, slabs ascending
       const unsigned par = gu_seq & 1u;
       float* red = fs.red[par][sb] + warp * 128;
+      if constexpr (F8) {
+        // the reducer needs each MMA column's token scale: warp 0 publishes them with the first sub-block
+        if (sb == 0 && warp == 0 && lane < 8)
+          fs.colscale[par][lane] = lane < cnt ? fs.xscale[(int)(((float)pl[lane] + 0.5f) * a.inv_k)] : 0.f;
+      }
       for (int s = 0; s < g.n_slab; ++s) {
       if (s > 0) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
       const uint32_t gbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
@@ -297,7 +406,44 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
       mbar_wait(ring.full0 + 8u * rpu.s, rpu.ph);
       const uint32_t ubase = ring.slot0 + (uint32_t)rpu.s * ring.stride;
       const int k_lo = s * g.slab + warp * (g.slab >> 3);     // this warp's K range of the slab
-      if constexpr (kMma) {
+      if constexpr (F8) {
+        // one core matrix (8 rows x 16 codes) is one k16 step; an ldmatrix.x4 = {gate, up} x two steps; 8 steps = one scale block
+        const int tok = col < cnt ? (int)(((float)pl[col] + 0.5f) * a.inv_k) : -1;
+        const uint32_t abase = ((lane >> 3) & 1 ? ubase : gbase) + (uint32_t)(lane & 7) * 16u + (uint32_t)(lane >> 4) * 128u +
+                               (uint32_t)(warp * g.steps) * 128u;
+        const __half* xrow = xh + (size_t)max(tok, 0) * xs_pitch + k_lo + (lane & 3) * 4;
+        const uint32_t sc = (uint32_t)g.part_bytes + (uint32_t)(warp * (g.steps >> 3)) * 4u;
+#pragma unroll
+        for (int kb = 0; kb < kDecMaxSteps / 8; ++kb) {
+          if (kb * 8 < g.steps) {
+            uint32_t af[4][4];
+            uint2 bf[8];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              ldmatrix_x4(af[j][0], af[j][1], af[j][2], af[j][3], abase + (uint32_t)(kb * 4 + j) * 256u);
+              bf[2 * j] = tok >= 0 ? *reinterpret_cast<const uint2*>(xrow + (kb * 8 + 2 * j) * 16) : make_uint2(0u, 0u);
+              bf[2 * j + 1] = tok >= 0 ? *reinterpret_cast<const uint2*>(xrow + (kb * 8 + 2 * j + 1) * 16) : make_uint2(0u, 0u);
+            }
+            float c8[4][4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { c8[j][0] = 0.f; c8[j][1] = 0.f; c8[j][2] = 0.f; c8[j][3] = 0.f; }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              // registers 0/1: gate / up codes of step 2j; registers 2/3: of step 2j + 1
+              mma_f16_16816(c8[(2 * j) & 3], cvt_e4m3x2_f16x2((uint16_t)af[j][0]), cvt_e4m3x2_f16x2((uint16_t)af[j][1]),
+                            cvt_e4m3x2_f16x2((uint16_t)(af[j][0] >> 16)), cvt_e4m3x2_f16x2((uint16_t)(af[j][1] >> 16)), bf[2 * j].x, bf[2 * j].y);
+              mma_f16_16816(c8[(2 * j + 1) & 3], cvt_e4m3x2_f16x2((uint16_t)af[j][2]), cvt_e4m3x2_f16x2((uint16_t)af[j][3]),
+                            cvt_e4m3x2_f16x2((uint16_t)(af[j][2] >> 16)), cvt_e4m3x2_f16x2((uint16_t)(af[j][3] >> 16)), bf[2 * j + 1].x, bf[2 * j + 1].y);
+            }
+            const float sg = lds_f32(gbase + sc + (uint32_t)kb * 4u), su = lds_f32(ubase + sc + (uint32_t)kb * 4u);
+            tot8[0] = fmaf(sg, (c8[0][0] + c8[1][0]) + (c8[2][0] + c8[3][0]), tot8[0]);
+            tot8[1] = fmaf(sg, (c8[0][1] + c8[1][1]) + (c8[2][1] + c8[3][1]), tot8[1]);
+            tot8[2] = fmaf(su, (c8[0][2] + c8[1][2]) + (c8[2][2] + c8[3][2]), tot8[2]);
+            tot8[3] = fmaf(su, (c8[0][3] + c8[1][3]) + (c8[2][3] + c8[3][3]), tot8[3]);
+          }
+        }
+        if (s == g.n_slab - 1) *reinterpret_cast<float4*>(red + lane * 4) = make_float4(tot8[0], tot8[1], tot8[2], tot8[3]);
+      } else if constexpr (kMma) {
         const int tok = col < cnt ? (int)(((float)pl[col] + 0.5f) * a.inv_k) : -1;   // token of MMA column `col` (-1: operand 0)
         const uint32_t abase = ((lane >> 3) & 1 ? ubase : gbase) + (uint32_t)(lane & 7) * 16u + (uint32_t)(lane >> 4) * 128u +
                                (uint32_t)(warp * g.steps) * 256u;
@@ -358,8 +504,8 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
       const int s = s0;
       const unsigned par = d_seq & 1u;
       if (s == 0) mbar_wait(smem_u32(&fs.act_ready[par]), (d_seq >> 1) & 1u);   // a[] of this unit is published
-      float yacc[kMma ? kDecMaxSteps : 1][4];                  // outputs j of this warp x token columns
-      if constexpr (kMma) {
+      float yacc[(kMma || F8) ? kDecMaxSteps : 1][4];          // outputs j of this warp x token columns
+      if constexpr (kMma || F8) {
 #pragma unroll
         for (int t = 0; t < kDecMaxSteps; ++t) { yacc[t][0] = 0.f; yacc[t][1] = 0.f; yacc[t][2] = 0.f; yacc[t][3] = 0.f; }
       }
@@ -368,7 +514,53 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
       const uint32_t dbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
       store_part(DecPart{2, sb, s});
       const AT* act = reinterpret_cast<const AT*>(fs.act[par][sb]);
-      if constexpr (kMma) {
+      if constexpr (F8) {
+        // a down core is 8 outputs x 8 act columns (64 bytes): lane quarters 0 / 1 hold columns 0-3 / 4-7 of outputs g and g + 8 and
+        // feed the k slots {2q, 2q+1, 2q+8, 2q+9}; quarters 2 / 3 contribute zeros (the unit has 8 columns, the MMA 16 slots)
+        const int tq = lane & 3;
+        const bool on = tq < 2;
+        const uint2 bv = *reinterpret_cast<const uint2*>(reinterpret_cast<const __half*>(act) + col * 8 + (tq & 1) * 4);
+        const uint32_t b0 = on ? bv.x : 0u, b1 = on ? bv.y : 0u;
+        const uint32_t abase = dbase + (uint32_t)(warp * g.steps) * 128u + (uint32_t)(lane >> 2) * 8u + (uint32_t)(tq & 1) * 4u;
+#pragma unroll
+        for (int t0 = 0; t0 < kDecMaxSteps; t0 += 4) {
+          if (t0 < g.steps) {
+            uint32_t lo[4], hi[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              lo[j] = lds_u32(abase + (uint32_t)(t0 + j) * 128u);
+              hi[j] = lds_u32(abase + (uint32_t)(t0 + j) * 128u + 64u);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const uint32_t l = on ? lo[j] : 0u, h = on ? hi[j] : 0u;
+              mma_f16_16816(yacc[t0 + j], cvt_e4m3x2_f16x2((uint16_t)l), cvt_e4m3x2_f16x2((uint16_t)h), cvt_e4m3x2_f16x2((uint16_t)(l >> 16)),
+                            cvt_e4m3x2_f16x2((uint16_t)(h >> 16)), b0, b1);
+            }
+          }
+        }
+        float s2v[kDecMaxSteps / 8];                           // block scales of this warp's output blocks (read before the slot is released)
+        if (sb == g.n_sb - 1) {
+#pragma unroll
+          for (int i = 0; i < kDecMaxSteps / 8; ++i)
+            s2v[i] = i * 8 < g.steps ? lds_f32(dbase + (uint32_t)g.part_bytes + (uint32_t)(warp * (g.steps >> 3) + i) * 4u) : 0.f;
+        }
+        release();
+        if (sb == g.n_sb - 1) {
+          const float as0 = fs.ascale[par][kq], as1 = fs.ascale[par][kq + 1];
+          const int j0 = s * g.slab + warp * (g.slab >> 3) + col;
+          float* p0 = a.partial + ((size_t)(pos0 + kq) * g.n_chunks + c) * g.d + j0;
+          float* p1 = p0 + (size_t)g.n_chunks * g.d;
+#pragma unroll
+          for (int t = 0; t < kDecMaxSteps; ++t) {
+            if (t < g.steps) {
+              const float sc0 = s2v[t >> 3] * as0, sc1 = s2v[t >> 3] * as1;
+              if (kq < cnt) { p0[t * 16] = yacc[t][0] * sc0; p0[t * 16 + 8] = yacc[t][2] * sc0; }
+              if (kq + 1 < cnt) { p1[t * 16] = yacc[t][1] * sc1; p1[t * 16 + 8] = yacc[t][3] * sc1; }
+            }
+          }
+        }
+      } else if constexpr (kMma) {
         // A[j][i]: 16 outputs j x (8 act columns i, upper half of K zero); B[i][n] = a[n][i]
         const uint32_t b0 = *reinterpret_cast<const uint32_t*>(act + col * 8 + kq);
         const uint32_t abase = dbase + (uint32_t)(lane & 7) * 16u + (uint32_t)((lane >> 3) & 1) * 128u + (uint32_t)(warp * g.steps) * 256u;

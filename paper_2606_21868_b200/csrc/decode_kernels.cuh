@@ -116,7 +116,7 @@ struct DecShared {
   DecPlan pl;
 };
 
-template <typename T>
+template <typename T, bool F8>
 __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const DecodeArgs a, const DecodeGeom g, int n_slots, int xs_pitch,
                                                                       int pre_off, int ring_off) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   DecRing ring;
   ring.slot0 = smem_u32(smem_raw) + (uint32_t)ring_off; ring.full0 = smem_u32(fs.full); ring.empty0 = smem_u32(fs.empty);
-  ring.n_slots = n_slots; ring.stride = g.part_bytes;
+  ring.n_slots = n_slots; ring.stride = g.slot_bytes;
   if (tid == 0) {
     mbar_init(smem_u32(&ds.go), 1);
     mbar_init(smem_u32(&ds.wpre), 1);
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
   fa.partial = a.partial;
 
   if (warp == kDecWarps + 1) {                           // ===================== reducer warp =====================
-    decode_reduce<T>(g, fs, lane);
+    decode_reduce<T, F8>(g, fs, lane);
     return;
   }
   if (warp == kDecWarps) {
@@ -176,6 +176,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
   unsigned gen = 0, qseq = 0, gu_seq = 0, d_seq = 0;
   const uint32_t w_off = (uint32_t)((E * sizeof(float) + 127) & ~(size_t)127);   // staged region: [router bias of the next layer][weight slice]
   T* xs = reinterpret_cast<T*>(smem_raw);               // current hidden state, [T][xs_pitch], in EVERY CTA
+  __half* xh = reinterpret_cast<__half*>(smem_raw + (((size_t)a.T * xs_pitch * sizeof(T) + 127) & ~(size_t)127));   // fp8 experts: f16 copy
   auto load_xs = [&](const void* src_) {
     const int vec_row = d * (int)sizeof(T) / 16;
     for (int i = tid; i < T_ * vec_row; i += kDecConsumers) {
@@ -245,6 +246,9 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
       }
     }
     asm volatile("bar.sync 1, 256;" ::: "memory");
+    if constexpr (F8)                                          // (the plan step's barriers order it before the consumers' reads)
+      stage_xh(reinterpret_cast<const __nv_bfloat16*>(xs), xh, fs, T_, d, xs_pitch, tid, kDecConsumers,
+               [] { asm volatile("bar.sync 1, 256;" ::: "memory"); });
     stamp(0);
     if (writer && tid < T_ * k) {
       const size_t off = (size_t)l * a.max_tokens * k;
@@ -303,7 +307,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
         }
       }
       fa.ticket = a.sync + 1 + (qseq & 1u);
-      decode_consume<T>(fa, g, pp, fs, ring, rp, gu_seq, d_seq, xs, xs_pitch);
+      decode_consume<T, F8>(fa, g, pp, fs, ring, rp, gu_seq, d_seq, xs, xh, xs_pitch);
     }
     if (n_waves == 0) ++qseq;                                  // (cannot happen: n_tokens >= 1) keeps the producer in step
     if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;  // C: every chunk partial of this layer is in place
@@ -390,7 +394,7 @@ __global__ void __launch_bounds__(NT) decode_plan_kernel(PlanArgs a, long long* 
 }
 
 // ffn: one wave of the plan in global memory; grid = SM count; `ticket` is zero at launch.
-template <typename T>
+template <typename T, bool F8>
 __global__ void __launch_bounds__(kDecThreads, 1) decode_ffn_kernel(DecodeFfnArgs fa, const DecodeGeom g, PlanPtrs gp, int wave, int C, int E,
                                                                     int n_tokens, const T* __restrict__ x, int n_slots, int xs_pitch,
                                                                     int ring_off) {
@@ -401,7 +405,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_ffn_kernel(DecodeFfnArg
   if (wave >= gp.hdr[0]) return;
   DecRing ring;
   ring.slot0 = smem_u32(smem_raw) + (uint32_t)ring_off; ring.full0 = smem_u32(fs.full); ring.empty0 = smem_u32(fs.empty);
-  ring.n_slots = n_slots; ring.stride = g.part_bytes;
+  ring.n_slots = n_slots; ring.stride = g.slot_bytes;
   if (tid == 0) dec_ffn_shared_init(fs, ring);
   // the plan -> shared memory (the consumers index it per part)
   const int nR = gp.hdr[1], n_pairs = gp.hdr[3];
@@ -419,16 +423,21 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_ffn_kernel(DecodeFfnArg
       reinterpret_cast<uint4*>(xs + (size_t)(i / vec_row) * xs_pitch)[i % vec_row] = reinterpret_cast<const uint4*>(x)[i];
   }
   __syncthreads();
+  __half* xh = reinterpret_cast<__half*>(smem_raw + (((size_t)n_tokens * xs_pitch * sizeof(T) + 127) & ~(size_t)127));
+  if constexpr (F8) {
+    stage_xh(reinterpret_cast<const __nv_bfloat16*>(xs), xh, fs, n_tokens, g.d, xs_pitch, tid, kDecThreads, [] { __syncthreads(); });
+    __syncthreads();
+  }
   DecRingPos rp{0, 0u};
   fa.inv_k = 1.0f / (float)fa.k;
   const int lo = wave * C, nw = min(nR, lo + C) - lo;
   if (warp == kDecWarps + 1) {
-    decode_reduce<T>(g, fs, lane);
+    decode_reduce<T, F8>(g, fs, lane);
   } else if (warp == kDecWarps) {
     if (lane == 0) decode_produce(fa, g, pp, fs, ring, rp, lo, nw, l2_evict_first_policy());
   } else {
     unsigned gu_seq = 0, d_seq = 0;
-    decode_consume<T>(fa, g, pp, fs, ring, rp, gu_seq, d_seq, xs, xs_pitch);
+    decode_consume<T, F8>(fa, g, pp, fs, ring, rp, gu_seq, d_seq, xs, xh, xs_pitch);
     asm volatile("bar.sync 1, 256;" ::: "memory");
     if (tid == 0) fs.final = 1;
   }

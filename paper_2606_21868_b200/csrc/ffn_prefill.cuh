@@ -11,13 +11,24 @@ namespace wisp {
 constexpr int kPfTile = 64;    // 64 pairs x 64 weight rows per CTA
 constexpr int kPfK = 32;
 
+// fp8 experts (f4): in-slot layout of the codes and scales (decode_ffn.cuh) read element by element and dequantised on the way
+// into shared memory, w = e4m3(code) * S[block] in fp32 -- the first correct prefill version of the quantised path.
+__device__ __forceinline__ float e4m3_to_f32(unsigned char c) {
+  return __half2float(__ushort_as_half((unsigned short)(cvt_e4m3x2_f16x2((uint16_t)c) & 0xffffu)));
+}
+__host__ __device__ __forceinline__ size_t tiled_down_index_f8(int j, int i, int d) {   // 8 outputs x 8 act columns per 64-byte core
+  return ((size_t)(i >> 3) * (d >> 3) + (j >> 3)) * 64 + (size_t)(j & 7) * 8 + (i & 7);
+}
+
 // grid: x = row tiles (n_rows/64), y = pair tiles (ceil(max_pairs_per_expert/64)), z = wave entry slot (C)
 // MODE 0: gate/up + SwiGLU (A rows gathered from x by token); MODE 1: down (A rows = act[pair]).
-template <typename T, int MODE>
+// F8: T is the hidden-state type (bf16), the weights are fp8 blobs of `blob_elems` BYTES with scales at s13_off / s2_off.
+template <typename T, int MODE, bool F8 = false>
 __global__ void __launch_bounds__(256) prefill_ffn_kernel(PlanPtrs plan, int wave, int C, const T* __restrict__ pool,
                                                           size_t blob_elems, int L, int layer,
                                                           const T* __restrict__ x, T* __restrict__ act,
-                                                          float* __restrict__ ystage, int d, int d_ff, int k) {
+                                                          float* __restrict__ ystage, int d, int d_ff, int k,
+                                                          size_t s13_off = 0, size_t s2_off = 0) {
   if (wave >= plan.hdr[0]) return;
   const int lo = wave * C, nw = min(plan.hdr[1], lo + C) - lo;
   if ((int)blockIdx.z >= nw) return;
@@ -29,12 +40,15 @@ __global__ void __launch_bounds__(256) prefill_ffn_kernel(PlanPtrs plan, int wav
   const int* pl = plan.pair_list + plan.exp_offset[e];
   const int K = MODE == 0 ? d : d_ff;
   const int r0 = blockIdx.x * kPfTile;
-  const T* blob = pool + ((size_t)plan.entry_slot[i] * L + layer) * blob_elems;
   // weights are read through the tiled in-slot layout (common.cuh): gate / up rows r0.., or down rows (outputs j) r0..
-  constexpr int kc = 16 / (int)sizeof(T);
+  constexpr int kc = F8 ? 16 : 16 / (int)sizeof(T);
+  const unsigned char* blob8 = reinterpret_cast<const unsigned char*>(pool) + ((size_t)plan.entry_slot[i] * L + layer) * blob_elems * (F8 ? 1 : sizeof(T));
+  const T* blob = reinterpret_cast<const T*>(blob8);
   const T* wg = blob;
   const T* wu = blob + (size_t)d_ff * d;
   const T* wd = blob + 2 * (size_t)d_ff * d;
+  const float* s13 = reinterpret_cast<const float*>(blob8 + s13_off);   // [2 d_ff / 128][d / 128]
+  const float* s2t = reinterpret_cast<const float*>(blob8 + s2_off);    // [d_ff / 128][d / 128]
 
   __shared__ float sA[kPfK][kPfTile + 1];
   __shared__ float sW0[kPfK][kPfTile + 1];
@@ -53,7 +67,17 @@ __global__ void __launch_bounds__(256) prefill_ffn_kernel(PlanPtrs plan, int wav
       float av = 0.f;
       if (pr >= 0) av = MODE == 0 ? to_f32<T>(x[(size_t)(pr / k) * d + k0 + kk]) : to_f32<T>(act[(size_t)pr * d_ff + k0 + kk]);
       sA[kk][row] = av;
-      if (MODE == 0) {
+      if constexpr (F8) {
+        if (MODE == 0) {
+          const size_t wi = tiled_gu_index(r0 + row, k0 + kk, d, kc);
+          const int kb = (k0 + kk) >> 7;
+          sW0[kk][row] = e4m3_to_f32(blob8[wi]) * s13[(size_t)((r0 + row) >> 7) * (d >> 7) + kb];
+          sW1[kk][row] = e4m3_to_f32(blob8[(size_t)d_ff * d + wi]) * s13[(size_t)((d_ff + r0 + row) >> 7) * (d >> 7) + kb];
+        } else {
+          sW0[kk][row] = e4m3_to_f32(blob8[2 * (size_t)d_ff * d + tiled_down_index_f8(r0 + row, k0 + kk, d)]) *
+                         s2t[(size_t)((k0 + kk) >> 7) * (d >> 7) + ((r0 + row) >> 7)];
+        }
+      } else if (MODE == 0) {
         const size_t wi = tiled_gu_index(r0 + row, k0 + kk, d, kc);
         sW0[kk][row] = to_f32<T>(wg[wi]);
         sW1[kk][row] = to_f32<T>(wu[wi]);

@@ -26,7 +26,10 @@ static_assert(sizeof(wisp_config) == 72 && sizeof(wisp_trace_event) == 32, "C AB
 struct wisp_ctx {
   wisp_config cfg{};
   u64 budget = 0;
-  size_t elem = 0, Me = 0, a_bytes = 0, blob_elems = 0;
+  size_t elem = 0, Me = 0, a_bytes = 0, blob_elems = 0;   // elem: bytes per hidden-state / router element
+  size_t welem = 0;                // bytes per expert-weight element (1 for WISP_FP8_E4M3)
+  bool f8 = false;
+  size_t s13_off = 0, s2_off = 0;  // fp8: byte offsets of the block scales inside a blob (S13, then S2 transposed)
   int C = 0;
   u64 kappa = 0, kv_reserved = 0, kv_peak = 0;
   u64 resize_count = 0, failed_resize = 0;
@@ -311,10 +314,11 @@ int fetch_wave(wisp_ctx* ctx, int layer, int wave, bool host_known, cudaStream_t
 
 // ---- decode path (decode_*.cuh) --------------------------------------------------------------------------------
 // Geometry of the fused FFN stream: slab = the largest multiple-of-256 divisor of d whose 8-row part fits 32 KiB.
-DecodeGeom make_decode_geom(int d, int dff, size_t elem, int rows_unit) {
+DecodeGeom make_decode_geom(int d, int dff, size_t elem, int rows_unit, bool f8 = false) {
   DecodeGeom g{};
   g.d = d; g.dff = dff; g.elem = (int)elem; g.kc = (int)(16 / elem);
   int m = (int)(kDecMaxPartBytes / (8 * elem)) / 256;
+  if (f8) m = std::min(m, kDecMaxSteps * 128 / 256);          // a warp's range of a slab is at most kDecMaxSteps cores
   const int q = d / 256;
   while (q % m) --m;
   g.slab = 256 * m;
@@ -325,10 +329,16 @@ DecodeGeom make_decode_geom(int d, int dff, size_t elem, int rows_unit) {
   g.n_chunks = dff / rows_unit;
   g.parts_unit = 3 * g.n_sb * g.n_slab;
   g.steps = g.slab / 128;
-  g.down_pieces = 8 / g.kc;
+  g.down_pieces = f8 ? 1 : 8 / g.kc;
   g.up_off = (unsigned long long)dff * d * elem;
   g.down_off = 2 * g.up_off;
   g.group_bytes = 8ull * d * elem;
+  g.f8 = f8 ? 1 : 0;
+  g.act_elem = f8 ? 2 : (int)elem;
+  g.scale_bytes = f8 ? 4 * (g.slab / 128) : 0;
+  g.slot_bytes = g.part_bytes + g.scale_bytes;
+  g.s13_off = 3ull * d * dff * elem;
+  g.s2_off = g.s13_off + 4ull * (2 * dff / 128) * (d / 128);
   return g;
 }
 
@@ -336,16 +346,16 @@ struct DecodeSmem { int n_slots, xs_pitch, pre_off, ring_off; size_t bytes; };
 // Shared-memory carve-up of a decode CTA: [hidden states, rows padded by 16 B][staged router-weight slice (fused kernel)]
 // [ring of n_slots parts].
 int decode_smem(wisp_ctx* ctx, const DecodeGeom& g, int T_, size_t avail, bool fused, DecodeSmem* out) {
-  out->xs_pitch = g.d + g.kc;
-  out->pre_off = (int)(((size_t)T_ * out->xs_pitch * g.elem + 127) & ~(size_t)127);
+  out->xs_pitch = g.d + 16 / g.act_elem;
+  out->pre_off = (int)(((size_t)T_ * out->xs_pitch * g.act_elem + 127) & ~(size_t)127) * (g.f8 ? 2 : 1);   // fp8: + the f16 copy
   const size_t pre = fused ? (((size_t)ctx->cfg.n_experts * sizeof(float) + 127) & ~(size_t)127) +
-                                 (((size_t)kSliceCols * ctx->cfg.n_experts * g.elem + 127) & ~(size_t)127) : 0;
+                                 (((size_t)kSliceCols * ctx->cfg.n_experts * g.act_elem + 127) & ~(size_t)127) : 0;
   out->ring_off = out->pre_off + (int)pre;
-  if ((size_t)out->ring_off + 2 * (size_t)g.part_bytes > avail) return fail(ctx, WISP_EINVAL, "decode kernel: shared memory too small for this shape");
-  int n = (int)std::min<size_t>(kDecMaxSlots, (avail - out->ring_off) / g.part_bytes);
+  if ((size_t)out->ring_off + 2 * (size_t)g.slot_bytes > avail) return fail(ctx, WISP_EINVAL, "decode kernel: shared memory too small for this shape");
+  int n = (int)std::min<size_t>(kDecMaxSlots, (avail - out->ring_off) / g.slot_bytes);
   if (ctx->cfg.ring_stages > 0) n = std::min(n, std::max(2, (int)ctx->cfg.ring_stages));
   out->n_slots = n;
-  out->bytes = (size_t)out->ring_off + (size_t)n * g.part_bytes;
+  out->bytes = (size_t)out->ring_off + (size_t)n * g.slot_bytes;
   return WISP_OK;
 }
 
@@ -359,7 +369,7 @@ int check_dev_err(wisp_ctx* ctx) {
   return fail(ctx, WISP_ECUDA, "fused decode kernel: a grid-wide barrier timed out; the outputs of that forward are invalid");
 }
 
-template <typename T>
+template <typename T, bool F8 = false>
 int launch_fused(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out, bool residual, cudaStream_t st) {
   const auto& cfg = ctx->cfg;
   DecodeArgs pa{};
@@ -382,7 +392,7 @@ int launch_fused(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out
   if (rc) return rc;
   CK(cudaMemsetAsync(ctx->dsync, 0, 4 * sizeof(unsigned), st));
   void* args[] = {&pa, &g, &sm.n_slots, &sm.xs_pitch, &sm.pre_off, &sm.ring_off};
-  CK(cudaLaunchCooperativeKernel((const void*)decode_fused_kernel<T>, dim3(ctx->num_sms), dim3(kDecThreads), args, sm.bytes, st));
+  CK(cudaLaunchCooperativeKernel((const void*)decode_fused_kernel<T, F8>, dim3(ctx->num_sms), dim3(kDecThreads), args, sm.bytes, st));
   ++ctx->launches;
   for (int l = lo; l < hi; ++l) ctx->last_T[l] = T_;
   ctx->last_layer = hi - 1;
@@ -391,13 +401,14 @@ int launch_fused(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out
 }
 
 int launch_fused_any(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out, bool residual, cudaStream_t st) {
+  if (ctx->f8) return launch_fused<__nv_bfloat16, true>(ctx, lo, hi, x, T_, out, residual, st);
   return ctx->cfg.dtype == WISP_F32 ? launch_fused<float>(ctx, lo, hi, x, T_, out, residual, st)
                                     : launch_fused<__nv_bfloat16>(ctx, lo, hi, x, T_, out, residual, st);
 }
 
 // Split form of one decode layer (MEMCPY / ZEROCOPY contexts, E > 256): logits, plan, per wave (fetch, ffn), combine -- the
 // same device functions as the fused kernel, so both give the same bits.  x_next != nullptr: residual successor instead of y.
-template <typename T>
+template <typename T, bool F8 = false>
 int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st,
                          const char* slot_base = nullptr) {
   const auto& cfg = ctx->cfg;
@@ -476,7 +487,7 @@ int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* 
     }
     CK(cudaMemsetAsync(ctx->dsync + 1, 0, sizeof(unsigned), st));
     Span sp(ctx, WISP_K_FFN, st);
-    decode_ffn_kernel<T><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, w, ctx->C, E, T_, reinterpret_cast<const T*>(x),
+    decode_ffn_kernel<T, F8><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, w, ctx->C, E, T_, reinterpret_cast<const T*>(x),
                                                                      sm.n_slots, sm.xs_pitch, sm.ring_off);
   }
   {
@@ -493,7 +504,7 @@ int forward_layer_decode(wisp_ctx* ctx, int layer, const void* x, int T_, void* 
 }
 
 // ---- prefill path: grouped GEMM per wave (n_tokens > kDecodeMaxTokens) ----------------------------------------------
-template <typename T>
+template <typename T, bool F8 = false>
 int launch_prefill_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T_, cudaStream_t st) {
   const auto& cfg = ctx->cfg;
   const int d = cfg.d_model, dff = cfg.d_ff, k = cfg.top_k, L = cfg.n_layers;
@@ -523,15 +534,15 @@ int launch_prefill_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T
     dim3 g0(dff / kPfTile, ptiles, ctx->C), g1(d / kPfTile, ptiles, ctx->C);
     {
       Span sp(ctx, WISP_K_PREFILL_GATE_UP, st);
-      prefill_ffn_kernel<T, 0><<<g0, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
-                                                   reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
-                                                   ctx->ystage, d, dff, k);
+      prefill_ffn_kernel<T, 0, F8><<<g0, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, F8 ? ctx->Me : ctx->blob_elems, L, layer,
+                                                       reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
+                                                       ctx->ystage, d, dff, k, ctx->s13_off, ctx->s2_off);
     }
     {
       Span sp(ctx, WISP_K_PREFILL_DOWN, st);
-      prefill_ffn_kernel<T, 1><<<g1, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, ctx->blob_elems, L, layer,
-                                                   reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
-                                                   ctx->ystage, d, dff, k);
+      prefill_ffn_kernel<T, 1, F8><<<g1, 256, 0, st>>>(ctx->plan, wave, ctx->C, pool, F8 ? ctx->Me : ctx->blob_elems, L, layer,
+                                                       reinterpret_cast<const T*>(x), reinterpret_cast<T*>(ctx->act_T),
+                                                       ctx->ystage, d, dff, k, ctx->s13_off, ctx->s2_off);
     }
   }
   CK(cudaGetLastError());
@@ -586,7 +597,7 @@ bool setup_mma_path(wisp_ctx* ctx) {
 }
 
 // One prefill MoE layer: router -> residency -> per wave (fetch, grouped GEMMs into ystage [T,k,d]) -> ordered combine (a5).
-template <typename T>
+template <typename T, bool F8 = false>
 int forward_layer_prefill(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
   const auto& cfg = ctx->cfg;
   const int k = cfg.top_k, E = cfg.n_experts;
@@ -613,7 +624,7 @@ int forward_layer_prefill(wisp_ctx* ctx, int layer, const void* x, int T_, void*
   for (int w = 0; w < n_waves; ++w) {
     rc = fetch_wave(ctx, layer, w, memcpy_path, st);   // prefill under FUSED uses the zero-copy kernel
     if (rc) return rc;
-    rc = launch_prefill_wave<T>(ctx, layer, w, x, T_, st);
+    rc = launch_prefill_wave<T, F8>(ctx, layer, w, x, T_, st);
     if (rc) return rc;
   }
   const size_t n = (size_t)T_ * cfg.d_model;
@@ -631,6 +642,9 @@ int forward_layer_prefill(wisp_ctx* ctx, int layer, const void* x, int T_, void*
 
 int forward_layer_any(wisp_ctx* ctx, int layer, const void* x, int T_, void* out, void* x_next, cudaStream_t st) {
   const bool f32 = ctx->cfg.dtype == WISP_F32;
+  if (ctx->f8)
+    return T_ <= kDecodeMaxTokens ? forward_layer_decode<__nv_bfloat16, true>(ctx, layer, x, T_, out, x_next, st)
+                                  : forward_layer_prefill<__nv_bfloat16, true>(ctx, layer, x, T_, out, x_next, st);
   if (T_ <= kDecodeMaxTokens)
     return f32 ? forward_layer_decode<float>(ctx, layer, x, T_, out, x_next, st)
                : forward_layer_decode<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st);
@@ -664,8 +678,9 @@ int forward_layer_static(wisp_ctx* ctx, int layer, const void* x, int T_, void* 
     }
     CK(cudaStreamWaitEvent(st, ctx->ev_buf_ready[b], 0));
   }
-  int rc = ctx->cfg.dtype == WISP_F32 ? forward_layer_decode<float>(ctx, layer, x, T_, out, x_next, st, base)
-                                      : forward_layer_decode<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st, base);
+  int rc = ctx->f8 ? forward_layer_decode<__nv_bfloat16, true>(ctx, layer, x, T_, out, x_next, st, base)
+           : ctx->cfg.dtype == WISP_F32 ? forward_layer_decode<float>(ctx, layer, x, T_, out, x_next, st, base)
+                                        : forward_layer_decode<__nv_bfloat16>(ctx, layer, x, T_, out, x_next, st, base);
   if (rc) return rc;
   if (!resident) {
     CK(cudaEventRecord(ctx->ev_buf_free[b], st));
@@ -696,8 +711,12 @@ int occupancy_grid(wisp_ctx* ctx, F kernel, int threads, int cap_per_sm) {
 // Re-tile the caller's canonical blobs ([gate | up | down], row-major out x in) into the in-slot layout of common.cuh:
 // 8-row x 16-byte core matrices, gate/up cores ordered (row group, K), down cores ordered (act-column block, output group).
 // Pure byte movement in 16-byte pieces, spread over host threads (a layer is 1-3 GiB).
-void retile_layer(const char* src, char* dst, size_t E, size_t d, size_t dff, size_t elem) {
-  const size_t kc = 16 / elem, Me = 3 * d * dff * elem, mat = d * dff * elem;
+// fp8 blobs: the codes of gate / up tile the same way (16 codes per 16-byte row of a core); down uses 8-output x 8-column cores of
+// 64 bytes (one decode work unit owns 8 act columns); the scales follow: S13 as given, S2 transposed to [d_ff / 128][d / 128].
+void retile_layer(const char* src, char* dst, size_t E, size_t d, size_t dff, size_t elem, bool f8) {
+  const size_t kc = 16 / elem, mat = d * dff * elem;
+  const size_t n13 = f8 ? (2 * dff / 128) * (d / 128) : 0, n2 = f8 ? (d / 128) * (dff / 128) : 0;
+  const size_t Me = 3 * mat + 4 * (n13 + n2);
   const size_t gu_items = E * 2 * (dff / 8);                 // (expert, gate|up, row group)
   const size_t ib_per = dff / kc, line_ib = std::max<size_t>(1, 64 / 16);   // down: 4 act-column blocks share a 64-byte line
   const size_t dn_items = E * ((ib_per + line_ib - 1) / line_ib);
@@ -717,6 +736,19 @@ void retile_layer(const char* src, char* dst, size_t E, size_t d, size_t dff, si
         const size_t nib = std::min(line_ib, ib_per - ib0);
         const char* s0 = src + e * Me + 2 * mat;             // down [d][dff]
         char* o = dst + e * Me + 2 * mat;
+        if (f8) {
+          for (size_t j = 0; j < d; ++j)
+            for (size_t b = 0; b < 2 * nib; ++b)               // 8-column blocks
+              std::memcpy(o + (((ib0 * 2 + b) * (d / 8) + j / 8) * 8 + (j & 7)) * 8, s0 + j * dff + (ib0 * 2 + b) * 8, 8);
+          if (ib0 == 0) {                                      // this expert's scales (once)
+            const float* sc = reinterpret_cast<const float*>(src + e * Me + 3 * mat);
+            float* so = reinterpret_cast<float*>(dst + e * Me + 3 * mat);
+            std::memcpy(so, sc, 4 * n13);
+            for (size_t jb = 0; jb < d / 128; ++jb)
+              for (size_t cb = 0; cb < dff / 128; ++cb) so[n13 + cb * (d / 128) + jb] = sc[n13 + jb * (dff / 128) + cb];
+          }
+          continue;
+        }
         for (size_t j = 0; j < d; ++j)
           for (size_t b = 0; b < nib; ++b)
             std::memcpy(o + (((ib0 + b) * (d / 8) + j / 8) * 8 + (j & 7)) * 16, s0 + (j * dff + (ib0 + b) * kc) * elem, 16);
@@ -748,7 +780,8 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   if (cfg->n_layers < 1 || cfg->n_experts < 1 || cfg->n_experts > kMaxExperts || cfg->top_k < 1 ||
       cfg->top_k > kMaxTopK || cfg->top_k > cfg->n_experts || cfg->d_model < 256 || cfg->d_model % 256 ||
       cfg->d_ff < 256 || cfg->d_ff % 256 || cfg->max_tokens < 1 ||
-      (cfg->dtype != WISP_F32 && cfg->dtype != WISP_BF16) || (cfg->policy != WISP_LRU && cfg->policy != WISP_LFU) ||
+      (cfg->dtype != WISP_F32 && cfg->dtype != WISP_BF16 && cfg->dtype != WISP_FP8_E4M3) ||
+      (cfg->dtype == WISP_FP8_E4M3 && cfg->d_model % 1024) || (cfg->policy != WISP_LRU && cfg->policy != WISP_LFU) ||
       (cfg->fetch != WISP_FETCH_MEMCPY && cfg->fetch != WISP_FETCH_ZEROCOPY && cfg->fetch != WISP_FETCH_FUSED &&
        cfg->fetch != WISP_FETCH_STATIC) ||
       cfg->ring_stages < 0 || cfg->ring_stages > kDecMaxSlots || cfg->unit_rows < 0 || cfg->unit_rows % 8 ||
@@ -760,8 +793,15 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   ctx->cfg = *cfg;
   ctx->budget = budget_bytes;
   ctx->elem = cfg->dtype == WISP_F32 ? 4 : 2;
+  ctx->f8 = cfg->dtype == WISP_FP8_E4M3;
+  ctx->welem = ctx->f8 ? 1 : ctx->elem;
   ctx->blob_elems = 3 * (size_t)cfg->d_model * cfg->d_ff;
-  ctx->Me = ctx->blob_elems * ctx->elem;
+  ctx->Me = ctx->blob_elems * ctx->welem;
+  if (ctx->f8) {                                   // + the fp32 block scales S13 and S2 (one per 128 x 128 block)
+    ctx->s13_off = ctx->Me;
+    ctx->s2_off = ctx->s13_off + 4 * (size_t)(2 * cfg->d_ff / 128) * (cfg->d_model / 128);
+    ctx->Me = ctx->s2_off + 4 * (size_t)(cfg->d_model / 128) * (cfg->d_ff / 128);
+  }
   ctx->a_bytes = ctx->Me * cfg->n_layers;
   const u64 b = cfg->kv_block_bytes;
   const u64 kv0 = b ? cfg->kv_floor_blocks * b : 0;
@@ -869,15 +909,17 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
     // (config 1, parity only) always use 8.
     const int r0 = cfg->unit_rows > 0 && cfg->dtype != WISP_F32 ? cfg->unit_rows : 8;
     const int r1 = cfg->dtype == WISP_F32 ? 8 : cfg->unit_rows > 0 ? cfg->unit_rows : 16;
-    ctx->dgeom[0] = make_decode_geom(d, dff, ctx->elem, r0);
-    ctx->dgeom[1] = make_decode_geom(d, dff, ctx->elem, r1);
+    ctx->dgeom[0] = make_decode_geom(d, dff, ctx->welem, r0, ctx->f8);
+    ctx->dgeom[1] = make_decode_geom(d, dff, ctx->welem, r1, ctx->f8);
     const size_t t_dec = std::min<size_t>(maxT, kDecodeMaxTokens);
     const size_t pairs0 = std::min<size_t>(t_dec, 2) * k, pairs1 = t_dec * k;
     const size_t n_part = std::max(pairs0 * ctx->dgeom[0].n_chunks, pairs1 * ctx->dgeom[1].n_chunks) * d;
     CKC(cudaMalloc(&ctx->partial, n_part * sizeof(float)));
     cudaFuncAttributes fa;
-    const void* kf = cfg->dtype == WISP_F32 ? (const void*)decode_fused_kernel<float> : (const void*)decode_fused_kernel<__nv_bfloat16>;
-    const void* kn = cfg->dtype == WISP_F32 ? (const void*)decode_ffn_kernel<float> : (const void*)decode_ffn_kernel<__nv_bfloat16>;
+    const void* kf = ctx->f8 ? (const void*)decode_fused_kernel<__nv_bfloat16, true>
+                     : cfg->dtype == WISP_F32 ? (const void*)decode_fused_kernel<float, false> : (const void*)decode_fused_kernel<__nv_bfloat16, false>;
+    const void* kn = ctx->f8 ? (const void*)decode_ffn_kernel<__nv_bfloat16, true>
+                     : cfg->dtype == WISP_F32 ? (const void*)decode_ffn_kernel<float, false> : (const void*)decode_ffn_kernel<__nv_bfloat16, false>;
     CKC(cudaFuncGetAttributes(&fa, kf));
     ctx->fused_smem = (227u << 10) - fa.sharedSizeBytes;
     CKC(cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->fused_smem));
@@ -954,7 +996,7 @@ int wisp_register_host_experts(wisp_ctx* ctx, int32_t layer, const void* experts
   const size_t E = ctx->cfg.n_experts, d = ctx->cfg.d_model;
   void* m = nullptr;
   CK(cudaHostAlloc(&m, E * ctx->Me, cudaHostAllocMapped | cudaHostAllocPortable));
-  retile_layer(static_cast<const char*>(experts), static_cast<char*>(m), E, d, ctx->cfg.d_ff, ctx->elem);
+  retile_layer(static_cast<const char*>(experts), static_cast<char*>(m), E, d, ctx->cfg.d_ff, ctx->welem, ctx->f8);
   ctx->master[layer] = m;
   CK(cudaMemcpy(ctx->d_masters + layer, &m, sizeof(char*), cudaMemcpyHostToDevice));
   CK(cudaMemcpy(ctx->router_w + (size_t)layer * E * d * ctx->elem, router_w, E * d * ctx->elem, cudaMemcpyHostToDevice));
@@ -1327,11 +1369,15 @@ int wisp_debug_ffn_launch(wisp_ctx* ctx, int32_t layer, const void* hidden, int3
   fa.partial = ctx->partial; fa.master = nullptr; fa.ticket = ctx->dsync + 1;
   CK(cudaMemsetAsync(ctx->dsync + 1, 0, sizeof(unsigned), st));
   ++ctx->launches;
-  if (ctx->cfg.dtype == WISP_F32)
-    decode_ffn_kernel<float><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, 0, ctx->C, ctx->cfg.n_experts, n_tokens,
-                                                                         static_cast<const float*>(hidden), sm.n_slots, sm.xs_pitch, sm.ring_off);
+  if (ctx->f8)
+    decode_ffn_kernel<__nv_bfloat16, true><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, 0, ctx->C, ctx->cfg.n_experts, n_tokens,
+                                                                                       static_cast<const __nv_bfloat16*>(hidden), sm.n_slots,
+                                                                                       sm.xs_pitch, sm.ring_off);
+  else if (ctx->cfg.dtype == WISP_F32)
+    decode_ffn_kernel<float, false><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, 0, ctx->C, ctx->cfg.n_experts, n_tokens,
+                                                                                static_cast<const float*>(hidden), sm.n_slots, sm.xs_pitch, sm.ring_off);
   else
-    decode_ffn_kernel<__nv_bfloat16><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, 0, ctx->C, ctx->cfg.n_experts, n_tokens,
+    decode_ffn_kernel<__nv_bfloat16, false><<<ctx->num_sms, kDecThreads, sm.bytes, st>>>(fa, g, ctx->plan, 0, ctx->C, ctx->cfg.n_experts, n_tokens,
                                                                                  static_cast<const __nv_bfloat16*>(hidden), sm.n_slots,
                                                                                  sm.xs_pitch, sm.ring_off);
   CK(cudaGetLastError());

@@ -22,7 +22,8 @@ def make_ctx(shape, slots=None, *, budget=None, policy=0, fetch=1, max_tokens=8,
     if budget is None:
         budget = slots * shape.slot_unit_bytes + kv_floor_blocks * kv_block_bytes
     ctx = wp.Wisp(budget, n_layers=shape.n_layers, n_experts=shape.n_experts, top_k=shape.top_k, d_model=shape.d_model,
-                  d_ff=shape.d_ff, max_tokens=max_tokens, dtype=wp.WISP_F32 if shape.dtype == "f32" else wp.WISP_BF16,
+                  d_ff=shape.d_ff, max_tokens=max_tokens,
+                  dtype={"f32": wp.WISP_F32, "bf16": wp.WISP_BF16, "fp8": wp.WISP_FP8_E4M3}[shape.dtype],
                   policy=policy, fetch=fetch, kv_block_bytes=kv_block_bytes, kv_floor_blocks=kv_floor_blocks,
                   trace_capacity=trace_capacity)
     experts, routers = model(shape)
