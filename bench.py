@@ -39,7 +39,8 @@ def parse():
     ap.add_argument("--steps", type=int, default=128)
     ap.add_argument("--warmup", type=int, default=16)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="qwen3", choices=["qwen3", "mixtral", "tiny", "mvwsa"])
+    ap.add_argument("--workload", default="qwen3", choices=["qwen3", "mixtral", "tiny", "mvwsa", "qwen3-fp8"],
+                    help="qwen3-fp8 = the headline shape with fp8 block-quantised experts (SURVEY.md 8(f) f4; PAPER.md:369) at the same budget")
     ap.add_argument("--mvwsa-decode", type=int, default=512, help="decode steps per request (config 5)")
     ap.add_argument("--mvwsa-prompt-scale", type=float, default=1.0, help="scale the U{1k..16k} prompt lengths (config 5)")
     ap.add_argument("--layers", type=int, default=0, help="override the layer count (0 = the config's)")
@@ -73,8 +74,8 @@ def parse():
 
 
 def workload(args):
-    shape = {"qwen3": si.QWEN3, "mixtral": si.MIXTRAL, "tiny": si.TINY}[args.workload]
-    budget = {"qwen3": 8 * GIB, "mixtral": 24 * GIB, "tiny": 6 * si.TINY.slot_unit_bytes}[args.workload]
+    shape = {"qwen3": si.QWEN3, "mixtral": si.MIXTRAL, "tiny": si.TINY, "qwen3-fp8": si.QWEN3_FP8}[args.workload]
+    budget = {"qwen3": 8 * GIB, "mixtral": 24 * GIB, "tiny": 6 * si.TINY.slot_unit_bytes, "qwen3-fp8": 8 * GIB}[args.workload]
     if args.budget_gib > 0:
         budget = int(args.budget_gib * GIB)
     if args.stress:
@@ -168,6 +169,11 @@ def profile_traffic(kernel):
     return None
 
 
+def wisp_dtype(shape):
+    import paper_2606_21868_b200 as wp
+    return {"f32": wp.WISP_F32, "bf16": wp.WISP_BF16, "fp8": wp.WISP_FP8_E4M3}[shape.dtype]
+
+
 def traffic_of(kernel, same_workload):
     t = profile_traffic(kernel)
     return int(t["traffic"]) if (t and same_workload) else None
@@ -177,7 +183,7 @@ def traffic_of(kernel, same_workload):
 def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=None, gen_device="cuda"):
     import paper_2606_21868_b200 as wp
     ctx = wp.Wisp(budget, n_layers=shape.n_layers, n_experts=shape.n_experts, top_k=shape.top_k, d_model=shape.d_model,
-                  d_ff=shape.d_ff, max_tokens=max_tokens, dtype=wp.WISP_F32 if shape.dtype == "f32" else wp.WISP_BF16,
+                  d_ff=shape.d_ff, max_tokens=max_tokens, dtype=wisp_dtype(shape),
                   policy=wp.WISP_LFU if args.policy == "lfu" else wp.WISP_LRU,
                   fetch={"memcpy": wp.WISP_FETCH_MEMCPY, "zerocopy": wp.WISP_FETCH_ZEROCOPY, "fused": wp.WISP_FETCH_FUSED,
                          "static": wp.WISP_FETCH_STATIC}[fetch or args.fetch],
@@ -186,7 +192,7 @@ def build_context(shape, budget, args, max_tokens, fetch=None, register_layers=N
         ctx.set_wave_order(wp.WISP_WAVES_HITS_FIRST)
     if getattr(args, "prefetch", 0) > 0 and (fetch or args.fetch) == "zerocopy":
         ctx.set_prefetch(args.prefetch, args.prefetch_gamma, args.prefetch_window)
-    staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
+    staging = torch.empty((shape.n_experts, shape.blob_len), dtype=shape.blob_dtype, pin_memory=True)
     for l in (register_layers if register_layers is not None else range(shape.n_layers)):
         si.gen_layer_experts(shape, l, gen_device, out=staging)
         w_r, bias = si.gen_router(shape, l)
@@ -420,7 +426,7 @@ def main_mvwsa(args):
                   kv_floor_blocks=floor_blocks)
     if args.wave_order == "hits-first":
         ctx.set_wave_order(wp.WISP_WAVES_HITS_FIRST)
-    staging = torch.empty((shape.n_experts, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
+    staging = torch.empty((shape.n_experts, shape.blob_len), dtype=shape.blob_dtype, pin_memory=True)
     for l in range(shape.n_layers):
         si.gen_layer_experts(shape, l, "cuda", out=staging)
         w_r, bias = si.gen_router(shape, l)
@@ -525,7 +531,7 @@ def ffn_microbench(shape, args, batches=(1, 4), n_steps=24):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     for B in batches:
         ctx = wp.Wisp(one.n_experts * one.slot_unit_bytes, n_layers=1, n_experts=one.n_experts, top_k=one.top_k, d_model=one.d_model,
-                      d_ff=one.d_ff, max_tokens=B, dtype=wp.WISP_BF16 if one.dtype == "bf16" else wp.WISP_F32, fetch=wp.WISP_FETCH_ZEROCOPY,
+                      d_ff=one.d_ff, max_tokens=B, dtype=wisp_dtype(one), fetch=wp.WISP_FETCH_ZEROCOPY,
                       unit_rows=getattr(args, "unit_rows", 0))
         blob = si.gen_layer_experts(one, 0, "cuda")
         w_r, bias = si.gen_router(one, 0)
@@ -568,7 +574,7 @@ def route_microbench(shape, args):
     one = shape.with_layers(1)
     T_max = 2048
     ctx = wp.Wisp(one.n_experts * one.slot_unit_bytes, n_layers=1, n_experts=one.n_experts, top_k=one.top_k, d_model=one.d_model,
-                  d_ff=one.d_ff, max_tokens=T_max, dtype=wp.WISP_BF16 if one.dtype == "bf16" else wp.WISP_F32, fetch=wp.WISP_FETCH_ZEROCOPY)
+                  d_ff=one.d_ff, max_tokens=T_max, dtype=wisp_dtype(one), fetch=wp.WISP_FETCH_ZEROCOPY)
     blob = si.gen_layer_experts(one, 0, "cuda")
     w_r, bias = si.gen_router(one, 0)
     ctx.register_host_experts(0, blob, w_r, bias)
@@ -609,8 +615,8 @@ def verify_stack(shape, runs, *, steps, batches, prefill_tokens=0, samples=((0, 
     a = shape.slot_unit_bytes
     max_tokens = max(max(batches), prefill_tokens, 1)
     ctx = wp.Wisp(E * a, n_layers=L, n_experts=E, top_k=k, d_model=d, d_ff=shape.d_ff, max_tokens=max_tokens,
-                  dtype=wp.WISP_F32 if shape.dtype == "f32" else wp.WISP_BF16, fetch=wp.WISP_FETCH_FUSED, trace_capacity=1 << 23)
-    staging = torch.empty((E, shape.expert_elems), dtype=shape.torch_dtype, pin_memory=True)
+                  dtype=wisp_dtype(shape), fetch=wp.WISP_FETCH_FUSED, trace_capacity=1 << 23)
+    staging = torch.empty((E, shape.blob_len), dtype=shape.blob_dtype, pin_memory=True)
     for l in range(L):
         si.gen_layer_experts(shape, l, "cuda", out=staging)
         w_r, bias = si.gen_router(shape, l)
@@ -889,7 +895,7 @@ def main_ours(args):
     roof = None
     fused = args.fetch == "fused" and B <= 8 and shape.n_experts <= 256 and not args.per_layer_api
     # roofline.traffic: the committed ncu capture's dram read + write bytes per launch -- only for the workload it was captured on
-    default_workload = (shape.name.startswith("qwen3") and "STRESS" not in shape.name and B == 1 and shape.n_layers == 48 and abs(budget / GIB - 8.0) < 1e-6
+    default_workload = (shape.name.startswith("qwen3") and shape.dtype == "bf16" and "STRESS" not in shape.name and B == 1 and shape.n_layers == 48 and abs(budget / GIB - 8.0) < 1e-6
                         and args.policy == "lru" and args.prefetch == 0)
     if "ffn" in kern:
         # FFN phase (fused kernel: %globaltimer stamps of CTA 0 over layer calls WITHOUT a miss, from the release of the
@@ -928,7 +934,8 @@ def main_ours(args):
                 "bytes_per_step_oracle_model": int(model), "bytes_match_oracle_model": bool(streamed == model * n_fwd)}
     line = {"metric": "decode_tokens_per_s", "value": value, "unit": "tokens/s", "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": warm_ms / K, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "bf16" if shape.dtype == "bf16" else "f32", "data": "synthetic",
+            "vs_baseline": None, "dtype": {"bf16": "bf16", "f32": "f32", "fp8": "fp8-e4m3 weights x bf16 activations (f16 mma, fp32 accumulate)"}[shape.dtype],
+            "data": "synthetic",
             "config": {"workload": f"{shape.name} decode, batch {B}, {shape.n_layers} layers, E={shape.n_experts}, top-{shape.top_k}, "
                                    f"d={shape.d_model}, d_ff={shape.d_ff}, expert pool {budget / GIB:.3f} GiB -> C={C} slots/layer, "
                                    f"{args.policy.upper()}, fetch={args.fetch}" + (", waves=hits-first" if args.wave_order == "hits-first" else "")
@@ -975,7 +982,7 @@ def main_ours(args):
                 roof["frac_of_step_lower_bound"] = round(roof["step_lower_bound_us"] / roof["avg_launch_us"], 4)
         except Exception as ex:                        # a microbenchmark must never take the headline down
             line["miss_path"] = {"error": repr(ex)[:200]}
-    if rank == 0 and world == 1 and not args.no_micro and shape.dtype == "bf16":
+    if rank == 0 and world == 1 and not args.no_micro and shape.dtype in ("bf16", "fp8"):
         try:
             line["ffn_only"] = {"this_shape": ffn_microbench(shape, args)}
             other = si.MIXTRAL if shape.name.startswith("qwen3") else si.QWEN3

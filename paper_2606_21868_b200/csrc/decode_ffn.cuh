@@ -72,6 +72,9 @@ struct DecodeGeom {
   int act_elem;          // bytes per hidden-state element (2 for fp8 experts)
   int scale_bytes;       // per part: 4 * slab / 128 (0 without scales)
   int slot_bytes;        // ring slot = part_bytes + scale_bytes
+  int merge;             // 1: one part holds ALL sub-blocks of the unit (consecutive 8-row groups are contiguous; fp8 with n_slab == 1):
+                         //    the producer lane's cost per part is what bounds 16 KiB parts, so fp8 parts are 32 KiB like bf16's
+  int sub_bytes;         // 8 * slab * elem: one sub-block inside a part
   unsigned long long s13_off, s2_off;
 };
 
@@ -241,7 +244,7 @@ __device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const Dec
   auto emit_down = [&](int q, int c) -> bool {
     const char* blob = blob_of(q);
     for (int s = 0; s < g.n_slab; ++s)
-      for (int sb = 0; sb < g.n_sb; ++sb)
+      for (int sb = 0; sb < (g.merge ? 1 : g.n_sb); ++sb)
         if (!emit(blob, q, c, DecPart{2, sb, s})) return false;
     return true;
   };
@@ -250,7 +253,7 @@ __device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const Dec
     const unsigned t = atomicAdd(a.ticket, 1u);                // next unit: its latency hides behind this unit's copies
     const int q = plan.unit_entry[lo + u / g.n_chunks], c = u % g.n_chunks;
     const char* blob = blob_of(q);
-    for (int sb = 0; sb < g.n_sb; ++sb)
+    for (int sb = 0; sb < (g.merge ? 1 : g.n_sb); ++sb)
       for (int s = 0; s < g.n_slab; ++s) {
         if (!emit(blob, q, c, DecPart{0, sb, s})) return;
         if (!emit(blob, q, c, DecPart{1, sb, s})) return;
@@ -407,42 +410,58 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
       const uint32_t ubase = ring.slot0 + (uint32_t)rpu.s * ring.stride;
       const int k_lo = s * g.slab + warp * (g.slab >> 3);     // this warp's K range of the slab
       if constexpr (F8) {
-        // one core matrix (8 rows x 16 codes) is one k16 step; an ldmatrix.x4 = {gate, up} x two steps; 8 steps = one scale block
+        // one core matrix (8 rows x 16 codes) is one k16 step; an ldmatrix.x4 = {gate, up} x two steps; 8 steps = one scale block.
+        // A merged part (g.merge) holds every sub-block of the unit: they are computed one after the other from the same two slots.
         const int tok = col < cnt ? (int)(((float)pl[col] + 0.5f) * a.inv_k) : -1;
-        const uint32_t abase = ((lane >> 3) & 1 ? ubase : gbase) + (uint32_t)(lane & 7) * 16u + (uint32_t)(lane >> 4) * 128u +
-                               (uint32_t)(warp * g.steps) * 128u;
         const __half* xrow = xh + (size_t)max(tok, 0) * xs_pitch + k_lo + (lane & 3) * 4;
         const uint32_t sc = (uint32_t)g.part_bytes + (uint32_t)(warp * (g.steps >> 3)) * 4u;
+        const int n_in = g.merge ? g.n_sb : 1;
+        for (int sbi = 0; sbi < n_in; ++sbi) {
+          const uint32_t abase = ((lane >> 3) & 1 ? ubase : gbase) + (uint32_t)sbi * (uint32_t)g.sub_bytes + (uint32_t)(lane & 7) * 16u +
+                                 (uint32_t)(lane >> 4) * 128u + (uint32_t)(warp * g.steps) * 128u;
+          if (g.merge) { tot8[0] = 0.f; tot8[1] = 0.f; tot8[2] = 0.f; tot8[3] = 0.f; }
 #pragma unroll
-        for (int kb = 0; kb < kDecMaxSteps / 8; ++kb) {
-          if (kb * 8 < g.steps) {
-            uint32_t af[4][4];
-            uint2 bf[8];
+          for (int kb = 0; kb < kDecMaxSteps / 8; ++kb) {
+            if (kb * 8 < g.steps) {
+              uint32_t af[4][4];
+              uint2 bf[8];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              ldmatrix_x4(af[j][0], af[j][1], af[j][2], af[j][3], abase + (uint32_t)(kb * 4 + j) * 256u);
-              bf[2 * j] = tok >= 0 ? *reinterpret_cast<const uint2*>(xrow + (kb * 8 + 2 * j) * 16) : make_uint2(0u, 0u);
-              bf[2 * j + 1] = tok >= 0 ? *reinterpret_cast<const uint2*>(xrow + (kb * 8 + 2 * j + 1) * 16) : make_uint2(0u, 0u);
+              for (int j = 0; j < 4; ++j) {
+                ldmatrix_x4(af[j][0], af[j][1], af[j][2], af[j][3], abase + (uint32_t)(kb * 4 + j) * 256u);
+                bf[2 * j] = tok >= 0 ? *reinterpret_cast<const uint2*>(xrow + (kb * 8 + 2 * j) * 16) : make_uint2(0u, 0u);
+                bf[2 * j + 1] = tok >= 0 ? *reinterpret_cast<const uint2*>(xrow + (kb * 8 + 2 * j + 1) * 16) : make_uint2(0u, 0u);
+              }
+              float c8[4][4];
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                // registers 0/1: gate / up codes of step 2j; registers 2/3: of step 2j + 1.  Chain (2j) & 3 / (2j + 1) & 3; the first
+                // product of a chain starts from a zero accumulator
+                const uint32_t g0 = cvt_e4m3x2_f16x2((uint16_t)af[j][0]), u0 = cvt_e4m3x2_f16x2((uint16_t)af[j][1]);
+                const uint32_t g1 = cvt_e4m3x2_f16x2((uint16_t)(af[j][0] >> 16)), u1 = cvt_e4m3x2_f16x2((uint16_t)(af[j][1] >> 16));
+                const uint32_t g2 = cvt_e4m3x2_f16x2((uint16_t)af[j][2]), u2 = cvt_e4m3x2_f16x2((uint16_t)af[j][3]);
+                const uint32_t g3 = cvt_e4m3x2_f16x2((uint16_t)(af[j][2] >> 16)), u3 = cvt_e4m3x2_f16x2((uint16_t)(af[j][3] >> 16));
+                if (j < 2) {
+                  mma_f16_16816_zero(c8[(2 * j) & 3], g0, u0, g1, u1, bf[2 * j].x, bf[2 * j].y);
+                  mma_f16_16816_zero(c8[(2 * j + 1) & 3], g2, u2, g3, u3, bf[2 * j + 1].x, bf[2 * j + 1].y);
+                } else {
+                  mma_f16_16816(c8[(2 * j) & 3], g0, u0, g1, u1, bf[2 * j].x, bf[2 * j].y);
+                  mma_f16_16816(c8[(2 * j + 1) & 3], g2, u2, g3, u3, bf[2 * j + 1].x, bf[2 * j + 1].y);
+                }
+              }
+              const float sg = lds_f32(gbase + sc + (uint32_t)kb * 4u), su = lds_f32(ubase + sc + (uint32_t)kb * 4u);
+              tot8[0] = fmaf(sg, (c8[0][0] + c8[1][0]) + (c8[2][0] + c8[3][0]), tot8[0]);
+              tot8[1] = fmaf(sg, (c8[0][1] + c8[1][1]) + (c8[2][1] + c8[3][1]), tot8[1]);
+              tot8[2] = fmaf(su, (c8[0][2] + c8[1][2]) + (c8[2][2] + c8[3][2]), tot8[2]);
+              tot8[3] = fmaf(su, (c8[0][3] + c8[1][3]) + (c8[2][3] + c8[3][3]), tot8[3]);
             }
-            float c8[4][4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) { c8[j][0] = 0.f; c8[j][1] = 0.f; c8[j][2] = 0.f; c8[j][3] = 0.f; }
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              // registers 0/1: gate / up codes of step 2j; registers 2/3: of step 2j + 1
-              mma_f16_16816(c8[(2 * j) & 3], cvt_e4m3x2_f16x2((uint16_t)af[j][0]), cvt_e4m3x2_f16x2((uint16_t)af[j][1]),
-                            cvt_e4m3x2_f16x2((uint16_t)(af[j][0] >> 16)), cvt_e4m3x2_f16x2((uint16_t)(af[j][1] >> 16)), bf[2 * j].x, bf[2 * j].y);
-              mma_f16_16816(c8[(2 * j + 1) & 3], cvt_e4m3x2_f16x2((uint16_t)af[j][2]), cvt_e4m3x2_f16x2((uint16_t)af[j][3]),
-                            cvt_e4m3x2_f16x2((uint16_t)(af[j][2] >> 16)), cvt_e4m3x2_f16x2((uint16_t)(af[j][3] >> 16)), bf[2 * j + 1].x, bf[2 * j + 1].y);
-            }
-            const float sg = lds_f32(gbase + sc + (uint32_t)kb * 4u), su = lds_f32(ubase + sc + (uint32_t)kb * 4u);
-            tot8[0] = fmaf(sg, (c8[0][0] + c8[1][0]) + (c8[2][0] + c8[3][0]), tot8[0]);
-            tot8[1] = fmaf(sg, (c8[0][1] + c8[1][1]) + (c8[2][1] + c8[3][1]), tot8[1]);
-            tot8[2] = fmaf(su, (c8[0][2] + c8[1][2]) + (c8[2][2] + c8[3][2]), tot8[2]);
-            tot8[3] = fmaf(su, (c8[0][3] + c8[1][3]) + (c8[2][3] + c8[3][3]), tot8[3]);
+          }
+          if (g.merge) {                                         // (n_slab == 1) sub-block sbi is complete: hand its tile to the reducer
+            *reinterpret_cast<float4*>(fs.red[par][sbi] + warp * 128 + lane * 4) = make_float4(tot8[0], tot8[1], tot8[2], tot8[3]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&fs.red_full[par][sbi]));
           }
         }
-        if (s == g.n_slab - 1) *reinterpret_cast<float4*>(red + lane * 4) = make_float4(tot8[0], tot8[1], tot8[2], tot8[3]);
+        if (!g.merge && s == g.n_slab - 1) *reinterpret_cast<float4*>(red + lane * 4) = make_float4(tot8[0], tot8[1], tot8[2], tot8[3]);
       } else if constexpr (kMma) {
         const int tok = col < cnt ? (int)(((float)pl[col] + 0.5f) * a.inv_k) : -1;   // token of MMA column `col` (-1: operand 0)
         const uint32_t abase = ((lane >> 3) & 1 ? ubase : gbase) + (uint32_t)(lane & 7) * 16u + (uint32_t)(lane >> 4) * 128u +
@@ -496,9 +515,11 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
       store_part(DecPart{1, sb, s});
       release();                                               // up part
       }
-      __syncwarp();                                            // the sub-block's partial tile is complete: tell the reducer
-      if (lane == 0) mbar_arrive(smem_u32(&fs.red_full[par][sb]));
-      if (sb == g.n_sb - 1) ++gu_seq;
+      if (!(F8 && g.merge)) {
+        __syncwarp();                                          // the sub-block's partial tile is complete: tell the reducer
+        if (lane == 0) mbar_arrive(smem_u32(&fs.red_full[par][sb]));
+      }
+      if (sb == g.n_sb - 1 || (F8 && g.merge)) ++gu_seq;
     } else {
       // ================= down group of slab s: P[pair][c][j] = sum_{i in chunk} a_i * D[j][i] for the outputs j of the slab =================
       const int s = s0;
@@ -509,10 +530,12 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
 #pragma unroll
         for (int t = 0; t < kDecMaxSteps; ++t) { yacc[t][0] = 0.f; yacc[t][1] = 0.f; yacc[t][2] = 0.f; yacc[t][3] = 0.f; }
       }
+      const bool mg = F8 && g.merge != 0;                       // one part holds the down columns of every sub-block
       for (int sb = 0; sb < g.n_sb; ++sb) {
-      if (sb > 0) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
-      const uint32_t dbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
-      store_part(DecPart{2, sb, s});
+      if (sb > 0 && !mg) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
+      const uint32_t pbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
+      const uint32_t dbase = pbase + (mg ? (uint32_t)sb * (uint32_t)g.sub_bytes : 0u);
+      if (!mg || sb == 0) store_part(DecPart{2, mg ? 0 : sb, s});
       const AT* act = reinterpret_cast<const AT*>(fs.act[par][sb]);
       if constexpr (F8) {
         // a down core is 8 outputs x 8 act columns (64 bytes): lane quarters 0 / 1 hold columns 0-3 / 4-7 of outputs g and g + 8 and
@@ -533,7 +556,7 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
             }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-              const uint32_t l = on ? lo[j] : 0u, h = on ? hi[j] : 0u;
+              const uint32_t l = lo[j], h = hi[j];             // (quarters 2 / 3 re-read quarter 0 / 1's finite codes against B = 0)
               mma_f16_16816(yacc[t0 + j], cvt_e4m3x2_f16x2((uint16_t)l), cvt_e4m3x2_f16x2((uint16_t)h), cvt_e4m3x2_f16x2((uint16_t)(l >> 16)),
                             cvt_e4m3x2_f16x2((uint16_t)(h >> 16)), b0, b1);
             }
@@ -543,21 +566,26 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
         if (sb == g.n_sb - 1) {
 #pragma unroll
           for (int i = 0; i < kDecMaxSteps / 8; ++i)
-            s2v[i] = i * 8 < g.steps ? lds_f32(dbase + (uint32_t)g.part_bytes + (uint32_t)(warp * (g.steps >> 3) + i) * 4u) : 0.f;
+            s2v[i] = i * 8 < g.steps ? lds_f32(pbase + (uint32_t)g.part_bytes + (uint32_t)(warp * (g.steps >> 3) + i) * 4u) : 0.f;
         }
-        release();
+        if (!mg || sb == g.n_sb - 1) release();
         if (sb == g.n_sb - 1) {
-          const float as0 = fs.ascale[par][kq], as1 = fs.ascale[par][kq + 1];
           const int j0 = s * g.slab + warp * (g.slab >> 3) + col;
           float* p0 = a.partial + ((size_t)(pos0 + kq) * g.n_chunks + c) * g.d + j0;
           float* p1 = p0 + (size_t)g.n_chunks * g.d;
+          if (kq < cnt) {                                      // (cnt is uniform over the warp: with one token only quarter 0 stores)
+            const float as0 = fs.ascale[par][kq];
+            const float sc[kDecMaxSteps / 8] = {s2v[0] * as0, s2v[1] * as0};
 #pragma unroll
-          for (int t = 0; t < kDecMaxSteps; ++t) {
-            if (t < g.steps) {
-              const float sc0 = s2v[t >> 3] * as0, sc1 = s2v[t >> 3] * as1;
-              if (kq < cnt) { p0[t * 16] = yacc[t][0] * sc0; p0[t * 16 + 8] = yacc[t][2] * sc0; }
-              if (kq + 1 < cnt) { p1[t * 16] = yacc[t][1] * sc1; p1[t * 16 + 8] = yacc[t][3] * sc1; }
-            }
+            for (int t = 0; t < kDecMaxSteps; ++t)
+              if (t < g.steps) { p0[t * 16] = yacc[t][0] * sc[t >> 3]; p0[t * 16 + 8] = yacc[t][2] * sc[t >> 3]; }
+          }
+          if (cnt > 1 && kq + 1 < cnt) {
+            const float as1 = fs.ascale[par][kq + 1];
+            const float sc[kDecMaxSteps / 8] = {s2v[0] * as1, s2v[1] * as1};
+#pragma unroll
+            for (int t = 0; t < kDecMaxSteps; ++t)
+              if (t < g.steps) { p1[t * 16] = yacc[t][1] * sc[t >> 3]; p1[t * 16 + 8] = yacc[t][3] * sc[t >> 3]; }
           }
         }
       } else if constexpr (kMma) {

@@ -323,9 +323,11 @@ DecodeGeom make_decode_geom(int d, int dff, size_t elem, int rows_unit, bool f8 
   while (q % m) --m;
   g.slab = 256 * m;
   g.n_slab = d / g.slab;
-  g.part_bytes = 8 * g.slab * (int)elem;
   g.rows_unit = rows_unit;
   g.n_sb = rows_unit / 8;
+  g.sub_bytes = 8 * g.slab * (int)elem;
+  g.merge = f8 && g.n_slab == 1 && g.n_sb * g.sub_bytes <= kDecMaxPartBytes ? 1 : 0;
+  g.part_bytes = g.sub_bytes * (g.merge ? g.n_sb : 1);
   g.n_chunks = dff / rows_unit;
   g.parts_unit = 3 * g.n_sb * g.n_slab;
   g.steps = g.slab / 128;
@@ -907,7 +909,7 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
     // Work-unit size of the decode FFN: 8 act rows (96 KiB of weights at the Qwen3 shape) for calls of at most 2 tokens, 16
     // for 3..8 tokens, where more experts are in flight and every routed pair writes its own chunk partials.  fp32 models
     // (config 1, parity only) always use 8.
-    const int r0 = cfg->unit_rows > 0 && cfg->dtype != WISP_F32 ? cfg->unit_rows : 8;
+    const int r0 = cfg->unit_rows > 0 && cfg->dtype != WISP_F32 ? cfg->unit_rows : ctx->f8 ? 16 : 8;   // fp8: half the bytes per row
     const int r1 = cfg->dtype == WISP_F32 ? 8 : cfg->unit_rows > 0 ? cfg->unit_rows : 16;
     ctx->dgeom[0] = make_decode_geom(d, dff, ctx->welem, r0, ctx->f8);
     ctx->dgeom[1] = make_decode_geom(d, dff, ctx->welem, r1, ctx->f8);
