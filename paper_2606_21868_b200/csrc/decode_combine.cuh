@@ -42,6 +42,26 @@ __device__ __forceinline__ void slice_logits(const T* w16, const float* xn, int 
   }
 }
 
+// The same for `ns` tokens at once (their fp32 images in xn[s][16]): each thread reads its 16 weights once.  Per token the
+// arithmetic is slice_logits' (fmaf in ascending j from 0.f).
+template <typename T, int S>
+__device__ __forceinline__ void slice_logits_multi(const T* w16, const float* xn, int ns, int E, long long* zfix_t0, int tid, int nthr) {
+  for (int e = tid; e < E; e += nthr) {
+    float wv[kSliceCols];
+#pragma unroll
+    for (int jj = 0; jj < kSliceCols; ++jj) wv[jj] = to_f32<T>(w16[(size_t)jj * E + e]);
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      if (s < ns) {
+        float zp = 0.f;
+#pragma unroll
+        for (int jj = 0; jj < kSliceCols; ++jj) zp = fmaf(wv[jj], xn[s * kSliceCols + jj], zp);
+        atomicAdd(reinterpret_cast<unsigned long long*>(zfix_t0 + (size_t)s * E + e), (unsigned long long)logit_to_fix(zp));
+      }
+    }
+  }
+}
+
 struct CombineArgs {
   const float* partial;      // P [pair position][NC][d]
   int n_chunks, d, k;
@@ -97,6 +117,72 @@ __device__ __forceinline__ void combine_slice(const CombineArgs& a, int t, int j
     if (x_row) o = from_f32<T>(to_f32<T>(x_row[j0 + tid]) + to_f32<T>(o));
     dst_row[j0 + tid] = o;
     s_xn[tid] = to_f32<T>(o);
+  }
+  asm volatile("bar.sync %0, 256;" ::"r"(bar) : "memory");
+}
+
+// The slices (t0 .. t0+ns-1, columns j0 .. j0+15) of up to S tokens in ONE pass: the partial loads of all of them are in flight
+// together (a decode batch's combine is bound by L2 round trips, not by bytes).  Per slice the arithmetic, and so every bit, is
+// combine_slice's: 8 groups of consecutive chunks (warp = group), ascending inside a group from its first partial, groups
+// ascending, ranks in order.  U: chunk loads per thread and slice in flight.
+//   x_base / xs_pitch: the tokens' hidden states (row t at x_base + t * xs_pitch) or nullptr; dst_base: result rows [t][d]
+//   s_yg: S * 8 * 8 * 16 floats, s_y: S * kMaxTopK * 16 floats, s_xn: S * 16 floats
+template <typename T, int S, int U>
+__device__ __forceinline__ void combine_tokens(const CombineArgs& a, int t0, int ns, int j0, const T* x_base, int xs_pitch, T* dst_base,
+                                               float* s_yg, float* s_y, float* s_xn, int bar) {
+  const int tid = threadIdx.x, grp = tid >> 5, lane = tid & 31, ri = lane >> 2, j4 = (lane & 3) * 4;
+  const int per = a.n_chunks >> 3;
+  for (int i0 = 0; i0 < a.k; i0 += 8) {
+    const int rank = i0 + ri;
+    float4 acc[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) acc[s] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (rank < a.k) {
+      const float* src[S];
+#pragma unroll
+      for (int s = 0; s < S; ++s) {
+        const int pos = a.pair_pos[min(t0 + s, t0 + ns - 1) * a.k + rank];
+        src[s] = a.partial + ((size_t)pos * a.n_chunks + (size_t)grp * per) * a.d + j0 + j4;
+      }
+      for (int c0 = 0; c0 < per; c0 += U) {
+        float4 v[S][U];
+#pragma unroll
+        for (int s = 0; s < S; ++s)
+#pragma unroll
+          for (int u = 0; u < U; ++u) v[s][u] = __ldcg(reinterpret_cast<const float4*>(src[s] + (size_t)min(c0 + u, per - 1) * a.d));
+#pragma unroll
+        for (int s = 0; s < S; ++s)
+#pragma unroll
+          for (int u = 0; u < U; ++u)
+            if (c0 + u < per) {
+              if (c0 + u == 0) acc[s] = v[s][0];
+              else { acc[s].x += v[s][u].x; acc[s].y += v[s][u].y; acc[s].z += v[s][u].z; acc[s].w += v[s][u].w; }
+            }
+      }
+    }
+#pragma unroll
+    for (int s = 0; s < S; ++s) *reinterpret_cast<float4*>(s_yg + ((s * 8 + grp) * 8 + ri) * kSliceCols + j4) = acc[s];
+    asm volatile("bar.sync %0, 256;" ::"r"(bar) : "memory");
+    if (tid < 32 * ns && rank < a.k) {                          // warp s adds the 8 group sums of slice s, ascending
+      const float* yg = s_yg + (size_t)grp * 8 * 8 * kSliceCols;
+      float4 y = *reinterpret_cast<const float4*>(yg + ri * kSliceCols + j4);
+#pragma unroll
+      for (int g = 1; g < 8; ++g) {
+        const float4 v = *reinterpret_cast<const float4*>(yg + (g * 8 + ri) * kSliceCols + j4);
+        y.x += v.x; y.y += v.y; y.z += v.z; y.w += v.w;
+      }
+      *reinterpret_cast<float4*>(s_y + ((size_t)grp * kMaxTopK + rank) * kSliceCols + j4) = y;
+    }
+    asm volatile("bar.sync %0, 256;" ::"r"(bar) : "memory");
+  }
+  if (tid < kSliceCols * ns) {
+    const int s = tid >> 4, col = tid & 15, t = t0 + s;
+    float acc = 0.f;
+    for (int i = 0; i < a.k; ++i) acc = fmaf(a.topw[t * a.k + i], s_y[((size_t)s * kMaxTopK + i) * kSliceCols + col], acc);
+    T o = from_f32<T>(acc);
+    if (x_base) o = from_f32<T>(to_f32<T>(x_base[(size_t)t * xs_pitch + j0 + col]) + to_f32<T>(o));
+    dst_base[(size_t)t * a.d + j0 + col] = o;
+    s_xn[s * kSliceCols + col] = to_f32<T>(o);
   }
   asm volatile("bar.sync %0, 256;" ::"r"(bar) : "memory");
 }

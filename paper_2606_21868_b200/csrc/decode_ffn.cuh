@@ -221,6 +221,7 @@ __device__ __forceinline__ bool mbar_wait_or_abort(uint32_t bar, uint32_t parity
 // The first unit of CTA b is b (no atomic on the critical path of a phase start), later ones come from the ticket counter.
 // Part order in the ring: gate/up parts of unit i+1 (sub-block major, slab minor, gate before up), then the down parts of
 // unit i (slab major, sub-block minor), ..., the down parts of the last unit, an END marker.
+template <bool F8>
 __device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const DecodeGeom& g, const PlanPtrs& plan, DecFfnShared& fs,
                                                const DecRing& ring, DecRingPos& rp, int lo, int nw, uint64_t pol) {
   const int n_units = nw * g.n_chunks;
@@ -228,11 +229,11 @@ __device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const Dec
     if (!mbar_wait_or_abort(ring.empty0 + 8u * rp.s, rp.ph ^ 1u, &fs.abort)) return false;
     fs.meta[rp.s] = part_meta(pt.mat, pt.sb, pt.slab, c, q);
     const uint32_t bar = ring.full0 + 8u * rp.s, dst = ring.slot0 + (uint32_t)rp.s * ring.stride;
-    mbar_expect_tx(bar, (uint32_t)g.slot_bytes);
+    mbar_expect_tx(bar, F8 ? (uint32_t)g.slot_bytes : (uint32_t)g.part_bytes);
     const int np = pt.mat == 2 ? g.down_pieces : 1;
     const uint32_t pb = (uint32_t)g.part_bytes / np;
     for (int piece = 0; piece < np; ++piece) bulk_g2s(dst + piece * pb, blob + dec_part_offset(g, c, pt, piece), pb, bar, pol);
-    if (g.scale_bytes) bulk_g2s(dst + (uint32_t)g.part_bytes, blob + dec_scale_offset(g, c, pt), (uint32_t)g.scale_bytes, bar, pol);
+    if constexpr (F8) bulk_g2s(dst + (uint32_t)g.part_bytes, blob + dec_scale_offset(g, c, pt), (uint32_t)g.scale_bytes, bar, pol);
     ring_advance(ring, rp);
     return true;
   };
@@ -244,7 +245,7 @@ __device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const Dec
   auto emit_down = [&](int q, int c) -> bool {
     const char* blob = blob_of(q);
     for (int s = 0; s < g.n_slab; ++s)
-      for (int sb = 0; sb < (g.merge ? 1 : g.n_sb); ++sb)
+      for (int sb = 0; sb < (F8 && g.merge ? 1 : g.n_sb); ++sb)
         if (!emit(blob, q, c, DecPart{2, sb, s})) return false;
     return true;
   };
@@ -253,7 +254,7 @@ __device__ __forceinline__ void decode_produce(const DecodeFfnArgs& a, const Dec
     const unsigned t = atomicAdd(a.ticket, 1u);                // next unit: its latency hides behind this unit's copies
     const int q = plan.unit_entry[lo + u / g.n_chunks], c = u % g.n_chunks;
     const char* blob = blob_of(q);
-    for (int sb = 0; sb < (g.merge ? 1 : g.n_sb); ++sb)
+    for (int sb = 0; sb < (F8 && g.merge ? 1 : g.n_sb); ++sb)
       for (int s = 0; s < g.n_slab; ++s) {
         if (!emit(blob, q, c, DecPart{0, sb, s})) return;
         if (!emit(blob, q, c, DecPart{1, sb, s})) return;
@@ -373,7 +374,7 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
         const int np = pt.mat == 2 ? g.down_pieces : 1;
         const uint32_t pb = (uint32_t)g.part_bytes / np, src = ring.slot0 + (uint32_t)rp.s * ring.stride;
         for (int piece = 0; piece < np; ++piece) bulk_s2g(slot_blob + dec_part_offset(g, c, pt, piece), src + piece * pb, pb);
-        if (g.scale_bytes) bulk_s2g(slot_blob + dec_scale_offset(g, c, pt), src + (uint32_t)g.part_bytes, (uint32_t)g.scale_bytes);
+        if constexpr (F8) bulk_s2g(slot_blob + dec_scale_offset(g, c, pt), src + (uint32_t)g.part_bytes, (uint32_t)g.scale_bytes);
         bulk_commit();
       }
     };

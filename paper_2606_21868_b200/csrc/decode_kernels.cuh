@@ -30,6 +30,7 @@ namespace wisp {
 constexpr int kPersistMaxExperts = 256;     // plan capacity of the fused kernel (larger E -> split form)
 constexpr int kDecPhases = 6;               // route, plan, prefetch of the next layer's state, ffn, ffn of layers with misses, combine
 constexpr unsigned kGridBarrierSpinLimit = 1u << 24;
+constexpr int kCombineBatch = 4;            // tokens whose slices of one column block a CTA combines in one pass
 
 struct DecodeArgs {
   int L, E, k, d, dff, T, C, policy;
@@ -109,14 +110,15 @@ __device__ __forceinline__ bool grid_barrier(unsigned* ctr, unsigned& gen, volat
 struct DecShared {
   unsigned long long go;                                  // the plan of the next wave exists: the producer may stream
   unsigned long long wpre;                                // the next layer's router-weight slice has landed in shared memory
-  alignas(16) float y[kMaxTopK * kSliceCols];
-  float xn[kSliceCols];
+  alignas(16) float y[kCombineBatch * kMaxTopK * kSliceCols];   // combine: per-rank sums of up to kCombineBatch slices
+  float xn[kCombineBatch * kSliceCols];
   int ids[kDecodeMaxTokens * kMaxTopK];
   float w[kDecodeMaxTokens * kMaxTopK];
   DecPlan pl;
 };
 
-template <typename T, bool F8>
+// MULTI: the launch has more than one token (adds the batched combine; the one-token instantiation keeps its registers).
+template <typename T, bool F8, bool MULTI>
 __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const DecodeArgs a, const DecodeGeom g, int n_slots, int xs_pitch,
                                                                       int pre_off, int ring_off) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -159,7 +161,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
         n_waves = ds.pl.hdr[0];
         const int nR = ds.pl.hdr[1], lo = w * C, nw = min(nR, lo + C) - lo;
         fa.ticket = a.sync + 1 + (qseq & 1u);
-        decode_produce(fa, g, pp, fs, ring, rp, lo, nw, pol);
+        decode_produce<F8>(fa, g, pp, fs, ring, rp, lo, nw, pol);
         if (fs.abort) return;
       }
     }
@@ -276,7 +278,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     const int miss_cls = ds.pl.hdr[2] > 0 ? 1 : 0;             // layers with misses are timed apart
     // this CTA's first combine slice is known now: its 16 rows of the NEXT layer's router weights (one contiguous block of
     // [d][E]) are staged in shared memory by a bulk copy while the FFN streams
-    const bool pre = !last && (int)blockIdx.x < n_slices;
+    const bool pre = !last && (int)blockIdx.x < d / kSliceCols;
     if (tid == 0) {
       if (writer) a.sync[1 + ((qseq + 1) & 1u)] = 0u;          // ticket counter of the NEXT wave (idle since the wave before this one)
       mbar_arrive(smem_u32(&ds.go));                           // the producer may start streaming
@@ -321,16 +323,30 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
       T* xg = reinterpret_cast<T*>(last ? a.out : a.xbuf[(l - a.layer_lo) & 1]);
       const T* wrt = reinterpret_cast<const T*>(a.router_wt) + (size_t)(l + 1) * d * E;
       long long* zf_n = a.zfix + (size_t)((l + 1) & 1) * kDecodeMaxTokens * E;
-      for (int sl = blockIdx.x; sl < n_slices; sl += gridDim.x) {
-        const int t = sl / (d / kSliceCols), j0 = (sl % (d / kSliceCols)) * kSliceCols;
-        combine_slice<T>(ca, t, j0, a.residual ? xs + (size_t)t * xs_pitch : nullptr, xg + (size_t)t * d, fs.red[0][0], ds.y, ds.xn, 1);
-        if (!last) {
-          const T* w16 = wrt + (size_t)j0 * E;
-          if (sl == (int)blockIdx.x) {                         // the staged slice
-            mbar_wait(smem_u32(&ds.wpre), (unsigned)(l - a.layer_lo) & 1u);
-            w16 = reinterpret_cast<const T*>(smem_raw + pre_off + w_off);
+      // CTA b owns the column blocks b, b + grid, ... of EVERY token: the tokens of a block are combined kCombineBatch at a time (their
+      // partial loads in flight together) and share the block's 16 rows of router weights (staged for the CTA's first block)
+      const int n_jb = d / kSliceCols;
+      for (int jb = blockIdx.x; jb < n_jb; jb += gridDim.x) {
+        const int j0 = jb * kSliceCols;
+        const T* w16 = wrt + (size_t)j0 * E;
+        if (!last && jb == (int)blockIdx.x) {
+          mbar_wait(smem_u32(&ds.wpre), (unsigned)(l - a.layer_lo) & 1u);
+          w16 = reinterpret_cast<const T*>(smem_raw + pre_off + w_off);
+        }
+        for (int t0 = 0; t0 < T_; t0 += MULTI ? kCombineBatch : 1) {
+          const int ns = MULTI ? min(kCombineBatch, T_ - t0) : 1;
+          const T* xres = a.residual ? xs : nullptr;
+          if (!MULTI || ns == 1) {
+            combine_slice<T>(ca, t0, j0, xres ? xres + (size_t)t0 * xs_pitch : nullptr, xg + (size_t)t0 * d, fs.red[0][0], ds.y, ds.xn, 1);
+            if (!last) slice_logits<T>(w16, ds.xn, E, zf_n + (size_t)t0 * E, tid, kDecConsumers);
+          } else if constexpr (!MULTI) {
+          } else if (ns == 2) {
+            combine_tokens<T, 2, 6>(ca, t0, ns, j0, xres, xs_pitch, xg, fs.red[0][0], ds.y, ds.xn, 1);
+            if (!last) slice_logits_multi<T, 2>(w16, ds.xn, ns, E, zf_n + (size_t)t0 * E, tid, kDecConsumers);
+          } else {
+            combine_tokens<T, kCombineBatch, 3>(ca, t0, ns, j0, xres, xs_pitch, xg, fs.red[0][0], ds.y, ds.xn, 1);
+            if (!last) slice_logits_multi<T, kCombineBatch>(w16, ds.xn, ns, E, zf_n + (size_t)t0 * E, tid, kDecConsumers);
           }
-          slice_logits<T>(w16, ds.xn, E, zf_n + (size_t)t * E, tid, kDecConsumers);
         }
       }
       if (!last) {
@@ -434,7 +450,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_ffn_kernel(DecodeFfnArg
   if (warp == kDecWarps + 1) {
     decode_reduce<T, F8>(g, fs, lane);
   } else if (warp == kDecWarps) {
-    if (lane == 0) decode_produce(fa, g, pp, fs, ring, rp, lo, nw, l2_evict_first_policy());
+    if (lane == 0) decode_produce<F8>(fa, g, pp, fs, ring, rp, lo, nw, l2_evict_first_policy());
   } else {
     unsigned gu_seq = 0, d_seq = 0;
     decode_consume<T, F8>(fa, g, pp, fs, ring, rp, gu_seq, d_seq, xs, xh, xs_pitch);

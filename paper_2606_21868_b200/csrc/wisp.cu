@@ -394,7 +394,7 @@ int launch_fused(wisp_ctx* ctx, int lo, int hi, const void* x, int T_, void* out
   if (rc) return rc;
   CK(cudaMemsetAsync(ctx->dsync, 0, 4 * sizeof(unsigned), st));
   void* args[] = {&pa, &g, &sm.n_slots, &sm.xs_pitch, &sm.pre_off, &sm.ring_off};
-  CK(cudaLaunchCooperativeKernel((const void*)decode_fused_kernel<T, F8>, dim3(ctx->num_sms), dim3(kDecThreads), args, sm.bytes, st));
+  CK(cudaLaunchCooperativeKernel(T_ > 1 ? (const void*)decode_fused_kernel<T, F8, true> : (const void*)decode_fused_kernel<T, F8, false>, dim3(ctx->num_sms), dim3(kDecThreads), args, sm.bytes, st));
   ++ctx->launches;
   for (int l = lo; l < hi; ++l) ctx->last_T[l] = T_;
   ctx->last_layer = hi - 1;
@@ -918,13 +918,16 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
     const size_t n_part = std::max(pairs0 * ctx->dgeom[0].n_chunks, pairs1 * ctx->dgeom[1].n_chunks) * d;
     CKC(cudaMalloc(&ctx->partial, n_part * sizeof(float)));
     cudaFuncAttributes fa;
-    const void* kf = ctx->f8 ? (const void*)decode_fused_kernel<__nv_bfloat16, true>
-                     : cfg->dtype == WISP_F32 ? (const void*)decode_fused_kernel<float, false> : (const void*)decode_fused_kernel<__nv_bfloat16, false>;
+    const void* kf = ctx->f8 ? (const void*)decode_fused_kernel<__nv_bfloat16, true, false>
+                     : cfg->dtype == WISP_F32 ? (const void*)decode_fused_kernel<float, false, false> : (const void*)decode_fused_kernel<__nv_bfloat16, false, false>;
+    const void* kf2 = ctx->f8 ? (const void*)decode_fused_kernel<__nv_bfloat16, true, true>
+                      : cfg->dtype == WISP_F32 ? (const void*)decode_fused_kernel<float, false, true> : (const void*)decode_fused_kernel<__nv_bfloat16, false, true>;
     const void* kn = ctx->f8 ? (const void*)decode_ffn_kernel<__nv_bfloat16, true>
                      : cfg->dtype == WISP_F32 ? (const void*)decode_ffn_kernel<float, false> : (const void*)decode_ffn_kernel<__nv_bfloat16, false>;
     CKC(cudaFuncGetAttributes(&fa, kf));
     ctx->fused_smem = (227u << 10) - fa.sharedSizeBytes;
     CKC(cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->fused_smem));
+    CKC(cudaFuncSetAttribute(kf2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->fused_smem));
     CKC(cudaFuncGetAttributes(&fa, kn));
     ctx->ffn_smem = (227u << 10) - fa.sharedSizeBytes;
     CKC(cudaFuncSetAttribute(kn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->ffn_smem));
