@@ -246,6 +246,19 @@ int wisp_trace_read(wisp_ctx* ctx, wisp_trace_event* buf, uint64_t cap, uint64_t
 int wisp_last_topk(wisp_ctx* ctx, int32_t layer, int32_t* ids, float* w, int32_t* n_tokens_out);
 /* Router logits of the most recent forward overall: host z [n_tokens, E] fp32.  Synchronises. */
 int wisp_last_logits(wisp_ctx* ctx, float* z, int32_t n_tokens);
+/* The router step of one layer (a1: logits, top-k ids in (z desc, id asc) order, softmax over the selected k) for a small token
+ * batch WITHOUT any allocation -- for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses
+ * that forbid it).  No context: the caller passes every input and output; the only scratch (the 2^-40 fixed-point int64 logit
+ * accumulators of the decode path) is a file-scope device array of 8192 words = 64 KiB that every GPU loading the library holds
+ * until exit.  Same arithmetic as the context's decode path, so the results equal wisp_last_logits / wisp_last_topk bit for bit.
+ *   hidden       device, [n_tokens, d_model] row-major, `dtype` (WISP_F32 or WISP_BF16)
+ *   router_w     device, [n_experts, d_model] row-major, `dtype`;  router_bias  device, [n_experts] fp32, or NULL (zeros)
+ *   logits       device, [n_tokens, n_experts] fp32 out, or NULL;  ids  device, [n_tokens, top_k] int32 out;  w  device, [n_tokens, top_k] fp32 out
+ * Limits: n_tokens * n_experts <= 8192 (else WISP_EINVAL, with the reason on stderr), n_experts <= 1024, top_k <= min(E, 32),
+ * d_model a multiple of 16.  Calls no cudaMalloc / cudaFree; work is queued on `cuda_stream` (memset + two kernels), not synchronised.
+ * All calls share the scratch array (each clears the words it uses first): calls that overlap on the GPU race -- serialise them. */
+int wisp_route_noalloc(const void* hidden, const void* router_w, const float* router_bias, int32_t n_tokens, int32_t n_experts,
+                       int32_t d_model, int32_t top_k, int32_t dtype, float* logits, int32_t* ids, float* w, void* cuda_stream);
 /* Drive the pager with a given routed-id list (host, n_ids ids, repeats allowed): runs the residency
  * lookup and the demand fetch of one step of `layer`, no router and no FFN.  Synchronises. */
 int wisp_debug_step_routing(wisp_ctx* ctx, int32_t layer, const int32_t* ids, int32_t n_ids);

@@ -7,5 +7,5 @@ fails with WISP_ECUDA without a CUDA device.
 """
 from .binding import (  # noqa: F401
     WISP_BF16, WISP_F32, WISP_FP8_E4M3, WISP_FETCH_FUSED, WISP_FETCH_MEMCPY, WISP_FETCH_STATIC, WISP_FETCH_ZEROCOPY, WISP_LFU, WISP_LRU, WISP_WAVES_ASCENDING, WISP_WAVES_HITS_FIRST, WispConfig, WispError,
-    WispLayerStats, WispMvwsaIn, WispStats, WispTraceEvent, Wisp, lib, lib_path, STATUS_NAMES, KERNEL_CLASSES,
+    WispLayerStats, WispMvwsaIn, WispStats, WispTraceEvent, Wisp, lib, lib_path, route_noalloc, STATUS_NAMES, KERNEL_CLASSES,
 )

@@ -74,6 +74,8 @@ _SIGS = {
     "wisp_trace_read": (C.c_int, [C.c_void_p, C.POINTER(WispTraceEvent), C.c_uint64, C.POINTER(C.c_uint64)]),
     "wisp_last_topk": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]),
     "wisp_last_logits": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32]),
+    "wisp_route_noalloc": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
+                                     C.c_void_p, C.c_void_p, C.c_void_p]),
     "wisp_debug_step_routing": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_int32]),
     "wisp_debug_reset_pool": (C.c_int, [C.c_void_p]),
     "wisp_debug_ffn_launch": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]),
@@ -109,6 +111,15 @@ def lib() -> C.CDLL:
 
 def _ptr(t):
     return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def route_noalloc(hidden, router_w, router_bias, top_k, dtype, logits, ids, w, stream):
+    """wisp_route_noalloc: device tensors in and out (hidden [T, d], router_w [E, d], router_bias [E] or None, logits [T, E] or None,
+    ids [T, k] int32, w [T, k] fp32); allocates nothing.  Raises WispError on a non-zero status."""
+    rc = lib().wisp_route_noalloc(_ptr(hidden), _ptr(router_w), _ptr(router_bias), hidden.shape[0], router_w.shape[0], hidden.shape[1],
+                                  top_k, dtype, _ptr(logits), _ptr(ids), _ptr(w), C.c_void_p(stream))
+    if rc:
+        raise WispError(rc, "wisp_route_noalloc")
 
 
 class Wisp:
