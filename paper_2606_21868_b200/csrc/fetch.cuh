@@ -16,7 +16,7 @@ __global__ void __launch_bounds__(kFetchThreads) fetch_zerocopy_kernel(PlanPtrs 
                                                                        const uint4* __restrict__ master,
                                                                        uint4* __restrict__ pool, size_t blob_vec,
                                                                        int L, int layer) {
-  if (wave >= plan.hdr[0]) return;
+  if (wave >= plan.hdr[0] || plan.hdr[2] == 0) return;       // nothing missed in this step: no walk over the entries
   const int lo = wave * C, hi = min(plan.hdr[1], lo + C);
   const size_t chunk_vec = kFetchChunk / 16;
   const size_t chunks_per_blob = (blob_vec + chunk_vec - 1) / chunk_vec;

@@ -121,14 +121,32 @@ template <typename T>
 __global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ ystage, const float* __restrict__ w,
                                                       T* __restrict__ out, const T* __restrict__ x_res,
                                                       T* __restrict__ x_next, int n_tokens, int d, int k) {
-  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= (size_t)n_tokens * d) return;
-  const int t = (int)(idx / d), j = (int)(idx % d);
-  float acc = 0.f;
-  for (int i = 0; i < k; ++i) acc = fmaf(w[(size_t)t * k + i], ystage[((size_t)t * k + i) * d + j], acc);
-  const T o = from_f32<T>(acc);
-  out[idx] = o;
-  if (x_res) x_next[idx] = from_f32<T>(to_f32<T>(x_res[idx]) + to_f32<T>(o));
+  // four consecutive columns per thread (d % 4 == 0): the k float4 loads of a thread are independent and in flight together;
+  // per element the arithmetic is the scalar chain (fmaf in rank order from 0.f)
+  const size_t idx4 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx4 * 4 >= (size_t)n_tokens * d) return;
+  const int t = (int)(idx4 * 4 / d), j = (int)(idx4 * 4 % d);
+  float acc[4] = {0.f, 0.f, 0.f, 0.f};
+  const float4* src = reinterpret_cast<const float4*>(ystage + (size_t)t * k * d + j);
+  for (int i0 = 0; i0 < k; i0 += 8) {
+    float4 v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = __ldcs(src + (size_t)min(i0 + u, k - 1) * (d / 4));
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+      if (i0 + u < k) {
+        const float wi = w[(size_t)t * k + i0 + u];
+        acc[0] = fmaf(wi, v[u].x, acc[0]); acc[1] = fmaf(wi, v[u].y, acc[1]);
+        acc[2] = fmaf(wi, v[u].z, acc[2]); acc[3] = fmaf(wi, v[u].w, acc[3]);
+      }
+  }
+  const size_t idx = idx4 * 4;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const T o = from_f32<T>(acc[c]);
+    out[idx + c] = o;
+    if (x_res) x_next[idx + c] = from_f32<T>(to_f32<T>(x_res[idx + c]) + to_f32<T>(o));
+  }
 }
 
 }  // namespace wisp

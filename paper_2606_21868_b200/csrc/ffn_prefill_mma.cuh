@@ -39,23 +39,23 @@ struct MmaArgs {
   float* z;               // [n_tokens][E] fp32
   const float* bias;      // [E] of this layer
   int n_tokens, E;
+  int b_rows;             // MODE 2: tokens per tile = rows of the B box (32: the router GEMM has few tiles, small ones fill the grid)
 };
 
 struct MmaTile { int pos0, nt, blob, r0; };
-// tile t -> (first B row, valid B rows, weight blob, first weight row)
+// tile t -> (first B row, valid B rows, weight blob, first weight row).  The work list holds one resolved item per
+// (wave entry, token tile): int4 (first sorted pair position, valid pairs, slot of the expert, plan entry) -- ONE 16-byte load per
+// tile (the chain work -> entry_expert -> exp_offset / exp_count / entry_slot cost each role ~2 us of dependent L2 loads per tile).
 template <int MODE>
 __device__ __forceinline__ MmaTile mma_tile(const MmaArgs& a, const int* work, int t, int RT) {
   MmaTile m;
   const int w = t / RT;
-  m.r0 = (t % RT) * kMmaM;
+  m.r0 = (t % RT) * (MODE == 1 ? 2 * kMmaM : kMmaM);           // MODE 1: a tile is TWO 128-row blocks of the down matrix
   if (MODE == 2) {
-    m.pos0 = w * kMmaNT; m.nt = min(kMmaNT, a.n_tokens - m.pos0); m.blob = a.layer;
+    m.pos0 = w * a.b_rows; m.nt = min(a.b_rows, a.n_tokens - m.pos0); m.blob = a.layer;
   } else {
-    const int i = work[2 * w], p0 = work[2 * w + 1];
-    const int e = a.plan.entry_expert[i];
-    m.pos0 = a.plan.exp_offset[e] + p0;
-    m.nt = min(kMmaNT, a.plan.exp_count[e] - p0);
-    m.blob = a.plan.entry_slot[i] * a.L + a.layer;
+    const int4 it = __ldg(reinterpret_cast<const int4*>(work) + w);
+    m.pos0 = it.x; m.nt = it.y; m.blob = it.z * a.L + a.layer;
   }
   return m;
 }
@@ -132,8 +132,8 @@ __device__ __forceinline__ uint32_t umma_idesc_bf16(int M, int N) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
-// Work list of one wave: one item per (wave entry, tile of kMmaNT routed pairs).  work[2*w] = plan entry index,
-// work[2*w+1] = first pair of the tile inside the expert's sorted range; *n_work = item count.  One warp.
+// Work list of one wave: one item per (wave entry, tile of kMmaNT routed pairs), resolved: work4[w] = (first sorted pair
+// position, valid pairs, slot, plan entry index); *n_work = item count.  One warp.
 __global__ void __launch_bounds__(32) build_work_kernel(PlanPtrs plan, int wave, int C, int* __restrict__ work, int* __restrict__ n_work) {
   const int lane = threadIdx.x;
   int n = 0;
@@ -141,13 +141,16 @@ __global__ void __launch_bounds__(32) build_work_kernel(PlanPtrs plan, int wave,
     const int lo = wave * C, hi = min(plan.hdr[1], lo + C);
     for (int i0 = lo; i0 < hi; i0 += 32) {                    // 32 entries at a time: tile counts, warp prefix sum, scatter
       const int i = i0 + lane;
-      const int cnt = i < hi ? plan.exp_count[plan.entry_expert[i]] : 0;
+      const int e = i < hi ? plan.entry_expert[i] : 0;
+      const int cnt = i < hi ? plan.exp_count[e] : 0;
+      const int off = i < hi ? plan.exp_offset[e] : 0, slot = i < hi ? plan.entry_slot[i] : 0;
       const int tiles = (cnt + kMmaNT - 1) / kMmaNT;
       int inc = tiles;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
       int pos = n + inc - tiles;
-      for (int p0 = 0; p0 < cnt; p0 += kMmaNT, ++pos) { work[2 * pos] = i; work[2 * pos + 1] = p0; }
+      for (int p0 = 0; p0 < cnt; p0 += kMmaNT, ++pos)
+        reinterpret_cast<int4*>(work)[pos] = make_int4(off + p0, min(kMmaNT, cnt - p0), slot, i);
       n += __shfl_sync(0xffffffffu, inc, 31);
     }
   }
@@ -166,15 +169,18 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
   extern __shared__ __align__(1024) unsigned char smem_mma[];
   __shared__ __align__(8) unsigned long long s_full[8], s_empty[8], s_tfull[2], s_tempty[2];
   __shared__ uint32_t s_tmem;
-  constexpr int NA = MODE == 0 ? 2 : 1;                       // weight tiles per stage (gate + up | down)
+  // weight tiles per stage: gate + up | two 128-row blocks of down (they share the B tile: the kernels run at the L2->SM rate
+  // of the TMA path, ~12 TB/s chip-wide, so every B re-read that is avoided is time) | router rows
+  constexpr int NA = MODE == 2 ? 1 : 2;
   constexpr uint32_t kStage = (NA + 1) * kMmaTileBytes;
-  constexpr uint32_t kAccCols = MODE == 0 ? 256 : 128;        // TMEM columns of one accumulator stage
+  const uint32_t stage_tx = MODE == 2 ? NA * kMmaTileBytes + (uint32_t)a.b_rows * (kMmaBK * 2) : kStage;   // bytes a stage receives
+  constexpr uint32_t kAccCols = MODE == 2 ? 128 : 256;        // TMEM columns of one accumulator stage
   constexpr uint32_t kCols = 2 * kAccCols;
 
   const int K = MODE == 1 ? a.dff : a.d;
   const int nkb = K / kMmaBK;
-  const int RT = (MODE == 0 ? a.dff : MODE == 1 ? a.d : a.E) / kMmaM;
-  const int n_tiles = (MODE == 2 ? (a.n_tokens + kMmaNT - 1) / kMmaNT : *n_work_p) * RT;
+  const int RT = MODE == 0 ? a.dff / kMmaM : MODE == 1 ? a.d / (2 * kMmaM) : a.E / kMmaM;
+  const int n_tiles = (MODE == 2 ? (a.n_tokens + a.b_rows - 1) / a.b_rows : *n_work_p) * RT;
   if ((int)blockIdx.x >= n_tiles) return;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -193,19 +199,22 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
   if (warp == 0) {
     if (lane == 0) {      // ===== TMA producer =====
       int s = 0; uint32_t ph = 0;
+      MmaTile nxt = mma_tile<MODE>(a, work, blockIdx.x, RT);
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        const MmaTile mt = mma_tile<MODE>(a, work, t, RT);
+        const MmaTile mt = nxt;
+        if (t + (int)gridDim.x < n_tiles) nxt = mma_tile<MODE>(a, work, t + gridDim.x, RT);   // in flight while this tile streams
         const int r0 = mt.r0, pos0 = mt.pos0, blob = mt.blob;
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(smem_u32(&s_empty[s]), ph ^ 1u);
           const uint32_t bar = smem_u32(&s_full[s]);
-          mbar_expect_tx(bar, kStage);
+          mbar_expect_tx(bar, stage_tx);
           const uint32_t base = smem0 + s * kStage;
           if (MODE == 0) {          // (core, core column = K block, core row = row group, blob): gate then up
             tma_load_4d(base, &tm_w, 0, kb * (kMmaBK / 8), r0 / 8, blob, bar);
             tma_load_4d(base + kMmaTileBytes, &tm_w, 0, kb * (kMmaBK / 8), (a.dff + r0) / 8, blob, bar);
           } else if (MODE == 1) {   // (core, output group j/8, act-column block i/8, blob)
             tma_load_4d(base, &tm_w, 0, r0 / 8, kb * (kMmaBK / 8), blob, bar);
+            tma_load_4d(base + kMmaTileBytes, &tm_w, 0, (r0 + kMmaM) / 8, kb * (kMmaBK / 8), blob, bar);
           } else {
             tma_load_3d(base, &tm_w, kb * kMmaBK, r0, blob, bar);
           }
@@ -218,8 +227,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
     if (lane == 0) {      // ===== MMA issuer =====
       int s = 0; uint32_t ph = 0;
       int j = 0;
+      int nt_next = mma_tile<MODE>(a, work, blockIdx.x, RT).nt;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++j) {
-        const int nt = mma_tile<MODE>(a, work, t, RT).nt;
+        const int nt = nt_next;
+        if (t + (int)gridDim.x < n_tiles) nt_next = mma_tile<MODE>(a, work, t + gridDim.x, RT).nt;
         const uint32_t idesc = umma_idesc_bf16(kMmaM, max(16, (nt + 15) & ~15));
         const int as = j & 1;
         mbar_wait(smem_u32(&s_tempty[as]), ((uint32_t)(j >> 1) & 1u) ^ 1u);   // the epilogue has drained this stage
@@ -234,14 +245,14 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
           //    MODE 1 tile = [8 K blocks][16 output groups][128 B] (K-adjacent cores 2 KiB apart, output groups 128 B apart;
           //                   4 KiB per MMA);  MODE 2 (router rows, row-major in global memory) = 128-byte swizzle
           const uint64_t da0 = MODE == 0 ? umma_desc_cores(base, 128u, 1024u) : MODE == 1 ? umma_desc_cores(base, 2048u, 128u) : umma_desc_sw128(base);
-          const uint64_t da1 = umma_desc_cores(base + kMmaTileBytes, 128u, 1024u);
+          const uint64_t da1 = MODE == 1 ? umma_desc_cores(base + kMmaTileBytes, 2048u, 128u) : umma_desc_cores(base + kMmaTileBytes, 128u, 1024u);
           const uint32_t a_step = MODE == 0 ? 256u >> 4 : MODE == 1 ? 4096u >> 4 : 2u;
           const uint64_t db = umma_desc_sw128(base + NA * kMmaTileBytes);
 #pragma unroll
           for (int k4 = 0; k4 < kMmaBK / 16; ++k4) {          // UMMA_K = 16 bf16
             const uint32_t acc = (kb | k4) != 0;
             umma_bf16(acc_base, da0 + a_step * k4, db + 2 * k4, idesc, acc);
-            if (MODE == 0) umma_bf16(acc_base + 128, da1 + a_step * k4, db + 2 * k4, idesc, acc);
+            if (MODE != 2) umma_bf16(acc_base + 128, da1 + a_step * k4, db + 2 * k4, idesc, acc);
           }
           umma_commit(smem_u32(&s_empty[s]));                 // frees the stage once these MMAs have read it
           if (++s == n_stages) { s = 0; ph ^= 1u; }
@@ -252,27 +263,34 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
   } else {                // ===== epilogue warps: TMEM lane quarter = warp % 4 =====
     const int q = warp & 3;
     int j = 0;
+    MmaTile nxt = mma_tile<MODE>(a, work, blockIdx.x, RT);
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++j) {
-      const MmaTile mt = mma_tile<MODE>(a, work, t, RT);
+      const MmaTile mt = nxt;
+      if (t + (int)gridDim.x < n_tiles) nxt = mma_tile<MODE>(a, work, t + gridDim.x, RT);
       const int r0 = mt.r0, pos0 = mt.pos0, nt = mt.nt;
       const int N = max(16, (nt + 15) & ~15);
       const int as = j & 1;
       mbar_wait(smem_u32(&s_tfull[as]), (uint32_t)(j >> 1) & 1u);
       tc_fence_after();
-      const int row = r0 + 32 * q + lane;                     // weight row = d_ff index (MODE 0) | d index (MODE 1)
+      const int row = r0 + 32 * q + lane;                     // weight row = d_ff index (MODE 0) | d index (MODE 1; second block: + 128)
       const uint32_t tlane = tmem + as * kAccCols + ((uint32_t)(32 * q) << 16);
       const int* pl = MODE == 2 ? nullptr : a.plan.pair_list + pos0;
       const float bias_r = MODE == 2 ? a.bias[row] : 0.f;
       for (int c0 = 0; c0 < N; c0 += 16) {
         float g[16], u[16];
+        // MODE 1: the pair ids of these 16 columns in ONE load (lane l holds column c0 + l % 16), handed round by shuffles --
+        // a dependent global load per column was half of this warp's time
+        int my_pair = 0;
+        if (MODE == 1) my_pair = pl[min(c0 + (lane & 15), nt - 1)];
         tmem_ld16(tlane + c0, g);
-        if (MODE == 0) tmem_ld16(tlane + 128 + c0, u);
+        if (MODE != 2) tmem_ld16(tlane + 128 + c0, u);
 #pragma unroll
         for (int jj = 0; jj < 16; ++jj) {
           const int col = c0 + jj;
+          const int pr = MODE == 1 ? __shfl_sync(0xffffffffu, my_pair, jj) : 0;
           if (col < nt) {
             if (MODE == 0) a.act[(size_t)(pos0 + col) * a.dff + row] = __float2bfloat16_rn(silu_f(g[jj]) * u[jj]);
-            else if (MODE == 1) a.ystage[(size_t)pl[col] * a.d + row] = g[jj];
+            else if (MODE == 1) { a.ystage[(size_t)pr * a.d + row] = g[jj]; a.ystage[(size_t)pr * a.d + row + kMmaM] = u[jj]; }
             else a.z[(size_t)(pos0 + col) * a.E + row] = g[jj] + bias_r;
           }
         }
@@ -287,13 +305,22 @@ __global__ void __launch_bounds__(kMmaThreads, 1) prefill_mma_kernel(const __gri
   if (warp == 1) tmem_dealloc(tmem, kCols);
 }
 
-// xg[pos][:] = x[pair_list[pos] / k][:] for every routed pair (sorted by expert): the B operand of GEMM 1.
+// xg[pos][:] = x[pair_list[pos] / k][:] for every routed pair (sorted by expert): the B operand of GEMM 1.  One warp per pair and
+// iteration, the row's 16-byte pieces of a lane loaded before any is stored (8 CTAs x 8 warps per SM keep the copies in flight).
 __global__ void __launch_bounds__(256) gather_tokens_kernel(const int* __restrict__ pair_list, int n_pairs, int k, int d_vec,
                                                             const uint4* __restrict__ x, uint4* __restrict__ xg) {
-  for (int pos = blockIdx.x; pos < n_pairs; pos += gridDim.x) {
-    const uint4* src = x + (size_t)(pair_list[pos] / k) * d_vec;
+  const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+  for (int pos = blockIdx.x * wpb + (threadIdx.x >> 5); pos < n_pairs; pos += gridDim.x * wpb) {
+    const uint4* src = x + (size_t)(__ldg(pair_list + pos) / k) * d_vec;
     uint4* dst = xg + (size_t)pos * d_vec;
-    for (int c = threadIdx.x; c < d_vec; c += blockDim.x) dst[c] = src[c];
+    for (int c0 = lane; c0 < d_vec; c0 += 32 * 8) {
+      uint4 v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) v[u] = __ldg(src + min(c0 + 32 * u, d_vec - 1));
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        if (c0 + 32 * u < d_vec) __stcs(dst + c0 + 32 * u, v[u]);
+    }
   }
 }
 

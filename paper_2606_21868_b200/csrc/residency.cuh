@@ -408,28 +408,40 @@ __global__ void __launch_bounds__(kPlanThreads) residency_plan_kernel(PlanArgs a
   plan_compute<kPlanThreads>(a, sh, /*writer=*/true, /*bar=*/0);
 }
 
-// Stable grouping of (token, rank) pairs by expert for large n_pairs: one CTA of kGroupThreads per expert.
+// Stable grouping of (token, rank) pairs by expert for large n_pairs: one CTA of kGroupThreads per expert, ONE pass: thread t
+// owns the contiguous range of pairs [t * per, (t + 1) * per), counts its matches, an exclusive block scan of the counts gives
+// the position of its first match, and it writes its matches in ascending pair order (so the order inside an expert is ascending).
 constexpr int kGroupThreads = 1024;
 __global__ void __launch_bounds__(kGroupThreads) group_pairs_kernel(const int* __restrict__ ids, int n_pairs, PlanPtrs plan) {
   constexpr int NW = kGroupThreads / 32;
   __shared__ int s_ws[NW];
   const int e = blockIdx.x;
   if (plan.exp_count[e] == 0) return;
-  int pos = plan.exp_offset[e];
+  const int pos0 = plan.exp_offset[e];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (int base = 0; base < n_pairs; base += kGroupThreads) {
-    const int p = base + threadIdx.x;
-    const bool m = p < n_pairs && ids[p] == e;
-    const unsigned bal = __ballot_sync(0xffffffffu, m);
-    if (lane == 0) s_ws[wid] = __popc(bal);
-    __syncthreads();
-    int before = 0, tot = 0;
-#pragma unroll
-    for (int i = 0; i < NW; ++i) { const int c = s_ws[i]; if (i < wid) before += c; tot += c; }
-    if (m) plan.pair_list[pos + before + __popc(bal & ((1u << lane) - 1u))] = p;
-    pos += tot;
-    __syncthreads();
+  const int per = (((n_pairs + kGroupThreads - 1) / kGroupThreads) + 3) & ~3;      // multiple of 4: int4 loads
+  const int lo = min(n_pairs, (int)threadIdx.x * per), hi = min(n_pairs, lo + per);
+  const bool vec = (n_pairs & 3) == 0;
+  int cnt = 0;
+  if (vec) {
+    for (int p = lo; p < hi; p += 4) {
+      const int4 v = __ldg(reinterpret_cast<const int4*>(ids + p));
+      cnt += (v.x == e) + (v.y == e) + (v.z == e) + (v.w == e);
+    }
+  } else {
+    for (int p = lo; p < hi; ++p) cnt += ids[p] == e;
   }
+  int inc = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+  if (lane == 31) s_ws[wid] = inc;
+  __syncthreads();
+  int before = inc - cnt;
+  for (int i = 0; i < wid; ++i) before += s_ws[i];
+  if (cnt == 0) return;
+  int pos = pos0 + before;
+  for (int p = lo; p < hi; ++p)
+    if (ids[p] == e) plan.pair_list[pos++] = p;
 }
 
 // ---- resize (a7, G13) -------------------------------------------------------

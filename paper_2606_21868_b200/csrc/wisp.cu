@@ -222,12 +222,13 @@ int launch_router(wisp_ctx* ctx, int layer, const void* x, int T_, cudaStream_t 
     // prefill: the router is a [T x d] x [d x E] GEMM -> same tcgen05 kernel (MODE 2), B operand = the caller's rows
     CUtensorMap tm_x;
     const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)T_}, str[1] = {(cuuint64_t)d * 2};
-    const cuuint32_t box2[2] = {kMmaBK, kMmaNT};
+    const int b_rows = 32;
+    const cuuint32_t box2[2] = {kMmaBK, (cuuint32_t)b_rows};
     if (!make_tmap(reinterpret_cast<EncodeTiledFn>(ctx->encode_fn), &tm_x, const_cast<void*>(x), 2, dims, str, box2, true))
       return fail(ctx, WISP_ECUDA, "tensor map over the hidden states failed (16-byte aligned rows required)");
     MmaArgs m{};
     m.L = cfg.n_layers; m.layer = layer; m.d = d; m.dff = cfg.d_ff; m.k = k;
-    m.z = ctx->logits; m.bias = ctx->router_bias + (size_t)layer * E; m.n_tokens = T_; m.E = E;
+    m.z = ctx->logits; m.bias = ctx->router_bias + (size_t)layer * E; m.n_tokens = T_; m.E = E; m.b_rows = b_rows;
     Span sp(ctx, WISP_K_ROUTER, st);
     const int ns = 6;
     prefill_mma_kernel<2><<<ctx->num_sms, kMmaThreads, ns * 2 * kMmaTileBytes + 1024, st>>>(ctx->tm_rw, tm_x, m, nullptr, nullptr, ns);
@@ -516,7 +517,7 @@ int launch_prefill_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T
     MmaArgs m{};
     m.plan = ctx->plan; m.wave = wave; m.C = ctx->C; m.L = L; m.layer = layer; m.d = d; m.dff = dff; m.k = k;
     m.act = reinterpret_cast<__nv_bfloat16*>(ctx->act_T); m.ystage = ctx->ystage;
-    int* n_work = ctx->mma_work + 2 * (cfg.n_experts + cfg.max_tokens * k / kMmaNT + 1);
+    int* n_work = ctx->mma_work + 4 * (cfg.n_experts + cfg.max_tokens * k / kMmaNT + 1);
     {
       Span sp(ctx, WISP_K_OTHER, st);
       build_work_kernel<<<1, 32, 0, st>>>(ctx->plan, wave, ctx->C, ctx->mma_work, n_work);
@@ -528,8 +529,8 @@ int launch_prefill_wave(wisp_ctx* ctx, int layer, int wave, const void* x, int T
     }
     {
       Span sp(ctx, WISP_K_PREFILL_DOWN, st);
-      const int ns = 6;
-      prefill_mma_kernel<1><<<ctx->num_sms, kMmaThreads, ns * 2 * kMmaTileBytes + 1024, st>>>(ctx->tm_dn, ctx->tm_act, m, ctx->mma_work, n_work, ns);
+      const int ns = 4;
+      prefill_mma_kernel<1><<<ctx->num_sms, kMmaThreads, ns * 3 * kMmaTileBytes + 1024, st>>>(ctx->tm_dn, ctx->tm_act, m, ctx->mma_work, n_work, ns);
     }
   } else {
     const int ptiles = (T_ + kPfTile - 1) / kPfTile;   // an expert can receive at most T pairs
@@ -578,7 +579,7 @@ bool setup_mma_path(wisp_ctx* ctx) {
     if (!make_tmap(fn, &ctx->tm_dn, ctx->arena + 2 * d * dff * 2, 4, dims, str, box, false)) return false;
   }
   if (cudaMalloc(&ctx->xg, rows * d * 2) != cudaSuccess) return false;
-  if (cudaMalloc(&ctx->mma_work, (2 * (size_t)(cfg.n_experts + cfg.max_tokens * cfg.top_k / kMmaNT + 1) + 1) * sizeof(int)) != cudaSuccess) return false;
+  if (cudaMalloc(&ctx->mma_work, (4 * (size_t)(cfg.n_experts + cfg.max_tokens * cfg.top_k / kMmaNT + 1) + 4) * sizeof(int)) != cudaSuccess) return false;
   {
     const cuuint64_t dims[2] = {d, rows}, str[1] = {d * 2};
     if (!make_tmap(fn, &ctx->tm_xg, ctx->xg, 2, dims, str, box2, true)) return false;
@@ -620,7 +621,7 @@ int forward_layer_prefill(wisp_ctx* ctx, int layer, const void* x, int T_, void*
   }
   if (ctx->mma_ok) {                               // B operand of GEMM 1: token rows in sorted-pair order
     Span sp(ctx, WISP_K_OTHER, st);
-    gather_tokens_kernel<<<std::min(n_pairs, 4 * ctx->num_sms), 256, 0, st>>>(ctx->plan.pair_list, n_pairs, k, cfg.d_model * 2 / 16,
+    gather_tokens_kernel<<<std::min((n_pairs + 7) / 8, 8 * ctx->num_sms), 256, 0, st>>>(ctx->plan.pair_list, n_pairs, k, cfg.d_model * 2 / 16,
                                                                              reinterpret_cast<const uint4*>(x), reinterpret_cast<uint4*>(ctx->xg));
   }
   for (int w = 0; w < n_waves; ++w) {
@@ -632,7 +633,7 @@ int forward_layer_prefill(wisp_ctx* ctx, int layer, const void* x, int T_, void*
   const size_t n = (size_t)T_ * cfg.d_model;
   {
     Span sp(ctx, WISP_K_COMBINE, st);
-    combine_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(ctx->ystage, ctx->topw + off, reinterpret_cast<T*>(out),
+    combine_kernel<T><<<(unsigned)((n / 4 + 255) / 256), 256, 0, st>>>(ctx->ystage, ctx->topw + off, reinterpret_cast<T*>(out),
                                                                    x_next ? reinterpret_cast<const T*>(x) : nullptr,
                                                                    reinterpret_cast<T*>(x_next), T_, cfg.d_model, k);
   }
