@@ -18,6 +18,17 @@
 namespace wisp {
 
 constexpr int kSliceCols = 16;
+// The accumulator of a (token, expert) exists in kZfixCopies copies; a CTA adds into copy blockIdx.x % kZfixCopies and the reader
+// sums the copies (integers: still one value whatever the order).  ~128 CTAs adding to the SAME word serialise in L2 at ~27 clk per
+// add (B300_MICROARCH.md: cyc/op = n_conc * 32 * 0.854); four copies cut that queue to a quarter.
+constexpr int kZfixCopies = 4;
+__host__ __device__ __forceinline__ size_t zfix_plane(int E) { return (size_t)kDecodeMaxTokens * E; }   // words per (parity, copy)
+__device__ __forceinline__ long long zfix_sum(const long long* z0, size_t plane) {       // z0 = the word in copy 0
+  long long v = 0;
+#pragma unroll
+  for (int c = 0; c < kZfixCopies; ++c) v += __ldcg(z0 + c * plane);
+  return v;
+}
 constexpr float kLogitFixScale = 1099511627776.f;        // 2^40
 constexpr float kLogitFixInv = 1.0f / 1099511627776.f;    // 2^-40 (exact)
 

@@ -49,7 +49,7 @@ struct DecodeArgs {
   float* topw;
   int max_tokens;
   float* partial;               // P [pair position][NC][d] fp32
-  long long* zfix;              // [2][kDecodeMaxTokens][E] int64 logit accumulators, all zero between launches
+  long long* zfix;              // [2][kZfixCopies][kDecodeMaxTokens][E] int64 logit accumulators, all zero between launches
   unsigned* sync;               // [0] grid barrier counter, [1..2] unit tickets; all zero at launch
   const void* x_in;             // input of layer_lo, [T][d]
   void* xbuf[2];                // intermediate hidden states
@@ -187,6 +187,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     }
   };
   const int n_slices = T_ * (d / kSliceCols);
+  const size_t zplane = zfix_plane(E);
   load_xs(a.x_in);
   plan_load<kPersistMaxExperts>(sh, layer_state_of(a, a.layer_lo), E, C);
   asm volatile("bar.sync 1, 256;" ::: "memory");
@@ -197,7 +198,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
       const int t = sl / (d / kSliceCols), j0 = (sl % (d / kSliceCols)) * kSliceCols;
       if (tid < kSliceCols) ds.xn[tid] = to_f32<T>(xs[(size_t)t * xs_pitch + j0 + tid]);
       asm volatile("bar.sync 1, 256;" ::: "memory");
-      slice_logits<T>(wrt + (size_t)j0 * E, ds.xn, E, a.zfix + ((size_t)(a.layer_lo & 1) * kDecodeMaxTokens + t) * E, tid, kDecConsumers);
+      slice_logits<T>(wrt + (size_t)j0 * E, ds.xn, E, a.zfix + ((size_t)(a.layer_lo & 1) * kZfixCopies + (blockIdx.x % kZfixCopies)) * zplane + (size_t)t * E, tid, kDecConsumers);
       asm volatile("bar.sync 1, 256;" ::: "memory");
     }
   }
@@ -206,7 +207,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
   for (int l = a.layer_lo; l < a.layer_hi; ++l) {
     const LayerState st = layer_state_of(a, l);
     const bool last = l == a.layer_hi - 1;
-    long long* zf_l = a.zfix + (size_t)(l & 1) * kDecodeMaxTokens * E;
+    long long* zf_l = a.zfix + (size_t)(l & 1) * kZfixCopies * zplane;        // copy 0 of this layer's accumulators
 
     // ---- route: logits -> top-k (one warp per token); the other threads' loads of x_l (written by the previous layer's
     // combine) are in flight meanwhile ----
@@ -228,7 +229,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
       }
       float* zout = writer ? a.logits : nullptr;               // test surface: wisp_last_logits
       auto zf = [&](int t, int e) {
-        const float z = logit_from_fix(__ldcg(zf_l + (size_t)t * E + e), bias[e]);
+        const float z = logit_from_fix(zfix_sum(zf_l + (size_t)t * E + e, zplane), bias[e]);
         if (zout) zout[(size_t)t * E + e] = z;
         return z;
       };
@@ -317,12 +318,14 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
 
     // ---- combine (+ residual) and the next layer's logits, 16-column slices over the grid ----
     {
-      if (writer) for (int i = tid; i < T_ * E; i += kDecConsumers) zf_l[(i / E) * E + (i % E)] = 0ll;   // consumed above by every CTA
+      if (writer)                                                // consumed above by every CTA
+        for (int c = 0; c < kZfixCopies; ++c)
+          for (int i = tid; i < T_ * E; i += kDecConsumers) zf_l[c * zplane + i] = 0ll;
       CombineArgs ca;
       ca.partial = a.partial; ca.n_chunks = g.n_chunks; ca.d = d; ca.k = k; ca.topw = ds.w; ca.pair_pos = ds.pl.pair_pos;
       T* xg = reinterpret_cast<T*>(last ? a.out : a.xbuf[(l - a.layer_lo) & 1]);
       const T* wrt = reinterpret_cast<const T*>(a.router_wt) + (size_t)(l + 1) * d * E;
-      long long* zf_n = a.zfix + (size_t)((l + 1) & 1) * kDecodeMaxTokens * E;
+      long long* zf_n = a.zfix + ((size_t)((l + 1) & 1) * kZfixCopies + (blockIdx.x % kZfixCopies)) * zplane;
       // CTA b owns the column blocks b, b + grid, ... of EVERY token: the tokens of a block are combined kCombineBatch at a time (their
       // partial loads in flight together) and share the block's 16 rows of router weights (staged for the CTA's first block)
       const int n_jb = d / kSliceCols;
@@ -370,7 +373,7 @@ __global__ void __launch_bounds__(256) decode_logits_kernel(const T* __restrict_
     const int t = sl / (d / kSliceCols), j0 = (sl % (d / kSliceCols)) * kSliceCols;
     if (threadIdx.x < kSliceCols) s_xn[threadIdx.x] = to_f32<T>(x[(size_t)t * d + j0 + threadIdx.x]);
     __syncthreads();
-    slice_logits<T>(wrt + (size_t)j0 * E, s_xn, E, zfix + (size_t)t * E, threadIdx.x, 256);
+    slice_logits<T>(wrt + (size_t)j0 * E, s_xn, E, zfix + (blockIdx.x % kZfixCopies) * zfix_plane(E) + (size_t)t * E, threadIdx.x, 256);
     __syncthreads();
   }
 }
@@ -385,12 +388,13 @@ __global__ void __launch_bounds__(NT) decode_plan_kernel(PlanArgs a, long long* 
   plan_load<NT>(sh, a.st, a.E, a.C);
   if (warp < n_tokens) {
     const long long* zt = zfix + (size_t)warp * a.E;
-    auto zf = [&](int e) { return logit_from_fix(zt[e], bias[e]); };
+    auto zf = [&](int e) { return logit_from_fix(zfix_sum(zt + e, zfix_plane(a.E)), bias[e]); };
     topk_softmax_warp<NT / 32>(zf, a.E, k, ids + warp * k, topw + warp * k, lane);
     for (int e = lane; e < a.E; e += 32) logits[(size_t)warp * a.E + e] = zf(e);
   }
   __syncthreads();
-  for (int i = tid; i < n_tokens * a.E; i += NT) zfix[i] = 0ll;
+  for (int c = 0; c < kZfixCopies; ++c)
+    for (int i = tid; i < n_tokens * a.E; i += NT) zfix[c * zfix_plane(a.E) + i] = 0ll;
   a.ids = ids;
   if (warp == 0) {
     const bool fast = plan_fast_warp<NT>(a, sh, true, lane);

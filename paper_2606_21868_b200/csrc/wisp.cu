@@ -88,7 +88,7 @@ struct wisp_ctx {
   // decode path (decode_*.cuh)
   DecodeGeom dgeom[2]{};             // [0]: calls of at most 2 tokens, [1]: 3..8 tokens (larger work units: fewer chunk partials)
   float* partial = nullptr;          // chunk partials P [pair position][NC][d]
-  long long* zfix = nullptr;         // [2][kDecodeMaxTokens][E] int64 logit accumulators (zero between launches)
+  long long* zfix = nullptr;         // [2][kZfixCopies][kDecodeMaxTokens][E] int64 logit accumulators (zero between launches)
   unsigned* dsync = nullptr;         // [0] grid barrier counter, [1..2] unit tickets
   const char** d_masters = nullptr;  // device [L]: mapped master pointers
   int* host_err = nullptr;           // mapped pinned flag: a grid barrier of the fused kernel timed out
@@ -367,7 +367,7 @@ int check_dev_err(wisp_ctx* ctx) {
   if (!ctx->host_err || !*reinterpret_cast<volatile int*>(ctx->host_err)) return WISP_OK;
   cudaDeviceSynchronize();
   *reinterpret_cast<volatile int*>(ctx->host_err) = 0;
-  cudaMemset(ctx->zfix, 0, 2 * (size_t)kDecodeMaxTokens * ctx->cfg.n_experts * sizeof(long long));
+  cudaMemset(ctx->zfix, 0, 2 * kZfixCopies * (size_t)kDecodeMaxTokens * ctx->cfg.n_experts * sizeof(long long));
   cudaMemset(ctx->dsync, 0, 4 * sizeof(unsigned));
   return fail(ctx, WISP_ECUDA, "fused decode kernel: a grid-wide barrier timed out; the outputs of that forward are invalid");
 }
@@ -899,8 +899,8 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   CKC(cudaMemset(ctx->d_masters, 0, (size_t)L * sizeof(char*)));
   CKC(cudaMalloc(&ctx->dsync, 4 * sizeof(unsigned)));
   CKC(cudaMemset(ctx->dsync, 0, 4 * sizeof(unsigned)));
-  CKC(cudaMalloc(&ctx->zfix, 2 * (size_t)kDecodeMaxTokens * E * sizeof(long long)));
-  CKC(cudaMemset(ctx->zfix, 0, 2 * (size_t)kDecodeMaxTokens * E * sizeof(long long)));
+  CKC(cudaMalloc(&ctx->zfix, 2 * kZfixCopies * (size_t)kDecodeMaxTokens * E * sizeof(long long)));
+  CKC(cudaMemset(ctx->zfix, 0, 2 * kZfixCopies * (size_t)kDecodeMaxTokens * E * sizeof(long long)));
   CKC(cudaHostAlloc(&ctx->host_err, sizeof(int), cudaHostAllocMapped));
   *ctx->host_err = 0;
   CKC(cudaHostGetDevicePointer(reinterpret_cast<void**>(&ctx->dev_err), ctx->host_err, 0));
