@@ -531,18 +531,22 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
 #pragma unroll
         for (int t = 0; t < kDecMaxSteps; ++t) { yacc[t][0] = 0.f; yacc[t][1] = 0.f; yacc[t][2] = 0.f; yacc[t][3] = 0.f; }
       }
-      const bool mg = F8 && g.merge != 0;                       // one part holds the down columns of every sub-block
-      for (int sb = 0; sb < g.n_sb; ++sb) {
-      if (sb > 0 && !mg) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
+      // fp8 merged parts (two sub-blocks = 16 act columns in one part): ONE pass whose MMAs use all 16 k slots -- lane quarters 0 / 1
+      // feed sub-block 0's columns 0-3 / 4-7, quarters 2 / 3 sub-block 1's
+      const bool mg = F8 && g.merge != 0 && g.n_sb == 2;
+      const int n_pass = mg ? 1 : g.n_sb;
+      for (int sb = 0; sb < n_pass; ++sb) {
+      if (sb > 0) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
       const uint32_t pbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
-      const uint32_t dbase = pbase + (mg ? (uint32_t)sb * (uint32_t)g.sub_bytes : 0u);
-      if (!mg || sb == 0) store_part(DecPart{2, mg ? 0 : sb, s});
-      const AT* act = reinterpret_cast<const AT*>(fs.act[par][sb]);
+      const int sbx = mg ? (lane & 3) >> 1 : sb;                // sub-block this lane's operands come from
+      const uint32_t dbase = pbase + (mg ? (uint32_t)sbx * (uint32_t)g.sub_bytes : 0u);
+      store_part(DecPart{2, sb, s});
+      const AT* act = reinterpret_cast<const AT*>(fs.act[par][sbx]);
       if constexpr (F8) {
         // a down core is 8 outputs x 8 act columns (64 bytes): lane quarters 0 / 1 hold columns 0-3 / 4-7 of outputs g and g + 8 and
-        // feed the k slots {2q, 2q+1, 2q+8, 2q+9}; quarters 2 / 3 contribute zeros (the unit has 8 columns, the MMA 16 slots)
+        // feed the k slots {2q, 2q+1, 2q+8, 2q+9}; unmerged, quarters 2 / 3 contribute zeros (8 columns, 16 slots)
         const int tq = lane & 3;
-        const bool on = tq < 2;
+        const bool on = mg || tq < 2;
         const uint2 bv = *reinterpret_cast<const uint2*>(reinterpret_cast<const __half*>(act) + col * 8 + (tq & 1) * 4);
         const uint32_t b0 = on ? bv.x : 0u, b1 = on ? bv.y : 0u;
         const uint32_t abase = dbase + (uint32_t)(warp * g.steps) * 128u + (uint32_t)(lane >> 2) * 8u + (uint32_t)(tq & 1) * 4u;
@@ -564,13 +568,13 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
           }
         }
         float s2v[kDecMaxSteps / 8];                           // block scales of this warp's output blocks (read before the slot is released)
-        if (sb == g.n_sb - 1) {
+        if (sb == n_pass - 1) {
 #pragma unroll
           for (int i = 0; i < kDecMaxSteps / 8; ++i)
             s2v[i] = i * 8 < g.steps ? lds_f32(pbase + (uint32_t)g.part_bytes + (uint32_t)(warp * (g.steps >> 3) + i) * 4u) : 0.f;
         }
-        if (!mg || sb == g.n_sb - 1) release();
-        if (sb == g.n_sb - 1) {
+        release();
+        if (sb == n_pass - 1) {
           const int j0 = s * g.slab + warp * (g.slab >> 3) + col;
           float* p0 = a.partial + ((size_t)(pos0 + kq) * g.n_chunks + c) * g.d + j0;
           float* p1 = p0 + (size_t)g.n_chunks * g.d;

@@ -327,7 +327,7 @@ DecodeGeom make_decode_geom(int d, int dff, size_t elem, int rows_unit, bool f8 
   g.rows_unit = rows_unit;
   g.n_sb = rows_unit / 8;
   g.sub_bytes = 8 * g.slab * (int)elem;
-  g.merge = f8 && g.n_slab == 1 && g.n_sb * g.sub_bytes <= kDecMaxPartBytes ? 1 : 0;
+  g.merge = f8 && g.n_slab == 1 && g.n_sb == 2 && g.n_sb * g.sub_bytes <= kDecMaxPartBytes ? 1 : 0;   // (the merged down pass feeds 16 k slots)
   g.part_bytes = g.sub_bytes * (g.merge ? g.n_sb : 1);
   g.n_chunks = dff / rows_unit;
   g.parts_unit = 3 * g.n_sb * g.n_slab;
