@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
   const bool timing = blockIdx.x == gridDim.x - 1 && tid == 0 && a.phase_ns != nullptr;   // a CTA that is not the writer
   u64 t_prev = timing ? globaltimer_ns() : 0ull;
   auto stamp = [&](int phase) {
-    if (timing) { const u64 t = globaltimer_ns(); a.phase_ns[phase] += t - t_prev; t_prev = t; }
+    if (timing) { const u64 t = globaltimer_ns(); atomicAdd(a.phase_ns + phase, t - t_prev); t_prev = t; }   // RED: no round trip
   };
   unsigned gen = 0, qseq = 0, gu_seq = 0, d_seq = 0;
   const uint32_t w_off = (uint32_t)((E * sizeof(float) + 127) & ~(size_t)127);   // staged region: [router bias of the next layer][weight slice]
@@ -296,7 +296,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
     stamp(1);
     if (!last) plan_load<kPersistMaxExperts>(sh, layer_state_of(a, l + 1), E, C);   // stable until that layer's own plan
     stamp(2);
-    if (timing) a.phase_ns[kDecPhases + miss_cls] += 1;
+    if (timing) atomicAdd(a.phase_ns + kDecPhases + miss_cls, 1ull);
 
     // ---- ffn, wave by wave ----
     fa.layer_base = a.pool + (size_t)l * a.blob_bytes;
