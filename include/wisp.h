@@ -248,7 +248,7 @@ int wisp_last_topk(wisp_ctx* ctx, int32_t layer, int32_t* ids, float* w, int32_t
 int wisp_last_logits(wisp_ctx* ctx, float* z, int32_t n_tokens);
 /* The router step of one layer (a1: logits, top-k ids in (z desc, id asc) order, softmax over the selected k) for a small token
  * batch WITHOUT any allocation -- for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses
- * that forbid it).  No context: the caller passes every input and output; the only scratch (the 2^-40 fixed-point int64 logit
+ * that forbid it).  No context: the caller passes every input and output; the only scratch (the 2^-32 fixed-point int64 logit
  * accumulators of the decode path) is a file-scope device array of 8192 words = 64 KiB that every GPU loading the library holds
  * until exit.  Same arithmetic as the context's decode path, so the results equal wisp_last_logits / wisp_last_topk bit for bit.
  *   hidden       device, [n_tokens, d_model] row-major, `dtype` (WISP_F32 or WISP_BF16)

@@ -7,10 +7,10 @@
 //   out_t[j]    = sum_{i = 0..k-1} w[t,i] * y_{t,i}[j]      fmaf in rank order from 0.f, stored in the model dtype (a4, G21)
 //   x'_t[j]     = x_t[j] + out_t[j]                         fp32 add of the two model-dtype values, stored in the model dtype (O3)
 //   z_e        += sum_{j in slice} W_r[e][j] * x'_t[j]      fmaf in ascending j from 0.f per slice, then added to the logit
-//                                                           accumulator as a 2^-40 fixed-point integer (a1)
+//                                                           accumulator as a 2^-32 fixed-point integer (a1)
 // The logit accumulator is an int64 per (token, expert): integer addition is associative, so the all-reduce of the
 // 16-column partial logits over the grid is bit-reproducible whatever order the CTAs' `red.add.u64` arrive in, and it needs
-// no second grid-wide exchange: after one barrier every CTA reads E words per token.  (A logit partial is O(1); 2^-40
+// no second grid-wide exchange: after one barrier every CTA reads E words per token.  (A logit partial is O(1); 2^-32
 // resolution is five orders of magnitude below fp32 rounding of the logit itself.)
 #pragma once
 #include "common.cuh"
@@ -23,19 +23,27 @@ constexpr int kSliceCols = 16;
 // add (B300_MICROARCH.md: cyc/op = n_conc * 32 * 0.854); four copies cut that queue to a quarter.
 constexpr int kZfixCopies = 4;
 __host__ __device__ __forceinline__ size_t zfix_plane(int E) { return (size_t)kDecodeMaxTokens * E; }   // words per (parity, copy)
-__device__ __forceinline__ long long zfix_sum(const long long* z0, size_t plane) {       // z0 = the word in copy 0
-  long long v = 0;
-#pragma unroll
-  for (int c = 0; c < kZfixCopies; ++c) v += __ldcg(z0 + c * plane);
-  return v;
-}
-constexpr float kLogitFixScale = 1099511627776.f;        // 2^40
-constexpr float kLogitFixInv = 1.0f / 1099511627776.f;    // 2^-40 (exact)
-
+// An accumulator word = (sum of the 2^-32 fixed-point partial logits) << 10 | number of partials added so far (< 1024 per copy:
+// d / 16 / kZfixCopies).  The count makes the word self-describing: a reader that knows how many partials a copy receives can tell
+// from the word alone that its sum is complete -- the fused kernel polls the words instead of crossing a grid barrier (E) and
+// then reading them.
+constexpr float kLogitFixScale = 4294967296.f;           // 2^32
+constexpr float kLogitFixInv = 1.0f / 4294967296.f;       // 2^-32 (exact)
 __device__ __forceinline__ long long logit_to_fix(float v) {
   const float s = v * kLogitFixScale;
-  if (!(fabsf(s) < 4.0e18f)) return s > 0.f ? (1ll << 62) : -(1ll << 62);   // non-finite input (G23): saturate, stay defined
+  if (!(fabsf(s) < 2.2e15f)) return s > 0.f ? (1ll << 51) : -(1ll << 51);   // |v| >= 2^19 or non-finite (G23): saturate, stay defined
   return __float2ll_rn(s);
+}
+constexpr int kZfixCountBits = 10;
+__device__ __forceinline__ unsigned long long zfix_pack(float v) { return ((unsigned long long)logit_to_fix(v) << kZfixCountBits) + 1ull; }   // one partial
+__device__ __forceinline__ unsigned long long zfix_pack_uncounted(float v) { return (unsigned long long)logit_to_fix(v) << kZfixCountBits; }
+__device__ __forceinline__ long long zfix_value(long long word) { return word >> kZfixCountBits; }
+__device__ __forceinline__ int zfix_count(long long word) { return (int)(word & ((1 << kZfixCountBits) - 1)); }
+__device__ __forceinline__ long long zfix_sum(const long long* z0, size_t plane) {       // z0 = the word in copy 0; complete words
+  long long v = 0;
+#pragma unroll
+  for (int c = 0; c < kZfixCopies; ++c) v += zfix_value(__ldcg(z0 + c * plane));
+  return v;
 }
 // one rounding (int64 -> fp32), an exact scaling, one fp32 add; no fp64 on the routing chain
 __device__ __forceinline__ float logit_from_fix(long long f, float bias) { return __ll2float_rn(f) * kLogitFixInv + bias; }
@@ -49,7 +57,7 @@ __device__ __forceinline__ void slice_logits(const T* w16, const float* xn, int 
     float zp = 0.f;
 #pragma unroll
     for (int jj = 0; jj < kSliceCols; ++jj) zp = fmaf(to_f32<T>(w16[(size_t)jj * E + e]), xn[jj], zp);
-    atomicAdd(reinterpret_cast<unsigned long long*>(zfix_t + e), (unsigned long long)logit_to_fix(zp));
+    atomicAdd(reinterpret_cast<unsigned long long*>(zfix_t + e), zfix_pack(zp));
   }
 }
 
@@ -67,7 +75,7 @@ __device__ __forceinline__ void slice_logits_multi(const T* w16, const float* xn
         float zp = 0.f;
 #pragma unroll
         for (int jj = 0; jj < kSliceCols; ++jj) zp = fmaf(wv[jj], xn[s * kSliceCols + jj], zp);
-        atomicAdd(reinterpret_cast<unsigned long long*>(zfix_t0 + (size_t)s * E + e), (unsigned long long)logit_to_fix(zp));
+        atomicAdd(reinterpret_cast<unsigned long long*>(zfix_t0 + (size_t)s * E + e), zfix_pack(zp));
       }
     }
   }

@@ -2,7 +2,8 @@
 //
 // Fused form (WISP_FETCH_FUSED, E <= 256): ONE persistent cooperative kernel per token batch, one CTA per SM, the whole
 // stack of layers inside the launch.  The paper runs the paging decision in Python on the host between kernels and names
-// that its overhead; here the whole chain stays on the chip with TWO grid-wide barriers per layer:
+// that its overhead; here the whole chain stays on the chip with ONE grid-wide barrier per layer (C) and one
+// data-carrying reduction (the logit accumulators count their own contributions, decode_combine.cuh):
 //
 //   route  every CTA: logits of this layer (bias + the int64 accumulator filled by the previous combine), top-k by warp
 //          arg-max (router.cuh), Algorithm 1 -- the one-warp hit fast path, or plan_compute when the step
@@ -11,8 +12,8 @@
 //   ffn    fused gate/up/SwiGLU/down per work unit (decode_ffn.cuh), units handed out by an atomic ticket, misses read
 //          from the mapped pinned master and written into their victim slot on the way (Alg. 1 line 6)      -> barrier C
 //   comb   16-column slices over the grid: ordered combine + residual -> x_{l+1}; partial router logits of layer l+1 into
-//          the int64 accumulator (decode_combine.cuh)                                                        -> barrier E
-//          then every CTA reloads x_{l+1} (4 KiB per token) into shared memory
+//          the int64 accumulators (decode_combine.cuh); no barrier: the next route step polls the accumulator words until each
+//          carries all its contributions, and one warp waits for the x-ready counter and reloads x_{l+1} (4 KiB per token)
 // An overflowing step (|R| > C) adds one barrier per extra wave (the next wave's fills reuse slots).
 //
 // Split form (MEMCPY / ZEROCOPY contexts, E > 256, event timing of kernel classes): the same device functions as four
@@ -50,7 +51,7 @@ struct DecodeArgs {
   int max_tokens;
   float* partial;               // P [pair position][NC][d] fp32
   long long* zfix;              // [2][kZfixCopies][kDecodeMaxTokens][E] int64 logit accumulators, all zero between launches
-  unsigned* sync;               // [0] grid barrier counter, [1..2] unit tickets; all zero at launch
+  unsigned* sync;               // [0] grid barrier counter, [1..2] unit tickets, [3] x-ready counter (slices of x written so far); zero at launch
   const void* x_in;             // input of layer_lo, [T][d]
   void* xbuf[2];                // intermediate hidden states
   void* out;                    // [T][d]
@@ -112,6 +113,7 @@ struct DecShared {
   unsigned long long wpre;                                // the next layer's router-weight slice has landed in shared memory
   alignas(16) float y[kCombineBatch * kMaxTopK * kSliceCols];   // combine: per-rank sums of up to kCombineBatch slices
   float xn[kCombineBatch * kSliceCols];
+  int zexp[kZfixCopies];                                  // partials a complete accumulator word of copy c carries (per token and layer)
   int ids[kDecodeMaxTokens * kMaxTopK];
   float w[kDecodeMaxTokens * kMaxTopK];
   DecPlan pl;
@@ -170,7 +172,8 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
 
   // ===================== consumer warps =====================
   const bool writer = blockIdx.x == 0;
-  const bool timing = blockIdx.x == gridDim.x - 1 && tid == 0 && a.phase_ns != nullptr;   // a CTA that is not the writer
+  // the timing CTA is not the writer and owns a combine slice (CTA 1); its route stamp includes the wait for the accumulators
+  const bool timing = blockIdx.x == (gridDim.x > 1 ? 1u : 0u) && tid == 0 && a.phase_ns != nullptr;
   u64 t_prev = timing ? globaltimer_ns() : 0ull;
   auto stamp = [&](int phase) {
     if (timing) { const u64 t = globaltimer_ns(); atomicAdd(a.phase_ns + phase, t - t_prev); t_prev = t; }   // RED: no round trip
@@ -189,18 +192,25 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
   const int n_slices = T_ * (d / kSliceCols);
   const size_t zplane = zfix_plane(E);
   load_xs(a.x_in);
+  if (tid < kZfixCopies) {
+    int n = 0;
+    for (int jb = 0; jb < d / kSliceCols; ++jb) n += ((jb % (int)gridDim.x) % kZfixCopies) == tid;
+    ds.zexp[tid] = n;
+  }
   plan_load<kPersistMaxExperts>(sh, layer_state_of(a, a.layer_lo), E, C);
   asm volatile("bar.sync 1, 256;" ::: "memory");
   // logits of the first layer: the same 16-column slices the combine uses for every later layer
   {
     const T* wrt = reinterpret_cast<const T*>(a.router_wt) + (size_t)a.layer_lo * d * E;
-    for (int sl = blockIdx.x; sl < n_slices; sl += gridDim.x) {
-      const int t = sl / (d / kSliceCols), j0 = (sl % (d / kSliceCols)) * kSliceCols;
-      if (tid < kSliceCols) ds.xn[tid] = to_f32<T>(xs[(size_t)t * xs_pitch + j0 + tid]);
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      slice_logits<T>(wrt + (size_t)j0 * E, ds.xn, E, a.zfix + ((size_t)(a.layer_lo & 1) * kZfixCopies + (blockIdx.x % kZfixCopies)) * zplane + (size_t)t * E, tid, kDecConsumers);
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-    }
+    // (the combine's mapping: CTA b owns the column blocks b, b + grid, ... of every token, so a copy receives ds.zexp[c] partials)
+    for (int jb = blockIdx.x; jb < d / kSliceCols; jb += gridDim.x)
+      for (int t = 0; t < T_; ++t) {
+        const int j0 = jb * kSliceCols;
+        if (tid < kSliceCols) ds.xn[tid] = to_f32<T>(xs[(size_t)t * xs_pitch + j0 + tid]);
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        slice_logits<T>(wrt + (size_t)j0 * E, ds.xn, E, a.zfix + ((size_t)(a.layer_lo & 1) * kZfixCopies + (blockIdx.x % kZfixCopies)) * zplane + (size_t)t * E, tid, kDecConsumers);
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+      }
   }
   if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;
 
@@ -211,17 +221,36 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
 
     // ---- route: logits -> top-k (one warp per token); the other threads' loads of x_l (written by the previous layer's
     // combine) are in flight meanwhile ----
-    constexpr int kXsRegs = 8;
-    const int xs_vec = T_ * (d * (int)sizeof(T) / 16);
-    const bool reload = l > a.layer_lo, reload_regs = xs_vec <= kXsRegs * kDecConsumers;
-    const void* x_src = a.xbuf[(l - 1 - a.layer_lo) & 1];
-    uint4 xr[kXsRegs];
-    if (reload && reload_regs) {
+    const bool reload = l > a.layer_lo;
+    const bool split = T_ * k <= kDecConsumers - 32;           // warp 7 loads x while warps 0-6 select (else: all select, then warp 7 loads)
+    auto reload_x = [&]() {
+      // ---- warp 7: x_l.  The previous combine's slices count themselves into the x-ready word after a gpu-scope fence ----
+      if (reload) {
+        if (lane == 0) {
+          const unsigned want = (unsigned)(l - a.layer_lo) * (unsigned)n_slices;
+          unsigned spins = 0;
+          while (ld_acquire(a.sync + 3) < want)
+            if (++spins > kGridBarrierSpinLimit || ((spins & 0xfffu) == 0u && *a.err)) { *a.err = 1; fs.abort = 1; break; }
+        }
+        __syncwarp();
+        const uint4* x_src = reinterpret_cast<const uint4*>(a.xbuf[(l - 1 - a.layer_lo) & 1]);
+        const int vec_row = d * (int)sizeof(T) / 16, xs_vec = T_ * vec_row;
+        for (int v0 = lane; v0 < xs_vec; v0 += 32 * 8) {
+          uint4 xr[8];
 #pragma unroll
-      for (int i = 0; i < kXsRegs; ++i)
-        if (i * kDecConsumers < xs_vec) xr[i] = __ldcg(reinterpret_cast<const uint4*>(x_src) + min(tid + i * kDecConsumers, xs_vec - 1));
-    }
-    {
+          for (int i = 0; i < 8; ++i) xr[i] = __ldcg(x_src + min(v0 + 32 * i, xs_vec - 1));
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int v = v0 + 32 * i;
+            if (v < xs_vec) reinterpret_cast<uint4*>(xs + (size_t)(v / vec_row) * xs_pitch)[v % vec_row] = xr[i];
+          }
+        }
+      }
+    };
+    if (split && warp == kDecWarps - 1) {
+      reload_x();
+    } else {
+      // ---- warps 0-6: logits -> top-k.  Every accumulator word is polled until it carries all its partials ----
       const float* bias = a.router_bias + (size_t)l * E;
       if (reload) {                                            // staged in shared memory during the previous layer's FFN
         mbar_wait(smem_u32(&ds.wpre), (unsigned)(l - 1 - a.layer_lo) & 1u);
@@ -229,26 +258,32 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
       }
       float* zout = writer ? a.logits : nullptr;               // test surface: wisp_last_logits
       auto zf = [&](int t, int e) {
-        const float z = logit_from_fix(zfix_sum(zf_l + (size_t)t * E + e, zplane), bias[e]);
+        const long long* w0 = zf_l + (size_t)t * E + e;
+        long long v[kZfixCopies];
+        unsigned spins = 0;
+        while (true) {
+          bool done = true;
+#pragma unroll
+          for (int c = 0; c < kZfixCopies; ++c) v[c] = ld_relaxed_s64(w0 + c * zplane);
+#pragma unroll
+          for (int c = 0; c < kZfixCopies; ++c) done = done && zfix_count(v[c]) == ds.zexp[c];
+          if (done) break;
+          if (++spins > kGridBarrierSpinLimit || ((spins & 0xfffu) == 0u && (*a.err || fs.abort))) { *a.err = 1; fs.abort = 1; break; }
+        }
+        long long sum = 0;
+#pragma unroll
+        for (int c = 0; c < kZfixCopies; ++c) sum += zfix_value(v[c]);
+        const float z = logit_from_fix(sum, bias[e]);
         if (zout) zout[(size_t)t * E + e] = z;
         return z;
       };
       // (T * k <= 256 pairs: kDecodeMaxTokens * kMaxTopK; the FFN dataflow's scratch is idle between waves)
-      topk_softmax_block(zf, T_, E, k, ds.ids, ds.w, reinterpret_cast<unsigned*>(&fs.red[0][0][0]), tid, kDecConsumers, 1);
+      if (split) topk_softmax_block(zf, T_, E, k, ds.ids, ds.w, reinterpret_cast<unsigned*>(&fs.red[0][0][0]), tid, kDecConsumers - 32, 2);
+      else topk_softmax_block(zf, T_, E, k, ds.ids, ds.w, reinterpret_cast<unsigned*>(&fs.red[0][0][0]), tid, kDecConsumers, 1);
     }
-    if (reload) {
-      if (reload_regs) {
-        const int vec_row = d * (int)sizeof(T) / 16;
-#pragma unroll
-        for (int i = 0; i < kXsRegs; ++i) {
-          const int v = tid + i * kDecConsumers;
-          if (v < xs_vec) reinterpret_cast<uint4*>(xs + (size_t)(v / vec_row) * xs_pitch)[v % vec_row] = xr[i];
-        }
-      } else {
-        load_xs(x_src);
-      }
-    }
+    if (!split && warp == kDecWarps - 1) reload_x();
     asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (fs.abort) return;                                      // a poll timed out: the host reports WISP_ECUDA
     if constexpr (F8)                                          // (the plan step's barriers order it before the consumers' reads)
       stage_xh(reinterpret_cast<const __nv_bfloat16*>(xs), xh, fs, T_, d, xs_pitch, tid, kDecConsumers,
                [] { asm volatile("bar.sync 1, 256;" ::: "memory"); });
@@ -341,19 +376,19 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
           const T* xres = a.residual ? xs : nullptr;
           if (!MULTI || ns == 1) {
             combine_slice<T>(ca, t0, j0, xres ? xres + (size_t)t0 * xs_pitch : nullptr, xg + (size_t)t0 * d, fs.red[0][0], ds.y, ds.xn, 1);
+            if (!last && tid == 255) { __threadfence(); atomicAdd(a.sync + 3, 1u); }    // x slice visible at gpu scope, then counted (a thread with no logit adds at E <= 255)
             if (!last) slice_logits<T>(w16, ds.xn, E, zf_n + (size_t)t0 * E, tid, kDecConsumers);
           } else if constexpr (!MULTI) {
           } else if (ns == 2) {
             combine_tokens<T, 2, 6>(ca, t0, ns, j0, xres, xs_pitch, xg, fs.red[0][0], ds.y, ds.xn, 1);
+            if (!last && tid == 255) { __threadfence(); atomicAdd(a.sync + 3, (unsigned)ns); }
             if (!last) slice_logits_multi<T, 2>(w16, ds.xn, ns, E, zf_n + (size_t)t0 * E, tid, kDecConsumers);
           } else {
             combine_tokens<T, kCombineBatch, 3>(ca, t0, ns, j0, xres, xs_pitch, xg, fs.red[0][0], ds.y, ds.xn, 1);
+            if (!last && tid == 255) { __threadfence(); atomicAdd(a.sync + 3, (unsigned)ns); }
             if (!last) slice_logits_multi<T, kCombineBatch>(w16, ds.xn, ns, E, zf_n + (size_t)t0 * E, tid, kDecConsumers);
           }
         }
-      }
-      if (!last) {
-        if (!grid_barrier(a.sync, gen, a.err, &fs.abort)) return;   // E: x_{l+1} and its logits are complete (reloaded by the route step)
       }
     }
     stamp(5);

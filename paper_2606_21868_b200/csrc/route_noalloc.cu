@@ -1,7 +1,7 @@
 // route_noalloc.cu -- wisp_route_noalloc: the router step (a1: logits + top-k + renormalised softmax) of one layer for a small
 // token batch WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
 // loops, harnesses that forbid it).  It is a variant of the decode path's logits kernel (decode_kernels.cuh:
-// decode_logits_kernel): the same 16-column slices of the hidden state, the same fmaf chain per slice, the same 2^-40
+// decode_logits_kernel): the same 16-column slices of the hidden state, the same fmaf chain per slice, the same 2^-32
 // fixed-point int64 accumulators (decode_combine.cuh) -- but the accumulators, which the context-owning path keeps in a
 // cudaMalloc'ed buffer, live here in ONE file-scope device array of fixed size:
 //
@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) route_logits_rowmajor_kernel(const T* __r
       float zp = 0.f;
 #pragma unroll
       for (int jj = 0; jj < kSliceCols; ++jj) zp = fmaf(to_f32<T>(row[jj]), s_xn[jj], zp);
-      atomicAdd(reinterpret_cast<unsigned long long*>(zfix + (size_t)t * E + e), (unsigned long long)logit_to_fix(zp));
+      atomicAdd(reinterpret_cast<unsigned long long*>(zfix + (size_t)t * E + e), zfix_pack_uncounted(zp));
     }
     __syncthreads();
   }
@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(128) route_finish_kernel(const long long* __re
   const int t = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (t >= n_tokens) return;
   const long long* zt = zfix + (size_t)t * E;
-  auto zf = [&](int e) { return logit_from_fix(zt[e], bias ? bias[e] : 0.f); };
+  auto zf = [&](int e) { return logit_from_fix(zfix_value(zt[e]), bias ? bias[e] : 0.f); };
   topk_softmax_warp<EPL>(zf, E, k, ids + (size_t)t * k, wts + (size_t)t * k, lane);
   if (logits)
     for (int e = lane; e < E; e += 32) logits[(size_t)t * E + e] = zf(e);
