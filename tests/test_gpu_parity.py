@@ -242,3 +242,29 @@ def test_static_layer_offload_arm(T):
         ctx.close()
     with pytest.raises(wp.WispError):                       # less than the two bounce buffers
         make_ctx(shape, budget=layer_bytes, fetch=wp.WISP_FETCH_STATIC, max_tokens=T, trace=False)
+
+
+def test_wide_topk_fused_route_without_a_spare_warp():
+    """T * k = 256 > 224: the fused kernel's route step cannot give warp 7 to the x reload (all eight warps select, then warp 7
+    loads): same four parities, fused vs split vs oracle."""
+    shape = si.MoEShape("wide-k", 2, 64, 32, 256, 256, "f32", 1.1)
+    hidden = si.gen_decode_hidden(shape, 6, 8)
+    ref = None
+    for slots, fetch in ((64, 2), (64, 1), (40, 2)):
+        ctx = make_ctx(shape, slots, max_tokens=8, fetch=fetch)
+        res = run_chain(ctx, shape, hidden)
+        routed = [[rec["ids"].flatten().tolist() for rec in per] for per in res]
+        want, _ = sim_trace(shape, slots, 0, routed)
+        assert ctx.trace_read() == want
+        if ref is None:
+            ref = res
+            check_vs_oracle(shape, res, TOL["f32"])
+        else:
+            assert_same_bytes(ref, res)
+        ctx2 = make_ctx(shape, slots, max_tokens=8, fetch=fetch)
+        fin = run_stack(ctx2, shape, hidden)                                       # all layers in one launch: the reload path
+        for t in range(hidden.shape[0]):
+            last = res[t][-1]
+            want_x = (last["x"].float() + last["out"].float()).to(shape.torch_dtype)
+            assert torch.equal(fin[t].view(torch.uint8), want_x.view(torch.uint8))
+        ctx.close(); ctx2.close()
