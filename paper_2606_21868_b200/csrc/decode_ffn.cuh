@@ -369,10 +369,10 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
     const bool fill = a.master != nullptr && plan.entry_miss[q] != 0;
     char* slot_blob = const_cast<char*>(a.layer_base) + (size_t)plan.entry_slot[q] * a.slot_stride;
     // on a miss, warp 0 stores the landed part into the victim slot before the ring slot is handed back
-    auto store_part = [&](const DecPart& pt) {
+    auto store_part = [&](const DecPart& pt, int ring_slot = -1) {
       if (fill && warp == 0 && lane == 0) {
         const int np = pt.mat == 2 ? g.down_pieces : 1;
-        const uint32_t pb = (uint32_t)g.part_bytes / np, src = ring.slot0 + (uint32_t)rp.s * ring.stride;
+        const uint32_t pb = (uint32_t)g.part_bytes / np, src = ring.slot0 + (uint32_t)(ring_slot < 0 ? rp.s : ring_slot) * ring.stride;
         for (int piece = 0; piece < np; ++piece) bulk_s2g(slot_blob + dec_part_offset(g, c, pt, piece), src + piece * pb, pb);
         if constexpr (F8) bulk_s2g(slot_blob + dec_scale_offset(g, c, pt), src + (uint32_t)g.part_bytes, (uint32_t)g.scale_bytes);
         bulk_commit();
@@ -534,7 +534,10 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
       // fp8 merged parts (two sub-blocks = 16 act columns in one part): ONE pass whose MMAs use all 16 k slots -- lane quarters 0 / 1
       // feed sub-block 0's columns 0-3 / 4-7, quarters 2 / 3 sub-block 1's
       const bool mg = F8 && g.merge != 0 && g.n_sb == 2;
-      const int n_pass = mg ? 1 : g.n_sb;
+      // bf16 units of two sub-blocks: their two down parts (consecutive in the ring) feed ONE pass whose MMAs use all 16 k slots
+      // (k 0-7 = sub-block 0's act columns, k 8-15 = sub-block 1's) instead of two passes with half of K zero
+      const bool pair = kMma && g.n_sb == 2;
+      const int n_pass = (mg || pair) ? 1 : g.n_sb;
       for (int sb = 0; sb < n_pass; ++sb) {
       if (sb > 0) mbar_wait(ring.full0 + 8u * rp.s, rp.ph);
       const uint32_t pbase = ring.slot0 + (uint32_t)rp.s * ring.stride;
@@ -594,6 +597,31 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
           }
         }
       } else if constexpr (kMma) {
+        if (pair) {
+          // A[j][i]: 16 outputs j x 16 act columns i (matrices 0, 1 from sub-block 0's part, 2, 3 from sub-block 1's); B[i][n] = a[n][i]
+          DecRingPos rp1 = rp;
+          ring_advance(ring, rp1);
+          mbar_wait(ring.full0 + 8u * rp1.s, rp1.ph);
+          const uint32_t d1base = ring.slot0 + (uint32_t)rp1.s * ring.stride;
+          store_part(DecPart{2, 1, s}, rp1.s);
+          const AT* act1 = reinterpret_cast<const AT*>(fs.act[par][1]);
+          const uint32_t b0 = *reinterpret_cast<const uint32_t*>(act + col * 8 + kq), b1 = *reinterpret_cast<const uint32_t*>(act1 + col * 8 + kq);
+          const uint32_t abase = ((lane >> 4) ? d1base : dbase) + (uint32_t)(lane & 7) * 16u + (uint32_t)((lane >> 3) & 1) * 128u +
+                                 (uint32_t)(warp * g.steps) * 256u;
+#pragma unroll
+          for (int t0 = 0; t0 < kDecMaxSteps; t0 += 4) {      // four output tiles per batch: loads first, then the MMAs
+            if (t0 < g.steps) {
+              uint32_t af[4][4];
+#pragma unroll
+              for (int j = 0; j < 4; ++j)
+                if (t0 + j < g.steps) ldmatrix_x4(af[j][0], af[j][1], af[j][2], af[j][3], abase + (uint32_t)(t0 + j) * 256u);
+#pragma unroll
+              for (int j = 0; j < 4; ++j)
+                if (t0 + j < g.steps) mma_bf16_16816(yacc[t0 + j], af[j][0], af[j][1], af[j][2], af[j][3], b0, b1);
+            }
+          }
+          release();                                           // sub-block 0's part
+        } else {
         // A[j][i]: 16 outputs j x (8 act columns i, upper half of K zero); B[i][n] = a[n][i]
         const uint32_t b0 = *reinterpret_cast<const uint32_t*>(act + col * 8 + kq);
         const uint32_t abase = dbase + (uint32_t)(lane & 7) * 16u + (uint32_t)((lane >> 3) & 1) * 128u + (uint32_t)(warp * g.steps) * 256u;
@@ -609,8 +637,9 @@ __device__ __forceinline__ void decode_consume(const DecodeFfnArgs& a, const Dec
               if (t0 + j < g.steps) mma_bf16_16816(yacc[t0 + j], af[j][0], af[j][1], 0u, 0u, b0, 0u);
           }
         }
+        }
         release();
-        if (sb == g.n_sb - 1) {
+        if (sb == n_pass - 1) {
           const int j0 = s * g.slab + warp * (g.slab >> 3) + col;
           float* p0 = a.partial + ((size_t)(pos0 + kq) * g.n_chunks + c) * g.d + j0;
           float* p1 = p0 + (size_t)g.n_chunks * g.d;

@@ -907,10 +907,10 @@ int wisp_create(uint64_t budget_bytes, const wisp_config* cfg, wisp_ctx** out) {
   CKC(cudaMalloc(&ctx->phase_ns, (kDecPhases + 2) * sizeof(u64)));
   CKC(cudaMemset(ctx->phase_ns, 0, (kDecPhases + 2) * sizeof(u64)));
   {
-    // Work-unit size of the decode FFN: 8 act rows (96 KiB of weights at the Qwen3 shape) for calls of at most 2 tokens, 16
-    // for 3..8 tokens, where more experts are in flight and every routed pair writes its own chunk partials.  fp32 models
-    // (config 1, parity only) always use 8.
-    const int r0 = cfg->unit_rows > 0 && cfg->dtype != WISP_F32 ? cfg->unit_rows : ctx->f8 ? 16 : 8;   // fp8: half the bytes per row
+    // Work-unit size of the decode FFN: 16 act rows (two sub-blocks of 8: 192 KiB of bf16 weights at the Qwen3 shape) -- the two
+    // sub-blocks' down parts feed one MMA pass with all 16 k slots used, and a pair has half as many chunk partials to combine.
+    // fp32 models (config 1, parity only) always use 8.
+    const int r0 = cfg->unit_rows > 0 && cfg->dtype != WISP_F32 ? cfg->unit_rows : cfg->dtype == WISP_F32 ? 8 : 16;
     const int r1 = cfg->dtype == WISP_F32 ? 8 : cfg->unit_rows > 0 ? cfg->unit_rows : 16;
     ctx->dgeom[0] = make_decode_geom(d, dff, ctx->welem, r0, ctx->f8);
     ctx->dgeom[1] = make_decode_geom(d, dff, ctx->welem, r1, ctx->f8);
