@@ -92,7 +92,7 @@ struct CombineArgs {
 //   x_row  : token t's current hidden state (model dtype) or nullptr (no residual: the result is out_t itself)
 //   dst_row: where the result row goes (global, model dtype)
 //   s_yg   : 8 * 8 * 16 floats, s_y: kMaxTopK * 16 floats, s_xn: 16 floats (receives the fp32 image of the stored result)
-template <typename T>
+template <typename T, int U = 16>
 __device__ __forceinline__ void combine_slice(const CombineArgs& a, int t, int j0, const T* x_row, T* dst_row, float* s_yg, float* s_y,
                                               float* s_xn, int bar) {
   const int tid = threadIdx.x, grp = tid >> 5, lane = tid & 31, ri = lane >> 2, j4 = (lane & 3) * 4;
@@ -103,13 +103,13 @@ __device__ __forceinline__ void combine_slice(const CombineArgs& a, int t, int j
     if (rank < a.k) {
       const int pos = a.pair_pos[t * a.k + rank];
       const float* src = a.partial + ((size_t)pos * a.n_chunks + (size_t)grp * per) * a.d + j0 + j4;
-      for (int c0 = 0; c0 < per; c0 += 16) {                 // up to 16 independent L2 reads in flight, added in ascending c
-        float4 v[16];
+      for (int c0 = 0; c0 < per; c0 += U) {                  // up to U independent L2 reads in flight, added in ascending c
+        float4 v[U];
 #pragma unroll
-        for (int u = 0; u < 16; ++u)                           // unpredicated (index clamped) so that all 16 loads issue before the first add
+        for (int u = 0; u < U; ++u)                            // unpredicated (index clamped) so that all loads issue before the first add
           v[u] = __ldcg(reinterpret_cast<const float4*>(src + (size_t)min(c0 + u, per - 1) * a.d));
 #pragma unroll
-        for (int u = 0; u < 16; ++u)
+        for (int u = 0; u < U; ++u)
           if (c0 + u < per) {
             if (c0 + u == 0) acc = v[0];
             else { acc.x += v[u].x; acc.y += v[u].y; acc.z += v[u].z; acc.w += v[u].w; }

@@ -375,7 +375,8 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
           const int ns = MULTI ? min(kCombineBatch, T_ - t0) : 1;
           const T* xres = a.residual ? xs : nullptr;
           if (!MULTI || ns == 1) {
-            combine_slice<T>(ca, t0, j0, xres ? xres + (size_t)t0 * xs_pitch : nullptr, xg + (size_t)t0 * d, fs.red[0][0], ds.y, ds.xn, 1);
+            if (g.n_chunks <= 64) combine_slice<T, 8>(ca, t0, j0, xres ? xres + (size_t)t0 * xs_pitch : nullptr, xg + (size_t)t0 * d, fs.red[0][0], ds.y, ds.xn, 1);
+            else combine_slice<T, 16>(ca, t0, j0, xres ? xres + (size_t)t0 * xs_pitch : nullptr, xg + (size_t)t0 * d, fs.red[0][0], ds.y, ds.xn, 1);
             if (!last && tid == 255) { __threadfence(); atomicAdd(a.sync + 3, 1u); }    // x slice visible at gpu scope, then counted (a thread with no logit adds at E <= 255)
             if (!last) slice_logits<T>(w16, ds.xn, E, zf_n + (size_t)t0 * E, tid, kDecConsumers);
           } else if constexpr (!MULTI) {
