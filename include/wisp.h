@@ -95,7 +95,7 @@ typedef struct {
   int32_t fetch;      /* wisp_fetch */
   int32_t ring_stages; /* shared-memory ring depth (parts of <= 32 KiB) of the decode FFN kernels, 2..8; 0 = as many as fit */
   int32_t unit_rows;   /* act rows per decode FFN work unit: multiple of 8 dividing d_ff with d_ff/unit_rows a multiple of 8;
-                          0 = library default (8 for calls of <= 2 tokens, 16 for 3..8 tokens).  Outputs are byte-identical across
+                          0 = library default (16 for bf16 / fp8 models, 8 for fp32).  Outputs are byte-identical across
                           budgets, policies and fetch paths for a GIVEN unit size; changing it regroups the fp32 partial sums. */
   int32_t reserved0;   /* must be 0 */
   uint64_t kv_block_bytes;  /* b: bytes per KV block summed over layers; 0 = no KV accounting */
