@@ -268,3 +268,31 @@ def test_wide_topk_fused_route_without_a_spare_warp():
             want_x = (last["x"].float() + last["out"].float()).to(shape.torch_dtype)
             assert torch.equal(fin[t].view(torch.uint8), want_x.view(torch.uint8))
         ctx.close(); ctx2.close()
+
+
+@pytest.mark.parametrize("T", [3, 5, 6, 7])
+def test_odd_batch_sizes_fused_vs_split(T):
+    """Token counts that are not a multiple of the combine batch (4): the fused kernel combines 4 + 1, 4 + 2, 4 + 3 or 3 tokens per
+    column block; the x-ready and accumulator counts must still add up.  bf16 (MMA path) and fp32, fused vs split vs oracle."""
+    for shape in (MED, si.TINY):
+        hidden = si.gen_decode_hidden(shape, 6, T)
+        E = shape.n_experts
+        ref = None
+        for slots, fetch in ((E, 2), (E, 1), (max(shape.top_k, E // 3), 2)):
+            ctx = make_ctx(shape, slots, max_tokens=T, fetch=fetch)
+            res = run_chain(ctx, shape, hidden)
+            routed = [[rec["ids"].flatten().tolist() for rec in per] for per in res]
+            want, _ = sim_trace(shape, slots, 0, routed)
+            assert ctx.trace_read() == want
+            if ref is None:
+                ref = res
+                check_vs_oracle(shape, res, TOL[shape.dtype])
+            else:
+                assert_same_bytes(ref, res)
+            ctx2 = make_ctx(shape, slots, max_tokens=T, fetch=fetch)
+            fin = run_stack(ctx2, shape, hidden)                                   # all layers in one launch: reload + polls
+            for t in range(hidden.shape[0]):
+                last = res[t][-1]
+                want_x = (last["x"].float() + last["out"].float()).to(shape.torch_dtype)
+                assert torch.equal(fin[t].view(torch.uint8), want_x.view(torch.uint8))
+            ctx.close(); ctx2.close()
