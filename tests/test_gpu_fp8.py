@@ -16,7 +16,7 @@ MED_F8 = si.MoEShape("medium-fp8", 2, 16, 4, 1024, 512, "fp8", 1.1)
 BIG_D_F8 = si.MoEShape("two-slab-fp8", 1, 8, 2, 4096, 256, "fp8", 1.1)       # d = 4096: two slabs per 8-row group
 
 
-@pytest.mark.parametrize("T", [1, 2, 4, 8])
+@pytest.mark.parametrize("T", [1, 2, 3, 4, 5, 8])
 def test_fp8_decode_parities(T):
     shape = MED_F8
     hidden = si.gen_decode_hidden(shape, 10, T)
