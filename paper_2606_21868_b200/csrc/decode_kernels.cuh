@@ -234,17 +234,34 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_fused_kernel(const Deco
           while (ld_acquire(a.sync + 3) < want)
             if (++spins > kGridBarrierSpinLimit || ((spins & 0xfffu) == 0u && *a.err)) { *a.err = 1; fs.abort = 1; break; }
         }
-        // one bulk copy per token row (rows are padded in shared memory): all in flight together, one L2 round trip whatever T is
-        if (lane == 0 && !fs.abort) {
-          asm volatile("fence.proxy.async;" ::: "memory");      // the acquire above orders the rows' generic-proxy writes before these reads
-          const uint32_t row_bytes = (uint32_t)(d * sizeof(T));
-          const char* x_src = reinterpret_cast<const char*>(a.xbuf[(l - 1 - a.layer_lo) & 1]);
-          mbar_expect_tx(smem_u32(&ds.xbar), (uint32_t)T_ * row_bytes);
-          for (int t = 0; t < T_; ++t)
-            bulk_g2s_nohint(smem_u32(xs) + (uint32_t)t * (uint32_t)(xs_pitch * sizeof(T)), x_src + (size_t)t * row_bytes, row_bytes, smem_u32(&ds.xbar));
+        if constexpr (MULTI && !F8) {
+          // bf16 batches: one bulk copy per token row (rows are padded in shared memory): all in flight together, one L2 round trip
+          // whatever T is.  (One token, and fp8 experts -- whose f16 staging pass follows -- measured faster with the loads below.)
+          if (lane == 0 && !fs.abort) {
+            asm volatile("fence.proxy.async;" ::: "memory");    // the acquire above orders the rows' generic-proxy writes before these reads
+            const uint32_t row_bytes = (uint32_t)(d * sizeof(T));
+            const char* x_src = reinterpret_cast<const char*>(a.xbuf[(l - 1 - a.layer_lo) & 1]);
+            mbar_expect_tx(smem_u32(&ds.xbar), (uint32_t)T_ * row_bytes);
+            for (int t = 0; t < T_; ++t)
+              bulk_g2s_nohint(smem_u32(xs) + (uint32_t)t * (uint32_t)(xs_pitch * sizeof(T)), x_src + (size_t)t * row_bytes, row_bytes, smem_u32(&ds.xbar));
+          }
+          __syncwarp();
+          mbar_wait_or_abort(smem_u32(&ds.xbar), (unsigned)(l - 1 - a.layer_lo) & 1u, &fs.abort);
+        } else {
+          __syncwarp();
+          const uint4* x_src = reinterpret_cast<const uint4*>(a.xbuf[(l - 1 - a.layer_lo) & 1]);
+          const int vec_row = d * (int)sizeof(T) / 16, xs_vec = T_ * vec_row;
+          for (int v0 = lane; v0 < xs_vec; v0 += 32 * 8) {
+            uint4 xr[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) xr[i] = __ldcg(x_src + min(v0 + 32 * i, xs_vec - 1));
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const int v = v0 + 32 * i;
+              if (v < xs_vec) reinterpret_cast<uint4*>(xs + (size_t)(v / vec_row) * xs_pitch)[v % vec_row] = xr[i];
+            }
+          }
         }
-        __syncwarp();
-        mbar_wait_or_abort(smem_u32(&ds.xbar), (unsigned)(l - 1 - a.layer_lo) & 1u, &fs.abort);
       }
     };
     if (split && warp == kDecWarps - 1) {
